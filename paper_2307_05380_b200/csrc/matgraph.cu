@@ -1,0 +1,361 @@
+// matgraph.cu — C ABI of libmatgraph (include/matgraph.h): argument checks, workspace, launches.
+// No torch types, no CPU fallback: every graph is produced by the sm_100a kernels in this
+// directory.
+#include "../../include/matgraph.h"
+
+#include <cuda_runtime.h>
+#include <math.h>
+#include <new>
+#include <stdlib.h>
+#include <string.h>
+
+#include "common.cuh"
+#include "cutoff_small.cuh"
+#include "knn_small.cuh"
+
+struct mg_ctx {
+    int device = 0;
+    int sm_count = 0;
+    unsigned *d_ctl = nullptr;            // [0..1] cutoff ticket/done, [2..3] knn ticket/done, [4] status
+    unsigned long long *d_desc = nullptr; // look-back descriptors
+    size_t desc_cap = 0;
+    int32_t *d_rowptr_tmp = nullptr;      // for mg_cutoff_count
+    size_t rowptr_cap = 0;
+    long long *d_count = nullptr;
+    unsigned epoch = 0;
+    int cutoff_occ = 0, knn_occ[2] = {0, 0};
+    int64_t launches = 0;
+    // device mirrors for the _host entry points
+    void *h_dev[9] = {nullptr};
+    size_t h_cap[9] = {0};
+};
+
+struct mg_graph {
+    mg_ctx *ctx;
+    int kind;
+    float r_c;
+    int32_t k;
+    const int32_t *struct_ptr;
+    int32_t n_struct, n_atoms;
+    float *d_hint = nullptr;
+    int have_hint = 0;
+};
+
+#define MG_CUDA(call) do { if ((call) != cudaSuccess) { cudaGetLastError(); return MG_ERR_CUDA; } } while (0)
+
+static mg_status decode_status(unsigned bits) {
+    if (bits & MGS_NONFINITE) return MG_ERR_NONFINITE;
+    if (bits & MGS_SINGULAR) return MG_ERR_SINGULAR_LATTICE;
+    if (bits & MGS_OFFSET) return MG_ERR_OFFSET_RANGE;
+    if (bits & MGS_UNSUPPORTED) return MG_ERR_UNSUPPORTED;
+    if (bits & MGS_CAPACITY) return MG_ERR_CAPACITY;
+    return MG_OK;
+}
+
+extern "C" const char *mg_status_string(mg_status s) {
+    switch (s) {
+        case MG_OK: return "ok";
+        case MG_ERR_INVALID_ARG: return "invalid argument";
+        case MG_ERR_CUDA: return "CUDA error (no device, launch or allocation failure)";
+        case MG_ERR_SINGULAR_LATTICE: return "singular lattice";
+        case MG_ERR_NONFINITE: return "non-finite lattice or position";
+        case MG_ERR_OFFSET_RANGE: return "search box needs |tau| > 127";
+        case MG_ERR_CAPACITY: return "edge capacity exceeded";
+        case MG_ERR_UNSUPPORTED: return "unsupported k or structure size";
+    }
+    return "unknown status";
+}
+
+extern "C" mg_status mg_create(mg_ctx **out, int device) {
+    if (!out) return MG_ERR_INVALID_ARG;
+    *out = nullptr;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) {
+        cudaGetLastError();
+        return MG_ERR_CUDA;
+    }
+    MG_CUDA(cudaSetDevice(device));
+    mg_ctx *c = new (std::nothrow) mg_ctx();
+    if (!c) return MG_ERR_CUDA;
+    c->device = device;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess || prop.major < 10) { delete c; return MG_ERR_CUDA; }
+    c->sm_count = prop.multiProcessorCount;
+    if (cudaMalloc(&c->d_ctl, 8 * sizeof(unsigned)) != cudaSuccess ||
+        cudaMemset(c->d_ctl, 0, 8 * sizeof(unsigned)) != cudaSuccess ||
+        cudaMalloc(&c->d_count, sizeof(long long)) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
+    if (cudaFuncSetAttribute(mg_cutoff_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)sizeof(CutoffSmem)) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->cutoff_occ, mg_cutoff_small_kernel, MG_BLOCK, sizeof(CutoffSmem));
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->knn_occ[0], mg_knn_small_kernel<1>, MG_BLOCK, 0);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->knn_occ[1], mg_knn_small_kernel<2>, MG_BLOCK, 0);
+    if (c->cutoff_occ < 1 || c->knn_occ[0] < 1 || c->knn_occ[1] < 1) { mg_destroy(c); return MG_ERR_CUDA; }
+    *out = c;
+    return MG_OK;
+}
+
+extern "C" void mg_destroy(mg_ctx *c) {
+    if (!c) return;
+    cudaSetDevice(c->device);
+    cudaFree(c->d_ctl);
+    cudaFree(c->d_desc);
+    cudaFree(c->d_rowptr_tmp);
+    cudaFree(c->d_count);
+    for (int i = 0; i < 9; ++i) cudaFree(c->h_dev[i]);
+    delete c;
+}
+
+extern "C" mg_status mg_reserve(mg_ctx *c, int32_t n_struct, int32_t n_atoms) {
+    if (!c || n_struct < 0 || n_atoms < 0) return MG_ERR_INVALID_ARG;
+    MG_CUDA(cudaSetDevice(c->device));
+    if ((size_t)n_struct > c->desc_cap) {
+        const size_t cap = (size_t)n_struct + 1024;
+        cudaFree(c->d_desc);
+        c->d_desc = nullptr; c->desc_cap = 0;
+        MG_CUDA(cudaMalloc(&c->d_desc, cap * sizeof(unsigned long long)));
+        MG_CUDA(cudaMemset(c->d_desc, 0, cap * sizeof(unsigned long long)));
+        c->desc_cap = cap;
+    }
+    if ((size_t)n_atoms + 1 > c->rowptr_cap) {
+        const size_t cap = (size_t)n_atoms + 1025;
+        cudaFree(c->d_rowptr_tmp);
+        c->d_rowptr_tmp = nullptr; c->rowptr_cap = 0;
+        MG_CUDA(cudaMalloc(&c->d_rowptr_tmp, cap * sizeof(int32_t)));
+        c->rowptr_cap = cap;
+    }
+    return MG_OK;
+}
+
+extern "C" int64_t mg_launch_count(const mg_ctx *c) { return c ? c->launches : 0; }
+
+static bool bad_inputs(const mg_ctx *c, const float *pos, const float *lat, const int32_t *sp,
+                       int32_t n_struct, int32_t n_atoms) {
+    if (!c || n_struct < 0 || n_atoms < 0 || !sp) return true;
+    if (n_struct > 0 && !lat) return true;
+    if (n_atoms > 0 && !pos) return true;
+    return false;
+}
+
+static bool bad_edges(const mg_edges *o, long long need) {
+    if (!o || !o->row_ptr || !o->n_edges || o->capacity < 0) return true;
+    if (o->capacity > 0 && (!o->src || !o->dst || !o->offset || !o->vec)) return true;
+    return o->capacity < need;
+}
+
+static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, const int32_t *sp,
+                               int32_t n_struct, int32_t n_atoms, float r_c, const mg_edges *o,
+                               int count_only, cudaStream_t st) {
+    MG_CUDA(cudaSetDevice(c->device));
+    mg_status rs = mg_reserve(c, n_struct, count_only ? n_atoms : 0);
+    if (rs != MG_OK) return rs;
+    if (n_struct == 0) {
+        MG_CUDA(cudaMemsetAsync(o->row_ptr, 0, sizeof(int32_t), st));
+        MG_CUDA(cudaMemsetAsync(o->n_edges, 0, sizeof(long long), st));
+        return MG_OK;
+    }
+    c->epoch = (c->epoch + 1u) & 0x3FFFFFFFu;
+    if (c->epoch == 0u) {   // 2^30 calls: clear stale descriptors before reusing epoch numbers
+        MG_CUDA(cudaMemsetAsync(c->d_desc, 0, c->desc_cap * sizeof(unsigned long long), st));
+        c->epoch = 1u;
+    }
+    CutoffArgs A;
+    A.pos = pos; A.lattice = lat; A.struct_ptr = sp;
+    A.n_struct = n_struct; A.n_atoms = n_atoms; A.r_c = r_c;
+    A.row_ptr = o->row_ptr; A.src = o->src; A.dst = o->dst; A.offset = o->offset;
+    A.vec = o->vec; A.dist = o->dist; A.capacity = o->capacity; A.n_edges = (long long *)o->n_edges;
+    A.desc = c->d_desc; A.ticket = c->d_ctl; A.status = c->d_ctl + 4;
+    A.epoch = c->epoch; A.count_only = count_only;
+    int grid = c->sm_count * c->cutoff_occ;
+    if (grid > n_struct) grid = n_struct;
+    mg_cutoff_small_kernel<<<grid, MG_BLOCK, sizeof(CutoffSmem), st>>>(A);
+    MG_CUDA(cudaGetLastError());
+    c->launches += 1;
+    return MG_OK;
+}
+
+extern "C" mg_status mg_cutoff_graph(mg_ctx *c, const float *pos, const float *lat, const int32_t *sp,
+                                     int32_t n_struct, int32_t n_atoms, float r_c, const mg_edges *o,
+                                     void *stream) {
+    if (bad_inputs(c, pos, lat, sp, n_struct, n_atoms) || bad_edges(o, 0) || !(r_c > 0.f) || !isfinite(r_c))
+        return MG_ERR_INVALID_ARG;
+    return launch_cutoff(c, pos, lat, sp, n_struct, n_atoms, r_c, o, 0, (cudaStream_t)stream);
+}
+
+extern "C" mg_status mg_cutoff_count(mg_ctx *c, const float *pos, const float *lat, const int32_t *sp,
+                                     int32_t n_struct, int32_t n_atoms, float r_c,
+                                     int64_t *n_edges_host, void *stream) {
+    if (bad_inputs(c, pos, lat, sp, n_struct, n_atoms) || !n_edges_host || !(r_c > 0.f) || !isfinite(r_c))
+        return MG_ERR_INVALID_ARG;
+    mg_status rs = mg_reserve(c, n_struct, n_atoms);
+    if (rs != MG_OK) return rs;
+    mg_edges o;
+    memset(&o, 0, sizeof(o));
+    o.row_ptr = c->d_rowptr_tmp;
+    o.n_edges = (int64_t *)c->d_count;
+    rs = launch_cutoff(c, pos, lat, sp, n_struct, n_atoms, r_c, &o, 1, (cudaStream_t)stream);
+    if (rs != MG_OK) return rs;
+    long long v = 0;
+    MG_CUDA(cudaMemcpyAsync(&v, c->d_count, sizeof(v), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    MG_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+    *n_edges_host = v;
+    return MG_OK;
+}
+
+static mg_status launch_knn(mg_ctx *c, const float *pos, const float *lat, const int32_t *sp,
+                            int32_t n_struct, int32_t n_atoms, int32_t k, const mg_edges *o,
+                            float *hint, int use_hint, cudaStream_t st) {
+    MG_CUDA(cudaSetDevice(c->device));
+    KnnArgs A;
+    A.pos = pos; A.lattice = lat; A.struct_ptr = sp;
+    A.n_struct = n_struct; A.n_atoms = n_atoms; A.k = k;
+    A.row_ptr = o->row_ptr; A.src = o->src; A.dst = o->dst; A.offset = o->offset;
+    A.vec = o->vec; A.dist = o->dist; A.n_edges = (long long *)o->n_edges;
+    A.radius_hint = hint; A.use_hint = use_hint;
+    A.ticket = c->d_ctl + 2; A.status = c->d_ctl + 4;
+    const int kpl = k <= 32 ? 0 : 1;
+    int grid = c->sm_count * c->knn_occ[kpl];
+    if (grid > n_struct) grid = n_struct;
+    if (grid < 1) grid = 1;
+    if (kpl == 0) mg_knn_small_kernel<1><<<grid, MG_BLOCK, 0, st>>>(A);
+    else mg_knn_small_kernel<2><<<grid, MG_BLOCK, 0, st>>>(A);
+    MG_CUDA(cudaGetLastError());
+    c->launches += 1;
+    return MG_OK;
+}
+
+extern "C" mg_status mg_knn_graph(mg_ctx *c, const float *pos, const float *lat, const int32_t *sp,
+                                  int32_t n_struct, int32_t n_atoms, int32_t k, const mg_edges *o,
+                                  void *stream) {
+    if (k < 1 || k > MG_MAX_K) return MG_ERR_INVALID_ARG;
+    if (bad_inputs(c, pos, lat, sp, n_struct, n_atoms) || bad_edges(o, (long long)k * n_atoms))
+        return MG_ERR_INVALID_ARG;
+    return launch_knn(c, pos, lat, sp, n_struct, n_atoms, k, o, nullptr, 0, (cudaStream_t)stream);
+}
+
+extern "C" mg_status mg_graph_create(mg_ctx *c, int kind, float r_c, int32_t k, const int32_t *sp,
+                                     int32_t n_struct, int32_t n_atoms, mg_graph **out) {
+    if (!out) return MG_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!c || !sp || n_struct < 0 || n_atoms < 0) return MG_ERR_INVALID_ARG;
+    if (kind == MG_KIND_CUTOFF) { if (!(r_c > 0.f) || !isfinite(r_c)) return MG_ERR_INVALID_ARG; }
+    else if (kind == MG_KIND_KNN) { if (k < 1 || k > MG_MAX_K) return MG_ERR_INVALID_ARG; }
+    else return MG_ERR_INVALID_ARG;
+    mg_status rs = mg_reserve(c, n_struct, n_atoms);
+    if (rs != MG_OK) return rs;
+    mg_graph *g = new (std::nothrow) mg_graph();
+    if (!g) return MG_ERR_CUDA;
+    g->ctx = c; g->kind = kind; g->r_c = r_c; g->k = k;
+    g->struct_ptr = sp; g->n_struct = n_struct; g->n_atoms = n_atoms;
+    if (kind == MG_KIND_KNN && n_atoms > 0) {
+        if (cudaMalloc(&g->d_hint, (size_t)n_atoms * sizeof(float)) != cudaSuccess ||
+            cudaMemset(g->d_hint, 0, (size_t)n_atoms * sizeof(float)) != cudaSuccess) {
+            cudaGetLastError();
+            cudaFree(g->d_hint);
+            delete g;
+            return MG_ERR_CUDA;
+        }
+    }
+    *out = g;
+    return MG_OK;
+}
+
+extern "C" void mg_graph_destroy(mg_graph *g) {
+    if (!g) return;
+    cudaSetDevice(g->ctx->device);
+    cudaFree(g->d_hint);
+    delete g;
+}
+
+extern "C" mg_status mg_update_graph(mg_ctx *c, mg_graph *g, const float *pos, const float *lat,
+                                     const mg_edges *o, void *stream) {
+    if (!c || !g || g->ctx != c) return MG_ERR_INVALID_ARG;
+    if (bad_inputs(c, pos, lat, g->struct_ptr, g->n_struct, g->n_atoms)) return MG_ERR_INVALID_ARG;
+    if (g->kind == MG_KIND_CUTOFF) {
+        if (bad_edges(o, 0)) return MG_ERR_INVALID_ARG;
+        return launch_cutoff(c, pos, lat, g->struct_ptr, g->n_struct, g->n_atoms, g->r_c, o, 0,
+                             (cudaStream_t)stream);
+    }
+    if (bad_edges(o, (long long)g->k * g->n_atoms)) return MG_ERR_INVALID_ARG;
+    mg_status rs = launch_knn(c, pos, lat, g->struct_ptr, g->n_struct, g->n_atoms, g->k, o, g->d_hint,
+                              g->have_hint, (cudaStream_t)stream);
+    if (rs == MG_OK) g->have_hint = 1;
+    return rs;
+}
+
+extern "C" mg_status mg_check(mg_ctx *c, void *stream) {
+    if (!c) return MG_ERR_INVALID_ARG;
+    MG_CUDA(cudaSetDevice(c->device));
+    unsigned bits = 0;
+    MG_CUDA(cudaMemcpyAsync(&bits, c->d_ctl + 4, sizeof(bits), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    MG_CUDA(cudaMemsetAsync(c->d_ctl + 4, 0, sizeof(unsigned), (cudaStream_t)stream));
+    MG_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+    return decode_status(bits);
+}
+
+// ---- host-buffer entry points -------------------------------------------------------------
+static mg_status host_buf(mg_ctx *c, int slot, size_t bytes) {
+    if (bytes <= c->h_cap[slot]) return MG_OK;
+    cudaFree(c->h_dev[slot]);
+    c->h_dev[slot] = nullptr; c->h_cap[slot] = 0;
+    const size_t cap = bytes + bytes / 4 + 256;
+    MG_CUDA(cudaMalloc(&c->h_dev[slot], cap));
+    c->h_cap[slot] = cap;
+    return MG_OK;
+}
+
+static mg_status run_host(mg_ctx *c, int kind, const float *pos, const float *lat, const int32_t *sp,
+                          int32_t n_struct, int32_t n_atoms, float r_c, int32_t k, const mg_edges *oh) {
+    if (!c || n_struct < 0 || n_atoms < 0 || !sp || (n_struct > 0 && !lat) || (n_atoms > 0 && !pos))
+        return MG_ERR_INVALID_ARG;
+    if (bad_edges(oh, kind == MG_KIND_KNN ? (long long)k * n_atoms : 0)) return MG_ERR_INVALID_ARG;
+    MG_CUDA(cudaSetDevice(c->device));
+    const size_t cap = (size_t)oh->capacity;
+    const size_t sz[9] = {(size_t)n_atoms * 12 + 4, (size_t)n_struct * 36 + 4, ((size_t)n_struct + 1) * 4,
+                          ((size_t)n_atoms + 1) * 4, cap * 4 + 4, cap * 4 + 4, cap * 3 + 4, cap * 12 + 4,
+                          (oh->dist ? cap * 4 : 0) + 16};
+    for (int i = 0; i < 9; ++i) { mg_status rs = host_buf(c, i, sz[i]); if (rs != MG_OK) return rs; }
+    cudaStream_t st = 0;
+    MG_CUDA(cudaMemcpyAsync(c->h_dev[0], pos, (size_t)n_atoms * 12, cudaMemcpyHostToDevice, st));
+    MG_CUDA(cudaMemcpyAsync(c->h_dev[1], lat, (size_t)n_struct * 36, cudaMemcpyHostToDevice, st));
+    MG_CUDA(cudaMemcpyAsync(c->h_dev[2], sp, ((size_t)n_struct + 1) * 4, cudaMemcpyHostToDevice, st));
+    mg_edges od;
+    od.row_ptr = (int32_t *)c->h_dev[3]; od.src = (int32_t *)c->h_dev[4]; od.dst = (int32_t *)c->h_dev[5];
+    od.offset = (int8_t *)c->h_dev[6]; od.vec = (float *)c->h_dev[7];
+    od.dist = oh->dist ? (float *)((char *)c->h_dev[8] + 16) : nullptr;
+    od.capacity = oh->capacity; od.n_edges = (int64_t *)c->h_dev[8];
+    mg_status rs;
+    if (kind == MG_KIND_CUTOFF)
+        rs = mg_cutoff_graph(c, (const float *)c->h_dev[0], (const float *)c->h_dev[1],
+                             (const int32_t *)c->h_dev[2], n_struct, n_atoms, r_c, &od, st);
+    else
+        rs = mg_knn_graph(c, (const float *)c->h_dev[0], (const float *)c->h_dev[1],
+                          (const int32_t *)c->h_dev[2], n_struct, n_atoms, k, &od, st);
+    if (rs != MG_OK) return rs;
+    long long ne = 0;
+    MG_CUDA(cudaMemcpyAsync(&ne, od.n_edges, 8, cudaMemcpyDeviceToHost, st));
+    MG_CUDA(cudaMemcpyAsync(oh->row_ptr, od.row_ptr, ((size_t)n_atoms + 1) * 4, cudaMemcpyDeviceToHost, st));
+    MG_CUDA(cudaStreamSynchronize(st));
+    *oh->n_edges = ne;
+    const size_t m = (size_t)(ne < oh->capacity ? ne : oh->capacity);
+    if (m) {
+        MG_CUDA(cudaMemcpyAsync(oh->src, od.src, m * 4, cudaMemcpyDeviceToHost, st));
+        MG_CUDA(cudaMemcpyAsync(oh->dst, od.dst, m * 4, cudaMemcpyDeviceToHost, st));
+        MG_CUDA(cudaMemcpyAsync(oh->offset, od.offset, m * 3, cudaMemcpyDeviceToHost, st));
+        MG_CUDA(cudaMemcpyAsync(oh->vec, od.vec, m * 12, cudaMemcpyDeviceToHost, st));
+        if (oh->dist) MG_CUDA(cudaMemcpyAsync(oh->dist, od.dist, m * 4, cudaMemcpyDeviceToHost, st));
+    }
+    return mg_check(c, st);
+}
+
+extern "C" mg_status mg_cutoff_graph_host(mg_ctx *c, const float *pos, const float *lat,
+                                          const int32_t *sp, int32_t n_struct, int32_t n_atoms,
+                                          float r_c, const mg_edges *oh) {
+    if (!(r_c > 0.f) || !isfinite(r_c)) return MG_ERR_INVALID_ARG;
+    return run_host(c, MG_KIND_CUTOFF, pos, lat, sp, n_struct, n_atoms, r_c, 0, oh);
+}
+
+extern "C" mg_status mg_knn_graph_host(mg_ctx *c, const float *pos, const float *lat, const int32_t *sp,
+                                       int32_t n_struct, int32_t n_atoms, int32_t k, const mg_edges *oh) {
+    if (k < 1 || k > MG_MAX_K) return MG_ERR_INVALID_ARG;
+    return run_host(c, MG_KIND_KNN, pos, lat, sp, n_struct, n_atoms, 0.f, k, oh);
+}

@@ -1,0 +1,186 @@
+"""GPU edge cases of the C ABI: empty and ragged batches, coordinates outside [0,1), dense cells
+that overflow the shared-memory stash and the translation-table tile, capacity overflow, error
+reporting, the two-phase count, and the host-buffer entry points."""
+import numpy as np
+import pytest
+
+import oracle
+from oracle import check
+from workloads import crystals as C
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mg():
+    import paper_2307_05380_b200 as m
+    return m
+
+
+@pytest.fixture(scope="module")
+def ctx(mg):
+    c = mg.Context(0)
+    yield c
+    c.close()
+
+
+def _run_cutoff(mg, ctx, b, r_c, capacity=None):
+    pos, lat, ptr = mg.to_device(b)
+    out = ctx.cutoff_graph(pos, lat, ptr, r_c, capacity=capacity, dist=True)
+    return out.to_numpy(), ctx.mg_check()
+
+
+def test_empty_batch(mg, ctx):
+    b = C.Batch(pos=np.zeros((0, 3), np.float32), lattice=np.zeros((0, 3, 3), np.float32),
+                struct_ptr=np.zeros(1, np.int32))
+    got, status = _run_cutoff(mg, ctx, b, 5.0, capacity=0)
+    assert status == 0 and got["n_edges"] == 0 and got["row_ptr"].tolist() == [0]
+    pos, lat, ptr = mg.to_device(b)
+    out = ctx.knn_graph(pos, lat, ptr, 4).to_numpy()
+    assert out["n_edges"] == 0 and out["row_ptr"].tolist() == [0]
+
+
+def test_empty_structures_inside_batch(mg, ctx):
+    a = C.small_batch(5, seed=7)
+    empty = C.Batch(pos=np.zeros((0, 3), np.float32), lattice=np.eye(3, dtype=np.float32)[None] * 4,
+                    struct_ptr=np.zeros(2, np.int32))
+    b = C.concat([empty, a, empty, empty, a, empty])
+    got, status = _run_cutoff(mg, ctx, b, 5.0)
+    assert status == 0
+    rep = check.check_cutoff(b, 5.0, got)
+    assert rep["extra"] == 0 and rep["missing"] == 0
+    pos, lat, ptr = mg.to_device(b)
+    got = ctx.knn_graph(pos, lat, ptr, 7, dist=True).to_numpy()
+    assert ctx.mg_check() == 0
+    check.check_knn(b, 7, got)
+
+
+def test_positions_outside_unit_cell(mg, ctx):
+    b = C.small_batch(24, seed=11)
+    rng = np.random.default_rng(5)
+    shift = rng.integers(-3, 4, size=b.pos.shape).astype(np.float32)
+    b2 = C.Batch(pos=(b.pos + shift + np.float32(0.25)).astype(np.float32), lattice=b.lattice,
+                 struct_ptr=b.struct_ptr)
+    got, status = _run_cutoff(mg, ctx, b2, 4.5)
+    assert status == 0
+    rep = check.check_cutoff(b2, 4.5, got)
+    assert rep["extra"] == 0 and rep["missing"] == 0 and rep["n_edges"] > 0
+    pos, lat, ptr = mg.to_device(b2)
+    gk = ctx.knn_graph(pos, lat, ptr, 9, dist=True).to_numpy()
+    assert ctx.mg_check() == 0
+    check.check_knn(b2, 9, gk)
+
+
+def test_dense_cells_overflow_stash_and_table(mg, ctx):
+    # 3-4 A cells with a 12 A cutoff: > 1024 cells per box (several table tiles) and thousands of
+    # edges per row (rows do not fit their stash segment -> re-search path)
+    items = []
+    for s in range(6):
+        rng = np.random.default_rng(100 + s)
+        n = int(rng.integers(1, 21))
+        cell = np.diag(rng.uniform(3.0, 4.0, 3)).astype(np.float32)
+        cell[1, 0] = np.float32(rng.uniform(-1, 1))
+        cell[2, 1] = np.float32(rng.uniform(-1, 1))
+        items.append((cell, rng.random((n, 3), dtype=np.float32)))
+    b = C._assemble(items)
+    got, status = _run_cutoff(mg, ctx, b, 12.0)
+    assert status == 0
+    rep = check.check_cutoff(b, 12.0, got)
+    assert rep["extra"] == 0 and rep["missing"] == 0
+    assert np.diff(got["row_ptr"]).max() > 1000
+
+
+def test_capacity_overflow_reports_required_count(mg, ctx):
+    b = C.small_batch(16, seed=2)
+    full, status = _run_cutoff(mg, ctx, b, 5.0)
+    assert status == 0
+    need = full["n_edges"]
+    cap = need // 2
+    got, status = _run_cutoff(mg, ctx, b, 5.0, capacity=cap)
+    assert status == 6                       # MG_ERR_CAPACITY
+    assert got["n_edges"] == need            # the required count is still reported
+    assert np.array_equal(got["row_ptr"], full["row_ptr"])
+    # edges below the capacity are complete rows' worth of valid data
+    keep = full["src"] < 0
+    keep[:cap] = True
+    fk = np.stack([full["src"][:cap], full["dst"][:cap]], 1)
+    gk = np.stack([got["src"], got["dst"]], 1)
+    assert gk.shape[0] == cap
+    # same multiset per row prefix is not guaranteed (row order is free): compare the src column
+    assert np.array_equal(fk[:, 0], gk[:, 0])
+    assert ctx.mg_check() == 0               # status word was cleared
+
+
+def test_invalid_lattices_are_reported(mg, ctx):
+    b = C.small_batch(6, seed=4)
+    lat = b.lattice.copy()
+    lat[2] = 0.0                              # singular
+    bad = C.Batch(pos=b.pos, lattice=lat, struct_ptr=b.struct_ptr)
+    got, status = _run_cutoff(mg, ctx, bad, 5.0)
+    assert status == 3                        # MG_ERR_SINGULAR_LATTICE
+    rows = np.diff(got["row_ptr"])
+    s2 = slice(b.struct_ptr[2], b.struct_ptr[3])
+    assert np.all(rows[s2] == 0)              # the invalid structure emits nothing
+    good = np.ones(b.n_atoms, bool)
+    good[s2] = False
+    ref = oracle.cutoff_graph(b.pos, b.lattice, b.struct_ptr, 5.0)
+    assert np.array_equal(rows[good], np.diff(ref["row_ptr"])[good])
+    lat = b.lattice.copy()
+    lat[1, 0, 0] = np.nan
+    bad = C.Batch(pos=b.pos, lattice=lat, struct_ptr=b.struct_ptr)
+    _, status = _run_cutoff(mg, ctx, bad, 5.0)
+    assert status == 4                        # MG_ERR_NONFINITE
+
+
+def test_offset_range_error(mg, ctx):
+    # plane spacing 0.05 A with r_c = 8 would need |tau| = 160 > 127
+    cell = np.diag([0.05, 5.0, 5.0]).astype(np.float32)
+    b = C.Batch(pos=np.zeros((1, 3), np.float32), lattice=cell[None], struct_ptr=np.array([0, 1], np.int32))
+    _, status = _run_cutoff(mg, ctx, b, 8.0, capacity=16)
+    assert status == 5                        # MG_ERR_OFFSET_RANGE
+
+
+def test_invalid_arguments(mg, ctx):
+    b = C.small_batch(2, seed=0)
+    pos, lat, ptr = mg.to_device(b)
+    out = mg.Edges.allocate(b.n_atoms, 10, "cuda")
+    with pytest.raises(mg.MatGraphError):
+        ctx.mg_cutoff_graph(pos, lat, ptr, -1.0, out)
+    with pytest.raises(mg.MatGraphError):
+        ctx.mg_cutoff_graph(pos, lat, ptr, float("nan"), out)
+    with pytest.raises(mg.MatGraphError):
+        ctx.mg_knn_graph(pos, lat, ptr, 0, out)
+    with pytest.raises(mg.MatGraphError):
+        ctx.mg_knn_graph(pos, lat, ptr, 65, out)
+    small = mg.Edges.allocate(b.n_atoms, 3, "cuda")
+    with pytest.raises(mg.MatGraphError):     # capacity < k * n_atoms
+        ctx.mg_knn_graph(pos, lat, ptr, 4, small)
+
+
+def test_count_matches_graph(mg, ctx):
+    b = C.small_batch(64, seed=9)
+    pos, lat, ptr = mg.to_device(b)
+    n = ctx.mg_cutoff_count(pos, lat, ptr, 5.5)
+    assert n == oracle.cutoff_graph(b.pos, b.lattice, b.struct_ptr, 5.5)["n_edges"]
+
+
+def test_host_entry_points(mg, ctx):
+    b = C.small_batch(32, seed=5)
+    ref = oracle.cutoff_graph(b.pos, b.lattice, b.struct_ptr, 5.0)
+    got = ctx.mg_cutoff_graph_host(b.pos, b.lattice, b.struct_ptr, 5.0, ref["n_edges"] + 10, dist=True)
+    assert got["status"] == 0
+    rep = check.check_cutoff(b, 5.0, got, ref)
+    assert rep["extra"] == 0 and rep["missing"] == 0
+    gk = ctx.mg_knn_graph_host(b.pos, b.lattice, b.struct_ptr, 12, dist=True)
+    assert gk["status"] == 0
+    check.check_knn(b, 12, gk)
+
+
+def test_repeated_calls_are_deterministic_sets(mg, ctx):
+    b = C.small_batch(128, seed=6)
+    a, _ = _run_cutoff(mg, ctx, b, 6.0)
+    c, _ = _run_cutoff(mg, ctx, b, 6.0)
+    assert a["n_edges"] == c["n_edges"] and np.array_equal(a["row_ptr"], c["row_ptr"])
+    ka = check._keys(a["src"], a["dst"], a["offset"])
+    kc = check._keys(c["src"], c["dst"], c["offset"])
+    assert np.array_equal(np.sort(ka), np.sort(kc))

@@ -1,0 +1,159 @@
+"""GPU parity: the CUDA path (through the C ABI binding) against the FP64 oracle, element by
+element on the same seeded inputs, with the acceptance rules of BASELINE.json north_star
+(oracle/check.py): bit-exact canonical edge sets outside a 1e-5 A band around r_c (the kernels
+decide the band in FP64, so in practice the sets are identical), KNN rows in oracle order up to
+the 1e-5 A tie band, vec / dist within 1e-5 A absolute."""
+import numpy as np
+import pytest
+
+import oracle
+from oracle import check
+from workloads import crystals as C
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mg():
+    import paper_2307_05380_b200 as m
+    return m
+
+
+@pytest.fixture(scope="module")
+def ctx(mg):
+    c = mg.Context(0)
+    yield c
+    c.close()
+
+
+def _cutoff(mg, ctx, batch, r_c, dist=True, capacity=None):
+    pos, lat, ptr = mg.to_device(batch)
+    out = ctx.cutoff_graph(pos, lat, ptr, r_c, capacity=capacity, dist=dist)
+    got = out.to_numpy()
+    status = ctx.mg_check()
+    return got, status
+
+
+def _knn(mg, ctx, batch, k, dist=True):
+    pos, lat, ptr = mg.to_device(batch)
+    out = ctx.knn_graph(pos, lat, ptr, k, dist=dist)
+    got = out.to_numpy()
+    status = ctx.mg_check()
+    return got, status
+
+
+# ------------------------------------------------------------------ the BASELINE.json configs
+def test_config0_cutoff(mg, ctx):
+    b = C.config_batch(0)
+    got, status = _cutoff(mg, ctx, b, 5.0)
+    assert status == 0
+    rep = check.check_cutoff(b, 5.0, got)
+    assert rep["extra"] == 0 and rep["missing"] == 0, rep    # FP64 window => identical sets
+    assert rep["n_edges"] == rep["n_ref"] > 0
+
+
+def test_config1_knn(mg, ctx):
+    b = C.config_batch(1)
+    got, status = _knn(mg, ctx, b, 12)
+    assert status == 0
+    rep = check.check_knn(b, 12, got)
+    assert rep["n_edges"] == 12 * b.n_atoms
+
+
+@pytest.fixture(scope="module")
+def batch2():
+    return C.config_batch(2)
+
+
+def test_config2_cutoff_full(mg, ctx, batch2):
+    got, status = _cutoff(mg, ctx, batch2, 6.0)
+    assert status == 0
+    rep = check.check_cutoff(batch2, 6.0, got)
+    assert rep["extra"] == 0 and rep["missing"] == 0, rep
+    assert rep["n_edges"] > 3_000_000
+
+
+def test_config2_knn_full(mg, ctx, batch2):
+    got, status = _knn(mg, ctx, batch2, 12)
+    assert status == 0
+    rep = check.check_knn(batch2, 12, got)
+    assert rep["n_edges"] == 12 * batch2.n_atoms
+    # FP64 re-ranking of the selected entries: nearly every row is identical to the oracle's
+    assert rep["exact_rows"] >= 0.999 * batch2.n_atoms, rep
+
+
+def test_config4_update_steps(mg, ctx):
+    import torch
+    k = 24
+    b0 = C.config_batch(4, n_struct=256)
+    ptr = torch.from_numpy(b0.struct_ptr).cuda()
+    graph = ctx.mg_graph_create(mg.MG_KIND_KNN, ptr, b0.n_atoms, k=k)
+    out = mg.Edges.allocate(b0.n_atoms, k * b0.n_atoms, "cuda", dist=True)
+    for step, b in enumerate(C.walk(b0, 6, seed=0)):
+        pos, lat, _ = mg.to_device(b)
+        ctx.mg_update_graph(graph, pos, lat, out)
+        got = out.to_numpy()
+        assert ctx.mg_check() == 0
+        rep = check.check_knn(b, k, got)
+        assert rep["n_edges"] == k * b.n_atoms
+        # R17: identical to a fresh build on the same inputs
+        fresh, _ = _knn(mg, ctx, b, k)
+        for key in ("src", "dst", "offset", "vec", "dist", "row_ptr"):
+            assert np.array_equal(fresh[key], got[key]), (step, key)
+    graph.close()
+
+
+def test_update_cutoff_matches_fresh(mg, ctx):
+    import torch
+    b0 = C.config_batch(4, n_struct=64)
+    ptr = torch.from_numpy(b0.struct_ptr).cuda()
+    graph = ctx.mg_graph_create(mg.MG_KIND_CUTOFF, ptr, b0.n_atoms, r_c=5.0)
+    for b in C.walk(b0, 3, seed=1):
+        pos, lat, _ = mg.to_device(b)
+        cap = ctx.mg_cutoff_count(pos, lat, ptr, 5.0)
+        out = mg.Edges.allocate(b.n_atoms, cap, "cuda", dist=True)
+        ctx.mg_update_graph(graph, pos, lat, out)
+        got = out.to_numpy()
+        assert ctx.mg_check() == 0
+        rep = check.check_cutoff(b, 5.0, got)
+        assert rep["extra"] == 0 and rep["missing"] == 0
+    graph.close()
+
+
+# ------------------------------------------------------------------ closed forms through the GPU
+@pytest.mark.parametrize("name,rc,count", [("sc", 1.01, 6), ("sc", 1.42, 18), ("sc", 2.01, 32),
+                                            ("fcc_conv", 0.7072, 12), ("fcc_prim", 0.7072, 12),
+                                            ("bcc_conv", 0.8661, 8), ("bcc_prim", 0.8661, 8),
+                                            ("diamond", 0.4331, 4), ("hcp", 1.0001, 12)])
+def test_textbook_coordination(mg, ctx, name, rc, count):
+    b = C.textbook(name)
+    got, status = _cutoff(mg, ctx, b, rc)
+    assert status == 0
+    assert np.all(np.diff(got["row_ptr"]) == count)
+    check.check_cutoff(b, rc, got)
+
+
+def test_strict_inequality_exact(mg, ctx):
+    # d == r_c exactly is not an edge (Def. 3 strict '<'): decided by the FP64 window path
+    b = C.textbook("sc")
+    got, _ = _cutoff(mg, ctx, b, 1.0)
+    assert got["n_edges"] == 0
+    got, _ = _cutoff(mg, ctx, b, float(np.nextafter(np.float32(1.0), np.float32(2.0))))
+    assert got["n_edges"] == 6
+
+
+def test_knn_sc_tiebreak_order(mg, ctx):
+    b = C.textbook("sc")
+    got, _ = _knn(mg, ctx, b, 12)
+    first6 = [(-1, 0, 0), (0, -1, 0), (0, 0, -1), (0, 0, 1), (0, 1, 0), (1, 0, 0)]
+    next6 = [(-1, -1, 0), (-1, 0, -1), (-1, 0, 1), (-1, 1, 0), (0, -1, -1), (0, -1, 1)]
+    assert list(map(tuple, got["offset"].tolist())) == first6 + next6
+    check.check_knn(b, 12, got)
+
+
+@pytest.mark.parametrize("k", [1, 6, 12, 24, 32, 33, 48, 64])
+def test_knn_k_sweep(mg, ctx, k):
+    b = C.small_batch(48, seed=3)
+    got, status = _knn(mg, ctx, b, k)
+    assert status == 0
+    check.check_knn(b, k, got)
