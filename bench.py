@@ -1,0 +1,333 @@
+#!/usr/bin/env python
+"""bench.py — headline benchmark of BASELINE.json: edges/s and structures/s for cutoff (6 A) +
+KNN (k=12) graph generation on a batch of 4096 synthetic crystals (configs[2]), one B200.
+
+A "step" is one pass of the whole hot path over the batch: mg_cutoff_graph then mg_knn_graph
+through the C ABI, inputs resident in HBM.  `value` = (cutoff edges + KNN edges) * steps / time.
+Between steps the outputs rotate over several buffer sets whose total size exceeds the L2, so
+the edge writes really go to HBM.  `--impl reference` times the FP64 CPU oracle instead.
+See DESIGN.md "Measurement" for the roofline arithmetic.
+"""
+from __future__ import annotations
+
+import argparse
+import ctypes
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from workloads import crystals as C  # noqa: E402
+
+R_C, K_NN, N_STRUCT = 6.0, 12, 4096
+FP32_LANES_PER_SM = 128
+INSTR_PER_CANDIDATE = 7          # 3 FADD + 1 FMUL + 2 FFMA + 1 FSETP
+BYTES_PER_EDGE = 23              # src 4 + dst 4 + offset 3 + vec 12
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return float(p["hbm_gbs"]), float(p.get("sm_max_mhz", 1965.0)), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+def box_candidates(batch, r_c):
+    """C = sum_s N_s^2 prod_a (2 ceil(r_c/h_a) + 1): the search box BASELINE.json's north_star
+    defines (workload statistic; plain numpy, no library code)."""
+    A = batch.lattice.astype(np.float64)
+    V = np.abs(np.linalg.det(A))
+    h = np.stack([V / np.linalg.norm(np.cross(A[:, (a + 1) % 3], A[:, (a + 2) % 3]), axis=1)
+                  for a in range(3)], axis=1)
+    n = np.diff(batch.struct_ptr).astype(np.float64)
+    if np.isscalar(r_c):
+        r = np.full(A.shape[0], float(r_c))
+    else:
+        r = np.asarray(r_c, np.float64)
+    cells = np.prod(2.0 * np.ceil(r[:, None] / h) + 1.0, axis=1)
+    return float(np.sum(n * n * cells))
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.samples, self.reasons, self.stop_flag = index, [], set(), False
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {"hw_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8),
+                 "hw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40),
+                 "sw_thermal_slowdown": getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20),
+                 "sw_power_cap": getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4)}
+        while not self.stop_flag:
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                bits = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                for k, v in names.items():
+                    if bits & v:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def result(self):
+        self.stop_flag = True
+        self.join(timeout=2)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def run_reference(args, rank, world):
+    """The FP64 oracle, as it stands, on the host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    import oracle
+    sample_struct = 1024
+    b = C.config_batch(2, n_struct=sample_struct)
+    oracle.build()
+    for _ in range(args.warmup):
+        oracle.cutoff_graph(b.pos, b.lattice, b.struct_ptr, R_C)
+    t0 = time.perf_counter()
+    edges = 0
+    for _ in range(args.steps):
+        gc = oracle.cutoff_graph(b.pos, b.lattice, b.struct_ptr, R_C)
+        gk = oracle.knn_graph(b.pos, b.lattice, b.struct_ptr, K_NN)
+        edges += gc["n_edges"] + gk["n_edges"]
+    dt = time.perf_counter() - t0
+    val = edges / dt
+    line = {"impl": "reference", "metric": "edges_per_s", "value": val, "unit": "edges/s", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "structures_per_s": sample_struct * args.steps / dt,
+            "config": {"workload": f"BASELINE configs[2]: cutoff {R_C} A + KNN k={K_NN}; each step a "
+                                   f"{sample_struct}-structure prefix of the 4096-crystal batch"},
+            "cpu_baseline": {"value": val, "unit": "edges/s", "cores": oracle.num_threads(), "kind": "oracle",
+                             "sample": f"{sample_struct}-structure prefix, {args.steps} steps"},
+            "e2e": {"value": val, "unit": "edges/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def run_gpu(args, rank, world, local_rank):
+    import torch
+    import paper_2307_05380_b200 as mg
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the graph kernels have no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=dev)
+    ctx = mg.Context(local_rank)
+    lib = mg._lib()
+    batch = C.config_batch(2, seed=rank)            # weak scaling: every rank has its own 4096 crystals
+    pos, lat, ptr = mg.to_device(batch, dev)
+    S, n_atoms = batch.n_struct, batch.n_atoms
+    ctx.mg_reserve(S, n_atoms)
+    e_cut = ctx.mg_cutoff_count(pos, lat, ptr, R_C)
+    e_knn = K_NN * n_atoms
+    bytes_cut = BYTES_PER_EDGE * e_cut + 4 * (n_atoms + 1) + 12 * n_atoms + 36 * S + 4 * (S + 1)
+    bytes_knn = (BYTES_PER_EDGE + 4) * e_knn + 4 * (n_atoms + 1) + 12 * n_atoms + 36 * S + 4 * (S + 1)
+    n_sets = max(2, int(np.ceil(2.2 * 126e6 / (bytes_cut + bytes_knn))))
+    cut_sets = [mg.Edges.allocate(n_atoms, e_cut, dev) for _ in range(n_sets)]
+    knn_sets = [mg.Edges.allocate(n_atoms, e_knn, dev, dist=True) for _ in range(n_sets)]
+    cut_c = [ctypes.byref(e._c()) for e in cut_sets]
+    knn_c = [ctypes.byref(e._c()) for e in knn_sets]
+    h = ctx._h
+    p_pos, p_lat, p_ptr = (ctypes.c_void_p(t.data_ptr()) for t in (pos, lat, ptr))
+    st = ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    rc32 = ctypes.c_float(R_C)
+
+    def cutoff(i):
+        r = lib.mg_cutoff_graph(h, p_pos, p_lat, p_ptr, S, n_atoms, rc32, cut_c[i % n_sets], st)
+        assert r == 0, r
+
+    def knn(i):
+        r = lib.mg_knn_graph(h, p_pos, p_lat, p_ptr, S, n_atoms, K_NN, knn_c[i % n_sets], st)
+        assert r == 0, r
+
+    for i in range(max(args.warmup, 3)):
+        cutoff(i)
+        knn(i)
+    assert ctx.mg_check() == 0, "device status after warm-up"
+    assert int(cut_sets[0].n_edges.item()) == e_cut and int(knn_sets[0].n_edges.item()) == e_knn
+
+    K = args.steps
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * K + 1)]
+    launches0 = ctx.mg_launch_count()
+    sampler = ClockSampler(local_rank)
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    sampler.start()
+    ev[0].record()
+    for i in range(K):
+        cutoff(i)
+        ev[2 * i + 1].record()
+        knn(i)
+        ev[2 * i + 2].record()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    clocks = sampler.result()
+    launches = ctx.mg_launch_count() - launches0
+    total_ms = ev[0].elapsed_time(ev[2 * K])
+    cut_ms = sum(ev[2 * i].elapsed_time(ev[2 * i + 1]) for i in range(K)) / K
+    knn_ms = sum(ev[2 * i + 1].elapsed_time(ev[2 * i + 2]) for i in range(K)) / K
+    assert ctx.mg_check() == 0, "device status after the timed region"
+    edges_rank = float(e_cut + e_knn)
+    if dist is not None:
+        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+        e = torch.tensor([edges_rank, float(S)], device=dev, dtype=torch.float64)
+        dist.all_reduce(e, op=dist.ReduceOp.SUM)
+        edges_all, structs_all = float(e[0].item()), float(e[1].item())
+    else:
+        edges_all, structs_all = edges_rank, float(S)
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    hbm_gbs, sm_mhz, peak_kind = measured_peaks()
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    fp32_rate = sms * FP32_LANES_PER_SM * sm_mhz * 1e6         # lane-instructions / s
+    c_cut = box_candidates(batch, R_C)
+    kn = knn_sets[(K - 1) % n_sets]
+    dk = kn.dist.view(n_atoms, K_NN)[:, K_NN - 1].cpu().numpy().astype(np.float64)
+    nz = np.diff(batch.struct_ptr) > 0
+    dmax = np.zeros(S)
+    dmax[nz] = np.maximum.reduceat(dk, batch.struct_ptr[:-1][nz])
+    c_knn = box_candidates(batch, np.maximum(dmax, 1e-6))
+    t_cut = {"hbm_us": bytes_cut / (hbm_gbs * 1e9) * 1e6, "fp32_us": c_cut * INSTR_PER_CANDIDATE / fp32_rate * 1e6}
+    t_knn = {"hbm_us": bytes_knn / (hbm_gbs * 1e9) * 1e6, "fp32_us": c_knn * INSTR_PER_CANDIDATE / fp32_rate * 1e6}
+    roof_cut, roof_knn = max(t_cut.values()), max(t_knn.values())
+    achieved = bytes_cut / (cut_ms * 1e-3) / 1e9
+
+    # ---- end to end through the host-buffer C ABI (pinned host memory, copies inside the call)
+    e2e_steps = max(3, min(K, 10))
+    hp = [torch.from_numpy(a).pin_memory() for a in (batch.pos, batch.lattice, batch.struct_ptr)]
+
+    def host_edges(cap, with_dist):
+        t = dict(row_ptr=torch.empty(n_atoms + 1, dtype=torch.int32).pin_memory(),
+                 src=torch.empty(cap, dtype=torch.int32).pin_memory(),
+                 dst=torch.empty(cap, dtype=torch.int32).pin_memory(),
+                 offset=torch.empty((cap, 3), dtype=torch.int8).pin_memory(),
+                 vec=torch.empty((cap, 3), dtype=torch.float32).pin_memory(),
+                 dist=torch.empty(cap, dtype=torch.float32).pin_memory() if with_dist else None,
+                 n_edges=torch.zeros(1, dtype=torch.int64).pin_memory())
+        c = mg._Edges(t["row_ptr"].data_ptr(), t["src"].data_ptr(), t["dst"].data_ptr(), t["offset"].data_ptr(),
+                      t["vec"].data_ptr(), t["dist"].data_ptr() if with_dist else None, cap, t["n_edges"].data_ptr())
+        return t, c
+
+    hc, hc_c = host_edges(e_cut, False)
+    hk, hk_c = host_edges(e_knn, False)
+    hargs = [ctypes.c_void_p(t.data_ptr()) for t in hp]
+
+    def e2e_step():
+        r1 = lib.mg_cutoff_graph_host(h, hargs[0], hargs[1], hargs[2], S, n_atoms, rc32, ctypes.byref(hc_c))
+        r2 = lib.mg_knn_graph_host(h, hargs[0], hargs[1], hargs[2], S, n_atoms, K_NN, ctypes.byref(hk_c))
+        assert r1 == 0 and r2 == 0, (r1, r2)
+
+    e2e_step()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        e2e_step()
+    torch.cuda.synchronize()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    assert int(hc["n_edges"][0]) == e_cut and int(hk["n_edges"][0]) == e_knn
+    in_bytes = 2 * (12 * n_atoms + 36 * S + 4 * (S + 1))
+    out_bytes = BYTES_PER_EDGE * (e_cut + e_knn) + 2 * (4 * (n_atoms + 1) + 8 + 4)
+
+    # ---- the oracle on the host cores, bounded sample (N=1 only)
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        import oracle
+        reps = 4
+        oracle.build()
+        t0 = time.perf_counter()
+        ne = 0
+        for _ in range(reps):
+            ne += oracle.cutoff_graph(batch.pos, batch.lattice, batch.struct_ptr, R_C)["n_edges"]
+            ne += oracle.knn_graph(batch.pos, batch.lattice, batch.struct_ptr, K_NN)["n_edges"]
+        dt = time.perf_counter() - t0
+        cpu = {"value": ne / dt, "unit": "edges/s", "cores": oracle.num_threads(), "kind": "oracle",
+               "sample": f"the full {S}-structure batch, cutoff + KNN, {reps} repetitions ({dt:.1f} s)",
+               "structures_per_s": S * reps / dt}
+
+    line = {
+        "metric": "edges_per_s", "value": edges_all * K / (total_ms * 1e-3), "unit": "edges/s",
+        "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / K,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": f"BASELINE configs[2]: cutoff r_c={R_C} A + KNN k={K_NN} on {S} crystals per GPU "
+                               f"(N in [1,20], lengths 3-10 A, angles 60-120 deg, min distance 1 A), seed = rank",
+                   "n_struct": S, "n_atoms": n_atoms, "cutoff_edges": e_cut, "knn_edges": e_knn,
+                   "l2": f"outputs rotate over {n_sets} buffer sets ({n_sets * (bytes_cut + bytes_knn) / 1e6:.0f} MB "
+                         f"> 126 MB L2); inputs are {12 * n_atoms + 40 * S} B"},
+        "structures_per_s": structs_all * K / (total_ms * 1e-3),
+        "kernel_us": {"cutoff": cut_ms * 1e3, "knn": knn_ms * 1e3},
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s",
+                     "frac": achieved / hbm_gbs, "traffic": None, "kernel": "mg_cutoff_small_kernel",
+                     "peak_kind": peak_kind, "algorithmic_bytes": bytes_cut},
+        "roofline_model": {"cutoff": dict(t_cut, candidates=c_cut, roof_us=roof_cut, frac=roof_cut / (cut_ms * 1e3)),
+                           "knn": dict(t_knn, candidates=c_knn, roof_us=roof_knn, frac=roof_knn / (knn_ms * 1e3)),
+                           "fp32_peak_lane_instr_per_s": fp32_rate,
+                           "step_frac": (roof_cut + roof_knn) / (total_ms / K * 1e3)},
+        "e2e": {"value": (e_cut + e_knn) / e2e_s, "unit": "edges/s", "h2d_bytes_per_step": in_bytes,
+                "d2h_bytes_per_step": out_bytes, "ms_per_step": e2e_s * 1e3, "steps": e2e_steps},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+    }
+    if cpu is not None:
+        line["cpu_baseline"] = cpu
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=300)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+    run_gpu(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

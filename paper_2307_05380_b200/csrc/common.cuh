@@ -7,8 +7,13 @@
 #include <stdint.h>
 
 #define MG_SMALL_MAX_ATOMS 64      // structures up to this size take the pair-lane "small" path
-#define MG_BLOCK 256               // threads per CTA of the graph kernels
+#define MG_BLOCK 128               // threads per CTA of the graph kernels
 #define MG_WARPS (MG_BLOCK / 32)
+#define MG_CHUNK_COST 16384u       // scheduling budget of one cutoff chunk (see prep.cuh)
+#define MG_ROW_OVERHEAD 256u
+#define MG_STRUCT_OVERHEAD 2048u
+#define MG_MAX_ROWS 64             // rows per chunk  <= MG_CHUNK_COST / MG_ROW_OVERHEAD
+#define MG_MAX_SEGS 16             // structure segments per chunk
 
 // device status word bits (first error wins when decoded by mg_check)
 #define MGS_SINGULAR   1u
@@ -21,16 +26,22 @@
 #define MG_FLAG_AGG  1ull
 #define MG_FLAG_PFX  2ull
 
-struct StructGeom {
-    float a[3][3];      // lattice rows (FP32 as given)
-    int   n[3];         // box half widths: every edge has |tau_a| <= n[a]
-    int   dim[3];       // 2 n + 1
-    int   ncell;        // dim0*dim1*dim2 (0 if the structure is invalid)
-    float lo2, hi2;     // FP32 filter: d2 < lo2 surely inside, d2 >= hi2 surely outside
+// Per-structure record written by mg_prep_kernel (K1: search bounds) and read by the graph kernels.
+struct StructRec {
+    int n[3];           // cutoff box half widths: every edge has |tau_a| <= n[a]
+    int ncell;          // (2n0+1)(2n1+1)(2n2+1); 0 if the structure is invalid / emits nothing
+    float lo2, hi2;     // FP32 filter window: d2 < lo2 surely inside, d2 >= hi2 surely outside
     float volume;
-    float h[3];         // plane spacings
     unsigned err;       // MGS_* bits
+    unsigned rowcost;   // scheduling cost of one source row (candidates + overheads)
+    float h_dn[3];      // plane spacings rounded down  (KNN bounds)
+    float invh_up[3];   // 1 / h rounded up
+    float xmin[3], xmax[3];
+    float amax[3];      // max |component| of each lattice row (rounding-window bound)
+    int first, natoms;
+    int pad[6];
 };
+static_assert(sizeof(StructRec) == 128, "StructRec is two 64-byte lines");
 
 __device__ __forceinline__ double mg_dot3(const double *u, const double *v) {
     return u[0] * v[0] + u[1] * v[1] + u[2] * v[2];

@@ -2,15 +2,18 @@
 //
 // Problem: per source the k smallest keys (d, dst, tau_x, tau_y, tau_z) over all periodic images
 // except (i,i,0) (Alg. 2 lines 2-5, made deterministic: DESIGN.md R2, R8).
-// Method (Alg. 1, re-designed): one warp per source atom keeps the ordered stack
-// of Alg. 2 in REGISTERS — a sorted list of 64-bit keys, one or two per lane — and explores an
-// expanding box of cells: lanes <-> cells, loop over target atoms j.  After a box of half widths
-// n_a every unexplored image is farther than R_safe = min_a (n_a + 1 - spread_a) h_a
-// (closest_distance of Alg. 1 line 4; proof in DESIGN.md R11), so the search stops as soon as the
-// k-th distance is <= R_safe; otherwise the box grows to the current k-th distance ("the search
-// radius decreases over time"), which is then guaranteed to finish.
-// The FP32 keys select the k entries; their final order and the emitted vec / dist use the exact
-// FP64 distance.
+// Method (Alg. 1, re-designed): one WARP per source atom, no block-level
+// synchronisation.  The ordered stack of Alg. 2 lives in registers — a sorted list of 64-bit keys
+// (d2 bits | dst | tau), one or two per lane.  The warp explores the box of cells that provably
+// holds every image closer than a search radius R (n_a = floor(R/h_a + spread_a); every unexplored
+// image is farther than R_safe = min_a (n_a + 1 - spread_a) h_a >= R: closest_distance of Alg. 1
+// line 4, R11): lanes <-> cells, loop over target atoms j, candidates with d <= R that
+// beat the current k-th key are appended to a 32-entry shared-memory buffer; a full buffer is
+// bitonic-sorted and merged into the list (Alg. 2's "concatenate, sort, keep k", batched).
+// If fewer than k images lie within R the radius grows and the search starts again (Alg. 1's
+// while loop).  R starts from the atomic density, or from the previous k-th distance when
+// mg_update_graph supplies it.  The FP32 keys select the k entries; their final order and the
+// emitted vec / dist use the exact FP64 distance.
 #pragma once
 #include "common.cuh"
 
@@ -28,189 +31,212 @@ struct KnnArgs {
     long long *n_edges;
     float *radius_hint;         // [n_atoms] k-th distance of the previous call, or NULL
     int use_hint;               // read radius_hint as the first search radius
-    unsigned *ticket;           // [0] next chunk, [1] CTAs done
+    const StructRec *rec;
+    const int32_t *atom_struct;
+    unsigned *ctl;              // [2] next atom, [3] CTAs done
     unsigned *status;
 };
 
-struct KnnSmem {
-    float4 p[MG_SMALL_MAX_ATOMS];
-    float x[MG_SMALL_MAX_ATOMS * 3];
-    float lat[9];
-    double h[3];
-    double vol;
-    float xmin[3], xmax[3];
-    int chunk, first, natoms;
-    unsigned err;
-};
+typedef unsigned long long mg_key;
 
-// Insert `key` into the warp-resident sorted list (slot s of lane l holds rank 32 s + l).
-template <int KPL>
-__device__ __forceinline__ void mg_knn_insert(unsigned long long (&keys)[KPL], unsigned long long key,
-                                              int lane) {
+__device__ __forceinline__ mg_key mg_kmin(mg_key a, mg_key b) { return a < b ? a : b; }
+__device__ __forceinline__ mg_key mg_kmax(mg_key a, mg_key b) { return a < b ? b : a; }
+
+// ascending bitonic sort of one key per lane
+__device__ __forceinline__ mg_key mg_sort32(mg_key v, int lane) {
 #pragma unroll
-    for (int s = 0; s < KPL; ++s) {
-        const unsigned less = __ballot_sync(0xFFFFFFFFu, keys[s] < key);
-        const int pos = __popc(less);                    // sorted: the smaller keys are a lane prefix
-        const unsigned long long up = __shfl_up_sync(0xFFFFFFFFu, keys[s], 1);
-        const unsigned long long last = __shfl_sync(0xFFFFFFFFu, keys[s], 31);
-        if (pos < 32) {
-            if (lane == pos) keys[s] = key;
-            else if (lane > pos) keys[s] = up;
-            key = last;                                  // evicted rank 31 goes to the next slot
+    for (int k2 = 2; k2 <= 32; k2 <<= 1) {
+#pragma unroll
+        for (int j = k2 >> 1; j > 0; j >>= 1) {
+            const mg_key p = __shfl_xor_sync(0xFFFFFFFFu, v, j);
+            const bool up = (lane & k2) == 0, lower = (lane & j) == 0;
+            v = (lower == up) ? mg_kmin(v, p) : mg_kmax(v, p);
         }
+    }
+    return v;
+}
+
+// ascending sort of a bitonic sequence
+__device__ __forceinline__ mg_key mg_sort_bitonic(mg_key v, int lane) {
+#pragma unroll
+    for (int j = 16; j > 0; j >>= 1) {
+        const mg_key p = __shfl_xor_sync(0xFFFFFFFFu, v, j);
+        v = (lane & j) == 0 ? mg_kmin(v, p) : mg_kmax(v, p);
+    }
+    return v;
+}
+
+// Merge up to 32 unsorted keys (one per lane, MG_KEY_INF = none) into the sorted list
+// (slot s of lane l holds rank 32 s + l); what falls off the end is dropped.
+template <int KPL>
+__device__ __forceinline__ void mg_knn_merge(mg_key (&keys)[KPL], mg_key b, int lane) {
+    b = mg_sort32(b, lane);
+    mg_key rb = __shfl_sync(0xFFFFFFFFu, b, 31 - lane);
+    if (KPL == 1) {
+        keys[0] = mg_sort_bitonic(mg_kmin(keys[0], rb), lane);
+    } else {
+        mg_key t = mg_sort_bitonic(mg_kmin(keys[KPL - 1], rb), lane);   // 32 smallest of (top slot, b)
+        const mg_key rt = __shfl_sync(0xFFFFFFFFu, t, 31 - lane);
+        const mg_key lo = mg_kmin(keys[0], rt), hi = mg_kmax(keys[0], rt);
+        keys[0] = mg_sort_bitonic(lo, lane);
+        keys[KPL - 1] = mg_sort_bitonic(hi, lane);
     }
 }
 
-__device__ __forceinline__ unsigned long long mg_knn_key(float d2, int j, int t0, int t1, int t2) {
-    return ((unsigned long long)__float_as_uint(d2) << 32) | ((unsigned long long)(unsigned)j << 24) |
-           ((unsigned long long)(unsigned)(t0 + 128) << 16) | ((unsigned)(t1 + 128) << 8) |
-           (unsigned)(t2 + 128);
+__device__ __forceinline__ mg_key mg_knn_key(float d2, int j, int t0, int t1, int t2) {
+    return ((mg_key)__float_as_uint(d2) << 32) | ((mg_key)(unsigned)j << 24) |
+           ((mg_key)(unsigned)(t0 + 128) << 16) | ((unsigned)(t1 + 128) << 8) | (unsigned)(t2 + 128);
 }
 
-// Search + emit for one source atom i of the staged structure; called by a full warp.
+// Search + emit for source atom gi = R.first + i; sp = this warp's cartesian positions of the
+// structure, buf = this warp's 32-entry candidate buffer.  Called by a full warp.
 template <int KPL>
-__device__ inline void mg_knn_source(const KnnSmem &sm, const KnnArgs &A, int i, int lane) {
-    const int N = sm.natoms, k = A.k;
+__device__ inline void mg_knn_source(const KnnArgs &A, const StructRec &R, const float *lat9,
+                                     const float4 *sp, mg_key *buf, int i, int lane) {
+    const int N = R.natoms, k = A.k, gi = R.first + i;
     const int kslot = (k - 1) >> 5, klane = (k - 1) & 31;
-    unsigned long long keys[KPL];
-#pragma unroll
-    for (int s = 0; s < KPL; ++s) keys[s] = MG_KEY_INF;
-    unsigned long long thr = MG_KEY_INF;
-    float thr_d2 = __int_as_float(0x7f800000);
-    const float4 pi = sm.p[i];
-    float a[3][3], hf[3], lo_off[3], hi_off[3];
-    double spread[3], amax[3];
+    const float *xs = A.pos + 3 * (size_t)R.first;
+    const float4 pi = sp[i];
+    float a[3][3], lo_off[3], hi_off[3], spread[3];
     float xabs = 1.f;
 #pragma unroll
     for (int r = 0; r < 3; ++r) {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) a[r][c] = sm.lat[3 * r + c];
-        hf[r] = __double2float_rd(sm.h[r] * (1.0 - 1e-6));
-        const float xi = sm.x[3 * i + r];
-        lo_off[r] = sm.xmin[r] - xi;                 // exact or rounded: only used for pruning,
-        hi_off[r] = sm.xmax[r] - xi;                 // with hf rounded down and a safety factor
-        spread[r] = (double)sm.xmax[r] - (double)sm.xmin[r];
-        amax[r] = fmax(fabs((double)a[r][0]), fmax(fabs((double)a[r][1]), fabs((double)a[r][2])));
-        xabs = fmaxf(xabs, fmaxf(fabsf(sm.xmin[r]), fabsf(sm.xmax[r])));
+        for (int c = 0; c < 3; ++c) a[r][c] = lat9[3 * r + c];
+        const float xi = xs[3 * i + r];
+        lo_off[r] = R.xmin[r] - xi;                  // only used for pruning, with h rounded down
+        hi_off[r] = R.xmax[r] - xi;                  // and a safety factor
+        spread[r] = __fadd_ru(R.xmax[r], -R.xmin[r]);
+        xabs = fmaxf(xabs, fmaxf(fabsf(R.xmin[r]), fabsf(R.xmax[r])));
     }
-    const int gi = sm.first + i;
-    double R;
-    if (A.use_hint && A.radius_hint[gi] > 0.f) R = 1.05 * (double)A.radius_hint[gi] + 1e-3;
-    else R = 1.1 * cbrt(0.2387324146 * (double)(k + 1) * sm.vol / (double)N);
-    int nprev[3] = {-1, -1, -1};
+    float Rad;
+    if (A.use_hint && A.radius_hint[gi] > 0.f) Rad = 1.03f * A.radius_hint[gi] + 1e-3f;
+    else Rad = 1.25f * cbrtf(0.2387324f * (float)(k + 1) * R.volume / (float)N);
+    mg_key keys[KPL];
+    mg_key thr;
     bool failed = false;
     for (;;) {
+        // ---- box that holds every image with d < Rad
         int n[3];
-        double rsafe = 1e300, M = 0.0;
+        float rsafe = 3.0e38f, M = 0.f;
         bool range_ok = true;
 #pragma unroll
         for (int r = 0; r < 3; ++r) {
-            double nn = floor(R / sm.h[r] * (1.0 + 1e-6) + spread[r]);
-            if (nn < (double)nprev[r]) nn = (double)nprev[r];
-            if (!(nn <= 127.0)) { range_ok = false; nn = 127.0; }
+            float nn = floorf(__fmaf_ru(Rad, R.invh_up[r], spread[r]));
+            if (!(nn <= 127.f)) { range_ok = false; nn = 127.f; }
             n[r] = (int)nn;
-            rsafe = fmin(rsafe, (nn + 1.0 - spread[r]) * sm.h[r]);
-            M += (nn + 2.0 * (double)xabs) * amax[r];
+            rsafe = fminf(rsafe, __fmul_rd(__fadd_rd(nn + 1.f, -spread[r]), R.h_dn[r]));
+            M += (nn + 2.f * xabs) * R.amax[r];
         }
-        const double W = 3.5 * 12.0 * 5.9604644775390625e-8 * M;
+        const float W = 3.5f * 12.f * 5.9604645e-8f * M * 1.01f;   // FP32 error bound of a distance
+        const float lim = fminf(Rad, rsafe);
+        const float lim2 = __fmul_ru(lim, lim);
+#pragma unroll
+        for (int s = 0; s < KPL; ++s) keys[s] = MG_KEY_INF;
+        thr = MG_KEY_INF;
+        float thr_d2 = lim2;
+        int nb = 0;
         const int D1 = 2 * n[1] + 1, D2 = 2 * n[2] + 1;
         const int ncell = (2 * n[0] + 1) * D1 * D2;
+        const float inv12 = 1.f / (float)(D1 * D2), inv2 = 1.f / (float)D2;
         for (int c0 = 0; c0 < ncell; c0 += 32) {
             const int c = c0 + lane;
-            const int u0 = c / (D1 * D2), rem = c - u0 * (D1 * D2), u1 = rem / D2;
+            const bool big = ncell >= (1 << 20);            // float reciprocal is exact below 2^20 only
+            const int u0 = big ? c / (D1 * D2) : __float2int_rz(((float)c + 0.5f) * inv12), rem = c - u0 * (D1 * D2);
+            const int u1 = big ? rem / D2 : __float2int_rz(((float)rem + 0.5f) * inv2);
             const int t0 = u0 - n[0], t1 = u1 - n[1], t2 = rem - u1 * D2 - n[2];
-            bool alive = c < ncell && !(abs(t0) <= nprev[0] && abs(t1) <= nprev[1] && abs(t2) <= nprev[2]);
             const float f0 = (float)t0, f1 = (float)t1, f2 = (float)t2;
             // lower bound of the distance to any image in this cell: max_a gap_a h_a
-            const float g0 = fmaxf(0.f, fmaxf(f0 + lo_off[0], -(f0 + hi_off[0]))) * hf[0];
-            const float g1 = fmaxf(0.f, fmaxf(f1 + lo_off[1], -(f1 + hi_off[1]))) * hf[1];
-            const float g2 = fmaxf(0.f, fmaxf(f2 + lo_off[2], -(f2 + hi_off[2]))) * hf[2];
+            const float g0 = fmaxf(0.f, fmaxf(f0 + lo_off[0], -(f0 + hi_off[0]))) * R.h_dn[0];
+            const float g1 = fmaxf(0.f, fmaxf(f1 + lo_off[1], -(f1 + hi_off[1]))) * R.h_dn[1];
+            const float g2 = fmaxf(0.f, fmaxf(f2 + lo_off[2], -(f2 + hi_off[2]))) * R.h_dn[2];
             const float lb = fmaxf(g0, fmaxf(g1, g2)) * 0.99999f;
-            alive = alive && lb * lb <= thr_d2;
+            const bool alive = c < ncell && lb * lb <= thr_d2;
             if (!__any_sync(0xFFFFFFFFu, alive)) continue;
             const float Tx = __fmaf_rn(f2, a[2][0], __fmaf_rn(f1, a[1][0], __fmul_rn(f0, a[0][0])));
             const float Ty = __fmaf_rn(f2, a[2][1], __fmaf_rn(f1, a[1][1], __fmul_rn(f0, a[0][1])));
             const float Tz = __fmaf_rn(f2, a[2][2], __fmaf_rn(f1, a[1][2], __fmul_rn(f0, a[0][2])));
             const bool home = (t0 | t1 | t2) == 0;
             for (int j = 0; j < N; ++j) {
-                const float4 pj = sm.p[j];
+                const float4 pj = sp[j];
                 const float d2 = mg_d2(__fsub_rn(pj.x, pi.x), __fsub_rn(pj.y, pi.y),
                                        __fsub_rn(pj.z, pi.z), Tx, Ty, Tz);
                 bool cand = alive && d2 <= thr_d2 && !(home && j == i);
-                const unsigned long long key = cand ? mg_knn_key(d2, j, t0, t1, t2) : MG_KEY_INF;
-                cand = key < thr;
-                unsigned m = __ballot_sync(0xFFFFFFFFu, cand);
+                const mg_key key = mg_knn_key(d2, j, t0, t1, t2);
+                cand = cand && key < thr;
+                const unsigned m = __ballot_sync(0xFFFFFFFFu, cand);
                 if (m) {
-                    while (m) {
-                        const int srcl = __ffs(m) - 1;
-                        m &= m - 1;
-                        const unsigned long long kk = __shfl_sync(0xFFFFFFFFu, key, srcl);
-                        if (kk < thr) {
-                            mg_knn_insert<KPL>(keys, kk, lane);
-                            thr = __shfl_sync(0xFFFFFFFFu, keys[kslot], klane);
-                        }
+                    const int pos = nb + __popc(m & ((1u << lane) - 1u));
+                    if (cand && pos < 32) buf[pos] = key;
+                    nb += __popc(m);
+                    if (nb >= 32) {                       // buffer full: sort + merge (Alg. 2)
+                        __syncwarp();
+                        mg_knn_merge<KPL>(keys, buf[lane], lane);
+                        thr = __shfl_sync(0xFFFFFFFFu, keys[kslot], klane);
+                        if (thr != MG_KEY_INF) thr_d2 = fminf(lim2, __uint_as_float((unsigned)(thr >> 32)));
+                        __syncwarp();
+                        if (cand && pos >= 32) buf[pos - 32] = key;
+                        nb -= 32;
                     }
-                    if (thr != MG_KEY_INF) thr_d2 = __uint_as_float((unsigned)(thr >> 32));
                 }
             }
         }
-        nprev[0] = n[0]; nprev[1] = n[1]; nprev[2] = n[2];
-        if (thr != MG_KEY_INF) {
-            const double dk = sqrt((double)thr_d2) + W;
-            if (dk <= rsafe) break;
-            if (!range_ok) { failed = true; break; }
-            R = dk * (1.0 + 1e-6);
-        } else {
-            if (!range_ok) { failed = true; break; }
-            R = fmax(1.5 * R, 1.01 * rsafe);
+        if (nb > 0) {
+            __syncwarp();
+            mg_knn_merge<KPL>(keys, lane < nb ? buf[lane] : MG_KEY_INF, lane);
+            thr = __shfl_sync(0xFFFFFFFFu, keys[kslot], klane);
+            __syncwarp();
         }
+        // ---- Alg. 1 line 4: stop when the k-th distance is inside the fully explored radius
+        if (thr != MG_KEY_INF) {
+            const float dk = sqrtf(__uint_as_float((unsigned)(thr >> 32)));
+            if (__fadd_ru(dk, 2.f * W) <= lim) break;
+        }
+        if (!range_ok) { failed = true; break; }
+        Rad = 1.3f * fmaxf(Rad, rsafe) + 4.f * W;
     }
     if (failed && lane == 0) atomicOr(A.status, MGS_OFFSET);
     // ---- exact FP64 distance of the selected entries, final order by (d, dst, tau), emit
     double dmax = 0.0;
+    double dd[KPL], vv[KPL][3];
+#pragma unroll
+    for (int s = 0; s < KPL; ++s) {
+        const unsigned tie = (unsigned)keys[s];
+        const bool valid = 32 * s + lane < k && keys[s] != MG_KEY_INF;
+        dd[s] = 1e300;
+        if (valid)
+            dd[s] = mg_exact_vec(xs + 3 * i, xs + 3 * (int)((tie >> 24) & 0xFFu), (int)((tie >> 16) & 0xFFu) - 128,
+                                 (int)((tie >> 8) & 0xFFu) - 128, (int)(tie & 0xFFu) - 128, lat9, vv[s]);
+    }
 #pragma unroll
     for (int s = 0; s < KPL; ++s) {
         const int r = 32 * s + lane;
-        const bool valid = r < k && keys[s] != MG_KEY_INF;
         const unsigned tie = (unsigned)keys[s];
-        const int j = valid ? (int)((tie >> 24) & 0xFFu) : i;
-        const int t0 = valid ? (int)((tie >> 16) & 0xFFu) - 128 : 0;
-        const int t1 = valid ? (int)((tie >> 8) & 0xFFu) - 128 : 0;
-        const int t2 = valid ? (int)(tie & 0xFFu) - 128 : 0;
-        double v[3];
-        double d = mg_exact_vec(sm.x + 3 * i, sm.x + 3 * j, t0, t1, t2, sm.lat, v);
-        if (!valid) d = 1e300;
+        const bool valid = r < k && keys[s] != MG_KEY_INF;
         int rank = 0;
 #pragma unroll
         for (int s2 = 0; s2 < KPL; ++s2) {
-            // my own slot-s2 values, to be broadcast
             const unsigned tie2 = (unsigned)keys[s2];
-            const bool valid2 = 32 * s2 + lane < k && keys[s2] != MG_KEY_INF;
-            double d2v = 1e300;
-            if (s2 == s) d2v = d;
-            else if (valid2) {
-                double vv[3];
-                d2v = mg_exact_vec(sm.x + 3 * i, sm.x + 3 * (int)((tie2 >> 24) & 0xFFu),
-                                   (int)((tie2 >> 16) & 0xFFu) - 128, (int)((tie2 >> 8) & 0xFFu) - 128,
-                                   (int)(tie2 & 0xFFu) - 128, sm.lat, vv);
-            }
             const int cnt2 = min(32, k - 32 * s2);
             for (int l = 0; l < cnt2; ++l) {
-                const double od = __shfl_sync(0xFFFFFFFFu, d2v, l);
+                const double od = __shfl_sync(0xFFFFFFFFu, dd[s2], l);
                 const unsigned ot = __shfl_sync(0xFFFFFFFFu, tie2, l);
-                rank += (od < d || (od == d && ot < tie)) ? 1 : 0;
+                rank += (od < dd[s] || (od == dd[s] && ot < tie)) ? 1 : 0;
             }
         }
         if (r < k) {
             const long long e = (long long)k * gi + (valid ? rank : r);
+            const int j = valid ? (int)((tie >> 24) & 0xFFu) : i;
             A.src[e] = gi;
-            A.dst[e] = sm.first + j;
-            A.offset[3 * e] = (int8_t)t0; A.offset[3 * e + 1] = (int8_t)t1; A.offset[3 * e + 2] = (int8_t)t2;
-            A.vec[3 * e] = valid ? (float)v[0] : 0.f;
-            A.vec[3 * e + 1] = valid ? (float)v[1] : 0.f;
-            A.vec[3 * e + 2] = valid ? (float)v[2] : 0.f;
-            if (A.dist) A.dist[e] = valid ? (float)d : 0.f;
-            if (valid) dmax = fmax(dmax, d);
+            A.dst[e] = R.first + j;
+            A.offset[3 * e] = valid ? (int8_t)((int)((tie >> 16) & 0xFFu) - 128) : (int8_t)0;
+            A.offset[3 * e + 1] = valid ? (int8_t)((int)((tie >> 8) & 0xFFu) - 128) : (int8_t)0;
+            A.offset[3 * e + 2] = valid ? (int8_t)((int)(tie & 0xFFu) - 128) : (int8_t)0;
+            A.vec[3 * e] = valid ? (float)vv[s][0] : 0.f;
+            A.vec[3 * e + 1] = valid ? (float)vv[s][1] : 0.f;
+            A.vec[3 * e + 2] = valid ? (float)vv[s][2] : 0.f;
+            if (A.dist) A.dist[e] = valid ? (float)dd[s] : 0.f;
+            if (valid) dmax = fmax(dmax, dd[s]);
         }
     }
     if (A.radius_hint) {
@@ -223,74 +249,50 @@ __device__ inline void mg_knn_source(const KnnSmem &sm, const KnnArgs &A, int i,
 template <int KPL>
 __global__ void __launch_bounds__(MG_BLOCK)
 mg_knn_small_kernel(const KnnArgs A) {
-    __shared__ KnnSmem sm;
+    __shared__ float4 s_p[MG_WARPS][MG_SMALL_MAX_ATOMS];
+    __shared__ mg_key s_buf[MG_WARPS][32];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     for (long long t = (long long)blockIdx.x * MG_BLOCK + tid; t <= A.n_atoms; t += (long long)gridDim.x * MG_BLOCK)
         A.row_ptr[t] = (int)((long long)A.k * t);
     if (blockIdx.x == 0 && tid == 0) *A.n_edges = (long long)A.k * A.n_atoms;
+    float4 *sp = s_p[warp];
     for (;;) {
-        __syncthreads();
-        if (tid == 0) sm.chunk = (int)atomicAdd(A.ticket, 1u);
-        __syncthreads();
-        const int s = sm.chunk;
-        if (s >= A.n_struct) break;
-        if (tid == 0) {
-            sm.first = A.struct_ptr[s];
-            sm.natoms = A.struct_ptr[s + 1] - sm.first;
-        }
-        if (tid >= 32 && tid < 41) sm.lat[tid - 32] = A.lattice[9 * (size_t)s + (tid - 32)];
-        __syncthreads();
-        int N = sm.natoms;
-        if (N > MG_SMALL_MAX_ATOMS) {
-            if (tid == 0) atomicOr(A.status, MGS_UNSUPPORTED);
-            continue;
-        }
-        if (tid < 3 * N) sm.x[tid] = A.pos[3 * (size_t)sm.first + tid];
-        __syncthreads();
-        if (tid == 0) {
-            double vol;
-            sm.err = mg_cell_spacings(sm.lat, &vol, sm.h);
-            sm.vol = vol;
-            bool finite = true;
-            for (int a = 0; a < 3; ++a) {
-                float lo = 0.f, hi = 0.f;
-                for (int i = 0; i < N; ++i) {
-                    const float v = sm.x[3 * i + a];
-                    finite = finite && isfinite(v);
-                    lo = i ? fminf(lo, v) : v;
-                    hi = i ? fmaxf(hi, v) : v;
-                }
-                sm.xmin[a] = lo; sm.xmax[a] = hi;
-            }
-            if (!finite) sm.err |= MGS_NONFINITE;
-            if (sm.err) atomicOr(A.status, sm.err);
-        }
-        __syncthreads();
-        if (tid < N) {
-            const float x0 = sm.x[3 * tid], x1 = sm.x[3 * tid + 1], x2 = sm.x[3 * tid + 2];
-            float4 p;
-            p.x = __fmaf_rn(x2, sm.lat[6], __fmaf_rn(x1, sm.lat[3], __fmul_rn(x0, sm.lat[0])));
-            p.y = __fmaf_rn(x2, sm.lat[7], __fmaf_rn(x1, sm.lat[4], __fmul_rn(x0, sm.lat[1])));
-            p.z = __fmaf_rn(x2, sm.lat[8], __fmaf_rn(x1, sm.lat[5], __fmul_rn(x0, sm.lat[2])));
-            p.w = 0.f;
-            sm.p[tid] = p;
-        }
-        __syncthreads();
-        if (sm.err) {
-            // invalid lattice: rows are filled with placeholders (src = dst, zero vec); see mg_check
-            for (int e = tid; e < N * A.k; e += MG_BLOCK) {
-                const long long o = (long long)A.k * sm.first + e;
-                A.src[o] = sm.first + e / A.k; A.dst[o] = sm.first + e / A.k;
+        int g = 0;
+        if (lane == 0) g = (int)atomicAdd(A.ctl + 2, 1u);
+        g = __shfl_sync(0xFFFFFFFFu, g, 0);
+        if (g >= A.n_atoms) break;
+        const int s = A.atom_struct[g];
+        const StructRec R = A.rec[s];
+        const float *lat9 = A.lattice + 9 * (size_t)s;
+        const int i = g - R.first;
+        if (R.err) {
+            // invalid lattice / unsupported size: placeholder rows (src = dst, zero vec); mg_check reports
+            for (int e = lane; e < A.k; e += 32) {
+                const long long o = (long long)A.k * g + e;
+                A.src[o] = g; A.dst[o] = g;
                 A.offset[3 * o] = 0; A.offset[3 * o + 1] = 0; A.offset[3 * o + 2] = 0;
                 A.vec[3 * o] = 0.f; A.vec[3 * o + 1] = 0.f; A.vec[3 * o + 2] = 0.f;
                 if (A.dist) A.dist[o] = 0.f;
             }
             continue;
         }
-        for (int i = warp; i < N; i += MG_WARPS) mg_knn_source<KPL>(sm, A, i, lane);
+        __syncwarp();
+        for (int j = lane; j < R.natoms; j += 32) {
+            const float *x = A.pos + 3 * (size_t)(R.first + j);
+            const float x0 = x[0], x1 = x[1], x2 = x[2];
+            float4 p;
+            p.x = __fmaf_rn(x2, lat9[6], __fmaf_rn(x1, lat9[3], __fmul_rn(x0, lat9[0])));
+            p.y = __fmaf_rn(x2, lat9[7], __fmaf_rn(x1, lat9[4], __fmul_rn(x0, lat9[1])));
+            p.z = __fmaf_rn(x2, lat9[8], __fmaf_rn(x1, lat9[5], __fmul_rn(x0, lat9[2])));
+            p.w = 0.f;
+            sp[j] = p;
+        }
+        __syncwarp();
+        mg_knn_source<KPL>(A, R, lat9, sp, s_buf[warp], i, lane);
     }
+    __syncthreads();
     if (tid == 0) {
         __threadfence();
-        if (atomicAdd(A.ticket + 1, 1u) == gridDim.x - 1) { A.ticket[0] = 0u; A.ticket[1] = 0u; }
+        if (atomicAdd(A.ctl + 3, 1u) == gridDim.x - 1) { A.ctl[2] = 0u; A.ctl[3] = 0u; }
     }
 }

@@ -10,13 +10,20 @@
 #include <string.h>
 
 #include "common.cuh"
+#include "prep.cuh"
 #include "cutoff_small.cuh"
 #include "knn_small.cuh"
 
 struct mg_ctx {
     int device = 0;
     int sm_count = 0;
-    unsigned *d_ctl = nullptr;            // [0..1] cutoff ticket/done, [2..3] knn ticket/done, [4] status
+    unsigned *d_ctl = nullptr;            // [0..1] cutoff ticket/done, [2..3] knn ticket/done, [4] status,
+                                          // [5] prep blocks done, [6] number of cutoff chunks
+    StructRec *d_rec = nullptr;           // per-structure records (prep.cuh)
+    unsigned long long *d_cost = nullptr; // [n_struct+1] cost prefix
+    size_t rec_cap = 0;
+    int32_t *d_atom_struct = nullptr;     // [n_atoms]
+    size_t atom_cap = 0;
     unsigned long long *d_desc = nullptr; // look-back descriptors
     size_t desc_cap = 0;
     int32_t *d_rowptr_tmp = nullptr;      // for mg_cutoff_count
@@ -99,6 +106,9 @@ extern "C" void mg_destroy(mg_ctx *c) {
     cudaSetDevice(c->device);
     cudaFree(c->d_ctl);
     cudaFree(c->d_desc);
+    cudaFree(c->d_rec);
+    cudaFree(c->d_cost);
+    cudaFree(c->d_atom_struct);
     cudaFree(c->d_rowptr_tmp);
     cudaFree(c->d_count);
     for (int i = 0; i < 9; ++i) cudaFree(c->h_dev[i]);
@@ -108,13 +118,28 @@ extern "C" void mg_destroy(mg_ctx *c) {
 extern "C" mg_status mg_reserve(mg_ctx *c, int32_t n_struct, int32_t n_atoms) {
     if (!c || n_struct < 0 || n_atoms < 0) return MG_ERR_INVALID_ARG;
     MG_CUDA(cudaSetDevice(c->device));
-    if ((size_t)n_struct > c->desc_cap) {
-        const size_t cap = (size_t)n_struct + 1024;
+    if ((size_t)n_atoms + 2 > c->desc_cap) {            // cutoff chunks <= n_atoms + 1 (prep.cuh)
+        const size_t cap = (size_t)n_atoms + 1026;
         cudaFree(c->d_desc);
         c->d_desc = nullptr; c->desc_cap = 0;
         MG_CUDA(cudaMalloc(&c->d_desc, cap * sizeof(unsigned long long)));
         MG_CUDA(cudaMemset(c->d_desc, 0, cap * sizeof(unsigned long long)));
         c->desc_cap = cap;
+    }
+    if ((size_t)n_struct + 1 > c->rec_cap) {
+        const size_t cap = (size_t)n_struct + 1025;
+        cudaFree(c->d_rec); cudaFree(c->d_cost);
+        c->d_rec = nullptr; c->d_cost = nullptr; c->rec_cap = 0;
+        MG_CUDA(cudaMalloc(&c->d_rec, cap * sizeof(StructRec)));
+        MG_CUDA(cudaMalloc(&c->d_cost, cap * sizeof(unsigned long long)));
+        c->rec_cap = cap;
+    }
+    if ((size_t)n_atoms + 1 > c->atom_cap) {
+        const size_t cap = (size_t)n_atoms + 1025;
+        cudaFree(c->d_atom_struct);
+        c->d_atom_struct = nullptr; c->atom_cap = 0;
+        MG_CUDA(cudaMalloc(&c->d_atom_struct, cap * sizeof(int32_t)));
+        c->atom_cap = cap;
     }
     if ((size_t)n_atoms + 1 > c->rowptr_cap) {
         const size_t cap = (size_t)n_atoms + 1025;
@@ -142,11 +167,23 @@ static bool bad_edges(const mg_edges *o, long long need) {
     return o->capacity < need;
 }
 
+static mg_status launch_prep(mg_ctx *c, const float *pos, const float *lat, const int32_t *sp,
+                             int32_t n_struct, int32_t n_atoms, float r_c, cudaStream_t st) {
+    PrepArgs P;
+    P.pos = pos; P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms;
+    P.r_c = r_c; P.rec = c->d_rec; P.cost_prefix = c->d_cost; P.atom_struct = c->d_atom_struct;
+    P.ctl = c->d_ctl; P.status = c->d_ctl + 4;
+    mg_prep_kernel<<<(n_struct + MG_PREP_BLOCK - 1) / MG_PREP_BLOCK, MG_PREP_BLOCK, 0, st>>>(P);
+    MG_CUDA(cudaGetLastError());
+    c->launches += 1;
+    return MG_OK;
+}
+
 static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, const int32_t *sp,
                                int32_t n_struct, int32_t n_atoms, float r_c, const mg_edges *o,
                                int count_only, cudaStream_t st) {
     MG_CUDA(cudaSetDevice(c->device));
-    mg_status rs = mg_reserve(c, n_struct, count_only ? n_atoms : 0);
+    mg_status rs = mg_reserve(c, n_struct, n_atoms);
     if (rs != MG_OK) return rs;
     if (n_struct == 0) {
         MG_CUDA(cudaMemsetAsync(o->row_ptr, 0, sizeof(int32_t), st));
@@ -158,15 +195,18 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
         MG_CUDA(cudaMemsetAsync(c->d_desc, 0, c->desc_cap * sizeof(unsigned long long), st));
         c->epoch = 1u;
     }
+    rs = launch_prep(c, pos, lat, sp, n_struct, n_atoms, r_c, st);
+    if (rs != MG_OK) return rs;
     CutoffArgs A;
     A.pos = pos; A.lattice = lat; A.struct_ptr = sp;
     A.n_struct = n_struct; A.n_atoms = n_atoms; A.r_c = r_c;
     A.row_ptr = o->row_ptr; A.src = o->src; A.dst = o->dst; A.offset = o->offset;
     A.vec = o->vec; A.dist = o->dist; A.capacity = o->capacity; A.n_edges = (long long *)o->n_edges;
-    A.desc = c->d_desc; A.ticket = c->d_ctl; A.status = c->d_ctl + 4;
+    A.rec = c->d_rec; A.cost_prefix = c->d_cost;
+    A.desc = c->d_desc; A.ctl = c->d_ctl; A.status = c->d_ctl + 4;
     A.epoch = c->epoch; A.count_only = count_only;
     int grid = c->sm_count * c->cutoff_occ;
-    if (grid > n_struct) grid = n_struct;
+    if (grid > n_atoms + 1) grid = n_atoms + 1;
     mg_cutoff_small_kernel<<<grid, MG_BLOCK, sizeof(CutoffSmem), st>>>(A);
     MG_CUDA(cudaGetLastError());
     c->launches += 1;
@@ -205,16 +245,23 @@ static mg_status launch_knn(mg_ctx *c, const float *pos, const float *lat, const
                             int32_t n_struct, int32_t n_atoms, int32_t k, const mg_edges *o,
                             float *hint, int use_hint, cudaStream_t st) {
     MG_CUDA(cudaSetDevice(c->device));
+    mg_status rs = mg_reserve(c, n_struct, n_atoms);
+    if (rs != MG_OK) return rs;
+    if (n_struct > 0) {
+        rs = launch_prep(c, pos, lat, sp, n_struct, n_atoms, 0.f, st);
+        if (rs != MG_OK) return rs;
+    }
     KnnArgs A;
     A.pos = pos; A.lattice = lat; A.struct_ptr = sp;
     A.n_struct = n_struct; A.n_atoms = n_atoms; A.k = k;
     A.row_ptr = o->row_ptr; A.src = o->src; A.dst = o->dst; A.offset = o->offset;
     A.vec = o->vec; A.dist = o->dist; A.n_edges = (long long *)o->n_edges;
     A.radius_hint = hint; A.use_hint = use_hint;
-    A.ticket = c->d_ctl + 2; A.status = c->d_ctl + 4;
+    A.rec = c->d_rec; A.atom_struct = c->d_atom_struct;
+    A.ctl = c->d_ctl; A.status = c->d_ctl + 4;
     const int kpl = k <= 32 ? 0 : 1;
     int grid = c->sm_count * c->knn_occ[kpl];
-    if (grid > n_struct) grid = n_struct;
+    if (grid > (n_atoms + MG_WARPS - 1) / MG_WARPS) grid = (n_atoms + MG_WARPS - 1) / MG_WARPS;
     if (grid < 1) grid = 1;
     if (kpl == 0) mg_knn_small_kernel<1><<<grid, MG_BLOCK, 0, st>>>(A);
     else mg_knn_small_kernel<2><<<grid, MG_BLOCK, 0, st>>>(A);
