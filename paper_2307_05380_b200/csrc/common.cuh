@@ -9,11 +9,10 @@
 #define MG_SMALL_MAX_ATOMS 64      // structures up to this size take the pair-lane "small" path
 #define MG_BLOCK 128               // threads per CTA of the graph kernels
 #define MG_WARPS (MG_BLOCK / 32)
-#define MG_CHUNK_COST 16384u       // scheduling budget of one cutoff chunk (see prep.cuh)
-#define MG_ROW_OVERHEAD 256u
-#define MG_STRUCT_OVERHEAD 2048u
-#define MG_MAX_ROWS 64             // rows per chunk  <= MG_CHUNK_COST / MG_ROW_OVERHEAD
-#define MG_MAX_SEGS 16             // structure segments per chunk
+#define MG_TASK_BUDGET 6144u        // candidates per cutoff task (one warp, one row group)
+#define MG_TASK_ROWS 32             // rows per task: one lane per row in the scan / look-back
+#define MG_WT 192                   // per-warp translation-table tile (cells)
+#define MG_WS 768                   // per-warp stash entries (x2: double buffered)
 
 // device status word bits (first error wins when decoded by mg_check)
 #define MGS_SINGULAR   1u
@@ -33,13 +32,14 @@ struct StructRec {
     float lo2, hi2;     // FP32 filter window: d2 < lo2 surely inside, d2 >= hi2 surely outside
     float volume;
     unsigned err;       // MGS_* bits
-    unsigned rowcost;   // scheduling cost of one source row (candidates + overheads)
+    int rpt;            // cutoff: source rows per task
+    int cap;            // cutoff: stash entries reserved per row
     float h_dn[3];      // plane spacings rounded down  (KNN bounds)
     float invh_up[3];   // 1 / h rounded up
     float xmin[3], xmax[3];
     float amax[3];      // max |component| of each lattice row (rounding-window bound)
     int first, natoms;
-    int pad[6];
+    int pad[5];
 };
 static_assert(sizeof(StructRec) == 128, "StructRec is two 64-byte lines");
 

@@ -11,7 +11,7 @@
 
 #include "common.cuh"
 #include "prep.cuh"
-#include "cutoff_small.cuh"
+#include "cutoff_warp.cuh"
 #include "knn_small.cuh"
 
 struct mg_ctx {
@@ -20,7 +20,7 @@ struct mg_ctx {
     unsigned *d_ctl = nullptr;            // [0..1] cutoff ticket/done, [2..3] knn ticket/done, [4] status,
                                           // [5] prep blocks done, [6] number of cutoff chunks
     StructRec *d_rec = nullptr;           // per-structure records (prep.cuh)
-    unsigned long long *d_cost = nullptr; // [n_struct+1] cost prefix
+    unsigned *d_cost = nullptr;           // [n_struct+1] task prefix
     size_t rec_cap = 0;
     int32_t *d_atom_struct = nullptr;     // [n_atoms]
     size_t atom_cap = 0;
@@ -91,9 +91,9 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
     if (cudaMalloc(&c->d_ctl, 8 * sizeof(unsigned)) != cudaSuccess ||
         cudaMemset(c->d_ctl, 0, 8 * sizeof(unsigned)) != cudaSuccess ||
         cudaMalloc(&c->d_count, sizeof(long long)) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
-    if (cudaFuncSetAttribute(mg_cutoff_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)sizeof(CutoffSmem)) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->cutoff_occ, mg_cutoff_small_kernel, MG_BLOCK, sizeof(CutoffSmem));
+    if (cudaFuncSetAttribute(mg_cutoff_warp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)(MG_WARPS * sizeof(WarpSmem))) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->cutoff_occ, mg_cutoff_warp_kernel, MG_BLOCK, (MG_WARPS * sizeof(WarpSmem)));
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->knn_occ[0], mg_knn_small_kernel<1>, MG_BLOCK, 0);
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->knn_occ[1], mg_knn_small_kernel<2>, MG_BLOCK, 0);
     if (c->cutoff_occ < 1 || c->knn_occ[0] < 1 || c->knn_occ[1] < 1) { mg_destroy(c); return MG_ERR_CUDA; }
@@ -131,7 +131,7 @@ extern "C" mg_status mg_reserve(mg_ctx *c, int32_t n_struct, int32_t n_atoms) {
         cudaFree(c->d_rec); cudaFree(c->d_cost);
         c->d_rec = nullptr; c->d_cost = nullptr; c->rec_cap = 0;
         MG_CUDA(cudaMalloc(&c->d_rec, cap * sizeof(StructRec)));
-        MG_CUDA(cudaMalloc(&c->d_cost, cap * sizeof(unsigned long long)));
+        MG_CUDA(cudaMalloc(&c->d_cost, cap * sizeof(unsigned)));
         c->rec_cap = cap;
     }
     if ((size_t)n_atoms + 1 > c->atom_cap) {
@@ -171,9 +171,9 @@ static mg_status launch_prep(mg_ctx *c, const float *pos, const float *lat, cons
                              int32_t n_struct, int32_t n_atoms, float r_c, cudaStream_t st) {
     PrepArgs P;
     P.pos = pos; P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms;
-    P.r_c = r_c; P.rec = c->d_rec; P.cost_prefix = c->d_cost; P.atom_struct = c->d_atom_struct;
+    P.r_c = r_c; P.rec = c->d_rec; P.task_prefix = c->d_cost; P.atom_struct = c->d_atom_struct;
     P.ctl = c->d_ctl; P.status = c->d_ctl + 4;
-    mg_prep_kernel<<<(n_struct + MG_PREP_BLOCK - 1) / MG_PREP_BLOCK, MG_PREP_BLOCK, 0, st>>>(P);
+    mg_prep_kernel<<<(n_struct + MG_PREP_BLOCK / 32 - 1) / (MG_PREP_BLOCK / 32), MG_PREP_BLOCK, 0, st>>>(P);
     MG_CUDA(cudaGetLastError());
     c->launches += 1;
     return MG_OK;
@@ -202,12 +202,12 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
     A.n_struct = n_struct; A.n_atoms = n_atoms; A.r_c = r_c;
     A.row_ptr = o->row_ptr; A.src = o->src; A.dst = o->dst; A.offset = o->offset;
     A.vec = o->vec; A.dist = o->dist; A.capacity = o->capacity; A.n_edges = (long long *)o->n_edges;
-    A.rec = c->d_rec; A.cost_prefix = c->d_cost;
+    A.rec = c->d_rec; A.task_prefix = c->d_cost;
     A.desc = c->d_desc; A.ctl = c->d_ctl; A.status = c->d_ctl + 4;
     A.epoch = c->epoch; A.count_only = count_only;
     int grid = c->sm_count * c->cutoff_occ;
-    if (grid > n_atoms + 1) grid = n_atoms + 1;
-    mg_cutoff_small_kernel<<<grid, MG_BLOCK, sizeof(CutoffSmem), st>>>(A);
+    if (grid > (n_atoms + MG_WARPS) / MG_WARPS) grid = (n_atoms + MG_WARPS) / MG_WARPS;
+    mg_cutoff_warp_kernel<<<grid, MG_BLOCK, (MG_WARPS * sizeof(WarpSmem)), st>>>(A);
     MG_CUDA(cudaGetLastError());
     c->launches += 1;
     return MG_OK;
