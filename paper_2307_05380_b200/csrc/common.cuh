@@ -11,7 +11,7 @@
 #define MG_WARPS (MG_BLOCK / 32)
 #define MG_TASK_BUDGET 6144u        // candidates per cutoff task (one warp, one row group)
 #define MG_TASK_ROWS 32             // rows per task: one lane per row in the scan / look-back
-#define MG_WT 192                   // per-warp translation-table tile (cells)
+#define MG_WT 256                   // per-warp translation-table tile (cells)
 #define MG_WS 768                   // per-warp stash entries (x2: double buffered)
 
 // device status word bits (first error wins when decoded by mg_check)

@@ -106,13 +106,12 @@ __device__ __forceinline__ void mg_warp_stage(WarpSmem &sw, const CutoffArgs &A,
 }
 
 // Translations of cells [cell0, cell0 + ncl): T = tau . L in FP32, .w = packed tau; padded to a
-// multiple of 8 with a far-away sentinel.
+// `pad` entries with a far-away sentinel.
 __device__ __forceinline__ void mg_warp_table(WarpSmem &sw, const int n[3], int ncell, int cell0,
-                                              int ncl, int lane) {
+                                              int ncl, int pad, int lane) {
     const int D1 = 2 * n[1] + 1, D2 = 2 * n[2] + 1;
     const float inv12 = 1.f / (float)(D1 * D2), inv2 = 1.f / (float)D2;
     const bool big = ncell >= (1 << 20);          // float reciprocal is exact below 2^20 only
-    const int pad = (ncl + 7) & ~7;
     __syncwarp();
     for (int c = lane; c < pad; c += 32) {
         float4 T = make_float4(1e18f, 1e18f, 1e18f, 0.f);
@@ -150,15 +149,35 @@ __device__ inline Task mg_warp_find(WarpSmem &sw, const CutoffArgs &A, unsigned 
     if (lane < MG_TASK_ROWS) { sw.rowcnt[buf][lane] = 0; sw.rowhole[buf][lane] = 0; }
     if (ncell > 0) {
         mg_warp_stage(sw, A, k, lane);
-        const int N = k.natoms, NP = k.nr * N, npb = (NP + 31) >> 5;
+        const int N = k.natoms, NP = k.nr * N;
         const float inv_N = 1.f / (float)N;
         const int center = (n[0] * (2 * n[1] + 1) + n[1]) * (2 * n[2] + 1) + n[2];   // tau = 0
         unsigned *stash = sw.stash[buf];
+        // lanes = P pair slots x C cell slots (P C = 32), chosen for the best lane utilisation:
+        // few pairs (small N) -> more lanes along the cells.  C <= 8 keeps the table loads within
+        // one shared-memory wavefront; C = 16, 32 cost 2 and 4.
+        int logC = 0;
+        {
+            const int nc0 = min(ncell, MG_WT);
+            float best = -1.f;
+#pragma unroll
+            for (int lc = 0; lc <= 5; ++lc) {
+                const int C = 1 << lc, P = 32 >> lc;
+                const int slots_p = ((NP + P - 1) / P) * P, slots_c = ((nc0 + 4 * C - 1) / (4 * C)) * (4 * C);
+                float u = (float)NP * (float)nc0 / ((float)slots_p * (float)slots_c);
+                if (lc == 5) u *= 0.6f;
+                if (u > best) { best = u; logC = lc; }
+            }
+        }
+        const int C = 1 << logC, P = 32 >> logC;
+        const int ps = lane >> logC, cs = lane & (C - 1);
+        const int npb = (NP + P - 1) / P;
         for (int cell0 = 0; cell0 < ncell; cell0 += MG_WT) {
-            const int ncl = min(MG_WT, ncell - cell0), pad = (ncl + 7) & ~7;
-            mg_warp_table(sw, n, ncell, cell0, ncl, lane);
+            const int ncl = min(MG_WT, ncell - cell0);
+            const int pad = ((ncl + 4 * C - 1) / (4 * C)) * (4 * C);
+            mg_warp_table(sw, n, ncell, cell0, ncl, pad, lane);
             for (int pb = 0; pb < npb; ++pb) {
-                const int q = pb * 32 + lane;
+                const int q = pb * P + ps;
                 const bool valid = q < NP;
                 const int ri = valid ? mg_fdiv(q, inv_N) : 0;
                 const int j = valid ? q - ri * N : 0;
@@ -168,22 +187,22 @@ __device__ inline Task mg_warp_find(WarpSmem &sw, const CutoffArgs &A, unsigned 
                     const float4 pi = sw.p[i], pj = sw.p[j];
                     qx = __fsub_rn(pj.x, pi.x); qy = __fsub_rn(pj.y, pi.y); qz = __fsub_rn(pj.z, pi.z);
                 }
-                for (int g0 = 0; g0 < pad; g0 += 32) {
-                    const float4 *Tg = sw.T + g0;
-                    const int nb8 = min(4, (pad - g0) >> 3);
+                for (int g0 = 0; g0 < pad; g0 += 32 * C) {      // this lane: cells g0 + m C + cs, m < 32
+                    const float4 *Tg = sw.T + g0 + cs;
+                    const int nb4 = min(32, (pad - g0) >> logC) >> 2;
                     unsigned mask = 0u;
-                    for (int b8 = 0; b8 < nb8; ++b8) {
+                    for (int b4 = 0; b4 < nb4; ++b4) {
                         unsigned sub = 0u;
 #pragma unroll
-                        for (int c = 0; c < 8; ++c) {
-                            const float4 T = Tg[8 * b8 + c];
+                        for (int c = 0; c < 4; ++c) {
+                            const float4 T = Tg[(4 * b4 + c) << logC];
                             if (mg_d2(qx, qy, qz, T.x, T.y, T.z) < hi2) sub |= (1u << c);
                         }
-                        mask |= sub << (8 * b8);
+                        mask |= sub << (4 * b4);
                     }
                     if (i == j) {                       // (i,i,0) is not an edge (R3)
-                        const int rel = center - (cell0 + g0);
-                        if (rel >= 0 && rel < 32) mask &= ~(1u << rel);
+                        const int rel = center - (cell0 + g0) - cs;
+                        if (rel >= 0 && (rel & (C - 1)) == 0 && (rel >> logC) < 32) mask &= ~(1u << (rel >> logC));
                     }
                     if (mask) {
                         int rank = atomicAdd(&sw.rowcnt[buf][ri], __popc(mask));
@@ -191,7 +210,7 @@ __device__ inline Task mg_warp_find(WarpSmem &sw, const CutoffArgs &A, unsigned 
                         while (mask) {
                             const int b = __ffs(mask) - 1;
                             mask &= mask - 1;
-                            const float4 T = Tg[b];
+                            const float4 T = Tg[b << logC];
                             unsigned code = ((unsigned)__float_as_int(T.w) << 6) | (unsigned)j;
                             if (mg_d2(qx, qy, qz, T.x, T.y, T.z) >= lo2) {     // inside the rounding window
                                 int t0, t1, t2;
@@ -237,31 +256,37 @@ __device__ inline Task mg_warp_find(WarpSmem &sw, const CutoffArgs &A, unsigned 
     return k;
 }
 
-// Decoupled look-back: exclusive prefix of the task totals before task t (spins on predecessors
-// that have not published yet; they are running, tickets are handed out in order).
-__device__ inline unsigned mg_warp_lookback(const CutoffArgs &A, int t, int lane) {
+// Decoupled look-back, resumable.  Walks back from task idx, adding the totals of predecessors
+// that have published, until it meets one that holds an inclusive prefix (then done = true).  A
+// predecessor that has not published yet stops the walk: blocking = false returns at once with
+// the partial sum kept in (idx, sum) — the caller overlaps the wait with its next find phase —
+// blocking = true spins (the predecessor is running: tickets are handed out in order).
+struct LookBack { int idx; unsigned sum; bool done; };
+
+__device__ inline void mg_warp_lookback(const CutoffArgs &A, LookBack &lb, bool blocking, int lane) {
     const unsigned ep = A.epoch & 0x3FFFFFFFu;
-    unsigned base = 0u;
-    int idx = t - 1;
-    while (idx >= 0) {
-        const int u = idx - lane;
+    while (!lb.done) {
+        if (lb.idx < 0) { lb.done = true; break; }
+        const int u = lb.idx - lane;
         unsigned long long d = mg_desc(MG_FLAG_PFX, ep, 0u);   // before task 0: prefix 0
-        for (;;) {
-            if (u >= 0) d = *(volatile const unsigned long long *)(A.desc + u);
-            const bool ok = ((unsigned)(d >> 32) & 0x3FFFFFFFu) == ep && (d >> 62) != 0ull;
-            if (__all_sync(0xFFFFFFFFu, ok)) break;
-            __nanosleep(100);
-        }
-        const unsigned pfx = __ballot_sync(0xFFFFFFFFu, (d >> 62) == MG_FLAG_PFX);
-        const int stop = pfx ? __ffs(pfx) - 1 : 31;           // nearest predecessor holding a prefix
-        unsigned val = lane <= stop ? (unsigned)d : 0u;
+        if (u >= 0) d = *(volatile const unsigned long long *)(A.desc + u);
+        const bool ok = ((unsigned)(d >> 32) & 0x3FFFFFFFu) == ep && (d >> 62) != 0ull;
+        const unsigned bad = __ballot_sync(0xFFFFFFFFu, !ok);
+        const unsigned pfx = __ballot_sync(0xFFFFFFFFu, ok && (d >> 62) == MG_FLAG_PFX);
+        const int first_bad = bad ? __ffs(bad) - 1 : 32, first_pfx = pfx ? __ffs(pfx) - 1 : 32;
+        // lanes nearer than the first unpublished predecessor count, up to the nearest prefix
+        const int take = first_pfx < first_bad ? first_pfx + 1 : first_bad;
+        unsigned val = lane < take ? (unsigned)d : 0u;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) val += __shfl_xor_sync(0xFFFFFFFFu, val, o);
-        base += val;
-        if (pfx) break;
-        idx -= 32;
+        lb.sum += val;
+        lb.idx -= take;
+        if (first_pfx < first_bad) { lb.done = true; break; }
+        if (first_bad < 32) {
+            if (!blocking) return;
+            __nanosleep(200);
+        }
     }
-    return base;
 }
 
 // Write one edge: vec = rho (x_j + tau - x_i) in FP64 (fused multiply-adds), rounded once.
@@ -294,8 +319,8 @@ __device__ inline void mg_warp_research(WarpSmem &sw, const CutoffArgs &A, const
     mg_warp_stage(sw, A, k, lane);
     int cur = 0;                                          // lane r: edges of row r written so far
     for (int cell0 = 0; cell0 < ncell; cell0 += MG_WT) {
-        const int ncl = min(MG_WT, ncell - cell0), pad = (ncl + 7) & ~7;
-        mg_warp_table(sw, n, ncell, cell0, ncl, lane);
+        const int ncl = min(MG_WT, ncell - cell0), pad = (ncl + 31) & ~31;
+        mg_warp_table(sw, n, ncell, cell0, ncl, pad, lane);
         for (int r = 0; r < k.nr; ++r) {
             if (__shfl_sync(0xFFFFFFFFu, k.cnt, r) <= k.cap) continue;
             const int i = k.i0 + r;
@@ -305,7 +330,7 @@ __device__ inline void mg_warp_research(WarpSmem &sw, const CutoffArgs &A, const
             int done = __shfl_sync(0xFFFFFFFFu, cur, r);
             for (int c0 = 0; c0 < pad; c0 += 32) {
                 const int c = c0 + lane;
-                const float4 T = c < pad ? sw.T[c] : make_float4(1e18f, 1e18f, 1e18f, 0.f);
+                const float4 T = sw.T[c];
                 int t0, t1, t2;
                 mg_unpack_tau((unsigned)__float_as_int(T.w), t0, t1, t2);
                 for (int j = 0; j < N; ++j) {
@@ -328,10 +353,10 @@ __device__ inline void mg_warp_research(WarpSmem &sw, const CutoffArgs &A, const
     }
 }
 
-// Resolve the output offset of task k (look-back), publish its prefix, write row_ptr, expand.
-__device__ inline void mg_warp_finish(WarpSmem &sw, const CutoffArgs &A, const Task &k, int n_tasks, int lane) {
+// Task k's output offset is known: publish its prefix, write row_ptr, expand.
+__device__ inline void mg_warp_finish(WarpSmem &sw, const CutoffArgs &A, const Task &k, unsigned base32,
+                                      int n_tasks, int lane) {
     const unsigned ep = A.epoch & 0x3FFFFFFFu;
-    const unsigned base32 = mg_warp_lookback(A, k.t, lane);
     if (lane == 0) {
         *(volatile unsigned long long *)(A.desc + k.t) = mg_desc(MG_FLAG_PFX, ep, base32 + k.total);
         if ((unsigned long long)base32 + k.total > 0x7FFFFFFFull) atomicOr(A.status, MGS_CAPACITY);
@@ -376,6 +401,7 @@ mg_cutoff_warp_kernel(const CutoffArgs A) {
     const int n_tasks = (int)*(volatile unsigned *)(A.ctl + 6);
     const unsigned ep = A.epoch & 0x3FFFFFFFu;
     Task pend;
+    LookBack plb;
     bool have_pend = false;
     for (;;) {
         unsigned t = 0u;
@@ -383,16 +409,26 @@ mg_cutoff_warp_kernel(const CutoffArgs A) {
         t = __shfl_sync(0xFFFFFFFFu, t, 0);
         const bool have_cur = t < (unsigned)n_tasks;
         Task cur;
+        LookBack clb;
         if (have_cur) {
             cur = mg_warp_find(sw, A, t, have_pend ? 1 - pend.buf : 0, lane);
             // publish the total right away: successors can look back through this task
             if (lane == 0)
                 *(volatile unsigned long long *)(A.desc + t) = mg_desc(t ? MG_FLAG_AGG : MG_FLAG_PFX, ep, cur.total);
+            clb.idx = (int)t - 1; clb.sum = 0u; clb.done = false;
         }
-        if (have_pend) mg_warp_finish(sw, A, pend, n_tasks, lane);
+        if (have_pend) {                                   // its predecessors had a whole find phase
+            mg_warp_lookback(A, plb, true, lane);
+            mg_warp_finish(sw, A, pend, plb.sum, n_tasks, lane);
+            have_pend = false;
+        }
         if (!have_cur) break;
-        pend = cur;
-        have_pend = true;
+        mg_warp_lookback(A, clb, false, lane);
+        if (clb.done) {
+            mg_warp_finish(sw, A, cur, clb.sum, n_tasks, lane);
+        } else {                                           // somebody before us is still searching:
+            pend = cur; plb = clb; have_pend = true;       // keep the stash, go on with the next task
+        }
     }
     // last CTA out resets the ticket for the next launch
     __syncthreads();
