@@ -73,6 +73,36 @@ __device__ inline unsigned mg_cell_spacings(const float *lat9, double *vol, doub
     return 0u;
 }
 
+// Same as mg_cell_spacings but the three 1/|a_b x a_c| come from FP32 rsqrt (relative error
+// < 1e-6; callers inflate): cross products, V and the validity test stay FP64.
+__device__ inline unsigned mg_cell_spacings_fast(const float *lat9, double *vol, double h[3]) {
+    double A[3][3];
+    bool finite = true;
+    for (int r = 0; r < 3; ++r)
+        for (int c = 0; c < 3; ++c) {
+            A[r][c] = (double)lat9[3 * r + c];
+            finite = finite && isfinite(A[r][c]);
+        }
+    if (!finite) return MGS_NONFINITE;
+    double c12[3] = {A[1][1] * A[2][2] - A[1][2] * A[2][1], A[1][2] * A[2][0] - A[1][0] * A[2][2],
+                     A[1][0] * A[2][1] - A[1][1] * A[2][0]};
+    double c20[3] = {A[2][1] * A[0][2] - A[2][2] * A[0][1], A[2][2] * A[0][0] - A[2][0] * A[0][2],
+                     A[2][0] * A[0][1] - A[2][1] * A[0][0]};
+    double c01[3] = {A[0][1] * A[1][2] - A[0][2] * A[1][1], A[0][2] * A[1][0] - A[0][0] * A[1][2],
+                     A[0][0] * A[1][1] - A[0][1] * A[1][0]};
+    const double V = fabs(mg_dot3(A[0], c12));
+    if (!(V > 1e-9) || !isfinite(V)) return MGS_SINGULAR;
+    const float n0 = (float)mg_dot3(c12, c12), n1 = (float)mg_dot3(c20, c20), n2 = (float)mg_dot3(c01, c01);
+    if (!(n0 > 0.f) || !(n1 > 0.f) || !(n2 > 0.f) || !isfinite(n0) || !isfinite(n1) || !isfinite(n2))
+        return MGS_SINGULAR;                       // |a_b x a_c|^2 under- or overflows FP32
+    const float Vf = (float)V;
+    h[0] = (double)(Vf * rsqrtf(n0));
+    h[1] = (double)(Vf * rsqrtf(n1));
+    h[2] = (double)(Vf * rsqrtf(n2));
+    *vol = V;
+    return 0u;
+}
+
 // Exact FP64 evaluation of one image (Def. 3): f = (x_j - x_i) + tau, v = f . L, no FMA
 // contraction, summation left to right (R15).  Returns d^2's square root.
 __device__ __forceinline__ double mg_exact_vec(const float *xi, const float *xj, int t0, int t1,

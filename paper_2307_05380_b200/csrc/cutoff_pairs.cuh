@@ -1,0 +1,475 @@
+// cutoff_pairs.cuh — fused cutoff-graph kernel (K3 distance filter + K4 count -> device-wide scan
+// -> emit + K6 batching): one autonomous WARP per task, no block barriers.
+//
+// A task = up to 32 consecutive source rows of ONE structure (split by mg_cut_prep_kernel).  Warps
+// take tasks in index order through an atomic ticket, so the decoupled look-back scan over the
+// per-task edge totals always makes progress.  Each warp is software-pipelined over two stash
+// buffers: it publishes the edge total of task A, runs the find phase of its next task B and only
+// then resolves A's output offset and emits A — the look-back wait hides behind useful work.
+//
+//  find   lane <-> ordered pair (row i, target j).  For a pair only the integers
+//         tau_a in (-rho_a - u_a, rho_a - u_a), u = x_j - x_i, rho_a = r_c / h_a can be edges
+//         (cut_prep.cuh), i.e. a sub-box of m_0 m_1 m_2 cells that starts at lo(pair).  The lane
+//         folds its own lo into q' = (u + lo) . L and then walks the SAME table of local
+//         translations T_t = t . L, t in [0,m) (broadcast float4 loads from shared memory):
+//         d2 = |q' + T_t|^2 in FP32 (3 FADD, 3 FFMA), hit mask in registers.  A lane that saw a
+//         candidate inside the FP32 rounding window decides its cells again with the exact FP64
+//         predicate, so the edge set equals Def. 3 evaluated in FP64.  A warp
+//         scan of the hit counts gives every pair its place in the stash: the task's edges land
+//         there as 4-byte codes (tau + 128 bytes, j), ordered by (row, j).
+//  emit   lanes over consecutive edges of the task: decode, vec = (p_j - p_i) + tau . L in FP64
+//         rounded once, coalesced stores of src, dst, offset, vec, dist.  A task whose edges did
+//         not fit the stash runs its find phase again and writes straight to global memory.
+#pragma once
+#include "common.cuh"
+#include "cut_prep.cuh"
+
+struct CutoffArgs {
+    const float *pos;
+    const float *lattice;
+    int n_struct, n_atoms;
+    float r_c;
+    int32_t *row_ptr, *src, *dst;
+    int8_t *offset;
+    float *vec, *dist;
+    long long capacity;
+    long long *n_edges;
+    const CutRec *rec;
+    const unsigned *task_struct;
+    unsigned long long *desc;      // [n_tasks] look-back descriptors
+    unsigned *ctl;                 // [0] next task, [1] CTAs done, [6] number of tasks
+    unsigned *status;
+    unsigned epoch;
+    int count_only;
+};
+
+#define MG_TLOC 128                // local translation table tile (cells) = 4 mask words
+
+struct WarpSmem {
+    float4 T[MG_TLOC];             // t . L (xyz), w unused
+    unsigned tcode[MG_TLOC];       // (t0 << 24 | t1 << 16 | t2 << 8)
+    float4 x[MG_SMALL_MAX_ATOMS];  // fractional coordinates
+    double pd[2][MG_SMALL_MAX_ATOMS][3];   // cartesian positions x . L in FP64 (per stash buffer)
+    unsigned stash[2][MG_STASH];
+    int rowoff[2][MG_TASK_ROWS + 1];
+};
+
+struct Task {
+    int t, s, first, natoms, i0, nr, buf;
+    int cnt, off;          // lane r: edges of row r, exclusive offset inside the task
+    unsigned total;
+};
+
+struct LookBack { int idx; unsigned sum; bool done; };
+
+// Decoupled look-back, resumable.  Walks back from task idx, adding the totals of predecessors
+// that have published, until it meets one that holds an inclusive prefix (then done = true).  A
+// predecessor that has not published yet stops the walk: blocking = false returns at once with
+// the partial sum kept in (idx, sum) — the caller overlaps the wait with its next find phase —
+// blocking = true spins (the predecessor is running: tickets are handed out in order).
+__device__ inline void mg_warp_lookback(const CutoffArgs &A, LookBack &lb, bool blocking, int lane) {
+    const unsigned ep = A.epoch & 0x3FFFFFFFu;
+    while (!lb.done) {
+        if (lb.idx < 0) { lb.done = true; break; }
+        const int u = lb.idx - lane;
+        unsigned long long d = mg_desc(MG_FLAG_PFX, ep, 0u);   // before task 0: prefix 0
+        if (u >= 0) d = *(volatile const unsigned long long *)(A.desc + u);
+        const bool ok = ((unsigned)(d >> 32) & 0x3FFFFFFFu) == ep && (d >> 62) != 0ull;
+        const unsigned bad = __ballot_sync(0xFFFFFFFFu, !ok);
+        const unsigned pfx = __ballot_sync(0xFFFFFFFFu, ok && (d >> 62) == MG_FLAG_PFX);
+        const int first_bad = bad ? __ffs(bad) - 1 : 32, first_pfx = pfx ? __ffs(pfx) - 1 : 32;
+        // lanes nearer than the first unpublished predecessor count, up to the nearest prefix
+        const int take = first_pfx < first_bad ? first_pfx + 1 : first_bad;
+        unsigned val = lane < take ? (unsigned)d : 0u;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) val += __shfl_xor_sync(0xFFFFFFFFu, val, o);
+        lb.sum += val;
+        lb.idx -= take;
+        if (first_pfx < first_bad) { lb.done = true; break; }
+        if (first_bad < 32) {
+            if (!blocking) return;
+            __nanosleep(100);
+        }
+    }
+}
+
+// q / n for 0 <= q < 2^20, 1 <= n (exact: (q + 0.5) / n is never within rounding of an integer)
+__device__ __forceinline__ int mg_fdiv(int q, float inv_n) {
+    return __float2int_rz(__fmul_rn((float)q + 0.5f, inv_n));
+}
+
+// Write one edge: vec = (p_j - p_i) + tau . L in FP64, rounded once (R24).
+// b0, b1, b2 = tau + 128.
+__device__ __forceinline__ void mg_emit_edge(const CutoffArgs &A, long long e, int gi, int gj,
+                                             const double *pdi, const double *pdj, const double Ld[9],
+                                             unsigned b0, unsigned b1, unsigned b2) {
+    // (double)(b - 128) without a conversion instruction: 2^52 + b has b in its low mantissa word
+    const double t0 = __hiloint2double(0x43300000, (int)b0) - 4503599627370624.0;
+    const double t1 = __hiloint2double(0x43300000, (int)b1) - 4503599627370624.0;
+    const double t2 = __hiloint2double(0x43300000, (int)b2) - 4503599627370624.0;
+    const double v0 = fma(t2, Ld[6], fma(t1, Ld[3], fma(t0, Ld[0], pdj[0] - pdi[0])));
+    const double v1 = fma(t2, Ld[7], fma(t1, Ld[4], fma(t0, Ld[1], pdj[1] - pdi[1])));
+    const double v2 = fma(t2, Ld[8], fma(t1, Ld[5], fma(t0, Ld[2], pdj[2] - pdi[2])));
+    const float f0 = (float)v0, f1 = (float)v1, f2 = (float)v2;
+    A.src[e] = gi;
+    A.dst[e] = gj;
+    A.offset[3 * e] = (int8_t)(b0 ^ 0x80u); A.offset[3 * e + 1] = (int8_t)(b1 ^ 0x80u);
+    A.offset[3 * e + 2] = (int8_t)(b2 ^ 0x80u);
+    A.vec[3 * e] = f0; A.vec[3 * e + 1] = f1; A.vec[3 * e + 2] = f2;
+    if (A.dist) A.dist[e] = (float)sqrt(fma(v2, v2, fma(v1, v1, v0 * v0)));
+}
+
+// Stage the structure of task k: wrapped fractional coordinates xw = x - floor(x) with the integer
+// part packed in .w (10 bits per axis, biased by 512), FP64 cartesian positions of the
+// coordinates AS GIVEN into pd[k.buf].  Returns false if a coordinate is non-finite or its
+// integer part does not fit (then the structure emits nothing and the status word is set).
+__device__ __forceinline__ bool mg_warp_stage(WarpSmem &sw, const CutoffArgs &A, const Task &k, int lane) {
+    const float *L = A.lattice + 9 * (size_t)k.s;
+    double Ld[9];
+#pragma unroll
+    for (int c = 0; c < 9; ++c) Ld[c] = (double)__ldg(L + c);
+    bool ok = true;
+    __syncwarp();
+    for (int j = lane; j < k.natoms; j += 32) {
+        const float *xp = A.pos + 3 * (size_t)(k.first + j);
+        const float x0 = xp[0], x1 = xp[1], x2 = xp[2];
+        const float g0 = floorf(x0), g1 = floorf(x1), g2 = floorf(x2);
+        ok = ok && fabsf(g0) <= 500.f && fabsf(g1) <= 500.f && fabsf(g2) <= 500.f;   // false for NaN / inf
+        const int kk = ((int)g0 + 512) | (((int)g1 + 512) << 10) | (((int)g2 + 512) << 20);
+        sw.x[j] = make_float4(x0 - g0, x1 - g1, x2 - g2, __int_as_float(ok ? kk : 0));
+        const double d0 = (double)x0, d1 = (double)x1, d2 = (double)x2;
+        double *pd = sw.pd[k.buf][j];
+        pd[0] = fma(d2, Ld[6], fma(d1, Ld[3], d0 * Ld[0]));
+        pd[1] = fma(d2, Ld[7], fma(d1, Ld[4], d0 * Ld[1]));
+        pd[2] = fma(d2, Ld[8], fma(d1, Ld[5], d0 * Ld[2]));
+    }
+    ok = __all_sync(0xFFFFFFFFu, ok);
+    __syncwarp();
+    return ok;
+}
+
+// Local translations of cells [tile0, tile0 + MG_TLOC) of the per-pair sub-box m0 x m1 x m2:
+// T = t . L in FP32, tcode = packed t; the tail is padded with a far-away sentinel.
+__device__ __forceinline__ void mg_warp_table(WarpSmem &sw, const float a[9], const int m[3], int mloc,
+                                              int tile0, int lane) {
+    const int M12 = m[1] * m[2];
+    const float inv12 = 1.f / (float)M12, inv2 = 1.f / (float)m[2];
+    __syncwarp();
+#pragma unroll
+    for (int cc = 0; cc < MG_TLOC; cc += 32) {
+        const int c = cc + lane, cell = tile0 + c;
+        float4 T = make_float4(1e18f, 1e18f, 1e18f, 0.f);
+        unsigned code = 0u;
+        if (cell < mloc) {
+            const bool big = mloc >= (1 << 20);          // float reciprocal is exact below 2^20 only
+            const int t0 = big ? cell / M12 : mg_fdiv(cell, inv12), r = cell - t0 * M12;
+            const int t1 = big ? r / m[2] : mg_fdiv(r, inv2), t2 = r - t1 * m[2];
+            const float f0 = (float)t0, f1 = (float)t1, f2 = (float)t2;
+            T.x = __fmaf_rn(f2, a[6], __fmaf_rn(f1, a[3], __fmul_rn(f0, a[0])));
+            T.y = __fmaf_rn(f2, a[7], __fmaf_rn(f1, a[4], __fmul_rn(f0, a[1])));
+            T.z = __fmaf_rn(f2, a[8], __fmaf_rn(f1, a[5], __fmul_rn(f0, a[2])));
+            code = ((unsigned)t0 << 24) | ((unsigned)t1 << 16) | ((unsigned)t2 << 8);
+        }
+        if (cc == 0 || tile0 + cc < mloc) { sw.T[c] = T; sw.tcode[c] = code; }
+    }
+    __syncwarp();
+}
+
+// Per-task constants of the find phase.
+struct FindCtx {
+    float a[9];            // lattice rows (FP32)
+    const float *lat;      // the same, global
+    float rho[3];
+    int m[3];
+    int mloc;
+    float nr2, win;        // -r_c^2, rounding window of d2
+};
+
+// One block of 32 ordered pairs against the cells [0, ncl) of the current table tile: hit masks in
+// registers (W words = 32 W cells).  Lanes that saw a candidate inside the rounding window decide
+// their window cells with the exact FP64 predicate.
+template <int W>
+__device__ __forceinline__ void mg_pair_masks(const WarpSmem &sw, const CutoffArgs &A, const FindCtx &F,
+                                              float qx, float qy, float qz, int gi, int gj,
+                                              int l0, int l1, int l2, int ncl, unsigned (&mask)[W]) {
+    bool near = false;
+    const float nr2 = F.nr2, win = F.win;
+#pragma unroll
+    for (int w = 0; w < W; ++w) {
+        mask[w] = 0u;
+        const int n4 = min(8, max(0, (ncl - 32 * w + 3) >> 2));      // warp-uniform
+        const float4 *Tp = sw.T + 32 * w;
+        for (int g = 0; g < n4; ++g) {
+            unsigned sub = 0u;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const float4 T = Tp[4 * g + c];
+                const float vx = __fadd_rn(qx, T.x), vy = __fadd_rn(qy, T.y), vz = __fadd_rn(qz, T.z);
+                const float y = __fmaf_rn(vz, vz, __fmaf_rn(vy, vy, __fmaf_rn(vx, vx, nr2)));
+                if (y < win) sub |= 1u << c;
+                near = near || fabsf(y) < win;
+            }
+            mask[w] |= sub << (4 * g);
+        }
+    }
+    if (near) {                                   // rare: decide the window cells in FP64
+        const float *xi = A.pos + 3 * (size_t)gi, *xj = A.pos + 3 * (size_t)gj;
+        for (int c = 0; c < ncl; ++c) {
+            const float4 T = sw.T[c];
+            const float vx = __fadd_rn(qx, T.x), vy = __fadd_rn(qy, T.y), vz = __fadd_rn(qz, T.z);
+            const float y = __fmaf_rn(vz, vz, __fmaf_rn(vy, vy, __fmaf_rn(vx, vx, nr2)));
+            if (fabsf(y) < win) {
+                const unsigned tc = sw.tcode[c];
+                double v[3];
+                const double d = mg_exact_vec(xi, xj, l0 + (int)(tc >> 24), l1 + (int)((tc >> 16) & 0xFFu),
+                                              l2 + (int)((tc >> 8) & 0xFFu), F.lat, v);
+                const unsigned bit = 1u << (c & 31);
+#pragma unroll
+                for (int w = 0; w < W; ++w)
+                    if (w == (c >> 5)) mask[w] = d < (double)A.r_c ? (mask[w] | bit) : (mask[w] & ~bit);
+            }
+        }
+    }
+}
+
+// Find phase of task k (rows k.i0 .. k.i0 + k.nr - 1 of structure k.s).  direct = false: the edge
+// codes go to stash[k.buf] and the row offsets to rowoff[k.buf]; direct = true (the task did not
+// fit the stash; its global offset `base` is known): the same walk writes the edges straight to
+// global memory.  Returns the number of edges of the task.
+template <int W>
+__device__ __forceinline__ unsigned mg_warp_find(WarpSmem &sw, const CutoffArgs &A, const Task &k, const FindCtx &F,
+                                                 bool direct, long long base, int lane) {
+    const int N = k.natoms, NP = k.nr * N;
+    const float inv_N = 1.f / (float)N;
+    unsigned *stash = sw.stash[k.buf];
+    int *rowoff = sw.rowoff[k.buf];
+    double Ld[9];
+    if (direct) {
+#pragma unroll
+        for (int c = 0; c < 9; ++c) Ld[c] = (double)F.a[c];
+    }
+    int run = 0;
+    for (int tile0 = 0; tile0 < F.mloc; tile0 += 32 * W) {
+        const int ncl = min(32 * W, F.mloc - tile0);
+        mg_warp_table(sw, F.a, F.m, F.mloc, tile0, lane);
+        for (int q0 = 0; q0 < NP; q0 += 32) {
+            const int q = q0 + lane;
+            const bool valid = q < NP;
+            const int ri = valid ? mg_fdiv(q, inv_N) : 0;
+            const int j = valid ? q - ri * N : 0;
+            const int i = k.i0 + ri;
+            const float4 xi = sw.x[i], xj = sw.x[j];
+            // u = x_j - x_i (wrapped coordinates), first cell of the pair's sub-box: floor(-rho - u) + 1
+            const float u0 = __fsub_rn(xj.x, xi.x), u1 = __fsub_rn(xj.y, xi.y), u2 = __fsub_rn(xj.z, xi.z);
+            const float e0 = floorf(__fsub_rn(-F.rho[0], u0)) + 1.f, e1 = floorf(__fsub_rn(-F.rho[1], u1)) + 1.f,
+                        e2 = floorf(__fsub_rn(-F.rho[2], u2)) + 1.f;
+            const float f0 = __fadd_rn(u0, e0), f1 = __fadd_rn(u1, e1), f2 = __fadd_rn(u2, e2);
+            float qx = __fmaf_rn(f2, F.a[6], __fmaf_rn(f1, F.a[3], __fmul_rn(f0, F.a[0])));
+            float qy = __fmaf_rn(f2, F.a[7], __fmaf_rn(f1, F.a[4], __fmul_rn(f0, F.a[1])));
+            float qz = __fmaf_rn(f2, F.a[8], __fmaf_rn(f1, F.a[5], __fmul_rn(f0, F.a[2])));
+            // cell offsets relative to the coordinates AS GIVEN: tau = tau_wrapped + k_i - k_j
+            const int ki = __float_as_int(xi.w), kj = __float_as_int(xj.w);
+            const int l0 = (int)e0 + (ki & 1023) - (kj & 1023);
+            const int l1 = (int)e1 + ((ki >> 10) & 1023) - ((kj >> 10) & 1023);
+            const int l2 = (int)e2 + ((ki >> 20) & 1023) - ((kj >> 20) & 1023);
+            bool inrange = l0 >= -127 && l1 >= -127 && l2 >= -127 && l0 + F.m[0] <= 128 && l1 + F.m[1] <= 128 &&
+                           l2 + F.m[2] <= 128;
+            if (valid && !inrange) atomicOr(A.status, MGS_OFFSET);
+            if (!valid || !inrange) { qx = 1e18f; qy = 1e18f; qz = 1e18f; }
+            const unsigned paircode = ((unsigned)(l0 + 128) << 24) | ((unsigned)(l1 + 128) << 16) |
+                                      ((unsigned)(l2 + 128) << 8) | (unsigned)j;
+            unsigned mask[W];
+            mg_pair_masks<W>(sw, A, F, qx, qy, qz, k.first + i, k.first + j, l0, l1, l2, ncl, mask);
+            if (i == j) {                           // (i,i,0) is not an edge (R3)
+                const int cs = (-(int)e0 * F.m[1] - (int)e1) * F.m[2] - (int)e2 - tile0;
+#pragma unroll
+                for (int w = 0; w < W; ++w)
+                    if (cs >= 32 * w && cs < 32 * w + 32) mask[w] &= ~(1u << (cs & 31));
+            }
+            int cnt = 0;
+#pragma unroll
+            for (int w = 0; w < W; ++w) cnt += __popc(mask[w]);
+            int incl = cnt;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+                if (lane >= o) incl += v;
+            }
+            const int tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
+            int pos = run + incl - cnt;
+            if (valid && j == 0 && tile0 == 0 && !direct) rowoff[ri] = pos;
+            if (!direct) {
+#pragma unroll
+                for (int w = 0; w < W; ++w) {
+                    unsigned mk = mask[w];
+                    while (mk) {
+                        const int b = __ffs(mk) - 1;
+                        mk &= mk - 1;
+                        if (pos < MG_STASH) stash[pos] = paircode + sw.tcode[32 * w + b];
+                        ++pos;
+                    }
+                }
+            } else if (!A.count_only) {
+                const double *pdi = sw.pd[k.buf][i], *pdj = sw.pd[k.buf][j];
+#pragma unroll
+                for (int w = 0; w < W; ++w) {
+                    unsigned mk = mask[w];
+                    while (mk) {
+                        const int b = __ffs(mk) - 1;
+                        mk &= mk - 1;
+                        const unsigned code = paircode + sw.tcode[32 * w + b];
+                        if (base + pos < A.capacity)
+                            mg_emit_edge(A, base + pos, k.first + i, k.first + j, pdi, pdj, Ld, code >> 24,
+                                         (code >> 16) & 0xFFu, (code >> 8) & 0xFFu);
+                        ++pos;
+                    }
+                }
+            }
+            run += tot;
+        }
+    }
+    if (!direct) {
+        __syncwarp();
+        if (lane == 0) rowoff[k.nr] = run;
+        __syncwarp();
+    }
+    return (unsigned)run;
+}
+
+// Stage + find for one task; fills k.cnt / k.off / k.total when direct == false.
+__device__ __noinline__ void mg_task_find(WarpSmem &sw, const CutoffArgs &A, Task &kref, bool direct,
+                                          long long base, int lane) {
+    Task k = kref;
+    const CutRec *R = A.rec + k.s;
+    FindCtx F;
+    F.lat = A.lattice + 9 * (size_t)k.s;
+#pragma unroll
+    for (int c = 0; c < 9; ++c) F.a[c] = __ldg(F.lat + c);
+#pragma unroll
+    for (int a = 0; a < 3; ++a) { F.rho[a] = R->rho[a]; F.m[a] = R->m[a]; }
+    F.mloc = R->mloc;
+    F.nr2 = -__fmul_rn(A.r_c, A.r_c);
+    // FP32 error bound of d2 - r_c^2 near the threshold (R23): the components of q', T
+    // and q' + T are below 3 Q, about 13 roundings of 2^-24 relative size reach v (the wrapped
+    // coordinates are below 1, their difference is rounded once), d2 = v . v adds 3 more
+    const float Q = R->qmax, SA = R->amax_sum;
+    F.win = 1.1920929e-7f * (2.f * A.r_c * (13.f * Q + 2.f * SA) + 4.f * A.r_c * A.r_c);
+    unsigned total = 0u;
+    if (F.mloc > 0) {
+        const bool ok = mg_warp_stage(sw, A, k, lane);
+        if (!ok) {
+            if (lane == 0) atomicOr(A.status, MGS_NONFINITE);
+            F.mloc = 0;
+        }
+    }
+    if (F.mloc > 0) {
+        if (F.mloc <= 32) total = mg_warp_find<1>(sw, A, k, F, direct, base, lane);
+        else if (F.mloc <= 64) total = mg_warp_find<2>(sw, A, k, F, direct, base, lane);
+        else total = mg_warp_find<4>(sw, A, k, F, direct, base, lane);
+    } else if (!direct) {
+        if (lane <= k.nr) sw.rowoff[k.buf][lane] = 0;
+        __syncwarp();
+    }
+    if (direct) return;
+    const int *rowoff = sw.rowoff[k.buf];
+    const int o0 = lane <= k.nr ? rowoff[min(lane, k.nr)] : (int)total;
+    const int o1 = lane < k.nr ? rowoff[lane + 1] : (int)total;
+    kref.off = o0;
+    kref.cnt = lane < k.nr ? o1 - o0 : 0;
+    kref.total = total;
+}
+
+// Task k's output offset is known: publish its prefix, write row_ptr, emit.
+__device__ __noinline__ void mg_task_finish(WarpSmem &sw, const CutoffArgs &A, Task &kref, unsigned base32,
+                                            int n_tasks, int lane) {
+    const Task k = kref;
+    const unsigned ep = A.epoch & 0x3FFFFFFFu;
+    if (lane == 0) {
+        *(volatile unsigned long long *)(A.desc + k.t) = mg_desc(MG_FLAG_PFX, ep, base32 + k.total);
+        if ((unsigned long long)base32 + k.total > 0x7FFFFFFFull) atomicOr(A.status, MGS_CAPACITY);
+    }
+    const long long base = base32;
+    if (lane < k.nr) A.row_ptr[k.first + k.i0 + lane] = (int)(base + k.off);
+    if (k.t == n_tasks - 1 && lane == 0) {
+        const long long tot = base + k.total;
+        A.row_ptr[A.n_atoms] = (int)tot;
+        *A.n_edges = tot;
+        if (!A.count_only && tot > A.capacity) atomicOr(A.status, MGS_CAPACITY);
+    }
+    if (A.count_only || k.total == 0u) return;
+    if (k.total > MG_STASH) {                      // did not fit: search again, write directly
+        mg_task_find(sw, A, kref, true, base, lane);
+        return;
+    }
+    const float *Lf = A.lattice + 9 * (size_t)k.s;
+    double Ld[9];
+#pragma unroll
+    for (int c = 0; c < 9; ++c) Ld[c] = (double)__ldg(Lf + c);
+    const unsigned *stash = sw.stash[k.buf];
+    const int *rowoff = sw.rowoff[k.buf];
+    int r = 0;
+    for (int e0 = 0; e0 < (int)k.total; e0 += 32) {
+        const int e = e0 + lane;
+        if (e < (int)k.total) {
+            while (e >= rowoff[r + 1]) ++r;
+            const unsigned code = stash[e];
+            const int j = (int)(code & 0xFFu);
+            if (base + e < A.capacity)
+                mg_emit_edge(A, base + e, k.first + k.i0 + r, k.first + j, sw.pd[k.buf][k.i0 + r], sw.pd[k.buf][j],
+                             Ld, code >> 24, (code >> 16) & 0xFFu, (code >> 8) & 0xFFu);
+        }
+    }
+}
+
+__global__ void __launch_bounds__(MG_BLOCK, 4)
+mg_cutoff_pairs_kernel(const __grid_constant__ CutoffArgs A) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    WarpSmem &sw = reinterpret_cast<WarpSmem *>(smem_raw)[warp];
+    const int n_tasks = (int)*(volatile unsigned *)(A.ctl + 6);
+    const unsigned ep = A.epoch & 0x3FFFFFFFu;
+    Task pend, cur;
+    LookBack plb, clb;
+    bool have_pend = false;
+    plb.idx = 0; plb.sum = 0u; plb.done = true;
+    for (;;) {
+        unsigned t = 0u;
+        if (lane == 0) t = atomicAdd(A.ctl, 1u);
+        t = __shfl_sync(0xFFFFFFFFu, t, 0);
+        const bool have_cur = t < (unsigned)n_tasks;
+        if (have_cur) {
+            cur.t = (int)t;
+            cur.buf = have_pend ? 1 - pend.buf : 0;
+            cur.s = (int)__ldg(A.task_struct + t);
+            const CutRec *R = A.rec + cur.s;
+            cur.first = R->first;
+            cur.natoms = R->natoms;
+            const int rpt = R->rpt;
+            cur.i0 = (int)(t - R->task0) * rpt;
+            cur.nr = min(rpt, cur.natoms - cur.i0);
+            mg_task_find(sw, A, cur, false, 0, lane);
+            // publish the total right away: successors can look back through this task
+            if (lane == 0)
+                *(volatile unsigned long long *)(A.desc + t) = mg_desc(t ? MG_FLAG_AGG : MG_FLAG_PFX, ep, cur.total);
+            clb.idx = (int)t - 1; clb.sum = 0u; clb.done = false;
+        }
+        if (have_pend) {                                   // its predecessors had a whole find phase
+            mg_warp_lookback(A, plb, true, lane);
+            mg_task_finish(sw, A, pend, plb.sum, n_tasks, lane);
+            have_pend = false;
+        }
+        if (!have_cur) break;
+        mg_warp_lookback(A, clb, false, lane);
+        if (clb.done) {
+            mg_task_finish(sw, A, cur, clb.sum, n_tasks, lane);
+        } else {                                           // somebody before us is still searching:
+            pend = cur; plb = clb; have_pend = true;       // keep the stash, go on with the next task
+        }
+    }
+    // last CTA out resets the ticket for the next launch
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(A.ctl + 1, 1u) == gridDim.x - 1) { A.ctl[0] = 0u; A.ctl[1] = 0u; }
+    }
+}

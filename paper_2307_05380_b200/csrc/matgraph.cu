@@ -11,21 +11,27 @@
 
 #include "common.cuh"
 #include "prep.cuh"
-#include "cutoff_warp.cuh"
+#include "cut_prep.cuh"
+#include "cutoff_pairs.cuh"
 #include "knn_small.cuh"
 
 struct mg_ctx {
     int device = 0;
     int sm_count = 0;
     unsigned *d_ctl = nullptr;            // [0..1] cutoff ticket/done, [2..3] knn ticket/done, [4] status,
-                                          // [5] prep blocks done, [6] number of cutoff chunks
+                                          // [5] knn prep blocks done, [6] number of cutoff tasks, [7] cut-prep block ticket
     StructRec *d_rec = nullptr;           // per-structure records (prep.cuh)
     unsigned *d_cost = nullptr;           // [n_struct+1] task prefix
     size_t rec_cap = 0;
     int32_t *d_atom_struct = nullptr;     // [n_atoms]
     size_t atom_cap = 0;
-    unsigned long long *d_desc = nullptr; // look-back descriptors
+    unsigned long long *d_desc = nullptr; // look-back descriptors of the cutoff tasks
     size_t desc_cap = 0;
+    CutRec *d_crec = nullptr;             // per-structure records of the cutoff path (cut_prep.cuh)
+    unsigned long long *d_pdesc = nullptr;// look-back descriptors of mg_cut_prep_kernel's blocks
+    size_t crec_cap = 0;
+    unsigned *d_task_struct = nullptr;    // [n_atoms + 1] cutoff task -> structure
+    size_t task_cap = 0;
     int32_t *d_rowptr_tmp = nullptr;      // for mg_cutoff_count
     size_t rowptr_cap = 0;
     long long *d_count = nullptr;
@@ -48,7 +54,8 @@ struct mg_graph {
     int have_hint = 0;
 };
 
-#define MG_CUDA(call) do { if ((call) != cudaSuccess) { cudaGetLastError(); return MG_ERR_CUDA; } } while (0)
+#include <stdio.h>
+#define MG_CUDA(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { if (getenv("MG_DEBUG")) fprintf(stderr, "[matgraph] %s:%d %s\n", __FILE__, __LINE__, cudaGetErrorString(e_)); cudaGetLastError(); return MG_ERR_CUDA; } } while (0)
 
 static mg_status decode_status(unsigned bits) {
     if (bits & MGS_NONFINITE) return MG_ERR_NONFINITE;
@@ -91,9 +98,9 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
     if (cudaMalloc(&c->d_ctl, 8 * sizeof(unsigned)) != cudaSuccess ||
         cudaMemset(c->d_ctl, 0, 8 * sizeof(unsigned)) != cudaSuccess ||
         cudaMalloc(&c->d_count, sizeof(long long)) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
-    if (cudaFuncSetAttribute(mg_cutoff_warp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    if (cudaFuncSetAttribute(mg_cutoff_pairs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)(MG_WARPS * sizeof(WarpSmem))) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->cutoff_occ, mg_cutoff_warp_kernel, MG_BLOCK, (MG_WARPS * sizeof(WarpSmem)));
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->cutoff_occ, mg_cutoff_pairs_kernel, MG_BLOCK, (MG_WARPS * sizeof(WarpSmem)));
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->knn_occ[0], mg_knn_small_kernel<1>, MG_BLOCK, 0);
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->knn_occ[1], mg_knn_small_kernel<2>, MG_BLOCK, 0);
     if (c->cutoff_occ < 1 || c->knn_occ[0] < 1 || c->knn_occ[1] < 1) { mg_destroy(c); return MG_ERR_CUDA; }
@@ -106,6 +113,9 @@ extern "C" void mg_destroy(mg_ctx *c) {
     cudaSetDevice(c->device);
     cudaFree(c->d_ctl);
     cudaFree(c->d_desc);
+    cudaFree(c->d_crec);
+    cudaFree(c->d_pdesc);
+    cudaFree(c->d_task_struct);
     cudaFree(c->d_rec);
     cudaFree(c->d_cost);
     cudaFree(c->d_atom_struct);
@@ -125,6 +135,23 @@ extern "C" mg_status mg_reserve(mg_ctx *c, int32_t n_struct, int32_t n_atoms) {
         MG_CUDA(cudaMalloc(&c->d_desc, cap * sizeof(unsigned long long)));
         MG_CUDA(cudaMemset(c->d_desc, 0, cap * sizeof(unsigned long long)));
         c->desc_cap = cap;
+    }
+    if ((size_t)n_struct + 1 > c->crec_cap) {
+        const size_t cap = (size_t)n_struct + 1025;
+        cudaFree(c->d_crec); cudaFree(c->d_pdesc);
+        c->d_crec = nullptr; c->d_pdesc = nullptr; c->crec_cap = 0;
+        MG_CUDA(cudaMalloc(&c->d_crec, cap * sizeof(CutRec)));
+        const size_t nb = cap / MG_CP_BLOCK + 2;
+        MG_CUDA(cudaMalloc(&c->d_pdesc, nb * sizeof(unsigned long long)));
+        MG_CUDA(cudaMemset(c->d_pdesc, 0, nb * sizeof(unsigned long long)));
+        c->crec_cap = cap;
+    }
+    if ((size_t)n_atoms + 2 > c->task_cap) {
+        const size_t cap = (size_t)n_atoms + 1026;
+        cudaFree(c->d_task_struct);
+        c->d_task_struct = nullptr; c->task_cap = 0;
+        MG_CUDA(cudaMalloc(&c->d_task_struct, cap * sizeof(unsigned)));
+        c->task_cap = cap;
     }
     if ((size_t)n_struct + 1 > c->rec_cap) {
         const size_t cap = (size_t)n_struct + 1025;
@@ -193,21 +220,30 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
     c->epoch = (c->epoch + 1u) & 0x3FFFFFFFu;
     if (c->epoch == 0u) {   // 2^30 calls: clear stale descriptors before reusing epoch numbers
         MG_CUDA(cudaMemsetAsync(c->d_desc, 0, c->desc_cap * sizeof(unsigned long long), st));
+        MG_CUDA(cudaMemsetAsync(c->d_pdesc, 0, (c->crec_cap / MG_CP_BLOCK + 2) * sizeof(unsigned long long), st));
         c->epoch = 1u;
     }
-    rs = launch_prep(c, pos, lat, sp, n_struct, n_atoms, r_c, st);
-    if (rs != MG_OK) return rs;
+    MG_CUDA(cudaGetLastError());
+    {
+        CutPrepArgs P;
+        P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms; P.r_c = r_c;
+        P.rec = c->d_crec; P.task_struct = c->d_task_struct; P.pdesc = c->d_pdesc;
+        P.ctl = c->d_ctl; P.status = c->d_ctl + 4; P.epoch = c->epoch;
+        mg_cut_prep_kernel<<<(n_struct + MG_CP_BLOCK - 1) / MG_CP_BLOCK, MG_CP_BLOCK, 0, st>>>(P);
+        MG_CUDA(cudaGetLastError());
+        c->launches += 1;
+    }
     CutoffArgs A;
-    A.pos = pos; A.lattice = lat; A.struct_ptr = sp;
+    A.pos = pos; A.lattice = lat;
     A.n_struct = n_struct; A.n_atoms = n_atoms; A.r_c = r_c;
     A.row_ptr = o->row_ptr; A.src = o->src; A.dst = o->dst; A.offset = o->offset;
     A.vec = o->vec; A.dist = o->dist; A.capacity = o->capacity; A.n_edges = (long long *)o->n_edges;
-    A.rec = c->d_rec; A.task_prefix = c->d_cost;
+    A.rec = c->d_crec; A.task_struct = c->d_task_struct;
     A.desc = c->d_desc; A.ctl = c->d_ctl; A.status = c->d_ctl + 4;
     A.epoch = c->epoch; A.count_only = count_only;
     int grid = c->sm_count * c->cutoff_occ;
     if (grid > (n_atoms + MG_WARPS) / MG_WARPS) grid = (n_atoms + MG_WARPS) / MG_WARPS;
-    mg_cutoff_warp_kernel<<<grid, MG_BLOCK, (MG_WARPS * sizeof(WarpSmem)), st>>>(A);
+    mg_cutoff_pairs_kernel<<<grid, MG_BLOCK, (MG_WARPS * sizeof(WarpSmem)), st>>>(A);
     MG_CUDA(cudaGetLastError());
     c->launches += 1;
     return MG_OK;
