@@ -1,11 +1,17 @@
-// cutoff_pairs.cuh — fused cutoff-graph kernel (K3 distance filter + K4 count -> device-wide scan
-// -> emit + K6 batching): one autonomous WARP per task, no block barriers.
+// cutoff_pairs.cuh — cutoff graph (K3 distance filter + K4 count -> device-wide scan -> emit + K6
+// batching) in two launches of autonomous WARPS, one task per warp at a time, no
+// block barriers and no spin waits:
 //
-// A task = up to 32 consecutive source rows of ONE structure (split by mg_cut_prep_kernel).  Warps
-// take tasks in index order through an atomic ticket, so the decoupled look-back scan over the
-// per-task edge totals always makes progress.  Each warp is software-pipelined over two stash
-// buffers: it publishes the edge total of task A, runs the find phase of its next task B and only
-// then resolves A's output offset and emits A — the look-back wait hides behind useful work.
+//   mg_cutoff_count_kernel  find phase of every task -> edges per source row (row offsets inside
+//                           the task go to row_ptr), edge total per task.  The 32nd task of a group
+//                           of 32 to arrive adds the group up; the last CTA out turns the group
+//                           sums into an exclusive scan.  (device-wide scan, no look-back chain)
+//   mg_cutoff_emit_kernel   base of a task = group prefix + totals of the tasks before it in its
+//                           group (one 32-wide load); final row_ptr; find phase again, now with the
+//                           hits compacted into a shared-memory stash in (row, j) order; emit.
+//
+// A task = up to 32 consecutive source rows of ONE structure (split by mg_cut_prep_kernel); tasks
+// are handed out through an atomic ticket in any order.
 //
 //  find   lane <-> ordered pair (row i, target j).  For a pair only the integers
 //         tau_a in (-rho_a - u_a, rho_a - u_a), u = x_j - x_i, rho_a = r_c / h_a can be edges
@@ -15,11 +21,11 @@
 //         d2 = |q' + T_t|^2 in FP32 (3 FADD, 3 FFMA), hit mask in registers.  A lane that saw a
 //         candidate inside the FP32 rounding window decides its cells again with the exact FP64
 //         predicate, so the edge set equals Def. 3 evaluated in FP64.  A warp
-//         scan of the hit counts gives every pair its place in the stash: the task's edges land
-//         there as 4-byte codes (tau + 128 bytes, j), ordered by (row, j).
+//         scan of the hit counts gives every pair its place: the task's edges are ordered by
+//         (row, j), 4-byte codes (tau + 128 bytes, j).
 //  emit   lanes over consecutive edges of the task: decode, vec = (p_j - p_i) + tau . L in FP64
-//         rounded once, coalesced stores of src, dst, offset, vec, dist.  A task whose edges did
-//         not fit the stash runs its find phase again and writes straight to global memory.
+//         rounded once, coalesced stores of src, dst, offset, vec, dist.  A task whose edges do
+//         not fit the stash writes straight from the find phase to global memory.
 #pragma once
 #include "common.cuh"
 #include "cut_prep.cuh"
@@ -36,62 +42,36 @@ struct CutoffArgs {
     long long *n_edges;
     const CutRec *rec;
     const unsigned *task_struct;
-    unsigned long long *desc;      // [n_tasks] look-back descriptors
-    unsigned *ctl;                 // [0] next task, [1] CTAs done, [6] number of tasks
+    unsigned *ttotal;              // [n_tasks] edges per task
+    unsigned *gsum;                // [n_tasks / 32 + 2] edges per group of 32 tasks -> exclusive scan
+    unsigned *gcount;              // [n_tasks / 32 + 2] arrivals per group (self-resetting)
+    unsigned *ctl;                 // [0] count ticket, [1] count CTAs done, [6] number of tasks,
+                                   // [8] emit ticket, [9] emit CTAs done
     unsigned *status;
-    unsigned epoch;
     int count_only;
 };
 
 #define MG_TLOC 128                // local translation table tile (cells) = 4 mask words
+#define MG_MODE_COUNT 0
+#define MG_MODE_STASH 1
+#define MG_MODE_DIRECT 2
 
 struct WarpSmem {
     float4 T[MG_TLOC];             // t . L (xyz), w unused
     unsigned tcode[MG_TLOC];       // (t0 << 24 | t1 << 16 | t2 << 8)
-    float4 x[MG_SMALL_MAX_ATOMS];  // fractional coordinates
-    double pd[2][MG_SMALL_MAX_ATOMS][3];   // cartesian positions x . L in FP64 (per stash buffer)
-    unsigned stash[2][MG_STASH];
-    int rowoff[2][MG_TASK_ROWS + 1];
+    float4 x[MG_SMALL_MAX_ATOMS];  // wrapped fractional coordinates, .w = packed integer parts
+    int rowoff[MG_TASK_ROWS + 1];
+};
+
+struct EmitSmem {
+    WarpSmem w;
+    double pd[MG_SMALL_MAX_ATOMS][3];   // cartesian positions x . L in FP64
+    unsigned stash[MG_STASH];
 };
 
 struct Task {
-    int t, s, first, natoms, i0, nr, buf;
-    int cnt, off;          // lane r: edges of row r, exclusive offset inside the task
-    unsigned total;
+    int t, s, first, natoms, i0, nr;
 };
-
-struct LookBack { int idx; unsigned sum; bool done; };
-
-// Decoupled look-back, resumable.  Walks back from task idx, adding the totals of predecessors
-// that have published, until it meets one that holds an inclusive prefix (then done = true).  A
-// predecessor that has not published yet stops the walk: blocking = false returns at once with
-// the partial sum kept in (idx, sum) — the caller overlaps the wait with its next find phase —
-// blocking = true spins (the predecessor is running: tickets are handed out in order).
-__device__ inline void mg_warp_lookback(const CutoffArgs &A, LookBack &lb, bool blocking, int lane) {
-    const unsigned ep = A.epoch & 0x3FFFFFFFu;
-    while (!lb.done) {
-        if (lb.idx < 0) { lb.done = true; break; }
-        const int u = lb.idx - lane;
-        unsigned long long d = mg_desc(MG_FLAG_PFX, ep, 0u);   // before task 0: prefix 0
-        if (u >= 0) d = *(volatile const unsigned long long *)(A.desc + u);
-        const bool ok = ((unsigned)(d >> 32) & 0x3FFFFFFFu) == ep && (d >> 62) != 0ull;
-        const unsigned bad = __ballot_sync(0xFFFFFFFFu, !ok);
-        const unsigned pfx = __ballot_sync(0xFFFFFFFFu, ok && (d >> 62) == MG_FLAG_PFX);
-        const int first_bad = bad ? __ffs(bad) - 1 : 32, first_pfx = pfx ? __ffs(pfx) - 1 : 32;
-        // lanes nearer than the first unpublished predecessor count, up to the nearest prefix
-        const int take = first_pfx < first_bad ? first_pfx + 1 : first_bad;
-        unsigned val = lane < take ? (unsigned)d : 0u;
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) val += __shfl_xor_sync(0xFFFFFFFFu, val, o);
-        lb.sum += val;
-        lb.idx -= take;
-        if (first_pfx < first_bad) { lb.done = true; break; }
-        if (first_bad < 32) {
-            if (!blocking) return;
-            __nanosleep(100);
-        }
-    }
-}
 
 // q / n for 0 <= q < 2^20, 1 <= n (exact: (q + 0.5) / n is never within rounding of an integer)
 __device__ __forceinline__ int mg_fdiv(int q, float inv_n) {
@@ -116,18 +96,16 @@ __device__ __forceinline__ void mg_emit_edge(const CutoffArgs &A, long long e, i
     A.offset[3 * e] = (int8_t)(b0 ^ 0x80u); A.offset[3 * e + 1] = (int8_t)(b1 ^ 0x80u);
     A.offset[3 * e + 2] = (int8_t)(b2 ^ 0x80u);
     A.vec[3 * e] = f0; A.vec[3 * e + 1] = f1; A.vec[3 * e + 2] = f2;
-    if (A.dist) A.dist[e] = (float)sqrt(fma(v2, v2, fma(v1, v1, v0 * v0)));
+    if (A.dist) A.dist[e] = __fsqrt_rn((float)fma(v2, v2, fma(v1, v1, v0 * v0)));
 }
 
 // Stage the structure of task k: wrapped fractional coordinates xw = x - floor(x) with the integer
-// part packed in .w (10 bits per axis, biased by 512), FP64 cartesian positions of the
-// coordinates AS GIVEN into pd[k.buf].  Returns false if a coordinate is non-finite or its
+// part packed in .w (10 bits per axis, biased by 512); with pd != nullptr also the FP64 cartesian
+// positions of the coordinates AS GIVEN.  Returns false if a coordinate is non-finite or its
 // integer part does not fit (then the structure emits nothing and the status word is set).
-__device__ __forceinline__ bool mg_warp_stage(WarpSmem &sw, const CutoffArgs &A, const Task &k, int lane) {
+__device__ __forceinline__ bool mg_warp_stage(WarpSmem &sw, double (*pd)[3], const CutoffArgs &A, const Task &k,
+                                              int lane) {
     const float *L = A.lattice + 9 * (size_t)k.s;
-    double Ld[9];
-#pragma unroll
-    for (int c = 0; c < 9; ++c) Ld[c] = (double)__ldg(L + c);
     bool ok = true;
     __syncwarp();
     for (int j = lane; j < k.natoms; j += 32) {
@@ -137,11 +115,12 @@ __device__ __forceinline__ bool mg_warp_stage(WarpSmem &sw, const CutoffArgs &A,
         ok = ok && fabsf(g0) <= 500.f && fabsf(g1) <= 500.f && fabsf(g2) <= 500.f;   // false for NaN / inf
         const int kk = ((int)g0 + 512) | (((int)g1 + 512) << 10) | (((int)g2 + 512) << 20);
         sw.x[j] = make_float4(x0 - g0, x1 - g1, x2 - g2, __int_as_float(ok ? kk : 0));
-        const double d0 = (double)x0, d1 = (double)x1, d2 = (double)x2;
-        double *pd = sw.pd[k.buf][j];
-        pd[0] = fma(d2, Ld[6], fma(d1, Ld[3], d0 * Ld[0]));
-        pd[1] = fma(d2, Ld[7], fma(d1, Ld[4], d0 * Ld[1]));
-        pd[2] = fma(d2, Ld[8], fma(d1, Ld[5], d0 * Ld[2]));
+        if (pd) {
+            const double d0 = (double)x0, d1 = (double)x1, d2 = (double)x2;
+            pd[j][0] = fma(d2, (double)__ldg(L + 6), fma(d1, (double)__ldg(L + 3), d0 * (double)__ldg(L + 0)));
+            pd[j][1] = fma(d2, (double)__ldg(L + 7), fma(d1, (double)__ldg(L + 4), d0 * (double)__ldg(L + 1)));
+            pd[j][2] = fma(d2, (double)__ldg(L + 8), fma(d1, (double)__ldg(L + 5), d0 * (double)__ldg(L + 2)));
+        }
     }
     ok = __all_sync(0xFFFFFFFFu, ok);
     __syncwarp();
@@ -232,19 +211,19 @@ __device__ __forceinline__ void mg_pair_masks(const WarpSmem &sw, const CutoffAr
     }
 }
 
-// Find phase of task k (rows k.i0 .. k.i0 + k.nr - 1 of structure k.s).  direct = false: the edge
-// codes go to stash[k.buf] and the row offsets to rowoff[k.buf]; direct = true (the task did not
-// fit the stash; its global offset `base` is known): the same walk writes the edges straight to
-// global memory.  Returns the number of edges of the task.
-template <int W>
-__device__ __forceinline__ unsigned mg_warp_find(WarpSmem &sw, const CutoffArgs &A, const Task &k, const FindCtx &F,
-                                                 bool direct, long long base, int lane) {
+// Find phase of task k (rows k.i0 .. k.i0 + k.nr - 1 of structure k.s).  Returns the number of
+// edges of the task.
+//   MG_MODE_COUNT   row offsets inside the task -> sw.rowoff[0 .. nr]
+//   MG_MODE_STASH   edge codes -> stash (positions >= MG_STASH are dropped: the caller checks)
+//   MG_MODE_DIRECT  edges straight to global memory at base + position
+template <int W, int MODE>
+__device__ __forceinline__ unsigned mg_warp_find(WarpSmem &sw, unsigned *stash, const double (*pd)[3],
+                                                 const CutoffArgs &A, const Task &k, const FindCtx &F,
+                                                 long long base, int lane) {
     const int N = k.natoms, NP = k.nr * N;
     const float inv_N = 1.f / (float)N;
-    unsigned *stash = sw.stash[k.buf];
-    int *rowoff = sw.rowoff[k.buf];
     double Ld[9];
-    if (direct) {
+    if (MODE == MG_MODE_DIRECT) {
 #pragma unroll
         for (int c = 0; c < 9; ++c) Ld[c] = (double)F.a[c];
     }
@@ -272,12 +251,10 @@ __device__ __forceinline__ unsigned mg_warp_find(WarpSmem &sw, const CutoffArgs 
             const int l0 = (int)e0 + (ki & 1023) - (kj & 1023);
             const int l1 = (int)e1 + ((ki >> 10) & 1023) - ((kj >> 10) & 1023);
             const int l2 = (int)e2 + ((ki >> 20) & 1023) - ((kj >> 20) & 1023);
-            bool inrange = l0 >= -127 && l1 >= -127 && l2 >= -127 && l0 + F.m[0] <= 128 && l1 + F.m[1] <= 128 &&
-                           l2 + F.m[2] <= 128;
-            if (valid && !inrange) atomicOr(A.status, MGS_OFFSET);
+            const bool inrange = l0 >= -127 && l1 >= -127 && l2 >= -127 && l0 + F.m[0] <= 128 &&
+                                 l1 + F.m[1] <= 128 && l2 + F.m[2] <= 128;
+            if (MODE == MG_MODE_COUNT && valid && !inrange) atomicOr(A.status, MGS_OFFSET);
             if (!valid || !inrange) { qx = 1e18f; qy = 1e18f; qz = 1e18f; }
-            const unsigned paircode = ((unsigned)(l0 + 128) << 24) | ((unsigned)(l1 + 128) << 16) |
-                                      ((unsigned)(l2 + 128) << 8) | (unsigned)j;
             unsigned mask[W];
             mg_pair_masks<W>(sw, A, F, qx, qy, qz, k.first + i, k.first + j, l0, l1, l2, ncl, mask);
             if (i == j) {                           // (i,i,0) is not an edge (R3)
@@ -297,20 +274,11 @@ __device__ __forceinline__ unsigned mg_warp_find(WarpSmem &sw, const CutoffArgs 
             }
             const int tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
             int pos = run + incl - cnt;
-            if (valid && j == 0 && tile0 == 0 && !direct) rowoff[ri] = pos;
-            if (!direct) {
-#pragma unroll
-                for (int w = 0; w < W; ++w) {
-                    unsigned mk = mask[w];
-                    while (mk) {
-                        const int b = __ffs(mk) - 1;
-                        mk &= mk - 1;
-                        if (pos < MG_STASH) stash[pos] = paircode + sw.tcode[32 * w + b];
-                        ++pos;
-                    }
-                }
-            } else if (!A.count_only) {
-                const double *pdi = sw.pd[k.buf][i], *pdj = sw.pd[k.buf][j];
+            if (MODE == MG_MODE_COUNT) {
+                if (valid && j == 0 && tile0 == 0) sw.rowoff[ri] = pos;
+            } else {
+                const unsigned paircode = ((unsigned)(l0 + 128) << 24) | ((unsigned)(l1 + 128) << 16) |
+                                          ((unsigned)(l2 + 128) << 8) | (unsigned)j;
 #pragma unroll
                 for (int w = 0; w < W; ++w) {
                     unsigned mk = mask[w];
@@ -318,9 +286,12 @@ __device__ __forceinline__ unsigned mg_warp_find(WarpSmem &sw, const CutoffArgs 
                         const int b = __ffs(mk) - 1;
                         mk &= mk - 1;
                         const unsigned code = paircode + sw.tcode[32 * w + b];
-                        if (base + pos < A.capacity)
-                            mg_emit_edge(A, base + pos, k.first + i, k.first + j, pdi, pdj, Ld, code >> 24,
+                        if (MODE == MG_MODE_STASH) {
+                            if (pos < MG_STASH) stash[pos] = code;
+                        } else if (base + pos < A.capacity) {
+                            mg_emit_edge(A, base + pos, k.first + i, k.first + j, pd[i], pd[j], Ld, code >> 24,
                                          (code >> 16) & 0xFFu, (code >> 8) & 0xFFu);
+                        }
                         ++pos;
                     }
                 }
@@ -328,20 +299,25 @@ __device__ __forceinline__ unsigned mg_warp_find(WarpSmem &sw, const CutoffArgs 
             run += tot;
         }
     }
-    if (!direct) {
-        __syncwarp();
-        if (lane == 0) rowoff[k.nr] = run;
+    __syncwarp();
+    if (MODE == MG_MODE_COUNT) {
+        if (lane == 0) sw.rowoff[k.nr] = run;
         __syncwarp();
     }
     return (unsigned)run;
 }
 
-// Stage + find for one task; fills k.cnt / k.off / k.total when direct == false.
-__device__ __noinline__ void mg_task_find(WarpSmem &sw, const CutoffArgs &A, Task &kref, bool direct,
-                                          long long base, int lane) {
-    Task k = kref;
+// Task t -> (structure, rows) and the constants of its find phase.  Returns false if the
+// structure emits nothing (invalid lattice: only row_ptr is written for its rows).
+__device__ __forceinline__ bool mg_task_setup(const CutoffArgs &A, unsigned t, Task &k, FindCtx &F) {
+    k.t = (int)t;
+    k.s = (int)__ldg(A.task_struct + t);
     const CutRec *R = A.rec + k.s;
-    FindCtx F;
+    k.first = R->first;
+    k.natoms = R->natoms;
+    const int rpt = R->rpt;
+    k.i0 = (int)(t - R->task0) * rpt;
+    k.nr = min(rpt, k.natoms - k.i0);
     F.lat = A.lattice + 9 * (size_t)k.s;
 #pragma unroll
     for (int c = 0; c < 9; ++c) F.a[c] = __ldg(F.lat + c);
@@ -352,124 +328,156 @@ __device__ __noinline__ void mg_task_find(WarpSmem &sw, const CutoffArgs &A, Tas
     // FP32 error bound of d2 - r_c^2 near the threshold (R23): the components of q', T
     // and q' + T are below 3 Q, about 13 roundings of 2^-24 relative size reach v (the wrapped
     // coordinates are below 1, their difference is rounded once), d2 = v . v adds 3 more
-    const float Q = R->qmax, SA = R->amax_sum;
-    F.win = 1.1920929e-7f * (2.f * A.r_c * (13.f * Q + 2.f * SA) + 4.f * A.r_c * A.r_c);
-    unsigned total = 0u;
-    if (F.mloc > 0) {
-        const bool ok = mg_warp_stage(sw, A, k, lane);
-        if (!ok) {
-            if (lane == 0) atomicOr(A.status, MGS_NONFINITE);
-            F.mloc = 0;
-        }
-    }
-    if (F.mloc > 0) {
-        if (F.mloc <= 32) total = mg_warp_find<1>(sw, A, k, F, direct, base, lane);
-        else if (F.mloc <= 64) total = mg_warp_find<2>(sw, A, k, F, direct, base, lane);
-        else total = mg_warp_find<4>(sw, A, k, F, direct, base, lane);
-    } else if (!direct) {
-        if (lane <= k.nr) sw.rowoff[k.buf][lane] = 0;
-        __syncwarp();
-    }
-    if (direct) return;
-    const int *rowoff = sw.rowoff[k.buf];
-    const int o0 = lane <= k.nr ? rowoff[min(lane, k.nr)] : (int)total;
-    const int o1 = lane < k.nr ? rowoff[lane + 1] : (int)total;
-    kref.off = o0;
-    kref.cnt = lane < k.nr ? o1 - o0 : 0;
-    kref.total = total;
+    F.win = 1.1920929e-7f * (2.f * A.r_c * (13.f * R->qmax + 2.f * R->amax_sum) + 4.f * A.r_c * A.r_c);
+    return F.mloc > 0;
 }
 
-// Task k's output offset is known: publish its prefix, write row_ptr, emit.
-__device__ __noinline__ void mg_task_finish(WarpSmem &sw, const CutoffArgs &A, Task &kref, unsigned base32,
-                                            int n_tasks, int lane) {
-    const Task k = kref;
-    const unsigned ep = A.epoch & 0x3FFFFFFFu;
-    if (lane == 0) {
-        *(volatile unsigned long long *)(A.desc + k.t) = mg_desc(MG_FLAG_PFX, ep, base32 + k.total);
-        if ((unsigned long long)base32 + k.total > 0x7FFFFFFFull) atomicOr(A.status, MGS_CAPACITY);
-    }
-    const long long base = base32;
-    if (lane < k.nr) A.row_ptr[k.first + k.i0 + lane] = (int)(base + k.off);
-    if (k.t == n_tasks - 1 && lane == 0) {
-        const long long tot = base + k.total;
-        A.row_ptr[A.n_atoms] = (int)tot;
-        *A.n_edges = tot;
-        if (!A.count_only && tot > A.capacity) atomicOr(A.status, MGS_CAPACITY);
-    }
-    if (A.count_only || k.total == 0u) return;
-    if (k.total > MG_STASH) {                      // did not fit: search again, write directly
-        mg_task_find(sw, A, kref, true, base, lane);
-        return;
-    }
-    const float *Lf = A.lattice + 9 * (size_t)k.s;
-    double Ld[9];
-#pragma unroll
-    for (int c = 0; c < 9; ++c) Ld[c] = (double)__ldg(Lf + c);
-    const unsigned *stash = sw.stash[k.buf];
-    const int *rowoff = sw.rowoff[k.buf];
-    int r = 0;
-    for (int e0 = 0; e0 < (int)k.total; e0 += 32) {
-        const int e = e0 + lane;
-        if (e < (int)k.total) {
-            while (e >= rowoff[r + 1]) ++r;
-            const unsigned code = stash[e];
-            const int j = (int)(code & 0xFFu);
-            if (base + e < A.capacity)
-                mg_emit_edge(A, base + e, k.first + k.i0 + r, k.first + j, sw.pd[k.buf][k.i0 + r], sw.pd[k.buf][j],
-                             Ld, code >> 24, (code >> 16) & 0xFFu, (code >> 8) & 0xFFu);
-        }
-    }
+template <int MODE>
+__device__ __forceinline__ unsigned mg_find_dispatch(WarpSmem &sw, unsigned *stash, const double (*pd)[3],
+                                                     const CutoffArgs &A, const Task &k, const FindCtx &F,
+                                                     long long base, int lane) {
+    if (F.mloc <= 32) return mg_warp_find<1, MODE>(sw, stash, pd, A, k, F, base, lane);
+    if (F.mloc <= 64) return mg_warp_find<2, MODE>(sw, stash, pd, A, k, F, base, lane);
+    return mg_warp_find<4, MODE>(sw, stash, pd, A, k, F, base, lane);
 }
 
+// ---------------------------------------------------------------------------------------------
+// Launch 1: count.
 __global__ void __launch_bounds__(MG_BLOCK, 4)
-mg_cutoff_pairs_kernel(const __grid_constant__ CutoffArgs A) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
+    __shared__ WarpSmem s_w[MG_WARPS];
+    __shared__ unsigned s_part[MG_BLOCK];
+    __shared__ bool s_last;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    WarpSmem &sw = reinterpret_cast<WarpSmem *>(smem_raw)[warp];
+    WarpSmem &sw = s_w[warp];
     const int n_tasks = (int)*(volatile unsigned *)(A.ctl + 6);
-    const unsigned ep = A.epoch & 0x3FFFFFFFu;
-    Task pend, cur;
-    LookBack plb, clb;
-    bool have_pend = false;
-    plb.idx = 0; plb.sum = 0u; plb.done = true;
+    const int GL = n_tasks > 0 ? (n_tasks - 1) >> 5 : 0;         // groups before the last one are full
     for (;;) {
         unsigned t = 0u;
         if (lane == 0) t = atomicAdd(A.ctl, 1u);
         t = __shfl_sync(0xFFFFFFFFu, t, 0);
-        const bool have_cur = t < (unsigned)n_tasks;
-        if (have_cur) {
-            cur.t = (int)t;
-            cur.buf = have_pend ? 1 - pend.buf : 0;
-            cur.s = (int)__ldg(A.task_struct + t);
-            const CutRec *R = A.rec + cur.s;
-            cur.first = R->first;
-            cur.natoms = R->natoms;
-            const int rpt = R->rpt;
-            cur.i0 = (int)(t - R->task0) * rpt;
-            cur.nr = min(rpt, cur.natoms - cur.i0);
-            mg_task_find(sw, A, cur, false, 0, lane);
-            // publish the total right away: successors can look back through this task
-            if (lane == 0)
-                *(volatile unsigned long long *)(A.desc + t) = mg_desc(t ? MG_FLAG_AGG : MG_FLAG_PFX, ep, cur.total);
-            clb.idx = (int)t - 1; clb.sum = 0u; clb.done = false;
+        if (t >= (unsigned)n_tasks) break;
+        Task k;
+        FindCtx F;
+        unsigned total = 0u;
+        bool live = mg_task_setup(A, t, k, F);
+        if (live && !mg_warp_stage(sw, nullptr, A, k, lane)) {
+            if (lane == 0) atomicOr(A.status, MGS_NONFINITE);
+            live = false;
         }
-        if (have_pend) {                                   // its predecessors had a whole find phase
-            mg_warp_lookback(A, plb, true, lane);
-            mg_task_finish(sw, A, pend, plb.sum, n_tasks, lane);
-            have_pend = false;
+        if (live) total = mg_find_dispatch<MG_MODE_COUNT>(sw, nullptr, nullptr, A, k, F, 0, lane);
+        // row offsets inside the task (the emit launch adds the task's base)
+        if (lane < k.nr) A.row_ptr[k.first + k.i0 + lane] = live ? sw.rowoff[lane] : 0;
+        unsigned old = 0u;
+        if (lane == 0) {
+            A.ttotal[t] = total;
+            if ((int)(t >> 5) < GL) {
+                __threadfence();
+                old = atomicInc(A.gcount + (t >> 5), 31u);   // 0..31, wraps to 0 on the 32nd arrival
+            }
         }
-        if (!have_cur) break;
-        mg_warp_lookback(A, clb, false, lane);
-        if (clb.done) {
-            mg_task_finish(sw, A, cur, clb.sum, n_tasks, lane);
-        } else {                                           // somebody before us is still searching:
-            pend = cur; plb = clb; have_pend = true;       // keep the stash, go on with the next task
+        old = __shfl_sync(0xFFFFFFFFu, old, 0);
+        if (old == 31u) {                                    // this task completes its group
+            __threadfence();
+            unsigned v = __ldcg(A.ttotal + ((t >> 5) << 5) + lane);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+            if (lane == 0) A.gsum[t >> 5] = v;
+        }
+        __syncwarp();
+    }
+    // ---- last CTA out: exclusive scan of the group sums, grand total
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = atomicAdd(A.ctl + 1, 1u) == gridDim.x - 1;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    const int per = (GL + MG_BLOCK - 1) / MG_BLOCK;
+    const int b = threadIdx.x * per, e = min(GL, b + per);
+    unsigned sum = 0u;
+    for (int g = b; g < e; ++g) sum += __ldcg(A.gsum + g);
+    s_part[threadIdx.x] = sum;
+    __syncthreads();
+    unsigned off = 0u;
+    for (int w = 0; w < (int)threadIdx.x; ++w) off += s_part[w];
+    for (int g = b; g < e; ++g) {
+        const unsigned v = __ldcg(A.gsum + g);
+        A.gsum[g] = off;
+        off += v;
+    }
+    if (threadIdx.x == MG_BLOCK - 1) {
+        // off = edges of all full groups; add the last (partial) group
+        unsigned long long tot = off;
+        A.gsum[GL] = off;
+        for (int t = GL << 5; t < n_tasks; ++t) tot += __ldcg(A.ttotal + t);
+        *A.n_edges = (long long)tot;
+        A.row_ptr[A.n_atoms] = (int)tot;
+        if (tot > 0x7FFFFFFFull || (!A.count_only && (long long)tot > A.capacity)) atomicOr(A.status, MGS_CAPACITY);
+        A.ctl[0] = 0u;
+        A.ctl[1] = 0u;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Launch 2: emit.
+__global__ void __launch_bounds__(MG_BLOCK, 4)
+mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    EmitSmem &se = reinterpret_cast<EmitSmem *>(smem_raw)[warp];
+    WarpSmem &sw = se.w;
+    const int n_tasks = (int)*(volatile unsigned *)(A.ctl + 6);
+    for (;;) {
+        unsigned t = 0u;
+        if (lane == 0) t = atomicAdd(A.ctl + 8, 1u);
+        t = __shfl_sync(0xFFFFFFFFu, t, 0);
+        if (t >= (unsigned)n_tasks) break;
+        Task k;
+        FindCtx F;
+        const bool live = mg_task_setup(A, t, k, F);
+        // base = prefix of the group + totals of the tasks before t in its group
+        const int p = (int)(t & 31u);
+        unsigned v = lane < p ? __ldg(A.ttotal + (t - p) + lane) : 0u;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+        const long long base = (long long)__ldg(A.gsum + (t >> 5)) + v;
+        const unsigned total = __ldg(A.ttotal + t);
+        __syncwarp();
+        if (lane < k.nr) {
+            const int r = A.row_ptr[k.first + k.i0 + lane];
+            sw.rowoff[lane] = r;
+            A.row_ptr[k.first + k.i0 + lane] = (int)(base + r);
+        }
+        if (lane == 0) sw.rowoff[k.nr] = (int)total;
+        __syncwarp();
+        if (!live || total == 0u) continue;
+        mg_warp_stage(sw, se.pd, A, k, lane);
+        if (total > MG_STASH) {                    // does not fit: write straight from the find phase
+            mg_find_dispatch<MG_MODE_DIRECT>(sw, nullptr, se.pd, A, k, F, base, lane);
+            continue;
+        }
+        mg_find_dispatch<MG_MODE_STASH>(sw, se.stash, se.pd, A, k, F, base, lane);
+        double Ld[9];
+#pragma unroll
+        for (int c = 0; c < 9; ++c) Ld[c] = (double)F.a[c];
+        int r = 0;
+        for (int e0 = 0; e0 < (int)total; e0 += 32) {
+            const int e = e0 + lane;
+            if (e < (int)total) {
+                while (e >= sw.rowoff[r + 1]) ++r;
+                const unsigned code = se.stash[e];
+                const int j = (int)(code & 0xFFu);
+                if (base + e < A.capacity)
+                    mg_emit_edge(A, base + e, k.first + k.i0 + r, k.first + j, se.pd[k.i0 + r], se.pd[j], Ld,
+                                 code >> 24, (code >> 16) & 0xFFu, (code >> 8) & 0xFFu);
+            }
         }
     }
     // last CTA out resets the ticket for the next launch
     __syncthreads();
     if (threadIdx.x == 0) {
         __threadfence();
-        if (atomicAdd(A.ctl + 1, 1u) == gridDim.x - 1) { A.ctl[0] = 0u; A.ctl[1] = 0u; }
+        if (atomicAdd(A.ctl + 9, 1u) == gridDim.x - 1) { A.ctl[8] = 0u; A.ctl[9] = 0u; }
     }
 }

@@ -19,13 +19,15 @@ struct mg_ctx {
     int device = 0;
     int sm_count = 0;
     unsigned *d_ctl = nullptr;            // [0..1] cutoff ticket/done, [2..3] knn ticket/done, [4] status,
-                                          // [5] knn prep blocks done, [6] number of cutoff tasks, [7] cut-prep block ticket
+                                          // [5] knn prep blocks done, [6] number of cutoff tasks, [7] cut-prep block ticket, [8..9] cutoff emit ticket/done
     StructRec *d_rec = nullptr;           // per-structure records (prep.cuh)
     unsigned *d_cost = nullptr;           // [n_struct+1] task prefix
     size_t rec_cap = 0;
     int32_t *d_atom_struct = nullptr;     // [n_atoms]
     size_t atom_cap = 0;
-    unsigned long long *d_desc = nullptr; // look-back descriptors of the cutoff tasks
+    unsigned *d_ttotal = nullptr;         // [n_atoms + ..] edges per cutoff task
+    unsigned *d_gsum = nullptr;           // edges per group of 32 tasks / their exclusive scan
+    unsigned *d_gcount = nullptr;         // arrivals per group
     size_t desc_cap = 0;
     CutRec *d_crec = nullptr;             // per-structure records of the cutoff path (cut_prep.cuh)
     unsigned long long *d_pdesc = nullptr;// look-back descriptors of mg_cut_prep_kernel's blocks
@@ -36,7 +38,7 @@ struct mg_ctx {
     size_t rowptr_cap = 0;
     long long *d_count = nullptr;
     unsigned epoch = 0;
-    int cutoff_occ = 0, knn_occ[2] = {0, 0};
+    int cutoff_occ = 0, count_occ = 0, knn_occ[2] = {0, 0};
     int64_t launches = 0;
     // device mirrors for the _host entry points
     void *h_dev[9] = {nullptr};
@@ -95,15 +97,16 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess || prop.major < 10) { delete c; return MG_ERR_CUDA; }
     c->sm_count = prop.multiProcessorCount;
-    if (cudaMalloc(&c->d_ctl, 8 * sizeof(unsigned)) != cudaSuccess ||
-        cudaMemset(c->d_ctl, 0, 8 * sizeof(unsigned)) != cudaSuccess ||
+    if (cudaMalloc(&c->d_ctl, 16 * sizeof(unsigned)) != cudaSuccess ||
+        cudaMemset(c->d_ctl, 0, 16 * sizeof(unsigned)) != cudaSuccess ||
         cudaMalloc(&c->d_count, sizeof(long long)) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
-    if (cudaFuncSetAttribute(mg_cutoff_pairs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)(MG_WARPS * sizeof(WarpSmem))) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->cutoff_occ, mg_cutoff_pairs_kernel, MG_BLOCK, (MG_WARPS * sizeof(WarpSmem)));
+    if (cudaFuncSetAttribute(mg_cutoff_emit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)(MG_WARPS * sizeof(EmitSmem))) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->cutoff_occ, mg_cutoff_emit_kernel, MG_BLOCK, (MG_WARPS * sizeof(EmitSmem)));
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->count_occ, mg_cutoff_count_kernel, MG_BLOCK, 0);
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->knn_occ[0], mg_knn_small_kernel<1>, MG_BLOCK, 0);
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->knn_occ[1], mg_knn_small_kernel<2>, MG_BLOCK, 0);
-    if (c->cutoff_occ < 1 || c->knn_occ[0] < 1 || c->knn_occ[1] < 1) { mg_destroy(c); return MG_ERR_CUDA; }
+    if (c->cutoff_occ < 1 || c->count_occ < 1 || c->knn_occ[0] < 1 || c->knn_occ[1] < 1) { mg_destroy(c); return MG_ERR_CUDA; }
     *out = c;
     return MG_OK;
 }
@@ -112,7 +115,9 @@ extern "C" void mg_destroy(mg_ctx *c) {
     if (!c) return;
     cudaSetDevice(c->device);
     cudaFree(c->d_ctl);
-    cudaFree(c->d_desc);
+    cudaFree(c->d_ttotal);
+    cudaFree(c->d_gsum);
+    cudaFree(c->d_gcount);
     cudaFree(c->d_crec);
     cudaFree(c->d_pdesc);
     cudaFree(c->d_task_struct);
@@ -128,12 +133,14 @@ extern "C" void mg_destroy(mg_ctx *c) {
 extern "C" mg_status mg_reserve(mg_ctx *c, int32_t n_struct, int32_t n_atoms) {
     if (!c || n_struct < 0 || n_atoms < 0) return MG_ERR_INVALID_ARG;
     MG_CUDA(cudaSetDevice(c->device));
-    if ((size_t)n_atoms + 2 > c->desc_cap) {            // cutoff chunks <= n_atoms + 1 (prep.cuh)
+    if ((size_t)n_atoms + 2 > c->desc_cap) {            // cutoff tasks <= n_atoms (cut_prep.cuh)
         const size_t cap = (size_t)n_atoms + 1026;
-        cudaFree(c->d_desc);
-        c->d_desc = nullptr; c->desc_cap = 0;
-        MG_CUDA(cudaMalloc(&c->d_desc, cap * sizeof(unsigned long long)));
-        MG_CUDA(cudaMemset(c->d_desc, 0, cap * sizeof(unsigned long long)));
+        cudaFree(c->d_ttotal); cudaFree(c->d_gsum); cudaFree(c->d_gcount);
+        c->d_ttotal = nullptr; c->d_gsum = nullptr; c->d_gcount = nullptr; c->desc_cap = 0;
+        MG_CUDA(cudaMalloc(&c->d_ttotal, cap * sizeof(unsigned)));
+        MG_CUDA(cudaMalloc(&c->d_gsum, (cap / 32 + 2) * sizeof(unsigned)));
+        MG_CUDA(cudaMalloc(&c->d_gcount, (cap / 32 + 2) * sizeof(unsigned)));
+        MG_CUDA(cudaMemset(c->d_gcount, 0, (cap / 32 + 2) * sizeof(unsigned)));
         c->desc_cap = cap;
     }
     if ((size_t)n_struct + 1 > c->crec_cap) {
@@ -219,7 +226,6 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
     }
     c->epoch = (c->epoch + 1u) & 0x3FFFFFFFu;
     if (c->epoch == 0u) {   // 2^30 calls: clear stale descriptors before reusing epoch numbers
-        MG_CUDA(cudaMemsetAsync(c->d_desc, 0, c->desc_cap * sizeof(unsigned long long), st));
         MG_CUDA(cudaMemsetAsync(c->d_pdesc, 0, (c->crec_cap / MG_CP_BLOCK + 2) * sizeof(unsigned long long), st));
         c->epoch = 1u;
     }
@@ -239,13 +245,22 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
     A.row_ptr = o->row_ptr; A.src = o->src; A.dst = o->dst; A.offset = o->offset;
     A.vec = o->vec; A.dist = o->dist; A.capacity = o->capacity; A.n_edges = (long long *)o->n_edges;
     A.rec = c->d_crec; A.task_struct = c->d_task_struct;
-    A.desc = c->d_desc; A.ctl = c->d_ctl; A.status = c->d_ctl + 4;
-    A.epoch = c->epoch; A.count_only = count_only;
-    int grid = c->sm_count * c->cutoff_occ;
-    if (grid > (n_atoms + MG_WARPS) / MG_WARPS) grid = (n_atoms + MG_WARPS) / MG_WARPS;
-    mg_cutoff_pairs_kernel<<<grid, MG_BLOCK, (MG_WARPS * sizeof(WarpSmem)), st>>>(A);
+    A.ttotal = c->d_ttotal; A.gsum = c->d_gsum; A.gcount = c->d_gcount;
+    A.ctl = c->d_ctl; A.status = c->d_ctl + 4;
+    A.count_only = count_only;
+    const int cap_grid = (n_atoms + MG_WARPS) / MG_WARPS;        // tasks <= n_atoms
+    int grid = c->sm_count * c->count_occ;
+    if (grid > cap_grid) grid = cap_grid;
+    mg_cutoff_count_kernel<<<grid, MG_BLOCK, 0, st>>>(A);
     MG_CUDA(cudaGetLastError());
     c->launches += 1;
+    if (!count_only) {
+        grid = c->sm_count * c->cutoff_occ;
+        if (grid > cap_grid) grid = cap_grid;
+        mg_cutoff_emit_kernel<<<grid, MG_BLOCK, MG_WARPS * sizeof(EmitSmem), st>>>(A);
+        MG_CUDA(cudaGetLastError());
+        c->launches += 1;
+    }
     return MG_OK;
 }
 
