@@ -1,5 +1,5 @@
 // cut_prep.cuh — K1 (per-structure search bounds) + K6 (batching) of the cutoff graph: one THREAD
-// per structure, one launch, decoupled look-back scan of the task counts across the blocks.
+// per structure, one launch, no waiting between blocks.
 //
 // For structure s with lattice rows a_0,a_1,a_2 (R5):
 //   * plane spacings h_a = V / |a_b x a_c| (BASELINE.json north_star).  The cross
@@ -8,29 +8,31 @@
 //   * an edge (i, j, tau) has |x_ja - x_ia + tau_a| h_a <= d < r_c (projection on the plane normal,
 //     DESIGN.md R14), so for the ordered pair (i, j) only the integers tau_a in the open interval
 //     (-rho_a - u_a, rho_a - u_a), u_a = x_ja - x_ia, can be edges: at most m_a = floor(2 rho_a) + 1
-//     of them.  The graph kernel evaluates exactly the m_0 m_1 m_2 cells of that per-pair sub-box
+//     of them.  The graph kernels evaluate exactly the m_0 m_1 m_2 cells of that per-pair sub-box
 //     (a subset of the box |tau_a| <= ceil(r_c / h_a) of north_star);
-//   * the rounding window `win` of the FP32 filter (R23);
-//   * the split of the structure's source rows into TASKS of about MG_TASK_COST instruction
-//     units whose expected edges fit the per-warp stash, the exclusive prefix of the task counts
-//     over the batch, and the task -> structure table.
+//   * the constants of the rounding window of the FP32 filter (R23);
+//   * an estimated cost per source row (warp instructions) and its prefix over the batch: the graph
+//     kernels cut the batch's rows into one contiguous, equally expensive range per warp.  The
+//     prefix is two-level: lpre[s] inside a block of MG_CP_BLOCK structures (32 bit) and, written
+//     by the last block to finish, bpre[b] over the blocks (64 bit).
 #pragma once
 #include "common.cuh"
 
 #define MG_CP_BLOCK 128
+#define MG_STASH 1024              // stash entries per warp of the emit kernel (cutoff_pairs.cuh)
 
 struct CutRec {              // 64 bytes
     float rho[3];            // upper bound of r_c / h_a (plus the guard eps)
-    float win;               // |d2_fp32 - r_c^2| < win  -> decide in FP64
-    int m[3];                // per-pair sub-box: m_a cells along axis a
+    int m;                   // per-pair sub-box m_0 | m_1 << 8 | m_2 << 16
     int mloc;                // m_0 m_1 m_2; 0: the structure emits nothing (invalid / empty)
     int first, natoms;
-    int rpt;                 // source rows per task
-    unsigned task0;          // index of the structure's first task
+    int rpt;                 // source rows per emit group (expected edges fit the stash)
+    unsigned rowcost;        // estimated warp instructions per source row (>= 1)
+    unsigned lpre;           // prefix of natoms * rowcost inside the structure's prep block
     unsigned err;            // MGS_* bits
     float amax_sum;          // sum_a max_c |L_ac|
     float qmax;              // Q = sum_a (rho_a + 1) max_c |L_ac|
-    int pad;
+    int pad[3];
 };
 static_assert(sizeof(CutRec) == 64, "CutRec is one 64-byte line");
 
@@ -40,26 +42,18 @@ struct CutPrepArgs {
     int n_struct, n_atoms;
     float r_c;
     CutRec *rec;                   // [n_struct]
-    unsigned *task_struct;         // [n_atoms + 1] task -> structure
-    unsigned long long *pdesc;     // [blocks] look-back descriptors of this kernel
-    unsigned *ctl;                 // [6] number of tasks (out), [7] block ticket
+    unsigned long long *bpre;      // [blocks + 1] block sums -> exclusive prefix; [blocks] = total
+    unsigned *ctl;                 // [7] blocks done
     unsigned *status;
-    unsigned epoch;
 };
-
-#define MG_TASK_COST 24000.f       // instruction units per task (10 per candidate, 50 per edge)
-#define MG_STASH 768               // stash entries per buffer (cutoff_pairs.cuh)
 
 __global__ void __launch_bounds__(MG_CP_BLOCK)
 mg_cut_prep_kernel(const CutPrepArgs A) {
     __shared__ unsigned s_warp[MG_CP_BLOCK / 32];
-    __shared__ unsigned s_block, s_base;
+    __shared__ bool s_last;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) s_block = atomicAdd(A.ctl + 7, 1u);     // blocks take chunks in order
-    __syncthreads();
-    const unsigned blk = s_block;
-    const int s = (int)blk * MG_CP_BLOCK + threadIdx.x;
-    unsigned ntask = 0;
+    const int s = blockIdx.x * MG_CP_BLOCK + threadIdx.x;
+    unsigned cost = 0;
     CutRec r;
     if (s < A.n_struct) {
         r.first = A.struct_ptr[s];
@@ -72,6 +66,7 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
         unsigned err = mg_cell_spacings_fast(lat, &vol, h);
         if (N > MG_SMALL_MAX_ATOMS) err |= MGS_UNSUPPORTED;
         r.mloc = 0;
+        r.m = 0;
         r.amax_sum = 0.f;
         float Q = 0.f;
         int mloc = 1;
@@ -79,38 +74,36 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
         for (int a = 0; a < 3; ++a) {
             const float amax = fmaxf(fabsf(lat[3 * a]), fmaxf(fabsf(lat[3 * a + 1]), fabsf(lat[3 * a + 2])));
             r.amax_sum += amax;
-            // rho = r_c / h rounded up, plus the guard for the FP32 rounding of u and z (the
-            // kernel adds the part that grows with |x|)
+            // rho = r_c / h rounded up, plus the guard for the FP32 rounding of u = x_j - x_i and
+            // of -rho - u (wrapped coordinates: |u| <= 1)
             const float rho = __double2float_ru((double)A.r_c / h[a] * (1.0 + 4e-6)) + 4e-6f;
             r.rho[a] = rho;
             float mf = floorf(2.f * rho + 1e-5f) + 1.f;
             if (!(mf <= 255.f)) { err |= MGS_OFFSET; mf = 1.f; }
-            r.m[a] = (int)mf;
-            mloc *= r.m[a];
+            r.m |= (int)mf << (8 * a);
+            mloc *= (int)mf;
             Q += (rho + 1.f) * amax;
         }
         if (!err && N > 0) r.mloc = mloc;
-        r.qmax = Q;       // Q = sum_a (rho_a + 1) max_c |L_ac| bounds every component of q'; T <= 2Q
-        r.win = 0.f;      // completed per task (depends on max |x|): mg_cut_window()
+        r.qmax = Q;
         r.err = err;
         if (err) atomicOr(A.status, err);
-        int rpt = 1;
+        r.rpt = MG_TASK_ROWS;
+        r.rowcost = 1u;
         if (r.mloc > 0) {
             const float lam = (float)N * 4.18879f * A.r_c * A.r_c * A.r_c / (float)vol;   // edges per row
-            const float rowcost = (float)N * ((float)((mloc + 3) & ~3) * 10.f + 40.f) + lam * 50.f;
-            rpt = (int)(MG_TASK_COST / rowcost);
-            const int fit = (int)((float)MG_STASH / (1.2f * lam + 16.f));
-            rpt = max(1, min(rpt, min(MG_TASK_ROWS, fit)));
-            if (mloc > 128) rpt = 1;                 // several table tiles: one row per task
-        } else {
-            rpt = MG_TASK_ROWS;                       // rows of invalid structures: row_ptr only
+            // warp instructions per row: 2 x (11 per candidate, 45 per pair) + 5 per edge
+            const float c = (float)N * ((float)((mloc + 3) & ~3) * 22.f + 90.f) * (1.f / 32.f) + lam * 5.f + 4.f;
+            r.rowcost = (unsigned)fminf(c, 1048576.f);
+            const int fit = (int)((float)MG_STASH / (1.15f * lam + 12.f));
+            r.rpt = max(1, min(MG_TASK_ROWS, fit));
+            if (mloc > 128) r.rpt = 1;                // several table tiles: one row per group
         }
-        r.rpt = rpt;
-        r.pad = 0;
-        ntask = (unsigned)((N + rpt - 1) / rpt);
+        r.pad[0] = r.pad[1] = r.pad[2] = 0;
+        cost = (unsigned)N * r.rowcost;                // N <= 64, rowcost <= 2^20
     }
-    // ---- block-wide exclusive scan of ntask
-    unsigned incl = ntask;
+    // ---- block-wide exclusive scan of the cost
+    unsigned incl = cost;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
         const unsigned t = __shfl_up_sync(0xFFFFFFFFu, incl, o);
@@ -124,39 +117,31 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
         if (w < warp) woff += s_warp[w];
         btotal += s_warp[w];
     }
-    // ---- decoupled look-back over the blocks before this one (warp 0)
-    const unsigned ep = A.epoch & 0x3FFFFFFFu;
-    if (warp == 0) {
-        if (lane == 0)
-            mg_st_release(A.pdesc + blk, mg_desc(blk ? MG_FLAG_AGG : MG_FLAG_PFX, ep, btotal));
-        unsigned sum = 0;
-        int idx = (int)blk - 1;
-        while (idx >= 0) {
-            const int u = idx - lane;
-            unsigned long long d = mg_desc(MG_FLAG_PFX, ep, 0u);
-            if (u >= 0) d = mg_ld_acquire(A.pdesc + u);
-            const bool ok = ((unsigned)(d >> 32) & 0x3FFFFFFFu) == ep && (d >> 62) != 0ull;
-            const unsigned bad = __ballot_sync(0xFFFFFFFFu, !ok);
-            if (bad) continue;                                      // predecessors are running
-            const unsigned pfx = __ballot_sync(0xFFFFFFFFu, (d >> 62) == MG_FLAG_PFX);
-            const int take = pfx ? __ffs(pfx) : 32;
-            unsigned val = lane < take ? (unsigned)d : 0u;
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) val += __shfl_xor_sync(0xFFFFFFFFu, val, o);
-            sum += val;
-            if (pfx) break;
-            idx -= 32;
-        }
-        if (lane == 0) {
-            s_base = sum;
-            if (blk) mg_st_release(A.pdesc + blk, mg_desc(MG_FLAG_PFX, ep, sum + btotal));
-            if (blk == gridDim.x - 1) { A.ctl[6] = sum + btotal; A.ctl[7] = 0u; }
-        }
-    }
-    __syncthreads();
     if (s < A.n_struct) {
-        r.task0 = s_base + woff + incl - ntask;
+        r.lpre = woff + incl - cost;
         A.rec[s] = r;
-        for (unsigned g = 0; g < ntask; ++g) A.task_struct[r.task0 + g] = (unsigned)s;
     }
+    if (threadIdx.x == 0) A.bpre[blockIdx.x] = btotal;
+    // ---- last block out: exclusive scan of the block sums (serial per thread chunk, 64 bit)
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = atomicAdd(A.ctl + 7, 1u) == gridDim.x - 1;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    __shared__ unsigned long long s_part[MG_CP_BLOCK];
+    const int nb = (int)gridDim.x, per = (nb + MG_CP_BLOCK - 1) / MG_CP_BLOCK;
+    const int b = threadIdx.x * per, e = min(nb, b + per);
+    unsigned long long sum = 0ull;
+    for (int g = b; g < e; ++g) sum += __ldcg(A.bpre + g);
+    s_part[threadIdx.x] = sum;
+    __syncthreads();
+    unsigned long long off = 0ull;
+    for (int w = 0; w < (int)threadIdx.x; ++w) off += s_part[w];
+    for (int g = b; g < e; ++g) {
+        const unsigned long long v = __ldcg(A.bpre + g);
+        A.bpre[g] = off;
+        off += v;
+    }
+    if (threadIdx.x == MG_CP_BLOCK - 1) { A.bpre[nb] = off; A.ctl[7] = 0u; }
 }

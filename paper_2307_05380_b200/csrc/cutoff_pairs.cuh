@@ -1,17 +1,15 @@
 // cutoff_pairs.cuh — cutoff graph (K3 distance filter + K4 count -> device-wide scan -> emit + K6
-// batching) in two launches of autonomous WARPS, one task per warp at a time, no
-// block barriers and no spin waits:
+// batching) in two launches of autonomous WARPS: no block barriers, no spin waits,
+// no tickets.  mg_cut_prep_kernel gives every source row an estimated cost; warp w of the grid owns
+// the contiguous range of rows whose cost prefix falls in [w, w+1) * total / n_warps and walks it
+// structure by structure (positions and the translation table are staged once per structure).
 //
-//   mg_cutoff_count_kernel  find phase of every task -> edges per source row (row offsets inside
-//                           the task go to row_ptr), edge total per task.  The 32nd task of a group
-//                           of 32 to arrive adds the group up; the last CTA out turns the group
-//                           sums into an exclusive scan.  (device-wide scan, no look-back chain)
-//   mg_cutoff_emit_kernel   base of a task = group prefix + totals of the tasks before it in its
-//                           group (one 32-wide load); final row_ptr; find phase again, now with the
-//                           hits compacted into a shared-memory stash in (row, j) order; emit.
-//
-// A task = up to 32 consecutive source rows of ONE structure (split by mg_cut_prep_kernel); tasks
-// are handed out through an atomic ticket in any order.
+//   mg_cutoff_count_kernel  find phase over the warp's rows -> edges per warp; the last CTA out
+//                           turns them into an exclusive scan (the device-wide scan of K4) and
+//                           writes n_edges.
+//   mg_cutoff_emit_kernel   find phase again, group of rows by group of rows, now with the hits
+//                           compacted into a shared-memory stash in (row, j) order; the running
+//                           offset gives row_ptr; emit.
 //
 //  find   lane <-> ordered pair (row i, target j).  For a pair only the integers
 //         tau_a in (-rho_a - u_a, rho_a - u_a), u = x_j - x_i, rho_a = r_c / h_a can be edges
@@ -21,11 +19,11 @@
 //         d2 = |q' + T_t|^2 in FP32 (3 FADD, 3 FFMA), hit mask in registers.  A lane that saw a
 //         candidate inside the FP32 rounding window decides its cells again with the exact FP64
 //         predicate, so the edge set equals Def. 3 evaluated in FP64.  A warp
-//         scan of the hit counts gives every pair its place: the task's edges are ordered by
+//         scan of the hit counts gives every pair its place: the group's edges are ordered by
 //         (row, j), 4-byte codes (tau + 128 bytes, j).
-//  emit   lanes over consecutive edges of the task: decode, vec = (p_j - p_i) + tau . L in FP64
-//         rounded once, coalesced stores of src, dst, offset, vec, dist.  A task whose edges do
-//         not fit the stash writes straight from the find phase to global memory.
+//  emit   lanes over consecutive edges of the group: decode, vec = (p_j - p_i) + tau . L in FP64
+//         rounded once, coalesced stores of src, dst, offset, vec, dist.  A group whose edges do
+//         not fit the stash is searched again, writing straight to global memory.
 #pragma once
 #include "common.cuh"
 #include "cut_prep.cuh"
@@ -41,12 +39,12 @@ struct CutoffArgs {
     long long capacity;
     long long *n_edges;
     const CutRec *rec;
-    const unsigned *task_struct;
-    unsigned *ttotal;              // [n_tasks] edges per task
-    unsigned *gsum;                // [n_tasks / 32 + 2] edges per group of 32 tasks -> exclusive scan
-    unsigned *gcount;              // [n_tasks / 32 + 2] arrivals per group (self-resetting)
-    unsigned *ctl;                 // [0] count ticket, [1] count CTAs done, [6] number of tasks,
-                                   // [8] emit ticket, [9] emit CTAs done
+    const unsigned long long *bpre;   // [n_blocks + 1] cost prefix over the prep blocks, [n_blocks] = total
+    int n_blocks;
+    int n_warps;                   // warps of the grid (same for both launches)
+    unsigned *wtotal;              // [n_warps + 1] edges per warp -> exclusive scan
+    int2 *wstart;                  // [n_warps] first (structure, row) of each warp's range
+    unsigned *ctl;                 // [1] count CTAs done
     unsigned *status;
     int count_only;
 };
@@ -70,7 +68,7 @@ struct EmitSmem {
 };
 
 struct Task {
-    int t, s, first, natoms, i0, nr;
+    int s, first, natoms, i0, nr;      // rows i0 .. i0 + nr - 1 of structure s
 };
 
 // q / n for 0 <= q < 2^20, 1 <= n (exact: (q + 0.5) / n is never within rounding of an integer)
@@ -129,10 +127,10 @@ __device__ __forceinline__ bool mg_warp_stage(WarpSmem &sw, double (*pd)[3], con
 
 // Local translations of cells [tile0, tile0 + MG_TLOC) of the per-pair sub-box m0 x m1 x m2:
 // T = t . L in FP32, tcode = packed t; the tail is padded with a far-away sentinel.
-__device__ __forceinline__ void mg_warp_table(WarpSmem &sw, const float a[9], const int m[3], int mloc,
+__device__ __forceinline__ void mg_warp_table(WarpSmem &sw, const float a[9], int m1, int m2, int mloc,
                                               int tile0, int lane) {
-    const int M12 = m[1] * m[2];
-    const float inv12 = 1.f / (float)M12, inv2 = 1.f / (float)m[2];
+    const int M12 = m1 * m2;
+    const float inv12 = 1.f / (float)M12, inv2 = 1.f / (float)m2;
     __syncwarp();
 #pragma unroll
     for (int cc = 0; cc < MG_TLOC; cc += 32) {
@@ -142,7 +140,7 @@ __device__ __forceinline__ void mg_warp_table(WarpSmem &sw, const float a[9], co
         if (cell < mloc) {
             const bool big = mloc >= (1 << 20);          // float reciprocal is exact below 2^20 only
             const int t0 = big ? cell / M12 : mg_fdiv(cell, inv12), r = cell - t0 * M12;
-            const int t1 = big ? r / m[2] : mg_fdiv(r, inv2), t2 = r - t1 * m[2];
+            const int t1 = big ? r / m2 : mg_fdiv(r, inv2), t2 = r - t1 * m2;
             const float f0 = (float)t0, f1 = (float)t1, f2 = (float)t2;
             T.x = __fmaf_rn(f2, a[6], __fmaf_rn(f1, a[3], __fmul_rn(f0, a[0])));
             T.y = __fmaf_rn(f2, a[7], __fmaf_rn(f1, a[4], __fmul_rn(f0, a[1])));
@@ -159,7 +157,7 @@ struct FindCtx {
     float a[9];            // lattice rows (FP32)
     const float *lat;      // the same, global
     float rho[3];
-    int m[3];
+    int m;                 // m_0 | m_1 << 8 | m_2 << 16
     int mloc;
     float nr2, win;        // -r_c^2, rounding window of d2
 };
@@ -211,17 +209,21 @@ __device__ __forceinline__ void mg_pair_masks(const WarpSmem &sw, const CutoffAr
     }
 }
 
-// Find phase of task k (rows k.i0 .. k.i0 + k.nr - 1 of structure k.s).  Returns the number of
-// edges of the task.
-//   MG_MODE_COUNT   row offsets inside the task -> sw.rowoff[0 .. nr]
-//   MG_MODE_STASH   edge codes -> stash (positions >= MG_STASH are dropped: the caller checks)
-//   MG_MODE_DIRECT  edges straight to global memory at base + position
+// Find phase over rows k.i0 .. k.i0 + k.nr - 1 of structure k.s (staged in sw).  Returns the number
+// of edges.
+//   MG_MODE_COUNT   nothing else
+//   MG_MODE_STASH   edge codes -> stash (positions >= MG_STASH are dropped: the caller checks),
+//                   row offsets inside the group -> sw.rowoff[0 .. nr], row_ptr = goff + offset
+//   MG_MODE_DIRECT  edges straight to global memory at goff + position, row_ptr
+// The tile loop is outside the pair loop only when the table does not fit (mloc > 32 W; then the
+// caller passes one row at a time in the STASH / DIRECT modes, so the (row, j) order holds).
 template <int W, int MODE>
 __device__ __forceinline__ unsigned mg_warp_find(WarpSmem &sw, unsigned *stash, const double (*pd)[3],
                                                  const CutoffArgs &A, const Task &k, const FindCtx &F,
-                                                 long long base, int lane) {
+                                                 long long goff, int lane) {
     const int N = k.natoms, NP = k.nr * N;
     const float inv_N = 1.f / (float)N;
+    const int m0 = F.m & 0xFF, m1 = (F.m >> 8) & 0xFF, m2 = (F.m >> 16) & 0xFF;
     double Ld[9];
     if (MODE == MG_MODE_DIRECT) {
 #pragma unroll
@@ -230,7 +232,7 @@ __device__ __forceinline__ unsigned mg_warp_find(WarpSmem &sw, unsigned *stash, 
     int run = 0;
     for (int tile0 = 0; tile0 < F.mloc; tile0 += 32 * W) {
         const int ncl = min(32 * W, F.mloc - tile0);
-        mg_warp_table(sw, F.a, F.m, F.mloc, tile0, lane);
+        if (F.mloc > 32 * W) mg_warp_table(sw, F.a, m1, m2, F.mloc, tile0, lane);
         for (int q0 = 0; q0 < NP; q0 += 32) {
             const int q = q0 + lane;
             const bool valid = q < NP;
@@ -251,14 +253,14 @@ __device__ __forceinline__ unsigned mg_warp_find(WarpSmem &sw, unsigned *stash, 
             const int l0 = (int)e0 + (ki & 1023) - (kj & 1023);
             const int l1 = (int)e1 + ((ki >> 10) & 1023) - ((kj >> 10) & 1023);
             const int l2 = (int)e2 + ((ki >> 20) & 1023) - ((kj >> 20) & 1023);
-            const bool inrange = l0 >= -127 && l1 >= -127 && l2 >= -127 && l0 + F.m[0] <= 128 &&
-                                 l1 + F.m[1] <= 128 && l2 + F.m[2] <= 128;
+            const bool inrange = l0 >= -127 && l1 >= -127 && l2 >= -127 && l0 + m0 <= 128 &&
+                                 l1 + m1 <= 128 && l2 + m2 <= 128;
             if (MODE == MG_MODE_COUNT && valid && !inrange) atomicOr(A.status, MGS_OFFSET);
             if (!valid || !inrange) { qx = 1e18f; qy = 1e18f; qz = 1e18f; }
             unsigned mask[W];
             mg_pair_masks<W>(sw, A, F, qx, qy, qz, k.first + i, k.first + j, l0, l1, l2, ncl, mask);
             if (i == j) {                           // (i,i,0) is not an edge (R3)
-                const int cs = (-(int)e0 * F.m[1] - (int)e1) * F.m[2] - (int)e2 - tile0;
+                const int cs = (-(int)e0 * m1 - (int)e1) * m2 - (int)e2 - tile0;
 #pragma unroll
                 for (int w = 0; w < W; ++w)
                     if (cs >= 32 * w && cs < 32 * w + 32) mask[w] &= ~(1u << (cs & 31));
@@ -266,17 +268,21 @@ __device__ __forceinline__ unsigned mg_warp_find(WarpSmem &sw, unsigned *stash, 
             int cnt = 0;
 #pragma unroll
             for (int w = 0; w < W; ++w) cnt += __popc(mask[w]);
-            int incl = cnt;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
-                if (lane >= o) incl += v;
-            }
-            const int tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
-            int pos = run + incl - cnt;
             if (MODE == MG_MODE_COUNT) {
-                if (valid && j == 0 && tile0 == 0) sw.rowoff[ri] = pos;
+                run += cnt;                         // per lane; reduced once at the end
             } else {
+                int incl = cnt;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+                    if (lane >= o) incl += v;
+                }
+                const int tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
+                int pos = run + incl - cnt;
+                if (valid && j == 0 && tile0 == 0) {
+                    sw.rowoff[ri] = pos;
+                    A.row_ptr[k.first + i] = (int)(goff + pos);
+                }
                 const unsigned paircode = ((unsigned)(l0 + 128) << 24) | ((unsigned)(l1 + 128) << 16) |
                                           ((unsigned)(l2 + 128) << 8) | (unsigned)j;
 #pragma unroll
@@ -288,57 +294,105 @@ __device__ __forceinline__ unsigned mg_warp_find(WarpSmem &sw, unsigned *stash, 
                         const unsigned code = paircode + sw.tcode[32 * w + b];
                         if (MODE == MG_MODE_STASH) {
                             if (pos < MG_STASH) stash[pos] = code;
-                        } else if (base + pos < A.capacity) {
-                            mg_emit_edge(A, base + pos, k.first + i, k.first + j, pd[i], pd[j], Ld, code >> 24,
+                        } else if (goff + pos < A.capacity) {
+                            mg_emit_edge(A, goff + pos, k.first + i, k.first + j, pd[i], pd[j], Ld, code >> 24,
                                          (code >> 16) & 0xFFu, (code >> 8) & 0xFFu);
                         }
                         ++pos;
                     }
                 }
+                run += tot;
             }
-            run += tot;
         }
     }
-    __syncwarp();
     if (MODE == MG_MODE_COUNT) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) run += __shfl_xor_sync(0xFFFFFFFFu, run, o);
+    } else {
+        __syncwarp();
         if (lane == 0) sw.rowoff[k.nr] = run;
         __syncwarp();
     }
     return (unsigned)run;
 }
 
-// Task t -> (structure, rows) and the constants of its find phase.  Returns false if the
-// structure emits nothing (invalid lattice: only row_ptr is written for its rows).
-__device__ __forceinline__ bool mg_task_setup(const CutoffArgs &A, unsigned t, Task &k, FindCtx &F) {
-    k.t = (int)t;
-    k.s = (int)__ldg(A.task_struct + t);
-    const CutRec *R = A.rec + k.s;
+// Constants of the find phase for structure s; stages the structure (positions, table when it
+// fits).  Returns false if the structure emits nothing (empty, invalid lattice or positions).
+__device__ __forceinline__ bool mg_struct_setup(WarpSmem &sw, double (*pd)[3], const CutoffArgs &A, const CutRec *R,
+                                                int s, Task &k, FindCtx &F, int lane) {
+    k.s = s;
     k.first = R->first;
     k.natoms = R->natoms;
-    const int rpt = R->rpt;
-    k.i0 = (int)(t - R->task0) * rpt;
-    k.nr = min(rpt, k.natoms - k.i0);
-    F.lat = A.lattice + 9 * (size_t)k.s;
+    F.lat = A.lattice + 9 * (size_t)s;
+    F.mloc = R->mloc;
+    if (F.mloc <= 0) return false;
 #pragma unroll
     for (int c = 0; c < 9; ++c) F.a[c] = __ldg(F.lat + c);
 #pragma unroll
-    for (int a = 0; a < 3; ++a) { F.rho[a] = R->rho[a]; F.m[a] = R->m[a]; }
-    F.mloc = R->mloc;
+    for (int a = 0; a < 3; ++a) F.rho[a] = R->rho[a];
+    F.m = R->m;
     F.nr2 = -__fmul_rn(A.r_c, A.r_c);
     // FP32 error bound of d2 - r_c^2 near the threshold (R23): the components of q', T
     // and q' + T are below 3 Q, about 13 roundings of 2^-24 relative size reach v (the wrapped
     // coordinates are below 1, their difference is rounded once), d2 = v . v adds 3 more
     F.win = 1.1920929e-7f * (2.f * A.r_c * (13.f * R->qmax + 2.f * R->amax_sum) + 4.f * A.r_c * A.r_c);
-    return F.mloc > 0;
+    if (!mg_warp_stage(sw, pd, A, k, lane)) {
+        if (lane == 0) atomicOr(A.status, MGS_NONFINITE);
+        F.mloc = 0;
+        return false;
+    }
+    if (F.mloc <= MG_TLOC) mg_warp_table(sw, F.a, (F.m >> 8) & 0xFF, (F.m >> 16) & 0xFF, F.mloc, 0, lane);
+    return true;
 }
 
 template <int MODE>
 __device__ __forceinline__ unsigned mg_find_dispatch(WarpSmem &sw, unsigned *stash, const double (*pd)[3],
                                                      const CutoffArgs &A, const Task &k, const FindCtx &F,
-                                                     long long base, int lane) {
-    if (F.mloc <= 32) return mg_warp_find<1, MODE>(sw, stash, pd, A, k, F, base, lane);
-    if (F.mloc <= 64) return mg_warp_find<2, MODE>(sw, stash, pd, A, k, F, base, lane);
-    return mg_warp_find<4, MODE>(sw, stash, pd, A, k, F, base, lane);
+                                                     long long goff, int lane) {
+    if (F.mloc <= 32) return mg_warp_find<1, MODE>(sw, stash, pd, A, k, F, goff, lane);
+    if (F.mloc <= 64) return mg_warp_find<2, MODE>(sw, stash, pd, A, k, F, goff, lane);
+    return mg_warp_find<4, MODE>(sw, stash, pd, A, k, F, goff, lane);
+}
+
+// First (structure, row) of warp w's range: the first row whose cost prefix is >= c0 = w * chunk.
+// The cost prefix of row r of structure s is bpre[s / MG_CP_BLOCK] + rec[s].lpre + r * rowcost.
+__device__ inline void mg_range_start(const CutoffArgs &A, unsigned long long c0, int &s_out, int &r_out, int lane) {
+    // level 1: last prep block b with bpre[b] <= c0 (32-ary search)
+    int lo = 0, hi = A.n_blocks;                   // answer in [lo, hi)
+    while (hi - lo > 1) {
+        const int step = (hi - lo + 31) / 32;
+        const int idx = lo + (lane + 1) * step;
+        const bool ok = idx < hi && __ldg(A.bpre + idx) <= c0;
+        lo += __popc(__ballot_sync(0xFFFFFFFFu, ok)) * step;
+        hi = min(hi, lo + step);
+    }
+    const int b = lo;
+    const unsigned long long bp = __ldg(A.bpre + b);
+    // level 2: last structure of the block whose prefix is <= c0
+    int cnt = 0;
+#pragma unroll
+    for (int q = 0; q < MG_CP_BLOCK / 32; ++q) {
+        const int s = b * MG_CP_BLOCK + q * 32 + lane;
+        const bool ok = s < A.n_struct && bp + A.rec[s].lpre <= c0;
+        cnt += __popc(__ballot_sync(0xFFFFFFFFu, ok));
+    }
+    int s = b * MG_CP_BLOCK + max(cnt, 1) - 1;
+    const CutRec *R = A.rec + s;
+    const unsigned long long cs = bp + R->lpre;
+    const unsigned rc = R->rowcost;
+    int r = c0 > cs ? (int)((c0 - cs + rc - 1) / rc) : 0;
+    if (r >= R->natoms) { s += 1; r = 0; }         // every later row starts at or after c0
+    s_out = s;
+    r_out = r;
+}
+
+// Cost range of warp w: [c0, c1); the last warp takes everything that is left.
+__device__ __forceinline__ void mg_warp_range(const CutoffArgs &A, int w, unsigned long long &c0,
+                                              unsigned long long &c1) {
+    const unsigned long long total = __ldg(A.bpre + A.n_blocks);
+    const unsigned long long chunk = (total + (unsigned)A.n_warps - 1) / (unsigned)A.n_warps;
+    c0 = (unsigned long long)w * chunk;
+    c1 = w == A.n_warps - 1 ? ~0ull : c0 + chunk;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -346,75 +400,59 @@ __device__ __forceinline__ unsigned mg_find_dispatch(WarpSmem &sw, unsigned *sta
 __global__ void __launch_bounds__(MG_BLOCK, 4)
 mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
     __shared__ WarpSmem s_w[MG_WARPS];
-    __shared__ unsigned s_part[MG_BLOCK];
+    __shared__ unsigned long long s_part[MG_BLOCK];
     __shared__ bool s_last;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     WarpSmem &sw = s_w[warp];
-    const int n_tasks = (int)*(volatile unsigned *)(A.ctl + 6);
-    const int GL = n_tasks > 0 ? (n_tasks - 1) >> 5 : 0;         // groups before the last one are full
-    for (;;) {
-        unsigned t = 0u;
-        if (lane == 0) t = atomicAdd(A.ctl, 1u);
-        t = __shfl_sync(0xFFFFFFFFu, t, 0);
-        if (t >= (unsigned)n_tasks) break;
+    const int w = blockIdx.x * MG_WARPS + warp;
+    unsigned long long c0, c1;
+    mg_warp_range(A, w, c0, c1);
+    int s, r;
+    mg_range_start(A, c0, s, r, lane);
+    if (lane == 0) A.wstart[w] = make_int2(s, r);
+    unsigned total = 0u;
+    for (; s < A.n_struct; ++s, r = 0) {
+        const CutRec *R = A.rec + s;
+        const unsigned long long cs = __ldg(A.bpre + s / MG_CP_BLOCK) + R->lpre;
+        if (cs + (unsigned long long)r * R->rowcost >= c1 && R->natoms > 0) break;
+        if (R->natoms == 0) continue;
+        // rows r .. rb - 1 start before c1
+        const unsigned long long room = (c1 - cs + R->rowcost - 1) / R->rowcost;
+        const int rb = (int)min((unsigned long long)R->natoms, room);
         Task k;
         FindCtx F;
-        unsigned total = 0u;
-        bool live = mg_task_setup(A, t, k, F);
-        if (live && !mg_warp_stage(sw, nullptr, A, k, lane)) {
-            if (lane == 0) atomicOr(A.status, MGS_NONFINITE);
-            live = false;
+        if (mg_struct_setup(sw, nullptr, A, R, s, k, F, lane)) {
+            k.i0 = r;
+            k.nr = rb - r;
+            total += mg_find_dispatch<MG_MODE_COUNT>(sw, nullptr, nullptr, A, k, F, 0, lane);
         }
-        if (live) total = mg_find_dispatch<MG_MODE_COUNT>(sw, nullptr, nullptr, A, k, F, 0, lane);
-        // row offsets inside the task (the emit launch adds the task's base)
-        if (lane < k.nr) A.row_ptr[k.first + k.i0 + lane] = live ? sw.rowoff[lane] : 0;
-        unsigned old = 0u;
-        if (lane == 0) {
-            A.ttotal[t] = total;
-            if ((int)(t >> 5) < GL) {
-                __threadfence();
-                old = atomicInc(A.gcount + (t >> 5), 31u);   // 0..31, wraps to 0 on the 32nd arrival
-            }
-        }
-        old = __shfl_sync(0xFFFFFFFFu, old, 0);
-        if (old == 31u) {                                    // this task completes its group
-            __threadfence();
-            unsigned v = __ldcg(A.ttotal + ((t >> 5) << 5) + lane);
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
-            if (lane == 0) A.gsum[t >> 5] = v;
-        }
-        __syncwarp();
+        if (rb < R->natoms) break;
     }
-    // ---- last CTA out: exclusive scan of the group sums, grand total
+    if (lane == 0) A.wtotal[w] = total;
+    // ---- last CTA out: exclusive scan of the warp totals, grand total
     __threadfence();
     __syncthreads();
     if (threadIdx.x == 0) s_last = atomicAdd(A.ctl + 1, 1u) == gridDim.x - 1;
     __syncthreads();
     if (!s_last) return;
     __threadfence();
-    const int per = (GL + MG_BLOCK - 1) / MG_BLOCK;
-    const int b = threadIdx.x * per, e = min(GL, b + per);
-    unsigned sum = 0u;
-    for (int g = b; g < e; ++g) sum += __ldcg(A.gsum + g);
+    const int nw = A.n_warps, per = (nw + MG_BLOCK - 1) / MG_BLOCK;
+    const int b = threadIdx.x * per, e = min(nw, b + per);
+    unsigned long long sum = 0ull;
+    for (int g = b; g < e; ++g) sum += __ldcg(A.wtotal + g);
     s_part[threadIdx.x] = sum;
     __syncthreads();
-    unsigned off = 0u;
-    for (int w = 0; w < (int)threadIdx.x; ++w) off += s_part[w];
+    unsigned long long off = 0ull;
+    for (int x = 0; x < (int)threadIdx.x; ++x) off += s_part[x];
     for (int g = b; g < e; ++g) {
-        const unsigned v = __ldcg(A.gsum + g);
-        A.gsum[g] = off;
+        const unsigned v = __ldcg(A.wtotal + g);
+        A.wtotal[g] = (unsigned)off;
         off += v;
     }
     if (threadIdx.x == MG_BLOCK - 1) {
-        // off = edges of all full groups; add the last (partial) group
-        unsigned long long tot = off;
-        A.gsum[GL] = off;
-        for (int t = GL << 5; t < n_tasks; ++t) tot += __ldcg(A.ttotal + t);
-        *A.n_edges = (long long)tot;
-        A.row_ptr[A.n_atoms] = (int)tot;
-        if (tot > 0x7FFFFFFFull || (!A.count_only && (long long)tot > A.capacity)) atomicOr(A.status, MGS_CAPACITY);
-        A.ctl[0] = 0u;
+        *A.n_edges = (long long)off;
+        A.row_ptr[A.n_atoms] = (int)off;
+        if (off > 0x7FFFFFFFull || (!A.count_only && (long long)off > A.capacity)) atomicOr(A.status, MGS_CAPACITY);
         A.ctl[1] = 0u;
     }
 }
@@ -427,57 +465,52 @@ mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     EmitSmem &se = reinterpret_cast<EmitSmem *>(smem_raw)[warp];
     WarpSmem &sw = se.w;
-    const int n_tasks = (int)*(volatile unsigned *)(A.ctl + 6);
-    for (;;) {
-        unsigned t = 0u;
-        if (lane == 0) t = atomicAdd(A.ctl + 8, 1u);
-        t = __shfl_sync(0xFFFFFFFFu, t, 0);
-        if (t >= (unsigned)n_tasks) break;
+    const int w = blockIdx.x * MG_WARPS + warp;
+    unsigned long long c0, c1;
+    mg_warp_range(A, w, c0, c1);
+    const int2 st = A.wstart[w];
+    int s = st.x, r = st.y;
+    long long goff = (long long)__ldg(A.wtotal + w);
+    for (; s < A.n_struct; ++s, r = 0) {
+        const CutRec *R = A.rec + s;
+        const unsigned long long cs = __ldg(A.bpre + s / MG_CP_BLOCK) + R->lpre;
+        if (cs + (unsigned long long)r * R->rowcost >= c1 && R->natoms > 0) break;
+        if (R->natoms == 0) continue;
+        const unsigned long long room = (c1 - cs + R->rowcost - 1) / R->rowcost;
+        const int rb = (int)min((unsigned long long)R->natoms, room);
         Task k;
         FindCtx F;
-        const bool live = mg_task_setup(A, t, k, F);
-        // base = prefix of the group + totals of the tasks before t in its group
-        const int p = (int)(t & 31u);
-        unsigned v = lane < p ? __ldg(A.ttotal + (t - p) + lane) : 0u;
+        if (!mg_struct_setup(sw, se.pd, A, R, s, k, F, lane)) {
+            for (int i = r + lane; i < rb; i += 32) A.row_ptr[R->first + i] = (int)goff;   // no edges
+        } else {
+            double Ld[9];
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
-        const long long base = (long long)__ldg(A.gsum + (t >> 5)) + v;
-        const unsigned total = __ldg(A.ttotal + t);
-        __syncwarp();
-        if (lane < k.nr) {
-            const int r = A.row_ptr[k.first + k.i0 + lane];
-            sw.rowoff[lane] = r;
-            A.row_ptr[k.first + k.i0 + lane] = (int)(base + r);
-        }
-        if (lane == 0) sw.rowoff[k.nr] = (int)total;
-        __syncwarp();
-        if (!live || total == 0u) continue;
-        mg_warp_stage(sw, se.pd, A, k, lane);
-        if (total > MG_STASH) {                    // does not fit: write straight from the find phase
-            mg_find_dispatch<MG_MODE_DIRECT>(sw, nullptr, se.pd, A, k, F, base, lane);
-            continue;
-        }
-        mg_find_dispatch<MG_MODE_STASH>(sw, se.stash, se.pd, A, k, F, base, lane);
-        double Ld[9];
-#pragma unroll
-        for (int c = 0; c < 9; ++c) Ld[c] = (double)F.a[c];
-        int r = 0;
-        for (int e0 = 0; e0 < (int)total; e0 += 32) {
-            const int e = e0 + lane;
-            if (e < (int)total) {
-                while (e >= sw.rowoff[r + 1]) ++r;
-                const unsigned code = se.stash[e];
-                const int j = (int)(code & 0xFFu);
-                if (base + e < A.capacity)
-                    mg_emit_edge(A, base + e, k.first + k.i0 + r, k.first + j, se.pd[k.i0 + r], se.pd[j], Ld,
-                                 code >> 24, (code >> 16) & 0xFFu, (code >> 8) & 0xFFu);
+            for (int c = 0; c < 9; ++c) Ld[c] = (double)F.a[c];
+            const int rpt = R->rpt;
+            for (int i0 = r; i0 < rb; i0 += rpt) {
+                k.i0 = i0;
+                k.nr = min(rpt, rb - i0);
+                const unsigned total = mg_find_dispatch<MG_MODE_STASH>(sw, se.stash, se.pd, A, k, F, goff, lane);
+                if (total > MG_STASH) {            // does not fit: search again, write directly
+                    mg_find_dispatch<MG_MODE_DIRECT>(sw, nullptr, se.pd, A, k, F, goff, lane);
+                } else {
+                    int rr = 0;
+                    for (int e0 = 0; e0 < (int)total; e0 += 32) {
+                        const int e = e0 + lane;
+                        if (e < (int)total) {
+                            while (e >= sw.rowoff[rr + 1]) ++rr;
+                            const unsigned code = se.stash[e];
+                            const int j = (int)(code & 0xFFu);
+                            if (goff + e < A.capacity)
+                                mg_emit_edge(A, goff + e, k.first + i0 + rr, k.first + j, se.pd[i0 + rr], se.pd[j], Ld,
+                                             code >> 24, (code >> 16) & 0xFFu, (code >> 8) & 0xFFu);
+                        }
+                    }
+                }
+                goff += total;
+                __syncwarp();
             }
         }
-    }
-    // last CTA out resets the ticket for the next launch
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        __threadfence();
-        if (atomicAdd(A.ctl + 9, 1u) == gridDim.x - 1) { A.ctl[8] = 0u; A.ctl[9] = 0u; }
+        if (rb < R->natoms) break;
     }
 }

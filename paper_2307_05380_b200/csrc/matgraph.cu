@@ -25,15 +25,12 @@ struct mg_ctx {
     size_t rec_cap = 0;
     int32_t *d_atom_struct = nullptr;     // [n_atoms]
     size_t atom_cap = 0;
-    unsigned *d_ttotal = nullptr;         // [n_atoms + ..] edges per cutoff task
-    unsigned *d_gsum = nullptr;           // edges per group of 32 tasks / their exclusive scan
-    unsigned *d_gcount = nullptr;         // arrivals per group
-    size_t desc_cap = 0;
+    unsigned *d_wtotal = nullptr;         // [n_warps + 1] cutoff edges per warp / their exclusive scan
+    int2 *d_wstart = nullptr;             // [n_warps] first (structure, row) of each warp's range
+    int cut_warps = 0;
     CutRec *d_crec = nullptr;             // per-structure records of the cutoff path (cut_prep.cuh)
-    unsigned long long *d_pdesc = nullptr;// look-back descriptors of mg_cut_prep_kernel's blocks
+    unsigned long long *d_bpre = nullptr; // cost prefix over the prep blocks
     size_t crec_cap = 0;
-    unsigned *d_task_struct = nullptr;    // [n_atoms + 1] cutoff task -> structure
-    size_t task_cap = 0;
     int32_t *d_rowptr_tmp = nullptr;      // for mg_cutoff_count
     size_t rowptr_cap = 0;
     long long *d_count = nullptr;
@@ -106,6 +103,12 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->count_occ, mg_cutoff_count_kernel, MG_BLOCK, 0);
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->knn_occ[0], mg_knn_small_kernel<1>, MG_BLOCK, 0);
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->knn_occ[1], mg_knn_small_kernel<2>, MG_BLOCK, 0);
+    {
+        const int occ = c->cutoff_occ < c->count_occ ? c->cutoff_occ : c->count_occ;
+        c->cut_warps = c->sm_count * occ * MG_WARPS;
+        if (occ >= 1 && (cudaMalloc(&c->d_wtotal, (c->cut_warps + 1) * sizeof(unsigned)) != cudaSuccess ||
+                         cudaMalloc(&c->d_wstart, c->cut_warps * sizeof(int2)) != cudaSuccess)) { mg_destroy(c); return MG_ERR_CUDA; }
+    }
     if (c->cutoff_occ < 1 || c->count_occ < 1 || c->knn_occ[0] < 1 || c->knn_occ[1] < 1) { mg_destroy(c); return MG_ERR_CUDA; }
     *out = c;
     return MG_OK;
@@ -115,12 +118,10 @@ extern "C" void mg_destroy(mg_ctx *c) {
     if (!c) return;
     cudaSetDevice(c->device);
     cudaFree(c->d_ctl);
-    cudaFree(c->d_ttotal);
-    cudaFree(c->d_gsum);
-    cudaFree(c->d_gcount);
+    cudaFree(c->d_wtotal);
+    cudaFree(c->d_wstart);
     cudaFree(c->d_crec);
-    cudaFree(c->d_pdesc);
-    cudaFree(c->d_task_struct);
+    cudaFree(c->d_bpre);
     cudaFree(c->d_rec);
     cudaFree(c->d_cost);
     cudaFree(c->d_atom_struct);
@@ -133,32 +134,13 @@ extern "C" void mg_destroy(mg_ctx *c) {
 extern "C" mg_status mg_reserve(mg_ctx *c, int32_t n_struct, int32_t n_atoms) {
     if (!c || n_struct < 0 || n_atoms < 0) return MG_ERR_INVALID_ARG;
     MG_CUDA(cudaSetDevice(c->device));
-    if ((size_t)n_atoms + 2 > c->desc_cap) {            // cutoff tasks <= n_atoms (cut_prep.cuh)
-        const size_t cap = (size_t)n_atoms + 1026;
-        cudaFree(c->d_ttotal); cudaFree(c->d_gsum); cudaFree(c->d_gcount);
-        c->d_ttotal = nullptr; c->d_gsum = nullptr; c->d_gcount = nullptr; c->desc_cap = 0;
-        MG_CUDA(cudaMalloc(&c->d_ttotal, cap * sizeof(unsigned)));
-        MG_CUDA(cudaMalloc(&c->d_gsum, (cap / 32 + 2) * sizeof(unsigned)));
-        MG_CUDA(cudaMalloc(&c->d_gcount, (cap / 32 + 2) * sizeof(unsigned)));
-        MG_CUDA(cudaMemset(c->d_gcount, 0, (cap / 32 + 2) * sizeof(unsigned)));
-        c->desc_cap = cap;
-    }
     if ((size_t)n_struct + 1 > c->crec_cap) {
         const size_t cap = (size_t)n_struct + 1025;
-        cudaFree(c->d_crec); cudaFree(c->d_pdesc);
-        c->d_crec = nullptr; c->d_pdesc = nullptr; c->crec_cap = 0;
+        cudaFree(c->d_crec); cudaFree(c->d_bpre);
+        c->d_crec = nullptr; c->d_bpre = nullptr; c->crec_cap = 0;
         MG_CUDA(cudaMalloc(&c->d_crec, cap * sizeof(CutRec)));
-        const size_t nb = cap / MG_CP_BLOCK + 2;
-        MG_CUDA(cudaMalloc(&c->d_pdesc, nb * sizeof(unsigned long long)));
-        MG_CUDA(cudaMemset(c->d_pdesc, 0, nb * sizeof(unsigned long long)));
+        MG_CUDA(cudaMalloc(&c->d_bpre, (cap / MG_CP_BLOCK + 3) * sizeof(unsigned long long)));
         c->crec_cap = cap;
-    }
-    if ((size_t)n_atoms + 2 > c->task_cap) {
-        const size_t cap = (size_t)n_atoms + 1026;
-        cudaFree(c->d_task_struct);
-        c->d_task_struct = nullptr; c->task_cap = 0;
-        MG_CUDA(cudaMalloc(&c->d_task_struct, cap * sizeof(unsigned)));
-        c->task_cap = cap;
     }
     if ((size_t)n_struct + 1 > c->rec_cap) {
         const size_t cap = (size_t)n_struct + 1025;
@@ -224,18 +206,12 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
         MG_CUDA(cudaMemsetAsync(o->n_edges, 0, sizeof(long long), st));
         return MG_OK;
     }
-    c->epoch = (c->epoch + 1u) & 0x3FFFFFFFu;
-    if (c->epoch == 0u) {   // 2^30 calls: clear stale descriptors before reusing epoch numbers
-        MG_CUDA(cudaMemsetAsync(c->d_pdesc, 0, (c->crec_cap / MG_CP_BLOCK + 2) * sizeof(unsigned long long), st));
-        c->epoch = 1u;
-    }
-    MG_CUDA(cudaGetLastError());
+    const int n_blocks = (n_struct + MG_CP_BLOCK - 1) / MG_CP_BLOCK;
     {
         CutPrepArgs P;
         P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms; P.r_c = r_c;
-        P.rec = c->d_crec; P.task_struct = c->d_task_struct; P.pdesc = c->d_pdesc;
-        P.ctl = c->d_ctl; P.status = c->d_ctl + 4; P.epoch = c->epoch;
-        mg_cut_prep_kernel<<<(n_struct + MG_CP_BLOCK - 1) / MG_CP_BLOCK, MG_CP_BLOCK, 0, st>>>(P);
+        P.rec = c->d_crec; P.bpre = c->d_bpre; P.ctl = c->d_ctl; P.status = c->d_ctl + 4;
+        mg_cut_prep_kernel<<<n_blocks, MG_CP_BLOCK, 0, st>>>(P);
         MG_CUDA(cudaGetLastError());
         c->launches += 1;
     }
@@ -244,19 +220,19 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
     A.n_struct = n_struct; A.n_atoms = n_atoms; A.r_c = r_c;
     A.row_ptr = o->row_ptr; A.src = o->src; A.dst = o->dst; A.offset = o->offset;
     A.vec = o->vec; A.dist = o->dist; A.capacity = o->capacity; A.n_edges = (long long *)o->n_edges;
-    A.rec = c->d_crec; A.task_struct = c->d_task_struct;
-    A.ttotal = c->d_ttotal; A.gsum = c->d_gsum; A.gcount = c->d_gcount;
+    A.rec = c->d_crec; A.bpre = c->d_bpre; A.n_blocks = n_blocks;
+    A.wtotal = c->d_wtotal; A.wstart = c->d_wstart;
     A.ctl = c->d_ctl; A.status = c->d_ctl + 4;
     A.count_only = count_only;
-    const int cap_grid = (n_atoms + MG_WARPS) / MG_WARPS;        // tasks <= n_atoms
-    int grid = c->sm_count * c->count_occ;
+    // one contiguous range of rows per warp; small batches use fewer warps (>= 1 row each)
+    int grid = c->cut_warps / MG_WARPS;
+    const int cap_grid = (n_atoms + MG_WARPS) / MG_WARPS;
     if (grid > cap_grid) grid = cap_grid;
+    A.n_warps = grid * MG_WARPS;
     mg_cutoff_count_kernel<<<grid, MG_BLOCK, 0, st>>>(A);
     MG_CUDA(cudaGetLastError());
     c->launches += 1;
     if (!count_only) {
-        grid = c->sm_count * c->cutoff_occ;
-        if (grid > cap_grid) grid = cap_grid;
         mg_cutoff_emit_kernel<<<grid, MG_BLOCK, MG_WARPS * sizeof(EmitSmem), st>>>(A);
         MG_CUDA(cudaGetLastError());
         c->launches += 1;
