@@ -11,28 +11,29 @@
 //     of them.  The graph kernels evaluate exactly the m_0 m_1 m_2 cells of that per-pair sub-box
 //     (a subset of the box |tau_a| <= ceil(r_c / h_a) of north_star);
 //   * the constants of the rounding window of the FP32 filter (R23);
-//   * an estimated cost per source row (warp instructions) and its prefix over the batch: the graph
-//     kernels cut the batch's rows into one contiguous, equally expensive range per warp.  The
-//     prefix is two-level: lpre[s] inside a block of MG_CP_BLOCK structures (32 bit) and, written
-//     by the last block to finish, bpre[b] over the blocks (64 bit).
+//   * an estimated cost per ordered pair (i, j) (1/16 warp instructions) and its prefix over the
+//     batch: the graph kernels cut the batch's pairs, in (structure, i, j) order, into one
+//     contiguous, equally expensive range per warp.  The prefix is two-level: lpre[s] inside a
+//     block of MG_CP_BLOCK structures and, written by the last block to finish, bpre[b] over the
+//     blocks.
 #pragma once
 #include "common.cuh"
 
 #define MG_CP_BLOCK 128
 #define MG_STASH 1024              // stash entries per warp of the emit kernel (cutoff_pairs.cuh)
+#define MG_STRUCT_COST 900.f        // warp instructions' worth of latency to stage one structure (both launches)
 
 struct CutRec {              // 64 bytes
     float rho[3];            // upper bound of r_c / h_a (plus the guard eps)
     int m;                   // per-pair sub-box m_0 | m_1 << 8 | m_2 << 16
     int mloc;                // m_0 m_1 m_2; 0: the structure emits nothing (invalid / empty)
     int first, natoms;
-    int rpt;                 // source rows per emit group (expected edges fit the stash)
-    unsigned rowcost;        // estimated warp instructions per source row (>= 1)
-    unsigned lpre;           // prefix of natoms * rowcost inside the structure's prep block
+    unsigned paircost;       // estimated cost of one ordered pair, 1/16 warp instructions (>= 1)
     unsigned err;            // MGS_* bits
+    unsigned long long lpre; // prefix of natoms^2 * paircost inside the structure's prep block
     float amax_sum;          // sum_a max_c |L_ac|
     float qmax;              // Q = sum_a (rho_a + 1) max_c |L_ac|
-    int pad[3];
+    int pad[2];
 };
 static_assert(sizeof(CutRec) == 64, "CutRec is one 64-byte line");
 
@@ -49,11 +50,11 @@ struct CutPrepArgs {
 
 __global__ void __launch_bounds__(MG_CP_BLOCK)
 mg_cut_prep_kernel(const CutPrepArgs A) {
-    __shared__ unsigned s_warp[MG_CP_BLOCK / 32];
+    __shared__ unsigned long long s_warp[MG_CP_BLOCK / 32];
     __shared__ bool s_last;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int s = blockIdx.x * MG_CP_BLOCK + threadIdx.x;
-    unsigned cost = 0;
+    unsigned long long cost = 0ull;
     CutRec r;
     if (s < A.n_struct) {
         r.first = A.struct_ptr[s];
@@ -88,30 +89,30 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
         r.qmax = Q;
         r.err = err;
         if (err) atomicOr(A.status, err);
-        r.rpt = MG_TASK_ROWS;
-        r.rowcost = 1u;
+        r.paircost = 1u;
         if (r.mloc > 0) {
             const float lam = (float)N * 4.18879f * A.r_c * A.r_c * A.r_c / (float)vol;   // edges per row
-            // warp instructions per row: 2 x (11 per candidate, 45 per pair) + 5 per edge
-            const float c = (float)N * ((float)((mloc + 3) & ~3) * 22.f + 90.f) * (1.f / 32.f) + lam * 5.f + 4.f;
-            r.rowcost = (unsigned)fminf(c, 1048576.f);
-            const int fit = (int)((float)MG_STASH / (1.15f * lam + 12.f));
-            r.rpt = max(1, min(MG_TASK_ROWS, fit));
-            if (mloc > 128) r.rpt = 1;                // several table tiles: one row per group
+            // warp instructions per pair (count + emit launches): 11 per candidate, ~250 per block
+            // of 32 pairs, 3.3 per edge; the per-structure staging is spread over its pairs
+            // (structures whose table is tiled evaluate their candidates again in the emit launch)
+            const float percell = mloc > 256 ? 60.f : 11.f;
+            const float c = ((float)((mloc + 3) & ~3) * percell + 250.f) * (1.f / 32.f) + 3.3f * lam / (float)N +
+                            MG_STRUCT_COST / (float)(N * N);
+            r.paircost = (unsigned)fminf(16.f * c + 1.f, 16777216.f);
         }
-        r.pad[0] = r.pad[1] = r.pad[2] = 0;
-        cost = (unsigned)N * r.rowcost;                // N <= 64, rowcost <= 2^20
+        r.pad[0] = r.pad[1] = 0;
+        cost = (unsigned long long)(N * N) * r.paircost;      // N <= 64
     }
     // ---- block-wide exclusive scan of the cost
-    unsigned incl = cost;
+    unsigned long long incl = cost;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-        const unsigned t = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+        const unsigned long long t = __shfl_up_sync(0xFFFFFFFFu, incl, o);
         if (lane >= o) incl += t;
     }
     if (lane == 31) s_warp[warp] = incl;
     __syncthreads();
-    unsigned woff = 0, btotal = 0;
+    unsigned long long woff = 0, btotal = 0;
 #pragma unroll
     for (int w = 0; w < MG_CP_BLOCK / 32; ++w) {
         if (w < warp) woff += s_warp[w];

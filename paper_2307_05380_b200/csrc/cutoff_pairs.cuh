@@ -43,22 +43,25 @@ struct CutoffArgs {
     int n_blocks;
     int n_warps;                   // warps of the grid (same for both launches)
     unsigned *wtotal;              // [n_warps + 1] edges per warp -> exclusive scan
-    int2 *wstart;                  // [n_warps] first (structure, row) of each warp's range
+    int2 *wstart;                  // [n_warps] first (structure, pair) of each warp's range
+    unsigned *wmask;               // [n_warps, MG_MASK_WORDS] hit masks kept from count to emit
+    unsigned *wclock;              // [2, n_warps] cycles each warp spent in count / emit (tuning aid)
     unsigned *ctl;                 // [1] count CTAs done
     unsigned *status;
     int count_only;
 };
 
-#define MG_TLOC 128                // local translation table tile (cells) = 4 mask words
+#define MG_TLOC 256                // local translation table tile (cells) = 8 mask words
 #define MG_MODE_COUNT 0
 #define MG_MODE_STASH 1
 #define MG_MODE_DIRECT 2
+
+#define MG_MASK_WORDS 4096         // per-warp mask scratch (32-bit words, multiple of 128)
 
 struct WarpSmem {
     float4 T[MG_TLOC];             // t . L (xyz), w unused
     unsigned tcode[MG_TLOC];       // (t0 << 24 | t1 << 16 | t2 << 8)
     float4 x[MG_SMALL_MAX_ATOMS];  // wrapped fractional coordinates, .w = packed integer parts
-    int rowoff[MG_TASK_ROWS + 1];
 };
 
 struct EmitSmem {
@@ -68,7 +71,7 @@ struct EmitSmem {
 };
 
 struct Task {
-    int s, first, natoms, i0, nr;      // rows i0 .. i0 + nr - 1 of structure s
+    int s, first, natoms;
 };
 
 // q / n for 0 <= q < 2^20, 1 <= n (exact: (q + 0.5) / n is never within rounding of an integer)
@@ -132,8 +135,7 @@ __device__ __forceinline__ void mg_warp_table(WarpSmem &sw, const float a[9], in
     const int M12 = m1 * m2;
     const float inv12 = 1.f / (float)M12, inv2 = 1.f / (float)m2;
     __syncwarp();
-#pragma unroll
-    for (int cc = 0; cc < MG_TLOC; cc += 32) {
+    for (int cc = 0; cc < MG_TLOC && (cc == 0 || tile0 + cc < mloc); cc += 32) {
         const int c = cc + lane, cell = tile0 + c;
         float4 T = make_float4(1e18f, 1e18f, 1e18f, 0.f);
         unsigned code = 0u;
@@ -147,7 +149,8 @@ __device__ __forceinline__ void mg_warp_table(WarpSmem &sw, const float a[9], in
             T.z = __fmaf_rn(f2, a[8], __fmaf_rn(f1, a[5], __fmul_rn(f0, a[2])));
             code = ((unsigned)t0 << 24) | ((unsigned)t1 << 16) | ((unsigned)t2 << 8);
         }
-        if (cc == 0 || tile0 + cc < mloc) { sw.T[c] = T; sw.tcode[c] = code; }
+        sw.T[c] = T;
+        sw.tcode[c] = code;
     }
     __syncwarp();
 }
@@ -209,111 +212,48 @@ __device__ __forceinline__ void mg_pair_masks(const WarpSmem &sw, const CutoffAr
     }
 }
 
-// Find phase over rows k.i0 .. k.i0 + k.nr - 1 of structure k.s (staged in sw).  Returns the number
-// of edges.
-//   MG_MODE_COUNT   nothing else
-//   MG_MODE_STASH   edge codes -> stash (positions >= MG_STASH are dropped: the caller checks),
-//                   row offsets inside the group -> sw.rowoff[0 .. nr], row_ptr = goff + offset
-//   MG_MODE_DIRECT  edges straight to global memory at goff + position, row_ptr
-// The tile loop is outside the pair loop only when the table does not fit (mloc > 32 W; then the
-// caller passes one row at a time in the STASH / DIRECT modes, so the (row, j) order holds).
-template <int W, int MODE>
-__device__ __forceinline__ unsigned mg_warp_find(WarpSmem &sw, unsigned *stash, const double (*pd)[3],
-                                                 const CutoffArgs &A, const Task &k, const FindCtx &F,
-                                                 long long goff, int lane) {
-    const int N = k.natoms, NP = k.nr * N;
-    const float inv_N = 1.f / (float)N;
+
+// One lane's ordered pair (i, j) of the staged structure: q' = (u + lo) . L with u = x_j - x_i
+// (wrapped coordinates) and lo = floor(-rho - u) + 1 the first cell of the pair's sub-box; the cell
+// offsets relative to the coordinates AS GIVEN start at l = lo + k_i - k_j.
+struct PairLane {
+    float qx, qy, qz;
+    int l0, l1, l2;       // first cell (absolute)
+    int self;             // index of the cell tau = 0 in the local table if i == j, else -1
+    bool ok;              // valid lane and offsets inside int8
+};
+
+__device__ __forceinline__ PairLane mg_pair_setup(const WarpSmem &sw, const FindCtx &F, bool valid, int i, int j) {
+    PairLane p;
     const int m0 = F.m & 0xFF, m1 = (F.m >> 8) & 0xFF, m2 = (F.m >> 16) & 0xFF;
-    double Ld[9];
-    if (MODE == MG_MODE_DIRECT) {
+    const float4 xi = sw.x[i], xj = sw.x[j];
+    const float u0 = __fsub_rn(xj.x, xi.x), u1 = __fsub_rn(xj.y, xi.y), u2 = __fsub_rn(xj.z, xi.z);
+    const float e0 = floorf(__fsub_rn(-F.rho[0], u0)) + 1.f, e1 = floorf(__fsub_rn(-F.rho[1], u1)) + 1.f,
+                e2 = floorf(__fsub_rn(-F.rho[2], u2)) + 1.f;
+    const float f0 = __fadd_rn(u0, e0), f1 = __fadd_rn(u1, e1), f2 = __fadd_rn(u2, e2);
+    p.qx = __fmaf_rn(f2, F.a[6], __fmaf_rn(f1, F.a[3], __fmul_rn(f0, F.a[0])));
+    p.qy = __fmaf_rn(f2, F.a[7], __fmaf_rn(f1, F.a[4], __fmul_rn(f0, F.a[1])));
+    p.qz = __fmaf_rn(f2, F.a[8], __fmaf_rn(f1, F.a[5], __fmul_rn(f0, F.a[2])));
+    const int ki = __float_as_int(xi.w), kj = __float_as_int(xj.w);
+    p.l0 = (int)e0 + (ki & 1023) - (kj & 1023);
+    p.l1 = (int)e1 + ((ki >> 10) & 1023) - ((kj >> 10) & 1023);
+    p.l2 = (int)e2 + ((ki >> 20) & 1023) - ((kj >> 20) & 1023);
+    p.ok = valid && p.l0 >= -127 && p.l1 >= -127 && p.l2 >= -127 && p.l0 + m0 <= 128 && p.l1 + m1 <= 128 &&
+           p.l2 + m2 <= 128;
+    if (!p.ok) { p.qx = 1e18f; p.qy = 1e18f; p.qz = 1e18f; }
+    p.self = i == j ? (-(int)e0 * m1 - (int)e1) * m2 - (int)e2 : -1;   // (i,i,0) is not an edge (R3)
+    return p;
+}
+
+template <int W>
+__device__ __forceinline__ void mg_block_masks(const WarpSmem &sw, const CutoffArgs &A, const FindCtx &F,
+                                               const PairLane &p, int gi, int gj, int tile0, int ncl,
+                                               unsigned (&mask)[W]) {
+    mg_pair_masks<W>(sw, A, F, p.qx, p.qy, p.qz, gi, gj, p.l0, p.l1, p.l2, ncl, mask);
+    const int cs = p.self - tile0;
 #pragma unroll
-        for (int c = 0; c < 9; ++c) Ld[c] = (double)F.a[c];
-    }
-    int run = 0;
-    for (int tile0 = 0; tile0 < F.mloc; tile0 += 32 * W) {
-        const int ncl = min(32 * W, F.mloc - tile0);
-        if (F.mloc > 32 * W) mg_warp_table(sw, F.a, m1, m2, F.mloc, tile0, lane);
-        for (int q0 = 0; q0 < NP; q0 += 32) {
-            const int q = q0 + lane;
-            const bool valid = q < NP;
-            const int ri = valid ? mg_fdiv(q, inv_N) : 0;
-            const int j = valid ? q - ri * N : 0;
-            const int i = k.i0 + ri;
-            const float4 xi = sw.x[i], xj = sw.x[j];
-            // u = x_j - x_i (wrapped coordinates), first cell of the pair's sub-box: floor(-rho - u) + 1
-            const float u0 = __fsub_rn(xj.x, xi.x), u1 = __fsub_rn(xj.y, xi.y), u2 = __fsub_rn(xj.z, xi.z);
-            const float e0 = floorf(__fsub_rn(-F.rho[0], u0)) + 1.f, e1 = floorf(__fsub_rn(-F.rho[1], u1)) + 1.f,
-                        e2 = floorf(__fsub_rn(-F.rho[2], u2)) + 1.f;
-            const float f0 = __fadd_rn(u0, e0), f1 = __fadd_rn(u1, e1), f2 = __fadd_rn(u2, e2);
-            float qx = __fmaf_rn(f2, F.a[6], __fmaf_rn(f1, F.a[3], __fmul_rn(f0, F.a[0])));
-            float qy = __fmaf_rn(f2, F.a[7], __fmaf_rn(f1, F.a[4], __fmul_rn(f0, F.a[1])));
-            float qz = __fmaf_rn(f2, F.a[8], __fmaf_rn(f1, F.a[5], __fmul_rn(f0, F.a[2])));
-            // cell offsets relative to the coordinates AS GIVEN: tau = tau_wrapped + k_i - k_j
-            const int ki = __float_as_int(xi.w), kj = __float_as_int(xj.w);
-            const int l0 = (int)e0 + (ki & 1023) - (kj & 1023);
-            const int l1 = (int)e1 + ((ki >> 10) & 1023) - ((kj >> 10) & 1023);
-            const int l2 = (int)e2 + ((ki >> 20) & 1023) - ((kj >> 20) & 1023);
-            const bool inrange = l0 >= -127 && l1 >= -127 && l2 >= -127 && l0 + m0 <= 128 &&
-                                 l1 + m1 <= 128 && l2 + m2 <= 128;
-            if (MODE == MG_MODE_COUNT && valid && !inrange) atomicOr(A.status, MGS_OFFSET);
-            if (!valid || !inrange) { qx = 1e18f; qy = 1e18f; qz = 1e18f; }
-            unsigned mask[W];
-            mg_pair_masks<W>(sw, A, F, qx, qy, qz, k.first + i, k.first + j, l0, l1, l2, ncl, mask);
-            if (i == j) {                           // (i,i,0) is not an edge (R3)
-                const int cs = (-(int)e0 * m1 - (int)e1) * m2 - (int)e2 - tile0;
-#pragma unroll
-                for (int w = 0; w < W; ++w)
-                    if (cs >= 32 * w && cs < 32 * w + 32) mask[w] &= ~(1u << (cs & 31));
-            }
-            int cnt = 0;
-#pragma unroll
-            for (int w = 0; w < W; ++w) cnt += __popc(mask[w]);
-            if (MODE == MG_MODE_COUNT) {
-                run += cnt;                         // per lane; reduced once at the end
-            } else {
-                int incl = cnt;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const int v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
-                    if (lane >= o) incl += v;
-                }
-                const int tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
-                int pos = run + incl - cnt;
-                if (valid && j == 0 && tile0 == 0) {
-                    sw.rowoff[ri] = pos;
-                    A.row_ptr[k.first + i] = (int)(goff + pos);
-                }
-                const unsigned paircode = ((unsigned)(l0 + 128) << 24) | ((unsigned)(l1 + 128) << 16) |
-                                          ((unsigned)(l2 + 128) << 8) | (unsigned)j;
-#pragma unroll
-                for (int w = 0; w < W; ++w) {
-                    unsigned mk = mask[w];
-                    while (mk) {
-                        const int b = __ffs(mk) - 1;
-                        mk &= mk - 1;
-                        const unsigned code = paircode + sw.tcode[32 * w + b];
-                        if (MODE == MG_MODE_STASH) {
-                            if (pos < MG_STASH) stash[pos] = code;
-                        } else if (goff + pos < A.capacity) {
-                            mg_emit_edge(A, goff + pos, k.first + i, k.first + j, pd[i], pd[j], Ld, code >> 24,
-                                         (code >> 16) & 0xFFu, (code >> 8) & 0xFFu);
-                        }
-                        ++pos;
-                    }
-                }
-                run += tot;
-            }
-        }
-    }
-    if (MODE == MG_MODE_COUNT) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) run += __shfl_xor_sync(0xFFFFFFFFu, run, o);
-    } else {
-        __syncwarp();
-        if (lane == 0) sw.rowoff[k.nr] = run;
-        __syncwarp();
-    }
-    return (unsigned)run;
+    for (int w = 0; w < W; ++w)
+        if (p.self >= 0 && cs >= 32 * w && cs < 32 * w + 32) mask[w] &= ~(1u << (cs & 31));
 }
 
 // Constants of the find phase for structure s; stages the structure (positions, table when it
@@ -345,47 +285,6 @@ __device__ __forceinline__ bool mg_struct_setup(WarpSmem &sw, double (*pd)[3], c
     return true;
 }
 
-template <int MODE>
-__device__ __forceinline__ unsigned mg_find_dispatch(WarpSmem &sw, unsigned *stash, const double (*pd)[3],
-                                                     const CutoffArgs &A, const Task &k, const FindCtx &F,
-                                                     long long goff, int lane) {
-    if (F.mloc <= 32) return mg_warp_find<1, MODE>(sw, stash, pd, A, k, F, goff, lane);
-    if (F.mloc <= 64) return mg_warp_find<2, MODE>(sw, stash, pd, A, k, F, goff, lane);
-    return mg_warp_find<4, MODE>(sw, stash, pd, A, k, F, goff, lane);
-}
-
-// First (structure, row) of warp w's range: the first row whose cost prefix is >= c0 = w * chunk.
-// The cost prefix of row r of structure s is bpre[s / MG_CP_BLOCK] + rec[s].lpre + r * rowcost.
-__device__ inline void mg_range_start(const CutoffArgs &A, unsigned long long c0, int &s_out, int &r_out, int lane) {
-    // level 1: last prep block b with bpre[b] <= c0 (32-ary search)
-    int lo = 0, hi = A.n_blocks;                   // answer in [lo, hi)
-    while (hi - lo > 1) {
-        const int step = (hi - lo + 31) / 32;
-        const int idx = lo + (lane + 1) * step;
-        const bool ok = idx < hi && __ldg(A.bpre + idx) <= c0;
-        lo += __popc(__ballot_sync(0xFFFFFFFFu, ok)) * step;
-        hi = min(hi, lo + step);
-    }
-    const int b = lo;
-    const unsigned long long bp = __ldg(A.bpre + b);
-    // level 2: last structure of the block whose prefix is <= c0
-    int cnt = 0;
-#pragma unroll
-    for (int q = 0; q < MG_CP_BLOCK / 32; ++q) {
-        const int s = b * MG_CP_BLOCK + q * 32 + lane;
-        const bool ok = s < A.n_struct && bp + A.rec[s].lpre <= c0;
-        cnt += __popc(__ballot_sync(0xFFFFFFFFu, ok));
-    }
-    int s = b * MG_CP_BLOCK + max(cnt, 1) - 1;
-    const CutRec *R = A.rec + s;
-    const unsigned long long cs = bp + R->lpre;
-    const unsigned rc = R->rowcost;
-    int r = c0 > cs ? (int)((c0 - cs + rc - 1) / rc) : 0;
-    if (r >= R->natoms) { s += 1; r = 0; }         // every later row starts at or after c0
-    s_out = s;
-    r_out = r;
-}
-
 // Cost range of warp w: [c0, c1); the last warp takes everything that is left.
 __device__ __forceinline__ void mg_warp_range(const CutoffArgs &A, int w, unsigned long long &c0,
                                               unsigned long long &c1) {
@@ -395,8 +294,100 @@ __device__ __forceinline__ void mg_warp_range(const CutoffArgs &A, int w, unsign
     c1 = w == A.n_warps - 1 ? ~0ull : c0 + chunk;
 }
 
+// First (structure, pair) of the range that starts at cost c0: the first pair whose cost prefix
+// bpre[s / MG_CP_BLOCK] + rec[s].lpre + q * paircost is >= c0.
+__device__ inline void mg_range_start(const CutoffArgs &A, unsigned long long c0, int &s_out, int &q_out, int lane) {
+    int lo = 0, hi = A.n_blocks;                   // last prep block b with bpre[b] <= c0 (32-ary search)
+    while (hi - lo > 1) {
+        const int step = (hi - lo + 31) / 32;
+        const int idx = lo + (lane + 1) * step;
+        const bool ok = idx < hi && __ldg(A.bpre + idx) <= c0;
+        lo += __popc(__ballot_sync(0xFFFFFFFFu, ok)) * step;
+        hi = min(hi, lo + step);
+    }
+    const int b = lo;
+    const unsigned long long bp = __ldg(A.bpre + b);
+    int cnt = 0;                                   // structures of the block whose prefix is <= c0
+#pragma unroll
+    for (int x = 0; x < MG_CP_BLOCK / 32; ++x) {
+        const int s = b * MG_CP_BLOCK + x * 32 + lane;
+        const bool ok = s < A.n_struct && bp + A.rec[s].lpre <= c0;
+        cnt += __popc(__ballot_sync(0xFFFFFFFFu, ok));
+    }
+    int s = b * MG_CP_BLOCK + max(cnt, 1) - 1;
+    const CutRec *R = A.rec + s;
+    const unsigned long long cs = bp + R->lpre;
+    const unsigned pc = R->paircost;
+    const unsigned long long q = c0 > cs ? (c0 - cs + pc - 1) / pc : 0ull;
+    if (q >= (unsigned long long)(R->natoms * R->natoms)) { s_out = s + 1; q_out = 0; }   // later pairs start >= c0
+    else { s_out = s; q_out = (int)q; }
+}
+
+// The part [qa, qb) of structure s's pairs that belongs to the range ending at cost c1 (qa is
+// given: 0, or the range's first pair).  Returns false when the range ends before qa.
+__device__ __forceinline__ bool mg_segment(const CutoffArgs &A, const CutRec *R, int s, int qa,
+                                           unsigned long long c1, int &qb) {
+    const unsigned long long cs = __ldg(A.bpre + s / MG_CP_BLOCK) + R->lpre;
+    const unsigned pc = R->paircost;
+    const int NN = R->natoms * R->natoms;
+    if (cs + (unsigned long long)qa * pc >= c1) return false;
+    const unsigned long long room = c1 == ~0ull ? ~0ull : (c1 - cs + pc - 1) / pc;   // pairs that start before c1
+    qb = (int)min((unsigned long long)NN, room);
+    return true;
+}
+
 // ---------------------------------------------------------------------------------------------
-// Launch 1: count.
+// Launch 1: count.  Pairs [qa, qb) of the staged structure: hit masks -> edge count (per lane);
+// the masks go to the warp's scratch for the emit launch while they fit.
+template <int W>
+__device__ __forceinline__ unsigned mg_count_segment(const WarpSmem &sw, const CutoffArgs &A, const Task &k,
+                                                     const FindCtx &F, int qa, int qb, unsigned *wmask, int &midx,
+                                                     int lane) {
+    const int N = k.natoms;
+    const float inv_N = 1.f / (float)N;
+    unsigned acc = 0u;
+    for (int q0 = qa; q0 < qb; q0 += 32) {
+        const int q = q0 + lane;
+        const bool valid = q < qb;
+        const int i = valid ? mg_fdiv(q, inv_N) : 0, j = valid ? q - i * N : 0;
+        const PairLane p = mg_pair_setup(sw, F, valid, i, j);
+        if (valid && !p.ok) atomicOr(A.status, MGS_OFFSET);
+        unsigned mask[W];
+        mg_block_masks<W>(sw, A, F, p, k.first + i, k.first + j, 0, F.mloc, mask);
+        const bool keep = midx + 32 * W <= MG_MASK_WORDS;
+#pragma unroll
+        for (int w = 0; w < W; ++w) {
+            acc += __popc(mask[w]);
+            if (keep) wmask[midx + 32 * w + lane] = mask[w];
+        }
+        midx += 32 * W;
+    }
+    return acc;
+}
+
+// Structures whose table does not fit (mloc > MG_TLOC): row by row, tile by tile.
+__device__ __noinline__ unsigned mg_count_tiled(WarpSmem &sw, const CutoffArgs &A, const Task &k, const FindCtx &F,
+                                                int qa, int qb, int lane) {
+    const int N = k.natoms;
+    unsigned acc = 0u;
+    for (int tile0 = 0; tile0 < F.mloc; tile0 += MG_TLOC) {
+        const int ncl = min(MG_TLOC, F.mloc - tile0);
+        mg_warp_table(sw, F.a, (F.m >> 8) & 0xFF, (F.m >> 16) & 0xFF, F.mloc, tile0, lane);
+        for (int q0 = qa; q0 < qb; q0 += 32) {
+            const int q = q0 + lane;
+            const bool valid = q < qb;
+            const int i = valid ? q / N : 0, j = valid ? q - i * N : 0;
+            const PairLane p = mg_pair_setup(sw, F, valid, i, j);
+            if (valid && !p.ok && tile0 == 0) atomicOr(A.status, MGS_OFFSET);
+            unsigned mask[8];
+            mg_block_masks<8>(sw, A, F, p, k.first + i, k.first + j, tile0, ncl, mask);
+#pragma unroll
+            for (int w = 0; w < 8; ++w) acc += __popc(mask[w]);
+        }
+    }
+    return acc;
+}
+
 __global__ void __launch_bounds__(MG_BLOCK, 4)
 mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
     __shared__ WarpSmem s_w[MG_WARPS];
@@ -405,30 +396,33 @@ mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     WarpSmem &sw = s_w[warp];
     const int w = blockIdx.x * MG_WARPS + warp;
+    const long long t_begin = clock64();
     unsigned long long c0, c1;
     mg_warp_range(A, w, c0, c1);
-    int s, r;
-    mg_range_start(A, c0, s, r, lane);
-    if (lane == 0) A.wstart[w] = make_int2(s, r);
+    int s, qa;
+    mg_range_start(A, c0, s, qa, lane);
+    if (lane == 0) A.wstart[w] = make_int2(s, qa);
+    unsigned *wmask = A.wmask + (size_t)w * MG_MASK_WORDS;
+    int midx = 0;
     unsigned total = 0u;
-    for (; s < A.n_struct; ++s, r = 0) {
+    for (; s < A.n_struct; ++s, qa = 0) {
         const CutRec *R = A.rec + s;
-        const unsigned long long cs = __ldg(A.bpre + s / MG_CP_BLOCK) + R->lpre;
-        if (cs + (unsigned long long)r * R->rowcost >= c1 && R->natoms > 0) break;
-        if (R->natoms == 0) continue;
-        // rows r .. rb - 1 start before c1
-        const unsigned long long room = (c1 - cs + R->rowcost - 1) / R->rowcost;
-        const int rb = (int)min((unsigned long long)R->natoms, room);
+        int qb;
+        if (!mg_segment(A, R, s, qa, c1, qb)) break;
         Task k;
         FindCtx F;
-        if (mg_struct_setup(sw, nullptr, A, R, s, k, F, lane)) {
-            k.i0 = r;
-            k.nr = rb - r;
-            total += mg_find_dispatch<MG_MODE_COUNT>(sw, nullptr, nullptr, A, k, F, 0, lane);
+        if (qb > qa && mg_struct_setup(sw, nullptr, A, R, s, k, F, lane)) {
+            if (F.mloc <= 32) total += mg_count_segment<1>(sw, A, k, F, qa, qb, wmask, midx, lane);
+            else if (F.mloc <= 64) total += mg_count_segment<2>(sw, A, k, F, qa, qb, wmask, midx, lane);
+            else if (F.mloc <= 128) total += mg_count_segment<4>(sw, A, k, F, qa, qb, wmask, midx, lane);
+            else if (F.mloc <= MG_TLOC) total += mg_count_segment<8>(sw, A, k, F, qa, qb, wmask, midx, lane);
+            else total += mg_count_tiled(sw, A, k, F, qa, qb, lane);
         }
-        if (rb < R->natoms) break;
+        if (qb < R->natoms * R->natoms) break;
     }
-    if (lane == 0) A.wtotal[w] = total;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) total += __shfl_xor_sync(0xFFFFFFFFu, total, o);
+    if (lane == 0) { A.wtotal[w] = total; A.wclock[w] = (unsigned)(clock64() - t_begin); }
     // ---- last CTA out: exclusive scan of the warp totals, grand total
     __threadfence();
     __syncthreads();
@@ -459,6 +453,145 @@ mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
 
 // ---------------------------------------------------------------------------------------------
 // Launch 2: emit.
+struct EmitCtx {
+    double Ld[9];
+    long long goff;        // global index of the first edge in the stash
+    int run, qb0;          // stash fill, first pair of the stash's batch
+};
+
+// Lanes <-> pairs: every lane writes its own hits of one block straight to global memory,
+// starting at edge index pos (slow path: blocks that do not fit the stash, tiled structures).
+template <int W>
+__device__ __forceinline__ void mg_direct_block(const WarpSmem &sw, const double (*pd)[3], const CutoffArgs &A,
+                                                const Task &k, const EmitCtx &E, const PairLane &p, int i, int j,
+                                                const unsigned (&mask)[W], long long pos) {
+    const unsigned paircode = ((unsigned)(p.l0 + 128) << 24) | ((unsigned)(p.l1 + 128) << 16) |
+                              ((unsigned)(p.l2 + 128) << 8);
+#pragma unroll
+    for (int w = 0; w < W; ++w) {
+        unsigned mk = mask[w];
+        while (mk) {
+            const int b = __ffs(mk) - 1;
+            mk &= mk - 1;
+            const unsigned code = paircode + sw.tcode[32 * w + b];
+            if (pos < A.capacity)
+                mg_emit_edge(A, pos, k.first + i, k.first + j, pd[i], pd[j], E.Ld, code >> 24, (code >> 16) & 0xFFu,
+                             (code >> 8) & 0xFFu);
+            ++pos;
+        }
+    }
+}
+
+// Stash -> global: lanes over consecutive edges; the low byte of a code is the pair's index
+// relative to qb0.
+__device__ __forceinline__ void mg_flush(const EmitSmem &se, const CutoffArgs &A, const Task &k, const EmitCtx &E,
+                                         int run, int qb0, float inv_N, int lane) {
+    const int N = k.natoms;
+    const bool fits = E.goff + run <= A.capacity;
+    for (int e0 = 0; e0 < run; e0 += 32) {
+        const int e = e0 + lane;
+        if (e < run && (fits || E.goff + e < A.capacity)) {
+            const unsigned code = se.stash[e];
+            const int q = qb0 + (int)(code & 0xFFu);
+            const int i = mg_fdiv(q, inv_N), j = q - i * N;
+            mg_emit_edge(A, E.goff + e, k.first + i, k.first + j, se.pd[i], se.pd[j], E.Ld, code >> 24,
+                         (code >> 16) & 0xFFu, (code >> 8) & 0xFFu);
+        }
+    }
+}
+
+// Blocks of 32 pairs [qa, qb) against the cells [tile0, tile0 + ncl) of the table: hits appended
+// to the stash (E.run entries so far, pair indices relative to E.qb0), written out when it is full.
+// scratch: read the masks the count launch kept instead of evaluating them again.
+// pinned: E.qb0 stays (the caller walks the same pairs again for the next tile).
+template <int W>
+__device__ __forceinline__ void mg_emit_blocks(EmitSmem &se, const CutoffArgs &A, const Task &k, const FindCtx &F,
+                                               EmitCtx &E, int qa, int qb, int tile0, int ncl, bool scratch,
+                                               bool pinned, const unsigned *wmask, int &midx, int lane) {
+    const WarpSmem &sw = se.w;
+    const int N = k.natoms;
+    const float inv_N = 1.f / (float)N;
+    for (int q0 = qa; q0 < qb; q0 += 32) {
+        const int q = q0 + lane;
+        const bool valid = q < qb;
+        const int i = valid ? mg_fdiv(q, inv_N) : 0, j = valid ? q - i * N : 0;
+        const PairLane p = mg_pair_setup(sw, F, valid, i, j);
+        unsigned mask[W];
+        if (scratch && midx + 32 * W <= MG_MASK_WORDS) {
+#pragma unroll
+            for (int w = 0; w < W; ++w) mask[w] = __ldg(wmask + midx + 32 * w + lane);
+        } else {
+            mg_block_masks<W>(sw, A, F, p, k.first + i, k.first + j, tile0, ncl, mask);
+        }
+        if (scratch) midx += 32 * W;
+        int cnt = 0;
+#pragma unroll
+        for (int w = 0; w < W; ++w) cnt += __popc(mask[w]);
+        int incl = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+            if (lane >= o) incl += v;
+        }
+        const int tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
+        if (E.run + tot > MG_STASH || (!pinned && q0 + 32 - E.qb0 > 256)) {   // stash full: write it out
+            __syncwarp();
+            mg_flush(se, A, k, E, E.run, E.qb0, inv_N, lane);
+            __syncwarp();
+            E.goff += E.run;
+            E.run = 0;
+            if (!pinned) E.qb0 = q0;
+        }
+        int pos = E.run + incl - cnt;
+        if (valid && j == 0 && tile0 == 0) A.row_ptr[k.first + i] = (int)(E.goff + pos);
+        if (tot > MG_STASH) {                                     // one block alone overflows (run == 0)
+            mg_direct_block<W>(sw, se.pd, A, k, E, p, i, j, mask, E.goff + pos);
+            E.goff += tot;
+            if (!pinned) E.qb0 = q0 + 32;
+            continue;
+        }
+        const unsigned paircode = ((unsigned)(p.l0 + 128) << 24) | ((unsigned)(p.l1 + 128) << 16) |
+                                  ((unsigned)(p.l2 + 128) << 8) | (unsigned)(q - E.qb0);
+#pragma unroll
+        for (int w = 0; w < W; ++w) {
+            unsigned mk = mask[w];
+            while (mk) {
+                const int b = __ffs(mk) - 1;
+                mk &= mk - 1;
+                se.stash[pos++] = paircode + sw.tcode[32 * w + b];
+            }
+        }
+        E.run += tot;
+    }
+}
+
+__device__ __forceinline__ void mg_flush_all(EmitSmem &se, const CutoffArgs &A, const Task &k, EmitCtx &E, int lane) {
+    __syncwarp();
+    mg_flush(se, A, k, E, E.run, E.qb0, 1.f / (float)k.natoms, lane);
+    __syncwarp();
+    E.goff += E.run;
+    E.run = 0;
+}
+
+// Structures whose table does not fit (mloc > MG_TLOC): one source row at a time (its edges may
+// come in any order), tile by tile.
+__device__ __noinline__ void mg_emit_tiled(EmitSmem &se, const CutoffArgs &A, const Task &k, const FindCtx &F,
+                                           EmitCtx &E, int qa, int qb, int lane) {
+    WarpSmem &sw = se.w;
+    const int N = k.natoms;
+    int dummy = 0;
+    for (int i = qa / N; i * N < qb; ++i) {
+        const int ra = max(qa, i * N), rb = min(qb, (i + 1) * N);
+        E.qb0 = ra;
+        for (int tile0 = 0; tile0 < F.mloc; tile0 += MG_TLOC) {
+            mg_warp_table(sw, F.a, (F.m >> 8) & 0xFF, (F.m >> 16) & 0xFF, F.mloc, tile0, lane);
+            mg_emit_blocks<8>(se, A, k, F, E, ra, rb, tile0, min(MG_TLOC, F.mloc - tile0), false, true, nullptr,
+                              dummy, lane);
+        }
+        mg_flush_all(se, A, k, E, lane);
+    }
+}
+
 __global__ void __launch_bounds__(MG_BLOCK, 4)
 mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -466,51 +599,39 @@ mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
     EmitSmem &se = reinterpret_cast<EmitSmem *>(smem_raw)[warp];
     WarpSmem &sw = se.w;
     const int w = blockIdx.x * MG_WARPS + warp;
+    const long long t_begin = clock64();
     unsigned long long c0, c1;
     mg_warp_range(A, w, c0, c1);
     const int2 st = A.wstart[w];
-    int s = st.x, r = st.y;
-    long long goff = (long long)__ldg(A.wtotal + w);
-    for (; s < A.n_struct; ++s, r = 0) {
+    int s = st.x, qa = st.y;
+    const unsigned *wmask = A.wmask + (size_t)w * MG_MASK_WORDS;
+    int midx = 0;
+    EmitCtx E;
+    E.goff = (long long)__ldg(A.wtotal + w);
+    for (; s < A.n_struct; ++s, qa = 0) {
         const CutRec *R = A.rec + s;
-        const unsigned long long cs = __ldg(A.bpre + s / MG_CP_BLOCK) + R->lpre;
-        if (cs + (unsigned long long)r * R->rowcost >= c1 && R->natoms > 0) break;
-        if (R->natoms == 0) continue;
-        const unsigned long long room = (c1 - cs + R->rowcost - 1) / R->rowcost;
-        const int rb = (int)min((unsigned long long)R->natoms, room);
+        int qb;
+        if (!mg_segment(A, R, s, qa, c1, qb)) break;
         Task k;
         FindCtx F;
-        if (!mg_struct_setup(sw, se.pd, A, R, s, k, F, lane)) {
-            for (int i = r + lane; i < rb; i += 32) A.row_ptr[R->first + i] = (int)goff;   // no edges
-        } else {
-            double Ld[9];
+        if (qb > qa) {
+            if (!mg_struct_setup(sw, se.pd, A, R, s, k, F, lane)) {
+                const int N = R->natoms;                           // no edges: rows that start in [qa, qb)
+                for (int i = (qa + N - 1) / N + lane; i * N < qb; i += 32) A.row_ptr[R->first + i] = (int)E.goff;
+            } else {
 #pragma unroll
-            for (int c = 0; c < 9; ++c) Ld[c] = (double)F.a[c];
-            const int rpt = R->rpt;
-            for (int i0 = r; i0 < rb; i0 += rpt) {
-                k.i0 = i0;
-                k.nr = min(rpt, rb - i0);
-                const unsigned total = mg_find_dispatch<MG_MODE_STASH>(sw, se.stash, se.pd, A, k, F, goff, lane);
-                if (total > MG_STASH) {            // does not fit: search again, write directly
-                    mg_find_dispatch<MG_MODE_DIRECT>(sw, nullptr, se.pd, A, k, F, goff, lane);
-                } else {
-                    int rr = 0;
-                    for (int e0 = 0; e0 < (int)total; e0 += 32) {
-                        const int e = e0 + lane;
-                        if (e < (int)total) {
-                            while (e >= sw.rowoff[rr + 1]) ++rr;
-                            const unsigned code = se.stash[e];
-                            const int j = (int)(code & 0xFFu);
-                            if (goff + e < A.capacity)
-                                mg_emit_edge(A, goff + e, k.first + i0 + rr, k.first + j, se.pd[i0 + rr], se.pd[j], Ld,
-                                             code >> 24, (code >> 16) & 0xFFu, (code >> 8) & 0xFFu);
-                        }
-                    }
-                }
-                goff += total;
-                __syncwarp();
+                for (int c = 0; c < 9; ++c) E.Ld[c] = (double)F.a[c];
+                E.run = 0;
+                E.qb0 = qa;
+                if (F.mloc <= 32) mg_emit_blocks<1>(se, A, k, F, E, qa, qb, 0, F.mloc, true, false, wmask, midx, lane);
+                else if (F.mloc <= 64) mg_emit_blocks<2>(se, A, k, F, E, qa, qb, 0, F.mloc, true, false, wmask, midx, lane);
+                else if (F.mloc <= 128) mg_emit_blocks<4>(se, A, k, F, E, qa, qb, 0, F.mloc, true, false, wmask, midx, lane);
+                else if (F.mloc <= MG_TLOC) mg_emit_blocks<8>(se, A, k, F, E, qa, qb, 0, F.mloc, true, false, wmask, midx, lane);
+                else mg_emit_tiled(se, A, k, F, E, qa, qb, lane);
+                mg_flush_all(se, A, k, E, lane);
             }
         }
-        if (rb < R->natoms) break;
+        if (qb < R->natoms * R->natoms) break;
     }
+    if (lane == 0) A.wclock[A.n_warps + w] = (unsigned)(clock64() - t_begin);
 }

@@ -26,8 +26,10 @@ struct mg_ctx {
     int32_t *d_atom_struct = nullptr;     // [n_atoms]
     size_t atom_cap = 0;
     unsigned *d_wtotal = nullptr;         // [n_warps + 1] cutoff edges per warp / their exclusive scan
-    int2 *d_wstart = nullptr;             // [n_warps] first (structure, row) of each warp's range
-    int cut_warps = 0;
+    int2 *d_wstart = nullptr;             // [n_warps] first (structure, pair) of each warp's range
+    unsigned *d_wclock = nullptr;         // [2, n_warps] per-warp cycles of the last cutoff call
+    unsigned *d_wmask = nullptr;          // [n_warps, MG_MASK_WORDS] hit masks kept from count to emit
+    int cut_warps = 0, last_cut_warps = 0;
     CutRec *d_crec = nullptr;             // per-structure records of the cutoff path (cut_prep.cuh)
     unsigned long long *d_bpre = nullptr; // cost prefix over the prep blocks
     size_t crec_cap = 0;
@@ -107,7 +109,9 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
         const int occ = c->cutoff_occ < c->count_occ ? c->cutoff_occ : c->count_occ;
         c->cut_warps = c->sm_count * occ * MG_WARPS;
         if (occ >= 1 && (cudaMalloc(&c->d_wtotal, (c->cut_warps + 1) * sizeof(unsigned)) != cudaSuccess ||
-                         cudaMalloc(&c->d_wstart, c->cut_warps * sizeof(int2)) != cudaSuccess)) { mg_destroy(c); return MG_ERR_CUDA; }
+                         cudaMalloc(&c->d_wstart, c->cut_warps * sizeof(int2)) != cudaSuccess ||
+                         cudaMalloc(&c->d_wmask, (size_t)c->cut_warps * MG_MASK_WORDS * sizeof(unsigned)) != cudaSuccess ||
+                         cudaMalloc(&c->d_wclock, 2 * (size_t)c->cut_warps * sizeof(unsigned)) != cudaSuccess)) { mg_destroy(c); return MG_ERR_CUDA; }
     }
     if (c->cutoff_occ < 1 || c->count_occ < 1 || c->knn_occ[0] < 1 || c->knn_occ[1] < 1) { mg_destroy(c); return MG_ERR_CUDA; }
     *out = c;
@@ -120,6 +124,8 @@ extern "C" void mg_destroy(mg_ctx *c) {
     cudaFree(c->d_ctl);
     cudaFree(c->d_wtotal);
     cudaFree(c->d_wstart);
+    cudaFree(c->d_wmask);
+    cudaFree(c->d_wclock);
     cudaFree(c->d_crec);
     cudaFree(c->d_bpre);
     cudaFree(c->d_rec);
@@ -165,6 +171,19 @@ extern "C" mg_status mg_reserve(mg_ctx *c, int32_t n_struct, int32_t n_atoms) {
         c->rowptr_cap = cap;
     }
     return MG_OK;
+}
+
+// Tuning aid (not part of the public header): per-warp cycles and range starts of the last cutoff call.
+extern "C" int mg_debug_cut_warps(mg_ctx *c, unsigned *clocks_host, int *starts_host, int max_warps) {
+    if (!c) return -1;
+    cudaDeviceSynchronize();
+    const int n = c->last_cut_warps < max_warps ? c->last_cut_warps : max_warps;
+    if (n > 0) {
+        cudaMemcpy(clocks_host, c->d_wclock, (size_t)n * 4, cudaMemcpyDeviceToHost);
+        cudaMemcpy(clocks_host + max_warps, c->d_wclock + c->last_cut_warps, (size_t)n * 4, cudaMemcpyDeviceToHost);
+        cudaMemcpy(starts_host, c->d_wstart, (size_t)n * 8, cudaMemcpyDeviceToHost);
+    }
+    return c->last_cut_warps;
 }
 
 extern "C" int64_t mg_launch_count(const mg_ctx *c) { return c ? c->launches : 0; }
@@ -221,7 +240,7 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
     A.row_ptr = o->row_ptr; A.src = o->src; A.dst = o->dst; A.offset = o->offset;
     A.vec = o->vec; A.dist = o->dist; A.capacity = o->capacity; A.n_edges = (long long *)o->n_edges;
     A.rec = c->d_crec; A.bpre = c->d_bpre; A.n_blocks = n_blocks;
-    A.wtotal = c->d_wtotal; A.wstart = c->d_wstart;
+    A.wtotal = c->d_wtotal; A.wstart = c->d_wstart; A.wmask = c->d_wmask; A.wclock = c->d_wclock;
     A.ctl = c->d_ctl; A.status = c->d_ctl + 4;
     A.count_only = count_only;
     // one contiguous range of rows per warp; small batches use fewer warps (>= 1 row each)
@@ -229,6 +248,7 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
     const int cap_grid = (n_atoms + MG_WARPS) / MG_WARPS;
     if (grid > cap_grid) grid = cap_grid;
     A.n_warps = grid * MG_WARPS;
+    c->last_cut_warps = A.n_warps;
     mg_cutoff_count_kernel<<<grid, MG_BLOCK, 0, st>>>(A);
     MG_CUDA(cudaGetLastError());
     c->launches += 1;
