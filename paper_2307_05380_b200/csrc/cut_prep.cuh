@@ -95,8 +95,10 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
             // warp instructions per pair (count + emit launches): 11 per candidate, ~250 per block
             // of 32 pairs, 3.3 per edge; the per-structure staging is spread over its pairs
             // (structures whose table is tiled evaluate their candidates again in the emit launch)
-            const float percell = mloc > 256 ? 60.f : 11.f;
-            const float c = ((float)((mloc + 3) & ~3) * percell + 250.f) * (1.f / 32.f) + 3.3f * lam / (float)N +
+            // and walk them one source row (N of 32 lanes) at a time)
+            const float percell = mloc > 256 ? 11.f + 900.f / (float)N : (mloc > 128 ? 19.f : 11.f);
+            const float perblock = mloc > 256 ? 120.f + 16000.f / (float)N : (mloc > 128 ? 500.f : 250.f);
+            const float c = ((float)((mloc + 3) & ~3) * percell + perblock) * (1.f / 32.f) + 3.3f * lam / (float)N +
                             MG_STRUCT_COST / (float)(N * N);
             r.paircost = (unsigned)fminf(16.f * c + 1.f, 16777216.f);
         }

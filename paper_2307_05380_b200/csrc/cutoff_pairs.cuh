@@ -41,12 +41,14 @@ struct CutoffArgs {
     const CutRec *rec;
     const unsigned long long *bpre;   // [n_blocks + 1] cost prefix over the prep blocks, [n_blocks] = total
     int n_blocks;
-    int n_warps;                   // warps of the grid (same for both launches)
-    unsigned *wtotal;              // [n_warps + 1] edges per warp -> exclusive scan
-    int2 *wstart;                  // [n_warps] first (structure, pair) of each warp's range
-    unsigned *wmask;               // [n_warps, MG_MASK_WORDS] hit masks kept from count to emit
+    int n_warps;                   // warps of the grid
+    int n_ranges;                  // MG_OVER * n_warps ranges: the first n_warps are taken by the warp of
+                                   // the same index, the others through a ticket (evens out the tail)
+    unsigned *wtotal;              // [n_ranges + 1] edges per range -> exclusive scan
+    int2 *wstart;                  // [n_ranges] first (structure, pair) of each range
+    unsigned *wmask;               // [n_ranges, MG_MASK_WORDS] hit masks kept from count to emit
     unsigned *wclock;              // [2, n_warps] cycles each warp spent in count / emit (tuning aid)
-    unsigned *ctl;                 // [1] count CTAs done
+    unsigned *ctl;                 // [0] count ticket, [1] count CTAs done, [8] emit ticket, [9] emit CTAs done
     unsigned *status;
     int count_only;
 };
@@ -56,6 +58,7 @@ struct CutoffArgs {
 #define MG_MODE_STASH 1
 #define MG_MODE_DIRECT 2
 
+#define MG_OVER 1                  // ranges per warp (> 1: the extra ranges go by ticket)
 #define MG_MASK_WORDS 4096         // per-warp mask scratch (32-bit words, multiple of 128)
 
 struct WarpSmem {
@@ -289,9 +292,9 @@ __device__ __forceinline__ bool mg_struct_setup(WarpSmem &sw, double (*pd)[3], c
 __device__ __forceinline__ void mg_warp_range(const CutoffArgs &A, int w, unsigned long long &c0,
                                               unsigned long long &c1) {
     const unsigned long long total = __ldg(A.bpre + A.n_blocks);
-    const unsigned long long chunk = (total + (unsigned)A.n_warps - 1) / (unsigned)A.n_warps;
+    const unsigned long long chunk = (total + (unsigned)A.n_ranges - 1) / (unsigned)A.n_ranges;
     c0 = (unsigned long long)w * chunk;
-    c1 = w == A.n_warps - 1 ? ~0ull : c0 + chunk;
+    c1 = w == A.n_ranges - 1 ? ~0ull : c0 + chunk;
 }
 
 // First (structure, pair) of the range that starts at cost c0: the first pair whose cost prefix
@@ -395,34 +398,41 @@ mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
     __shared__ bool s_last;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     WarpSmem &sw = s_w[warp];
-    const int w = blockIdx.x * MG_WARPS + warp;
+    // consecutive ranges (often parts of one expensive structure) go to different SMs
+    const int wid = warp * gridDim.x + blockIdx.x;
     const long long t_begin = clock64();
-    unsigned long long c0, c1;
-    mg_warp_range(A, w, c0, c1);
-    int s, qa;
-    mg_range_start(A, c0, s, qa, lane);
-    if (lane == 0) A.wstart[w] = make_int2(s, qa);
-    unsigned *wmask = A.wmask + (size_t)w * MG_MASK_WORDS;
-    int midx = 0;
-    unsigned total = 0u;
-    for (; s < A.n_struct; ++s, qa = 0) {
-        const CutRec *R = A.rec + s;
-        int qb;
-        if (!mg_segment(A, R, s, qa, c1, qb)) break;
-        Task k;
-        FindCtx F;
-        if (qb > qa && mg_struct_setup(sw, nullptr, A, R, s, k, F, lane)) {
-            if (F.mloc <= 32) total += mg_count_segment<1>(sw, A, k, F, qa, qb, wmask, midx, lane);
-            else if (F.mloc <= 64) total += mg_count_segment<2>(sw, A, k, F, qa, qb, wmask, midx, lane);
-            else if (F.mloc <= 128) total += mg_count_segment<4>(sw, A, k, F, qa, qb, wmask, midx, lane);
-            else if (F.mloc <= MG_TLOC) total += mg_count_segment<8>(sw, A, k, F, qa, qb, wmask, midx, lane);
-            else total += mg_count_tiled(sw, A, k, F, qa, qb, lane);
+    for (int w = wid; w < A.n_ranges;) {
+        int w_next = 0;
+        if (lane == 0) w_next = (int)atomicAdd(A.ctl, 1u) + A.n_warps;     // needed only at the end
+        unsigned long long c0, c1;
+        mg_warp_range(A, w, c0, c1);
+        int s, qa;
+        mg_range_start(A, c0, s, qa, lane);
+        if (lane == 0) A.wstart[w] = make_int2(s, qa);
+        unsigned *wmask = A.wmask + (size_t)w * MG_MASK_WORDS;
+        int midx = 0;
+        unsigned total = 0u;
+        for (; s < A.n_struct; ++s, qa = 0) {
+            const CutRec *R = A.rec + s;
+            int qb;
+            if (!mg_segment(A, R, s, qa, c1, qb)) break;
+            Task k;
+            FindCtx F;
+            if (qb > qa && mg_struct_setup(sw, nullptr, A, R, s, k, F, lane)) {
+                if (F.mloc <= 32) total += mg_count_segment<1>(sw, A, k, F, qa, qb, wmask, midx, lane);
+                else if (F.mloc <= 64) total += mg_count_segment<2>(sw, A, k, F, qa, qb, wmask, midx, lane);
+                else if (F.mloc <= 128) total += mg_count_segment<4>(sw, A, k, F, qa, qb, wmask, midx, lane);
+                else if (F.mloc <= MG_TLOC) total += mg_count_segment<8>(sw, A, k, F, qa, qb, wmask, midx, lane);
+                else total += mg_count_tiled(sw, A, k, F, qa, qb, lane);
+            }
+            if (qb < R->natoms * R->natoms) break;
         }
-        if (qb < R->natoms * R->natoms) break;
-    }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) total += __shfl_xor_sync(0xFFFFFFFFu, total, o);
-    if (lane == 0) { A.wtotal[w] = total; A.wclock[w] = (unsigned)(clock64() - t_begin); }
+        for (int o = 16; o > 0; o >>= 1) total += __shfl_xor_sync(0xFFFFFFFFu, total, o);
+        if (lane == 0) A.wtotal[w] = total;
+        w = __shfl_sync(0xFFFFFFFFu, w_next, 0);
+    }
+    if (lane == 0) A.wclock[wid] = (unsigned)(clock64() - t_begin);
     // ---- last CTA out: exclusive scan of the warp totals, grand total
     __threadfence();
     __syncthreads();
@@ -430,7 +440,7 @@ mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
     __syncthreads();
     if (!s_last) return;
     __threadfence();
-    const int nw = A.n_warps, per = (nw + MG_BLOCK - 1) / MG_BLOCK;
+    const int nw = A.n_ranges, per = (nw + MG_BLOCK - 1) / MG_BLOCK;
     const int b = threadIdx.x * per, e = min(nw, b + per);
     unsigned long long sum = 0ull;
     for (int g = b; g < e; ++g) sum += __ldcg(A.wtotal + g);
@@ -447,6 +457,7 @@ mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
         *A.n_edges = (long long)off;
         A.row_ptr[A.n_atoms] = (int)off;
         if (off > 0x7FFFFFFFull || (!A.count_only && (long long)off > A.capacity)) atomicOr(A.status, MGS_CAPACITY);
+        A.ctl[0] = 0u;
         A.ctl[1] = 0u;
     }
 }
@@ -483,20 +494,38 @@ __device__ __forceinline__ void mg_direct_block(const WarpSmem &sw, const double
 }
 
 // Stash -> global: lanes over consecutive edges; the low byte of a code is the pair's index
-// relative to qb0.
+// relative to qb0.  vec = (p_j - p_i) + tau . L in FP64, rounded once (R24).
 __device__ __forceinline__ void mg_flush(const EmitSmem &se, const CutoffArgs &A, const Task &k, const EmitCtx &E,
                                          int run, int qb0, float inv_N, int lane) {
+    if (run == 0) return;
     const int N = k.natoms;
-    const bool fits = E.goff + run <= A.capacity;
-    for (int e0 = 0; e0 < run; e0 += 32) {
-        const int e = e0 + lane;
-        if (e < run && (fits || E.goff + e < A.capacity)) {
-            const unsigned code = se.stash[e];
-            const int q = qb0 + (int)(code & 0xFFu);
-            const int i = mg_fdiv(q, inv_N), j = q - i * N;
-            mg_emit_edge(A, E.goff + e, k.first + i, k.first + j, se.pd[i], se.pd[j], E.Ld, code >> 24,
-                         (code >> 16) & 0xFFu, (code >> 8) & 0xFFu);
-        }
+    // edges that fit the caller's arrays (all of them unless the capacity is exceeded)
+    const long long room = A.capacity - E.goff;
+    const int lim = room >= run ? run : (room > 0 ? (int)room : 0);
+    int32_t *psrc = A.src + E.goff, *pdst = A.dst + E.goff;
+    int8_t *poff = A.offset + 3 * E.goff;
+    float *pvec = A.vec + 3 * E.goff;
+    float *pdist = A.dist ? A.dist + E.goff : nullptr;
+    for (int e = lane; e < lim; e += 32) {
+        const unsigned code = se.stash[e];
+        const int q = qb0 + (int)(code & 0xFFu);
+        const int i = mg_fdiv(q, inv_N), j = q - i * N;
+        const double *pi = se.pd[i], *pj = se.pd[j];
+        // (double)(b - 128) without a conversion instruction: 2^52 + b has b in its low mantissa word
+        const double t0 = __hiloint2double(0x43300000, (int)(code >> 24)) - 4503599627370624.0;
+        const double t1 = __hiloint2double(0x43300000, (int)((code >> 16) & 0xFFu)) - 4503599627370624.0;
+        const double t2 = __hiloint2double(0x43300000, (int)((code >> 8) & 0xFFu)) - 4503599627370624.0;
+        const double v0 = fma(t2, E.Ld[6], fma(t1, E.Ld[3], fma(t0, E.Ld[0], pj[0] - pi[0])));
+        const double v1 = fma(t2, E.Ld[7], fma(t1, E.Ld[4], fma(t0, E.Ld[1], pj[1] - pi[1])));
+        const double v2 = fma(t2, E.Ld[8], fma(t1, E.Ld[5], fma(t0, E.Ld[2], pj[2] - pi[2])));
+        const unsigned tb = code ^ 0x80808000u;              // tau bytes as int8
+        psrc[e] = k.first + i;
+        pdst[e] = k.first + j;
+        int8_t *po = poff + 3 * e;
+        po[0] = (int8_t)(tb >> 24); po[1] = (int8_t)(tb >> 16); po[2] = (int8_t)(tb >> 8);
+        float *pv = pvec + 3 * e;
+        pv[0] = (float)v0; pv[1] = (float)v1; pv[2] = (float)v2;
+        if (pdist) pdist[e] = __fsqrt_rn((float)fma(v2, v2, fma(v1, v1, v0 * v0)));
     }
 }
 
@@ -598,40 +627,52 @@ mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     EmitSmem &se = reinterpret_cast<EmitSmem *>(smem_raw)[warp];
     WarpSmem &sw = se.w;
-    const int w = blockIdx.x * MG_WARPS + warp;
+    // consecutive ranges (often parts of one expensive structure) go to different SMs
+    const int wid = warp * gridDim.x + blockIdx.x;
     const long long t_begin = clock64();
-    unsigned long long c0, c1;
-    mg_warp_range(A, w, c0, c1);
-    const int2 st = A.wstart[w];
-    int s = st.x, qa = st.y;
-    const unsigned *wmask = A.wmask + (size_t)w * MG_MASK_WORDS;
-    int midx = 0;
-    EmitCtx E;
-    E.goff = (long long)__ldg(A.wtotal + w);
-    for (; s < A.n_struct; ++s, qa = 0) {
-        const CutRec *R = A.rec + s;
-        int qb;
-        if (!mg_segment(A, R, s, qa, c1, qb)) break;
-        Task k;
-        FindCtx F;
-        if (qb > qa) {
-            if (!mg_struct_setup(sw, se.pd, A, R, s, k, F, lane)) {
-                const int N = R->natoms;                           // no edges: rows that start in [qa, qb)
-                for (int i = (qa + N - 1) / N + lane; i * N < qb; i += 32) A.row_ptr[R->first + i] = (int)E.goff;
-            } else {
+    for (int w = wid; w < A.n_ranges;) {
+        int w_next = 0;
+        if (lane == 0) w_next = (int)atomicAdd(A.ctl + 8, 1u) + A.n_warps;
+        unsigned long long c0, c1;
+        mg_warp_range(A, w, c0, c1);
+        const int2 st = A.wstart[w];
+        int s = st.x, qa = st.y;
+        const unsigned *wmask = A.wmask + (size_t)w * MG_MASK_WORDS;
+        int midx = 0;
+        EmitCtx E;
+        E.goff = (long long)__ldg(A.wtotal + w);
+        for (; s < A.n_struct; ++s, qa = 0) {
+            const CutRec *R = A.rec + s;
+            int qb;
+            if (!mg_segment(A, R, s, qa, c1, qb)) break;
+            Task k;
+            FindCtx F;
+            if (qb > qa) {
+                if (!mg_struct_setup(sw, se.pd, A, R, s, k, F, lane)) {
+                    const int N = R->natoms;                       // no edges: rows that start in [qa, qb)
+                    for (int i = (qa + N - 1) / N + lane; i * N < qb; i += 32) A.row_ptr[R->first + i] = (int)E.goff;
+                } else {
 #pragma unroll
-                for (int c = 0; c < 9; ++c) E.Ld[c] = (double)F.a[c];
-                E.run = 0;
-                E.qb0 = qa;
-                if (F.mloc <= 32) mg_emit_blocks<1>(se, A, k, F, E, qa, qb, 0, F.mloc, true, false, wmask, midx, lane);
-                else if (F.mloc <= 64) mg_emit_blocks<2>(se, A, k, F, E, qa, qb, 0, F.mloc, true, false, wmask, midx, lane);
-                else if (F.mloc <= 128) mg_emit_blocks<4>(se, A, k, F, E, qa, qb, 0, F.mloc, true, false, wmask, midx, lane);
-                else if (F.mloc <= MG_TLOC) mg_emit_blocks<8>(se, A, k, F, E, qa, qb, 0, F.mloc, true, false, wmask, midx, lane);
-                else mg_emit_tiled(se, A, k, F, E, qa, qb, lane);
-                mg_flush_all(se, A, k, E, lane);
+                    for (int c = 0; c < 9; ++c) E.Ld[c] = (double)F.a[c];
+                    E.run = 0;
+                    E.qb0 = qa;
+                    if (F.mloc <= 32) mg_emit_blocks<1>(se, A, k, F, E, qa, qb, 0, F.mloc, true, false, wmask, midx, lane);
+                    else if (F.mloc <= 64) mg_emit_blocks<2>(se, A, k, F, E, qa, qb, 0, F.mloc, true, false, wmask, midx, lane);
+                    else if (F.mloc <= 128) mg_emit_blocks<4>(se, A, k, F, E, qa, qb, 0, F.mloc, true, false, wmask, midx, lane);
+                    else if (F.mloc <= MG_TLOC) mg_emit_blocks<8>(se, A, k, F, E, qa, qb, 0, F.mloc, true, false, wmask, midx, lane);
+                    else mg_emit_tiled(se, A, k, F, E, qa, qb, lane);
+                    mg_flush_all(se, A, k, E, lane);
+                }
             }
+            if (qb < R->natoms * R->natoms) break;
         }
-        if (qb < R->natoms * R->natoms) break;
+        w = __shfl_sync(0xFFFFFFFFu, w_next, 0);
     }
-    if (lane == 0) A.wclock[A.n_warps + w] = (unsigned)(clock64() - t_begin);
+    if (lane == 0) A.wclock[A.n_warps + wid] = (unsigned)(clock64() - t_begin);
+    // last CTA out resets the ticket for the next launch
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        if (atomicAdd(A.ctl + 9, 1u) == gridDim.x - 1) { A.ctl[8] = 0u; A.ctl[9] = 0u; }
+    }
 }

@@ -108,9 +108,9 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
     {
         const int occ = c->cutoff_occ < c->count_occ ? c->cutoff_occ : c->count_occ;
         c->cut_warps = c->sm_count * occ * MG_WARPS;
-        if (occ >= 1 && (cudaMalloc(&c->d_wtotal, (c->cut_warps + 1) * sizeof(unsigned)) != cudaSuccess ||
-                         cudaMalloc(&c->d_wstart, c->cut_warps * sizeof(int2)) != cudaSuccess ||
-                         cudaMalloc(&c->d_wmask, (size_t)c->cut_warps * MG_MASK_WORDS * sizeof(unsigned)) != cudaSuccess ||
+        if (occ >= 1 && (cudaMalloc(&c->d_wtotal, (MG_OVER * c->cut_warps + 1) * sizeof(unsigned)) != cudaSuccess ||
+                         cudaMalloc(&c->d_wstart, MG_OVER * c->cut_warps * sizeof(int2)) != cudaSuccess ||
+                         cudaMalloc(&c->d_wmask, (size_t)MG_OVER * c->cut_warps * MG_MASK_WORDS * sizeof(unsigned)) != cudaSuccess ||
                          cudaMalloc(&c->d_wclock, 2 * (size_t)c->cut_warps * sizeof(unsigned)) != cudaSuccess)) { mg_destroy(c); return MG_ERR_CUDA; }
     }
     if (c->cutoff_occ < 1 || c->count_occ < 1 || c->knn_occ[0] < 1 || c->knn_occ[1] < 1) { mg_destroy(c); return MG_ERR_CUDA; }
@@ -248,6 +248,7 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
     const int cap_grid = (n_atoms + MG_WARPS) / MG_WARPS;
     if (grid > cap_grid) grid = cap_grid;
     A.n_warps = grid * MG_WARPS;
+    A.n_ranges = MG_OVER * A.n_warps;
     c->last_cut_warps = A.n_warps;
     mg_cutoff_count_kernel<<<grid, MG_BLOCK, 0, st>>>(A);
     MG_CUDA(cudaGetLastError());
