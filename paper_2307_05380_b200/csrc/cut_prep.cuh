@@ -21,6 +21,7 @@
 
 #define MG_CP_BLOCK 128
 #define MG_STASH 1024              // stash entries per warp of the emit kernel (cutoff_pairs.cuh)
+#define MG_KNN_ALPHA 1.8f           // KNN: expected images inside the first search radius, in units of k
 #define MG_STRUCT_COST 900.f        // warp instructions' worth of latency to stage one structure (both launches)
 
 struct CutRec {              // 64 bytes
@@ -33,7 +34,8 @@ struct CutRec {              // 64 bytes
     unsigned long long lpre; // prefix of natoms^2 * paircost inside the structure's prep block
     float amax_sum;          // sum_a max_c |L_ac|
     float qmax;              // Q = sum_a (rho_a + 1) max_c |L_ac|
-    int pad[2];
+    float radius;            // KNN: search radius of the structure (cutoff graph: r_c)
+    int pad;
 };
 static_assert(sizeof(CutRec) == 64, "CutRec is one 64-byte line");
 
@@ -41,7 +43,12 @@ struct CutPrepArgs {
     const float *lattice;
     const int32_t *struct_ptr;
     int n_struct, n_atoms;
-    float r_c;
+    float r_c;                     // cutoff graph: the cutoff.  KNN (k > 0): unused
+    int k;                         // KNN: neighbours per atom; the radius of structure s is chosen so that
+                                   // about MG_KNN_ALPHA * k images are expected inside (or taken from hint[s])
+    float *hint;                   // KNN, [n_struct] or NULL: largest k-th distance of the previous call
+                                   // (read when use_hint, then reset to 0: the graph kernel maxes into it)
+    int use_hint;
     CutRec *rec;                   // [n_struct]
     unsigned long long *bpre;      // [blocks + 1] block sums -> exclusive prefix; [blocks] = total
     unsigned *ctl;                 // [7] blocks done
@@ -65,6 +72,15 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
         for (int c = 0; c < 9; ++c) lat[c] = A.lattice[9 * (size_t)s + c];
         double vol = 0.0, h[3] = {1.0, 1.0, 1.0};
         unsigned err = mg_cell_spacings_fast(lat, &vol, h);
+        float rc = A.r_c;
+        if (A.k > 0) {                                 // KNN: radius from the density, or from the last call
+            const float hv = A.hint && A.use_hint ? A.hint[s] : 0.f;
+            rc = 1.08f * cbrtf(0.2387324f * (MG_KNN_ALPHA * (float)A.k + 1.f) * (float)vol / (float)max(N, 1));
+            if (hv > 0.f && isfinite(hv)) rc = 1.02f * hv + 1e-3f;
+            if (!(rc > 1e-6f) || !isfinite(rc)) rc = 1.f;
+            if (A.hint) A.hint[s] = 0.f;
+        }
+        r.radius = rc;
         if (N > MG_SMALL_MAX_ATOMS) err |= MGS_UNSUPPORTED;
         r.mloc = 0;
         r.m = 0;
@@ -77,7 +93,7 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
             r.amax_sum += amax;
             // rho = r_c / h rounded up, plus the guard for the FP32 rounding of u = x_j - x_i and
             // of -rho - u (wrapped coordinates: |u| <= 1)
-            const float rho = __double2float_ru((double)A.r_c / h[a] * (1.0 + 4e-6)) + 4e-6f;
+            const float rho = __double2float_ru((double)rc / h[a] * (1.0 + 4e-6)) + 4e-6f;
             r.rho[a] = rho;
             float mf = floorf(2.f * rho + 1e-5f) + 1.f;
             if (!(mf <= 255.f)) { err |= MGS_OFFSET; mf = 1.f; }
@@ -91,7 +107,7 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
         if (err) atomicOr(A.status, err);
         r.paircost = 1u;
         if (r.mloc > 0) {
-            const float lam = (float)N * 4.18879f * A.r_c * A.r_c * A.r_c / (float)vol;   // edges per row
+            const float lam = (float)N * 4.18879f * rc * rc * rc / (float)vol;   // edges per row
             // warp instructions per pair (count + emit launches): 11 per candidate, ~250 per block
             // of 32 pairs, 3.3 per edge; the per-structure staging is spread over its pairs
             // (structures whose table is tiled evaluate their candidates again in the emit launch)
@@ -100,9 +116,12 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
             const float perblock = mloc > 256 ? 120.f + 16000.f / (float)N : (mloc > 128 ? 500.f : 250.f);
             const float c = ((float)((mloc + 3) & ~3) * percell + perblock) * (1.f / 32.f) + 3.3f * lam / (float)N +
                             MG_STRUCT_COST / (float)(N * N);
-            r.paircost = (unsigned)fminf(16.f * c + 1.f, 16777216.f);
+            // KNN: one launch, no edge stream; selecting k per row costs about 350
+            const float ck = ((float)((mloc + 3) & ~3) * 11.f + 150.f) * (1.f / 32.f) + 350.f / (float)N +
+                             0.5f * MG_STRUCT_COST / (float)(N * N);
+            r.paircost = (unsigned)fminf(16.f * (A.k > 0 ? ck : c) + 1.f, 16777216.f);
         }
-        r.pad[0] = r.pad[1] = 0;
+        r.pad = 0;
         cost = (unsigned long long)(N * N) * r.paircost;      // N <= 64
     }
     // ---- block-wide exclusive scan of the cost

@@ -77,6 +77,13 @@ struct Task {
     int s, first, natoms;
 };
 
+// What the range walk needs (shared by the cutoff and the KNN kernels).
+struct RangeCtx {
+    const CutRec *rec;
+    const unsigned long long *bpre;
+    int n_blocks, n_struct, n_ranges;
+};
+
 // q / n for 0 <= q < 2^20, 1 <= n (exact: (q + 0.5) / n is never within rounding of an integer)
 __device__ __forceinline__ int mg_fdiv(int q, float inv_n) {
     return __float2int_rz(__fmul_rn((float)q + 0.5f, inv_n));
@@ -107,13 +114,13 @@ __device__ __forceinline__ void mg_emit_edge(const CutoffArgs &A, long long e, i
 // part packed in .w (10 bits per axis, biased by 512); with pd != nullptr also the FP64 cartesian
 // positions of the coordinates AS GIVEN.  Returns false if a coordinate is non-finite or its
 // integer part does not fit (then the structure emits nothing and the status word is set).
-__device__ __forceinline__ bool mg_warp_stage(WarpSmem &sw, double (*pd)[3], const CutoffArgs &A, const Task &k,
-                                              int lane) {
-    const float *L = A.lattice + 9 * (size_t)k.s;
+__device__ __forceinline__ bool mg_warp_stage(WarpSmem &sw, double (*pd)[3], const float *pos, const float *lattice,
+                                              const Task &k, int lane) {
+    const float *L = lattice + 9 * (size_t)k.s;
     bool ok = true;
     __syncwarp();
     for (int j = lane; j < k.natoms; j += 32) {
-        const float *xp = A.pos + 3 * (size_t)(k.first + j);
+        const float *xp = pos + 3 * (size_t)(k.first + j);
         const float x0 = xp[0], x1 = xp[1], x2 = xp[2];
         const float g0 = floorf(x0), g1 = floorf(x1), g2 = floorf(x2);
         ok = ok && fabsf(g0) <= 500.f && fabsf(g1) <= 500.f && fabsf(g2) <= 500.f;   // false for NaN / inf
@@ -162,6 +169,8 @@ __device__ __forceinline__ void mg_warp_table(WarpSmem &sw, const float a[9], in
 struct FindCtx {
     float a[9];            // lattice rows (FP32)
     const float *lat;      // the same, global
+    const float *pos;      // positions of the batch (exact predicate)
+    float rc;              // radius of the predicate d < rc
     float rho[3];
     int m;                 // m_0 | m_1 << 8 | m_2 << 16
     int mloc;
@@ -172,7 +181,7 @@ struct FindCtx {
 // registers (W words = 32 W cells).  Lanes that saw a candidate inside the rounding window decide
 // their window cells with the exact FP64 predicate.
 template <int W>
-__device__ __forceinline__ void mg_pair_masks(const WarpSmem &sw, const CutoffArgs &A, const FindCtx &F,
+__device__ __forceinline__ void mg_pair_masks(const WarpSmem &sw, const FindCtx &F,
                                               float qx, float qy, float qz, int gi, int gj,
                                               int l0, int l1, int l2, int ncl, unsigned (&mask)[W]) {
     bool near = false;
@@ -196,7 +205,7 @@ __device__ __forceinline__ void mg_pair_masks(const WarpSmem &sw, const CutoffAr
         }
     }
     if (near) {                                   // rare: decide the window cells in FP64
-        const float *xi = A.pos + 3 * (size_t)gi, *xj = A.pos + 3 * (size_t)gj;
+        const float *xi = F.pos + 3 * (size_t)gi, *xj = F.pos + 3 * (size_t)gj;
         for (int c = 0; c < ncl; ++c) {
             const float4 T = sw.T[c];
             const float vx = __fadd_rn(qx, T.x), vy = __fadd_rn(qy, T.y), vz = __fadd_rn(qz, T.z);
@@ -209,7 +218,7 @@ __device__ __forceinline__ void mg_pair_masks(const WarpSmem &sw, const CutoffAr
                 const unsigned bit = 1u << (c & 31);
 #pragma unroll
                 for (int w = 0; w < W; ++w)
-                    if (w == (c >> 5)) mask[w] = d < (double)A.r_c ? (mask[w] | bit) : (mask[w] & ~bit);
+                    if (w == (c >> 5)) mask[w] = d < (double)F.rc ? (mask[w] | bit) : (mask[w] & ~bit);
             }
         }
     }
@@ -249,24 +258,28 @@ __device__ __forceinline__ PairLane mg_pair_setup(const WarpSmem &sw, const Find
 }
 
 template <int W>
-__device__ __forceinline__ void mg_block_masks(const WarpSmem &sw, const CutoffArgs &A, const FindCtx &F,
+__device__ __forceinline__ void mg_block_masks(const WarpSmem &sw, const FindCtx &F,
                                                const PairLane &p, int gi, int gj, int tile0, int ncl,
                                                unsigned (&mask)[W]) {
-    mg_pair_masks<W>(sw, A, F, p.qx, p.qy, p.qz, gi, gj, p.l0, p.l1, p.l2, ncl, mask);
+    mg_pair_masks<W>(sw, F, p.qx, p.qy, p.qz, gi, gj, p.l0, p.l1, p.l2, ncl, mask);
     const int cs = p.self - tile0;
 #pragma unroll
     for (int w = 0; w < W; ++w)
         if (p.self >= 0 && cs >= 32 * w && cs < 32 * w + 32) mask[w] &= ~(1u << (cs & 31));
 }
 
-// Constants of the find phase for structure s; stages the structure (positions, table when it
-// fits).  Returns false if the structure emits nothing (empty, invalid lattice or positions).
-__device__ __forceinline__ bool mg_struct_setup(WarpSmem &sw, double (*pd)[3], const CutoffArgs &A, const CutRec *R,
-                                                int s, Task &k, FindCtx &F, int lane) {
+// Constants of the find phase for structure s with radius rc; stages the structure (positions,
+// table when it fits).  Returns false if the structure emits nothing (empty, invalid lattice or
+// positions).
+__device__ __forceinline__ bool mg_struct_setup(WarpSmem &sw, double (*pd)[3], const float *pos, const float *lattice,
+                                                unsigned *status, float rc, const CutRec *R, int s, Task &k,
+                                                FindCtx &F, int lane) {
     k.s = s;
     k.first = R->first;
     k.natoms = R->natoms;
-    F.lat = A.lattice + 9 * (size_t)s;
+    F.lat = lattice + 9 * (size_t)s;
+    F.pos = pos;
+    F.rc = rc;
     F.mloc = R->mloc;
     if (F.mloc <= 0) return false;
 #pragma unroll
@@ -274,13 +287,13 @@ __device__ __forceinline__ bool mg_struct_setup(WarpSmem &sw, double (*pd)[3], c
 #pragma unroll
     for (int a = 0; a < 3; ++a) F.rho[a] = R->rho[a];
     F.m = R->m;
-    F.nr2 = -__fmul_rn(A.r_c, A.r_c);
-    // FP32 error bound of d2 - r_c^2 near the threshold (R23): the components of q', T
+    F.nr2 = -__fmul_rn(rc, rc);
+    // FP32 error bound of d2 - rc^2 near the threshold (R23): the components of q', T
     // and q' + T are below 3 Q, about 13 roundings of 2^-24 relative size reach v (the wrapped
     // coordinates are below 1, their difference is rounded once), d2 = v . v adds 3 more
-    F.win = 1.1920929e-7f * (2.f * A.r_c * (13.f * R->qmax + 2.f * R->amax_sum) + 4.f * A.r_c * A.r_c);
-    if (!mg_warp_stage(sw, pd, A, k, lane)) {
-        if (lane == 0) atomicOr(A.status, MGS_NONFINITE);
+    F.win = 1.1920929e-7f * (2.f * rc * (13.f * R->qmax + 2.f * R->amax_sum) + 4.f * rc * rc);
+    if (!mg_warp_stage(sw, pd, pos, lattice, k, lane)) {
+        if (lane == 0) atomicOr(status, MGS_NONFINITE);
         F.mloc = 0;
         return false;
     }
@@ -289,7 +302,7 @@ __device__ __forceinline__ bool mg_struct_setup(WarpSmem &sw, double (*pd)[3], c
 }
 
 // Cost range of warp w: [c0, c1); the last warp takes everything that is left.
-__device__ __forceinline__ void mg_warp_range(const CutoffArgs &A, int w, unsigned long long &c0,
+__device__ __forceinline__ void mg_warp_range(const RangeCtx &A, int w, unsigned long long &c0,
                                               unsigned long long &c1) {
     const unsigned long long total = __ldg(A.bpre + A.n_blocks);
     const unsigned long long chunk = (total + (unsigned)A.n_ranges - 1) / (unsigned)A.n_ranges;
@@ -299,7 +312,7 @@ __device__ __forceinline__ void mg_warp_range(const CutoffArgs &A, int w, unsign
 
 // First (structure, pair) of the range that starts at cost c0: the first pair whose cost prefix
 // bpre[s / MG_CP_BLOCK] + rec[s].lpre + q * paircost is >= c0.
-__device__ inline void mg_range_start(const CutoffArgs &A, unsigned long long c0, int &s_out, int &q_out, int lane) {
+__device__ inline void mg_range_start(const RangeCtx &A, unsigned long long c0, int &s_out, int &q_out, int lane) {
     int lo = 0, hi = A.n_blocks;                   // last prep block b with bpre[b] <= c0 (32-ary search)
     while (hi - lo > 1) {
         const int step = (hi - lo + 31) / 32;
@@ -328,7 +341,7 @@ __device__ inline void mg_range_start(const CutoffArgs &A, unsigned long long c0
 
 // The part [qa, qb) of structure s's pairs that belongs to the range ending at cost c1 (qa is
 // given: 0, or the range's first pair).  Returns false when the range ends before qa.
-__device__ __forceinline__ bool mg_segment(const CutoffArgs &A, const CutRec *R, int s, int qa,
+__device__ __forceinline__ bool mg_segment(const RangeCtx &A, const CutRec *R, int s, int qa,
                                            unsigned long long c1, int &qb) {
     const unsigned long long cs = __ldg(A.bpre + s / MG_CP_BLOCK) + R->lpre;
     const unsigned pc = R->paircost;
@@ -356,7 +369,7 @@ __device__ __forceinline__ unsigned mg_count_segment(const WarpSmem &sw, const C
         const PairLane p = mg_pair_setup(sw, F, valid, i, j);
         if (valid && !p.ok) atomicOr(A.status, MGS_OFFSET);
         unsigned mask[W];
-        mg_block_masks<W>(sw, A, F, p, k.first + i, k.first + j, 0, F.mloc, mask);
+        mg_block_masks<W>(sw, F, p, k.first + i, k.first + j, 0, F.mloc, mask);
         const bool keep = midx + 32 * W <= MG_MASK_WORDS;
 #pragma unroll
         for (int w = 0; w < W; ++w) {
@@ -383,7 +396,7 @@ __device__ __noinline__ unsigned mg_count_tiled(WarpSmem &sw, const CutoffArgs &
             const PairLane p = mg_pair_setup(sw, F, valid, i, j);
             if (valid && !p.ok && tile0 == 0) atomicOr(A.status, MGS_OFFSET);
             unsigned mask[8];
-            mg_block_masks<8>(sw, A, F, p, k.first + i, k.first + j, tile0, ncl, mask);
+            mg_block_masks<8>(sw, F, p, k.first + i, k.first + j, tile0, ncl, mask);
 #pragma unroll
             for (int w = 0; w < 8; ++w) acc += __popc(mask[w]);
         }
@@ -401,13 +414,15 @@ mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
     // consecutive ranges (often parts of one expensive structure) go to different SMs
     const int wid = warp * gridDim.x + blockIdx.x;
     const long long t_begin = clock64();
+    RangeCtx RC;
+    RC.rec = A.rec; RC.bpre = A.bpre; RC.n_blocks = A.n_blocks; RC.n_struct = A.n_struct; RC.n_ranges = A.n_ranges;
     for (int w = wid; w < A.n_ranges;) {
         int w_next = 0;
         if (lane == 0) w_next = (int)atomicAdd(A.ctl, 1u) + A.n_warps;     // needed only at the end
         unsigned long long c0, c1;
-        mg_warp_range(A, w, c0, c1);
+        mg_warp_range(RC, w, c0, c1);
         int s, qa;
-        mg_range_start(A, c0, s, qa, lane);
+        mg_range_start(RC, c0, s, qa, lane);
         if (lane == 0) A.wstart[w] = make_int2(s, qa);
         unsigned *wmask = A.wmask + (size_t)w * MG_MASK_WORDS;
         int midx = 0;
@@ -415,10 +430,10 @@ mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
         for (; s < A.n_struct; ++s, qa = 0) {
             const CutRec *R = A.rec + s;
             int qb;
-            if (!mg_segment(A, R, s, qa, c1, qb)) break;
+            if (!mg_segment(RC, R, s, qa, c1, qb)) break;
             Task k;
             FindCtx F;
-            if (qb > qa && mg_struct_setup(sw, nullptr, A, R, s, k, F, lane)) {
+            if (qb > qa && mg_struct_setup(sw, nullptr, A.pos, A.lattice, A.status, A.r_c, R, s, k, F, lane)) {
                 if (F.mloc <= 32) total += mg_count_segment<1>(sw, A, k, F, qa, qb, wmask, midx, lane);
                 else if (F.mloc <= 64) total += mg_count_segment<2>(sw, A, k, F, qa, qb, wmask, midx, lane);
                 else if (F.mloc <= 128) total += mg_count_segment<4>(sw, A, k, F, qa, qb, wmask, midx, lane);
@@ -550,7 +565,7 @@ __device__ __forceinline__ void mg_emit_blocks(EmitSmem &se, const CutoffArgs &A
 #pragma unroll
             for (int w = 0; w < W; ++w) mask[w] = __ldg(wmask + midx + 32 * w + lane);
         } else {
-            mg_block_masks<W>(sw, A, F, p, k.first + i, k.first + j, tile0, ncl, mask);
+            mg_block_masks<W>(sw, F, p, k.first + i, k.first + j, tile0, ncl, mask);
         }
         if (scratch) midx += 32 * W;
         int cnt = 0;
@@ -630,11 +645,13 @@ mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
     // consecutive ranges (often parts of one expensive structure) go to different SMs
     const int wid = warp * gridDim.x + blockIdx.x;
     const long long t_begin = clock64();
+    RangeCtx RC;
+    RC.rec = A.rec; RC.bpre = A.bpre; RC.n_blocks = A.n_blocks; RC.n_struct = A.n_struct; RC.n_ranges = A.n_ranges;
     for (int w = wid; w < A.n_ranges;) {
         int w_next = 0;
         if (lane == 0) w_next = (int)atomicAdd(A.ctl + 8, 1u) + A.n_warps;
         unsigned long long c0, c1;
-        mg_warp_range(A, w, c0, c1);
+        mg_warp_range(RC, w, c0, c1);
         const int2 st = A.wstart[w];
         int s = st.x, qa = st.y;
         const unsigned *wmask = A.wmask + (size_t)w * MG_MASK_WORDS;
@@ -644,11 +661,11 @@ mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
         for (; s < A.n_struct; ++s, qa = 0) {
             const CutRec *R = A.rec + s;
             int qb;
-            if (!mg_segment(A, R, s, qa, c1, qb)) break;
+            if (!mg_segment(RC, R, s, qa, c1, qb)) break;
             Task k;
             FindCtx F;
             if (qb > qa) {
-                if (!mg_struct_setup(sw, se.pd, A, R, s, k, F, lane)) {
+                if (!mg_struct_setup(sw, se.pd, A.pos, A.lattice, A.status, A.r_c, R, s, k, F, lane)) {
                     const int N = R->natoms;                       // no edges: rows that start in [qa, qb)
                     for (int i = (qa + N - 1) / N + lane; i * N < qb; i += 32) A.row_ptr[R->first + i] = (int)E.goff;
                 } else {

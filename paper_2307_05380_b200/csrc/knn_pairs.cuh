@@ -1,0 +1,284 @@
+// knn_pairs.cuh — k-nearest-neighbour multigraph, k <= 32, structures of <= MG_SMALL_MAX_ATOMS atoms.
+//
+// Problem: per source the k smallest keys (d, dst, tau_x, tau_y, tau_z) over all periodic images
+// except (i,i,0) (Alg. 2 lines 2-5, made deterministic: DESIGN.md R2, R8).
+// Method (Alg. 1, re-designed).  mg_cut_prep_kernel picks one search radius R per
+// structure (expected MG_KNN_ALPHA * k images inside, or the largest k-th distance of the previous
+// mg_update_graph call) and, like for the cutoff graph, the per-pair sub-box that holds every image
+// closer than R.  One launch, autonomous warps, each owning a contiguous equally expensive range
+// of source rows (cutoff_pairs.cuh):
+//   find    lane <-> ordered pair (i, j): hit mask over the pair's sub-box (d2 < R^2 in FP32),
+//           hits -> shared-memory stash as 64-bit keys (d2 bits | tau + 128 bytes, j) in (row, j)
+//           order: "evaluate_area" + "concatenate" of Alg. 1-2;
+//   select  per source row: bitonic sort of its keys, 32 at a time, keeping the 32 smallest (Alg. 2's
+//           "sort, keep k").  Alg. 1 line 4: if the k-th key is not safely inside R (or fewer than k
+//           images were found) the row is searched again by the growing-radius routine of
+//           knn_small.cuh.  The k selected entries get their exact FP64 distance and their final
+//           order (d, dst, tau); vec / dist are the FP64 values rounded once.
+#pragma once
+#include "common.cuh"
+#include "cut_prep.cuh"
+#include "cutoff_pairs.cuh"
+#include "knn_small.cuh"
+
+#define MG_KSTASH 768              // 64-bit keys per warp
+
+struct KnnPairsArgs {
+    const float *pos;
+    const float *lattice;
+    const int32_t *struct_ptr;
+    int n_struct, n_atoms;
+    int k;
+    int32_t *row_ptr, *src, *dst;
+    int8_t *offset;
+    float *vec, *dist;
+    long long *n_edges;
+    float *hint;                   // [n_struct] or NULL: max k-th distance per structure (atomicMax)
+    const CutRec *rec;
+    const unsigned long long *bpre;
+    int n_blocks;
+    int n_warps;
+    unsigned *status;
+};
+
+struct KnnSmem {
+    WarpSmem w;                    // table, staged positions
+    unsigned long long stash[MG_KSTASH];
+    int rowoff[MG_SMALL_MAX_ATOMS + 1];
+};
+
+// Growing-radius search of one source row with the routine of knn_small.cuh (rare path).  Uses the
+// table area of the warp's shared memory as scratch: the caller rebuilds the table afterwards.
+__device__ __noinline__ void mg_knn_row_fallback(KnnSmem &ks, const KnnPairsArgs &A, int s, int first, int N, int i,
+                                                 int lane) {
+    const float *lat9 = A.lattice + 9 * (size_t)s;
+    float4 *sp = reinterpret_cast<float4 *>(ks.w.T);
+    mg_key *buf = reinterpret_cast<mg_key *>(ks.w.T + MG_SMALL_MAX_ATOMS);
+    StructRec R;
+    float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f};
+    __syncwarp();
+    for (int j = lane; j < N; j += 32) {
+        const float *x = A.pos + 3 * (size_t)(first + j);
+        const float x0 = x[0], x1 = x[1], x2 = x[2];
+        lo[0] = fminf(lo[0], x0); lo[1] = fminf(lo[1], x1); lo[2] = fminf(lo[2], x2);
+        hi[0] = fmaxf(hi[0], x0); hi[1] = fmaxf(hi[1], x1); hi[2] = fmaxf(hi[2], x2);
+        float4 p;
+        p.x = __fmaf_rn(x2, lat9[6], __fmaf_rn(x1, lat9[3], __fmul_rn(x0, lat9[0])));
+        p.y = __fmaf_rn(x2, lat9[7], __fmaf_rn(x1, lat9[4], __fmul_rn(x0, lat9[1])));
+        p.z = __fmaf_rn(x2, lat9[8], __fmaf_rn(x1, lat9[5], __fmul_rn(x0, lat9[2])));
+        p.w = 0.f;
+        sp[j] = p;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            lo[a] = fminf(lo[a], __shfl_xor_sync(0xFFFFFFFFu, lo[a], o));
+            hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xFFFFFFFFu, hi[a], o));
+        }
+    __syncwarp();
+    float lat[9];
+#pragma unroll
+    for (int c = 0; c < 9; ++c) lat[c] = lat9[c];
+    double vol = 1.0, h[3] = {1.0, 1.0, 1.0};
+    mg_cell_spacings(lat, &vol, h);                   // the lattice is valid: prep checked it
+    R.first = first;
+    R.natoms = N;
+    R.volume = (float)vol;
+    R.err = 0u;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        R.xmin[a] = lo[a];
+        R.xmax[a] = hi[a];
+        R.h_dn[a] = __double2float_rd(h[a] * (1.0 - 1e-6));
+        R.invh_up[a] = __double2float_ru((1.0 + 1e-6) / h[a]);
+        R.amax[a] = fmaxf(fabsf(lat[3 * a]), fmaxf(fabsf(lat[3 * a + 1]), fabsf(lat[3 * a + 2])));
+    }
+    KnnArgs K;
+    K.pos = A.pos; K.lattice = A.lattice; K.struct_ptr = A.struct_ptr;
+    K.n_struct = A.n_struct; K.n_atoms = A.n_atoms; K.k = A.k;
+    K.row_ptr = A.row_ptr; K.src = A.src; K.dst = A.dst; K.offset = A.offset;
+    K.vec = A.vec; K.dist = A.dist; K.n_edges = A.n_edges;
+    float *slot = reinterpret_cast<float *>(ks.w.T + MG_SMALL_MAX_ATOMS + 16);   // k-th distance comes back here
+    K.radius_hint = A.hint ? slot - (first + i) : nullptr; K.use_hint = 0;
+    K.rec = nullptr; K.atom_struct = nullptr; K.ctl = nullptr; K.status = A.status;
+    mg_knn_source<1>(K, R, lat9, sp, buf, i, lane);
+    __syncwarp();
+    if (A.hint && lane == 0) atomicMax(reinterpret_cast<int *>(A.hint + s), __float_as_int(*slot));
+    __syncwarp();
+}
+
+// Hits of the pairs [qa, qb) (whole rows) of the staged structure -> stash, row offsets -> rowoff.
+// Returns the number of hits (positions >= MG_KSTASH are dropped: the caller checks).
+template <int W>
+__device__ __forceinline__ int mg_knn_find(KnnSmem &ks, const Task &k, const FindCtx &F, int i0, int qa, int qb,
+                                           int lane) {
+    const WarpSmem &sw = ks.w;
+    const int N = k.natoms;
+    const float inv_N = 1.f / (float)N;
+    int run = 0;
+    for (int q0 = qa; q0 < qb; q0 += 32) {
+        const int q = q0 + lane;
+        const bool valid = q < qb;
+        const int i = valid ? mg_fdiv(q, inv_N) : 0, j = valid ? q - i * N : 0;
+        const PairLane p = mg_pair_setup(sw, F, valid, i, j);
+        unsigned mask[W];
+        mg_block_masks<W>(sw, F, p, k.first + i, k.first + j, 0, F.mloc, mask);
+        int cnt = 0;
+#pragma unroll
+        for (int w = 0; w < W; ++w) cnt += __popc(mask[w]);
+        int incl = cnt;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+            if (lane >= o) incl += v;
+        }
+        int pos = run + incl - cnt;
+        if (valid && j == 0) ks.rowoff[i - i0] = pos;
+        const unsigned paircode = ((unsigned)(p.l0 + 128) << 24) | ((unsigned)(p.l1 + 128) << 16) |
+                                  ((unsigned)(p.l2 + 128) << 8) | (unsigned)j;
+#pragma unroll
+        for (int w = 0; w < W; ++w) {
+            unsigned mk = mask[w];
+            while (mk) {
+                const int b = __ffs(mk) - 1;
+                mk &= mk - 1;
+                const float4 T = sw.T[32 * w + b];
+                const float vx = __fadd_rn(p.qx, T.x), vy = __fadd_rn(p.qy, T.y), vz = __fadd_rn(p.qz, T.z);
+                const float d2 = __fmaf_rn(vz, vz, __fmaf_rn(vy, vy, __fmul_rn(vx, vx)));
+                if (pos < MG_KSTASH)
+                    ks.stash[pos] = ((unsigned long long)__float_as_uint(d2) << 32) | (paircode + sw.tcode[32 * w + b]);
+                ++pos;
+            }
+        }
+        run += __shfl_sync(0xFFFFFFFFu, incl, 31);
+    }
+    return run;
+}
+
+__global__ void __launch_bounds__(MG_BLOCK, 4)
+mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    KnnSmem &ks = reinterpret_cast<KnnSmem *>(smem_raw)[warp];
+    WarpSmem &sw = ks.w;
+    for (long long t = (long long)blockIdx.x * MG_BLOCK + threadIdx.x; t <= A.n_atoms; t += (long long)gridDim.x * MG_BLOCK)
+        A.row_ptr[t] = (int)((long long)A.k * t);
+    if (blockIdx.x == 0 && threadIdx.x == 0) *A.n_edges = (long long)A.k * A.n_atoms;
+    const int K = A.k;
+    RangeCtx RC;
+    RC.rec = A.rec; RC.bpre = A.bpre; RC.n_blocks = A.n_blocks; RC.n_struct = A.n_struct; RC.n_ranges = A.n_warps;
+    const int wid = warp * gridDim.x + blockIdx.x;
+    unsigned long long c0, c1;
+    mg_warp_range(RC, wid, c0, c1);
+    int s, qa;
+    mg_range_start(RC, c0, s, qa, lane);
+    for (; s < A.n_struct; ++s, qa = 0) {
+        const CutRec *R = A.rec + s;
+        int qb;
+        if (!mg_segment(RC, R, s, qa, c1, qb)) break;
+        const int N = R->natoms;
+        // source rows whose first pair lies in [qa, qb)
+        const int ia = N ? (qa + N - 1) / N : 0, ib = N ? (qb + N - 1) / N : 0;
+        Task k;
+        FindCtx F;
+        if (ib > ia) {
+            const float rad = R->radius;
+            if (!mg_struct_setup(sw, nullptr, A.pos, A.lattice, A.status, rad, R, s, k, F, lane)) {
+                // invalid lattice / positions: placeholder rows (src = dst, zero vec); mg_check reports
+                for (int e = ia * K + lane; e < ib * K; e += 32) {
+                    const long long o = (long long)K * R->first + e;
+                    const int g = R->first + e / K;
+                    A.src[o] = g; A.dst[o] = g;
+                    A.offset[3 * o] = 0; A.offset[3 * o + 1] = 0; A.offset[3 * o + 2] = 0;
+                    A.vec[3 * o] = 0.f; A.vec[3 * o + 1] = 0.f; A.vec[3 * o + 2] = 0.f;
+                    if (A.dist) A.dist[o] = 0.f;
+                }
+            } else {
+                F.win = 0.f;                                   // no exact threshold decision here
+                // every image with true d2 < R^2 - win is a hit; a k-th key below R^2 - 2 win is safe
+                const float win = 1.1920929e-7f * (2.f * rad * (13.f * R->qmax + 2.f * R->amax_sum) + 4.f * rad * rad);
+                const float lim2 = __fmaf_rn(-2.f, win, __fmul_rn(rad, rad));
+                // rows per group: expected hits fit the stash
+                const int rpt = max(1, min(MG_SMALL_MAX_ATOMS, (int)((float)MG_KSTASH / (2.2f * MG_KNN_ALPHA * (float)K + 8.f))));
+                float dkmax = 0.f;
+                for (int i0 = ia; i0 < ib; i0 += rpt) {
+                    const int nr = min(rpt, ib - i0);
+                    int total;
+                    if (F.mloc > MG_TLOC) total = MG_KSTASH + 1;          // table does not fit: row by row below
+                    else if (F.mloc <= 32) total = mg_knn_find<1>(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
+                    else if (F.mloc <= 64) total = mg_knn_find<2>(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
+                    else if (F.mloc <= 128) total = mg_knn_find<4>(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
+                    else total = mg_knn_find<8>(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
+                    __syncwarp();
+                    if (lane == 0) ks.rowoff[nr] = total;
+                    __syncwarp();
+                    bool dirty = false;
+                    for (int r = 0; r < nr; ++r) {
+                        const int i = i0 + r, gi = k.first + i;
+                        bool ok = total <= MG_KSTASH;
+                        mg_key key = MG_KEY_INF;
+                        float kth_d2 = 0.f;
+                        if (ok) {
+                            const int b0 = ks.rowoff[r], cnt = ks.rowoff[r + 1] - b0;
+                            ok = cnt >= K;
+                            if (ok) {
+                                key = mg_sort32(lane < cnt ? ks.stash[b0 + lane] : MG_KEY_INF, lane);
+                                for (int c = 32; c < cnt; c += 32) {
+                                    mg_key keys1[1] = {key};
+                                    mg_knn_merge<1>(keys1, c + lane < cnt ? ks.stash[b0 + c + lane] : MG_KEY_INF, lane);
+                                    key = keys1[0];
+                                }
+                                const mg_key kth = __shfl_sync(0xFFFFFFFFu, key, K - 1);
+                                kth_d2 = __uint_as_float((unsigned)(kth >> 32));
+                                ok = kth != MG_KEY_INF && kth_d2 < lim2;
+                            }
+                        }
+                        if (!ok) {                             // Alg. 1 line 4: not settled inside R
+                            mg_knn_row_fallback(ks, A, s, k.first, N, i, lane);
+                            dirty = true;
+                            continue;
+                        }
+                        // exact FP64 distance of the selected entries, final order (d, dst, tau), emit
+                        const unsigned tie = (unsigned)key;    // tau + 128 bytes | j: orders like (dst, tau)... see below
+                        const int j = (int)(tie & 0xFFu);
+                        const int t0 = (int)(tie >> 24) - 128, t1 = (int)((tie >> 16) & 0xFFu) - 128,
+                                  t2 = (int)((tie >> 8) & 0xFFu) - 128;
+                        const unsigned ord = ((unsigned)j << 24) | (tie >> 8);      // (dst, tau_x, tau_y, tau_z)
+                        // entries after the k-th that FP32 cannot tell from it take part in the exact ranking
+                        const bool amb = lane >= K && key != MG_KEY_INF &&
+                                         __uint_as_float((unsigned)(key >> 32)) <= __fmaf_rn(2.f, win, kth_d2);
+                        const int nsel = K + __popc(__ballot_sync(0xFFFFFFFFu, amb));
+                        double dd = 1e300, vv[3] = {0.0, 0.0, 0.0};
+                        if (lane < nsel)
+                            dd = mg_exact_vec(A.pos + 3 * (size_t)gi, A.pos + 3 * (size_t)(k.first + j), t0, t1, t2, F.lat, vv);
+                        int rank = 0;
+                        for (int l = 0; l < nsel; ++l) {
+                            const double od = __shfl_sync(0xFFFFFFFFu, dd, l);
+                            const unsigned oo = __shfl_sync(0xFFFFFFFFu, ord, l);
+                            rank += (od < dd || (od == dd && oo < ord)) ? 1 : 0;
+                        }
+                        if (lane < nsel && rank < K) {
+                            const long long e = (long long)K * gi + rank;
+                            A.src[e] = gi;
+                            A.dst[e] = k.first + j;
+                            A.offset[3 * e] = (int8_t)t0; A.offset[3 * e + 1] = (int8_t)t1; A.offset[3 * e + 2] = (int8_t)t2;
+                            A.vec[3 * e] = (float)vv[0]; A.vec[3 * e + 1] = (float)vv[1]; A.vec[3 * e + 2] = (float)vv[2];
+                            if (A.dist) A.dist[e] = (float)dd;
+                            if (rank == K - 1) dkmax = fmaxf(dkmax, __double2float_ru(dd));
+                        }
+                    }
+                    if (dirty && F.mloc <= MG_TLOC) {          // the fallback used the table area as scratch
+                        mg_warp_table(sw, F.a, (F.m >> 8) & 0xFF, (F.m >> 16) & 0xFF, F.mloc, 0, lane);
+                    }
+                }
+                if (A.hint) {
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) dkmax = fmaxf(dkmax, __shfl_xor_sync(0xFFFFFFFFu, dkmax, o));
+                    if (lane == 0 && dkmax > 0.f) atomicMax(reinterpret_cast<int *>(A.hint + s), __float_as_int(dkmax));
+                }
+            }
+        }
+        if (qb < N * N) break;
+    }
+}

@@ -14,6 +14,7 @@
 #include "cut_prep.cuh"
 #include "cutoff_pairs.cuh"
 #include "knn_small.cuh"
+#include "knn_pairs.cuh"
 
 struct mg_ctx {
     int device = 0;
@@ -37,7 +38,7 @@ struct mg_ctx {
     size_t rowptr_cap = 0;
     long long *d_count = nullptr;
     unsigned epoch = 0;
-    int cutoff_occ = 0, count_occ = 0, knn_occ[2] = {0, 0};
+    int cutoff_occ = 0, count_occ = 0, knn_occ[2] = {0, 0}, knnp_occ = 0;
     int64_t launches = 0;
     // device mirrors for the _host entry points
     void *h_dev[9] = {nullptr};
@@ -103,6 +104,9 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
                              (int)(MG_WARPS * sizeof(EmitSmem))) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->cutoff_occ, mg_cutoff_emit_kernel, MG_BLOCK, (MG_WARPS * sizeof(EmitSmem)));
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->count_occ, mg_cutoff_count_kernel, MG_BLOCK, 0);
+    if (cudaFuncSetAttribute(mg_knn_pairs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)(MG_WARPS * sizeof(KnnSmem))) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->knnp_occ, mg_knn_pairs_kernel, MG_BLOCK, (MG_WARPS * sizeof(KnnSmem)));
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->knn_occ[0], mg_knn_small_kernel<1>, MG_BLOCK, 0);
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->knn_occ[1], mg_knn_small_kernel<2>, MG_BLOCK, 0);
     {
@@ -113,7 +117,7 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
                          cudaMalloc(&c->d_wmask, (size_t)MG_OVER * c->cut_warps * MG_MASK_WORDS * sizeof(unsigned)) != cudaSuccess ||
                          cudaMalloc(&c->d_wclock, 2 * (size_t)c->cut_warps * sizeof(unsigned)) != cudaSuccess)) { mg_destroy(c); return MG_ERR_CUDA; }
     }
-    if (c->cutoff_occ < 1 || c->count_occ < 1 || c->knn_occ[0] < 1 || c->knn_occ[1] < 1) { mg_destroy(c); return MG_ERR_CUDA; }
+    if (c->cutoff_occ < 1 || c->count_occ < 1 || c->knnp_occ < 1 || c->knn_occ[0] < 1 || c->knn_occ[1] < 1) { mg_destroy(c); return MG_ERR_CUDA; }
     *out = c;
     return MG_OK;
 }
@@ -229,6 +233,7 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
     {
         CutPrepArgs P;
         P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms; P.r_c = r_c;
+        P.k = 0; P.hint = nullptr; P.use_hint = 0;
         P.rec = c->d_crec; P.bpre = c->d_bpre; P.ctl = c->d_ctl; P.status = c->d_ctl + 4;
         mg_cut_prep_kernel<<<n_blocks, MG_CP_BLOCK, 0, st>>>(P);
         MG_CUDA(cudaGetLastError());
@@ -295,6 +300,31 @@ static mg_status launch_knn(mg_ctx *c, const float *pos, const float *lat, const
     MG_CUDA(cudaSetDevice(c->device));
     mg_status rs = mg_reserve(c, n_struct, n_atoms);
     if (rs != MG_OK) return rs;
+    if (k <= 32 && n_struct > 0) {                      // pair-lane kernel (knn_pairs.cuh)
+        const int n_blocks = (n_struct + MG_CP_BLOCK - 1) / MG_CP_BLOCK;
+        CutPrepArgs P;
+        P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms; P.r_c = 0.f;
+        P.k = k; P.hint = hint; P.use_hint = use_hint;
+        P.rec = c->d_crec; P.bpre = c->d_bpre; P.ctl = c->d_ctl; P.status = c->d_ctl + 4;
+        mg_cut_prep_kernel<<<n_blocks, MG_CP_BLOCK, 0, st>>>(P);
+        MG_CUDA(cudaGetLastError());
+        c->launches += 1;
+        KnnPairsArgs A;
+        A.pos = pos; A.lattice = lat; A.struct_ptr = sp;
+        A.n_struct = n_struct; A.n_atoms = n_atoms; A.k = k;
+        A.row_ptr = o->row_ptr; A.src = o->src; A.dst = o->dst; A.offset = o->offset;
+        A.vec = o->vec; A.dist = o->dist; A.n_edges = (long long *)o->n_edges;
+        A.hint = hint; A.rec = c->d_crec; A.bpre = c->d_bpre; A.n_blocks = n_blocks;
+        A.status = c->d_ctl + 4;
+        int grid = c->sm_count * c->knnp_occ;
+        const int cap_grid = (n_atoms + MG_WARPS) / MG_WARPS;
+        if (grid > cap_grid) grid = cap_grid;
+        A.n_warps = grid * MG_WARPS;
+        mg_knn_pairs_kernel<<<grid, MG_BLOCK, MG_WARPS * sizeof(KnnSmem), st>>>(A);
+        MG_CUDA(cudaGetLastError());
+        c->launches += 1;
+        return MG_OK;
+    }
     if (n_struct > 0) {
         rs = launch_prep(c, pos, lat, sp, n_struct, n_atoms, 0.f, st);
         if (rs != MG_OK) return rs;
@@ -342,8 +372,9 @@ extern "C" mg_status mg_graph_create(mg_ctx *c, int kind, float r_c, int32_t k, 
     g->ctx = c; g->kind = kind; g->r_c = r_c; g->k = k;
     g->struct_ptr = sp; g->n_struct = n_struct; g->n_atoms = n_atoms;
     if (kind == MG_KIND_KNN && n_atoms > 0) {
-        if (cudaMalloc(&g->d_hint, (size_t)n_atoms * sizeof(float)) != cudaSuccess ||
-            cudaMemset(g->d_hint, 0, (size_t)n_atoms * sizeof(float)) != cudaSuccess) {
+        const size_t nh = (size_t)(n_atoms > n_struct ? n_atoms : n_struct) + 1;   // per atom (k > 32) or per structure
+        if (cudaMalloc(&g->d_hint, nh * sizeof(float)) != cudaSuccess ||
+            cudaMemset(g->d_hint, 0, nh * sizeof(float)) != cudaSuccess) {
             cudaGetLastError();
             cudaFree(g->d_hint);
             delete g;
