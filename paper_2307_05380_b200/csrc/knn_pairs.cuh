@@ -199,6 +199,7 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                 // every image with true d2 < R^2 - win is a hit; a k-th key below R^2 - 2 win is safe
                 const float win = 1.1920929e-7f * (2.f * rad * (13.f * R->qmax + 2.f * R->amax_sum) + 4.f * rad * rad);
                 const float lim2 = __fmaf_rn(-2.f, win, __fmul_rn(rad, rad));
+                const double lim2d = (double)rad * (double)rad - (double)win;
                 // rows per group: expected hits fit the stash
                 const int rpt = max(1, min(MG_SMALL_MAX_ATOMS, (int)((float)MG_KSTASH / (2.2f * MG_KNN_ALPHA * (float)K + 8.f))));
                 float dkmax = 0.f;
@@ -222,6 +223,42 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                         if (ok) {
                             const int b0 = ks.rowoff[r], cnt = ks.rowoff[r + 1] - b0;
                             ok = cnt >= K;
+                            if (ok && cnt <= 32) {
+                                // fast path: one hit per lane, exact FP64 distance of every hit, rank by
+                                // counting in the order (d, dst, tau): the oracle's selection itself
+                                const unsigned tie = lane < cnt ? (unsigned)ks.stash[b0 + lane] : 0xFFFFFFFFu;
+                                const int j = (int)(tie & 0xFFu);
+                                const int t0 = (int)(tie >> 24) - 128, t1 = (int)((tie >> 16) & 0xFFu) - 128,
+                                          t2 = (int)((tie >> 8) & 0xFFu) - 128;
+                                const unsigned ord = ((unsigned)j << 24) | (tie >> 8);
+                                double dd = 1e300, vv[3] = {0.0, 0.0, 0.0};
+                                if (lane < cnt)
+                                    dd = mg_exact_vec(A.pos + 3 * (size_t)gi, A.pos + 3 * (size_t)(k.first + j), t0, t1, t2,
+                                                      F.lat, vv);
+                                int rank = 0;
+                                for (int l = 0; l < cnt; ++l) {
+                                    const double od = __shfl_sync(0xFFFFFFFFu, dd, l);
+                                    const unsigned oo = __shfl_sync(0xFFFFFFFFu, ord, l);
+                                    rank += (od < dd || (od == dd && oo < ord)) ? 1 : 0;
+                                }
+                                // Alg. 1 line 4: the k-th image must be safely inside the explored radius
+                                const bool settled = rank != K - 1 || dd * dd < lim2d;
+                                if (__all_sync(0xFFFFFFFFu, settled)) {
+                                    if (rank < K) {
+                                        const long long e = (long long)K * gi + rank;
+                                        A.src[e] = gi;
+                                        A.dst[e] = k.first + j;
+                                        A.offset[3 * e] = (int8_t)t0; A.offset[3 * e + 1] = (int8_t)t1;
+                                        A.offset[3 * e + 2] = (int8_t)t2;
+                                        A.vec[3 * e] = (float)vv[0]; A.vec[3 * e + 1] = (float)vv[1];
+                                        A.vec[3 * e + 2] = (float)vv[2];
+                                        if (A.dist) A.dist[e] = (float)dd;
+                                        if (rank == K - 1) dkmax = fmaxf(dkmax, __double2float_ru(dd));
+                                    }
+                                    continue;
+                                }
+                                ok = false;
+                            }
                             if (ok) {
                                 key = mg_sort32(lane < cnt ? ks.stash[b0 + lane] : MG_KEY_INF, lane);
                                 for (int c = 32; c < cnt; c += 32) {
