@@ -81,7 +81,8 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
             if (A.hint) A.hint[s] = 0.f;
         }
         r.radius = rc;
-        if (N > MG_SMALL_MAX_ATOMS) err |= MGS_UNSUPPORTED;
+        if (N > MG_SMALL_MAX_ATOMS && A.k > 0) err |= MGS_UNSUPPORTED;   // KNN: small structures only
+        if (N > 46000) err |= MGS_UNSUPPORTED;                            // pair indices are 32 bit
         r.mloc = 0;
         r.m = 0;
         r.amax_sum = 0.f;
@@ -115,14 +116,14 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
             const float percell = mloc > 256 ? 11.f + 900.f / (float)N : (mloc > 128 ? 19.f : 11.f);
             const float perblock = mloc > 256 ? 120.f + 16000.f / (float)N : (mloc > 128 ? 500.f : 250.f);
             const float c = ((float)((mloc + 3) & ~3) * percell + perblock) * (1.f / 32.f) + 3.3f * lam / (float)N +
-                            MG_STRUCT_COST / (float)(N * N);
+                            MG_STRUCT_COST / ((float)N * (float)N);
             // KNN: one launch, no edge stream; selecting k per row costs about 350
             const float ck = ((float)((mloc + 3) & ~3) * 11.f + 150.f) * (1.f / 32.f) + 350.f / (float)N +
-                             0.5f * MG_STRUCT_COST / (float)(N * N);
+                             0.5f * MG_STRUCT_COST / ((float)N * (float)N);
             r.paircost = (unsigned)fminf(16.f * (A.k > 0 ? ck : c) + 1.f, 16777216.f);
         }
         r.pad = 0;
-        cost = (unsigned long long)(N * N) * r.paircost;      // N <= 64
+        cost = (unsigned long long)((long long)N * N) * r.paircost;
     }
     // ---- block-wide exclusive scan of the cost
     unsigned long long incl = cost;

@@ -89,6 +89,30 @@ __device__ __forceinline__ int mg_fdiv(int q, float inv_n) {
     return __float2int_rz(__fmul_rn((float)q + 0.5f, inv_n));
 }
 
+// Pair index q -> (i, j), q = i N + j.
+__device__ __forceinline__ void mg_qsplit(int q, int N, float inv_N, int &i, int &j) {
+    i = N <= 1024 ? mg_fdiv(q, inv_N) : q / N;
+    j = q - i * N;
+}
+
+// Wrapped fractional coordinates of one atom: x - floor(x), integer parts packed in .w (10 bits per
+// axis, biased by 512); .w = 0 marks a non-finite or far-away coordinate.
+__device__ __forceinline__ float4 mg_wrap_x(const float *xp) {
+    const float x0 = xp[0], x1 = xp[1], x2 = xp[2];
+    const float g0 = floorf(x0), g1 = floorf(x1), g2 = floorf(x2);
+    const bool ok = fabsf(g0) <= 500.f && fabsf(g1) <= 500.f && fabsf(g2) <= 500.f;   // false for NaN / inf
+    const int kk = ((int)g0 + 512) | (((int)g1 + 512) << 10) | (((int)g2 + 512) << 20);
+    return make_float4(x0 - g0, x1 - g1, x2 - g2, __int_as_float(ok ? kk : 0));
+}
+
+// FP64 cartesian position x . L of atom idx (from the staged copy, or evaluated on the fly).
+__device__ __forceinline__ void mg_pd_big(const float *gx, const double Ld[9], int idx, double out[3]) {
+    const double d0 = (double)gx[3 * idx], d1 = (double)gx[3 * idx + 1], d2 = (double)gx[3 * idx + 2];
+    out[0] = fma(d2, Ld[6], fma(d1, Ld[3], d0 * Ld[0]));
+    out[1] = fma(d2, Ld[7], fma(d1, Ld[4], d0 * Ld[1]));
+    out[2] = fma(d2, Ld[8], fma(d1, Ld[5], d0 * Ld[2]));
+}
+
 // Write one edge: vec = (p_j - p_i) + tau . L in FP64, rounded once (R24).
 // b0, b1, b2 = tau + 128.
 __device__ __forceinline__ void mg_emit_edge(const CutoffArgs &A, long long e, int gi, int gj,
@@ -122,10 +146,9 @@ __device__ __forceinline__ bool mg_warp_stage(WarpSmem &sw, double (*pd)[3], con
     for (int j = lane; j < k.natoms; j += 32) {
         const float *xp = pos + 3 * (size_t)(k.first + j);
         const float x0 = xp[0], x1 = xp[1], x2 = xp[2];
-        const float g0 = floorf(x0), g1 = floorf(x1), g2 = floorf(x2);
-        ok = ok && fabsf(g0) <= 500.f && fabsf(g1) <= 500.f && fabsf(g2) <= 500.f;   // false for NaN / inf
-        const int kk = ((int)g0 + 512) | (((int)g1 + 512) << 10) | (((int)g2 + 512) << 20);
-        sw.x[j] = make_float4(x0 - g0, x1 - g1, x2 - g2, __int_as_float(ok ? kk : 0));
+        const float4 xw = mg_wrap_x(xp);
+        ok = ok && __float_as_int(xw.w) != 0;
+        sw.x[j] = xw;
         if (pd) {
             const double d0 = (double)x0, d1 = (double)x1, d2 = (double)x2;
             pd[j][0] = fma(d2, (double)__ldg(L + 6), fma(d1, (double)__ldg(L + 3), d0 * (double)__ldg(L + 0)));
@@ -171,6 +194,8 @@ struct FindCtx {
     const float *lat;      // the same, global
     const float *pos;      // positions of the batch (exact predicate)
     float rc;              // radius of the predicate d < rc
+    const float *gx;       // positions of the structure's first atom
+    bool big;              // more than MG_SMALL_MAX_ATOMS atoms: positions are read from global memory
     float rho[3];
     int m;                 // m_0 | m_1 << 8 | m_2 << 16
     int mloc;
@@ -238,7 +263,7 @@ struct PairLane {
 __device__ __forceinline__ PairLane mg_pair_setup(const WarpSmem &sw, const FindCtx &F, bool valid, int i, int j) {
     PairLane p;
     const int m0 = F.m & 0xFF, m1 = (F.m >> 8) & 0xFF, m2 = (F.m >> 16) & 0xFF;
-    const float4 xi = sw.x[i], xj = sw.x[j];
+    const float4 xi = F.big ? mg_wrap_x(F.gx + 3 * i) : sw.x[i], xj = F.big ? mg_wrap_x(F.gx + 3 * j) : sw.x[j];
     const float u0 = __fsub_rn(xj.x, xi.x), u1 = __fsub_rn(xj.y, xi.y), u2 = __fsub_rn(xj.z, xi.z);
     const float e0 = floorf(__fsub_rn(-F.rho[0], u0)) + 1.f, e1 = floorf(__fsub_rn(-F.rho[1], u1)) + 1.f,
                 e2 = floorf(__fsub_rn(-F.rho[2], u2)) + 1.f;
@@ -250,7 +275,7 @@ __device__ __forceinline__ PairLane mg_pair_setup(const WarpSmem &sw, const Find
     p.l0 = (int)e0 + (ki & 1023) - (kj & 1023);
     p.l1 = (int)e1 + ((ki >> 10) & 1023) - ((kj >> 10) & 1023);
     p.l2 = (int)e2 + ((ki >> 20) & 1023) - ((kj >> 20) & 1023);
-    p.ok = valid && p.l0 >= -127 && p.l1 >= -127 && p.l2 >= -127 && p.l0 + m0 <= 128 && p.l1 + m1 <= 128 &&
+    p.ok = valid && ki != 0 && kj != 0 && p.l0 >= -127 && p.l1 >= -127 && p.l2 >= -127 && p.l0 + m0 <= 128 && p.l1 + m1 <= 128 &&
            p.l2 + m2 <= 128;
     if (!p.ok) { p.qx = 1e18f; p.qy = 1e18f; p.qz = 1e18f; }
     p.self = i == j ? (-(int)e0 * m1 - (int)e1) * m2 - (int)e2 : -1;   // (i,i,0) is not an edge (R3)
@@ -292,7 +317,9 @@ __device__ __forceinline__ bool mg_struct_setup(WarpSmem &sw, double (*pd)[3], c
     // and q' + T are below 3 Q, about 13 roundings of 2^-24 relative size reach v (the wrapped
     // coordinates are below 1, their difference is rounded once), d2 = v . v adds 3 more
     F.win = 1.1920929e-7f * (2.f * rc * (13.f * R->qmax + 2.f * R->amax_sum) + 4.f * rc * rc);
-    if (!mg_warp_stage(sw, pd, pos, lattice, k, lane)) {
+    F.gx = pos + 3 * (size_t)k.first;
+    F.big = k.natoms > MG_SMALL_MAX_ATOMS;
+    if (!F.big && !mg_warp_stage(sw, pd, pos, lattice, k, lane)) {
         if (lane == 0) atomicOr(status, MGS_NONFINITE);
         F.mloc = 0;
         return false;
@@ -365,7 +392,8 @@ __device__ __forceinline__ unsigned mg_count_segment(const WarpSmem &sw, const C
     for (int q0 = qa; q0 < qb; q0 += 32) {
         const int q = q0 + lane;
         const bool valid = q < qb;
-        const int i = valid ? mg_fdiv(q, inv_N) : 0, j = valid ? q - i * N : 0;
+        int i = 0, j = 0;
+        if (valid) mg_qsplit(q, N, inv_N, i, j);
         const PairLane p = mg_pair_setup(sw, F, valid, i, j);
         if (valid && !p.ok) atomicOr(A.status, MGS_OFFSET);
         unsigned mask[W];
@@ -483,6 +511,8 @@ struct EmitCtx {
     double Ld[9];
     long long goff;        // global index of the first edge in the stash
     int run, qb0;          // stash fill, first pair of the stash's batch
+    const float *gx;       // positions of the structure's first atom
+    bool big;              // positions are not staged: FP64 cartesian positions on the fly
 };
 
 // Lanes <-> pairs: every lane writes its own hits of one block straight to global memory,
@@ -500,9 +530,18 @@ __device__ __forceinline__ void mg_direct_block(const WarpSmem &sw, const double
             const int b = __ffs(mk) - 1;
             mk &= mk - 1;
             const unsigned code = paircode + sw.tcode[32 * w + b];
-            if (pos < A.capacity)
-                mg_emit_edge(A, pos, k.first + i, k.first + j, pd[i], pd[j], E.Ld, code >> 24, (code >> 16) & 0xFFu,
-                             (code >> 8) & 0xFFu);
+            if (pos < A.capacity) {
+                if (E.big) {
+                    double pi[3], pj[3];
+                    mg_pd_big(E.gx, E.Ld, i, pi);
+                    mg_pd_big(E.gx, E.Ld, j, pj);
+                    mg_emit_edge(A, pos, k.first + i, k.first + j, pi, pj, E.Ld, code >> 24, (code >> 16) & 0xFFu,
+                                 (code >> 8) & 0xFFu);
+                } else {
+                    mg_emit_edge(A, pos, k.first + i, k.first + j, pd[i], pd[j], E.Ld, code >> 24,
+                                 (code >> 16) & 0xFFu, (code >> 8) & 0xFFu);
+                }
+            }
             ++pos;
         }
     }
@@ -524,8 +563,16 @@ __device__ __forceinline__ void mg_flush(const EmitSmem &se, const CutoffArgs &A
     for (int e = lane; e < lim; e += 32) {
         const unsigned code = se.stash[e];
         const int q = qb0 + (int)(code & 0xFFu);
-        const int i = mg_fdiv(q, inv_N), j = q - i * N;
+        int i, j;
+        mg_qsplit(q, N, inv_N, i, j);
+        double pib[3], pjb[3];
         const double *pi = se.pd[i], *pj = se.pd[j];
+        if (E.big) {
+            mg_pd_big(E.gx, E.Ld, i, pib);
+            mg_pd_big(E.gx, E.Ld, j, pjb);
+            pi = pib;
+            pj = pjb;
+        }
         // (double)(b - 128) without a conversion instruction: 2^52 + b has b in its low mantissa word
         const double t0 = __hiloint2double(0x43300000, (int)(code >> 24)) - 4503599627370624.0;
         const double t1 = __hiloint2double(0x43300000, (int)((code >> 16) & 0xFFu)) - 4503599627370624.0;
@@ -558,7 +605,8 @@ __device__ __forceinline__ void mg_emit_blocks(EmitSmem &se, const CutoffArgs &A
     for (int q0 = qa; q0 < qb; q0 += 32) {
         const int q = q0 + lane;
         const bool valid = q < qb;
-        const int i = valid ? mg_fdiv(q, inv_N) : 0, j = valid ? q - i * N : 0;
+        int i = 0, j = 0;
+        if (valid) mg_qsplit(q, N, inv_N, i, j);
         const PairLane p = mg_pair_setup(sw, F, valid, i, j);
         unsigned mask[W];
         if (scratch && midx + 32 * W <= MG_MASK_WORDS) {
@@ -673,6 +721,8 @@ mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
                     for (int c = 0; c < 9; ++c) E.Ld[c] = (double)F.a[c];
                     E.run = 0;
                     E.qb0 = qa;
+                    E.gx = F.gx;
+                    E.big = F.big;
                     if (F.mloc <= 32) mg_emit_blocks<1>(se, A, k, F, E, qa, qb, 0, F.mloc, true, false, wmask, midx, lane);
                     else if (F.mloc <= 64) mg_emit_blocks<2>(se, A, k, F, E, qa, qb, 0, F.mloc, true, false, wmask, midx, lane);
                     else if (F.mloc <= 128) mg_emit_blocks<4>(se, A, k, F, E, qa, qb, 0, F.mloc, true, false, wmask, midx, lane);

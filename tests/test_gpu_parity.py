@@ -82,6 +82,33 @@ def test_config2_knn_full(mg, ctx, batch2):
     assert rep["exact_rows"] >= 0.999 * batch2.n_atoms, rep
 
 
+def test_config3_cutoff_supercells(mg, ctx):
+    # 16 cells of 500-2000 atoms, r_c = 8 A: plane spacings > 2 r_c, so every ordered pair has a
+    # single candidate image (the minimum-image limit of the per-pair sub-box)
+    b = C.config_batch(3)
+    assert b.n_struct == 16 and 500 <= np.diff(b.struct_ptr).min() and np.diff(b.struct_ptr).max() <= 2000
+    got, status = _cutoff(mg, ctx, b, 8.0)
+    assert status == 0
+    rep = check.check_cutoff(b, 8.0, got)
+    assert rep["extra"] == 0 and rep["missing"] == 0, rep
+    assert rep["n_edges"] == rep["n_ref"] > 1_000_000
+
+
+def test_mixed_small_and_large_structures(mg, ctx):
+    # structures above and below the shared-memory staging limit in one batch, dense enough that
+    # the large one has several images per pair
+    small = C.small_batch(12, seed=21)
+    rng = np.random.default_rng(7)
+    cell = (np.diag([9.0, 10.0, 11.0]) + rng.uniform(-1, 1, (3, 3))).astype(np.float32)
+    big = C.Batch(pos=rng.random((150, 3), dtype=np.float32), lattice=cell[None],
+                  struct_ptr=np.array([0, 150], np.int32))
+    b = C.concat([small, big, small])
+    got, status = _cutoff(mg, ctx, b, 6.5)
+    assert status == 0
+    rep = check.check_cutoff(b, 6.5, got)
+    assert rep["extra"] == 0 and rep["missing"] == 0, rep
+
+
 def test_config4_update_steps(mg, ctx):
     import torch
     k = 24
