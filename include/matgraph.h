@@ -130,6 +130,15 @@ mg_status mg_check(mg_ctx *ctx, void *cuda_stream);
 /* Number of kernels this library launched on behalf of ctx since mg_create (bench bookkeeping). */
 int64_t mg_launch_count(const mg_ctx *ctx);
 
+/* Profiling aid.  mg_set_profile(ctx, 1): every following mg_cutoff_graph / mg_knn_graph /
+ * mg_update_graph call brackets its kernels with CUDA events on the caller's stream (a few event
+ * records per call; off by default).  mg_profile_read SYNCHRONISES on the last recorded event and
+ * returns the mean duration in milliseconds of [0] the search-bounds kernel (K1), [1] the cutoff
+ * count kernel, [2] the cutoff emit kernel, [3] the KNN kernel over the calls made since
+ * mg_set_profile, and how many calls each mean covers (count4 may be NULL). */
+mg_status mg_set_profile(mg_ctx *ctx, int on);
+mg_status mg_profile_read(mg_ctx *ctx, double *mean_ms4, int64_t *count4);
+
 const char *mg_status_string(mg_status status);
 
 #ifdef __cplusplus

@@ -22,7 +22,7 @@ MG_MAX_K = 64
 EXPORTS = ["mg_create", "mg_destroy", "mg_reserve", "mg_cutoff_graph", "mg_cutoff_count",
            "mg_knn_graph", "mg_graph_create", "mg_graph_destroy", "mg_update_graph",
            "mg_cutoff_graph_host", "mg_knn_graph_host", "mg_check", "mg_launch_count",
-           "mg_status_string"]
+           "mg_status_string", "mg_set_profile", "mg_profile_read"]
 
 
 class MatGraphError(RuntimeError):
@@ -64,6 +64,8 @@ def _lib():
         lib.mg_check.argtypes = [vp, vp]
         lib.mg_launch_count.argtypes = [vp]
         lib.mg_launch_count.restype = i64
+        lib.mg_set_profile.argtypes = [vp, ctypes.c_int]
+        lib.mg_profile_read.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(i64)]
         lib.mg_status_string.argtypes = [ctypes.c_int]
         lib.mg_status_string.restype = ctypes.c_char_p
         _LIBH = lib
@@ -234,6 +236,21 @@ class Context:
 
     def mg_launch_count(self) -> int:
         return int(_lib().mg_launch_count(self._h))
+
+    def mg_set_profile(self, on: bool):
+        rc = _lib().mg_set_profile(self._h, 1 if on else 0)
+        if rc != 0:
+            raise MatGraphError(rc, "mg_set_profile")
+
+    def mg_profile_read(self) -> dict:
+        """Mean kernel durations (ms) since mg_set_profile(True): prep, count, emit, knn."""
+        ms = (ctypes.c_double * 4)()
+        n = (ctypes.c_int64 * 4)()
+        rc = _lib().mg_profile_read(self._h, ms, n)
+        if rc != 0:
+            raise MatGraphError(rc, "mg_profile_read")
+        names = ("prep", "count", "emit", "knn")
+        return {k: dict(ms=float(ms[i]), calls=int(n[i])) for i, k in enumerate(names)}
 
     # ---- host-buffer calls (numpy in, numpy out; copies inside the call) ----------------
     def _host(self, fn, pos, lattice, struct_ptr, param, capacity, dist):

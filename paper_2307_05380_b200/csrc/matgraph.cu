@@ -40,6 +40,11 @@ struct mg_ctx {
     unsigned epoch = 0;
     int cutoff_occ = 0, count_occ = 0, knn_occ[2] = {0, 0}, knnp_occ = 0;
     int64_t launches = 0;
+    int profile = 0;                      // mg_set_profile: events around the kernels of the next calls
+    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
+    double prof_ms[4] = {0, 0, 0, 0};     // accumulated: prep, count, emit, knn
+    int64_t prof_n[4] = {0, 0, 0, 0};
+    int pend_kind = -1;                   // events of the last call not read yet: 0 cutoff, 1 knn
     // device mirrors for the _host entry points
     void *h_dev[9] = {nullptr};
     size_t h_cap[9] = {0};
@@ -138,6 +143,7 @@ extern "C" void mg_destroy(mg_ctx *c) {
     cudaFree(c->d_rowptr_tmp);
     cudaFree(c->d_count);
     for (int i = 0; i < 9; ++i) cudaFree(c->h_dev[i]);
+    for (int i = 0; i < 5; ++i) if (c->ev[i]) cudaEventDestroy(c->ev[i]);
     delete c;
 }
 
@@ -206,6 +212,46 @@ static bool bad_edges(const mg_edges *o, long long need) {
     return o->capacity < need;
 }
 
+// Profiling aid: with mg_set_profile(ctx, 1) every graph call brackets its kernels with CUDA events on
+// the caller's stream; the durations are collected at the next call (or mg_profile_read).
+static void prof_collect(mg_ctx *c) {
+    if (c->pend_kind < 0) return;
+    if (cudaEventSynchronize(c->ev[3]) == cudaSuccess) {
+        float ms = 0.f;
+        if (c->pend_kind == 0) {
+            for (int i = 0; i < 3; ++i)
+                if (cudaEventElapsedTime(&ms, c->ev[i], c->ev[i + 1]) == cudaSuccess) { c->prof_ms[i] += ms; c->prof_n[i] += 1; }
+        } else {
+            if (cudaEventElapsedTime(&ms, c->ev[0], c->ev[1]) == cudaSuccess) { c->prof_ms[0] += ms; c->prof_n[0] += 1; }
+            if (cudaEventElapsedTime(&ms, c->ev[1], c->ev[3]) == cudaSuccess) { c->prof_ms[3] += ms; c->prof_n[3] += 1; }
+        }
+    }
+    cudaGetLastError();
+    c->pend_kind = -1;
+}
+
+extern "C" mg_status mg_set_profile(mg_ctx *c, int on) {
+    if (!c) return MG_ERR_INVALID_ARG;
+    MG_CUDA(cudaSetDevice(c->device));
+    prof_collect(c);
+    if (on && !c->ev[0])
+        for (int i = 0; i < 5; ++i) MG_CUDA(cudaEventCreate(&c->ev[i]));
+    c->profile = on ? 1 : 0;
+    for (int i = 0; i < 4; ++i) { c->prof_ms[i] = 0; c->prof_n[i] = 0; }
+    return MG_OK;
+}
+
+extern "C" mg_status mg_profile_read(mg_ctx *c, double *mean_ms4, int64_t *count4) {
+    if (!c || !mean_ms4) return MG_ERR_INVALID_ARG;
+    MG_CUDA(cudaSetDevice(c->device));
+    prof_collect(c);
+    for (int i = 0; i < 4; ++i) {
+        mean_ms4[i] = c->prof_n[i] ? c->prof_ms[i] / (double)c->prof_n[i] : 0.0;
+        if (count4) count4[i] = c->prof_n[i];
+    }
+    return MG_OK;
+}
+
 static mg_status launch_prep(mg_ctx *c, const float *pos, const float *lat, const int32_t *sp,
                              int32_t n_struct, int32_t n_atoms, float r_c, cudaStream_t st) {
     PrepArgs P;
@@ -230,6 +276,8 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
         return MG_OK;
     }
     const int n_blocks = (n_struct + MG_CP_BLOCK - 1) / MG_CP_BLOCK;
+    const bool prof = c->profile && !count_only;
+    if (prof) { prof_collect(c); cudaEventRecord(c->ev[0], st); }
     {
         CutPrepArgs P;
         P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms; P.r_c = r_c;
@@ -255,14 +303,17 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
     A.n_warps = grid * MG_WARPS;
     A.n_ranges = MG_OVER * A.n_warps;
     c->last_cut_warps = A.n_warps;
+    if (prof) cudaEventRecord(c->ev[1], st);
     mg_cutoff_count_kernel<<<grid, MG_BLOCK, 0, st>>>(A);
     MG_CUDA(cudaGetLastError());
     c->launches += 1;
+    if (prof) cudaEventRecord(c->ev[2], st);
     if (!count_only) {
         mg_cutoff_emit_kernel<<<grid, MG_BLOCK, MG_WARPS * sizeof(EmitSmem), st>>>(A);
         MG_CUDA(cudaGetLastError());
         c->launches += 1;
     }
+    if (prof) { cudaEventRecord(c->ev[3], st); c->pend_kind = 0; }
     return MG_OK;
 }
 
@@ -302,6 +353,7 @@ static mg_status launch_knn(mg_ctx *c, const float *pos, const float *lat, const
     if (rs != MG_OK) return rs;
     if (k <= 32 && n_struct > 0) {                      // pair-lane kernel (knn_pairs.cuh)
         const int n_blocks = (n_struct + MG_CP_BLOCK - 1) / MG_CP_BLOCK;
+        if (c->profile) { prof_collect(c); cudaEventRecord(c->ev[0], st); }
         CutPrepArgs P;
         P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms; P.r_c = 0.f;
         P.k = k; P.hint = hint; P.use_hint = use_hint;
@@ -320,9 +372,11 @@ static mg_status launch_knn(mg_ctx *c, const float *pos, const float *lat, const
         const int cap_grid = (n_atoms + MG_WARPS) / MG_WARPS;
         if (grid > cap_grid) grid = cap_grid;
         A.n_warps = grid * MG_WARPS;
+        if (c->profile) cudaEventRecord(c->ev[1], st);
         mg_knn_pairs_kernel<<<grid, MG_BLOCK, MG_WARPS * sizeof(KnnSmem), st>>>(A);
         MG_CUDA(cudaGetLastError());
         c->launches += 1;
+        if (c->profile) { cudaEventRecord(c->ev[3], st); c->pend_kind = 1; }
         return MG_OK;
     }
     if (n_struct > 0) {
