@@ -374,8 +374,9 @@ __device__ __forceinline__ bool mg_segment(const RangeCtx &A, const CutRec *R, i
     const unsigned pc = R->paircost;
     const int NN = R->natoms * R->natoms;
     if (cs + (unsigned long long)qa * pc >= c1) return false;
-    const unsigned long long room = c1 == ~0ull ? ~0ull : (c1 - cs + pc - 1) / pc;   // pairs that start before c1
-    qb = (int)min((unsigned long long)NN, room);
+    // pairs that start before c1: ceil((c1 - cs) / pc), at most NN
+    if (c1 == ~0ull || c1 - cs >= (unsigned long long)NN * pc) { qb = NN; return true; }
+    qb = (int)((c1 - cs + pc - 1) / pc);
     return true;
 }
 
@@ -513,7 +514,17 @@ struct EmitCtx {
     int run, qb0;          // stash fill, first pair of the stash's batch
     const float *gx;       // positions of the structure's first atom
     bool big;              // positions are not staged: FP64 cartesian positions on the fly
+#ifdef MG_PHASE_CLOCKS
+    long long tc[4];       // cycles: pair setup + masks + scan, extraction, flush, structure setup
+#endif
 };
+#ifdef MG_PHASE_CLOCKS
+#define MG_TIC const long long tic_ = clock64();
+#define MG_TOC(i) E.tc[i] += clock64() - tic_;
+#else
+#define MG_TIC
+#define MG_TOC(i)
+#endif
 
 // Lanes <-> pairs: every lane writes its own hits of one block straight to global memory,
 // starting at edge index pos (slow path: blocks that do not fit the stash, tiled structures).
@@ -560,34 +571,40 @@ __device__ __forceinline__ void mg_flush(const EmitSmem &se, const CutoffArgs &A
     int8_t *poff = A.offset + 3 * E.goff;
     float *pvec = A.vec + 3 * E.goff;
     float *pdist = A.dist ? A.dist + E.goff : nullptr;
-    for (int e = lane; e < lim; e += 32) {
-        const unsigned code = se.stash[e];
-        const int q = qb0 + (int)(code & 0xFFu);
-        int i, j;
-        mg_qsplit(q, N, inv_N, i, j);
-        double pib[3], pjb[3];
-        const double *pi = se.pd[i], *pj = se.pd[j];
-        if (E.big) {
-            mg_pd_big(E.gx, E.Ld, i, pib);
-            mg_pd_big(E.gx, E.Ld, j, pjb);
-            pi = pib;
-            pj = pjb;
+    // two edges per lane and iteration: two independent load -> FP64 -> store chains in flight
+    for (int e0 = lane; e0 < lim; e0 += 32) {
+#pragma unroll
+        for (int h = 0; h < 1; ++h) {
+            const int e = e0 + 32 * h;
+            if (e >= lim) break;
+            const unsigned code = se.stash[e];
+            const int q = qb0 + (int)(code & 0xFFu);
+            int i, j;
+            mg_qsplit(q, N, inv_N, i, j);
+            double pib[3], pjb[3];
+            const double *pi = se.pd[i], *pj = se.pd[j];
+            if (E.big) {
+                mg_pd_big(E.gx, E.Ld, i, pib);
+                mg_pd_big(E.gx, E.Ld, j, pjb);
+                pi = pib;
+                pj = pjb;
+            }
+            // (double)(b - 128) without a conversion instruction: 2^52 + b has b in its low mantissa word
+            const double t0 = __hiloint2double(0x43300000, (int)(code >> 24)) - 4503599627370624.0;
+            const double t1 = __hiloint2double(0x43300000, (int)((code >> 16) & 0xFFu)) - 4503599627370624.0;
+            const double t2 = __hiloint2double(0x43300000, (int)((code >> 8) & 0xFFu)) - 4503599627370624.0;
+            const double v0 = fma(t2, E.Ld[6], fma(t1, E.Ld[3], fma(t0, E.Ld[0], pj[0] - pi[0])));
+            const double v1 = fma(t2, E.Ld[7], fma(t1, E.Ld[4], fma(t0, E.Ld[1], pj[1] - pi[1])));
+            const double v2 = fma(t2, E.Ld[8], fma(t1, E.Ld[5], fma(t0, E.Ld[2], pj[2] - pi[2])));
+            const unsigned tb = code ^ 0x80808000u;              // tau bytes as int8
+            psrc[e] = k.first + i;
+            pdst[e] = k.first + j;
+            int8_t *po = poff + 3 * e;
+            po[0] = (int8_t)(tb >> 24); po[1] = (int8_t)(tb >> 16); po[2] = (int8_t)(tb >> 8);
+            float *pv = pvec + 3 * e;
+            pv[0] = (float)v0; pv[1] = (float)v1; pv[2] = (float)v2;
+            if (pdist) pdist[e] = __fsqrt_rn((float)fma(v2, v2, fma(v1, v1, v0 * v0)));
         }
-        // (double)(b - 128) without a conversion instruction: 2^52 + b has b in its low mantissa word
-        const double t0 = __hiloint2double(0x43300000, (int)(code >> 24)) - 4503599627370624.0;
-        const double t1 = __hiloint2double(0x43300000, (int)((code >> 16) & 0xFFu)) - 4503599627370624.0;
-        const double t2 = __hiloint2double(0x43300000, (int)((code >> 8) & 0xFFu)) - 4503599627370624.0;
-        const double v0 = fma(t2, E.Ld[6], fma(t1, E.Ld[3], fma(t0, E.Ld[0], pj[0] - pi[0])));
-        const double v1 = fma(t2, E.Ld[7], fma(t1, E.Ld[4], fma(t0, E.Ld[1], pj[1] - pi[1])));
-        const double v2 = fma(t2, E.Ld[8], fma(t1, E.Ld[5], fma(t0, E.Ld[2], pj[2] - pi[2])));
-        const unsigned tb = code ^ 0x80808000u;              // tau bytes as int8
-        psrc[e] = k.first + i;
-        pdst[e] = k.first + j;
-        int8_t *po = poff + 3 * e;
-        po[0] = (int8_t)(tb >> 24); po[1] = (int8_t)(tb >> 16); po[2] = (int8_t)(tb >> 8);
-        float *pv = pvec + 3 * e;
-        pv[0] = (float)v0; pv[1] = (float)v1; pv[2] = (float)v2;
-        if (pdist) pdist[e] = __fsqrt_rn((float)fma(v2, v2, fma(v1, v1, v0 * v0)));
     }
 }
 
@@ -602,20 +619,33 @@ __device__ __forceinline__ void mg_emit_blocks(EmitSmem &se, const CutoffArgs &A
     const WarpSmem &sw = se.w;
     const int N = k.natoms;
     const float inv_N = 1.f / (float)N;
+    unsigned nmask[W];                       // masks of the next block, loaded one block ahead
+    bool nhave = scratch && qa < qb && midx + 32 * W <= MG_MASK_WORDS;
+#pragma unroll
+    for (int w = 0; w < W; ++w) nmask[w] = nhave ? __ldg(wmask + midx + 32 * w + lane) : 0u;
     for (int q0 = qa; q0 < qb; q0 += 32) {
         const int q = q0 + lane;
         const bool valid = q < qb;
         int i = 0, j = 0;
+        long long t0_ = 0;
+#ifdef MG_PHASE_CLOCKS
+        t0_ = clock64();
+#endif
         if (valid) mg_qsplit(q, N, inv_N, i, j);
         const PairLane p = mg_pair_setup(sw, F, valid, i, j);
         unsigned mask[W];
-        if (scratch && midx + 32 * W <= MG_MASK_WORDS) {
+        if (nhave) {
 #pragma unroll
-            for (int w = 0; w < W; ++w) mask[w] = __ldg(wmask + midx + 32 * w + lane);
+            for (int w = 0; w < W; ++w) mask[w] = nmask[w];
         } else {
             mg_block_masks<W>(sw, F, p, k.first + i, k.first + j, tile0, ncl, mask);
         }
-        if (scratch) midx += 32 * W;
+        if (scratch) {
+            midx += 32 * W;
+            nhave = q0 + 32 < qb && midx + 32 * W <= MG_MASK_WORDS;
+#pragma unroll
+            for (int w = 0; w < W; ++w) nmask[w] = nhave ? __ldg(wmask + midx + 32 * w + lane) : 0u;
+        }
         int cnt = 0;
 #pragma unroll
         for (int w = 0; w < W; ++w) cnt += __popc(mask[w]);
@@ -626,9 +656,13 @@ __device__ __forceinline__ void mg_emit_blocks(EmitSmem &se, const CutoffArgs &A
             if (lane >= o) incl += v;
         }
         const int tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
+#ifdef MG_PHASE_CLOCKS
+        E.tc[0] += clock64() - t0_;
+#endif
+        (void)t0_;
         if (E.run + tot > MG_STASH || (!pinned && q0 + 32 - E.qb0 > 256)) {   // stash full: write it out
             __syncwarp();
-            mg_flush(se, A, k, E, E.run, E.qb0, inv_N, lane);
+            { MG_TIC mg_flush(se, A, k, E, E.run, E.qb0, inv_N, lane); MG_TOC(2) }
             __syncwarp();
             E.goff += E.run;
             E.run = 0;
@@ -644,6 +678,7 @@ __device__ __forceinline__ void mg_emit_blocks(EmitSmem &se, const CutoffArgs &A
         }
         const unsigned paircode = ((unsigned)(p.l0 + 128) << 24) | ((unsigned)(p.l1 + 128) << 16) |
                                   ((unsigned)(p.l2 + 128) << 8) | (unsigned)(q - E.qb0);
+        { MG_TIC
 #pragma unroll
         for (int w = 0; w < W; ++w) {
             unsigned mk = mask[w];
@@ -653,13 +688,14 @@ __device__ __forceinline__ void mg_emit_blocks(EmitSmem &se, const CutoffArgs &A
                 se.stash[pos++] = paircode + sw.tcode[32 * w + b];
             }
         }
+        MG_TOC(1) }
         E.run += tot;
     }
 }
 
 __device__ __forceinline__ void mg_flush_all(EmitSmem &se, const CutoffArgs &A, const Task &k, EmitCtx &E, int lane) {
     __syncwarp();
-    mg_flush(se, A, k, E, E.run, E.qb0, 1.f / (float)k.natoms, lane);
+    { MG_TIC mg_flush(se, A, k, E, E.run, E.qb0, 1.f / (float)k.natoms, lane); MG_TOC(2) }
     __syncwarp();
     E.goff += E.run;
     E.run = 0;
@@ -705,6 +741,9 @@ mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
         const unsigned *wmask = A.wmask + (size_t)w * MG_MASK_WORDS;
         int midx = 0;
         EmitCtx E;
+#ifdef MG_PHASE_CLOCKS
+        E.tc[0] = E.tc[1] = E.tc[2] = E.tc[3] = 0;
+#endif
         E.goff = (long long)__ldg(A.wtotal + w);
         for (; s < A.n_struct; ++s, qa = 0) {
             const CutRec *R = A.rec + s;
@@ -713,7 +752,9 @@ mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
             Task k;
             FindCtx F;
             if (qb > qa) {
-                if (!mg_struct_setup(sw, se.pd, A.pos, A.lattice, A.status, A.r_c, R, s, k, F, lane)) {
+                bool live_;
+                { MG_TIC live_ = mg_struct_setup(sw, se.pd, A.pos, A.lattice, A.status, A.r_c, R, s, k, F, lane); MG_TOC(3) }
+                if (!live_) {
                     const int N = R->natoms;                       // no edges: rows that start in [qa, qb)
                     for (int i = (qa + N - 1) / N + lane; i * N < qb; i += 32) A.row_ptr[R->first + i] = (int)E.goff;
                 } else {
@@ -733,6 +774,9 @@ mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
             }
             if (qb < R->natoms * R->natoms) break;
         }
+#ifdef MG_PHASE_CLOCKS
+        if (lane == 0) for (int x = 0; x < 4; ++x) A.wmask[(size_t)w * MG_MASK_WORDS + MG_MASK_WORDS - 4 + x] = (unsigned)E.tc[x];
+#endif
         w = __shfl_sync(0xFFFFFFFFu, w_next, 0);
     }
     if (lane == 0) A.wclock[A.n_warps + wid] = (unsigned)(clock64() - t_begin);

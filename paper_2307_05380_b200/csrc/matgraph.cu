@@ -196,6 +196,13 @@ extern "C" int mg_debug_cut_warps(mg_ctx *c, unsigned *clocks_host, int *starts_
     return c->last_cut_warps;
 }
 
+extern "C" int mg_debug_cut_masks(mg_ctx *c, unsigned *host, int n_words) {
+    if (!c) return -1;
+    cudaDeviceSynchronize();
+    cudaMemcpy(host, c->d_wmask, (size_t)n_words * 4, cudaMemcpyDeviceToHost);
+    return 0;
+}
+
 extern "C" int64_t mg_launch_count(const mg_ctx *c) { return c ? c->launches : 0; }
 
 static bool bad_inputs(const mg_ctx *c, const float *pos, const float *lat, const int32_t *sp,
