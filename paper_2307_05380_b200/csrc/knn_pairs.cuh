@@ -224,23 +224,49 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                             const int b0 = ks.rowoff[r], cnt = ks.rowoff[r + 1] - b0;
                             ok = cnt >= K;
                             if (ok && cnt <= 32) {
-                                // fast path: one hit per lane, exact FP64 distance of every hit, rank by
-                                // counting in the order (d, dst, tau): the oracle's selection itself
-                                const unsigned tie = lane < cnt ? (unsigned)ks.stash[b0 + lane] : 0xFFFFFFFFu;
+                                // fast path: one hit per lane.  A 32-bit bitonic sort of (FP32 d2 with the lane
+                                // in its low 5 bits) brings the hits in near order; the first k plus every hit
+                                // FP32 cannot tell from the k-th get their exact FP64 distance; if they are
+                                // already in the order (d, dst, tau) the lane is the rank, else rank by counting
+                                const mg_key mine = lane < cnt ? ks.stash[b0 + lane] : MG_KEY_INF;
+                                unsigned sk = lane < cnt ? (((unsigned)(mine >> 32) & ~31u) | (unsigned)lane) : 0xFFFFFFFFu;
+#pragma unroll
+                                for (int k2 = 2; k2 <= 32; k2 <<= 1)
+#pragma unroll
+                                    for (int jj = k2 >> 1; jj > 0; jj >>= 1) {
+                                        const unsigned o = __shfl_xor_sync(0xFFFFFFFFu, sk, jj);
+                                        const bool up = (lane & k2) == 0, lower = (lane & jj) == 0;
+                                        sk = (lower == up) ? min(sk, o) : max(sk, o);
+                                    }
+                                const unsigned tie = __shfl_sync(0xFFFFFFFFu, (unsigned)mine, (int)(sk & 31u));
+                                const float d2q = __uint_as_float(sk & ~31u);
+                                const float d2k = __shfl_sync(0xFFFFFFFFu, d2q, K - 1);
+                                // 2 win: FP32 error of both; 2^-17 d2: the 5 bits given to the lane
+                                const bool sel = lane < cnt && (lane < K || d2q <= __fmaf_rn(d2k, 1.6e-5f, __fmaf_rn(2.f, win, d2k)));
+                                const int nsel = __popc(__ballot_sync(0xFFFFFFFFu, sel));       // sorted: a prefix
                                 const int j = (int)(tie & 0xFFu);
                                 const int t0 = (int)(tie >> 24) - 128, t1 = (int)((tie >> 16) & 0xFFu) - 128,
                                           t2 = (int)((tie >> 8) & 0xFFu) - 128;
                                 const unsigned ord = ((unsigned)j << 24) | (tie >> 8);
                                 double dd = 1e300, vv[3] = {0.0, 0.0, 0.0};
-                                if (lane < cnt)
+                                if (sel)
                                     dd = mg_exact_vec(A.pos + 3 * (size_t)gi, A.pos + 3 * (size_t)(k.first + j), t0, t1, t2,
                                                       F.lat, vv);
-                                int rank = 0;
-                                for (int l = 0; l < cnt; ++l) {
-                                    const double od = __shfl_sync(0xFFFFFFFFu, dd, l);
-                                    const unsigned oo = __shfl_sync(0xFFFFFFFFu, ord, l);
-                                    rank += (od < dd || (od == dd && oo < ord)) ? 1 : 0;
+                                int rank = lane;
+                                {
+                                    const double nd = __shfl_down_sync(0xFFFFFFFFu, dd, 1);
+                                    const unsigned no = __shfl_down_sync(0xFFFFFFFFu, ord, 1);
+                                    const bool inv = lane + 1 < nsel && (nd < dd || (nd == dd && no < ord));
+                                    if (__any_sync(0xFFFFFFFFu, inv)) {
+                                        rank = 0;
+                                        for (int l = 0; l < nsel; ++l) {
+                                            const double od = __shfl_sync(0xFFFFFFFFu, dd, l);
+                                            const unsigned oo = __shfl_sync(0xFFFFFFFFu, ord, l);
+                                            rank += (od < dd || (od == dd && oo < ord)) ? 1 : 0;
+                                        }
+                                    }
                                 }
+                                if (!sel) rank = 64;
                                 // Alg. 1 line 4: the k-th image must be safely inside the explored radius
                                 const bool settled = rank != K - 1 || dd * dd < lim2d;
                                 if (__all_sync(0xFFFFFFFFu, settled)) {
