@@ -411,7 +411,7 @@ __device__ __forceinline__ unsigned mg_count_segment(const WarpSmem &sw, const C
 }
 
 // Structures whose table does not fit (mloc > MG_TLOC): row by row, tile by tile.
-__device__ __noinline__ unsigned mg_count_tiled(WarpSmem &sw, const CutoffArgs &A, const Task &k, const FindCtx &F,
+__device__ __forceinline__ unsigned mg_count_tiled(WarpSmem &sw, const CutoffArgs &A, const Task &k, const FindCtx &F,
                                                 int qa, int qb, int lane) {
     const int N = k.natoms;
     unsigned acc = 0u;
@@ -703,7 +703,7 @@ __device__ __forceinline__ void mg_flush_all(EmitSmem &se, const CutoffArgs &A, 
 
 // Structures whose table does not fit (mloc > MG_TLOC): one source row at a time (its edges may
 // come in any order), tile by tile.
-__device__ __noinline__ void mg_emit_tiled(EmitSmem &se, const CutoffArgs &A, const Task &k, const FindCtx &F,
+__device__ __forceinline__ void mg_emit_tiled(EmitSmem &se, const CutoffArgs &A, const Task &k, const FindCtx &F,
                                            EmitCtx &E, int qa, int qb, int lane) {
     WarpSmem &sw = se.w;
     const int N = k.natoms;
