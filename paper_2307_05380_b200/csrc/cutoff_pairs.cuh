@@ -71,6 +71,7 @@ struct EmitSmem {
     WarpSmem w;
     double pd[MG_SMALL_MAX_ATOMS][3];   // cartesian positions x . L in FP64
     unsigned stash[MG_STASH];
+    unsigned pairij[256];              // (i << 16 | j) of the pairs of the stash's batch
 };
 
 struct Task {
@@ -678,6 +679,7 @@ __device__ __forceinline__ void mg_emit_blocks(EmitSmem &se, const CutoffArgs &A
         }
         const unsigned paircode = ((unsigned)(p.l0 + 128) << 24) | ((unsigned)(p.l1 + 128) << 16) |
                                   ((unsigned)(p.l2 + 128) << 8) | (unsigned)(q - E.qb0);
+        if (valid) se.pairij[q - E.qb0] = ((unsigned)i << 16) | (unsigned)j;
         { MG_TIC
 #pragma unroll
         for (int w = 0; w < W; ++w) {
@@ -709,14 +711,17 @@ __device__ __forceinline__ void mg_emit_tiled(EmitSmem &se, const CutoffArgs &A,
     const int N = k.natoms;
     int dummy = 0;
     for (int i = qa / N; i * N < qb; ++i) {
-        const int ra = max(qa, i * N), rb = min(qb, (i + 1) * N);
-        E.qb0 = ra;
-        for (int tile0 = 0; tile0 < F.mloc; tile0 += MG_TLOC) {
-            mg_warp_table(sw, F.a, (F.m >> 8) & 0xFF, (F.m >> 16) & 0xFF, F.mloc, tile0, lane);
-            mg_emit_blocks<8>(se, A, k, F, E, ra, rb, tile0, min(MG_TLOC, F.mloc - tile0), false, true, nullptr,
-                              dummy, lane);
+        const int ra0 = max(qa, i * N), rb0 = min(qb, (i + 1) * N);
+        for (int ra = ra0; ra < rb0; ra += 256) {                  // pair indices in the stash are 8 bit
+            const int rb = min(rb0, ra + 256);
+            E.qb0 = ra;
+            for (int tile0 = 0; tile0 < F.mloc; tile0 += MG_TLOC) {
+                mg_warp_table(sw, F.a, (F.m >> 8) & 0xFF, (F.m >> 16) & 0xFF, F.mloc, tile0, lane);
+                mg_emit_blocks<8>(se, A, k, F, E, ra, rb, tile0, min(MG_TLOC, F.mloc - tile0), false, true, nullptr,
+                                  dummy, lane);
+            }
+            mg_flush_all(se, A, k, E, lane);
         }
-        mg_flush_all(se, A, k, E, lane);
     }
 }
 

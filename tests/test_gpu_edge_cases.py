@@ -90,6 +90,19 @@ def test_dense_cells_overflow_stash_and_table(mg, ctx):
     assert np.diff(got["row_ptr"]).max() > 1000
 
 
+def test_large_structure_with_tiled_table(mg, ctx):
+    # 280 atoms (above the shared-memory staging limit) in a 5 A cell with a 15.5 A cutoff: the
+    # per-pair sub-box has 7^3 = 343 cells (several table tiles) and a source row has > 256 pairs
+    rng = np.random.default_rng(3)
+    cell = (np.diag([5.0, 5.2, 5.4]) + rng.uniform(-0.3, 0.3, (3, 3))).astype(np.float32)
+    b = C.Batch(pos=rng.random((280, 3), dtype=np.float32), lattice=cell[None],
+                struct_ptr=np.array([0, 280], np.int32))
+    got, status = _run_cutoff(mg, ctx, b, 15.5)
+    assert status == 0
+    rep = check.check_cutoff(b, 15.5, got)
+    assert rep["extra"] == 0 and rep["missing"] == 0 and rep["n_edges"] > 5_000_000
+
+
 def test_capacity_overflow_reports_required_count(mg, ctx):
     b = C.small_batch(16, seed=2)
     full, status = _run_cutoff(mg, ctx, b, 5.0)
