@@ -297,6 +297,39 @@ def run_gpu(args, rank, world, local_rank):
                "sample": f"the full {S}-structure batch, cutoff + KNN, {reps} repetitions ({dt:.1f} s)",
                "structures_per_s": S * reps / dt}
 
+    # ---- config 4: dynamic geometry, mg_update_graph KNN k=24 on 1024 skewed crystals, 100 steps of
+    # a pre-generated trajectory resident on the device (per-step latency, BASELINE.json metric)
+    upd = None
+    if world == 1 and not args.no_update:
+        k4, n_steps = 24, 100
+        b4 = C.config_batch(4)
+        traj = list(C.walk(b4, n_steps, seed=0))
+        tpos = torch.from_numpy(np.stack([t.pos for t in traj])).to(dev)
+        tlat = torch.from_numpy(np.stack([t.lattice for t in traj])).to(dev)
+        ptr4 = torch.from_numpy(b4.struct_ptr).to(dev)
+        graph = ctx.mg_graph_create(mg.MG_KIND_KNN, ptr4, b4.n_atoms, k=k4)
+        out4 = mg.Edges.allocate(b4.n_atoms, k4 * b4.n_atoms, dev, dist=True)
+        c4 = ctypes.byref(out4._c())
+        for i in range(5):
+            lib.mg_update_graph(h, graph._h, ctypes.c_void_p(tpos[i].data_ptr()), ctypes.c_void_p(tlat[i].data_ptr()), c4, st)
+        torch.cuda.synchronize()
+        ev4 = [torch.cuda.Event(enable_timing=True) for _ in range(n_steps + 1)]
+        ev4[0].record()
+        for i in range(n_steps):
+            r = lib.mg_update_graph(h, graph._h, ctypes.c_void_p(tpos[i].data_ptr()),
+                                    ctypes.c_void_p(tlat[i].data_ptr()), c4, st)
+            assert r == 0, r
+            ev4[i + 1].record()
+        torch.cuda.synchronize()
+        assert ctx.mg_check() == 0, "device status after the update steps"
+        lat_us = np.array([ev4[i].elapsed_time(ev4[i + 1]) * 1e3 for i in range(n_steps)])
+        upd = {"workload": f"BASELINE configs[4]: mg_update_graph KNN k={k4}, {b4.n_struct} skewed crystals, "
+                           f"{b4.n_atoms} atoms, {n_steps} steps enqueued back to back",
+               "us_per_step": {"mean": float(lat_us.mean()), "median": float(np.median(lat_us)),
+                               "max": float(lat_us.max())},
+               "edges_per_s": float(k4 * b4.n_atoms / (lat_us.mean() * 1e-6))}
+        graph.close()
+
     line = {
         "metric": "edges_per_s", "value": edges_all * K / (total_ms * 1e-3), "unit": "edges/s",
         "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / K,
@@ -323,6 +356,8 @@ def run_gpu(args, rank, world, local_rank):
         "gpu_launches": int(launches),
         "clocks": clocks,
     }
+    if upd is not None:
+        line["update_graph"] = upd
     if cpu is not None:
         line["cpu_baseline"] = cpu
     print(json.dumps(line))
@@ -337,6 +372,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-update", action="store_true", help="skip the configs[4] mg_update_graph latency leg")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
