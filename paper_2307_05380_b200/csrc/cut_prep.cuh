@@ -81,7 +81,6 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
             if (A.hint) A.hint[s] = 0.f;
         }
         r.radius = rc;
-        if (N > MG_SMALL_MAX_ATOMS && A.k > 0) err |= MGS_UNSUPPORTED;   // KNN: small structures only
         if (N > 46000) err |= MGS_UNSUPPORTED;                            // pair indices are 32 bit
         r.mloc = 0;
         r.m = 0;
@@ -120,7 +119,9 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
             // KNN: one launch, no edge stream; selecting k per row costs about 350
             const float ck = ((float)((mloc + 3) & ~3) * 11.f + 150.f) * (1.f / 32.f) + 350.f / (float)N +
                              0.5f * MG_STRUCT_COST / ((float)N * (float)N);
-            r.paircost = (unsigned)fminf(16.f * (A.k > 0 ? ck : c) + 1.f, 16777216.f);
+            // (KNN above the staging limit: warp-per-row growing-radius search, about 40 per pair-cell)
+            const float ckb = 40.f * (float)mloc / 32.f + 600.f / (float)N;
+            r.paircost = (unsigned)fminf(16.f * (A.k > 0 ? (N > MG_SMALL_MAX_ATOMS ? ckb : ck) : c) + 1.f, 16777216.f);
         }
         r.pad = 0;
         cost = (unsigned long long)((long long)N * N) * r.paircost;

@@ -57,11 +57,13 @@ __device__ __noinline__ void mg_knn_row_fallback(KnnSmem &ks, const KnnPairsArgs
     StructRec R;
     float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f};
     __syncwarp();
+    const bool big = N > MG_SMALL_MAX_ATOMS;      // too large to stage: positions on the fly
     for (int j = lane; j < N; j += 32) {
         const float *x = A.pos + 3 * (size_t)(first + j);
         const float x0 = x[0], x1 = x[1], x2 = x[2];
         lo[0] = fminf(lo[0], x0); lo[1] = fminf(lo[1], x1); lo[2] = fminf(lo[2], x2);
         hi[0] = fmaxf(hi[0], x0); hi[1] = fmaxf(hi[1], x1); hi[2] = fmaxf(hi[2], x2);
+        if (big) continue;
         float4 p;
         p.x = __fmaf_rn(x2, lat9[6], __fmaf_rn(x1, lat9[3], __fmul_rn(x0, lat9[0])));
         p.y = __fmaf_rn(x2, lat9[7], __fmaf_rn(x1, lat9[4], __fmul_rn(x0, lat9[1])));
@@ -102,7 +104,7 @@ __device__ __noinline__ void mg_knn_row_fallback(KnnSmem &ks, const KnnPairsArgs
     float *slot = reinterpret_cast<float *>(ks.w.T + MG_SMALL_MAX_ATOMS + 16);   // k-th distance comes back here
     K.radius_hint = A.hint ? slot - (first + i) : nullptr; K.use_hint = 0;
     K.rec = nullptr; K.atom_struct = nullptr; K.ctl = nullptr; K.status = A.status;
-    mg_knn_source<1>(K, R, lat9, sp, buf, i, lane);
+    mg_knn_source<1>(K, R, lat9, big ? nullptr : sp, buf, i, lane);
     __syncwarp();
     if (A.hint && lane == 0) atomicMax(reinterpret_cast<int *>(A.hint + s), __float_as_int(*slot));
     __syncwarp();
@@ -194,6 +196,9 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                     A.vec[3 * o] = 0.f; A.vec[3 * o + 1] = 0.f; A.vec[3 * o + 2] = 0.f;
                     if (A.dist) A.dist[o] = 0.f;
                 }
+            } else if (F.big) {
+                // above the staging limit: every row by the growing-radius routine (round 1)
+                for (int i = ia; i < ib; ++i) mg_knn_row_fallback(ks, A, s, k.first, N, i, lane);
             } else {
                 F.win = 0.f;                                   // no exact threshold decision here
                 // every image with true d2 < R^2 - win is a hit; a k-th key below R^2 - 2 win is safe

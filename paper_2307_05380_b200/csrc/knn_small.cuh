@@ -88,15 +88,27 @@ __device__ __forceinline__ mg_key mg_knn_key(float d2, int j, int t0, int t1, in
            ((mg_key)(unsigned)(t0 + 128) << 16) | ((unsigned)(t1 + 128) << 8) | (unsigned)(t2 + 128);
 }
 
+// FP32 cartesian position of atom j of the structure (x . L, the same arithmetic as the staged copy).
+__device__ __forceinline__ float4 mg_knn_cart(const float *xs, const float *lat9, int j) {
+    const float x0 = xs[3 * j], x1 = xs[3 * j + 1], x2 = xs[3 * j + 2];
+    float4 p;
+    p.x = __fmaf_rn(x2, lat9[6], __fmaf_rn(x1, lat9[3], __fmul_rn(x0, lat9[0])));
+    p.y = __fmaf_rn(x2, lat9[7], __fmaf_rn(x1, lat9[4], __fmul_rn(x0, lat9[1])));
+    p.z = __fmaf_rn(x2, lat9[8], __fmaf_rn(x1, lat9[5], __fmul_rn(x0, lat9[2])));
+    p.w = 0.f;
+    return p;
+}
+
 // Search + emit for source atom gi = R.first + i; sp = this warp's cartesian positions of the
-// structure, buf = this warp's 32-entry candidate buffer.  Called by a full warp.
+// structure (nullptr: evaluated on the fly from pos, for structures too large to stage),
+// buf = this warp's 32-entry candidate buffer.  Called by a full warp.
 template <int KPL>
 __device__ inline void mg_knn_source(const KnnArgs &A, const StructRec &R, const float *lat9,
                                      const float4 *sp, mg_key *buf, int i, int lane) {
     const int N = R.natoms, k = A.k, gi = R.first + i;
     const int kslot = (k - 1) >> 5, klane = (k - 1) & 31;
     const float *xs = A.pos + 3 * (size_t)R.first;
-    const float4 pi = sp[i];
+    const float4 pi = sp ? sp[i] : mg_knn_cart(xs, lat9, i);
     float a[3][3], lo_off[3], hi_off[3], spread[3];
     float xabs = 1.f;
 #pragma unroll
@@ -158,7 +170,7 @@ __device__ inline void mg_knn_source(const KnnArgs &A, const StructRec &R, const
             const float Tz = __fmaf_rn(f2, a[2][2], __fmaf_rn(f1, a[1][2], __fmul_rn(f0, a[0][2])));
             const bool home = (t0 | t1 | t2) == 0;
             for (int j = 0; j < N; ++j) {
-                const float4 pj = sp[j];
+                const float4 pj = sp ? sp[j] : mg_knn_cart(xs, lat9, j);
                 const float d2 = mg_d2(__fsub_rn(pj.x, pi.x), __fsub_rn(pj.y, pi.y),
                                        __fsub_rn(pj.z, pi.z), Tx, Ty, Tz);
                 bool cand = alive && d2 <= thr_d2 && !(home && j == i);

@@ -109,6 +109,19 @@ def test_mixed_small_and_large_structures(mg, ctx):
     assert rep["extra"] == 0 and rep["missing"] == 0, rep
 
 
+def test_knn_large_structures(mg, ctx):
+    # structures above the shared-memory staging limit take the growing-radius routine row by row
+    small = C.small_batch(6, seed=31)
+    rng = np.random.default_rng(11)
+    cell = (np.diag([11.0, 12.0, 13.0]) + rng.uniform(-1, 1, (3, 3))).astype(np.float32)
+    big = C.Batch(pos=rng.random((200, 3), dtype=np.float32), lattice=cell[None],
+                  struct_ptr=np.array([0, 200], np.int32))
+    b = C.concat([small, big, small])
+    got, status = _knn(mg, ctx, b, 12)
+    assert status == 0
+    check.check_knn(b, 12, got)
+
+
 def test_config4_update_steps(mg, ctx):
     import torch
     k = 24
