@@ -22,7 +22,17 @@
 #define MG_CP_BLOCK 128
 #define MG_STASH 1024              // stash entries per warp of the emit kernel (cutoff_pairs.cuh)
 #define MG_KNN_ALPHA 1.45f          // KNN: expected images inside the first search radius, in units of k
-#define MG_STRUCT_COST 900.f        // warp instructions' worth of latency to stage one structure (both launches)
+// cost model of the cutoff path, in warp instructions (tuned on config 2, profiles/)
+#ifndef MG_STRUCT_COST
+#define MG_STRUCT_COST 900.f       // staging one structure (latency, both launches)
+#endif
+#ifndef MG_C_CELL
+#define MG_C_CELL 14.f             // per candidate cell of a pair (x 1/32 per lane)
+#define MG_C_CELL_WIDE 24.f        // ... tables of 129-256 cells
+#define MG_C_BLOCK 250.f           // per block of 32 pairs
+#define MG_C_BLOCK_WIDE 500.f
+#define MG_C_EDGE 3.3f             // per emitted edge
+#endif
 
 struct CutRec {              // 64 bytes
     float rho[3];            // upper bound of r_c / h_a (plus the guard eps)
@@ -112,9 +122,9 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
             // of 32 pairs, 3.3 per edge; the per-structure staging is spread over its pairs
             // (structures whose table is tiled evaluate their candidates again in the emit launch)
             // and walk them one source row (N of 32 lanes) at a time)
-            const float percell = mloc > 256 ? 11.f + 900.f / (float)N : (mloc > 128 ? 19.f : 11.f);
-            const float perblock = mloc > 256 ? 120.f + 16000.f / (float)N : (mloc > 128 ? 500.f : 250.f);
-            const float c = ((float)((mloc + 3) & ~3) * percell + perblock) * (1.f / 32.f) + 3.3f * lam / (float)N +
+            const float percell = mloc > 256 ? 11.f + 900.f / (float)N : (mloc > 128 ? MG_C_CELL_WIDE : MG_C_CELL);
+            const float perblock = mloc > 256 ? 120.f + 16000.f / (float)N : (mloc > 128 ? MG_C_BLOCK_WIDE : MG_C_BLOCK);
+            const float c = ((float)((mloc + 3) & ~3) * percell + perblock) * (1.f / 32.f) + MG_C_EDGE * lam / (float)N +
                             MG_STRUCT_COST / ((float)N * (float)N);
             // KNN: one launch, no edge stream; selecting k per row costs about 350
             const float ck = ((float)((mloc + 3) & ~3) * 11.f + 150.f) * (1.f / 32.f) + 350.f / (float)N +
