@@ -211,11 +211,10 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                 for (int i0 = ia; i0 < ib; i0 += rpt) {
                     const int nr = min(rpt, ib - i0);
                     int total;
-                    if (F.mloc > MG_TLOC) total = MG_KSTASH + 1;          // table does not fit: row by row below
-                    else if (F.mloc <= 32) total = mg_knn_find<1>(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
+                    if (F.mloc <= 32) total = mg_knn_find<1>(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
                     else if (F.mloc <= 64) total = mg_knn_find<2>(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
                     else if (F.mloc <= 128) total = mg_knn_find<4>(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
-                    else total = mg_knn_find<8>(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
+                    else total = MG_KSTASH + 1;                  // wide tables: row by row below
                     __syncwarp();
                     if (lane == 0) ks.rowoff[nr] = total;
                     __syncwarp();
