@@ -143,6 +143,39 @@ def test_config4_update_steps(mg, ctx):
     graph.close()
 
 
+def test_update_graph_in_a_cuda_graph(mg, ctx):
+    # mg_update_graph allocates nothing and never synchronises: capture one step in a CUDA graph,
+    # replay it on new geometry written into the captured input buffers, compare with fresh calls
+    import torch
+    k = 12
+    b0 = C.config_batch(4, n_struct=128)
+    steps = list(C.walk(b0, 4, seed=3))
+    ptr = torch.from_numpy(b0.struct_ptr).cuda()
+    pos_buf = torch.from_numpy(steps[0].pos).cuda()
+    lat_buf = torch.from_numpy(steps[0].lattice).cuda()
+    graph = ctx.mg_graph_create(mg.MG_KIND_KNN, ptr, b0.n_atoms, k=k)
+    out = mg.Edges.allocate(b0.n_atoms, k * b0.n_atoms, "cuda", dist=True)
+    ctx.mg_update_graph(graph, pos_buf, lat_buf, out)            # warm-up outside the capture
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    cg = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        with torch.cuda.graph(cg, stream=side):
+            ctx.mg_update_graph(graph, pos_buf, lat_buf, out)
+    for b in steps[1:]:
+        pos_buf.copy_(torch.from_numpy(b.pos))
+        lat_buf.copy_(torch.from_numpy(b.lattice))
+        cg.replay()
+        torch.cuda.synchronize()
+        got = out.to_numpy()
+        assert ctx.mg_check() == 0
+        check.check_knn(b, k, got)
+        fresh, _ = _knn(mg, ctx, b, k)
+        for key in ("dst", "offset", "vec", "dist"):
+            assert np.array_equal(fresh[key], got[key]), key
+    graph.close()
+
+
 def test_update_cutoff_matches_fresh(mg, ctx):
     import torch
     b0 = C.config_batch(4, n_struct=64)
