@@ -21,7 +21,10 @@
 
 #define MG_CP_BLOCK 128
 #define MG_STASH 1024              // stash entries per warp of the emit kernel (cutoff_pairs.cuh)
-#define MG_KNN_ALPHA 1.45f          // KNN: expected images inside the first search radius, in units of k
+#ifndef MG_KNN_ALPHA
+#define MG_KNN_ALPHA 1.45f         // KNN: expected images inside the first search radius, in units of k
+#define MG_KNN_RSCALE 1.05f        // ... and the safety factor on that radius
+#endif
 // cost model of the cutoff path, in warp instructions (tuned on config 2, profiles/)
 #ifndef MG_STRUCT_COST
 #define MG_STRUCT_COST 900.f       // staging one structure (latency, both launches)
@@ -85,7 +88,7 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
         float rc = A.r_c;
         if (A.k > 0) {                                 // KNN: radius from the density, or from the last call
             const float hv = A.hint && A.use_hint ? A.hint[s] : 0.f;
-            rc = 1.05f * cbrtf(0.2387324f * (MG_KNN_ALPHA * (float)A.k + 1.f) * (float)vol / (float)max(N, 1));
+            rc = MG_KNN_RSCALE * cbrtf(0.2387324f * (MG_KNN_ALPHA * (float)A.k + 1.f) * (float)vol / (float)max(N, 1));
             if (hv > 0.f && isfinite(hv)) rc = 1.02f * hv + 1e-3f;
             if (!(rc > 1e-6f) || !isfinite(rc)) rc = 1.f;
             if (A.hint) A.hint[s] = 0.f;

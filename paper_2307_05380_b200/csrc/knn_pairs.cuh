@@ -39,12 +39,15 @@ struct KnnPairsArgs {
     int n_blocks;
     int n_warps;
     unsigned *status;
+    unsigned *dbg;                 // [8, n_warps] phase cycles (MG_PHASE_CLOCKS builds) or NULL
 };
 
 struct KnnSmem {
     WarpSmem w;                    // table, staged positions
     unsigned long long stash[MG_KSTASH];
     int rowoff[MG_SMALL_MAX_ATOMS + 1];
+    float xo[MG_SMALL_MAX_ATOMS][3];   // positions as given + lattice: operands of the exact FP64 distance
+    float lat[12];
 };
 
 // Growing-radius search of one source row with the routine of knn_small.cuh (rare path).  Uses the
@@ -171,10 +174,17 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
     RangeCtx RC;
     RC.rec = A.rec; RC.bpre = A.bpre; RC.n_blocks = A.n_blocks; RC.n_struct = A.n_struct; RC.n_ranges = A.n_warps;
     const int wid = warp * gridDim.x + blockIdx.x;
+#ifdef MG_PHASE_CLOCKS
+    long long tk[6] = {0, 0, 0, 0, 0, 0};
+    const long long tk_begin = clock64();
+#define MG_KT(i, stmt) { const long long t_ = clock64(); stmt; tk[i] += clock64() - t_; }
+#else
+#define MG_KT(i, stmt) { stmt; }
+#endif
     unsigned long long c0, c1;
     mg_warp_range(RC, wid, c0, c1);
     int s, qa;
-    mg_range_start(RC, c0, s, qa, lane);
+    MG_KT(0, mg_range_start(RC, c0, s, qa, lane))
     for (; s < A.n_struct; ++s, qa = 0) {
         const CutRec *R = A.rec + s;
         int qb;
@@ -186,7 +196,9 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
         FindCtx F;
         if (ib > ia) {
             const float rad = R->radius;
-            if (!mg_struct_setup(sw, nullptr, A.pos, A.lattice, A.status, rad, R, s, k, F, lane)) {
+            bool live_;
+            MG_KT(1, live_ = mg_struct_setup(sw, nullptr, A.pos, A.lattice, A.status, rad, R, s, k, F, lane))
+            if (!live_) {
                 // invalid lattice / positions: placeholder rows (src = dst, zero vec); mg_check reports
                 for (int e = ia * K + lane; e < ib * K; e += 32) {
                     const long long o = (long long)K * R->first + e;
@@ -200,6 +212,10 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                 // above the staging limit: every row by the growing-radius routine (round 1)
                 for (int i = ia; i < ib; ++i) mg_knn_row_fallback(ks, A, s, k.first, N, i, lane);
             } else {
+                __syncwarp();
+                for (int j = lane; j < 3 * N; j += 32) (&ks.xo[0][0])[j] = A.pos[3 * (size_t)k.first + j];
+                if (lane < 9) ks.lat[lane] = F.lat[lane];
+                __syncwarp();
                 F.win = 0.f;                                   // no exact threshold decision here
                 // every image with true d2 < R^2 - win is a hit; a k-th key below R^2 - 2 win is safe
                 const float win = 1.1920929e-7f * (2.f * rad * (13.f * R->qmax + 2.f * R->amax_sum) + 4.f * rad * rad);
@@ -211,10 +227,17 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                 for (int i0 = ia; i0 < ib; i0 += rpt) {
                     const int nr = min(rpt, ib - i0);
                     int total;
+#ifdef MG_PHASE_CLOCKS
+                    const long long tf_ = clock64();
+#endif
                     if (F.mloc <= 32) total = mg_knn_find<1>(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
                     else if (F.mloc <= 64) total = mg_knn_find<2>(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
                     else if (F.mloc <= 128) total = mg_knn_find<4>(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
                     else total = MG_KSTASH + 1;                  // wide tables: row by row below
+#ifdef MG_PHASE_CLOCKS
+                    tk[2] += clock64() - tf_;
+                    const long long ts_ = clock64();
+#endif
                     __syncwarp();
                     if (lane == 0) ks.rowoff[nr] = total;
                     __syncwarp();
@@ -254,8 +277,7 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                                 const unsigned ord = ((unsigned)j << 24) | (tie >> 8);
                                 double dd = 1e300, vv[3] = {0.0, 0.0, 0.0};
                                 if (sel)
-                                    dd = mg_exact_vec(A.pos + 3 * (size_t)gi, A.pos + 3 * (size_t)(k.first + j), t0, t1, t2,
-                                                      F.lat, vv);
+                                    dd = mg_exact_vec(ks.xo[i], ks.xo[j], t0, t1, t2, ks.lat, vv);
                                 int rank = lane;
                                 {
                                     const double nd = __shfl_down_sync(0xFFFFFFFFu, dd, 1);
@@ -302,7 +324,10 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                             }
                         }
                         if (!ok) {                             // Alg. 1 line 4: not settled inside R
-                            mg_knn_row_fallback(ks, A, s, k.first, N, i, lane);
+                            MG_KT(4, mg_knn_row_fallback(ks, A, s, k.first, N, i, lane))
+#ifdef MG_PHASE_CLOCKS
+                            tk[5] += 1;
+#endif
                             dirty = true;
                             continue;
                         }
@@ -318,7 +343,7 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                         const int nsel = K + __popc(__ballot_sync(0xFFFFFFFFu, amb));
                         double dd = 1e300, vv[3] = {0.0, 0.0, 0.0};
                         if (lane < nsel)
-                            dd = mg_exact_vec(A.pos + 3 * (size_t)gi, A.pos + 3 * (size_t)(k.first + j), t0, t1, t2, F.lat, vv);
+                            dd = mg_exact_vec(ks.xo[i], ks.xo[j], t0, t1, t2, ks.lat, vv);
                         int rank = 0;
                         for (int l = 0; l < nsel; ++l) {
                             const double od = __shfl_sync(0xFFFFFFFFu, dd, l);
@@ -335,6 +360,9 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                             if (rank == K - 1) dkmax = fmaxf(dkmax, __double2float_ru(dd));
                         }
                     }
+#ifdef MG_PHASE_CLOCKS
+                    tk[3] += clock64() - ts_;
+#endif
                     if (dirty && F.mloc <= MG_TLOC) {          // the fallback used the table area as scratch
                         mg_warp_table(sw, F.a, (F.m >> 8) & 0xFF, (F.m >> 16) & 0xFF, F.mloc, 0, lane);
                     }
@@ -348,4 +376,10 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
         }
         if (qb < N * N) break;
     }
+#ifdef MG_PHASE_CLOCKS
+    if (A.dbg && lane == 0) {
+        for (int x = 0; x < 6; ++x) A.dbg[(size_t)x * A.n_warps + wid] = (unsigned)tk[x];
+        A.dbg[(size_t)6 * A.n_warps + wid] = (unsigned)(clock64() - tk_begin);
+    }
+#endif
 }

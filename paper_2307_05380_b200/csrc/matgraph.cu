@@ -120,7 +120,7 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
         if (occ >= 1 && (cudaMalloc(&c->d_wtotal, (MG_OVER * c->cut_warps + 1) * sizeof(unsigned)) != cudaSuccess ||
                          cudaMalloc(&c->d_wstart, MG_OVER * c->cut_warps * sizeof(int2)) != cudaSuccess ||
                          cudaMalloc(&c->d_wmask, (size_t)MG_OVER * c->cut_warps * MG_MASK_WORDS * sizeof(unsigned)) != cudaSuccess ||
-                         cudaMalloc(&c->d_wclock, 2 * (size_t)c->cut_warps * sizeof(unsigned)) != cudaSuccess)) { mg_destroy(c); return MG_ERR_CUDA; }
+                         cudaMalloc(&c->d_wclock, 8 * (size_t)c->cut_warps * sizeof(unsigned)) != cudaSuccess)) { mg_destroy(c); return MG_ERR_CUDA; }
     }
     if (c->cutoff_occ < 1 || c->count_occ < 1 || c->knnp_occ < 1 || c->knn_occ[0] < 1 || c->knn_occ[1] < 1) { mg_destroy(c); return MG_ERR_CUDA; }
     *out = c;
@@ -194,6 +194,13 @@ extern "C" int mg_debug_cut_warps(mg_ctx *c, unsigned *clocks_host, int *starts_
         cudaMemcpy(starts_host, c->d_wstart, (size_t)n * 8, cudaMemcpyDeviceToHost);
     }
     return c->last_cut_warps;
+}
+
+extern "C" int mg_debug_clock_words(mg_ctx *c, unsigned *host, int n_words) {
+    if (!c) return -1;
+    cudaDeviceSynchronize();
+    cudaMemcpy(host, c->d_wclock, (size_t)n_words * 4, cudaMemcpyDeviceToHost);
+    return c->cut_warps;
 }
 
 extern "C" int mg_debug_cut_masks(mg_ctx *c, unsigned *host, int n_words) {
@@ -375,6 +382,7 @@ static mg_status launch_knn(mg_ctx *c, const float *pos, const float *lat, const
         A.vec = o->vec; A.dist = o->dist; A.n_edges = (long long *)o->n_edges;
         A.hint = hint; A.rec = c->d_crec; A.bpre = c->d_bpre; A.n_blocks = n_blocks;
         A.status = c->d_ctl + 4;
+        A.dbg = c->d_wclock;
         int grid = c->sm_count * c->knnp_occ;
         const int cap_grid = (n_atoms + MG_WARPS) / MG_WARPS;
         if (grid > cap_grid) grid = cap_grid;
