@@ -162,6 +162,14 @@ __device__ __forceinline__ int mg_knn_find(KnnSmem &ks, const Task &k, const Fin
 }
 
 // 3 CTAs per SM: 168 registers per thread and no spills beat 4 CTAs at 128 registers (A/B: -12 %)
+// Wide tables are rare in the headline workload: kept out of line so that they do not cost the
+// common path registers.
+__device__ __noinline__ int mg_knn_find_wide(KnnSmem &ks, const Task &k, const FindCtx &F, int i0, int qa, int qb,
+                                             int lane) {
+    if (F.mloc <= 128) return mg_knn_find<4>(ks, k, F, i0, qa, qb, lane);
+    return mg_knn_find<8>(ks, k, F, i0, qa, qb, lane);
+}
+
 __global__ void __launch_bounds__(MG_BLOCK, 3)
 mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -233,8 +241,8 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
 #endif
                     if (F.mloc <= 32) total = mg_knn_find<1>(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
                     else if (F.mloc <= 64) total = mg_knn_find<2>(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
-                    else if (F.mloc <= 128) total = mg_knn_find<4>(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
-                    else total = MG_KSTASH + 1;                  // wide tables: row by row below
+                    else if (F.mloc <= MG_TLOC) total = mg_knn_find_wide(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
+                    else total = MG_KSTASH + 1;                  // table does not fit: row by row below
 #ifdef MG_PHASE_CLOCKS
                     tk[2] += clock64() - tf_;
                     const long long ts_ = clock64();
