@@ -1,15 +1,15 @@
 // cutoff_pairs.cuh — cutoff graph (K3 distance filter + K4 count -> device-wide scan -> emit + K6
-// batching) in two launches of autonomous WARPS: no block barriers, no spin waits,
-// no tickets.  mg_cut_prep_kernel gives every source row an estimated cost; warp w of the grid owns
-// the contiguous range of rows whose cost prefix falls in [w, w+1) * total / n_warps and walks it
-// structure by structure (positions and the translation table are staged once per structure).
+// batching) in two launches of autonomous WARPS: no block barriers, no spin waits.
+// mg_cut_prep_kernel gives every ordered pair (i, j) an estimated cost; warp w of the grid owns the
+// contiguous range of pairs, in (structure, i, j) order, whose cost prefix falls in
+// [w, w+1) * total / n_warps and walks it structure by structure (positions and the translation
+// table are staged once per structure; a range may split a source row or a large structure).
 //
-//   mg_cutoff_count_kernel  find phase over the warp's rows -> edges per warp; the last CTA out
-//                           turns them into an exclusive scan (the device-wide scan of K4) and
-//                           writes n_edges.
-//   mg_cutoff_emit_kernel   find phase again, group of rows by group of rows, now with the hits
-//                           compacted into a shared-memory stash in (row, j) order; the running
-//                           offset gives row_ptr; emit.
+//   mg_cutoff_count_kernel  find phase over the warp's pairs -> hit masks (kept in a per-warp
+//                           scratch) and edges per warp; the last CTA out turns the totals into an
+//                           exclusive scan (the device-wide scan of K4) and writes n_edges.
+//   mg_cutoff_emit_kernel   same ranges: masks read back, hits compacted into a shared-memory stash
+//                           in (row, j) order; the running offset gives row_ptr; emit.
 //
 //  find   lane <-> ordered pair (row i, target j).  For a pair only the integers
 //         tau_a in (-rho_a - u_a, rho_a - u_a), u = x_j - x_i, rho_a = r_c / h_a can be edges
@@ -42,8 +42,7 @@ struct CutoffArgs {
     const unsigned long long *bpre;   // [n_blocks + 1] cost prefix over the prep blocks, [n_blocks] = total
     int n_blocks;
     int n_warps;                   // warps of the grid
-    int n_ranges;                  // MG_OVER * n_warps ranges: the first n_warps are taken by the warp of
-                                   // the same index, the others through a ticket (evens out the tail)
+    int n_ranges;                  // MG_OVER * n_warps ranges (MG_OVER = 1: one per warp; more were slower)
     unsigned *wtotal;              // [n_ranges + 1] edges per range -> exclusive scan
     int2 *wstart;                  // [n_ranges] first (structure, pair) of each range
     unsigned *wmask;               // [n_ranges, MG_MASK_WORDS] hit masks kept from count to emit

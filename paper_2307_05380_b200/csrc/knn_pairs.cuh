@@ -1,4 +1,5 @@
-// knn_pairs.cuh — k-nearest-neighbour multigraph, k <= 32, structures of <= MG_SMALL_MAX_ATOMS atoms.
+// knn_pairs.cuh — k-nearest-neighbour multigraph, k <= 32 (structures above MG_SMALL_MAX_ATOMS atoms
+// go row by row through the growing-radius routine of knn_small.cuh).
 //
 // Problem: per source the k smallest keys (d, dst, tau_x, tau_y, tau_z) over all periodic images
 // except (i,i,0) (Alg. 2 lines 2-5, made deterministic: DESIGN.md R2, R8).
