@@ -43,6 +43,12 @@ struct StructRec {
 };
 static_assert(sizeof(StructRec) == 128, "StructRec is two 64-byte lines");
 
+// First statement of a kernel launched with programmatic stream serialisation: wait until the
+// kernel before it on the stream has completed and its writes are visible (a no-op otherwise).
+__device__ __forceinline__ void mg_grid_dependency_wait() {
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 __device__ __forceinline__ double mg_dot3(const double *u, const double *v) {
     return u[0] * v[0] + u[1] * v[1] + u[2] * v[2];
 }

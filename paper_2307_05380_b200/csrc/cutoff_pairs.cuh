@@ -435,6 +435,7 @@ __device__ __forceinline__ unsigned mg_count_tiled(WarpSmem &sw, const CutoffArg
 
 __global__ void __launch_bounds__(MG_BLOCK, 4)
 mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
+    mg_grid_dependency_wait();
     __shared__ WarpSmem s_w[MG_WARPS];
     __shared__ unsigned long long s_part[MG_BLOCK];
     __shared__ bool s_last;
@@ -726,6 +727,7 @@ __device__ __forceinline__ void mg_emit_tiled(EmitSmem &se, const CutoffArgs &A,
 
 __global__ void __launch_bounds__(MG_BLOCK, 4)
 mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
+    mg_grid_dependency_wait();
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     EmitSmem &se = reinterpret_cast<EmitSmem *>(smem_raw)[warp];

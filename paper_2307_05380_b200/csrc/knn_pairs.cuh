@@ -173,6 +173,7 @@ __device__ __noinline__ int mg_knn_find_wide(KnnSmem &ks, const Task &k, const F
 
 __global__ void __launch_bounds__(MG_BLOCK, 3)
 mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
+    mg_grid_dependency_wait();
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     KnnSmem &ks = reinterpret_cast<KnnSmem *>(smem_raw)[warp];

@@ -40,6 +40,7 @@ struct mg_ctx {
     unsigned epoch = 0;
     int cutoff_occ = 0, count_occ = 0, knn_occ[2] = {0, 0}, knnp_occ = 0;
     int64_t launches = 0;
+    int pdl = 1;                          // programmatic dependent launch (MATGRAPH_NO_PDL=1 turns it off)
     int profile = 0;                      // mg_set_profile: events around the kernels of the next calls
     cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     double prof_ms[4] = {0, 0, 0, 0};     // accumulated: prep, count, emit, knn
@@ -99,6 +100,7 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
     mg_ctx *c = new (std::nothrow) mg_ctx();
     if (!c) return MG_ERR_CUDA;
     c->device = device;
+    c->pdl = getenv("MATGRAPH_NO_PDL") ? 0 : 1;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess || prop.major < 10) { delete c; return MG_ERR_CUDA; }
     c->sm_count = prop.multiProcessorCount;
@@ -266,6 +268,26 @@ extern "C" mg_status mg_profile_read(mg_ctx *c, double *mean_ms4, int64_t *count
     return MG_OK;
 }
 
+// Launch a kernel that consumes the output of the kernel before it on the same stream with
+// programmatic dependent launch: its CTAs may be scheduled while the producer drains and wait in
+// mg_grid_dependency_wait() (common.cuh), which hides the launch latency of the dependent kernel.
+template <class Args>
+static cudaError_t launch_after(mg_ctx *c, void (*kern)(const Args), int grid, int block, size_t smem,
+                                cudaStream_t st, const Args &a) {
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof(cfg));
+    cfg.gridDim = dim3((unsigned)grid);
+    cfg.blockDim = dim3((unsigned)block);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = c->pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kern, a);
+}
+
 static mg_status launch_prep(mg_ctx *c, const float *pos, const float *lat, const int32_t *sp,
                              int32_t n_struct, int32_t n_atoms, float r_c, cudaStream_t st) {
     PrepArgs P;
@@ -318,13 +340,11 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
     A.n_ranges = MG_OVER * A.n_warps;
     c->last_cut_warps = A.n_warps;
     if (prof) cudaEventRecord(c->ev[1], st);
-    mg_cutoff_count_kernel<<<grid, MG_BLOCK, 0, st>>>(A);
-    MG_CUDA(cudaGetLastError());
+    MG_CUDA(launch_after(c, mg_cutoff_count_kernel, grid, MG_BLOCK, 0, st, A));
     c->launches += 1;
     if (prof) cudaEventRecord(c->ev[2], st);
     if (!count_only) {
-        mg_cutoff_emit_kernel<<<grid, MG_BLOCK, MG_WARPS * sizeof(EmitSmem), st>>>(A);
-        MG_CUDA(cudaGetLastError());
+        MG_CUDA(launch_after(c, mg_cutoff_emit_kernel, grid, MG_BLOCK, MG_WARPS * sizeof(EmitSmem), st, A));
         c->launches += 1;
     }
     if (prof) { cudaEventRecord(c->ev[3], st); c->pend_kind = 0; }
@@ -388,8 +408,7 @@ static mg_status launch_knn(mg_ctx *c, const float *pos, const float *lat, const
         if (grid > cap_grid) grid = cap_grid;
         A.n_warps = grid * MG_WARPS;
         if (c->profile) cudaEventRecord(c->ev[1], st);
-        mg_knn_pairs_kernel<<<grid, MG_BLOCK, MG_WARPS * sizeof(KnnSmem), st>>>(A);
-        MG_CUDA(cudaGetLastError());
+        MG_CUDA(launch_after(c, mg_knn_pairs_kernel, grid, MG_BLOCK, MG_WARPS * sizeof(KnnSmem), st, A));
         c->launches += 1;
         if (c->profile) { cudaEventRecord(c->ev[3], st); c->pend_kind = 1; }
         return MG_OK;
