@@ -70,6 +70,7 @@ struct CutPrepArgs {
 
 __global__ void __launch_bounds__(MG_CP_BLOCK)
 mg_cut_prep_kernel(const CutPrepArgs A) {
+    mg_grid_dependency_wait();      // the kernels of the previous call still read rec / bpre
     __shared__ unsigned long long s_warp[MG_CP_BLOCK / 32];
     __shared__ bool s_last;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;

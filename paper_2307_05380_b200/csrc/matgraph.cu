@@ -319,8 +319,7 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
         P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms; P.r_c = r_c;
         P.k = 0; P.hint = nullptr; P.use_hint = 0;
         P.rec = c->d_crec; P.bpre = c->d_bpre; P.ctl = c->d_ctl; P.status = c->d_ctl + 4;
-        mg_cut_prep_kernel<<<n_blocks, MG_CP_BLOCK, 0, st>>>(P);
-        MG_CUDA(cudaGetLastError());
+        MG_CUDA(launch_after(c, mg_cut_prep_kernel, n_blocks, MG_CP_BLOCK, 0, st, P));
         c->launches += 1;
     }
     CutoffArgs A;
@@ -392,8 +391,7 @@ static mg_status launch_knn(mg_ctx *c, const float *pos, const float *lat, const
         P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms; P.r_c = 0.f;
         P.k = k; P.hint = hint; P.use_hint = use_hint;
         P.rec = c->d_crec; P.bpre = c->d_bpre; P.ctl = c->d_ctl; P.status = c->d_ctl + 4;
-        mg_cut_prep_kernel<<<n_blocks, MG_CP_BLOCK, 0, st>>>(P);
-        MG_CUDA(cudaGetLastError());
+        MG_CUDA(launch_after(c, mg_cut_prep_kernel, n_blocks, MG_CP_BLOCK, 0, st, P));
         c->launches += 1;
         KnnPairsArgs A;
         A.pos = pos; A.lattice = lat; A.struct_ptr = sp;
