@@ -160,6 +160,7 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
         A.rec[s] = r;
     }
     if (threadIdx.x == 0) A.bpre[blockIdx.x] = btotal;
+    if (gridDim.x <= 32) return;          // few blocks: the graph kernels scan the raw sums themselves
     // ---- last block out: exclusive scan of the block sums (serial per thread chunk, 64 bit)
     __threadfence();
     __syncthreads();

@@ -82,7 +82,36 @@ struct RangeCtx {
     const CutRec *rec;
     const unsigned long long *bpre;
     int n_blocks, n_struct, n_ranges;
+    // n_blocks <= 32: the prep kernel leaves the raw block sums in bpre and every warp scans them
+    // itself (lane b holds the exclusive prefix of block b): no last-block phase in the prep kernel
+    bool small;
+    unsigned long long my_pre, total;
 };
+
+__device__ __forceinline__ void mg_range_init(RangeCtx &RC, const CutRec *rec, const unsigned long long *bpre,
+                                              int n_blocks, int n_struct, int n_ranges, int lane) {
+    RC.rec = rec; RC.bpre = bpre; RC.n_blocks = n_blocks; RC.n_struct = n_struct; RC.n_ranges = n_ranges;
+    RC.small = n_blocks <= 32;
+    if (RC.small) {
+        const unsigned long long v = lane < n_blocks ? __ldg(bpre + lane) : 0ull;
+        unsigned long long incl = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned long long t = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+            if (lane >= o) incl += t;
+        }
+        RC.my_pre = incl - v;
+        RC.total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+    } else {
+        RC.my_pre = 0ull;
+        RC.total = __ldg(bpre + n_blocks);
+    }
+}
+
+// Cost prefix of prep block b (b warp-uniform).
+__device__ __forceinline__ unsigned long long mg_block_pre(const RangeCtx &RC, int b) {
+    return RC.small ? __shfl_sync(0xFFFFFFFFu, RC.my_pre, b) : __ldg(RC.bpre + b);
+}
 
 // q / n for 0 <= q < 2^20, 1 <= n (exact: (q + 0.5) / n is never within rounding of an integer)
 __device__ __forceinline__ int mg_fdiv(int q, float inv_n) {
@@ -331,7 +360,7 @@ __device__ __forceinline__ bool mg_struct_setup(WarpSmem &sw, double (*pd)[3], c
 // Cost range of warp w: [c0, c1); the last warp takes everything that is left.
 __device__ __forceinline__ void mg_warp_range(const RangeCtx &A, int w, unsigned long long &c0,
                                               unsigned long long &c1) {
-    const unsigned long long total = __ldg(A.bpre + A.n_blocks);
+    const unsigned long long total = A.total;
     const unsigned long long chunk = (total + (unsigned)A.n_ranges - 1) / (unsigned)A.n_ranges;
     c0 = (unsigned long long)w * chunk;
     c1 = w == A.n_ranges - 1 ? ~0ull : c0 + chunk;
@@ -341,6 +370,10 @@ __device__ __forceinline__ void mg_warp_range(const RangeCtx &A, int w, unsigned
 // bpre[s / MG_CP_BLOCK] + rec[s].lpre + q * paircost is >= c0.
 __device__ inline void mg_range_start(const RangeCtx &A, unsigned long long c0, int &s_out, int &q_out, int lane) {
     int lo = 0, hi = A.n_blocks;                   // last prep block b with bpre[b] <= c0 (32-ary search)
+    if (A.small) {
+        lo = max(1, __popc(__ballot_sync(0xFFFFFFFFu, lane < A.n_blocks && A.my_pre <= c0))) - 1;
+        hi = lo + 1;
+    }
     while (hi - lo > 1) {
         const int step = (hi - lo + 31) / 32;
         const int idx = lo + (lane + 1) * step;
@@ -349,7 +382,7 @@ __device__ inline void mg_range_start(const RangeCtx &A, unsigned long long c0, 
         hi = min(hi, lo + step);
     }
     const int b = lo;
-    const unsigned long long bp = __ldg(A.bpre + b);
+    const unsigned long long bp = mg_block_pre(A, b);
     int cnt = 0;                                   // structures of the block whose prefix is <= c0
 #pragma unroll
     for (int x = 0; x < MG_CP_BLOCK / 32; ++x) {
@@ -370,7 +403,7 @@ __device__ inline void mg_range_start(const RangeCtx &A, unsigned long long c0, 
 // given: 0, or the range's first pair).  Returns false when the range ends before qa.
 __device__ __forceinline__ bool mg_segment(const RangeCtx &A, const CutRec *R, int s, int qa,
                                            unsigned long long c1, int &qb) {
-    const unsigned long long cs = __ldg(A.bpre + s / MG_CP_BLOCK) + R->lpre;
+    const unsigned long long cs = mg_block_pre(A, s / MG_CP_BLOCK) + R->lpre;
     const unsigned pc = R->paircost;
     const int NN = R->natoms * R->natoms;
     if (cs + (unsigned long long)qa * pc >= c1) return false;
@@ -445,7 +478,7 @@ mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
     const int wid = warp * gridDim.x + blockIdx.x;
     const long long t_begin = clock64();
     RangeCtx RC;
-    RC.rec = A.rec; RC.bpre = A.bpre; RC.n_blocks = A.n_blocks; RC.n_struct = A.n_struct; RC.n_ranges = A.n_ranges;
+    mg_range_init(RC, A.rec, A.bpre, A.n_blocks, A.n_struct, A.n_ranges, lane);
     for (int w = wid; w < A.n_ranges;) {
         int w_next = 0;
         if (lane == 0) w_next = (int)atomicAdd(A.ctl, 1u) + A.n_warps;     // needed only at the end
@@ -736,7 +769,7 @@ mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
     const int wid = warp * gridDim.x + blockIdx.x;
     const long long t_begin = clock64();
     RangeCtx RC;
-    RC.rec = A.rec; RC.bpre = A.bpre; RC.n_blocks = A.n_blocks; RC.n_struct = A.n_struct; RC.n_ranges = A.n_ranges;
+    mg_range_init(RC, A.rec, A.bpre, A.n_blocks, A.n_struct, A.n_ranges, lane);
     for (int w = wid; w < A.n_ranges;) {
         int w_next = 0;
         if (lane == 0) w_next = (int)atomicAdd(A.ctl + 8, 1u) + A.n_warps;

@@ -183,7 +183,7 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
     if (blockIdx.x == 0 && threadIdx.x == 0) *A.n_edges = (long long)A.k * A.n_atoms;
     const int K = A.k;
     RangeCtx RC;
-    RC.rec = A.rec; RC.bpre = A.bpre; RC.n_blocks = A.n_blocks; RC.n_struct = A.n_struct; RC.n_ranges = A.n_warps;
+    mg_range_init(RC, A.rec, A.bpre, A.n_blocks, A.n_struct, A.n_warps, lane);
     const int wid = warp * gridDim.x + blockIdx.x;
 #ifdef MG_PHASE_CLOCKS
     long long tk[6] = {0, 0, 0, 0, 0, 0};

@@ -103,6 +103,21 @@ def test_large_structure_with_tiled_table(mg, ctx):
     assert rep["extra"] == 0 and rep["missing"] == 0 and rep["n_edges"] > 5_000_000
 
 
+def test_more_than_32_prep_blocks(mg, ctx):
+    # above 4096 structures the search-bounds kernel scans its block sums itself (last block out);
+    # below, the graph kernels scan the raw sums: this batch takes the first path
+    part = C.small_batch(300, seed=17)
+    b = C.concat([part] * 15)                       # 4500 structures
+    got, status = _run_cutoff(mg, ctx, b, 4.0)
+    assert status == 0
+    rep = check.check_cutoff(b, 4.0, got)
+    assert rep["extra"] == 0 and rep["missing"] == 0 and rep["n_edges"] > 100_000
+    pos, lat, ptr = mg.to_device(b)
+    gk = ctx.knn_graph(pos, lat, ptr, 8, dist=True).to_numpy()
+    assert ctx.mg_check() == 0
+    check.check_knn(b, 8, gk)
+
+
 def test_capacity_overflow_reports_required_count(mg, ctx):
     b = C.small_batch(16, seed=2)
     full, status = _run_cutoff(mg, ctx, b, 5.0)
