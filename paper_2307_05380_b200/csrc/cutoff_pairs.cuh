@@ -511,7 +511,10 @@ mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
         w = __shfl_sync(0xFFFFFFFFu, w_next, 0);
     }
     if (lane == 0) A.wclock[wid] = (unsigned)(clock64() - t_begin);
-    // ---- last CTA out: exclusive scan of the warp totals, grand total
+    // The emit launch sums the totals of the ranges before its own itself (one coalesced pass per
+    // warp, overlapped with the other warps' work): no tail in this launch.  mg_cutoff_count has no
+    // emit launch: ---- last CTA out: exclusive scan of the warp totals, grand total
+    if (!A.count_only) return;
     __threadfence();
     __syncthreads();
     if (threadIdx.x == 0) s_last = atomicAdd(A.ctl + 1, 1u) == gridDim.x - 1;
@@ -783,7 +786,19 @@ mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
 #ifdef MG_PHASE_CLOCKS
         E.tc[0] = E.tc[1] = E.tc[2] = E.tc[3] = 0;
 #endif
-        E.goff = (long long)__ldg(A.wtotal + w);
+        {   // device-wide scan of K4, consumer side: edges of the ranges before this one
+            unsigned long long before = 0ull;
+            for (int c = lane; c < w; c += 32) before += __ldg(A.wtotal + c);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) before += __shfl_xor_sync(0xFFFFFFFFu, before, o);
+            E.goff = (long long)before;
+            if (w == A.n_ranges - 1 && lane == 0) {          // the last range also knows the grand total
+                const unsigned long long tot = before + __ldg(A.wtotal + w);
+                *A.n_edges = (long long)tot;
+                A.row_ptr[A.n_atoms] = (int)tot;
+                if (tot > 0x7FFFFFFFull || (long long)tot > A.capacity) atomicOr(A.status, MGS_CAPACITY);
+            }
+        }
         for (; s < A.n_struct; ++s, qa = 0) {
             const CutRec *R = A.rec + s;
             int qb;
