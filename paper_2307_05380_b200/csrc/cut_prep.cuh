@@ -31,6 +31,7 @@
 #endif
 #ifndef MG_C_CELL
 #define MG_C_CELL 14.f             // per candidate cell of a pair (x 1/32 per lane)
+#define MG_C_CELL_MID 14.f         // ... tables of 65-128 cells
 #define MG_C_CELL_WIDE 24.f        // ... tables of 129-256 cells
 #define MG_C_BLOCK 250.f           // per block of 32 pairs
 #define MG_C_BLOCK_WIDE 500.f
@@ -126,7 +127,7 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
             // of 32 pairs, 3.3 per edge; the per-structure staging is spread over its pairs
             // (structures whose table is tiled evaluate their candidates again in the emit launch)
             // and walk them one source row (N of 32 lanes) at a time)
-            const float percell = mloc > 256 ? 11.f + 900.f / (float)N : (mloc > 128 ? MG_C_CELL_WIDE : MG_C_CELL);
+            const float percell = mloc > 256 ? 11.f + 900.f / (float)N : (mloc > 128 ? MG_C_CELL_WIDE : (mloc > 64 ? MG_C_CELL_MID : MG_C_CELL));
             const float perblock = mloc > 256 ? 120.f + 16000.f / (float)N : (mloc > 128 ? MG_C_BLOCK_WIDE : MG_C_BLOCK);
             const float c = ((float)((mloc + 3) & ~3) * percell + perblock) * (1.f / 32.f) + MG_C_EDGE * lam / (float)N +
                             MG_STRUCT_COST / ((float)N * (float)N);
