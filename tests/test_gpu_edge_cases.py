@@ -40,6 +40,16 @@ def test_empty_batch(mg, ctx):
     assert out["n_edges"] == 0 and out["row_ptr"].tolist() == [0]
 
 
+def test_batch_of_empty_structures_only(mg, ctx):
+    b = C.Batch(pos=np.zeros((0, 3), np.float32), lattice=np.tile(np.eye(3, dtype=np.float32) * 5, (7, 1, 1)),
+                struct_ptr=np.zeros(8, np.int32))
+    got, status = _run_cutoff(mg, ctx, b, 5.0, capacity=0)
+    assert status == 0 and got["n_edges"] == 0 and got["row_ptr"].tolist() == [0]
+    pos, lat, ptr = mg.to_device(b)
+    out = ctx.knn_graph(pos, lat, ptr, 4).to_numpy()
+    assert ctx.mg_check() == 0 and out["n_edges"] == 0 and out["row_ptr"].tolist() == [0]
+
+
 def test_empty_structures_inside_batch(mg, ctx):
     a = C.small_batch(5, seed=7)
     empty = C.Batch(pos=np.zeros((0, 3), np.float32), lattice=np.eye(3, dtype=np.float32)[None] * 4,
