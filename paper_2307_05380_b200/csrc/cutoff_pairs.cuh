@@ -240,6 +240,11 @@ __device__ __forceinline__ void mg_pair_masks(const WarpSmem &sw, const FindCtx 
                                               int l0, int l1, int l2, int ncl, unsigned (&mask)[W]) {
     bool near = false;
     const float nr2 = F.nr2, win = F.win;
+    if (W == 1 && ncl == 1) {                     // one image per pair (cells wider than 2 r_c): T_0 = 0
+        const float y = __fmaf_rn(qz, qz, __fmaf_rn(qy, qy, __fmaf_rn(qx, qx, nr2)));
+        mask[0] = y < win ? 1u : 0u;
+        near = fabsf(y) < win;
+    } else
 #pragma unroll
     for (int w = 0; w < W; ++w) {
         mask[w] = 0u;
