@@ -70,7 +70,6 @@ struct EmitSmem {
     WarpSmem w;
     double pd[MG_SMALL_MAX_ATOMS][3];   // cartesian positions x . L in FP64
     unsigned stash[MG_STASH];
-    unsigned pairij[256];              // (i << 16 | j) of the pairs of the stash's batch
 };
 
 struct Task {
@@ -250,6 +249,7 @@ __device__ __forceinline__ void mg_pair_masks(const WarpSmem &sw, const FindCtx 
         mask[w] = 0u;
         const int n4 = min(8, max(0, (ncl - 32 * w + 3) >> 2));      // warp-uniform
         const float4 *Tp = sw.T + 32 * w;
+#pragma unroll 1                  // a loop, not 8 copies: the kernels are bound by instruction fetch
         for (int g = 0; g < n4; ++g) {
             unsigned sub = 0u;
 #pragma unroll
@@ -325,6 +325,56 @@ __device__ __forceinline__ void mg_block_masks(const WarpSmem &sw, const FindCtx
 #pragma unroll
     for (int w = 0; w < W; ++w)
         if (p.self >= 0 && cs >= 32 * w && cs < 32 * w + 32) mask[w] &= ~(1u << (cs & 31));
+}
+
+// The same for ONE word of the mask — cells [32 w, 32 w + 32) of the table tile that starts at cell
+// tile0 and holds ncl cells — with the word index a run-time value: the cutoff kernels have one copy
+// of this code for tables of every size (they are bound by instruction fetch, profiles/).
+__device__ __forceinline__ unsigned mg_word_mask(const WarpSmem &sw, const FindCtx &F, const PairLane &p, int gi,
+                                                 int gj, int tile0, int w, int ncl) {
+    const float nr2 = F.nr2, win = F.win;
+    const int nw = min(32, ncl - 32 * w);                        // cells of the word (warp-uniform)
+    const float4 *Tp = sw.T + 32 * w;
+    unsigned mask = 0u;
+    bool near = false;
+    if (nw == 1) {                                               // one image per pair: T_0 = 0
+        const float y = __fmaf_rn(p.qz, p.qz, __fmaf_rn(p.qy, p.qy, __fmaf_rn(p.qx, p.qx, nr2)));
+        mask = y < win ? 1u : 0u;
+        near = fabsf(y) < win;
+    } else {
+        const int n4 = (nw + 3) >> 2;
+#pragma unroll 1
+        for (int g = 0; g < n4; ++g) {
+            unsigned sub = 0u;
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+                const float4 T = Tp[4 * g + c];
+                const float vx = __fadd_rn(p.qx, T.x), vy = __fadd_rn(p.qy, T.y), vz = __fadd_rn(p.qz, T.z);
+                const float y = __fmaf_rn(vz, vz, __fmaf_rn(vy, vy, __fmaf_rn(vx, vx, nr2)));
+                if (y < win) sub |= 1u << c;
+                near = near || fabsf(y) < win;
+            }
+            mask |= sub << (4 * g);
+        }
+    }
+    if (near) {                                   // rare: decide the window cells in FP64
+        const float *xi = F.pos + 3 * (size_t)gi, *xj = F.pos + 3 * (size_t)gj;
+        for (int c = 0; c < nw; ++c) {
+            const float4 T = Tp[c];
+            const float vx = __fadd_rn(p.qx, T.x), vy = __fadd_rn(p.qy, T.y), vz = __fadd_rn(p.qz, T.z);
+            const float y = __fmaf_rn(vz, vz, __fmaf_rn(vy, vy, __fmaf_rn(vx, vx, nr2)));
+            if (fabsf(y) < win) {
+                const unsigned tc = sw.tcode[32 * w + c];
+                double v[3];
+                const double d = mg_exact_vec(xi, xj, p.l0 + (int)(tc >> 24), p.l1 + (int)((tc >> 16) & 0xFFu),
+                                              p.l2 + (int)((tc >> 8) & 0xFFu), F.lat, v);
+                mask = d < (double)F.rc ? (mask | (1u << c)) : (mask & ~(1u << c));
+            }
+        }
+    }
+    const int cs = p.self - tile0 - 32 * w;       // (i, i, 0) is not an edge
+    if (p.self >= 0 && cs >= 0 && cs < 32) mask &= ~(1u << cs);
+    return mask;
 }
 
 // Constants of the find phase for structure s with radius rc; stages the structure (positions,
@@ -420,70 +470,77 @@ __device__ __forceinline__ bool mg_segment(const RangeCtx &A, const CutRec *R, i
 
 // ---------------------------------------------------------------------------------------------
 // Launch 1: count.  Pairs [qa, qb) of the staged structure: hit masks -> edge count (per lane);
-// the masks go to the warp's scratch for the emit launch while they fit.
-template <int W>
-__device__ __forceinline__ unsigned mg_count_segment(const WarpSmem &sw, const CutoffArgs &A, const Task &k,
-                                                     const FindCtx &F, int qa, int qb, unsigned *wmask, int &midx,
-                                                     int lane) {
+// the masks go to the warp's scratch for the emit launch while they fit (ceil(mloc / 32) words per
+// lane and block of 32 pairs).  Structures whose table does not fit (mloc > MG_TLOC) walk their
+// pairs once per tile of the table and keep nothing.
+__device__ __forceinline__ unsigned mg_count_struct(WarpSmem &sw, const CutoffArgs &A, const Task &k,
+                                                    const FindCtx &F, int qa, int qb, unsigned *wmask, int &midx,
+                                                    int lane) {
     const int N = k.natoms;
     const float inv_N = 1.f / (float)N;
-    unsigned acc = 0u;
-    for (int q0 = qa; q0 < qb; q0 += 32) {
-        const int q = q0 + lane;
-        const bool valid = q < qb;
-        int i = 0, j = 0;
-        if (valid) mg_qsplit(q, N, inv_N, i, j);
-        const PairLane p = mg_pair_setup(sw, F, valid, i, j);
-        if (valid && !p.ok) atomicOr(A.status, MGS_OFFSET);
-        unsigned mask[W];
-        mg_block_masks<W>(sw, F, p, k.first + i, k.first + j, 0, F.mloc, mask);
-        const bool keep = midx + 32 * W <= MG_MASK_WORDS;
-#pragma unroll
-        for (int w = 0; w < W; ++w) {
-            acc += __popc(mask[w]);
-            if (keep) wmask[midx + 32 * w + lane] = mask[w];
-        }
-        midx += 32 * W;
-    }
-    return acc;
-}
-
-// Structures whose table does not fit (mloc > MG_TLOC): row by row, tile by tile.
-__device__ __forceinline__ unsigned mg_count_tiled(WarpSmem &sw, const CutoffArgs &A, const Task &k, const FindCtx &F,
-                                                int qa, int qb, int lane) {
-    const int N = k.natoms;
+    const bool tiled = F.mloc > MG_TLOC;
     unsigned acc = 0u;
     for (int tile0 = 0; tile0 < F.mloc; tile0 += MG_TLOC) {
-        const int ncl = min(MG_TLOC, F.mloc - tile0);
-        mg_warp_table(sw, F.a, (F.m >> 8) & 0xFF, (F.m >> 16) & 0xFF, F.mloc, tile0, lane);
+        const int ncl = min(MG_TLOC, F.mloc - tile0), nW = (ncl + 31) >> 5;
+        if (tiled) mg_warp_table(sw, F.a, (F.m >> 8) & 0xFF, (F.m >> 16) & 0xFF, F.mloc, tile0, lane);
         for (int q0 = qa; q0 < qb; q0 += 32) {
             const int q = q0 + lane;
             const bool valid = q < qb;
-            const int i = valid ? q / N : 0, j = valid ? q - i * N : 0;
+            int i = 0, j = 0;
+            if (valid) mg_qsplit(q, N, inv_N, i, j);
             const PairLane p = mg_pair_setup(sw, F, valid, i, j);
             if (valid && !p.ok && tile0 == 0) atomicOr(A.status, MGS_OFFSET);
-            unsigned mask[8];
-            mg_block_masks<8>(sw, F, p, k.first + i, k.first + j, tile0, ncl, mask);
-#pragma unroll
-            for (int w = 0; w < 8; ++w) acc += __popc(mask[w]);
+            const bool keep = !tiled && midx + 32 * nW <= MG_MASK_WORDS;
+#pragma unroll 1
+            for (int w = 0; w < nW; ++w) {
+                const unsigned m = mg_word_mask(sw, F, p, k.first + i, k.first + j, tile0, w, ncl);
+                acc += __popc(m);
+                if (keep) wmask[midx + 32 * w + lane] = m;
+            }
+            if (!tiled) midx += 32 * nW;
         }
     }
     return acc;
 }
 
-__global__ void __launch_bounds__(MG_BLOCK, 4)
-mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
-    mg_grid_dependency_wait();
-    __shared__ WarpSmem s_w[MG_WARPS];
-    __shared__ unsigned long long s_part[MG_BLOCK];
-    __shared__ bool s_last;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    WarpSmem &sw = s_w[warp];
-    // consecutive ranges (often parts of one expensive structure) go to different SMs
-    const int wid = warp * gridDim.x + blockIdx.x;
-    const long long t_begin = clock64();
-    RangeCtx RC;
-    mg_range_init(RC, A.rec, A.bpre, A.n_blocks, A.n_struct, A.n_ranges, lane);
+// Structures with ONE candidate image per pair (mloc == 1: every plane spacing above 2 r_c, e.g. the
+// supercells of BASELINE configs[3] — the minimum-image limit): the hit mask of a block of 32 pairs
+// is one ballot word.  Returns the block's hits on lane 0 only (the caller reduces over lanes).
+__device__ __forceinline__ unsigned mg_single_word(const WarpSmem &sw, const CutoffArgs &A, const Task &k,
+                                                   const FindCtx &F, int q0, int qb, float inv_N, bool report,
+                                                   int lane) {
+    const int q = q0 + lane;
+    const bool valid = q < qb;
+    int i = 0, j = 0;
+    if (valid) mg_qsplit(q, k.natoms, inv_N, i, j);
+    const PairLane p = mg_pair_setup(sw, F, valid, i, j);
+    if (report && valid && !p.ok) atomicOr(A.status, MGS_OFFSET);
+    const unsigned m = mg_word_mask(sw, F, p, k.first + i, k.first + j, 0, 0, 1);
+    return __ballot_sync(0xFFFFFFFFu, (m & 1u) != 0u);
+}
+
+// (its own structure setup: no table, no FP64 positions in the count launch)
+__device__ __forceinline__ unsigned mg_count_single(WarpSmem &sw, const CutoffArgs &A, const CutRec *R, int s, int qa,
+                                                 int qb, unsigned *wmask, int midx, int lane) {
+    Task k;
+    FindCtx F;
+    if (!mg_struct_setup(sw, nullptr, A.pos, A.lattice, A.status, A.r_c, R, s, k, F, lane)) return 0u;
+    const float inv_N = 1.f / (float)k.natoms;
+    unsigned acc = 0u;
+    for (int q0 = qa; q0 < qb; q0 += 32) {
+        const unsigned word = mg_single_word(sw, A, k, F, q0, qb, inv_N, true, lane);
+        if (lane == 0) {
+            acc += __popc(word);
+            if (midx < MG_MASK_WORDS) wmask[midx] = word;
+        }
+        midx += 1;
+    }
+    return acc;
+}
+
+// The ranges of one warp.
+__device__ __forceinline__ void mg_count_ranges(WarpSmem &sw, const CutoffArgs &A, const RangeCtx &RC, int wid,
+                                                int lane) {
     for (int w = wid; w < A.n_ranges;) {
         int w_next = 0;
         if (lane == 0) w_next = (int)atomicAdd(A.ctl, 1u) + A.n_warps;     // needed only at the end
@@ -501,12 +558,11 @@ mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
             if (!mg_segment(RC, R, s, qa, c1, qb)) break;
             Task k;
             FindCtx F;
-            if (qb > qa && mg_struct_setup(sw, nullptr, A.pos, A.lattice, A.status, A.r_c, R, s, k, F, lane)) {
-                if (F.mloc <= 32) total += mg_count_segment<1>(sw, A, k, F, qa, qb, wmask, midx, lane);
-                else if (F.mloc <= 64) total += mg_count_segment<2>(sw, A, k, F, qa, qb, wmask, midx, lane);
-                else if (F.mloc <= 128) total += mg_count_segment<4>(sw, A, k, F, qa, qb, wmask, midx, lane);
-                else if (F.mloc <= MG_TLOC) total += mg_count_segment<8>(sw, A, k, F, qa, qb, wmask, midx, lane);
-                else total += mg_count_tiled(sw, A, k, F, qa, qb, lane);
+            if (qb > qa && R->mloc == 1) {
+                total += mg_count_single(sw, A, R, s, qa, qb, wmask, midx, lane);
+                midx += (qb - qa + 31) >> 5;
+            } else if (qb > qa && mg_struct_setup(sw, nullptr, A.pos, A.lattice, A.status, A.r_c, R, s, k, F, lane)) {
+                total += mg_count_struct(sw, A, k, F, qa, qb, wmask, midx, lane);
             }
             if (qb < R->natoms * R->natoms) break;
         }
@@ -515,6 +571,22 @@ mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
         if (lane == 0) A.wtotal[w] = total;
         w = __shfl_sync(0xFFFFFFFFu, w_next, 0);
     }
+}
+
+__global__ void __launch_bounds__(MG_BLOCK, 4)
+mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
+    mg_grid_dependency_wait();
+    __shared__ WarpSmem s_w[MG_WARPS];
+    __shared__ unsigned long long s_part[MG_BLOCK];
+    __shared__ bool s_last;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    WarpSmem &sw = s_w[warp];
+    // consecutive ranges (often parts of one expensive structure) go to different SMs
+    const int wid = warp * gridDim.x + blockIdx.x;
+    const long long t_begin = clock64();
+    RangeCtx RC;
+    mg_range_init(RC, A.rec, A.bpre, A.n_blocks, A.n_struct, A.n_ranges, lane);
+    mg_count_ranges(sw, A, RC, wid, lane);
     if (lane == 0) A.wclock[wid] = (unsigned)(clock64() - t_begin);
     // The emit launch sums the totals of the ranges before its own itself (one coalesced pass per
     // warp, overlapped with the other warps' work): no tail in this launch.  mg_cutoff_count has no
@@ -568,38 +640,6 @@ struct EmitCtx {
 #define MG_TOC(i)
 #endif
 
-// Lanes <-> pairs: every lane writes its own hits of one block straight to global memory,
-// starting at edge index pos (slow path: blocks that do not fit the stash, tiled structures).
-template <int W>
-__device__ __forceinline__ void mg_direct_block(const WarpSmem &sw, const double (*pd)[3], const CutoffArgs &A,
-                                                const Task &k, const EmitCtx &E, const PairLane &p, int i, int j,
-                                                const unsigned (&mask)[W], long long pos) {
-    const unsigned paircode = ((unsigned)(p.l0 + 128) << 24) | ((unsigned)(p.l1 + 128) << 16) |
-                              ((unsigned)(p.l2 + 128) << 8);
-#pragma unroll
-    for (int w = 0; w < W; ++w) {
-        unsigned mk = mask[w];
-        while (mk) {
-            const int b = __ffs(mk) - 1;
-            mk &= mk - 1;
-            const unsigned code = paircode + sw.tcode[32 * w + b];
-            if (pos < A.capacity) {
-                if (E.big) {
-                    double pi[3], pj[3];
-                    mg_pd_big(E.gx, E.Ld, i, pi);
-                    mg_pd_big(E.gx, E.Ld, j, pj);
-                    mg_emit_edge(A, pos, k.first + i, k.first + j, pi, pj, E.Ld, code >> 24, (code >> 16) & 0xFFu,
-                                 (code >> 8) & 0xFFu);
-                } else {
-                    mg_emit_edge(A, pos, k.first + i, k.first + j, pd[i], pd[j], E.Ld, code >> 24,
-                                 (code >> 16) & 0xFFu, (code >> 8) & 0xFFu);
-                }
-            }
-            ++pos;
-        }
-    }
-}
-
 // Stash -> global: lanes over consecutive edges; the low byte of a code is the pair's index
 // relative to qb0.  vec = (p_j - p_i) + tau . L in FP64, rounded once (R24).
 __device__ __forceinline__ void mg_flush(const EmitSmem &se, const CutoffArgs &A, const Task &k, const EmitCtx &E,
@@ -650,134 +690,219 @@ __device__ __forceinline__ void mg_flush(const EmitSmem &se, const CutoffArgs &A
     }
 }
 
-// Blocks of 32 pairs [qa, qb) against the cells [tile0, tile0 + ncl) of the table: hits appended
-// to the stash (E.run entries so far, pair indices relative to E.qb0), written out when it is full.
-// scratch: read the masks the count launch kept instead of evaluating them again.
-// pinned: E.qb0 stays (the caller walks the same pairs again for the next tile).
-template <int W>
-__device__ __forceinline__ void mg_emit_blocks(EmitSmem &se, const CutoffArgs &A, const Task &k, const FindCtx &F,
-                                               EmitCtx &E, int qa, int qb, int tile0, int ncl, bool scratch,
-                                               bool pinned, const unsigned *wmask, int &midx, int lane) {
-    const WarpSmem &sw = se.w;
+// Pairs [qa, qb) of the staged structure -> edges.  The hit masks of a block of 32 pairs live in MW
+// registers, of which the first nW = ceil(cells / 32) are used: three instances (MW = 1, 2: 98 % of
+// the pairs of an MP-like batch; 8: everything else), not one per table size — the kernel is bound
+// by instruction fetch (profiles/).
+//   * the table fits (mloc <= MG_TLOC): one segment [qa, qb), the masks are read back from the
+//     scratch of the count launch one block ahead (evaluated again once the scratch is exhausted);
+//   * it does not: segments of at most 256 pairs of ONE source row (pair indices in the stash are
+//     8 bit), each walked once per tile of the table; the edges of a row then come tile by tile,
+//     the row stays contiguous (canonical order inside a row is not kept).
+// Hits go to the stash (pair indices relative to E.qb0) and are written out when it is full, when
+// the pair index would overflow, and at the end of a segment: the pass q0 >= rb of the block loop
+// only flushes (one flush site).
+template <int MW>
+__device__ __forceinline__ void mg_emit_struct(EmitSmem &se, const CutoffArgs &A, const Task &k, const FindCtx &F,
+                                               EmitCtx &E, int qa, int qb, const unsigned *wmask, int &midx,
+                                               int lane) {
+    WarpSmem &sw = se.w;
     const int N = k.natoms;
     const float inv_N = 1.f / (float)N;
-    unsigned nmask[W];                       // masks of the next block, loaded one block ahead
-    bool nhave = scratch && qa < qb && midx + 32 * W <= MG_MASK_WORDS;
+    const bool tiled = F.mloc > MG_TLOC;
+    for (int ra = qa; ra < qb;) {
+        int rb = qb;
+        if (tiled) rb = min(min(qb, (ra / N + 1) * N), ra + 256);
+        E.qb0 = ra;
+        for (int tile0 = 0; tile0 < F.mloc; tile0 += MG_TLOC) {
+            const int ncl = min(MG_TLOC, F.mloc - tile0), nW = (ncl + 31) >> 5;
+            const bool last_tile = tile0 + MG_TLOC >= F.mloc;
+            if (tiled) mg_warp_table(sw, F.a, (F.m >> 8) & 0xFF, (F.m >> 16) & 0xFF, F.mloc, tile0, lane);
+            unsigned nmask[MW];                   // masks of the next block, loaded one block ahead
+            bool nhave = !tiled && midx + 32 * nW <= MG_MASK_WORDS;
 #pragma unroll
-    for (int w = 0; w < W; ++w) nmask[w] = nhave ? __ldg(wmask + midx + 32 * w + lane) : 0u;
-    for (int q0 = qa; q0 < qb; q0 += 32) {
-        const int q = q0 + lane;
-        const bool valid = q < qb;
-        int i = 0, j = 0;
-        long long t0_ = 0;
-#ifdef MG_PHASE_CLOCKS
-        t0_ = clock64();
-#endif
-        if (valid) mg_qsplit(q, N, inv_N, i, j);
-        const PairLane p = mg_pair_setup(sw, F, valid, i, j);
-        unsigned mask[W];
-        if (nhave) {
+            for (int w = 0; w < MW; ++w) nmask[w] = nhave && w < nW ? __ldg(wmask + midx + 32 * w + lane) : 0u;
+            for (int q0 = ra;; q0 += 32) {
+                const bool last = q0 >= rb;      // flush-only pass
+                const int q = q0 + lane;
+                const bool valid = q < rb;
+                int i = 0, j = 0, cnt = 0, tot = 0, incl = 0;
+                unsigned mask[MW];
+                PairLane p;
+                if (!last) {
+                    MG_TIC
+                    if (valid) mg_qsplit(q, N, inv_N, i, j);
+                    p = mg_pair_setup(sw, F, valid, i, j);
 #pragma unroll
-            for (int w = 0; w < W; ++w) mask[w] = nmask[w];
-        } else {
-            mg_block_masks<W>(sw, F, p, k.first + i, k.first + j, tile0, ncl, mask);
+                    for (int w = 0; w < MW; ++w) mask[w] = nmask[w];
+                    if (!nhave) {
+#pragma unroll 1
+                        for (int w = 0; w < nW; ++w) {
+                            const unsigned m = mg_word_mask(sw, F, p, k.first + i, k.first + j, tile0, w, ncl);
+#pragma unroll
+                            for (int x = 0; x < MW; ++x)
+                                if (x == w) mask[x] = m;
+                        }
+                    }
+                    if (!tiled) {
+                        midx += 32 * nW;
+                        nhave = q0 + 32 < rb && midx + 32 * nW <= MG_MASK_WORDS;
+#pragma unroll
+                        for (int w = 0; w < MW; ++w)
+                            nmask[w] = nhave && w < nW ? __ldg(wmask + midx + 32 * w + lane) : 0u;
+                    }
+#pragma unroll
+                    for (int w = 0; w < MW; ++w) {
+                        if (w >= nW) break;
+                        cnt += __popc(mask[w]);
+                    }
+                    incl = cnt;                  // inclusive scan of the lanes' hit counts
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const int v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+                        if (lane >= o) incl += v;
+                    }
+                    tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
+                    MG_TOC(0)
+                }
+                // a block with more hits than the stash holds goes in several passes of consecutive
+                // lanes (a lane has at most 256 hits): done = hits of the lanes already written
+                const bool split = tot > MG_STASH;
+                for (int done = 0, l0 = 0;;) {
+                    bool mine = true;
+                    int c = cnt, t = tot;
+                    if (split) {                 // rare
+                        mine = lane >= l0 && incl - done <= MG_STASH;
+                        const int nl = __popc(__ballot_sync(0xFFFFFFFFu, mine));
+                        t = __shfl_sync(0xFFFFFFFFu, incl, l0 + nl - 1) - done;
+                        c = mine ? cnt : 0;
+                        l0 += nl;
+                    }
+                    const bool full = E.run + t > MG_STASH || (!tiled && q0 + 32 - E.qb0 > 256);
+                    if (last ? (last_tile && E.run > 0) : full) {              // write the stash out
+                        __syncwarp();
+                        { MG_TIC mg_flush(se, A, k, E, E.run, E.qb0, inv_N, lane); MG_TOC(2) }
+                        __syncwarp();
+                        E.goff += E.run;
+                        E.run = 0;
+                        if (!tiled) E.qb0 = q0;
+                    }
+                    if (last) break;
+                    int pos = E.run + incl - cnt - done;
+                    if (valid && j == 0 && tile0 == 0 && mine)
+                        A.row_ptr[k.first + i] = (int)(E.goff + pos);
+                    const unsigned paircode = ((unsigned)(p.l0 + 128) << 24) | ((unsigned)(p.l1 + 128) << 16) |
+                                              ((unsigned)(p.l2 + 128) << 8) | (unsigned)(q - E.qb0);
+                    { MG_TIC
+#pragma unroll
+                    for (int w = 0; w < MW; ++w) {
+                        if (w >= nW) break;
+                        unsigned mk = mine ? mask[w] : 0u;
+                        while (mk) {
+                            const int b = __ffs(mk) - 1;
+                            mk &= mk - 1;
+                            se.stash[pos++] = paircode + sw.tcode[32 * w + b];
+                        }
+                    }
+                    MG_TOC(1) }
+                    E.run += t;
+                    done += t;
+                    if (done >= tot) break;
+                }
+                if (last) break;
+            }
         }
-        if (scratch) {
-            midx += 32 * W;
-            nhave = q0 + 32 < qb && midx + 32 * W <= MG_MASK_WORDS;
+        ra = rb;
+    }
+}
+
+// Emit for structures with one candidate image per pair (mloc == 1): 32 blocks (1024 pairs) at a
+// time, one ballot word per lane; the hits are expanded into a list and then LANES <-> HITS, so the
+// per-pair work (cell offsets, FP64 vec) is done for the edges only and the stores are coalesced.
+// Returns the edge offset after the segment; the caller advances midx by ceil((qb - qa) / 32).
+__device__ __forceinline__ long long mg_emit_single(EmitSmem &se, const CutoffArgs &A, const CutRec *R, int s, int qa,
+                                                 int qb, const unsigned *wmask, int midx, long long goff, int lane) {
+    WarpSmem &sw = se.w;
+    Task k;
+    FindCtx F;
+    if (!mg_struct_setup(sw, se.pd, A.pos, A.lattice, A.status, A.r_c, R, s, k, F, lane)) {
+        const int N0 = R->natoms;                  // no edges: rows that start in [qa, qb)
+        for (int i = (qa + N0 - 1) / N0 + lane; i * N0 < qb; i += 32) A.row_ptr[R->first + i] = (int)goff;
+        return goff;
+    }
+    double Ld[9];
 #pragma unroll
-            for (int w = 0; w < W; ++w) nmask[w] = nhave ? __ldg(wmask + midx + 32 * w + lane) : 0u;
+    for (int c = 0; c < 9; ++c) Ld[c] = (double)F.a[c];
+    const int N = k.natoms;
+    const float inv_N = 1.f / (float)N;
+    for (int g0 = qa; g0 < qb; g0 += 1024) {
+        const int gend = min(qb, g0 + 1024), nb = (gend - g0 + 31) >> 5;
+        unsigned word = 0u;
+        if (midx + nb <= MG_MASK_WORDS) {
+            if (lane < nb) word = __ldg(wmask + midx + lane);
+        } else {                                   // scratch exhausted in the count launch: evaluate again
+            for (int b = 0; b < nb; ++b) {
+                const unsigned wb = mg_single_word(sw, A, k, F, g0 + 32 * b, qb, inv_N, false, lane);
+                if (lane == b) word = wb;
+            }
         }
-        int cnt = 0;
-#pragma unroll
-        for (int w = 0; w < W; ++w) cnt += __popc(mask[w]);
+        midx += nb;
+        const int cnt = __popc(word);
         int incl = cnt;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             const int v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
             if (lane >= o) incl += v;
         }
-        const int tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
-#ifdef MG_PHASE_CLOCKS
-        E.tc[0] += clock64() - t0_;
-#endif
-        (void)t0_;
-        if (E.run + tot > MG_STASH || (!pinned && q0 + 32 - E.qb0 > 256)) {   // stash full: write it out
-            __syncwarp();
-            { MG_TIC mg_flush(se, A, k, E, E.run, E.qb0, inv_N, lane); MG_TOC(2) }
-            __syncwarp();
-            E.goff += E.run;
-            E.run = 0;
-            if (!pinned) E.qb0 = q0;
+        const int excl = incl - cnt, T = __shfl_sync(0xFFFFFFFFu, incl, 31);
+        // row_ptr of the source rows whose first pair lies in this group
+        for (int r0 = (g0 + N - 1) / N; r0 * N < gend; r0 += 32) {
+            const int r = r0 + lane;
+            const bool act = (long long)r * N < gend;
+            const int qr = act ? r * N - g0 : 0;
+            const unsigned wv = __shfl_sync(0xFFFFFFFFu, word, qr >> 5);
+            const int ev = __shfl_sync(0xFFFFFFFFu, excl, qr >> 5);
+            if (act) A.row_ptr[k.first + r] = (int)(goff + ev + __popc(wv & ((1u << (qr & 31)) - 1u)));
         }
-        int pos = E.run + incl - cnt;
-        if (valid && j == 0 && tile0 == 0) A.row_ptr[k.first + i] = (int)(E.goff + pos);
-        if (tot > MG_STASH) {                                     // one block alone overflows (run == 0)
-            mg_direct_block<W>(sw, se.pd, A, k, E, p, i, j, mask, E.goff + pos);
-            E.goff += tot;
-            if (!pinned) E.qb0 = q0 + 32;
-            continue;
-        }
-        const unsigned paircode = ((unsigned)(p.l0 + 128) << 24) | ((unsigned)(p.l1 + 128) << 16) |
-                                  ((unsigned)(p.l2 + 128) << 8) | (unsigned)(q - E.qb0);
-        if (valid) se.pairij[q - E.qb0] = ((unsigned)i << 16) | (unsigned)j;
-        { MG_TIC
-#pragma unroll
-        for (int w = 0; w < W; ++w) {
-            unsigned mk = mask[w];
+        // hit list: pair indices relative to g0, in (i, j) order
+        __syncwarp();
+        {
+            unsigned mk = word;
+            int pos = excl;
             while (mk) {
                 const int b = __ffs(mk) - 1;
                 mk &= mk - 1;
-                se.stash[pos++] = paircode + sw.tcode[32 * w + b];
+                se.stash[pos++] = (unsigned)(32 * lane + b);
             }
         }
-        MG_TOC(1) }
-        E.run += tot;
-    }
-}
-
-__device__ __forceinline__ void mg_flush_all(EmitSmem &se, const CutoffArgs &A, const Task &k, EmitCtx &E, int lane) {
-    __syncwarp();
-    { MG_TIC mg_flush(se, A, k, E, E.run, E.qb0, 1.f / (float)k.natoms, lane); MG_TOC(2) }
-    __syncwarp();
-    E.goff += E.run;
-    E.run = 0;
-}
-
-// Structures whose table does not fit (mloc > MG_TLOC): one source row at a time (its edges may
-// come in any order), tile by tile.
-__device__ __forceinline__ void mg_emit_tiled(EmitSmem &se, const CutoffArgs &A, const Task &k, const FindCtx &F,
-                                           EmitCtx &E, int qa, int qb, int lane) {
-    WarpSmem &sw = se.w;
-    const int N = k.natoms;
-    int dummy = 0;
-    for (int i = qa / N; i * N < qb; ++i) {
-        const int ra0 = max(qa, i * N), rb0 = min(qb, (i + 1) * N);
-        for (int ra = ra0; ra < rb0; ra += 256) {                  // pair indices in the stash are 8 bit
-            const int rb = min(rb0, ra + 256);
-            E.qb0 = ra;
-            for (int tile0 = 0; tile0 < F.mloc; tile0 += MG_TLOC) {
-                mg_warp_table(sw, F.a, (F.m >> 8) & 0xFF, (F.m >> 16) & 0xFF, F.mloc, tile0, lane);
-                mg_emit_blocks<8>(se, A, k, F, E, ra, rb, tile0, min(MG_TLOC, F.mloc - tile0), false, true, nullptr,
-                                  dummy, lane);
+        __syncwarp();
+        const long long room = A.capacity - goff;
+        const int lim = room >= T ? T : (room > 0 ? (int)room : 0);
+        for (int h = lane; h < lim; h += 32) {
+            const int q = g0 + (int)se.stash[h];
+            int i, j;
+            mg_qsplit(q, N, inv_N, i, j);
+            const PairLane p = mg_pair_setup(sw, F, true, i, j);         // tau = first (only) cell of the pair
+            double pib[3], pjb[3];
+            const double *pi = se.pd[F.big ? 0 : i], *pj = se.pd[F.big ? 0 : j];
+            if (F.big) {
+                mg_pd_big(F.gx, Ld, i, pib);
+                mg_pd_big(F.gx, Ld, j, pjb);
+                pi = pib;
+                pj = pjb;
             }
-            mg_flush_all(se, A, k, E, lane);
+            mg_emit_edge(A, goff + h, k.first + i, k.first + j, pi, pj, Ld, (unsigned)(p.l0 + 128),
+                         (unsigned)(p.l1 + 128), (unsigned)(p.l2 + 128));
         }
+        __syncwarp();
+        goff += T;
     }
+    return goff;
 }
 
-__global__ void __launch_bounds__(MG_BLOCK, 4)
-mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
-    mg_grid_dependency_wait();
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    EmitSmem &se = reinterpret_cast<EmitSmem *>(smem_raw)[warp];
+__device__ __forceinline__ void mg_emit_ranges(EmitSmem &se, const CutoffArgs &A, const RangeCtx &RC, int wid,
+                                               int lane) {
     WarpSmem &sw = se.w;
-    // consecutive ranges (often parts of one expensive structure) go to different SMs
-    const int wid = warp * gridDim.x + blockIdx.x;
-    const long long t_begin = clock64();
-    RangeCtx RC;
-    mg_range_init(RC, A.rec, A.bpre, A.n_blocks, A.n_struct, A.n_ranges, lane);
     for (int w = wid; w < A.n_ranges;) {
         int w_next = 0;
         if (lane == 0) w_next = (int)atomicAdd(A.ctl + 8, 1u) + A.n_warps;
@@ -810,7 +935,10 @@ mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
             if (!mg_segment(RC, R, s, qa, c1, qb)) break;
             Task k;
             FindCtx F;
-            if (qb > qa) {
+            if (qb > qa && R->mloc == 1) {
+                E.goff = mg_emit_single(se, A, R, s, qa, qb, wmask, midx, E.goff, lane);
+                midx += (qb - qa + 31) >> 5;
+            } else if (qb > qa) {
                 bool live_;
                 { MG_TIC live_ = mg_struct_setup(sw, se.pd, A.pos, A.lattice, A.status, A.r_c, R, s, k, F, lane); MG_TOC(3) }
                 if (!live_) {
@@ -823,12 +951,9 @@ mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
                     E.qb0 = qa;
                     E.gx = F.gx;
                     E.big = F.big;
-                    if (F.mloc <= 32) mg_emit_blocks<1>(se, A, k, F, E, qa, qb, 0, F.mloc, true, false, wmask, midx, lane);
-                    else if (F.mloc <= 64) mg_emit_blocks<2>(se, A, k, F, E, qa, qb, 0, F.mloc, true, false, wmask, midx, lane);
-                    else if (F.mloc <= 128) mg_emit_blocks<4>(se, A, k, F, E, qa, qb, 0, F.mloc, true, false, wmask, midx, lane);
-                    else if (F.mloc <= MG_TLOC) mg_emit_blocks<8>(se, A, k, F, E, qa, qb, 0, F.mloc, true, false, wmask, midx, lane);
-                    else mg_emit_tiled(se, A, k, F, E, qa, qb, lane);
-                    mg_flush_all(se, A, k, E, lane);
+                    if (F.mloc <= 32) mg_emit_struct<1>(se, A, k, F, E, qa, qb, wmask, midx, lane);
+                    else if (F.mloc <= 64) mg_emit_struct<2>(se, A, k, F, E, qa, qb, wmask, midx, lane);
+                    else mg_emit_struct<8>(se, A, k, F, E, qa, qb, wmask, midx, lane);
                 }
             }
             if (qb < R->natoms * R->natoms) break;
@@ -838,6 +963,20 @@ mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
 #endif
         w = __shfl_sync(0xFFFFFFFFu, w_next, 0);
     }
+}
+
+__global__ void __launch_bounds__(MG_BLOCK, 4)
+mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
+    mg_grid_dependency_wait();
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    EmitSmem &se = reinterpret_cast<EmitSmem *>(smem_raw)[warp];
+    // consecutive ranges (often parts of one expensive structure) go to different SMs
+    const int wid = warp * gridDim.x + blockIdx.x;
+    const long long t_begin = clock64();
+    RangeCtx RC;
+    mg_range_init(RC, A.rec, A.bpre, A.n_blocks, A.n_struct, A.n_ranges, lane);
+    mg_emit_ranges(se, A, RC, wid, lane);
     if (lane == 0) A.wclock[A.n_warps + wid] = (unsigned)(clock64() - t_begin);
     // last CTA out resets the ticket for the next launch
     __syncthreads();
