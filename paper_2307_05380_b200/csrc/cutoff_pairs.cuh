@@ -44,6 +44,7 @@ struct CutoffArgs {
     int n_warps;                   // warps of the grid
     int n_ranges;                  // MG_OVER * n_warps ranges (MG_OVER = 1: one per warp; more were slower)
     unsigned *wtotal;              // [n_ranges + 1] edges per range -> exclusive scan
+    unsigned *gtotal;              // [64] edges per group of ceil(n_ranges / 64) ranges (zero between calls)
     int2 *wstart;                  // [n_ranges] first (structure, pair) of each range
     unsigned *wmask;               // [n_ranges, MG_MASK_WORDS] hit masks kept from count to emit
     unsigned *wclock;              // [2, n_warps] cycles each warp spent in count / emit (tuning aid)
@@ -196,6 +197,7 @@ __device__ __forceinline__ void mg_warp_table(WarpSmem &sw, const float a[9], in
     const int M12 = m1 * m2;
     const float inv12 = 1.f / (float)M12, inv2 = 1.f / (float)m2;
     __syncwarp();
+#pragma unroll 1
     for (int cc = 0; cc < MG_TLOC && (cc == 0 || tile0 + cc < mloc); cc += 32) {
         const int c = cc + lane, cell = tile0 + c;
         float4 T = make_float4(1e18f, 1e18f, 1e18f, 0.f);
@@ -568,7 +570,10 @@ __device__ __forceinline__ void mg_count_ranges(WarpSmem &sw, const CutoffArgs &
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) total += __shfl_xor_sync(0xFFFFFFFFu, total, o);
-        if (lane == 0) A.wtotal[w] = total;
+        if (lane == 0) {
+            A.wtotal[w] = total;
+            atomicAdd(A.gtotal + w / ((A.n_ranges + 63) >> 6), total);
+        }
         w = __shfl_sync(0xFFFFFFFFu, w_next, 0);
     }
 }
@@ -618,6 +623,7 @@ mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
         A.ctl[0] = 0u;
         A.ctl[1] = 0u;
     }
+    if (threadIdx.x < 64) A.gtotal[threadIdx.x] = 0u;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -629,7 +635,8 @@ struct EmitCtx {
     const float *gx;       // positions of the structure's first atom
     bool big;              // positions are not staged: FP64 cartesian positions on the fly
 #ifdef MG_PHASE_CLOCKS
-    long long tc[4];       // cycles: pair setup + masks + scan, extraction, flush, structure setup
+    long long tc[6];       // cycles: pair setup + masks + scan, extraction, flush, structure setup,
+                           // range prologue, segment bounds
 #endif
 };
 #ifdef MG_PHASE_CLOCKS
@@ -905,6 +912,9 @@ __device__ __forceinline__ void mg_emit_ranges(EmitSmem &se, const CutoffArgs &A
     WarpSmem &sw = se.w;
     for (int w = wid; w < A.n_ranges;) {
         int w_next = 0;
+#ifdef MG_PHASE_CLOCKS
+        const long long t_range = clock64();
+#endif
         if (lane == 0) w_next = (int)atomicAdd(A.ctl + 8, 1u) + A.n_warps;
         unsigned long long c0, c1;
         mg_warp_range(RC, w, c0, c1);
@@ -914,11 +924,14 @@ __device__ __forceinline__ void mg_emit_ranges(EmitSmem &se, const CutoffArgs &A
         int midx = 0;
         EmitCtx E;
 #ifdef MG_PHASE_CLOCKS
-        E.tc[0] = E.tc[1] = E.tc[2] = E.tc[3] = 0;
+        E.tc[0] = E.tc[1] = E.tc[2] = E.tc[3] = E.tc[4] = E.tc[5] = 0;
 #endif
         {   // device-wide scan of K4, consumer side: edges of the ranges before this one
+            // (group totals + the ranges of the own group: 4 independent loads per lane)
             unsigned long long before = 0ull;
-            for (int c = lane; c < w; c += 32) before += __ldg(A.wtotal + c);
+            const int gs = (A.n_ranges + 63) >> 6, g = w / gs;
+            for (int x = lane; x < g; x += 32) before += __ldg(A.gtotal + x);
+            for (int c = g * gs + lane; c < w; c += 32) before += __ldg(A.wtotal + c);
 #pragma unroll
             for (int o = 16; o > 0; o >>= 1) before += __shfl_xor_sync(0xFFFFFFFFu, before, o);
             E.goff = (long long)before;
@@ -929,10 +942,15 @@ __device__ __forceinline__ void mg_emit_ranges(EmitSmem &se, const CutoffArgs &A
                 if (tot > 0x7FFFFFFFull || (long long)tot > A.capacity) atomicOr(A.status, MGS_CAPACITY);
             }
         }
+#ifdef MG_PHASE_CLOCKS
+        E.tc[4] = clock64() - t_range;
+#endif
         for (; s < A.n_struct; ++s, qa = 0) {
             const CutRec *R = A.rec + s;
             int qb;
-            if (!mg_segment(RC, R, s, qa, c1, qb)) break;
+            bool more_;
+            { MG_TIC more_ = mg_segment(RC, R, s, qa, c1, qb); MG_TOC(5) }
+            if (!more_) break;
             Task k;
             FindCtx F;
             if (qb > qa && R->mloc == 1) {
@@ -951,15 +969,14 @@ __device__ __forceinline__ void mg_emit_ranges(EmitSmem &se, const CutoffArgs &A
                     E.qb0 = qa;
                     E.gx = F.gx;
                     E.big = F.big;
-                    if (F.mloc <= 32) mg_emit_struct<1>(se, A, k, F, E, qa, qb, wmask, midx, lane);
-                    else if (F.mloc <= 64) mg_emit_struct<2>(se, A, k, F, E, qa, qb, wmask, midx, lane);
+                    if (F.mloc <= 64) mg_emit_struct<2>(se, A, k, F, E, qa, qb, wmask, midx, lane);
                     else mg_emit_struct<8>(se, A, k, F, E, qa, qb, wmask, midx, lane);
                 }
             }
             if (qb < R->natoms * R->natoms) break;
         }
 #ifdef MG_PHASE_CLOCKS
-        if (lane == 0) for (int x = 0; x < 4; ++x) A.wmask[(size_t)w * MG_MASK_WORDS + MG_MASK_WORDS - 4 + x] = (unsigned)E.tc[x];
+        if (lane == 0) for (int x = 0; x < 6; ++x) A.wmask[(size_t)w * MG_MASK_WORDS + MG_MASK_WORDS - 6 + x] = (unsigned)E.tc[x];
 #endif
         w = __shfl_sync(0xFFFFFFFFu, w_next, 0);
     }
@@ -982,6 +999,10 @@ mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
     __syncthreads();
     if (threadIdx.x == 0) {
         __threadfence();
-        if (atomicAdd(A.ctl + 9, 1u) == gridDim.x - 1) { A.ctl[8] = 0u; A.ctl[9] = 0u; }
+        if (atomicAdd(A.ctl + 9, 1u) == gridDim.x - 1) {
+            A.ctl[8] = 0u;
+            A.ctl[9] = 0u;
+            for (int x = 0; x < 64; ++x) A.gtotal[x] = 0u;
+        }
     }
 }

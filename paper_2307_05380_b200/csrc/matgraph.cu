@@ -26,7 +26,7 @@ struct mg_ctx {
     size_t rec_cap = 0;
     int32_t *d_atom_struct = nullptr;     // [n_atoms]
     size_t atom_cap = 0;
-    unsigned *d_wtotal = nullptr;         // [n_warps + 1] cutoff edges per warp / their exclusive scan
+    unsigned *d_wtotal = nullptr;         // [n_warps + 1] cutoff edges per warp / their exclusive scan, [64] group totals
     int2 *d_wstart = nullptr;             // [n_warps] first (structure, pair) of each warp's range
     unsigned *d_wclock = nullptr;         // [2, n_warps] per-warp cycles of the last cutoff call
     unsigned *d_wmask = nullptr;          // [n_warps, MG_MASK_WORDS] hit masks kept from count to emit
@@ -119,7 +119,8 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
     {
         const int occ = c->cutoff_occ < c->count_occ ? c->cutoff_occ : c->count_occ;
         c->cut_warps = c->sm_count * occ * MG_WARPS;
-        if (occ >= 1 && (cudaMalloc(&c->d_wtotal, (MG_OVER * c->cut_warps + 1) * sizeof(unsigned)) != cudaSuccess ||
+        if (occ >= 1 && (cudaMalloc(&c->d_wtotal, (MG_OVER * c->cut_warps + 1 + 64) * sizeof(unsigned)) != cudaSuccess ||
+                         cudaMemset(c->d_wtotal, 0, (MG_OVER * c->cut_warps + 1 + 64) * sizeof(unsigned)) != cudaSuccess ||
                          cudaMalloc(&c->d_wstart, MG_OVER * c->cut_warps * sizeof(int2)) != cudaSuccess ||
                          cudaMalloc(&c->d_wmask, (size_t)MG_OVER * c->cut_warps * MG_MASK_WORDS * sizeof(unsigned)) != cudaSuccess ||
                          cudaMalloc(&c->d_wclock, 8 * (size_t)c->cut_warps * sizeof(unsigned)) != cudaSuccess)) { mg_destroy(c); return MG_ERR_CUDA; }
@@ -328,7 +329,7 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
     A.row_ptr = o->row_ptr; A.src = o->src; A.dst = o->dst; A.offset = o->offset;
     A.vec = o->vec; A.dist = o->dist; A.capacity = o->capacity; A.n_edges = (long long *)o->n_edges;
     A.rec = c->d_crec; A.bpre = c->d_bpre; A.n_blocks = n_blocks;
-    A.wtotal = c->d_wtotal; A.wstart = c->d_wstart; A.wmask = c->d_wmask; A.wclock = c->d_wclock;
+    A.wtotal = c->d_wtotal; A.gtotal = c->d_wtotal + MG_OVER * c->cut_warps + 1; A.wstart = c->d_wstart; A.wmask = c->d_wmask; A.wclock = c->d_wclock;
     A.ctl = c->d_ctl; A.status = c->d_ctl + 4;
     A.count_only = count_only;
     // one contiguous range of rows per warp; small batches use fewer warps (>= 1 row each)
