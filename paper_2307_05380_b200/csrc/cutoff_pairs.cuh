@@ -62,7 +62,7 @@ struct CutoffArgs {
 #define MG_MASK_WORDS 4096         // per-warp mask scratch (32-bit words, multiple of 128)
 
 struct WarpSmem {
-    float4 T[MG_TLOC];             // t . L (xyz), w unused
+    float4 T[MG_TLOC];             // t . L: planes x | y | z of MG_TLOC floats (mg_tplane); the rest is unused
     unsigned tcode[MG_TLOC];       // (t0 << 24 | t1 << 16 | t2 << 8)
     float4 x[MG_SMALL_MAX_ATOMS];  // wrapped fractional coordinates, .w = packed integer parts
 };
@@ -190,6 +190,41 @@ __device__ __forceinline__ bool mg_warp_stage(WarpSmem &sw, double (*pd)[3], con
     return ok;
 }
 
+// The table of translations is stored as three planes (x | y | z, MG_TLOC floats each) inside
+// WarpSmem::T: four consecutive cells of one component are one LDS.128, and two cells go through
+// one packed FP32 instruction (add / fma .f32x2 of sm_100: each half rounds like the scalar
+// instruction, so the masks are those of the scalar filter).
+__device__ __forceinline__ const float *mg_tplane(const WarpSmem &sw, int a) {
+    return reinterpret_cast<const float *>(sw.T) + a * MG_TLOC;
+}
+__device__ __forceinline__ float4 mg_tcell(const WarpSmem &sw, int c) {
+    return make_float4(mg_tplane(sw, 0)[c], mg_tplane(sw, 1)[c], mg_tplane(sw, 2)[c], 0.f);
+}
+__device__ __forceinline__ float2 mg_add2(float2 a, float2 b) {
+    float2 r;
+    asm("{\n\t.reg .b64 x, y, z;\n\tmov.b64 x, {%2, %3};\n\tmov.b64 y, {%4, %5};\n\tadd.rn.f32x2 z, x, y;\n\t"
+        "mov.b64 {%0, %1}, z;\n\t}"
+        : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return r;
+}
+__device__ __forceinline__ float2 mg_fma2(float2 a, float2 b, float2 c) {
+    float2 r;
+    asm("{\n\t.reg .b64 x, y, z, w;\n\tmov.b64 x, {%2, %3};\n\tmov.b64 y, {%4, %5};\n\tmov.b64 z, {%6, %7};\n\t"
+        "fma.rn.f32x2 w, x, y, z;\n\tmov.b64 {%0, %1}, w;\n\t}"
+        : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y), "f"(c.x), "f"(c.y));
+    return r;
+}
+// y = |q + T|^2 - r^2 of four consecutive cells (operation order of the scalar filter).
+__device__ __forceinline__ void mg_filter4(const float4 X, const float4 Y, const float4 Z, float2 qx, float2 qy,
+                                           float2 qz, float2 nr2, float (&y)[4]) {
+    const float2 vx0 = mg_add2(qx, make_float2(X.x, X.y)), vx1 = mg_add2(qx, make_float2(X.z, X.w));
+    const float2 vy0 = mg_add2(qy, make_float2(Y.x, Y.y)), vy1 = mg_add2(qy, make_float2(Y.z, Y.w));
+    const float2 vz0 = mg_add2(qz, make_float2(Z.x, Z.y)), vz1 = mg_add2(qz, make_float2(Z.z, Z.w));
+    const float2 y0 = mg_fma2(vz0, vz0, mg_fma2(vy0, vy0, mg_fma2(vx0, vx0, nr2)));
+    const float2 y1 = mg_fma2(vz1, vz1, mg_fma2(vy1, vy1, mg_fma2(vx1, vx1, nr2)));
+    y[0] = y0.x; y[1] = y0.y; y[2] = y1.x; y[3] = y1.y;
+}
+
 // Local translations of cells [tile0, tile0 + MG_TLOC) of the per-pair sub-box m0 x m1 x m2:
 // T = t . L in FP32, tcode = packed t; the tail is padded with a far-away sentinel.
 __device__ __forceinline__ void mg_warp_table(WarpSmem &sw, const float a[9], int m1, int m2, int mloc,
@@ -212,7 +247,8 @@ __device__ __forceinline__ void mg_warp_table(WarpSmem &sw, const float a[9], in
             T.z = __fmaf_rn(f2, a[8], __fmaf_rn(f1, a[5], __fmul_rn(f0, a[2])));
             code = ((unsigned)t0 << 24) | ((unsigned)t1 << 16) | ((unsigned)t2 << 8);
         }
-        sw.T[c] = T;
+        float *tp = reinterpret_cast<float *>(sw.T);
+        tp[c] = T.x; tp[MG_TLOC + c] = T.y; tp[2 * MG_TLOC + c] = T.z;
         sw.tcode[c] = code;
     }
     __syncwarp();
@@ -250,17 +286,19 @@ __device__ __forceinline__ void mg_pair_masks(const WarpSmem &sw, const FindCtx 
     for (int w = 0; w < W; ++w) {
         mask[w] = 0u;
         const int n4 = min(8, max(0, (ncl - 32 * w + 3) >> 2));      // warp-uniform
-        const float4 *Tp = sw.T + 32 * w;
+        const float4 *Xp = reinterpret_cast<const float4 *>(mg_tplane(sw, 0) + 32 * w);
+        const float4 *Yp = reinterpret_cast<const float4 *>(mg_tplane(sw, 1) + 32 * w);
+        const float4 *Zp = reinterpret_cast<const float4 *>(mg_tplane(sw, 2) + 32 * w);
 #pragma unroll 1                  // a loop, not 8 copies: the kernels are bound by instruction fetch
         for (int g = 0; g < n4; ++g) {
             unsigned sub = 0u;
+            float y[4];
+            mg_filter4(Xp[g], Yp[g], Zp[g], make_float2(qx, qx), make_float2(qy, qy), make_float2(qz, qz),
+                       make_float2(nr2, nr2), y);
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
-                const float4 T = Tp[4 * g + c];
-                const float vx = __fadd_rn(qx, T.x), vy = __fadd_rn(qy, T.y), vz = __fadd_rn(qz, T.z);
-                const float y = __fmaf_rn(vz, vz, __fmaf_rn(vy, vy, __fmaf_rn(vx, vx, nr2)));
-                if (y < win) sub |= 1u << c;
-                near = near || fabsf(y) < win;
+                if (y[c] < win) sub |= 1u << c;
+                near = near || fabsf(y[c]) < win;
             }
             mask[w] |= sub << (4 * g);
         }
@@ -268,7 +306,7 @@ __device__ __forceinline__ void mg_pair_masks(const WarpSmem &sw, const FindCtx 
     if (near) {                                   // rare: decide the window cells in FP64
         const float *xi = F.pos + 3 * (size_t)gi, *xj = F.pos + 3 * (size_t)gj;
         for (int c = 0; c < ncl; ++c) {
-            const float4 T = sw.T[c];
+            const float4 T = mg_tcell(sw, c);
             const float vx = __fadd_rn(qx, T.x), vy = __fadd_rn(qy, T.y), vz = __fadd_rn(qz, T.z);
             const float y = __fmaf_rn(vz, vz, __fmaf_rn(vy, vy, __fmaf_rn(vx, vx, nr2)));
             if (fabsf(y) < win) {
@@ -336,7 +374,9 @@ __device__ __forceinline__ unsigned mg_word_mask(const WarpSmem &sw, const FindC
                                                  int gj, int tile0, int w, int ncl) {
     const float nr2 = F.nr2, win = F.win;
     const int nw = min(32, ncl - 32 * w);                        // cells of the word (warp-uniform)
-    const float4 *Tp = sw.T + 32 * w;
+    const float4 *Xp = reinterpret_cast<const float4 *>(mg_tplane(sw, 0) + 32 * w);
+    const float4 *Yp = reinterpret_cast<const float4 *>(mg_tplane(sw, 1) + 32 * w);
+    const float4 *Zp = reinterpret_cast<const float4 *>(mg_tplane(sw, 2) + 32 * w);
     unsigned mask = 0u;
     bool near = false;
     if (nw == 1) {                                               // one image per pair: T_0 = 0
@@ -348,13 +388,13 @@ __device__ __forceinline__ unsigned mg_word_mask(const WarpSmem &sw, const FindC
 #pragma unroll 1
         for (int g = 0; g < n4; ++g) {
             unsigned sub = 0u;
+            float y[4];
+            mg_filter4(Xp[g], Yp[g], Zp[g], make_float2(p.qx, p.qx), make_float2(p.qy, p.qy),
+                       make_float2(p.qz, p.qz), make_float2(nr2, nr2), y);
 #pragma unroll
             for (int c = 0; c < 4; ++c) {
-                const float4 T = Tp[4 * g + c];
-                const float vx = __fadd_rn(p.qx, T.x), vy = __fadd_rn(p.qy, T.y), vz = __fadd_rn(p.qz, T.z);
-                const float y = __fmaf_rn(vz, vz, __fmaf_rn(vy, vy, __fmaf_rn(vx, vx, nr2)));
-                if (y < win) sub |= 1u << c;
-                near = near || fabsf(y) < win;
+                if (y[c] < win) sub |= 1u << c;
+                near = near || fabsf(y[c]) < win;
             }
             mask |= sub << (4 * g);
         }
@@ -362,7 +402,7 @@ __device__ __forceinline__ unsigned mg_word_mask(const WarpSmem &sw, const FindC
     if (near) {                                   // rare: decide the window cells in FP64
         const float *xi = F.pos + 3 * (size_t)gi, *xj = F.pos + 3 * (size_t)gj;
         for (int c = 0; c < nw; ++c) {
-            const float4 T = Tp[c];
+            const float4 T = mg_tcell(sw, 32 * w + c);
             const float vx = __fadd_rn(p.qx, T.x), vy = __fadd_rn(p.qy, T.y), vz = __fadd_rn(p.qz, T.z);
             const float y = __fmaf_rn(vz, vz, __fmaf_rn(vy, vy, __fmaf_rn(vx, vx, nr2)));
             if (fabsf(y) < win) {
