@@ -47,6 +47,7 @@ struct CutoffArgs {
     unsigned *gtotal;              // [64] edges per group of ceil(n_ranges / 64) ranges (zero between calls)
     int2 *wstart;                  // [n_ranges] first (structure, pair) of each range
     unsigned *wmask;               // [n_ranges, MG_MASK_WORDS] hit masks kept from count to emit
+    int mask_words;                // words of a range's scratch that may be used (MG_MASK_WORDS; tests: less)
     unsigned *wclock;              // [2, n_warps] cycles each warp spent in count / emit (tuning aid)
     unsigned *ctl;                 // [0] count ticket, [1] count CTAs done, [8] emit ticket, [9] emit CTAs done
     unsigned *status;
@@ -532,7 +533,7 @@ __device__ __forceinline__ unsigned mg_count_struct(WarpSmem &sw, const CutoffAr
             if (valid) mg_qsplit(q, N, inv_N, i, j);
             const PairLane p = mg_pair_setup(sw, F, valid, i, j);
             if (valid && !p.ok && tile0 == 0) atomicOr(A.status, MGS_OFFSET);
-            const bool keep = !tiled && midx + 32 * nW <= MG_MASK_WORDS;
+            const bool keep = !tiled && midx + 32 * nW <= A.mask_words;
 #pragma unroll 1
             for (int w = 0; w < nW; ++w) {
                 const unsigned m = mg_word_mask(sw, F, p, k.first + i, k.first + j, tile0, w, ncl);
@@ -573,7 +574,7 @@ __device__ __forceinline__ unsigned mg_count_single(WarpSmem &sw, const CutoffAr
         const unsigned word = mg_single_word(sw, A, k, F, q0, qb, inv_N, true, lane);
         if (lane == 0) {
             acc += __popc(word);
-            if (midx < MG_MASK_WORDS) wmask[midx] = word;
+            if (midx < A.mask_words) wmask[midx] = word;
         }
         midx += 1;
     }
@@ -766,7 +767,7 @@ __device__ __forceinline__ void mg_emit_struct(EmitSmem &se, const CutoffArgs &A
             const bool last_tile = tile0 + MG_TLOC >= F.mloc;
             if (tiled) mg_warp_table(sw, F.a, (F.m >> 8) & 0xFF, (F.m >> 16) & 0xFF, F.mloc, tile0, lane);
             unsigned nmask[MW];                   // masks of the next block, loaded one block ahead
-            bool nhave = !tiled && midx + 32 * nW <= MG_MASK_WORDS;
+            bool nhave = !tiled && midx + 32 * nW <= A.mask_words;
 #pragma unroll
             for (int w = 0; w < MW; ++w) nmask[w] = nhave && w < nW ? __ldg(wmask + midx + 32 * w + lane) : 0u;
             for (int q0 = ra;; q0 += 32) {
@@ -793,7 +794,7 @@ __device__ __forceinline__ void mg_emit_struct(EmitSmem &se, const CutoffArgs &A
                     }
                     if (!tiled) {
                         midx += 32 * nW;
-                        nhave = q0 + 32 < rb && midx + 32 * nW <= MG_MASK_WORDS;
+                        nhave = q0 + 32 < rb && midx + 32 * nW <= A.mask_words;
 #pragma unroll
                         for (int w = 0; w < MW; ++w)
                             nmask[w] = nhave && w < nW ? __ldg(wmask + midx + 32 * w + lane) : 0u;
@@ -885,7 +886,7 @@ __device__ __forceinline__ long long mg_emit_single(EmitSmem &se, const CutoffAr
     for (int g0 = qa; g0 < qb; g0 += 1024) {
         const int gend = min(qb, g0 + 1024), nb = (gend - g0 + 31) >> 5;
         unsigned word = 0u;
-        if (midx + nb <= MG_MASK_WORDS) {
+        if (midx + nb <= A.mask_words) {
             if (lane < nb) word = __ldg(wmask + midx + lane);
         } else {                                   // scratch exhausted in the count launch: evaluate again
             for (int b = 0; b < nb; ++b) {

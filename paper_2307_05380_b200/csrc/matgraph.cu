@@ -29,6 +29,7 @@ struct mg_ctx {
     unsigned *d_wtotal = nullptr;         // [n_warps + 1] cutoff edges per warp / their exclusive scan, [64] group totals
     int2 *d_wstart = nullptr;             // [n_warps] first (structure, pair) of each warp's range
     unsigned *d_wclock = nullptr;         // [2, n_warps] per-warp cycles of the last cutoff call
+    int mask_words = 0;                   // usable words of a range's mask scratch (MATGRAPH_MASK_WORDS)
     unsigned *d_wmask = nullptr;          // [n_warps, MG_MASK_WORDS] hit masks kept from count to emit
     int cut_warps = 0, last_cut_warps = 0;
     CutRec *d_crec = nullptr;             // per-structure records of the cutoff path (cut_prep.cuh)
@@ -101,6 +102,12 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
     if (!c) return MG_ERR_CUDA;
     c->device = device;
     c->pdl = getenv("MATGRAPH_NO_PDL") ? 0 : 1;
+    // test knob: a smaller mask scratch per range makes the emit launch evaluate masks again
+    c->mask_words = MG_MASK_WORDS;
+    if (const char *mw = getenv("MATGRAPH_MASK_WORDS")) {
+        const int v = atoi(mw);
+        if (v >= 0 && v <= MG_MASK_WORDS) c->mask_words = v;
+    }
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess || prop.major < 10) { delete c; return MG_ERR_CUDA; }
     c->sm_count = prop.multiProcessorCount;
@@ -329,7 +336,7 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
     A.row_ptr = o->row_ptr; A.src = o->src; A.dst = o->dst; A.offset = o->offset;
     A.vec = o->vec; A.dist = o->dist; A.capacity = o->capacity; A.n_edges = (long long *)o->n_edges;
     A.rec = c->d_crec; A.bpre = c->d_bpre; A.n_blocks = n_blocks;
-    A.wtotal = c->d_wtotal; A.gtotal = c->d_wtotal + MG_OVER * c->cut_warps + 1; A.wstart = c->d_wstart; A.wmask = c->d_wmask; A.wclock = c->d_wclock;
+    A.wtotal = c->d_wtotal; A.gtotal = c->d_wtotal + MG_OVER * c->cut_warps + 1; A.wstart = c->d_wstart; A.wmask = c->d_wmask; A.mask_words = c->mask_words; A.wclock = c->d_wclock;
     A.ctl = c->d_ctl; A.status = c->d_ctl + 4;
     A.count_only = count_only;
     // one contiguous range of rows per warp; small batches use fewer warps (>= 1 row each)

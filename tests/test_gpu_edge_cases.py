@@ -128,6 +128,34 @@ def test_more_than_32_prep_blocks(mg, ctx):
     check.check_knn(b, 8, gk)
 
 
+def test_mask_scratch_exhausted(mg, monkeypatch):
+    # The count launch keeps the hit masks of a range in a fixed scratch (4096 words per warp); a
+    # range with more blocks x words than that is evaluated again by the emit launch.  Real batches
+    # reach this only above ~1e8 edges, so the test shrinks the scratch through the library's knob:
+    # 0 words (everything evaluated twice), 8 and 40 (the switch happens in the middle of a range, for
+    # tables of 1, 2 and up to 8 words per pair) — single-image structures included.
+    small = C.small_batch(48, seed=5)
+    big = C.config_batch(3, n_struct=1, seed=2)
+    b = C.concat([small, big, small])
+    want6 = None
+    for words in ("0", "8", "40", "4096"):
+        monkeypatch.setenv("MATGRAPH_MASK_WORDS", words)
+        c = mg.Context(0)
+        try:
+            for r_c in (3.0, 6.0, 9.0):
+                pos, lat, ptr = mg.to_device(b)
+                got = c.cutoff_graph(pos, lat, ptr, r_c, dist=True).to_numpy()
+                assert c.mg_check() == 0
+                rep = check.check_cutoff(b, r_c, got)
+                assert rep["extra"] == 0 and rep["missing"] == 0
+                if r_c == 6.0:
+                    key = (got["n_edges"], got["row_ptr"].tobytes())
+                    want6 = want6 or key
+                    assert key == want6
+        finally:
+            c.close()
+
+
 def test_capacity_overflow_reports_required_count(mg, ctx):
     b = C.small_batch(16, seed=2)
     full, status = _run_cutoff(mg, ctx, b, 5.0)
