@@ -76,7 +76,12 @@ typedef struct {
 
 /* Context.  `device` is a CUDA ordinal.  mg_reserve grows the scratch workspace for batches of up
  * to (n_struct, n_atoms) outside the hot path; the graph calls grow it themselves when needed
- * (which allocates, hence is not capturable in a CUDA graph the first time). */
+ * (which allocates, hence is not capturable in a CUDA graph the first time).
+ * Environment read by mg_create (diagnostics only; results do not depend on them):
+ *   MATGRAPH_NO_PDL      launch the kernels without programmatic dependent launch;
+ *   MATGRAPH_MASK_WORDS  words (0..4096) of the per-warp hit-mask scratch the cutoff count launch
+ *                        may use; beyond it the emit launch evaluates the masks again (tests);
+ *   MG_DEBUG             print the CUDA error behind an MG_ERR_CUDA to stderr. */
 mg_status mg_create(mg_ctx **ctx, int device);
 void      mg_destroy(mg_ctx *ctx);
 mg_status mg_reserve(mg_ctx *ctx, int32_t n_struct, int32_t n_atoms);
