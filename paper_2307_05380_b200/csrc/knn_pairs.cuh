@@ -268,14 +268,20 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                                 // already in the order (d, dst, tau) the lane is the rank, else rank by counting
                                 const mg_key mine = lane < cnt ? ks.stash[b0 + lane] : MG_KEY_INF;
                                 unsigned sk = lane < cnt ? (((unsigned)(mine >> 32) & ~31u) | (unsigned)lane) : 0xFFFFFFFFu;
+                                // (bitonic network in its "flip" form: every exchange gives the minimum to the
+                                // lower lane, so the 15 directions are 5 lane bits kept in predicates)
 #pragma unroll
-                                for (int k2 = 2; k2 <= 32; k2 <<= 1)
-#pragma unroll
-                                    for (int jj = k2 >> 1; jj > 0; jj >>= 1) {
-                                        const unsigned o = __shfl_xor_sync(0xFFFFFFFFu, sk, jj);
-                                        const bool up = (lane & k2) == 0, lower = (lane & jj) == 0;
-                                        sk = (lower == up) ? min(sk, o) : max(sk, o);
+                                for (int k2 = 2; k2 <= 32; k2 <<= 1) {
+                                    {
+                                        const unsigned o = __shfl_xor_sync(0xFFFFFFFFu, sk, k2 - 1);
+                                        sk = (lane & (k2 >> 1)) == 0 ? min(sk, o) : max(sk, o);
                                     }
+#pragma unroll
+                                    for (int jj = k2 >> 2; jj > 0; jj >>= 1) {
+                                        const unsigned o = __shfl_xor_sync(0xFFFFFFFFu, sk, jj);
+                                        sk = (lane & jj) == 0 ? min(sk, o) : max(sk, o);
+                                    }
+                                }
                                 const unsigned tie = __shfl_sync(0xFFFFFFFFu, (unsigned)mine, (int)(sk & 31u));
                                 const float d2q = __uint_as_float(sk & ~31u);
                                 const float d2k = __shfl_sync(0xFFFFFFFFu, d2q, K - 1);

@@ -45,12 +45,15 @@ __device__ __forceinline__ mg_key mg_kmax(mg_key a, mg_key b) { return a < b ? b
 // ascending bitonic sort of one key per lane
 __device__ __forceinline__ mg_key mg_sort32(mg_key v, int lane) {
 #pragma unroll
-    for (int k2 = 2; k2 <= 32; k2 <<= 1) {
+    for (int k2 = 2; k2 <= 32; k2 <<= 1) {      // "flip" form: the lower lane of every exchange takes the minimum
+        {
+            const mg_key p = __shfl_xor_sync(0xFFFFFFFFu, v, k2 - 1);
+            v = (lane & (k2 >> 1)) == 0 ? mg_kmin(v, p) : mg_kmax(v, p);
+        }
 #pragma unroll
-        for (int j = k2 >> 1; j > 0; j >>= 1) {
+        for (int j = k2 >> 2; j > 0; j >>= 1) {
             const mg_key p = __shfl_xor_sync(0xFFFFFFFFu, v, j);
-            const bool up = (lane & k2) == 0, lower = (lane & j) == 0;
-            v = (lower == up) ? mg_kmin(v, p) : mg_kmax(v, p);
+            v = (lane & j) == 0 ? mg_kmin(v, p) : mg_kmax(v, p);
         }
     }
     return v;
