@@ -37,6 +37,20 @@
 #define MG_C_BLOCK_WIDE 500.f
 #define MG_C_EDGE 3.3f             // per emitted edge
 #endif
+// ... and of the KNN launch: per candidate cell, per block of 32 pairs, per source row (selection),
+// per structure
+#ifndef MG_KC_CELL
+#define MG_KC_CELL 17.f
+#endif
+#ifndef MG_KC_BLOCK
+#define MG_KC_BLOCK 150.f
+#endif
+#ifndef MG_KC_ROW
+#define MG_KC_ROW 250.f
+#endif
+#ifndef MG_KC_STRUCT
+#define MG_KC_STRUCT 1300.f
+#endif
 
 struct CutRec {              // 64 bytes
     float rho[3];            // upper bound of r_c / h_a (plus the guard eps)
@@ -131,9 +145,9 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
             const float perblock = mloc > 256 ? 120.f + 16000.f / (float)N : (mloc > 128 ? MG_C_BLOCK_WIDE : MG_C_BLOCK);
             const float c = ((float)((mloc + 3) & ~3) * percell + perblock) * (1.f / 32.f) + MG_C_EDGE * lam / (float)N +
                             MG_STRUCT_COST / ((float)N * (float)N);
-            // KNN: one launch, no edge stream; selecting k per row costs about 350
-            const float ck = ((float)((mloc + 3) & ~3) * 11.f + 150.f) * (1.f / 32.f) + 350.f / (float)N +
-                             0.5f * MG_STRUCT_COST / ((float)N * (float)N);
+            // KNN: one launch, no edge stream (constants from a sweep over four seeds of config 2 and config 4)
+            const float ck = ((float)((mloc + 3) & ~3) * MG_KC_CELL + MG_KC_BLOCK) * (1.f / 32.f) + MG_KC_ROW / (float)N +
+                             MG_KC_STRUCT / ((float)N * (float)N);
             // (KNN above the staging limit: warp-per-row growing-radius search, about 40 per pair-cell)
             const float ckb = 40.f * (float)mloc / 32.f + 600.f / (float)N;
             r.paircost = (unsigned)fminf(16.f * (A.k > 0 ? (N > MG_SMALL_MAX_ATOMS ? ckb : ck) : c) + 1.f, 16777216.f);
