@@ -49,7 +49,7 @@ struct CutoffArgs {
     unsigned *wmask;               // [n_ranges, MG_MASK_WORDS] hit masks kept from count to emit
     int mask_words;                // words of a range's scratch that may be used (MG_MASK_WORDS; tests: less)
     unsigned *wclock;              // [2, n_warps] cycles each warp spent in count / emit (tuning aid)
-    unsigned *ctl;                 // [0] count ticket, [1] count CTAs done, [8] emit ticket, [9] emit CTAs done
+    unsigned *ctl;                 // [1] count CTAs done (mg_cutoff_count), [9] emit CTAs done
     unsigned *status;
     int count_only;
 };
@@ -59,7 +59,7 @@ struct CutoffArgs {
 #define MG_MODE_STASH 1
 #define MG_MODE_DIRECT 2
 
-#define MG_OVER 1                  // ranges per warp (> 1: the extra ranges go by ticket)
+#define MG_OVER 1                  // ranges per warp (more, handed out by ticket, measured slower: DESIGN.md)
 #define MG_MASK_WORDS 4096         // per-warp mask scratch (32-bit words, multiple of 128)
 
 struct WarpSmem {
@@ -584,9 +584,8 @@ __device__ __forceinline__ unsigned mg_count_single(WarpSmem &sw, const CutoffAr
 // The ranges of one warp.
 __device__ __forceinline__ void mg_count_ranges(WarpSmem &sw, const CutoffArgs &A, const RangeCtx &RC, int wid,
                                                 int lane) {
-    for (int w = wid; w < A.n_ranges;) {
-        int w_next = 0;
-        if (lane == 0) w_next = (int)atomicAdd(A.ctl, 1u) + A.n_warps;     // needed only at the end
+    // one range per warp (n_ranges == n_warps): no ticket, nothing that counts calls
+    for (int w = wid; w < A.n_ranges; w += A.n_warps) {
         unsigned long long c0, c1;
         mg_warp_range(RC, w, c0, c1);
         int s, qa;
@@ -615,7 +614,6 @@ __device__ __forceinline__ void mg_count_ranges(WarpSmem &sw, const CutoffArgs &
             A.wtotal[w] = total;
             atomicAdd(A.gtotal + w / ((A.n_ranges + 63) >> 6), total);
         }
-        w = __shfl_sync(0xFFFFFFFFu, w_next, 0);
     }
 }
 
@@ -661,7 +659,6 @@ mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
         *A.n_edges = (long long)off;
         A.row_ptr[A.n_atoms] = (int)off;
         if (off > 0x7FFFFFFFull || (!A.count_only && (long long)off > A.capacity)) atomicOr(A.status, MGS_CAPACITY);
-        A.ctl[0] = 0u;
         A.ctl[1] = 0u;
     }
     if (threadIdx.x < 64) A.gtotal[threadIdx.x] = 0u;
@@ -951,12 +948,10 @@ __device__ __forceinline__ long long mg_emit_single(EmitSmem &se, const CutoffAr
 __device__ __forceinline__ void mg_emit_ranges(EmitSmem &se, const CutoffArgs &A, const RangeCtx &RC, int wid,
                                                int lane) {
     WarpSmem &sw = se.w;
-    for (int w = wid; w < A.n_ranges;) {
-        int w_next = 0;
+    for (int w = wid; w < A.n_ranges; w += A.n_warps) {
 #ifdef MG_PHASE_CLOCKS
         const long long t_range = clock64();
 #endif
-        if (lane == 0) w_next = (int)atomicAdd(A.ctl + 8, 1u) + A.n_warps;
         unsigned long long c0, c1;
         mg_warp_range(RC, w, c0, c1);
         const int2 st = A.wstart[w];
@@ -1019,7 +1014,6 @@ __device__ __forceinline__ void mg_emit_ranges(EmitSmem &se, const CutoffArgs &A
 #ifdef MG_PHASE_CLOCKS
         if (lane == 0) for (int x = 0; x < 6; ++x) A.wmask[(size_t)w * MG_MASK_WORDS + MG_MASK_WORDS - 6 + x] = (unsigned)E.tc[x];
 #endif
-        w = __shfl_sync(0xFFFFFFFFu, w_next, 0);
     }
 }
 
@@ -1036,12 +1030,11 @@ mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
     mg_range_init(RC, A.rec, A.bpre, A.n_blocks, A.n_struct, A.n_ranges, lane);
     mg_emit_ranges(se, A, RC, wid, lane);
     if (lane == 0) A.wclock[A.n_warps + wid] = (unsigned)(clock64() - t_begin);
-    // last CTA out resets the ticket for the next launch
+    // last CTA out zeroes the group totals for the next call
     __syncthreads();
     if (threadIdx.x == 0) {
         __threadfence();
         if (atomicAdd(A.ctl + 9, 1u) == gridDim.x - 1) {
-            A.ctl[8] = 0u;
             A.ctl[9] = 0u;
             for (int x = 0; x < 64; ++x) A.gtotal[x] = 0u;
         }

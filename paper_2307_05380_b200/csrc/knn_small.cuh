@@ -86,9 +86,12 @@ __device__ __forceinline__ void mg_knn_merge(mg_key (&keys)[KPL], mg_key b, int 
     }
 }
 
-__device__ __forceinline__ mg_key mg_knn_key(float d2, int j, int t0, int t1, int t2) {
-    return ((mg_key)__float_as_uint(d2) << 32) | ((mg_key)(unsigned)j << 24) |
-           ((mg_key)(unsigned)(t0 + 128) << 16) | ((unsigned)(t1 + 128) << 8) | (unsigned)(t2 + 128);
+// Key of the growing-radius search: FP32 d2 bits | j * ncell + c, c the index of the image's cell in
+// the explored box (lexicographic in tau), so that the low word orders like (dst, tau_x, tau_y, tau_z)
+// for structures of any size (an 8-bit dst field would wrap above 256 atoms).  The caller makes sure
+// that natoms * ncell fits 32 bits.
+__device__ __forceinline__ mg_key mg_knn_key(float d2, unsigned tie) {
+    return ((mg_key)__float_as_uint(d2) << 32) | (mg_key)tie;
 }
 
 // FP32 cartesian position of atom j of the structure (x . L, the same arithmetic as the staged copy).
@@ -129,10 +132,10 @@ __device__ inline void mg_knn_source(const KnnArgs &A, const StructRec &R, const
     else Rad = 1.25f * cbrtf(0.2387324f * (float)(k + 1) * R.volume / (float)N);
     mg_key keys[KPL];
     mg_key thr;
-    bool failed = false;
+    bool failed = false, too_big = false;
+    int n[3] = {0, 0, 0};
     for (;;) {
         // ---- box that holds every image with d < Rad
-        int n[3];
         float rsafe = 3.0e38f, M = 0.f;
         bool range_ok = true;
 #pragma unroll
@@ -153,6 +156,7 @@ __device__ inline void mg_knn_source(const KnnArgs &A, const StructRec &R, const
         int nb = 0;
         const int D1 = 2 * n[1] + 1, D2 = 2 * n[2] + 1;
         const int ncell = (2 * n[0] + 1) * D1 * D2;
+        if ((unsigned long long)N * (unsigned long long)ncell > 0xFFFFFFFFull) { too_big = true; break; }
         const float inv12 = 1.f / (float)(D1 * D2), inv2 = 1.f / (float)D2;
         for (int c0 = 0; c0 < ncell; c0 += 32) {
             const int c = c0 + lane;
@@ -177,7 +181,7 @@ __device__ inline void mg_knn_source(const KnnArgs &A, const StructRec &R, const
                 const float d2 = mg_d2(__fsub_rn(pj.x, pi.x), __fsub_rn(pj.y, pi.y),
                                        __fsub_rn(pj.z, pi.z), Tx, Ty, Tz);
                 bool cand = alive && d2 <= thr_d2 && !(home && j == i);
-                const mg_key key = mg_knn_key(d2, j, t0, t1, t2);
+                const mg_key key = mg_knn_key(d2, (unsigned)j * (unsigned)ncell + (unsigned)c);
                 cand = cand && key < thr;
                 const unsigned m = __ballot_sync(0xFFFFFFFFu, cand);
                 if (m) {
@@ -211,17 +215,31 @@ __device__ inline void mg_knn_source(const KnnArgs &A, const StructRec &R, const
         Rad = 1.3f * fmaxf(Rad, rsafe) + 4.f * W;
     }
     if (failed && lane == 0) atomicOr(A.status, MGS_OFFSET);
+    if (too_big) {                                      // natoms * box cells does not fit the key
+        if (lane == 0) atomicOr(A.status, MGS_UNSUPPORTED);
+#pragma unroll
+        for (int s = 0; s < KPL; ++s) keys[s] = MG_KEY_INF;
+    }
+    // tie word -> (j, tau): cell index c = ((t0 + n0) D1 + t1 + n1) D2 + t2 + n2 of the last box
+    const unsigned D1f = 2u * (unsigned)n[1] + 1u, D2f = 2u * (unsigned)n[2] + 1u;
+    const unsigned ncellf = (2u * (unsigned)n[0] + 1u) * D1f * D2f;
     // ---- exact FP64 distance of the selected entries, final order by (d, dst, tau), emit
     double dmax = 0.0;
     double dd[KPL], vv[KPL][3];
+    int jj[KPL], tt[KPL][3];
 #pragma unroll
     for (int s = 0; s < KPL; ++s) {
         const unsigned tie = (unsigned)keys[s];
         const bool valid = 32 * s + lane < k && keys[s] != MG_KEY_INF;
         dd[s] = 1e300;
-        if (valid)
-            dd[s] = mg_exact_vec(xs + 3 * i, xs + 3 * (int)((tie >> 24) & 0xFFu), (int)((tie >> 16) & 0xFFu) - 128,
-                                 (int)((tie >> 8) & 0xFFu) - 128, (int)(tie & 0xFFu) - 128, lat9, vv[s]);
+        jj[s] = 0; tt[s][0] = tt[s][1] = tt[s][2] = 0;
+        if (valid) {
+            const unsigned j = tie / ncellf, c = tie - j * ncellf;
+            const unsigned u0 = c / (D1f * D2f), rem = c - u0 * (D1f * D2f), u1 = rem / D2f;
+            jj[s] = (int)j;
+            tt[s][0] = (int)u0 - n[0]; tt[s][1] = (int)u1 - n[1]; tt[s][2] = (int)(rem - u1 * D2f) - n[2];
+            dd[s] = mg_exact_vec(xs + 3 * i, xs + 3 * jj[s], tt[s][0], tt[s][1], tt[s][2], lat9, vv[s]);
+        }
     }
 #pragma unroll
     for (int s = 0; s < KPL; ++s) {
@@ -241,12 +259,12 @@ __device__ inline void mg_knn_source(const KnnArgs &A, const StructRec &R, const
         }
         if (r < k) {
             const long long e = (long long)k * gi + (valid ? rank : r);
-            const int j = valid ? (int)((tie >> 24) & 0xFFu) : i;
+            const int j = valid ? jj[s] : i;
             A.src[e] = gi;
             A.dst[e] = R.first + j;
-            A.offset[3 * e] = valid ? (int8_t)((int)((tie >> 16) & 0xFFu) - 128) : (int8_t)0;
-            A.offset[3 * e + 1] = valid ? (int8_t)((int)((tie >> 8) & 0xFFu) - 128) : (int8_t)0;
-            A.offset[3 * e + 2] = valid ? (int8_t)((int)(tie & 0xFFu) - 128) : (int8_t)0;
+            A.offset[3 * e] = valid ? (int8_t)tt[s][0] : (int8_t)0;
+            A.offset[3 * e + 1] = valid ? (int8_t)tt[s][1] : (int8_t)0;
+            A.offset[3 * e + 2] = valid ? (int8_t)tt[s][2] : (int8_t)0;
             A.vec[3 * e] = valid ? (float)vv[s][0] : 0.f;
             A.vec[3 * e + 1] = valid ? (float)vv[s][1] : 0.f;
             A.vec[3 * e + 2] = valid ? (float)vv[s][2] : 0.f;

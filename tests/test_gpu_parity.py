@@ -122,6 +122,72 @@ def test_knn_large_structures(mg, ctx):
     check.check_knn(b, 12, got)
 
 
+@pytest.mark.parametrize("n_big", [300, 600, 1500])
+def test_knn_structures_above_256_atoms(mg, ctx, n_big):
+    # the growing-radius routine carries dst in a tie word that must not wrap above 256 atoms
+    small = C.small_batch(4, seed=33)
+    rng = np.random.default_rng(n_big)
+    side = (n_big / 0.08) ** (1.0 / 3.0)
+    cell = (np.diag([side, 1.1 * side, 0.9 * side]) + rng.uniform(-1, 1, (3, 3))).astype(np.float32)
+    big = C.Batch(pos=rng.random((n_big, 3), dtype=np.float32), lattice=cell[None],
+                  struct_ptr=np.array([0, n_big], np.int32))
+    b = C.concat([small, big, small])
+    got, status = _knn(mg, ctx, b, 12)
+    assert status == 0
+    rep = check.check_knn(b, 12, got)
+    assert rep["exact_rows"] >= 0.99 * b.n_atoms, rep
+
+
+def test_knn_supercell_config3_sized(mg, ctx):
+    # one BASELINE configs[3]-sized supercell (500-2000 atoms) through the KNN call
+    b = C.config_batch(3, n_struct=2)
+    got, status = _knn(mg, ctx, b, 12)
+    assert status == 0
+    check.check_knn(b, 12, got)
+
+
+def test_cutoff_graph_many_calls_no_count_between(mg, ctx):
+    # back-to-back mg_cutoff_graph calls on one context with no mg_cutoff_count in between: nothing in
+    # the library may depend on how many calls were made (a per-call ticket once grew without bound)
+    b = C.small_batch(64, seed=5)
+    pos, lat, ptr = mg.to_device(b)
+    ref = oracle.cutoff_graph(b.pos, b.lattice, b.struct_ptr, 5.0)
+    cap = int(ref["n_edges"])
+    out = mg.Edges.allocate(b.n_atoms, cap, "cuda", dist=True)
+    for _ in range(3000):
+        ctx.mg_cutoff_graph(pos, lat, ptr, 5.0, out)
+    got = out.to_numpy()
+    assert ctx.mg_check() == 0
+    rep = check.check_cutoff(b, 5.0, got, ref=ref)
+    assert rep["extra"] == 0 and rep["missing"] == 0
+
+
+def test_config4_full_size_walk(mg, ctx):
+    # BASELINE configs[4] at full size: 1024 crystals, 100 update steps; steps 1, 25, 50, 75, 100 are
+    # checked against the oracle and against a fresh mg_knn_graph call on the same inputs (R17)
+    import torch
+    k = 24
+    b0 = C.config_batch(4)
+    assert b0.n_struct == 1024
+    ptr = torch.from_numpy(b0.struct_ptr).cuda()
+    graph = ctx.mg_graph_create(mg.MG_KIND_KNN, ptr, b0.n_atoms, k=k)
+    out = mg.Edges.allocate(b0.n_atoms, k * b0.n_atoms, "cuda", dist=True)
+    for step, b in enumerate(C.walk(b0, 100, seed=0), start=1):
+        pos, lat, _ = mg.to_device(b)
+        ctx.mg_update_graph(graph, pos, lat, out)
+        if step not in (1, 25, 50, 75, 100):
+            continue
+        got = out.to_numpy()
+        assert ctx.mg_check() == 0
+        rep = check.check_knn(b, k, got)
+        assert rep["n_edges"] == k * b.n_atoms
+        fresh, _ = _knn(mg, ctx, b, k)
+        for key in ("src", "dst", "offset", "vec", "dist", "row_ptr"):
+            assert np.array_equal(fresh[key], got[key]), (step, key)
+    assert ctx.mg_check() == 0
+    graph.close()
+
+
 def test_config4_update_steps(mg, ctx):
     import torch
     k = 24
