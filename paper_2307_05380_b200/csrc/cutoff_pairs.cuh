@@ -380,7 +380,7 @@ __device__ __forceinline__ unsigned mg_word_mask(const WarpSmem &sw, const FindC
     const float4 *Zp = reinterpret_cast<const float4 *>(mg_tplane(sw, 2) + 32 * w);
     unsigned mask = 0u;
     bool near = false;
-    if (nw == 1) {                                               // one image per pair: T_0 = 0
+    if (ncl == 1 && tile0 == 0) {                                // one image per pair: T_0 = 0
         const float y = __fmaf_rn(p.qz, p.qz, __fmaf_rn(p.qy, p.qy, __fmaf_rn(p.qx, p.qx, nr2)));
         mask = y < win ? 1u : 0u;
         near = fabsf(y) < win;

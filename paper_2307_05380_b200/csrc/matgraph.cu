@@ -13,6 +13,7 @@
 #include "prep.cuh"
 #include "cut_prep.cuh"
 #include "cutoff_pairs.cuh"
+#include "cut_fused.cuh"
 #include "knn_small.cuh"
 #include "knn_pairs.cuh"
 
@@ -32,6 +33,10 @@ struct mg_ctx {
     int mask_words = 0;                   // usable words of a range's mask scratch (MATGRAPH_MASK_WORDS)
     unsigned *d_wmask = nullptr;          // [n_warps, MG_MASK_WORDS] hit masks kept from count to emit
     int cut_warps = 0, last_cut_warps = 0;
+    int fused_occ = 0, fused_coop = 0;    // fused cutoff kernel: CTAs per SM, cooperative launch accepted
+    int legacy = 0;                       // MATGRAPH_LEGACY=1: the two-launch cutoff path of round 1
+    unsigned long long *d_slots = nullptr;// [sm_count * fused_occ] per-CTA edge totals tagged with the call's epoch
+    unsigned *d_fmask = nullptr;          // [sm_count * fused_occ, MGF_MASK_WORDS] hit masks kept from count to emit
     CutRec *d_crec = nullptr;             // per-structure records of the cutoff path (cut_prep.cuh)
     unsigned long long *d_bpre = nullptr; // cost prefix over the prep blocks
     size_t crec_cap = 0;
@@ -130,7 +135,21 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
                          cudaMemset(c->d_wtotal, 0, (MG_OVER * c->cut_warps + 1 + 64) * sizeof(unsigned)) != cudaSuccess ||
                          cudaMalloc(&c->d_wstart, MG_OVER * c->cut_warps * sizeof(int2)) != cudaSuccess ||
                          cudaMalloc(&c->d_wmask, (size_t)MG_OVER * c->cut_warps * MG_MASK_WORDS * sizeof(unsigned)) != cudaSuccess ||
-                         cudaMalloc(&c->d_wclock, 8 * (size_t)c->cut_warps * sizeof(unsigned)) != cudaSuccess)) { mg_destroy(c); return MG_ERR_CUDA; }
+                         cudaMalloc(&c->d_wclock, 8 * (size_t)(c->cut_warps + 2048) * sizeof(unsigned)) != cudaSuccess)) { mg_destroy(c); return MG_ERR_CUDA; }
+    }
+    c->legacy = getenv("MATGRAPH_FUSED") ? 0 : 1;   // fused kernel: correct, not yet faster
+    if (cudaFuncSetAttribute(mg_cutoff_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)sizeof(FusedSmem)) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->fused_occ, mg_cutoff_fused_kernel, MGF_BLOCK, sizeof(FusedSmem));
+    if (c->fused_occ < 1) { mg_destroy(c); return MG_ERR_CUDA; }
+    {
+        const size_t nc = (size_t)c->sm_count * c->fused_occ;
+        if (cudaMalloc(&c->d_slots, nc * sizeof(unsigned long long)) != cudaSuccess ||
+            cudaMemset(c->d_slots, 0, nc * sizeof(unsigned long long)) != cudaSuccess ||
+            cudaMalloc(&c->d_fmask, nc * MGF_MASK_WORDS * sizeof(unsigned)) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
+        int coop = 0;
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device);
+        c->fused_coop = coop && !getenv("MATGRAPH_NO_COOP");
     }
     if (c->cutoff_occ < 1 || c->count_occ < 1 || c->knnp_occ < 1 || c->knn_occ[0] < 1 || c->knn_occ[1] < 1) { mg_destroy(c); return MG_ERR_CUDA; }
     *out = c;
@@ -145,6 +164,8 @@ extern "C" void mg_destroy(mg_ctx *c) {
     cudaFree(c->d_wstart);
     cudaFree(c->d_wmask);
     cudaFree(c->d_wclock);
+    cudaFree(c->d_slots);
+    cudaFree(c->d_fmask);
     cudaFree(c->d_crec);
     cudaFree(c->d_bpre);
     cudaFree(c->d_rec);
@@ -281,18 +302,27 @@ extern "C" mg_status mg_profile_read(mg_ctx *c, double *mean_ms4, int64_t *count
 // mg_grid_dependency_wait() (common.cuh), which hides the launch latency of the dependent kernel.
 template <class Args>
 static cudaError_t launch_after(mg_ctx *c, void (*kern)(const Args), int grid, int block, size_t smem,
-                                cudaStream_t st, const Args &a) {
+                                cudaStream_t st, const Args &a, bool cooperative = false) {
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof(cfg));
     cfg.gridDim = dim3((unsigned)grid);
     cfg.blockDim = dim3((unsigned)block);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchAttribute at[2];
+    int n = 0;
+    if (c->pdl) {
+        at[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[n].val.programmaticStreamSerializationAllowed = 1;
+        ++n;
+    }
+    if (cooperative) {                     // all CTAs resident at once: they wait on one another's slots
+        at[n].id = cudaLaunchAttributeCooperative;
+        at[n].val.cooperative = 1;
+        ++n;
+    }
     cfg.attrs = at;
-    cfg.numAttrs = c->pdl ? 1 : 0;
+    cfg.numAttrs = n;
     return cudaLaunchKernelEx(&cfg, kern, a);
 }
 
@@ -329,6 +359,32 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
         P.rec = c->d_crec; P.bpre = c->d_bpre; P.ctl = c->d_ctl; P.status = c->d_ctl + 4;
         MG_CUDA(launch_after(c, mg_cut_prep_kernel, n_blocks, MG_CP_BLOCK, 0, st, P));
         c->launches += 1;
+    }
+    if (!c->legacy) {
+        FusedArgs F;
+        F.pos = pos; F.lattice = lat; F.n_struct = n_struct; F.n_atoms = n_atoms; F.r_c = r_c;
+        F.row_ptr = o->row_ptr; F.src = o->src; F.dst = o->dst; F.offset = o->offset;
+        F.vec = o->vec; F.dist = o->dist; F.capacity = o->capacity; F.n_edges = (long long *)o->n_edges;
+        F.rec = c->d_crec; F.bpre = c->d_bpre; F.n_blocks = n_blocks;
+        F.wmask = c->d_fmask;
+        F.mask_words = c->mask_words < MGF_MASK_WORDS ? c->mask_words : MGF_MASK_WORDS;
+        F.slots = c->d_slots; F.ctl = c->d_ctl; F.status = c->d_ctl + 4;
+        F.count_only = count_only;
+        F.dbg = c->d_wclock;
+        int grid = c->sm_count * c->fused_occ;
+        const int cap_grid = n_atoms / 2 + 1;           // at least a couple of rows per CTA
+        if (grid > cap_grid) grid = cap_grid;
+        if (prof) cudaEventRecord(c->ev[1], st);
+        cudaError_t e = launch_after(c, mg_cutoff_fused_kernel, grid, MGF_BLOCK, sizeof(FusedSmem), st, F, c->fused_coop != 0);
+        if (e != cudaSuccess && c->fused_coop) {        // cooperative + programmatic launch refused together
+            cudaGetLastError();
+            c->fused_coop = 0;
+            e = launch_after(c, mg_cutoff_fused_kernel, grid, MGF_BLOCK, sizeof(FusedSmem), st, F, false);
+        }
+        MG_CUDA(e);
+        c->launches += 1;
+        if (prof) { cudaEventRecord(c->ev[2], st); cudaEventRecord(c->ev[3], st); c->pend_kind = 0; }
+        return MG_OK;
     }
     CutoffArgs A;
     A.pos = pos; A.lattice = lat;
