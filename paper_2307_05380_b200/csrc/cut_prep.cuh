@@ -37,6 +37,13 @@
 #define MG_C_BLOCK_WIDE 500.f
 #define MG_C_EDGE 3.3f             // per emitted edge
 #endif
+// ... of the fused kernel (cut_fused.cuh): per emitted edge, per candidate cell of its rows path
+#ifndef MG_CF_EDGE
+#define MG_CF_EDGE 7.f
+#endif
+#ifndef MG_C_ROWCELL
+#define MG_C_ROWCELL 12.f
+#endif
 // ... and of the KNN launch: per candidate cell, per block of 32 pairs, per source row (selection),
 // per structure
 #ifndef MG_KC_CELL
@@ -77,6 +84,7 @@ struct CutPrepArgs {
     float *hint;                   // KNN, [n_struct] or NULL: largest k-th distance of the previous call
                                    // (read when use_hint, then reset to 0: the graph kernel maxes into it)
     int use_hint;
+    int rows_cost;                 // cutoff: cost model of the fused kernel (rows path for large structures / tables)
     CutRec *rec;                   // [n_struct]
     unsigned long long *bpre;      // [blocks + 1] block sums -> exclusive prefix; [blocks] = total
     unsigned *ctl;                 // [7] blocks done
@@ -143,14 +151,18 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
             // and walk them one source row (N of 32 lanes) at a time)
             const float percell = mloc > 256 ? 11.f + 900.f / (float)N : (mloc > 128 ? MG_C_CELL_WIDE : (mloc > 64 ? MG_C_CELL_MID : MG_C_CELL));
             const float perblock = mloc > 256 ? 120.f + 16000.f / (float)N : (mloc > 128 ? MG_C_BLOCK_WIDE : MG_C_BLOCK);
-            const float c = ((float)((mloc + 3) & ~3) * percell + perblock) * (1.f / 32.f) + MG_C_EDGE * lam / (float)N +
-                            MG_STRUCT_COST / ((float)N * (float)N);
+            const float c = ((float)((mloc + 3) & ~3) * percell + perblock) * (1.f / 32.f) +
+                            (A.rows_cost ? MG_CF_EDGE : MG_C_EDGE) * lam / (float)N + MG_STRUCT_COST / ((float)N * (float)N);
             // KNN: one launch, no edge stream (constants from a sweep over four seeds of config 2 and config 4)
             const float ck = ((float)((mloc + 3) & ~3) * MG_KC_CELL + MG_KC_BLOCK) * (1.f / 32.f) + MG_KC_ROW / (float)N +
                              MG_KC_STRUCT / ((float)N * (float)N);
             // (KNN above the staging limit: warp-per-row growing-radius search, about 40 per pair-cell)
             const float ckb = 40.f * (float)mloc / 32.f + 600.f / (float)N;
-            r.paircost = (unsigned)fminf(16.f * (A.k > 0 ? (N > MG_SMALL_MAX_ATOMS ? ckb : ck) : c) + 1.f, 16777216.f);
+            // cutoff, structures the pair-lane path does not take (cut_fused.cuh: one candidate per lane
+            // and ~60 instructions, evaluated in both phases)
+            const float crow = MG_C_ROWCELL * (float)mloc + MG_CF_EDGE * lam / (float)N;
+            const bool rows = N > MG_SMALL_MAX_ATOMS || mloc > MG_PAIR_TL;
+            r.paircost = (unsigned)fminf(16.f * (A.k > 0 ? (N > MG_SMALL_MAX_ATOMS ? ckb : ck) : (rows && A.rows_cost ? crow : c)) + 1.f, 16777216.f);
         }
         r.pad = 0;
         cost = (unsigned long long)((long long)N * N) * r.paircost;

@@ -135,7 +135,7 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
                          cudaMemset(c->d_wtotal, 0, (MG_OVER * c->cut_warps + 1 + 64) * sizeof(unsigned)) != cudaSuccess ||
                          cudaMalloc(&c->d_wstart, MG_OVER * c->cut_warps * sizeof(int2)) != cudaSuccess ||
                          cudaMalloc(&c->d_wmask, (size_t)MG_OVER * c->cut_warps * MG_MASK_WORDS * sizeof(unsigned)) != cudaSuccess ||
-                         cudaMalloc(&c->d_wclock, 8 * (size_t)(c->cut_warps + 2048) * sizeof(unsigned)) != cudaSuccess)) { mg_destroy(c); return MG_ERR_CUDA; }
+                         cudaMalloc(&c->d_wclock, 64 * (size_t)(c->cut_warps + 2048) * sizeof(unsigned)) != cudaSuccess)) { mg_destroy(c); return MG_ERR_CUDA; }
     }
     c->legacy = getenv("MATGRAPH_FUSED") ? 0 : 1;   // fused kernel: correct, not yet faster
     if (cudaFuncSetAttribute(mg_cutoff_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -355,7 +355,7 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
     {
         CutPrepArgs P;
         P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms; P.r_c = r_c;
-        P.k = 0; P.hint = nullptr; P.use_hint = 0;
+        P.k = 0; P.hint = nullptr; P.use_hint = 0; P.rows_cost = c->legacy ? 0 : 1;
         P.rec = c->d_crec; P.bpre = c->d_bpre; P.ctl = c->d_ctl; P.status = c->d_ctl + 4;
         MG_CUDA(launch_after(c, mg_cut_prep_kernel, n_blocks, MG_CP_BLOCK, 0, st, P));
         c->launches += 1;
@@ -367,12 +367,12 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
         F.vec = o->vec; F.dist = o->dist; F.capacity = o->capacity; F.n_edges = (long long *)o->n_edges;
         F.rec = c->d_crec; F.bpre = c->d_bpre; F.n_blocks = n_blocks;
         F.wmask = c->d_fmask;
-        F.mask_words = c->mask_words < MGF_MASK_WORDS ? c->mask_words : MGF_MASK_WORDS;
+        F.mask_words = c->mask_words < MGW_MASK_WORDS ? c->mask_words : MGW_MASK_WORDS;
         F.slots = c->d_slots; F.ctl = c->d_ctl; F.status = c->d_ctl + 4;
         F.count_only = count_only;
         F.dbg = c->d_wclock;
         int grid = c->sm_count * c->fused_occ;
-        const int cap_grid = n_atoms / 2 + 1;           // at least a couple of rows per CTA
+        const int cap_grid = (n_atoms + MGF_WARPS) / MGF_WARPS;   // >= 1 row per warp
         if (grid > cap_grid) grid = cap_grid;
         if (prof) cudaEventRecord(c->ev[1], st);
         cudaError_t e = launch_after(c, mg_cutoff_fused_kernel, grid, MGF_BLOCK, sizeof(FusedSmem), st, F, c->fused_coop != 0);
@@ -453,7 +453,7 @@ static mg_status launch_knn(mg_ctx *c, const float *pos, const float *lat, const
         if (c->profile) { prof_collect(c); cudaEventRecord(c->ev[0], st); }
         CutPrepArgs P;
         P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms; P.r_c = 0.f;
-        P.k = k; P.hint = hint; P.use_hint = use_hint;
+        P.k = k; P.hint = hint; P.use_hint = use_hint; P.rows_cost = 0;
         P.rec = c->d_crec; P.bpre = c->d_bpre; P.ctl = c->d_ctl; P.status = c->d_ctl + 4;
         MG_CUDA(launch_after(c, mg_cut_prep_kernel, n_blocks, MG_CP_BLOCK, 0, st, P));
         c->launches += 1;
