@@ -1,179 +1,88 @@
-// cut_fused.cuh — cutoff graph (K3 distance filter, K4 count -> device-wide scan -> emit, K6 batching,
-// SURVEY.md 8(a)) in ONE launch of co-resident CTAs whose warps work on their own.
+// cut_scan.cuh — cutoff graph (K3 distance filter, K4 count -> device-wide scan -> emit, K6 batching,
+// SURVEY.md 8(a)) in two launches:
 //
-// mg_cut_prep_kernel gives every ordered pair (i, j) an estimated cost; warp r of the grid (r = 4 *
-// blockIdx.x + warp: the warps of a CTA own consecutive ranges) owns the source rows whose first pair
-// lies in the r-th of n_ranges equally expensive, contiguous ranges of the batch's pairs in
-// (structure, i, j) order — which is the CSR order of the output.  A warp walks its rows twice:
+//   mg_cutoff_scan_kernel   finds the edges.  Co-resident CTAs whose warps work on their own:
+//     warp r of the grid (r = 4 * blockIdx.x + warp) owns the source rows whose first pair lies in the r-th of
+//     n_ranges equally expensive, contiguous ranges of the batch's ordered pairs in (structure, i, j)
+//     order — the CSR order of the output (cut_prep.cuh).  It walks its rows twice:
+//       count   per structure: wrapped positions and the table of local translations staged in the
+//               warp's shared memory; blocks of 32 ordered pairs, lane <-> pair: FP32 filter over the
+//               pair's sub-box (FP64 decision inside the rounding window, R23); the 32-bit
+//               hit masks go to the warp's scratch in global memory (L2 resident);
+//       scan    warp totals -> CTA total, published in a slot tagged with the call's epoch; warp 0
+//               sums the slots of the CTAs before its own (all CTAs are resident: cooperative launch):
+//               the device-wide exclusive scan of K4 without a launch of its own;
+//       list    the same walk: masks read back, the hits of a block compacted in (row, j, t) order
+//               into 8-byte codes (dst, tau) at their FINAL position in one code stream; row_ptr,
+//               the atom -> structure map, FP64 copies of positions and lattices, and for every 128th
+//               edge the row it belongs to.
+//   mg_cutoff_write_kernel  turns the code stream into the caller's arrays.  Perfectly balanced (a warp
+//     takes slices of 128 consecutive edges, whatever structure they come from), no staging, lane <-> four
+//     consecutive edges: src from row_ptr, vec = ((x_dst - x_src) + tau) . L in FP64 in the oracle's
+//     operation order, rounded once (R24); every array leaves in aligned 16-byte stores.
 //
-//   count   per structure: stage the wrapped positions and the table of local translations in the
-//           warp's shared memory, then blocks of 32 ordered pairs: lane <-> pair, FP32 filter over
-//           the pair's sub-box (cut_prep.cuh; FP64 decision inside the rounding window, R23).
-//           The 32-bit hit masks go to the warp's scratch in global memory (L2 resident).
-//   scan    warp totals -> CTA total, published in a slot tagged with the call's epoch; warp 0 sums
-//           the slots of the CTAs before its own (all CTAs are resident: cooperative launch): the
-//           device-wide exclusive scan of K4 without a second launch and without a look-back chain.
-//   emit    the same walk: masks read back, the hits of a block compacted into the warp's stash in
-//           (row, j, t) order, row_ptr from the running offset; then LANES <-> EDGES: vec = (x_j - x_i
-//           + l) . L + t . L in FP64 (the pair's part once per pair, the table's part from an FP64
-//           table), rounded once (R24).  src / dst leave as coalesced 4-byte stores; vec and offset
-//           are staged in shared memory at the misalignment of their global address and leave as
-//           aligned 16-byte stores (scalar stores only for a ragged first / last piece).
-//
-// Structures the pair-lane path does not take (more than MGW_NMAX atoms, a sub-box of more than MGW_TL
-// cells) go row by row through mgw_rows_*: lanes over the candidates (j, t) of one source row, ballot
-// compaction, no table — exact and general, not tuned.
+// Structures the pair-lane path does not take (more than MGS_NMAX atoms, a sub-box of more than MGS_TL
+// cells) go row by row: lanes over the candidates (j, t) of one source row, ballot compaction.
 #pragma once
 #include "common.cuh"
 #include "cut_prep.cuh"
-#include "cutoff_pairs.cuh"
+#include "ranges.cuh"
 
-#define MGF_BLOCK 128
-#define MGF_WARPS (MGF_BLOCK / 32)
-#define MGW_TL MG_PAIR_TL          // cells of a warp's table
-#define MGW_NMAX 64                // atoms of a staged structure
-#define MGW_STASH 256              // edges per pass
-#define MGW_RING 512               // units (floats of vec / bytes of offset) of the output rings
-#define MGF_MASK_WORDS 16384       // 32-bit words of mask scratch per CTA
-#define MGW_MASK_WORDS (MGF_MASK_WORDS / MGF_WARPS)
+#define MGS_BLOCK 128
+#define MGS_WARPS (MGS_BLOCK / 32)
+#define MGS_TL MG_PAIR_TL          // cells of a warp's table
+#define MGS_NMAX MG_SMALL_MAX_ATOMS // atoms of a staged structure
+#define MGS_STASH 256              // codes per pass
+#define MGS_MASK_WORDS 4096        // 32-bit words of mask scratch per warp
+#define MGS_SLICE 128              // edges per slice of the write kernel
 
-struct FusedArgs {
+struct ScanArgs {
     const float *pos;
     const float *lattice;
     int n_struct, n_atoms;
     float r_c;
-    int32_t *row_ptr, *src, *dst;
-    int8_t *offset;
-    float *vec, *dist;
+    int32_t *row_ptr;
     long long capacity;
     long long *n_edges;
     const CutRec *rec;
     const unsigned long long *bpre;
     int n_blocks;
-    unsigned *wmask;               // [gridDim.x, MGF_MASK_WORDS]
+    unsigned *wmask;               // [n_ranges, MGS_MASK_WORDS]
     int mask_words;                // words of a warp's scratch that may be used (tests: less)
-    unsigned long long *slots;     // [gridDim.x] (epoch + 1) << 32 | edges of the CTA
+    unsigned long long *slots;     // [gridDim.x] epoch << 32 | edges of the CTA
     unsigned *ctl;                 // [10] epoch of the last finished call, [11] CTAs done
     unsigned *status;
     int count_only;
-    unsigned *dbg;                 // MG_PHASE_CLOCKS builds: [gridDim.x, 4] globaltimer at the phase boundaries
+    // products for the write kernel
+    uint2 *codes;                  // [capacity] .x = dst, .y = (tau + 128) bytes << 8
+    int32_t *slice_row;            // [ceil(capacity / MGS_SLICE) + 1] row of edge MGS_SLICE * k
+    int32_t *atom_struct;          // [n_atoms]
+    double *pos64;                 // [n_atoms, 3]
+    double *lat64;                 // [n_struct, 9]
+    unsigned *dbg;                 // MG_PHASE_CLOCKS builds: globaltimer at the phase boundaries, per-warp cycles
 };
 
 #ifdef MG_PHASE_CLOCKS
-__device__ __forceinline__ unsigned mgf_now() {
+__device__ __forceinline__ unsigned mgs_now() {
     unsigned long long t;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     return (unsigned)t;
 }
-#define MGF_STAMP(i) if (threadIdx.x == 0 && A.dbg) A.dbg[4 * blockIdx.x + (i)] = mgf_now();
+#define MGS_STAMP(i) if (threadIdx.x == 0 && A.dbg) A.dbg[4 * blockIdx.x + (i)] = mgs_now();
 #else
-#define MGF_STAMP(i)
+#define MGS_STAMP(i)
 #endif
 
-struct __align__(16) PairRec {         // per pair of the block: (x_j - x_i + l) . L, (l + 128) bytes << 8, i | j << 16
-    double bx, by, bz;
-    unsigned plc, pij;
-};
-struct __align__(16) CellRec {         // per cell of the table: t . L in FP64, t0 << 24 | t1 << 16 | t2 << 8
-    double tx, ty, tz;
-    unsigned tcode, pad;
+struct SSmem {                         // one warp's shared memory
+    float T[3][MGS_TL + 4];            // t . L: planes x | y | z (+ one group read ahead)
+    unsigned tcode[MGS_TL];            // t0 << 24 | t1 << 16 | t2 << 8
+    float4 x[MGS_NMAX];                // wrapped fractional coordinates, .w = packed integer parts
+    uint2 stash[MGS_STASH];            // codes of one pass
 };
 
-#define MGW_RE 128                     // edges of the output rings
-#define MGW_BATCH 96                   // edges per flush batch (+ the carried ragged piece < MGW_RE)
-
-struct WSmem {                         // one warp's shared memory
-    float T[3][MGW_TL + 4];            // t . L: planes x | y | z (+ one group read ahead)
-    unsigned tcode[MGW_TL];            // t0 << 24 | t1 << 16 | t2 << 8
-    CellRec cr[MGW_TL];                // (emit)
-    float4 x[MGW_NMAX];                // wrapped fractional coordinates, .w = packed integer parts
-    unsigned stash[MGW_STASH];         // (pair of the block) << 8 | cell
-    PairRec pr[32];
-    // output rings: unit 3 e + a of the OUTPUT (global edge e, component a) lives at 3 (e % MGW_RE) + a, so
-    // that aligned 16-byte pieces of the rings are aligned pieces of vec / offset
-    float vr[3 * MGW_RE];
-    unsigned char br[3 * MGW_RE];
-};
-
-// Output state of a warp (the same on every lane).  A unit is one float of vec = one byte of offset:
-// unit 3 e + a belongs to edge e.  Whole 16-byte pieces leave as STG.128; the ragged first piece of the
-// warp's range, its last piece and the piece cut by the capacity leave as scalar stores.
-struct OutCtx {
-    long long u0;          // first unit of the warp's range
-    long long vdone;       // vec units written as pieces so far (multiple of 4); head = [u0, vhead)
-    long long bdone;       // offset units written as pieces so far (multiple of 16); head = [u0, bhead)
-    long long vhead, bhead;
-    long long cap3;        // 3 * capacity
-    int vpos, bpos;        // vdone, bdone modulo the ring size
-    bool vec16, off16;     // the arrays are 16-byte aligned (else: scalar stores only)
-};
-
-__device__ __forceinline__ void mgw_out_init(OutCtx &O, const FusedArgs &A, unsigned long long goff0) {
-    O.u0 = 3 * (long long)goff0;
-    O.vhead = O.vdone = (O.u0 + 3) & ~3ll;
-    O.bhead = O.bdone = (O.u0 + 15) & ~15ll;
-    O.vpos = (int)(O.vdone % (3 * MGW_RE));
-    O.bpos = (int)(O.bdone % (3 * MGW_RE));
-    O.cap3 = 3 * A.capacity;
-    O.vec16 = (reinterpret_cast<unsigned long long>(A.vec) & 15ull) == 0ull;
-    O.off16 = (reinterpret_cast<unsigned long long>(A.offset) & 15ull) == 0ull;
-}
-
-// Units [lo, hi) from the rings, one by one (rare paths).
-__device__ __forceinline__ void mgw_out_scalar_v(const WSmem &ws, const FusedArgs &A, long long lo, long long hi, int lane) {
-    for (long long u = lo + lane; u < hi; u += 32) A.vec[u] = ws.vr[(int)(u % (3 * MGW_RE))];
-}
-__device__ __forceinline__ void mgw_out_scalar_b(const WSmem &ws, const FusedArgs &A, long long lo, long long hi, int lane) {
-    for (long long u = lo + lane; u < hi; u += 32) A.offset[u] = (int8_t)ws.br[(int)(u % (3 * MGW_RE))];
-}
-
-// The rings hold the units [lo, up) that were produced last: write out what is complete.
-__device__ __forceinline__ void mgw_out_pieces(const WSmem &ws, const FusedArgs &A, OutCtx &O, long long lo, long long up,
-                                               int lane) {
-    const long long hi = up < O.cap3 ? up : O.cap3;
-    if (O.vec16) {
-        if (lo < O.vhead) mgw_out_scalar_v(ws, A, lo > O.u0 ? lo : O.u0, hi < O.vhead ? hi : O.vhead, lane);
-        const long long npl = ((hi & ~3ll) - O.vdone) >> 2;                  // whole pieces (< 3 MGW_RE / 4)
-        const int np = npl > 0 ? (int)npl : 0;
-        float4 *dst = reinterpret_cast<float4 *>(A.vec + O.vdone);
-        for (int k = lane; k < np; k += 32) {
-            int pos = O.vpos + 4 * k;
-            if (pos >= 3 * MGW_RE) pos -= 3 * MGW_RE;
-            dst[k] = *reinterpret_cast<const float4 *>(&ws.vr[pos]);
-        }
-        if (np > 0) { O.vdone += 4ll * np; O.vpos = (O.vpos + 4 * np) % (3 * MGW_RE); }
-        if (hi < up) { mgw_out_scalar_v(ws, A, O.vdone, hi, lane); O.vdone = 1ll << 60; }     // cut by the capacity
-    } else {
-        mgw_out_scalar_v(ws, A, lo, hi, lane);
-    }
-    if (O.off16) {
-        if (lo < O.bhead) mgw_out_scalar_b(ws, A, lo > O.u0 ? lo : O.u0, hi < O.bhead ? hi : O.bhead, lane);
-        const long long npl = ((hi & ~15ll) - O.bdone) >> 4;
-        const int np = npl > 0 ? (int)npl : 0;
-        uint4 *dst = reinterpret_cast<uint4 *>(A.offset + O.bdone);
-        for (int k = lane; k < np; k += 32) {
-            int pos = O.bpos + 16 * k;
-            if (pos >= 3 * MGW_RE) pos -= 3 * MGW_RE;
-            dst[k] = *reinterpret_cast<const uint4 *>(&ws.br[pos]);
-        }
-        if (np > 0) { O.bdone += 16ll * np; O.bpos = (O.bpos + 16 * np) % (3 * MGW_RE); }
-        if (hi < up) { mgw_out_scalar_b(ws, A, O.bdone, hi, lane); O.bdone = 1ll << 60; }
-    } else {
-        mgw_out_scalar_b(ws, A, lo, hi, lane);
-    }
-}
-
-// End of the warp's range (uend = its last unit + 1): the ragged last pieces.
-__device__ __forceinline__ void mgw_out_finish(const WSmem &ws, const FusedArgs &A, const OutCtx &O, long long uend, int lane) {
-    const long long hi = uend < O.cap3 ? uend : O.cap3;
-    __syncwarp();
-    if (O.vec16 && O.vdone < hi) mgw_out_scalar_v(ws, A, O.vdone, hi, lane);
-    if (O.off16 && O.bdone < hi) mgw_out_scalar_b(ws, A, O.bdone, hi, lane);
-}
-
-struct FusedSmem {
-    WSmem w[MGF_WARPS];
-    unsigned wsum[MGF_WARPS];
+struct ScanSmem {
+    SSmem w[MGS_WARPS];
+    unsigned wsum[MGS_WARPS];
     unsigned long long prefix;
     int last;
 };
@@ -189,7 +98,7 @@ struct WCtx {
     int first, N;
 };
 
-__device__ __forceinline__ void mgw_ctx(WCtx &C, const FusedArgs &A, const CutRec *R, int s) {
+__device__ __forceinline__ void mgs_ctx(WCtx &C, const ScanArgs &A, const CutRec *R, int s) {
     C.lat = A.lattice + 9 * (size_t)s;
 #pragma unroll
     for (int c = 0; c < 9; ++c) C.a[c] = __ldg(C.lat + c);
@@ -206,10 +115,10 @@ __device__ __forceinline__ void mgw_ctx(WCtx &C, const FusedArgs &A, const CutRe
     C.gx = A.pos + 3 * (size_t)R->first;
 }
 
+
 // ---- staging of one structure in the warp's shared memory ---------------------------------------
 // Returns false (on every lane) if a coordinate is non-finite or too far from the cell.
-template <bool EMIT>
-__device__ __forceinline__ bool mgw_stage(WSmem &ws, const WCtx &C, int lane) {
+__device__ __forceinline__ bool mgs_stage(SSmem &ws, const WCtx &C, int lane) {
     __syncwarp();
     bool ok = true;
     for (int j = lane; j < C.N; j += 32) {
@@ -221,7 +130,7 @@ __device__ __forceinline__ bool mgw_stage(WSmem &ws, const WCtx &C, int lane) {
     // a multiple of 32 and one group beyond (the filter reads one group ahead)
     const int M12 = C.m1 * C.m2;
     const float inv12 = 1.f / (float)M12, inv2 = 1.f / (float)C.m2;
-    const int pad = min(MGW_TL + 4, ((C.mloc + 31) & ~31) + 4);
+    const int pad = min(MGS_TL + 4, ((C.mloc + 31) & ~31) + 4);
     for (int c = lane; c < pad; c += 32) {
         float Tx = 1e18f, Ty = 1e18f, Tz = 1e18f;
         if (c < C.mloc) {
@@ -231,17 +140,7 @@ __device__ __forceinline__ bool mgw_stage(WSmem &ws, const WCtx &C, int lane) {
             Tx = __fmaf_rn(f2, C.a[6], __fmaf_rn(f1, C.a[3], __fmul_rn(f0, C.a[0])));
             Ty = __fmaf_rn(f2, C.a[7], __fmaf_rn(f1, C.a[4], __fmul_rn(f0, C.a[1])));
             Tz = __fmaf_rn(f2, C.a[8], __fmaf_rn(f1, C.a[5], __fmul_rn(f0, C.a[2])));
-            const unsigned tcode = ((unsigned)t0 << 24) | ((unsigned)t1 << 16) | ((unsigned)t2 << 8);
-            ws.tcode[c] = tcode;
-            if (EMIT) {                // exact: small integers times FP32 values, three terms
-                const double g0 = (double)t0, g1 = (double)t1, g2 = (double)t2;
-                CellRec r;
-                r.tx = fma(g2, (double)C.a[6], fma(g1, (double)C.a[3], g0 * (double)C.a[0]));
-                r.ty = fma(g2, (double)C.a[7], fma(g1, (double)C.a[4], g0 * (double)C.a[1]));
-                r.tz = fma(g2, (double)C.a[8], fma(g1, (double)C.a[5], g0 * (double)C.a[2]));
-                r.tcode = tcode; r.pad = 0u;
-                ws.cr[c] = r;
-            }
+            ws.tcode[c] = ((unsigned)t0 << 24) | ((unsigned)t1 << 16) | ((unsigned)t2 << 8);
         }
         ws.T[0][c] = Tx; ws.T[1][c] = Ty; ws.T[2][c] = Tz;
     }
@@ -253,15 +152,15 @@ __device__ __forceinline__ bool mgw_stage(WSmem &ws, const WCtx &C, int lane) {
 // One lane's ordered pair (i, j) of the staged structure: q' = (u + lo) . L with u = x_j - x_i
 // (wrapped coordinates) and lo = floor(-rho - u) + 1 the first cell of the pair's sub-box
 // (cut_prep.cuh); the cell offsets relative to the coordinates AS GIVEN start at l = lo + k_i - k_j.
-struct WPair {
+struct SPair {
     float qx, qy, qz;
     int l0, l1, l2;
     int self;              // index of the cell tau = 0 in the table if i == j, else -1
     bool ok;               // valid lane, offsets inside int8
 };
 
-__device__ __forceinline__ WPair mgw_pair(const WSmem &ws, const WCtx &C, bool valid, int i, int j) {
-    WPair p;
+__device__ __forceinline__ SPair mgs_pair(const SSmem &ws, const WCtx &C, bool valid, int i, int j) {
+    SPair p;
     const float4 xi = ws.x[i], xj = ws.x[j];
     const float u0 = __fsub_rn(xj.x, xi.x), u1 = __fsub_rn(xj.y, xi.y), u2 = __fsub_rn(xj.z, xi.z);
     const float e0 = floorf(__fsub_rn(-C.rho[0], u0)) + 1.f, e1 = floorf(__fsub_rn(-C.rho[1], u1)) + 1.f,
@@ -285,7 +184,7 @@ __device__ __forceinline__ WPair mgw_pair(const WSmem &ws, const WCtx &C, bool v
 // bits of y = |q' + T|^2 - r_c^2 are shifted in one by one).  Two cells per packed FP32 instruction,
 // table groups read one ahead.  A lane that saw |y| < win decides those cells again with the exact
 // FP64 predicate, so the mask is Def. 3's in FP64.
-__device__ __forceinline__ unsigned mgw_word_mask(const WSmem &ws, const WCtx &C, const WPair &p, int i, int j, int w) {
+__device__ __forceinline__ unsigned mgs_word_mask(const SSmem &ws, const WCtx &C, const SPair &p, int i, int j, int w) {
     const int nw = min(32, C.mloc - 32 * w), n4 = (nw + 3) >> 2;      // warp-uniform
     const float4 *Xp = reinterpret_cast<const float4 *>(&ws.T[0][32 * w]);
     const float4 *Yp = reinterpret_cast<const float4 *>(&ws.T[1][32 * w]);
@@ -330,12 +229,13 @@ __device__ __forceinline__ unsigned mgw_word_mask(const WSmem &ws, const WCtx &C
     return mask;
 }
 
+
 // ---- generic rows: any structure size, any sub-box (not tuned) -----------------------------------
 // One warp per source row, lanes over candidates (j, t) of the row.  For the pair (i, j): u = x_j - x_i
 // (wrapped coordinates), the sub-box starts at lo_a = floor(-rho_a - u_a) + 1 (cut_prep.cuh);
 // d2 = |(u + lo + t) . L|^2 in FP32, FP64 decision inside the rounding window (R23).
 // Candidate (j, t) of row i: hit?  tau (relative to the coordinates as given) in tau[3].
-__device__ __forceinline__ bool mgw_cand(const WCtx &C, const float4 xi, int i, int j, int t0, int t1, int t2,
+__device__ __forceinline__ bool mgs_cand(const WCtx &C, const float4 xi, int i, int j, int t0, int t1, int t2,
                                          int tau[3], bool &bad) {
     const float4 xj = mg_wrap_x(C.gx + 3 * j);
     const int ki = __float_as_int(xi.w), kj = __float_as_int(xj.w);
@@ -361,23 +261,35 @@ __device__ __forceinline__ bool mgw_cand(const WCtx &C, const float4 xi, int i, 
     return hit;
 }
 
-__device__ __forceinline__ void mgw_emit_one(const FusedArgs &A, long long e, int gi, int gj, const float *gx, int i,
-                                             int j, const int t[3], const float *lat) {
-    if (e >= A.capacity) return;
-    double v[3];
-    const double d = mg_exact_vec(gx + 3 * i, gx + 3 * j, t[0], t[1], t[2], lat, v);
-    A.src[e] = gi;
-    A.dst[e] = gj;
-    A.offset[3 * e] = (int8_t)t[0]; A.offset[3 * e + 1] = (int8_t)t[1]; A.offset[3 * e + 2] = (int8_t)t[2];
-    A.vec[3 * e] = (float)v[0]; A.vec[3 * e + 1] = (float)v[1]; A.vec[3 * e + 2] = (float)v[2];
-    if (A.dist) A.dist[e] = (float)d;
+
+// What the list phase leaves for the write kernel, per source row [first + ia, first + ib) of structure s.
+__device__ __forceinline__ void mgs_row_products(const ScanArgs &A, const WCtx &C, int s, int ia, int ib, int lane) {
+    for (int i = ia + lane; i < ib; i += 32) {
+        const int g = C.first + i;
+        A.atom_struct[g] = s;
+        A.pos64[3 * (size_t)g] = (double)C.gx[3 * i];
+        A.pos64[3 * (size_t)g + 1] = (double)C.gx[3 * i + 1];
+        A.pos64[3 * (size_t)g + 2] = (double)C.gx[3 * i + 2];
+    }
+    if (ia == 0 && lane < 9) A.lat64[9 * (size_t)s + lane] = (double)C.lat[lane];
 }
 
-// One source row: returns its edges; EMIT: writes them from goff on (any order inside the row).
+// The edges [g0, g0 + n) belong to rows in such a way that edge g0 + p is in the row `row` on the lane
+// that holds p in [excl, excl + cnt): every MGS_SLICE-th edge records its row.
+__device__ __forceinline__ void mgs_slice_rows(const ScanArgs &A, unsigned long long g0, unsigned n, unsigned excl,
+                                               unsigned cnt, int row) {
+    const unsigned long long b0 = (g0 + MGS_SLICE - 1) & ~(unsigned long long)(MGS_SLICE - 1);
+    for (unsigned long long b = b0; b < g0 + n && (long long)b < A.capacity; b += MGS_SLICE) {
+        const unsigned p = (unsigned)(b - g0);
+        if (p >= excl && p < excl + cnt) A.slice_row[b / MGS_SLICE] = row;
+    }
+}
+
+// One source row: returns its edges; LIST: writes their codes from goff on (any order inside the row).
 // Tables of 32 cells and more: lane <-> cell (decoded once per 32 cells), loop over the targets j.
 // Smaller tables: lane <-> (target, cell), floor(32 / mloc) targets per pass.
-template <bool EMIT>
-__device__ __forceinline__ unsigned mgw_row(const FusedArgs &A, const WCtx &C, int i, unsigned long long goff, int lane,
+template <bool LIST>
+__device__ __forceinline__ unsigned mgs_row(const ScanArgs &A, const WCtx &C, int i, unsigned long long goff, int lane,
                                             bool &anybad) {
     const float4 xi = mg_wrap_x(C.gx + 3 * i);
     const int M12 = C.m1 * C.m2;
@@ -394,84 +306,26 @@ __device__ __forceinline__ unsigned mgw_row(const FusedArgs &A, const WCtx &C, i
             const int j = j0 + jl;
             int tau[3] = {0, 0, 0};
             bool bad = false;
-            const bool hit = cv && j < C.N && mgw_cand(C, xi, i, j, t0, t1, t2, tau, bad);
+            const bool hit = cv && j < C.N && mgs_cand(C, xi, i, j, t0, t1, t2, tau, bad);
             anybad = anybad || bad;
             const unsigned bal = __ballot_sync(0xFFFFFFFFu, hit);
-            if (EMIT && hit)
-                mgw_emit_one(A, (long long)(goff + cnt) + __popc(bal & ((1u << lane) - 1u)), C.first + i, C.first + j, C.gx, i, j, tau, C.lat);
+            if (LIST && hit) {
+                const long long e = (long long)(goff + cnt) + __popc(bal & ((1u << lane) - 1u));
+                if (e < A.capacity)
+                    A.codes[e] = make_uint2((unsigned)(C.first + j), ((unsigned)(tau[0] + 128) << 24) |
+                                            ((unsigned)(tau[1] + 128) << 16) | ((unsigned)(tau[2] + 128) << 8));
+            }
             cnt += __popc(bal);
         }
     }
     return cnt;
 }
 
-// Rows [ia, ib) of structure s, counted by one warp; row totals go to the scratch while they fit.
-__device__ __forceinline__ unsigned mgw_rows_count(const FusedArgs &A, const WCtx &C, int ia, int ib, unsigned *wm,
-                                                   int midx, int lane) {
-    unsigned total = 0u;
-    for (int i = ia; i < ib; ++i) {
-        bool anybad = false;
-        const unsigned cnt = mgw_row<false>(A, C, i, 0ull, lane, anybad);
-        if (anybad) atomicOr(A.status, __float_as_int(mg_wrap_x(C.gx + 3 * i).w) == 0 ? MGS_NONFINITE : MGS_OFFSET);
-        total += cnt;
-    }
-    return total;
-}
-
-// Emit rows [ia, ib) from goff; returns the offset after them.
-__device__ __forceinline__ unsigned long long mgw_rows_emit(const FusedArgs &A, const WCtx &C, int ia, int ib,
-                                                            unsigned long long goff, int lane) {
-    for (int i = ia; i < ib; ++i) {
-        if (lane == 0) A.row_ptr[C.first + i] = (int)goff;
-        bool anybad = false;
-        goff += mgw_row<true>(A, C, i, goff, lane, anybad);
-    }
-    return goff;
-}
-
-// ---- stash -> global ------------------------------------------------------------------------------
-// Edges [0, n) of the warp's stash are the edges [goff, goff + n) of the output.  Batches of MGW_BATCH
-// edges: lane <-> edge, src / dst / dist as coalesced 4-byte stores, vec and offset into the output
-// rings; after every batch the complete 16-byte pieces of the rings are written out.
-__device__ __forceinline__ void mgw_flush(WSmem &ws, const FusedArgs &A, OutCtx &O, int first, long long goff, int n,
-                                          int lane) {
-    for (int e0 = 0; e0 < n; e0 += MGW_BATCH) {
-        const int nb = min(MGW_BATCH, n - e0);
-        const long long E0 = goff + e0;                 // global index of the batch's first edge
-        const long long room = A.capacity - E0;
-        const int nst = room >= nb ? nb : (room > 0 ? (int)room : 0);       // edges that fit src / dst / dist
-        int32_t *psrc = A.src + E0, *pdst = A.dst + E0;
-        float *pdist = A.dist ? A.dist + E0 : nullptr;
-        const int em = (int)(E0 & (MGW_RE - 1));
-#pragma unroll 1
-        for (int x = lane; x < nb; x += 32) {
-            const unsigned code = ws.stash[e0 + x];
-            const PairRec P = ws.pr[code >> 8];
-            const CellRec Q = ws.cr[code & 0xFFu];
-            const double v0 = P.bx + Q.tx, v1 = P.by + Q.ty, v2 = P.bz + Q.tz;
-            const unsigned tb = (P.plc + Q.tcode) ^ 0x80808000u;             // tau bytes as int8
-            if (x < nst) {
-                psrc[x] = first + (int)(P.pij & 0xFFFFu);
-                pdst[x] = first + (int)(P.pij >> 16);
-                if (pdist) pdist[x] = __fsqrt_rn((float)fma(v2, v2, fma(v1, v1, v0 * v0)));
-            }
-            const int u = 3 * ((em + x) & (MGW_RE - 1));
-            ws.vr[u] = (float)v0; ws.vr[u + 1] = (float)v1; ws.vr[u + 2] = (float)v2;
-            ws.br[u] = (unsigned char)(tb >> 24); ws.br[u + 1] = (unsigned char)(tb >> 16); ws.br[u + 2] = (unsigned char)(tb >> 8);
-        }
-        __syncwarp();
-        mgw_out_pieces(ws, A, O, 3 * E0, 3 * (E0 + nb), lane);
-        __syncwarp();
-    }
-}
-
 // ---- the walk of a warp over its rows -------------------------------------------------------------
-// PHASE 0: count (returns the warp's edges, the same value on every lane); PHASE 1: emit from goff.
+// PHASE 0: count (returns the warp's edges, the same value on every lane); PHASE 1: list from goff.
 template <int PHASE>
-__device__ __forceinline__ unsigned long long mgw_walk(WSmem &ws, const FusedArgs &A, const RangeCtx &RC, int rid,
+__device__ __forceinline__ unsigned long long mgs_walk(SSmem &ws, const ScanArgs &A, const RangeCtx &RC, int rid,
                                                        unsigned *wm, unsigned long long goff, int lane) {
-    OutCtx O;
-    if (PHASE == 1) mgw_out_init(O, A, goff);
     unsigned long long c0, c1;
     mg_warp_range(RC, rid, c0, c1);
     int s, qa;
@@ -493,25 +347,32 @@ __device__ __forceinline__ unsigned long long mgw_walk(WSmem &ws, const FusedArg
         const int ia = N ? (qa + N - 1) / N : 0, ib = N ? (qb + N - 1) / N : 0;
         if (ib > ia) {
             const int mloc = R->mloc;
+            WCtx C;
+            mgs_ctx(C, A, R, s);
+            if (PHASE == 1) mgs_row_products(A, C, s, ia, ib, lane);
             if (mloc <= 0) {                       // invalid structure: empty rows
                 if (PHASE == 1)
-                    for (int i = ia + lane; i < ib; i += 32) A.row_ptr[R->first + i] = (int)goff;
-            } else if (N > MGW_NMAX || mloc > MGW_TL) {
-                WCtx C;
-                mgw_ctx(C, A, R, s);
-                if (PHASE == 0) total += mgw_rows_count(A, C, ia, ib, wm, midx, lane);
-                else {                             // these rows bypass the output rings
-                    mgw_out_finish(ws, A, O, 3 * (long long)goff, lane);
-                    goff = mgw_rows_emit(A, C, ia, ib, goff, lane);
-                    mgw_out_init(O, A, goff);
+                    for (int i = ia + lane; i < ib; i += 32) A.row_ptr[C.first + i] = (int)goff;
+            } else if (N > MGS_NMAX || mloc > MGS_TL) {
+                for (int i = ia; i < ib; ++i) {
+                    bool anybad = false;
+                    const unsigned cnt = mgs_row<PHASE == 1>(A, C, i, goff, lane, anybad);
+                    if (PHASE == 0) {
+                        if (anybad) atomicOr(A.status, __float_as_int(mg_wrap_x(C.gx + 3 * i).w) == 0 ? MGS_NONFINITE : MGS_OFFSET);
+                        total += cnt;
+                    } else {
+                        if (lane == 0) {
+                            A.row_ptr[C.first + i] = (int)goff;
+                            mgs_slice_rows(A, goff, cnt, 0u, cnt, C.first + i);
+                        }
+                        goff += cnt;
+                    }
                 }
-                #ifdef MG_PHASE_CLOCKS
+#ifdef MG_PHASE_CLOCKS
                 dbg_rows += ib - ia; dbg_seg += 1;
 #endif
             } else {
-                WCtx C;
-                mgw_ctx(C, A, R, s);
-                const bool live = mgw_stage<PHASE == 1>(ws, C, lane);
+                const bool live = mgs_stage(ws, C, lane);
                 const int nW = (mloc + 31) >> 5, recw = 32 * nW;
                 const int q0 = ia * N, q1 = ib * N, nblk = (q1 - q0 + 31) >> 5;
                 const float inv_N = 1.f / (float)N;
@@ -526,7 +387,7 @@ __device__ __forceinline__ unsigned long long mgw_walk(WSmem &ws, const FusedArg
                         const bool valid = q < q1;
                         int i = 0, j = 0;
                         if (valid) { i = mg_fdiv(q, inv_N); j = q - i * N; }
-                        const WPair p = mgw_pair(ws, C, valid, i, j);
+                        const SPair p = mgs_pair(ws, C, valid, i, j);
                         const int base = midx + b * recw;
                         const bool have = base + recw <= A.mask_words;
                         unsigned *mp = wm + base + lane;
@@ -535,7 +396,7 @@ __device__ __forceinline__ unsigned long long mgw_walk(WSmem &ws, const FusedArg
                             unsigned cnt = 0u;
 #pragma unroll 1
                             for (int w = 0; w < nW; ++w) {
-                                const unsigned m = mgw_word_mask(ws, C, p, i, j, w);
+                                const unsigned m = mgs_word_mask(ws, C, p, i, j, w);
                                 cnt += __popc(m);
                                 if (have) mp[32 * w] = m;
                             }
@@ -544,7 +405,7 @@ __device__ __forceinline__ unsigned long long mgw_walk(WSmem &ws, const FusedArg
                             unsigned cnt = 0u;
 #pragma unroll 1
                             for (int w = 0; w < nW; ++w)
-                                cnt += __popc(have ? __ldcg(mp + 32 * w) : mgw_word_mask(ws, C, p, i, j, w));
+                                cnt += __popc(have ? __ldcg(mp + 32 * w) : mgs_word_mask(ws, C, p, i, j, w));
                             unsigned incl = cnt;
 #pragma unroll
                             for (int o = 1; o < 32; o <<= 1) {
@@ -554,43 +415,37 @@ __device__ __forceinline__ unsigned long long mgw_walk(WSmem &ws, const FusedArg
                             const unsigned tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
                             if (valid && j == 0) A.row_ptr[C.first + i] = (int)(goff + incl - cnt);
                             if (tot == 0u) continue;
-                            // the pair's part of vec: (x_j - x_i + l) . L in FP64, coordinates as given
-                            if (valid) {
-                                const float *xi = C.gx + 3 * i, *xj = C.gx + 3 * j;
-                                const double f0 = ((double)xj[0] - (double)xi[0]) + (double)p.l0;
-                                const double f1 = ((double)xj[1] - (double)xi[1]) + (double)p.l1;
-                                const double f2 = ((double)xj[2] - (double)xi[2]) + (double)p.l2;
-                                PairRec P;
-                                P.bx = fma(f2, (double)C.a[6], fma(f1, (double)C.a[3], f0 * (double)C.a[0]));
-                                P.by = fma(f2, (double)C.a[7], fma(f1, (double)C.a[4], f0 * (double)C.a[1]));
-                                P.bz = fma(f2, (double)C.a[8], fma(f1, (double)C.a[5], f0 * (double)C.a[2]));
-                                P.plc = ((unsigned)(p.l0 + 128) << 24) | ((unsigned)(p.l1 + 128) << 16) |
-                                        ((unsigned)(p.l2 + 128) << 8);
-                                P.pij = (unsigned)i | ((unsigned)j << 16);
-                                ws.pr[lane] = P;
-                            }
+                            mgs_slice_rows(A, goff, tot, incl - cnt, cnt, C.first + i);
                             // passes of consecutive lanes whose hits fit the stash (nearly always one)
+                            const unsigned pc = ((unsigned)(p.l0 + 128) << 24) | ((unsigned)(p.l1 + 128) << 16) |
+                                                ((unsigned)(p.l2 + 128) << 8);
+                            const unsigned gj = (unsigned)(C.first + j);
                             unsigned done = 0u;
                             int l0 = 0;
                             while (done < tot) {
-                                const bool mine = lane >= l0 && incl - done <= MGW_STASH;
-                                const int nl = __popc(__ballot_sync(0xFFFFFFFFu, mine));   // >= 1: a lane has <= MGW_TL hits
+                                const bool mine = lane >= l0 && incl - done <= MGS_STASH;
+                                const int nl = __popc(__ballot_sync(0xFFFFFFFFu, mine));   // >= 1: a lane has <= MGS_TL hits
                                 const unsigned t = __shfl_sync(0xFFFFFFFFu, incl, l0 + nl - 1) - done;
                                 if (mine) {
                                     unsigned pos = incl - cnt - done;
-                                    const unsigned pc = (unsigned)lane << 8;
 #pragma unroll 1
                                     for (int w = 0; w < nW; ++w) {
-                                        unsigned mk = have ? __ldcg(mp + 32 * w) : mgw_word_mask(ws, C, p, i, j, w);
+                                        unsigned mk = have ? __ldcg(mp + 32 * w) : mgs_word_mask(ws, C, p, i, j, w);
                                         while (mk) {
                                             const int bit = __clz(mk);
                                             mk &= ~(0x80000000u >> bit);
-                                            ws.stash[pos++] = pc | (unsigned)(32 * w + bit);
+                                            ws.stash[pos++] = make_uint2(gj, pc + ws.tcode[32 * w + bit]);
                                         }
                                     }
                                 }
                                 __syncwarp();
-                                mgw_flush(ws, A, O, C.first, (long long)goff, (int)t, lane);
+                                {   // codes -> their final place in the stream
+                                    const long long room = A.capacity - (long long)goff;
+                                    const int lim = room >= (long long)t ? (int)t : (room > 0 ? (int)room : 0);
+                                    uint2 *dst = A.codes + goff;
+                                    for (int x = lane; x < lim; x += 32) dst[x] = ws.stash[x];
+                                }
+                                __syncwarp();
                                 goff += t;
                                 done += t;
                                 l0 += nl;
@@ -612,7 +467,6 @@ __device__ __forceinline__ unsigned long long mgw_walk(WSmem &ws, const FusedArg
         d[0] = (unsigned)(clock64() - wt0); d[1] = dbg_s0; d[2] = dbg_seg; d[3] = dbg_blk; d[4] = dbg_rows; d[5] = midx;
     }
 #endif
-    if (PHASE == 1) mgw_out_finish(ws, A, O, 3 * (long long)goff, lane);
     if (PHASE == 0) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) lane_total += __shfl_xor_sync(0xFFFFFFFFu, lane_total, o);
@@ -621,30 +475,30 @@ __device__ __forceinline__ unsigned long long mgw_walk(WSmem &ws, const FusedArg
     return goff;
 }
 
-// ---- the kernel -------------------------------------------------------------------------------------
-#ifndef MGF_MIN_CTAS
-#define MGF_MIN_CTAS 5
+// ---- launch 1 ---------------------------------------------------------------------------------------
+#ifndef MGS_MIN_CTAS
+#define MGS_MIN_CTAS 5
 #endif
-__global__ void __launch_bounds__(MGF_BLOCK, MGF_MIN_CTAS)
-mg_cutoff_fused_kernel(const __grid_constant__ FusedArgs A) {
+__global__ void __launch_bounds__(MGS_BLOCK, MGS_MIN_CTAS)
+mg_cutoff_scan_kernel(const __grid_constant__ ScanArgs A) {
     mg_grid_dependency_wait();
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    FusedSmem &sm = *reinterpret_cast<FusedSmem *>(smem_raw);
+    ScanSmem &sm = *reinterpret_cast<ScanSmem *>(smem_raw);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    WSmem &ws = sm.w[warp];
+    SSmem &ws = sm.w[warp];
     const unsigned epoch = *reinterpret_cast<volatile unsigned *>(A.ctl + 10) + 1u;   // tag of this call's slots
     RangeCtx RC;
-    mg_range_init(RC, A.rec, A.bpre, A.n_blocks, A.n_struct, (int)gridDim.x * MGF_WARPS, lane);
-    const int rid = (int)blockIdx.x * MGF_WARPS + warp;
-    unsigned *wm = A.wmask + (size_t)rid * MGW_MASK_WORDS;
-    MGF_STAMP(0)
-    const unsigned long long wtotal = mgw_walk<0>(ws, A, RC, rid, wm, 0ull, lane);
+    mg_range_init(RC, A.rec, A.bpre, A.n_blocks, A.n_struct, (int)gridDim.x * MGS_WARPS, lane);
+    const int rid = (int)blockIdx.x * MGS_WARPS + warp;
+    unsigned *wm = A.wmask + (size_t)rid * MGS_MASK_WORDS;
+    MGS_STAMP(0)
+    const unsigned long long wtotal = mgs_walk<0>(ws, A, RC, rid, wm, 0ull, lane);
     if (lane == 0) sm.wsum[warp] = (unsigned)wtotal;
     __syncthreads();
-    MGF_STAMP(1)
+    MGS_STAMP(1)
     unsigned long long total = 0ull, mine = 0ull;
 #pragma unroll
-    for (int w = 0; w < MGF_WARPS; ++w) {
+    for (int w = 0; w < MGS_WARPS; ++w) {
         if (w < warp) mine += sm.wsum[w];
         total += sm.wsum[w];
     }
@@ -667,15 +521,17 @@ mg_cutoff_fused_kernel(const __grid_constant__ FusedArgs A) {
         }
         __syncthreads();
         const unsigned long long before = sm.prefix;
-        MGF_STAMP(2)
+        MGS_STAMP(2)
         if (blockIdx.x == gridDim.x - 1 && tid == 0) {           // the last range knows the grand total
             const unsigned long long tot = before + total;
             *A.n_edges = (long long)tot;
             A.row_ptr[A.n_atoms] = (int)tot;
             if (tot > 0x7FFFFFFFull || (long long)tot > A.capacity) atomicOr(A.status, MGS_CAPACITY);
+            // the slice that starts at the end of the list (the write kernel reads one entry ahead)
+            if ((tot & (MGS_SLICE - 1)) == 0 && (long long)tot < A.capacity) A.slice_row[tot / MGS_SLICE] = A.n_atoms;
         }
-        mgw_walk<1>(ws, A, RC, rid, wm, before + mine, lane);
-        MGF_STAMP(3)
+        mgs_walk<1>(ws, A, RC, rid, wm, before + mine, lane);
+        MGS_STAMP(3)
     }
     // last CTA out: the call is over (count_only: it also adds the totals up)
     __syncthreads();
@@ -689,7 +545,7 @@ mg_cutoff_fused_kernel(const __grid_constant__ FusedArgs A) {
         unsigned long long sum = 0ull;
         for (int c = lane; c < (int)gridDim.x; c += 32) {
             unsigned long long v;
-            do { v = mg_ld_acquire(A.slots + c); } while ((unsigned)(v >> 32) != epoch);
+            while ((unsigned)((v = mg_ld_acquire(A.slots + c)) >> 32) != epoch) __nanosleep(100);
             sum += v & 0xFFFFFFFFull;
         }
 #pragma unroll
@@ -703,5 +559,127 @@ mg_cutoff_fused_kernel(const __grid_constant__ FusedArgs A) {
         A.ctl[11] = 0u;
         __threadfence();
         *reinterpret_cast<volatile unsigned *>(A.ctl + 10) = epoch;
+    }
+}
+
+// ---- launch 2 ---------------------------------------------------------------------------------------
+struct WriteArgs {
+    const uint2 *codes;
+    const int32_t *slice_row;
+    const int32_t *atom_struct;
+    const double *pos64, *lat64;
+    const int32_t *row_ptr;
+    const long long *n_edges;
+    int n_atoms;
+    long long capacity;
+    int32_t *src, *dst;
+    int8_t *offset;
+    float *vec, *dist;
+};
+
+#define MGWR_BLOCK 256
+
+// Edge e of the stream: src = the row that holds e (row_ptr), dst and tau from the code,
+// vec = ((x_dst - x_src) + tau) . L evaluated like the oracle does (Def. 3, R15: no FMA
+// contraction, sums left to right), rounded once to FP32.
+__global__ void __launch_bounds__(MGWR_BLOCK)
+mg_cutoff_write_kernel(const __grid_constant__ WriteArgs A) {
+    mg_grid_dependency_wait();
+    __shared__ int s_cnt[MGWR_BLOCK / 32][MGS_SLICE];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    int *cnt = s_cnt[warp];
+    const long long E = *A.n_edges < A.capacity ? *A.n_edges : A.capacity;       // edges to write
+    const long long n_slices = (E + MGS_SLICE - 1) / MGS_SLICE;
+    const bool al16 = ((reinterpret_cast<unsigned long long>(A.src) | reinterpret_cast<unsigned long long>(A.dst) |
+                        reinterpret_cast<unsigned long long>(A.vec)) & 15ull) == 0ull &&
+                      (reinterpret_cast<unsigned long long>(A.offset) & 3ull) == 0ull;
+    for (long long sl = (long long)blockIdx.x * (MGWR_BLOCK / 32) + warp; sl < n_slices;
+         sl += (long long)gridDim.x * (MGWR_BLOCK / 32)) {
+        const long long g0 = sl * MGS_SLICE;
+        const int n = (int)(E - g0 < MGS_SLICE ? E - g0 : MGS_SLICE);
+        // ---- rows of the slice's edges: row of edge p = r0 + number of rows r0 < r with row_ptr[r] <= g0 + p
+        const int r0 = __ldg(A.slice_row + sl);
+        __syncwarp();
+#pragma unroll
+        for (int x = 0; x < MGS_SLICE / 32; ++x) cnt[32 * x + lane] = 0;
+        __syncwarp();
+        for (int rb = r0 + 1;; rb += 32) {
+            const int r = rb + lane;
+            long long start = 1ll << 62;
+            if (r <= A.n_atoms) start = (long long)__ldg(A.row_ptr + r);
+            const bool in = start < g0 + n;
+            if (in) atomicAdd(&cnt[(int)(start - g0)], 1);        // start >= g0: row r0 holds g0 and r > r0
+            if (!__all_sync(0xFFFFFFFFu, in)) break;
+        }
+        __syncwarp();
+        // lane <-> edges 4 lane .. 4 lane + 3
+        int c4[4];
+#pragma unroll
+        for (int y = 0; y < 4; ++y) c4[y] = cnt[4 * lane + y];
+        int incl = c4[0] + c4[1] + c4[2] + c4[3];
+        const int own = incl;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+            if (lane >= o) incl += v;
+        }
+        int row = r0 + incl - own;
+        int gi[4], gj[4];
+        float v[4][3], d[4];
+        unsigned tb[4];
+#pragma unroll
+        for (int y = 0; y < 4; ++y) {
+            row += c4[y];
+            gi[y] = row;
+            const int p = 4 * lane + y;
+            gj[y] = row; tb[y] = 0u; v[y][0] = v[y][1] = v[y][2] = 0.f; d[y] = 0.f;
+            if (p < n) {
+                const uint2 code = __ldg(A.codes + g0 + p);
+                gj[y] = (int)code.x;
+                tb[y] = code.y;
+                const int s = __ldg(A.atom_struct + row);
+                const double *L = A.lat64 + 9 * (size_t)s;
+                const double *xi = A.pos64 + 3 * (size_t)row, *xj = A.pos64 + 3 * (size_t)gj[y];
+                // (double)(b - 128) without a conversion instruction: 2^52 + b has b in its low mantissa word
+                const double f0 = __dadd_rn(__dsub_rn(xj[0], xi[0]), __hiloint2double(0x43300000, (int)(code.y >> 24)) - 4503599627370624.0);
+                const double f1 = __dadd_rn(__dsub_rn(xj[1], xi[1]), __hiloint2double(0x43300000, (int)((code.y >> 16) & 0xFFu)) - 4503599627370624.0);
+                const double f2 = __dadd_rn(__dsub_rn(xj[2], xi[2]), __hiloint2double(0x43300000, (int)((code.y >> 8) & 0xFFu)) - 4503599627370624.0);
+                double w3[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+                    w3[c] = __dadd_rn(__dadd_rn(__dmul_rn(f0, L[c]), __dmul_rn(f1, L[3 + c])), __dmul_rn(f2, L[6 + c]));
+                v[y][0] = (float)w3[0]; v[y][1] = (float)w3[1]; v[y][2] = (float)w3[2];
+                if (A.dist)
+                    d[y] = __fsqrt_rn((float)__dadd_rn(__dadd_rn(__dmul_rn(w3[0], w3[0]), __dmul_rn(w3[1], w3[1])), __dmul_rn(w3[2], w3[2])));
+            }
+        }
+        const long long e = g0 + 4 * lane;
+        if (al16 && 4 * lane + 4 <= n) {
+            *reinterpret_cast<int4 *>(A.src + e) = make_int4(gi[0], gi[1], gi[2], gi[3]);
+            *reinterpret_cast<int4 *>(A.dst + e) = make_int4(gj[0], gj[1], gj[2], gj[3]);
+            float4 *pv = reinterpret_cast<float4 *>(A.vec + 3 * e);
+            pv[0] = make_float4(v[0][0], v[0][1], v[0][2], v[1][0]);
+            pv[1] = make_float4(v[1][1], v[1][2], v[2][0], v[2][1]);
+            pv[2] = make_float4(v[2][2], v[3][0], v[3][1], v[3][2]);
+            // 12 offset bytes: tau of four edges (code.y = b0 b1 b2 0 from the top byte down), signed
+            const unsigned t0 = tb[0] ^ 0x80808000u, t1 = tb[1] ^ 0x80808000u, t2 = tb[2] ^ 0x80808000u, t3 = tb[3] ^ 0x80808000u;
+            unsigned *po = reinterpret_cast<unsigned *>(A.offset + 3 * e);
+            po[0] = __byte_perm(t0, t1, 0x7123);       // bytes: t0.b3 t0.b2 t0.b1 t1.b3  (little endian)
+            po[1] = __byte_perm(t1, t2, 0x6712);       //        t1.b2 t1.b1 t2.b3 t2.b2
+            po[2] = __byte_perm(t2, t3, 0x5671);       //        t2.b1 t3.b3 t3.b2 t3.b1
+            if (A.dist) *reinterpret_cast<float4 *>(A.dist + e) = make_float4(d[0], d[1], d[2], d[3]);
+        } else {
+#pragma unroll
+            for (int y = 0; y < 4; ++y)
+                if (4 * lane + y < n) {
+                    A.src[e + y] = gi[y];
+                    A.dst[e + y] = gj[y];
+                    A.vec[3 * (e + y)] = v[y][0]; A.vec[3 * (e + y) + 1] = v[y][1]; A.vec[3 * (e + y) + 2] = v[y][2];
+                    const unsigned t = tb[y] ^ 0x80808000u;
+                    A.offset[3 * (e + y)] = (int8_t)(t >> 24); A.offset[3 * (e + y) + 1] = (int8_t)(t >> 16);
+                    A.offset[3 * (e + y) + 2] = (int8_t)(t >> 8);
+                    if (A.dist) A.dist[e + y] = d[y];
+                }
+        }
     }
 }

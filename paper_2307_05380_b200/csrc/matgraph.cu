@@ -13,7 +13,7 @@
 #include "prep.cuh"
 #include "cut_prep.cuh"
 #include "cutoff_pairs.cuh"
-#include "cut_fused.cuh"
+#include "cut_scan.cuh"
 #include "knn_small.cuh"
 #include "knn_pairs.cuh"
 
@@ -36,7 +36,16 @@ struct mg_ctx {
     int fused_occ = 0, fused_coop = 0;    // fused cutoff kernel: CTAs per SM, cooperative launch accepted
     int legacy = 0;                       // MATGRAPH_LEGACY=1: the two-launch cutoff path of round 1
     unsigned long long *d_slots = nullptr;// [sm_count * fused_occ] per-CTA edge totals tagged with the call's epoch
-    unsigned *d_fmask = nullptr;          // [sm_count * fused_occ, MGF_MASK_WORDS] hit masks kept from count to emit
+    unsigned *d_fmask = nullptr;          // [sm_count * fused_occ * MGS_WARPS, MGS_MASK_WORDS] hit masks kept from count to list
+    // products of the scan kernel for the write kernel (cut_scan.cuh)
+    uint2 *d_codes = nullptr;             // [code_cap] (dst, tau) of every edge, in output order
+    int32_t *d_slice_row = nullptr;       // [code_cap / MGS_SLICE + 2]
+    size_t code_cap = 0;
+    double *d_pos64 = nullptr;            // [atom64_cap, 3]
+    size_t atom64_cap = 0;
+    double *d_lat64 = nullptr;            // [lat64_cap, 9]
+    size_t lat64_cap = 0;
+    int write_occ = 0;
     CutRec *d_crec = nullptr;             // per-structure records of the cutoff path (cut_prep.cuh)
     unsigned long long *d_bpre = nullptr; // cost prefix over the prep blocks
     size_t crec_cap = 0;
@@ -138,15 +147,16 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
                          cudaMalloc(&c->d_wclock, 64 * (size_t)(c->cut_warps + 2048) * sizeof(unsigned)) != cudaSuccess)) { mg_destroy(c); return MG_ERR_CUDA; }
     }
     c->legacy = getenv("MATGRAPH_FUSED") ? 0 : 1;   // fused kernel: correct, not yet faster
-    if (cudaFuncSetAttribute(mg_cutoff_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)sizeof(FusedSmem)) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->fused_occ, mg_cutoff_fused_kernel, MGF_BLOCK, sizeof(FusedSmem));
-    if (c->fused_occ < 1) { mg_destroy(c); return MG_ERR_CUDA; }
+    if (cudaFuncSetAttribute(mg_cutoff_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)sizeof(ScanSmem)) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->fused_occ, mg_cutoff_scan_kernel, MGS_BLOCK, sizeof(ScanSmem));
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->write_occ, mg_cutoff_write_kernel, MGWR_BLOCK, 0);
+    if (c->fused_occ < 1 || c->write_occ < 1) { mg_destroy(c); return MG_ERR_CUDA; }
     {
         const size_t nc = (size_t)c->sm_count * c->fused_occ;
         if (cudaMalloc(&c->d_slots, nc * sizeof(unsigned long long)) != cudaSuccess ||
             cudaMemset(c->d_slots, 0, nc * sizeof(unsigned long long)) != cudaSuccess ||
-            cudaMalloc(&c->d_fmask, nc * MGF_MASK_WORDS * sizeof(unsigned)) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
+            cudaMalloc(&c->d_fmask, nc * MGS_WARPS * MGS_MASK_WORDS * sizeof(unsigned)) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
         int coop = 0;
         cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device);
         c->fused_coop = coop && !getenv("MATGRAPH_NO_COOP");
@@ -166,6 +176,10 @@ extern "C" void mg_destroy(mg_ctx *c) {
     cudaFree(c->d_wclock);
     cudaFree(c->d_slots);
     cudaFree(c->d_fmask);
+    cudaFree(c->d_codes);
+    cudaFree(c->d_slice_row);
+    cudaFree(c->d_pos64);
+    cudaFree(c->d_lat64);
     cudaFree(c->d_crec);
     cudaFree(c->d_bpre);
     cudaFree(c->d_rec);
@@ -203,6 +217,20 @@ extern "C" mg_status mg_reserve(mg_ctx *c, int32_t n_struct, int32_t n_atoms) {
         c->d_atom_struct = nullptr; c->atom_cap = 0;
         MG_CUDA(cudaMalloc(&c->d_atom_struct, cap * sizeof(int32_t)));
         c->atom_cap = cap;
+    }
+    if ((size_t)n_atoms + 1 > c->atom64_cap) {
+        const size_t cap = (size_t)n_atoms + 1025;
+        cudaFree(c->d_pos64);
+        c->d_pos64 = nullptr; c->atom64_cap = 0;
+        MG_CUDA(cudaMalloc(&c->d_pos64, cap * 3 * sizeof(double)));
+        c->atom64_cap = cap;
+    }
+    if ((size_t)n_struct + 1 > c->lat64_cap) {
+        const size_t cap = (size_t)n_struct + 1025;
+        cudaFree(c->d_lat64);
+        c->d_lat64 = nullptr; c->lat64_cap = 0;
+        MG_CUDA(cudaMalloc(&c->d_lat64, cap * 9 * sizeof(double)));
+        c->lat64_cap = cap;
     }
     if ((size_t)n_atoms + 1 > c->rowptr_cap) {
         const size_t cap = (size_t)n_atoms + 1025;
@@ -361,29 +389,54 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
         c->launches += 1;
     }
     if (!c->legacy) {
-        FusedArgs F;
+        // the code stream holds one 8-byte code per edge the caller's arrays can take
+        const size_t need = count_only ? 0 : (size_t)o->capacity;
+        if (need > c->code_cap) {
+            cudaFree(c->d_codes); cudaFree(c->d_slice_row);
+            c->d_codes = nullptr; c->d_slice_row = nullptr; c->code_cap = 0;
+            const size_t cap = need + need / 8 + 4096;
+            MG_CUDA(cudaMalloc(&c->d_codes, cap * sizeof(uint2)));
+            MG_CUDA(cudaMalloc(&c->d_slice_row, (cap / MGS_SLICE + 2) * sizeof(int32_t)));
+            c->code_cap = cap;
+        }
+        ScanArgs F;
         F.pos = pos; F.lattice = lat; F.n_struct = n_struct; F.n_atoms = n_atoms; F.r_c = r_c;
-        F.row_ptr = o->row_ptr; F.src = o->src; F.dst = o->dst; F.offset = o->offset;
-        F.vec = o->vec; F.dist = o->dist; F.capacity = o->capacity; F.n_edges = (long long *)o->n_edges;
+        F.row_ptr = o->row_ptr; F.capacity = o->capacity; F.n_edges = (long long *)o->n_edges;
         F.rec = c->d_crec; F.bpre = c->d_bpre; F.n_blocks = n_blocks;
         F.wmask = c->d_fmask;
-        F.mask_words = c->mask_words < MGW_MASK_WORDS ? c->mask_words : MGW_MASK_WORDS;
+        F.mask_words = c->mask_words < MGS_MASK_WORDS ? c->mask_words : MGS_MASK_WORDS;
         F.slots = c->d_slots; F.ctl = c->d_ctl; F.status = c->d_ctl + 4;
         F.count_only = count_only;
+        F.codes = c->d_codes; F.slice_row = c->d_slice_row; F.atom_struct = c->d_atom_struct;
+        F.pos64 = c->d_pos64; F.lat64 = c->d_lat64;
         F.dbg = c->d_wclock;
         int grid = c->sm_count * c->fused_occ;
-        const int cap_grid = (n_atoms + MGF_WARPS) / MGF_WARPS;   // >= 1 row per warp
+        const int cap_grid = (n_atoms + MGS_WARPS) / MGS_WARPS;   // >= 1 row per warp
         if (grid > cap_grid) grid = cap_grid;
         if (prof) cudaEventRecord(c->ev[1], st);
-        cudaError_t e = launch_after(c, mg_cutoff_fused_kernel, grid, MGF_BLOCK, sizeof(FusedSmem), st, F, c->fused_coop != 0);
+        cudaError_t e = launch_after(c, mg_cutoff_scan_kernel, grid, MGS_BLOCK, sizeof(ScanSmem), st, F, c->fused_coop != 0);
         if (e != cudaSuccess && c->fused_coop) {        // cooperative + programmatic launch refused together
             cudaGetLastError();
             c->fused_coop = 0;
-            e = launch_after(c, mg_cutoff_fused_kernel, grid, MGF_BLOCK, sizeof(FusedSmem), st, F, false);
+            e = launch_after(c, mg_cutoff_scan_kernel, grid, MGS_BLOCK, sizeof(ScanSmem), st, F, false);
         }
         MG_CUDA(e);
         c->launches += 1;
-        if (prof) { cudaEventRecord(c->ev[2], st); cudaEventRecord(c->ev[3], st); c->pend_kind = 0; }
+        if (prof) cudaEventRecord(c->ev[2], st);
+        if (!count_only && o->capacity > 0) {
+            WriteArgs W;
+            W.codes = c->d_codes; W.slice_row = c->d_slice_row; W.atom_struct = c->d_atom_struct;
+            W.pos64 = c->d_pos64; W.lat64 = c->d_lat64; W.row_ptr = o->row_ptr;
+            W.n_edges = (const long long *)o->n_edges; W.n_atoms = n_atoms; W.capacity = o->capacity;
+            W.src = o->src; W.dst = o->dst; W.offset = o->offset; W.vec = o->vec; W.dist = o->dist;
+            const long long n_slices = (o->capacity + MGS_SLICE - 1) / MGS_SLICE;
+            long long wgrid = (n_slices + MGWR_BLOCK / 32 - 1) / (MGWR_BLOCK / 32);
+            const long long wmax = (long long)c->sm_count * c->write_occ;
+            if (wgrid > wmax) wgrid = wmax;
+            MG_CUDA(launch_after(c, mg_cutoff_write_kernel, (int)wgrid, MGWR_BLOCK, 0, st, W));
+            c->launches += 1;
+        }
+        if (prof) { cudaEventRecord(c->ev[3], st); c->pend_kind = 0; }
         return MG_OK;
     }
     CutoffArgs A;
