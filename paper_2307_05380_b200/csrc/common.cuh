@@ -7,7 +7,7 @@
 #include <stdint.h>
 
 #define MG_SMALL_MAX_ATOMS 64      // structures up to this size take the pair-lane "small" path
-#define MG_PAIR_TL 128             // cells of the per-warp translation table of the fused cutoff kernel
+#define MG_PAIR_TL 320             // cells of the per-warp translation table of the fused cutoff kernel
 #define MG_BLOCK 128               // threads per CTA of the graph kernels
 #define MG_WARPS (MG_BLOCK / 32)
 #define MG_TASK_BUDGET 6144u        // candidates per cutoff task (one warp, one row group)

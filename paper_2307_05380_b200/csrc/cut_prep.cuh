@@ -37,12 +37,13 @@
 #define MG_C_BLOCK_WIDE 500.f
 #define MG_C_EDGE 3.3f             // per emitted edge
 #endif
-// ... of the fused kernel (cut_fused.cuh): per emitted edge, per candidate cell of its rows path
-#ifndef MG_CF_EDGE
-#define MG_CF_EDGE 7.f
-#endif
-#ifndef MG_C_ROWCELL
-#define MG_C_ROWCELL 12.f
+// ... of the scan kernel (cut_scan.cuh), in cycles: see the comment where they are used
+#ifndef MG_CS_BLOCK
+#define MG_CS_BLOCK 735.f
+#define MG_CS_GROUP 182.f
+#define MG_CS_EDGE 17.f
+#define MG_CS_STRUCT 4000.f
+#define MG_CS_ROWCELL 25.f
 #endif
 // ... and of the KNN launch: per candidate cell, per block of 32 pairs, per source row (selection),
 // per structure
@@ -152,17 +153,24 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
             const float percell = mloc > 256 ? 11.f + 900.f / (float)N : (mloc > 128 ? MG_C_CELL_WIDE : (mloc > 64 ? MG_C_CELL_MID : MG_C_CELL));
             const float perblock = mloc > 256 ? 120.f + 16000.f / (float)N : (mloc > 128 ? MG_C_BLOCK_WIDE : MG_C_BLOCK);
             const float c = ((float)((mloc + 3) & ~3) * percell + perblock) * (1.f / 32.f) +
-                            (A.rows_cost ? MG_CF_EDGE : MG_C_EDGE) * lam / (float)N + MG_STRUCT_COST / ((float)N * (float)N);
+                            MG_C_EDGE * lam / (float)N + MG_STRUCT_COST / ((float)N * (float)N);
             // KNN: one launch, no edge stream (constants from a sweep over four seeds of config 2 and config 4)
             const float ck = ((float)((mloc + 3) & ~3) * MG_KC_CELL + MG_KC_BLOCK) * (1.f / 32.f) + MG_KC_ROW / (float)N +
                              MG_KC_STRUCT / ((float)N * (float)N);
             // (KNN above the staging limit: warp-per-row growing-radius search, about 40 per pair-cell)
             const float ckb = 40.f * (float)mloc / 32.f + 600.f / (float)N;
-            // cutoff, structures the pair-lane path does not take (cut_fused.cuh: one candidate per lane
-            // and ~60 instructions, evaluated in both phases)
-            const float crow = MG_C_ROWCELL * (float)mloc + MG_CF_EDGE * lam / (float)N;
+            // cutoff, scan kernel (cut_scan.cuh), in cycles a warp spends (fit on BASELINE configs[2], per-warp
+            // clocks of an MG_PHASE_CLOCKS build): per block of 32 pairs 735 + 182 per group of four cells it
+            // evaluates (two groups per trip), 17 per edge, 4000 per structure visited; a structure the
+            // pair-lane path does not take costs about 25 per candidate cell of a pair
+            float groups = 0.f;
+            for (int w0 = 0; w0 < mloc; w0 += 32) groups += (float)((((min(32, mloc - w0) + 3) >> 2) + 1) & ~1);
+            const float cscan = (MG_CS_BLOCK + MG_CS_GROUP * groups) * (1.f / 32.f) + MG_CS_EDGE * lam / (float)N +
+                                MG_CS_STRUCT / ((float)N * (float)N);
+            const float crow = MG_CS_ROWCELL * (float)mloc + MG_CS_EDGE * lam / (float)N + MG_CS_STRUCT / ((float)N * (float)N);
             const bool rows = N > MG_SMALL_MAX_ATOMS || mloc > MG_PAIR_TL;
-            r.paircost = (unsigned)fminf(16.f * (A.k > 0 ? (N > MG_SMALL_MAX_ATOMS ? ckb : ck) : (rows && A.rows_cost ? crow : c)) + 1.f, 16777216.f);
+            const float cnew = 0.25f * (rows ? crow : cscan);      // (quarter cycles: keeps the prefix far from overflow)
+            r.paircost = (unsigned)fminf(16.f * (A.k > 0 ? (N > MG_SMALL_MAX_ATOMS ? ckb : ck) : (A.rows_cost ? cnew : c)) + 1.f, 16777216.f);
         }
         r.pad = 0;
         cost = (unsigned long long)((long long)N * N) * r.paircost;

@@ -33,7 +33,8 @@
 #define MGS_TL MG_PAIR_TL          // cells of a warp's table
 #define MGS_NMAX MG_SMALL_MAX_ATOMS // atoms of a staged structure
 #define MGS_STASH 256              // codes per pass
-#define MGS_MASK_WORDS 4096        // 32-bit words of mask scratch per warp
+#define MGS_CHUNK 512              // codes per chunk of the pool
+#define MGS_MAXCH 128              // chunks a warp can hold (beyond: its rows are listed again in the second phase)
 #define MGS_SLICE 128              // edges per slice of the write kernel
 
 struct ScanArgs {
@@ -47,15 +48,16 @@ struct ScanArgs {
     const CutRec *rec;
     const unsigned long long *bpre;
     int n_blocks;
-    unsigned *wmask;               // [n_ranges, MGS_MASK_WORDS]
-    int mask_words;                // words of a warp's scratch that may be used (tests: less)
+    uint2 *pool;                   // [n_pool, MGS_CHUNK] codes of the warps before their final place is known
+    int n_pool;                    // chunks of the pool (tests: less)
     unsigned long long *slots;     // [gridDim.x] epoch << 32 | edges of the CTA
-    unsigned *ctl;                 // [10] epoch of the last finished call, [11] CTAs done
+    unsigned *ctl;                 // [10] epoch of the last finished call, [11] CTAs done, [12] pool chunks taken
     unsigned *status;
     int count_only;
     // products for the write kernel
     uint2 *codes;                  // [capacity] .x = dst, .y = (tau + 128) bytes << 8
-    int32_t *slice_row;            // [ceil(capacity / MGS_SLICE) + 1] row of edge MGS_SLICE * k
+    int4 *slice_row;               // [ceil(capacity / MGS_SLICE) + 1] for edge MGS_SLICE * k: its row, first atom and
+                                   // end of the atoms of the row's structure, the structure
     int32_t *atom_struct;          // [n_atoms]
     double *pos64;                 // [n_atoms, 3]
     double *lat64;                 // [n_struct, 9]
@@ -78,11 +80,14 @@ struct SSmem {                         // one warp's shared memory
     unsigned tcode[MGS_TL];            // t0 << 24 | t1 << 16 | t2 << 8
     float4 x[MGS_NMAX];                // wrapped fractional coordinates, .w = packed integer parts
     uint2 stash[MGS_STASH];            // codes of one pass
+    unsigned mk[MGS_TL / 32][32];      // hit masks of the current block
+    int chunks[MGS_MAXCH];             // the warp's chunks of the pool
 };
 
 struct ScanSmem {
     SSmem w[MGS_WARPS];
     unsigned wsum[MGS_WARPS];
+    int wok[MGS_WARPS];
     unsigned long long prefix;
     int last;
 };
@@ -277,20 +282,49 @@ __device__ __forceinline__ void mgs_row_products(const ScanArgs &A, const WCtx &
 // The edges [g0, g0 + n) belong to rows in such a way that edge g0 + p is in the row `row` on the lane
 // that holds p in [excl, excl + cnt): every MGS_SLICE-th edge records its row.
 __device__ __forceinline__ void mgs_slice_rows(const ScanArgs &A, unsigned long long g0, unsigned n, unsigned excl,
-                                               unsigned cnt, int row) {
+                                               unsigned cnt, int row, int first, int natoms, int s) {
     const unsigned long long b0 = (g0 + MGS_SLICE - 1) & ~(unsigned long long)(MGS_SLICE - 1);
     for (unsigned long long b = b0; b < g0 + n && (long long)b < A.capacity; b += MGS_SLICE) {
         const unsigned p = (unsigned)(b - g0);
-        if (p >= excl && p < excl + cnt) A.slice_row[b / MGS_SLICE] = row;
+        if (p >= excl && p < excl + cnt) A.slice_row[b / MGS_SLICE] = make_int4(row, first, first + natoms, s);
     }
 }
 
-// One source row: returns its edges; LIST: writes their codes from goff on (any order inside the row).
+// ---- the code pool ------------------------------------------------------------------------------------
+// While a warp finds its edges it does not know where they go in the output, so their codes go to
+// chunks of MGS_CHUNK codes taken from a pool (one atomic per chunk); the chunk list stays in the warp's
+// shared memory.  Local position p of the warp's codes lives at chunk list[p / MGS_CHUNK], p % MGS_CHUNK.
+struct PoolState {
+    unsigned wcount;       // codes of the warp so far (the same on every lane)
+    int nch;               // chunks taken
+    bool ok;               // false: the pool or the list ran out; the warp only counts from then on and
+                           // lists its rows again in the second phase (mgs_walk<1>)
+};
+
+__device__ __forceinline__ uint2 *mgs_pool_addr(const ScanArgs &A, const SSmem &ws, unsigned p) {
+    return A.pool + (size_t)ws.chunks[p / MGS_CHUNK] * MGS_CHUNK + (p % MGS_CHUNK);
+}
+
+// Make sure the chunks for local positions < upto exist.
+__device__ __forceinline__ void mgs_pool_reserve(const ScanArgs &A, SSmem &ws, PoolState &P, unsigned upto, int lane) {
+    while (P.ok && (unsigned)P.nch * MGS_CHUNK < upto) {
+        int c = 0;
+        if (lane == 0) c = (int)atomicAdd(A.ctl + 12, 1u);
+        c = __shfl_sync(0xFFFFFFFFu, c, 0);
+        if (c >= A.n_pool || P.nch >= MGS_MAXCH) { P.ok = false; break; }
+        if (lane == 0) ws.chunks[P.nch] = c;
+        P.nch += 1;
+        __syncwarp();
+    }
+}
+
+// One source row: returns its edges; their codes go to the pool (PHASE 0) or to their final place from
+// goff on (PHASE 1), in any order inside the row.
 // Tables of 32 cells and more: lane <-> cell (decoded once per 32 cells), loop over the targets j.
 // Smaller tables: lane <-> (target, cell), floor(32 / mloc) targets per pass.
-template <bool LIST>
-__device__ __forceinline__ unsigned mgs_row(const ScanArgs &A, const WCtx &C, int i, unsigned long long goff, int lane,
-                                            bool &anybad) {
+template <int PHASE>
+__device__ __forceinline__ unsigned mgs_row(const ScanArgs &A, SSmem &ws, PoolState &P, const WCtx &C, int i,
+                                            unsigned long long goff, int lane, bool &anybad) {
     const float4 xi = mg_wrap_x(C.gx + 3 * i);
     const int M12 = C.m1 * C.m2;
     unsigned cnt = 0u;
@@ -309,11 +343,14 @@ __device__ __forceinline__ unsigned mgs_row(const ScanArgs &A, const WCtx &C, in
             const bool hit = cv && j < C.N && mgs_cand(C, xi, i, j, t0, t1, t2, tau, bad);
             anybad = anybad || bad;
             const unsigned bal = __ballot_sync(0xFFFFFFFFu, hit);
-            if (LIST && hit) {
-                const long long e = (long long)(goff + cnt) + __popc(bal & ((1u << lane) - 1u));
-                if (e < A.capacity)
-                    A.codes[e] = make_uint2((unsigned)(C.first + j), ((unsigned)(tau[0] + 128) << 24) |
-                                            ((unsigned)(tau[1] + 128) << 16) | ((unsigned)(tau[2] + 128) << 8));
+            if (PHASE == 0 && bal) mgs_pool_reserve(A, ws, P, P.wcount + cnt + 32u, lane);
+            if (hit) {
+                const uint2 code = make_uint2((unsigned)(C.first + j), ((unsigned)(tau[0] + 128) << 24) |
+                                              ((unsigned)(tau[1] + 128) << 16) | ((unsigned)(tau[2] + 128) << 8));
+                const unsigned k = cnt + __popc(bal & ((1u << lane) - 1u));
+                if (PHASE == 0) {
+                    if (P.ok) *mgs_pool_addr(A, ws, P.wcount + k) = code;
+                } else if ((long long)(goff + k) < A.capacity) A.codes[goff + k] = code;
             }
             cnt += __popc(bal);
         }
@@ -322,20 +359,23 @@ __device__ __forceinline__ unsigned mgs_row(const ScanArgs &A, const WCtx &C, in
 }
 
 // ---- the walk of a warp over its rows -------------------------------------------------------------
-// PHASE 0: count (returns the warp's edges, the same value on every lane); PHASE 1: list from goff.
+// PHASE 0 (find): hits of every block -> codes in the pool, row_ptr = offsets LOCAL to the warp, the
+//   products of the rows (atom_struct, pos64, lat64); returns the warp's edge count (on every lane).
+// PHASE 1 (list again): for a warp whose codes did not fit the pool: the same walk with the final
+//   offset goff known: row_ptr, slice records and codes go straight to their place.
 template <int PHASE>
 __device__ __forceinline__ unsigned long long mgs_walk(SSmem &ws, const ScanArgs &A, const RangeCtx &RC, int rid,
-                                                       unsigned *wm, unsigned long long goff, int lane) {
+                                                       PoolState &P, int &row_lo, int &row_hi,
+                                                       unsigned long long goff, int lane) {
     unsigned long long c0, c1;
     mg_warp_range(RC, rid, c0, c1);
     int s, qa;
     mg_range_start(RC, c0, s, qa, lane);
-    int midx = 0;
-    unsigned total = 0u, lane_total = 0u;          // warp-uniform part (rows path), per-lane part (pair-lane path)
 #ifdef MG_PHASE_CLOCKS
     const long long wt0 = clock64();
     const int dbg_s0 = s;
-    int dbg_seg = 0, dbg_blk = 0, dbg_rows = 0;
+    int dbg_seg = 0, dbg_blk = 0, dbg_rows = 0, dbg_grp = 0;
+    const unsigned long long dbg_g0 = goff;
 #endif
     for (; s < A.n_struct; ++s, qa = 0) {
         const CutRec *R = A.rec + s;
@@ -349,22 +389,25 @@ __device__ __forceinline__ unsigned long long mgs_walk(SSmem &ws, const ScanArgs
             const int mloc = R->mloc;
             WCtx C;
             mgs_ctx(C, A, R, s);
-            if (PHASE == 1) mgs_row_products(A, C, s, ia, ib, lane);
+            if (PHASE == 0) {
+                mgs_row_products(A, C, s, ia, ib, lane);
+                if (row_lo < 0) row_lo = C.first + ia;
+                row_hi = C.first + ib;
+            }
+            // where the next edge goes: local position (find) or final position (list again)
+#define MGS_HERE (PHASE == 0 ? (unsigned long long)P.wcount : goff)
             if (mloc <= 0) {                       // invalid structure: empty rows
-                if (PHASE == 1)
-                    for (int i = ia + lane; i < ib; i += 32) A.row_ptr[C.first + i] = (int)goff;
+                for (int i = ia + lane; i < ib; i += 32) A.row_ptr[C.first + i] = (int)MGS_HERE;
             } else if (N > MGS_NMAX || mloc > MGS_TL) {
                 for (int i = ia; i < ib; ++i) {
                     bool anybad = false;
-                    const unsigned cnt = mgs_row<PHASE == 1>(A, C, i, goff, lane, anybad);
+                    if (lane == 0) A.row_ptr[C.first + i] = (int)MGS_HERE;
+                    const unsigned cnt = mgs_row<PHASE>(A, ws, P, C, i, goff, lane, anybad);
                     if (PHASE == 0) {
                         if (anybad) atomicOr(A.status, __float_as_int(mg_wrap_x(C.gx + 3 * i).w) == 0 ? MGS_NONFINITE : MGS_OFFSET);
-                        total += cnt;
+                        P.wcount += cnt;
                     } else {
-                        if (lane == 0) {
-                            A.row_ptr[C.first + i] = (int)goff;
-                            mgs_slice_rows(A, goff, cnt, 0u, cnt, C.first + i);
-                        }
+                        if (lane == 0) mgs_slice_rows(A, goff, cnt, 0u, cnt, C.first + i, C.first, C.N, s);
                         goff += cnt;
                     }
                 }
@@ -373,13 +416,12 @@ __device__ __forceinline__ unsigned long long mgs_walk(SSmem &ws, const ScanArgs
 #endif
             } else {
                 const bool live = mgs_stage(ws, C, lane);
-                const int nW = (mloc + 31) >> 5, recw = 32 * nW;
+                const int nW = (mloc + 31) >> 5;
                 const int q0 = ia * N, q1 = ib * N, nblk = (q1 - q0 + 31) >> 5;
                 const float inv_N = 1.f / (float)N;
                 if (!live) {
-                    if (lane == 0) atomicOr(A.status, MGS_NONFINITE);
-                    if (PHASE == 1)
-                        for (int i = ia + lane; i < ib; i += 32) A.row_ptr[C.first + i] = (int)goff;
+                    if (PHASE == 0 && lane == 0) atomicOr(A.status, MGS_NONFINITE);
+                    for (int i = ia + lane; i < ib; i += 32) A.row_ptr[C.first + i] = (int)MGS_HERE;
                 } else {
 #pragma unroll 1
                     for (int b = 0; b < nblk; ++b) {
@@ -388,91 +430,121 @@ __device__ __forceinline__ unsigned long long mgs_walk(SSmem &ws, const ScanArgs
                         int i = 0, j = 0;
                         if (valid) { i = mg_fdiv(q, inv_N); j = q - i * N; }
                         const SPair p = mgs_pair(ws, C, valid, i, j);
-                        const int base = midx + b * recw;
-                        const bool have = base + recw <= A.mask_words;
-                        unsigned *mp = wm + base + lane;
-                        if (PHASE == 0) {
-                            if (valid && !p.ok) atomicOr(A.status, MGS_OFFSET);
-                            unsigned cnt = 0u;
+                        if (PHASE == 0 && valid && !p.ok) atomicOr(A.status, MGS_OFFSET);
+                        unsigned cnt = 0u;
 #pragma unroll 1
-                            for (int w = 0; w < nW; ++w) {
-                                const unsigned m = mgs_word_mask(ws, C, p, i, j, w);
-                                cnt += __popc(m);
-                                if (have) mp[32 * w] = m;
-                            }
-                            lane_total += cnt;         // reduced over the lanes at the end
-                        } else {
-                            unsigned cnt = 0u;
-#pragma unroll 1
-                            for (int w = 0; w < nW; ++w)
-                                cnt += __popc(have ? __ldcg(mp + 32 * w) : mgs_word_mask(ws, C, p, i, j, w));
-                            unsigned incl = cnt;
+                        for (int w = 0; w < nW; ++w) {
+                            const unsigned m = mgs_word_mask(ws, C, p, i, j, w);
+                            cnt += __popc(m);
+                            ws.mk[w][lane] = m;
+                        }
+                        unsigned incl = cnt;
 #pragma unroll
-                            for (int o = 1; o < 32; o <<= 1) {
-                                const unsigned v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
-                                if (lane >= o) incl += v;
-                            }
-                            const unsigned tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
-                            if (valid && j == 0) A.row_ptr[C.first + i] = (int)(goff + incl - cnt);
-                            if (tot == 0u) continue;
-                            mgs_slice_rows(A, goff, tot, incl - cnt, cnt, C.first + i);
-                            // passes of consecutive lanes whose hits fit the stash (nearly always one)
-                            const unsigned pc = ((unsigned)(p.l0 + 128) << 24) | ((unsigned)(p.l1 + 128) << 16) |
-                                                ((unsigned)(p.l2 + 128) << 8);
-                            const unsigned gj = (unsigned)(C.first + j);
-                            unsigned done = 0u;
-                            int l0 = 0;
-                            while (done < tot) {
-                                const bool mine = lane >= l0 && incl - done <= MGS_STASH;
-                                const int nl = __popc(__ballot_sync(0xFFFFFFFFu, mine));   // >= 1: a lane has <= MGS_TL hits
-                                const unsigned t = __shfl_sync(0xFFFFFFFFu, incl, l0 + nl - 1) - done;
-                                if (mine) {
-                                    unsigned pos = incl - cnt - done;
+                        for (int o = 1; o < 32; o <<= 1) {
+                            const unsigned v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+                            if (lane >= o) incl += v;
+                        }
+                        const unsigned tot = __shfl_sync(0xFFFFFFFFu, incl, 31);
+                        if (valid && j == 0) A.row_ptr[C.first + i] = (int)(MGS_HERE + incl - cnt);
+                        if (tot == 0u) continue;
+                        if (PHASE == 1) mgs_slice_rows(A, goff, tot, incl - cnt, cnt, C.first + i, C.first, C.N, s);
+                        if (PHASE == 0) mgs_pool_reserve(A, ws, P, P.wcount + tot, lane);
+                        if (PHASE == 0 && !P.ok) { P.wcount += tot; continue; }       // count only from here on
+                        // passes of consecutive lanes whose hits fit the stash (nearly always one)
+                        const unsigned pc = ((unsigned)(p.l0 + 128) << 24) | ((unsigned)(p.l1 + 128) << 16) |
+                                            ((unsigned)(p.l2 + 128) << 8);
+                        const unsigned gj = (unsigned)(C.first + j);
+                        unsigned done = 0u;
+                        int l0 = 0;
+                        while (done < tot) {
+                            const bool mine = lane >= l0 && incl - done <= MGS_STASH;
+                            const int nl = __popc(__ballot_sync(0xFFFFFFFFu, mine));   // >= 1: a lane has <= MGS_TL hits
+                            const unsigned t = __shfl_sync(0xFFFFFFFFu, incl, l0 + nl - 1) - done;
+                            if (mine) {
+                                unsigned pos = incl - cnt - done;
 #pragma unroll 1
-                                    for (int w = 0; w < nW; ++w) {
-                                        unsigned mk = have ? __ldcg(mp + 32 * w) : mgs_word_mask(ws, C, p, i, j, w);
-                                        while (mk) {
-                                            const int bit = __clz(mk);
-                                            mk &= ~(0x80000000u >> bit);
-                                            ws.stash[pos++] = make_uint2(gj, pc + ws.tcode[32 * w + bit]);
-                                        }
+                                for (int w = 0; w < nW; ++w) {
+                                    unsigned mk = ws.mk[w][lane];
+                                    while (mk) {
+                                        const int bit = __clz(mk);
+                                        mk &= ~(0x80000000u >> bit);
+                                        ws.stash[pos++] = make_uint2(gj, pc + ws.tcode[32 * w + bit]);
                                     }
                                 }
-                                __syncwarp();
-                                {   // codes -> their final place in the stream
-                                    const long long room = A.capacity - (long long)goff;
-                                    const int lim = room >= (long long)t ? (int)t : (room > 0 ? (int)room : 0);
-                                    uint2 *dst = A.codes + goff;
-                                    for (int x = lane; x < lim; x += 32) dst[x] = ws.stash[x];
-                                }
-                                __syncwarp();
-                                goff += t;
-                                done += t;
-                                l0 += nl;
                             }
+                            __syncwarp();
+                            if (PHASE == 0) {          // codes -> the pool, at the warp's local positions
+                                for (unsigned x = lane; x < t; x += 32) *mgs_pool_addr(A, ws, P.wcount + x) = ws.stash[x];
+                                P.wcount += t;
+                            } else {                   // codes -> their final place in the stream
+                                const long long room = A.capacity - (long long)goff;
+                                const int lim = room >= (long long)t ? (int)t : (room > 0 ? (int)room : 0);
+                                uint2 *dst = A.codes + goff;
+                                for (int x = lane; x < lim; x += 32) dst[x] = ws.stash[x];
+                                goff += t;
+                            }
+                            __syncwarp();
+                            done += t;
+                            l0 += nl;
                         }
                     }
                 }
-                midx += nblk * recw;
 #ifdef MG_PHASE_CLOCKS
                 dbg_blk += nblk; dbg_seg += 1;
+                for (int w = 0; w < nW; ++w) dbg_grp += nblk * ((((min(32, mloc - 32 * w) + 3) >> 2) + 1) & ~1);
 #endif
             }
+#undef MGS_HERE
         }
         if (!more) break;
     }
 #ifdef MG_PHASE_CLOCKS
     if (lane == 0 && A.dbg) {
         unsigned *d = A.dbg + 4 * 2048 + 16 * rid + 8 * PHASE;
-        d[0] = (unsigned)(clock64() - wt0); d[1] = dbg_s0; d[2] = dbg_seg; d[3] = dbg_blk; d[4] = dbg_rows; d[5] = midx;
+        d[0] = (unsigned)(clock64() - wt0); d[1] = dbg_s0; d[2] = dbg_seg; d[3] = dbg_blk; d[4] = dbg_rows; d[5] = P.nch;
+        d[6] = dbg_grp; d[7] = PHASE == 1 ? (unsigned)(goff - dbg_g0) : P.wcount;
     }
 #endif
-    if (PHASE == 0) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) lane_total += __shfl_xor_sync(0xFFFFFFFFu, lane_total, o);
-        goff = (unsigned long long)(total + lane_total);
+    return PHASE == 0 ? (unsigned long long)P.wcount : goff;
+}
+
+// Second phase of a warp whose codes are in the pool: codes -> their final place, row_ptr from local to
+// final offsets, and for every MGS_SLICE-th edge of the output the record the write kernel starts from.
+__device__ __forceinline__ void mgs_place(const ScanArgs &A, const SSmem &ws, unsigned total, int row_lo, int row_hi,
+                                          unsigned long long base, int lane) {
+    {
+        const long long room = A.capacity - (long long)base;
+        const unsigned lim = room >= (long long)total ? total : (room > 0 ? (unsigned)room : 0u);
+        uint2 *dst = A.codes + base;
+        unsigned x = lane;
+        for (; x + 96 < lim; x += 128) {               // four loads in flight
+            const uint2 c0 = *mgs_pool_addr(A, ws, x), c1 = *mgs_pool_addr(A, ws, x + 32),
+                        c2 = *mgs_pool_addr(A, ws, x + 64), c3 = *mgs_pool_addr(A, ws, x + 96);
+            dst[x] = c0; dst[x + 32] = c1; dst[x + 64] = c2; dst[x + 96] = c3;
+        }
+        for (; x < lim; x += 32) dst[x] = *mgs_pool_addr(A, ws, x);
     }
-    return goff;
+    for (int r0 = row_lo; r0 < row_hi; r0 += 32) {
+        const int r = r0 + lane;
+        unsigned v = total, vn = total;
+        if (r < row_hi) v = (unsigned)A.row_ptr[r];
+        if (lane == 31 && r + 1 < row_hi) vn = (unsigned)A.row_ptr[r + 1];
+        const unsigned down = __shfl_down_sync(0xFFFFFFFFu, v, 1);
+        if (lane < 31) vn = down;                   // (rows past row_hi hold `total`)
+        __syncwarp();
+        if (r < row_hi) {
+            A.row_ptr[r] = (int)(base + v);
+            if (vn > v) {
+                const unsigned long long b0 = (base + v + MGS_SLICE - 1) & ~(unsigned long long)(MGS_SLICE - 1);
+                if (b0 < base + vn && (long long)b0 < A.capacity) {
+                    const int s = A.atom_struct[r];
+                    const int first = A.rec[s].first, nat = A.rec[s].natoms;
+                    for (unsigned long long b = b0; b < base + vn && (long long)b < A.capacity; b += MGS_SLICE)
+                        A.slice_row[b / MGS_SLICE] = make_int4(r, first, first + nat, s);
+                }
+            }
+        }
+    }
 }
 
 // ---- launch 1 ---------------------------------------------------------------------------------------
@@ -490,9 +562,11 @@ mg_cutoff_scan_kernel(const __grid_constant__ ScanArgs A) {
     RangeCtx RC;
     mg_range_init(RC, A.rec, A.bpre, A.n_blocks, A.n_struct, (int)gridDim.x * MGS_WARPS, lane);
     const int rid = (int)blockIdx.x * MGS_WARPS + warp;
-    unsigned *wm = A.wmask + (size_t)rid * MGS_MASK_WORDS;
     MGS_STAMP(0)
-    const unsigned long long wtotal = mgs_walk<0>(ws, A, RC, rid, wm, 0ull, lane);
+    PoolState P;
+    P.wcount = 0u; P.nch = 0; P.ok = true;
+    int row_lo = -1, row_hi = -1;
+    const unsigned long long wtotal = mgs_walk<0>(ws, A, RC, rid, P, row_lo, row_hi, 0ull, lane);
     if (lane == 0) sm.wsum[warp] = (unsigned)wtotal;
     __syncthreads();
     MGS_STAMP(1)
@@ -527,10 +601,9 @@ mg_cutoff_scan_kernel(const __grid_constant__ ScanArgs A) {
             *A.n_edges = (long long)tot;
             A.row_ptr[A.n_atoms] = (int)tot;
             if (tot > 0x7FFFFFFFull || (long long)tot > A.capacity) atomicOr(A.status, MGS_CAPACITY);
-            // the slice that starts at the end of the list (the write kernel reads one entry ahead)
-            if ((tot & (MGS_SLICE - 1)) == 0 && (long long)tot < A.capacity) A.slice_row[tot / MGS_SLICE] = A.n_atoms;
         }
-        mgs_walk<1>(ws, A, RC, rid, wm, before + mine, lane);
+        if (P.ok) mgs_place(A, ws, (unsigned)wtotal, row_lo, row_hi, before + mine, lane);
+        else mgs_walk<1>(ws, A, RC, rid, P, row_lo, row_hi, before + mine, lane);
         MGS_STAMP(3)
     }
     // last CTA out: the call is over (count_only: it also adds the totals up)
@@ -557,15 +630,17 @@ mg_cutoff_scan_kernel(const __grid_constant__ ScanArgs A) {
     }
     if (tid == 0) {
         A.ctl[11] = 0u;
+        A.ctl[12] = 0u;
         __threadfence();
         *reinterpret_cast<volatile unsigned *>(A.ctl + 10) = epoch;
     }
 }
 
+
 // ---- launch 2 ---------------------------------------------------------------------------------------
 struct WriteArgs {
     const uint2 *codes;
-    const int32_t *slice_row;
+    const int4 *slice_row;
     const int32_t *atom_struct;
     const double *pos64, *lat64;
     const int32_t *row_ptr;
@@ -578,41 +653,85 @@ struct WriteArgs {
 };
 
 #define MGWR_BLOCK 256
+#define MGWR_WARPS (MGWR_BLOCK / 32)
+#define MGWR_WIN MGS_NMAX          // atoms of the position window a warp stages per slice
+#ifndef MGWR_MIN_CTAS
+#define MGWR_MIN_CTAS 3
+#endif
 
-// Edge e of the stream: src = the row that holds e (row_ptr), dst and tau from the code,
-// vec = ((x_dst - x_src) + tau) . L evaluated like the oracle does (Def. 3, R15: no FMA
-// contraction, sums left to right), rounded once to FP32.
-__global__ void __launch_bounds__(MGWR_BLOCK)
+// ((x_dst - x_src) + tau) . L evaluated like the oracle does (Def. 3, R15: no FMA contraction,
+// sums left to right); tb = (tau + 128) bytes << 8.
+__device__ __forceinline__ void mgwr_vec(const double xi[3], const double xj[3], unsigned tb, const double L[9], double w3[3]) {
+    // (double)(b - 128) without a conversion instruction: 2^52 + b has b in its low mantissa word
+    const double f0 = __dadd_rn(__dsub_rn(xj[0], xi[0]), __hiloint2double(0x43300000, (int)(tb >> 24)) - 4503599627370624.0);
+    const double f1 = __dadd_rn(__dsub_rn(xj[1], xi[1]), __hiloint2double(0x43300000, (int)((tb >> 16) & 0xFFu)) - 4503599627370624.0);
+    const double f2 = __dadd_rn(__dsub_rn(xj[2], xi[2]), __hiloint2double(0x43300000, (int)((tb >> 8) & 0xFFu)) - 4503599627370624.0);
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+        w3[c] = __dadd_rn(__dadd_rn(__dmul_rn(f0, L[c]), __dmul_rn(f1, L[3 + c])), __dmul_rn(f2, L[6 + c]));
+}
+
+// A warp takes slices of MGS_SLICE consecutive edges; lane <-> edges 4 lane .. 4 lane + 3 of the slice.
+// Per slice, two rounds of loads: (1) its record (row of the first edge, the atoms of that row's
+// structure, the structure) and the lane's four codes; (2) the row_ptr entries after that row, the
+// structure's lattice and positions (FP64 copies of the scan kernel).  An edge of a later structure
+// (the slice crosses a structure boundary) takes its operands from global memory instead.
+__global__ void __launch_bounds__(MGWR_BLOCK, MGWR_MIN_CTAS)
 mg_cutoff_write_kernel(const __grid_constant__ WriteArgs A) {
     mg_grid_dependency_wait();
-    __shared__ int s_cnt[MGWR_BLOCK / 32][MGS_SLICE];
+    __shared__ int s_cnt[MGWR_WARPS][MGS_SLICE];
+    __shared__ double s_x[MGWR_WARPS][3 * MGWR_WIN];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     int *cnt = s_cnt[warp];
+    double *xs = s_x[warp];
     const long long E = *A.n_edges < A.capacity ? *A.n_edges : A.capacity;       // edges to write
     const long long n_slices = (E + MGS_SLICE - 1) / MGS_SLICE;
     const bool al16 = ((reinterpret_cast<unsigned long long>(A.src) | reinterpret_cast<unsigned long long>(A.dst) |
                         reinterpret_cast<unsigned long long>(A.vec)) & 15ull) == 0ull &&
                       (reinterpret_cast<unsigned long long>(A.offset) & 3ull) == 0ull;
-    for (long long sl = (long long)blockIdx.x * (MGWR_BLOCK / 32) + warp; sl < n_slices;
-         sl += (long long)gridDim.x * (MGWR_BLOCK / 32)) {
+    const long long stride = (long long)gridDim.x * MGWR_WARPS;
+    long long sl = (long long)blockIdx.x * MGWR_WARPS + warp;
+    int4 info = make_int4(0, 0, 0, 0);
+    if (sl < n_slices) info = __ldg(A.slice_row + sl);
+    for (; sl < n_slices; sl += stride) {
         const long long g0 = sl * MGS_SLICE;
         const int n = (int)(E - g0 < MGS_SLICE ? E - g0 : MGS_SLICE);
-        // ---- rows of the slice's edges: row of edge p = r0 + number of rows r0 < r with row_ptr[r] <= g0 + p
-        const int r0 = __ldg(A.slice_row + sl);
+        const int r0 = info.x, a_lo = info.y, a_hi = info.z, s0 = info.w;
+        if (sl + stride < n_slices) info = __ldg(A.slice_row + sl + stride);     // the next slice's record
+        // ---- round of loads: codes (the stream is padded beyond the last edge), row_ptr, lattice, positions
+        const uint4 *cp = reinterpret_cast<const uint4 *>(A.codes + g0 + 4 * lane);
+        const uint4 ca = __ldg(cp), cb = __ldg(cp + 1);
+        double L[9];
+        {
+            const double *pl = A.lat64 + 9 * (size_t)s0;
+#pragma unroll
+            for (int c = 0; c < 9; ++c) L[c] = __ldg(pl + c);
+        }
+        // (the first 32 row_ptr entries after r0 in the same round of loads)
+        long long start0 = 1ll << 62;
+        if (r0 + 1 + lane <= A.n_atoms) start0 = (long long)__ldg(A.row_ptr + r0 + 1 + lane);
         __syncwarp();
+        {
+            const int nx = 3 * min(MGWR_WIN, a_hi - a_lo);
+            const double *px = A.pos64 + 3 * (size_t)a_lo;
+            for (int x = lane; x < nx; x += 32) xs[x] = __ldg(px + x);
+        }
 #pragma unroll
         for (int x = 0; x < MGS_SLICE / 32; ++x) cnt[32 * x + lane] = 0;
         __syncwarp();
+        // ---- rows: row of edge p = r0 + number of rows r > r0 with row_ptr[r] <= g0 + p
         for (int rb = r0 + 1;; rb += 32) {
             const int r = rb + lane;
-            long long start = 1ll << 62;
-            if (r <= A.n_atoms) start = (long long)__ldg(A.row_ptr + r);
+            long long start = start0;
+            if (rb != r0 + 1) {
+                start = 1ll << 62;
+                if (r <= A.n_atoms) start = (long long)__ldg(A.row_ptr + r);
+            }
             const bool in = start < g0 + n;
-            if (in) atomicAdd(&cnt[(int)(start - g0)], 1);        // start >= g0: row r0 holds g0 and r > r0
+            if (in) atomicAdd(&cnt[(int)(start - g0)], 1);        // start > g0: row r0 holds g0 and r > r0
             if (!__all_sync(0xFFFFFFFFu, in)) break;
         }
         __syncwarp();
-        // lane <-> edges 4 lane .. 4 lane + 3
         int c4[4];
 #pragma unroll
         for (int y = 0; y < 4; ++y) c4[y] = cnt[4 * lane + y];
@@ -625,34 +744,38 @@ mg_cutoff_write_kernel(const __grid_constant__ WriteArgs A) {
         }
         int row = r0 + incl - own;
         int gi[4], gj[4];
-        float v[4][3], d[4];
         unsigned tb[4];
+        gj[0] = (int)ca.x; tb[0] = ca.y; gj[1] = (int)ca.z; tb[1] = ca.w;
+        gj[2] = (int)cb.x; tb[2] = cb.y; gj[3] = (int)cb.z; tb[3] = cb.w;
+        float v[4][3], d[4];
+        const int win = min(MGWR_WIN, a_hi - a_lo);
 #pragma unroll
         for (int y = 0; y < 4; ++y) {
             row += c4[y];
             gi[y] = row;
-            const int p = 4 * lane + y;
-            gj[y] = row; tb[y] = 0u; v[y][0] = v[y][1] = v[y][2] = 0.f; d[y] = 0.f;
-            if (p < n) {
-                const uint2 code = __ldg(A.codes + g0 + p);
-                gj[y] = (int)code.x;
-                tb[y] = code.y;
+            v[y][0] = v[y][1] = v[y][2] = 0.f; d[y] = 0.f;
+            if (4 * lane + y >= n) { gj[y] = row; tb[y] = 0x80808000u; continue; }
+            double w3[3];
+            const unsigned wi = (unsigned)(row - a_lo), wj = (unsigned)(gj[y] - a_lo);
+            if (wi < (unsigned)win && wj < (unsigned)win) {
+                mgwr_vec(xs + 3 * wi, xs + 3 * wj, tb[y], L, w3);
+            } else {                                   // another structure, or a structure above the window
                 const int s = __ldg(A.atom_struct + row);
-                const double *L = A.lat64 + 9 * (size_t)s;
-                const double *xi = A.pos64 + 3 * (size_t)row, *xj = A.pos64 + 3 * (size_t)gj[y];
-                // (double)(b - 128) without a conversion instruction: 2^52 + b has b in its low mantissa word
-                const double f0 = __dadd_rn(__dsub_rn(xj[0], xi[0]), __hiloint2double(0x43300000, (int)(code.y >> 24)) - 4503599627370624.0);
-                const double f1 = __dadd_rn(__dsub_rn(xj[1], xi[1]), __hiloint2double(0x43300000, (int)((code.y >> 16) & 0xFFu)) - 4503599627370624.0);
-                const double f2 = __dadd_rn(__dsub_rn(xj[2], xi[2]), __hiloint2double(0x43300000, (int)((code.y >> 8) & 0xFFu)) - 4503599627370624.0);
-                double w3[3];
+                double L2[9], xi[3], xj[3];
 #pragma unroll
-                for (int c = 0; c < 3; ++c)
-                    w3[c] = __dadd_rn(__dadd_rn(__dmul_rn(f0, L[c]), __dmul_rn(f1, L[3 + c])), __dmul_rn(f2, L[6 + c]));
-                v[y][0] = (float)w3[0]; v[y][1] = (float)w3[1]; v[y][2] = (float)w3[2];
-                if (A.dist)
-                    d[y] = __fsqrt_rn((float)__dadd_rn(__dadd_rn(__dmul_rn(w3[0], w3[0]), __dmul_rn(w3[1], w3[1])), __dmul_rn(w3[2], w3[2])));
+                for (int c = 0; c < 9; ++c) L2[c] = __ldg(A.lat64 + 9 * (size_t)s + c);
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    xi[c] = __ldg(A.pos64 + 3 * (size_t)row + c);
+                    xj[c] = __ldg(A.pos64 + 3 * (size_t)gj[y] + c);
+                }
+                mgwr_vec(xi, xj, tb[y], L2, w3);
             }
+            v[y][0] = (float)w3[0]; v[y][1] = (float)w3[1]; v[y][2] = (float)w3[2];
+            if (A.dist)
+                d[y] = __fsqrt_rn((float)__dadd_rn(__dadd_rn(__dmul_rn(w3[0], w3[0]), __dmul_rn(w3[1], w3[1])), __dmul_rn(w3[2], w3[2])));
         }
+        // ---- stores: four edges per lane, every array in aligned 16-byte (offset: 4-byte) pieces
         const long long e = g0 + 4 * lane;
         if (al16 && 4 * lane + 4 <= n) {
             *reinterpret_cast<int4 *>(A.src + e) = make_int4(gi[0], gi[1], gi[2], gi[3]);
@@ -661,12 +784,12 @@ mg_cutoff_write_kernel(const __grid_constant__ WriteArgs A) {
             pv[0] = make_float4(v[0][0], v[0][1], v[0][2], v[1][0]);
             pv[1] = make_float4(v[1][1], v[1][2], v[2][0], v[2][1]);
             pv[2] = make_float4(v[2][2], v[3][0], v[3][1], v[3][2]);
-            // 12 offset bytes: tau of four edges (code.y = b0 b1 b2 0 from the top byte down), signed
+            // 12 offset bytes: tau of four edges (a code's .y = b0 b1 b2 0 from the top byte down), signed
             const unsigned t0 = tb[0] ^ 0x80808000u, t1 = tb[1] ^ 0x80808000u, t2 = tb[2] ^ 0x80808000u, t3 = tb[3] ^ 0x80808000u;
             unsigned *po = reinterpret_cast<unsigned *>(A.offset + 3 * e);
-            po[0] = __byte_perm(t0, t1, 0x7123);       // bytes: t0.b3 t0.b2 t0.b1 t1.b3  (little endian)
-            po[1] = __byte_perm(t1, t2, 0x6712);       //        t1.b2 t1.b1 t2.b3 t2.b2
-            po[2] = __byte_perm(t2, t3, 0x5671);       //        t2.b1 t3.b3 t3.b2 t3.b1
+            po[0] = __byte_perm(t0, t1, 0x7123);       // bytes in memory: t0.b3 t0.b2 t0.b1 t1.b3
+            po[1] = __byte_perm(t1, t2, 0x6712);       //                  t1.b2 t1.b1 t2.b3 t2.b2
+            po[2] = __byte_perm(t2, t3, 0x5671);       //                  t2.b1 t3.b3 t3.b2 t3.b1
             if (A.dist) *reinterpret_cast<float4 *>(A.dist + e) = make_float4(d[0], d[1], d[2], d[3]);
         } else {
 #pragma unroll

@@ -36,10 +36,11 @@ struct mg_ctx {
     int fused_occ = 0, fused_coop = 0;    // fused cutoff kernel: CTAs per SM, cooperative launch accepted
     int legacy = 0;                       // MATGRAPH_LEGACY=1: the two-launch cutoff path of round 1
     unsigned long long *d_slots = nullptr;// [sm_count * fused_occ] per-CTA edge totals tagged with the call's epoch
-    unsigned *d_fmask = nullptr;          // [sm_count * fused_occ * MGS_WARPS, MGS_MASK_WORDS] hit masks kept from count to list
+    uint2 *d_pool = nullptr;              // [pool_chunks, MGS_CHUNK] codes before their final place is known
+    size_t pool_chunks = 0;
     // products of the scan kernel for the write kernel (cut_scan.cuh)
     uint2 *d_codes = nullptr;             // [code_cap] (dst, tau) of every edge, in output order
-    int32_t *d_slice_row = nullptr;       // [code_cap / MGS_SLICE + 2]
+    int4 *d_slice_row = nullptr;          // [code_cap / MGS_SLICE + 2]
     size_t code_cap = 0;
     double *d_pos64 = nullptr;            // [atom64_cap, 3]
     size_t atom64_cap = 0;
@@ -156,7 +157,7 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
         const size_t nc = (size_t)c->sm_count * c->fused_occ;
         if (cudaMalloc(&c->d_slots, nc * sizeof(unsigned long long)) != cudaSuccess ||
             cudaMemset(c->d_slots, 0, nc * sizeof(unsigned long long)) != cudaSuccess ||
-            cudaMalloc(&c->d_fmask, nc * MGS_WARPS * MGS_MASK_WORDS * sizeof(unsigned)) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
+            false) { mg_destroy(c); return MG_ERR_CUDA; }
         int coop = 0;
         cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, device);
         c->fused_coop = coop && !getenv("MATGRAPH_NO_COOP");
@@ -175,7 +176,7 @@ extern "C" void mg_destroy(mg_ctx *c) {
     cudaFree(c->d_wmask);
     cudaFree(c->d_wclock);
     cudaFree(c->d_slots);
-    cudaFree(c->d_fmask);
+    cudaFree(c->d_pool);
     cudaFree(c->d_codes);
     cudaFree(c->d_slice_row);
     cudaFree(c->d_pos64);
@@ -396,23 +397,33 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
             c->d_codes = nullptr; c->d_slice_row = nullptr; c->code_cap = 0;
             const size_t cap = need + need / 8 + 4096;
             MG_CUDA(cudaMalloc(&c->d_codes, cap * sizeof(uint2)));
-            MG_CUDA(cudaMalloc(&c->d_slice_row, (cap / MGS_SLICE + 2) * sizeof(int32_t)));
+            MG_CUDA(cudaMalloc(&c->d_slice_row, (cap / MGS_SLICE + 2) * sizeof(int4)));
             c->code_cap = cap;
+        }
+        int grid = c->sm_count * c->fused_occ;
+        const int cap_grid = (n_atoms + MGS_WARPS) / MGS_WARPS;   // >= 1 row per warp
+        if (grid > cap_grid) grid = cap_grid;
+        // pool: the edges the caller can take, in chunks, plus one partly filled chunk per warp
+        const size_t want_chunks = count_only ? 0 : need / MGS_CHUNK + (size_t)grid * MGS_WARPS + 8;
+        if (want_chunks > c->pool_chunks) {
+            cudaFree(c->d_pool);
+            c->d_pool = nullptr; c->pool_chunks = 0;
+            const size_t cap = want_chunks + want_chunks / 8;
+            MG_CUDA(cudaMalloc(&c->d_pool, cap * MGS_CHUNK * sizeof(uint2)));
+            c->pool_chunks = cap;
         }
         ScanArgs F;
         F.pos = pos; F.lattice = lat; F.n_struct = n_struct; F.n_atoms = n_atoms; F.r_c = r_c;
         F.row_ptr = o->row_ptr; F.capacity = o->capacity; F.n_edges = (long long *)o->n_edges;
         F.rec = c->d_crec; F.bpre = c->d_bpre; F.n_blocks = n_blocks;
-        F.wmask = c->d_fmask;
-        F.mask_words = c->mask_words < MGS_MASK_WORDS ? c->mask_words : MGS_MASK_WORDS;
+        F.pool = c->d_pool;
+        // (test knob MATGRAPH_MASK_WORDS < 4096: a pool this small, so that warps list their rows again)
+        F.n_pool = count_only ? 0 : (c->mask_words < MG_MASK_WORDS ? c->mask_words : (int)(c->pool_chunks < 0x7FFFFFFF ? c->pool_chunks : 0x7FFFFFFF));
         F.slots = c->d_slots; F.ctl = c->d_ctl; F.status = c->d_ctl + 4;
         F.count_only = count_only;
         F.codes = c->d_codes; F.slice_row = c->d_slice_row; F.atom_struct = c->d_atom_struct;
         F.pos64 = c->d_pos64; F.lat64 = c->d_lat64;
         F.dbg = c->d_wclock;
-        int grid = c->sm_count * c->fused_occ;
-        const int cap_grid = (n_atoms + MGS_WARPS) / MGS_WARPS;   // >= 1 row per warp
-        if (grid > cap_grid) grid = cap_grid;
         if (prof) cudaEventRecord(c->ev[1], st);
         cudaError_t e = launch_after(c, mg_cutoff_scan_kernel, grid, MGS_BLOCK, sizeof(ScanSmem), st, F, c->fused_coop != 0);
         if (e != cudaSuccess && c->fused_coop) {        // cooperative + programmatic launch refused together
