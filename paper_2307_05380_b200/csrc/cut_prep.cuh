@@ -85,7 +85,11 @@ struct CutPrepArgs {
     float *hint;                   // KNN, [n_struct] or NULL: largest k-th distance of the previous call
                                    // (read when use_hint, then reset to 0: the graph kernel maxes into it)
     int use_hint;
-    int rows_cost;                 // cutoff: cost model of the fused kernel (rows path for large structures / tables)
+    int rows_cost;                 // cutoff: cost model of the scan kernel (cut_scan.cuh)
+    const float *pos;              // with xw4: positions of the batch
+    float4 *xw4;                   // [n_atoms] or NULL: wrapped fractional coordinates x - floor(x), .w = the integer
+                                   // parts packed (mg_wrap_x): written by the blocks after the first n_sblocks ones
+    int n_sblocks;                 // blocks that hold structures (the grid may have more: they only wrap coordinates)
     CutRec *rec;                   // [n_struct]
     unsigned long long *bpre;      // [blocks + 1] block sums -> exclusive prefix; [blocks] = total
     unsigned *ctl;                 // [7] blocks done
@@ -95,6 +99,19 @@ struct CutPrepArgs {
 __global__ void __launch_bounds__(MG_CP_BLOCK)
 mg_cut_prep_kernel(const CutPrepArgs A) {
     mg_grid_dependency_wait();      // the kernels of the previous call still read rec / bpre
+    if (A.xw4) {                     // K2 staging: every atom's wrapped coordinates, once per call
+        const int nx = (int)gridDim.x - A.n_sblocks;       // (no extra blocks: the structure blocks do it)
+        const int b0 = nx > 0 ? (int)blockIdx.x - A.n_sblocks : (int)blockIdx.x, nb = nx > 0 ? nx : (int)gridDim.x;
+        if (b0 >= 0)
+            for (int g = b0 * MG_CP_BLOCK + (int)threadIdx.x; g < A.n_atoms; g += nb * MG_CP_BLOCK) {
+                const float x0 = A.pos[3 * (size_t)g], x1 = A.pos[3 * (size_t)g + 1], x2 = A.pos[3 * (size_t)g + 2];
+                const float g0 = floorf(x0), g1 = floorf(x1), g2 = floorf(x2);
+                const bool ok = fabsf(g0) <= 500.f && fabsf(g1) <= 500.f && fabsf(g2) <= 500.f;   // false for NaN / inf
+                const int kk = ((int)g0 + 512) | (((int)g1 + 512) << 10) | (((int)g2 + 512) << 20);
+                A.xw4[g] = make_float4(x0 - g0, x1 - g1, x2 - g2, __int_as_float(ok ? kk : 0));
+            }
+        if ((int)blockIdx.x >= A.n_sblocks) return;
+    }
     __shared__ unsigned long long s_warp[MG_CP_BLOCK / 32];
     __shared__ bool s_last;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -195,16 +212,16 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
         A.rec[s] = r;
     }
     if (threadIdx.x == 0) A.bpre[blockIdx.x] = btotal;
-    if (gridDim.x <= 32) return;          // few blocks: the graph kernels scan the raw sums themselves
+    if (A.n_sblocks <= 32) return;        // few blocks: the graph kernels scan the raw sums themselves
     // ---- last block out: exclusive scan of the block sums (serial per thread chunk, 64 bit)
     __threadfence();
     __syncthreads();
-    if (threadIdx.x == 0) s_last = atomicAdd(A.ctl + 7, 1u) == gridDim.x - 1;
+    if (threadIdx.x == 0) s_last = atomicAdd(A.ctl + 7, 1u) == (unsigned)A.n_sblocks - 1u;
     __syncthreads();
     if (!s_last) return;
     __threadfence();
     __shared__ unsigned long long s_part[MG_CP_BLOCK];
-    const int nb = (int)gridDim.x, per = (nb + MG_CP_BLOCK - 1) / MG_CP_BLOCK;
+    const int nb = A.n_sblocks, per = (nb + MG_CP_BLOCK - 1) / MG_CP_BLOCK;
     const int b = threadIdx.x * per, e = min(nb, b + per);
     unsigned long long sum = 0ull;
     for (int g = b; g < e; ++g) sum += __ldcg(A.bpre + g);

@@ -34,12 +34,17 @@
 #define MGS_NMAX MG_SMALL_MAX_ATOMS // atoms of a staged structure
 #define MGS_STASH 256              // codes per pass
 #define MGS_CHUNK 512              // codes per chunk of the pool
-#define MGS_MAXCH 128              // chunks a warp can hold (beyond: its rows are listed again in the second phase)
+#define MGS_MAXCH 64               // chunks a range can hold (beyond: its rows are listed again in the second phase)
+#ifndef MGS_WAVES
+#define MGS_WAVES 1
+#endif
+//                // ranges per warp: wave w of the grid holds the ranges w * n_warps .. (w + 1) * n_warps - 1
 #define MGS_SLICE 128              // edges per slice of the write kernel
 
 struct ScanArgs {
     const float *pos;
     const float *lattice;
+    const float4 *xw4;             // [n_atoms] wrapped coordinates + packed integer parts (cut_prep.cuh)
     int n_struct, n_atoms;
     float r_c;
     int32_t *row_ptr;
@@ -50,11 +55,16 @@ struct ScanArgs {
     int n_blocks;
     uint2 *pool;                   // [n_pool, MGS_CHUNK] codes of the warps before their final place is known
     int n_pool;                    // chunks of the pool (tests: less)
-    unsigned long long *slots;     // [gridDim.x] epoch << 32 | edges of the CTA
+    unsigned long long *slots;     // [MGS_WAVES, gridDim.x] epoch << 32 | edges of the CTA's ranges of a wave
     unsigned *ctl;                 // [10] epoch of the last finished call, [11] CTAs done, [12] pool chunks taken
     unsigned *status;
     int count_only;
-    // products for the write kernel
+    // the caller's edge arrays: written by this kernel itself when write_here
+    int32_t *src, *dst;
+    int8_t *offset;
+    float *vec, *dist;
+    int write_here;
+    // products for the write kernel (write_here == 0)
     uint2 *codes;                  // [capacity] .x = dst, .y = (tau + 128) bytes << 8
     int4 *slice_row;               // [ceil(capacity / MGS_SLICE) + 1] for edge MGS_SLICE * k: its row, first atom and
                                    // end of the atoms of the row's structure, the structure
@@ -81,14 +91,15 @@ struct SSmem {                         // one warp's shared memory
     float4 x[MGS_NMAX];                // wrapped fractional coordinates, .w = packed integer parts
     uint2 stash[MGS_STASH];            // codes of one pass
     unsigned mk[MGS_TL / 32][32];      // hit masks of the current block
-    int chunks[MGS_MAXCH];             // the warp's chunks of the pool
+    int chunks[MGS_WAVES][MGS_MAXCH];  // the chunks of the pool that hold the codes of the warp's ranges
+    int wave[MGS_WAVES][8];            // per range: edges, chunks, pool ok, first row, end of rows, edges of the warps before (2 words)
 };
 
 struct ScanSmem {
     SSmem w[MGS_WARPS];
     unsigned wsum[MGS_WARPS];
     int wok[MGS_WARPS];
-    unsigned long long prefix;
+    unsigned long long prefix, wave_all;
     int last;
 };
 
@@ -99,6 +110,7 @@ struct WCtx {
     int m0, m1, m2, mloc;
     float nr2, win, rc;
     const float *gx;       // positions of the structure's first atom
+    const float4 *xw;      // ... and their wrapped copies
     const float *lat;
     int first, N;
 };
@@ -118,6 +130,7 @@ __device__ __forceinline__ void mgs_ctx(WCtx &C, const ScanArgs &A, const CutRec
     C.first = R->first;
     C.N = R->natoms;
     C.gx = A.pos + 3 * (size_t)R->first;
+    C.xw = A.xw4 + R->first;
 }
 
 
@@ -127,7 +140,7 @@ __device__ __forceinline__ bool mgs_stage(SSmem &ws, const WCtx &C, int lane) {
     __syncwarp();
     bool ok = true;
     for (int j = lane; j < C.N; j += 32) {
-        const float4 xw = mg_wrap_x(C.gx + 3 * j);
+        const float4 xw = C.xw[j];
         ok = ok && __float_as_int(xw.w) != 0;
         ws.x[j] = xw;
     }
@@ -242,7 +255,7 @@ __device__ __forceinline__ unsigned mgs_word_mask(const SSmem &ws, const WCtx &C
 // Candidate (j, t) of row i: hit?  tau (relative to the coordinates as given) in tau[3].
 __device__ __forceinline__ bool mgs_cand(const WCtx &C, const float4 xi, int i, int j, int t0, int t1, int t2,
                                          int tau[3], bool &bad) {
-    const float4 xj = mg_wrap_x(C.gx + 3 * j);
+    const float4 xj = C.xw[j];
     const int ki = __float_as_int(xi.w), kj = __float_as_int(xj.w);
     const float u0 = __fsub_rn(xj.x, xi.x), u1 = __fsub_rn(xj.y, xi.y), u2 = __fsub_rn(xj.z, xi.z);
     const float e0 = floorf(__fsub_rn(-C.rho[0], u0)) + 1.f, e1 = floorf(__fsub_rn(-C.rho[1], u1)) + 1.f,
@@ -290,6 +303,19 @@ __device__ __forceinline__ void mgs_slice_rows(const ScanArgs &A, unsigned long 
     }
 }
 
+// One edge written directly (the rare second walk of a warp whose codes did not fit the pool, PHASE 2).
+__device__ __forceinline__ void mgs_emit_one(const ScanArgs &A, long long e, int gi, int gj, const float *gx, int i,
+                                             int j, const int t[3], const float *lat) {
+    if (e >= A.capacity) return;
+    double v[3];
+    const double d = mg_exact_vec(gx + 3 * i, gx + 3 * j, t[0], t[1], t[2], lat, v);
+    A.src[e] = gi;
+    A.dst[e] = gj;
+    A.offset[3 * e] = (int8_t)t[0]; A.offset[3 * e + 1] = (int8_t)t[1]; A.offset[3 * e + 2] = (int8_t)t[2];
+    A.vec[3 * e] = (float)v[0]; A.vec[3 * e + 1] = (float)v[1]; A.vec[3 * e + 2] = (float)v[2];
+    if (A.dist) A.dist[e] = (float)d;
+}
+
 // ---- the code pool ------------------------------------------------------------------------------------
 // While a warp finds its edges it does not know where they go in the output, so their codes go to
 // chunks of MGS_CHUNK codes taken from a pool (one atomic per chunk); the chunk list stays in the warp's
@@ -297,12 +323,13 @@ __device__ __forceinline__ void mgs_slice_rows(const ScanArgs &A, unsigned long 
 struct PoolState {
     unsigned wcount;       // codes of the warp so far (the same on every lane)
     int nch;               // chunks taken
+    int *list;             // the range's chunk list (shared memory)
     bool ok;               // false: the pool or the list ran out; the warp only counts from then on and
                            // lists its rows again in the second phase (mgs_walk<1>)
 };
 
-__device__ __forceinline__ uint2 *mgs_pool_addr(const ScanArgs &A, const SSmem &ws, unsigned p) {
-    return A.pool + (size_t)ws.chunks[p / MGS_CHUNK] * MGS_CHUNK + (p % MGS_CHUNK);
+__device__ __forceinline__ uint2 *mgs_pool_addr(const ScanArgs &A, const int *list, unsigned p) {
+    return A.pool + (size_t)list[p / MGS_CHUNK] * MGS_CHUNK + (p % MGS_CHUNK);
 }
 
 // Make sure the chunks for local positions < upto exist.
@@ -312,7 +339,7 @@ __device__ __forceinline__ void mgs_pool_reserve(const ScanArgs &A, SSmem &ws, P
         if (lane == 0) c = (int)atomicAdd(A.ctl + 12, 1u);
         c = __shfl_sync(0xFFFFFFFFu, c, 0);
         if (c >= A.n_pool || P.nch >= MGS_MAXCH) { P.ok = false; break; }
-        if (lane == 0) ws.chunks[P.nch] = c;
+        if (lane == 0) P.list[P.nch] = c;
         P.nch += 1;
         __syncwarp();
     }
@@ -325,7 +352,7 @@ __device__ __forceinline__ void mgs_pool_reserve(const ScanArgs &A, SSmem &ws, P
 template <int PHASE>
 __device__ __forceinline__ unsigned mgs_row(const ScanArgs &A, SSmem &ws, PoolState &P, const WCtx &C, int i,
                                             unsigned long long goff, int lane, bool &anybad) {
-    const float4 xi = mg_wrap_x(C.gx + 3 * i);
+    const float4 xi = C.xw[i];
     const int M12 = C.m1 * C.m2;
     unsigned cnt = 0u;
     const bool wide = C.mloc >= 32;
@@ -349,7 +376,9 @@ __device__ __forceinline__ unsigned mgs_row(const ScanArgs &A, SSmem &ws, PoolSt
                                               ((unsigned)(tau[1] + 128) << 16) | ((unsigned)(tau[2] + 128) << 8));
                 const unsigned k = cnt + __popc(bal & ((1u << lane) - 1u));
                 if (PHASE == 0) {
-                    if (P.ok) *mgs_pool_addr(A, ws, P.wcount + k) = code;
+                    if (P.ok) *mgs_pool_addr(A, P.list, P.wcount + k) = code;
+                } else if (PHASE == 2) {
+                    mgs_emit_one(A, (long long)(goff + k), C.first + i, C.first + j, C.gx, i, j, tau, C.lat);
                 } else if ((long long)(goff + k) < A.capacity) A.codes[goff + k] = code;
             }
             cnt += __popc(bal);
@@ -404,10 +433,10 @@ __device__ __forceinline__ unsigned long long mgs_walk(SSmem &ws, const ScanArgs
                     if (lane == 0) A.row_ptr[C.first + i] = (int)MGS_HERE;
                     const unsigned cnt = mgs_row<PHASE>(A, ws, P, C, i, goff, lane, anybad);
                     if (PHASE == 0) {
-                        if (anybad) atomicOr(A.status, __float_as_int(mg_wrap_x(C.gx + 3 * i).w) == 0 ? MGS_NONFINITE : MGS_OFFSET);
+                        if (anybad) atomicOr(A.status, __float_as_int(C.xw[i].w) == 0 ? MGS_NONFINITE : MGS_OFFSET);
                         P.wcount += cnt;
                     } else {
-                        if (lane == 0) mgs_slice_rows(A, goff, cnt, 0u, cnt, C.first + i, C.first, C.N, s);
+                        if (PHASE == 1 && lane == 0) mgs_slice_rows(A, goff, cnt, 0u, cnt, C.first + i, C.first, C.N, s);
                         goff += cnt;
                     }
                 }
@@ -468,14 +497,22 @@ __device__ __forceinline__ unsigned long long mgs_walk(SSmem &ws, const ScanArgs
                                     while (mk) {
                                         const int bit = __clz(mk);
                                         mk &= ~(0x80000000u >> bit);
-                                        ws.stash[pos++] = make_uint2(gj, pc + ws.tcode[32 * w + bit]);
+                                        const unsigned tbits = pc + ws.tcode[32 * w + bit];
+                                        if (PHASE == 2) {
+                                            const int tau[3] = {(int)(tbits >> 24) - 128, (int)((tbits >> 16) & 0xFFu) - 128,
+                                                                (int)((tbits >> 8) & 0xFFu) - 128};
+                                            mgs_emit_one(A, (long long)(goff + pos), C.first + i, (int)gj, C.gx, i, j, tau, C.lat);
+                                            ++pos;
+                                        } else ws.stash[pos++] = make_uint2(gj, tbits);
                                     }
                                 }
                             }
                             __syncwarp();
                             if (PHASE == 0) {          // codes -> the pool, at the warp's local positions
-                                for (unsigned x = lane; x < t; x += 32) *mgs_pool_addr(A, ws, P.wcount + x) = ws.stash[x];
+                                for (unsigned x = lane; x < t; x += 32) *mgs_pool_addr(A, P.list, P.wcount + x) = ws.stash[x];
                                 P.wcount += t;
+                            } else if (PHASE == 2) {
+                                goff += t;
                             } else {                   // codes -> their final place in the stream
                                 const long long room = A.capacity - (long long)goff;
                                 const int lim = room >= (long long)t ? (int)t : (room > 0 ? (int)room : 0);
@@ -508,9 +545,61 @@ __device__ __forceinline__ unsigned long long mgs_walk(SSmem &ws, const ScanArgs
     return PHASE == 0 ? (unsigned long long)P.wcount : goff;
 }
 
+// ((x_dst - x_src) + tau) . L evaluated like the oracle does (Def. 3, R15: no FMA contraction,
+// sums left to right); tb = (tau + 128) bytes << 8.
+__device__ __forceinline__ void mgs_vec(const double xi[3], const double xj[3], unsigned tb, const double L[9], double w3[3]) {
+    // (double)(b - 128) without a conversion instruction: 2^52 + b has b in its low mantissa word
+    const double f0 = __dadd_rn(__dsub_rn(xj[0], xi[0]), __hiloint2double(0x43300000, (int)(tb >> 24)) - 4503599627370624.0);
+    const double f1 = __dadd_rn(__dsub_rn(xj[1], xi[1]), __hiloint2double(0x43300000, (int)((tb >> 16) & 0xFFu)) - 4503599627370624.0);
+    const double f2 = __dadd_rn(__dsub_rn(xj[2], xi[2]), __hiloint2double(0x43300000, (int)((tb >> 8) & 0xFFu)) - 4503599627370624.0);
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+        w3[c] = __dadd_rn(__dadd_rn(__dmul_rn(f0, L[c]), __dmul_rn(f1, L[3 + c])), __dmul_rn(f2, L[6 + c]));
+}
+
+// What the caller's arrays look like to the writers.
+struct OutArrays {
+    int32_t *src, *dst;
+    int8_t *offset;
+    float *vec, *dist;
+    bool al16;             // src, dst, vec (, dist) 16-byte aligned, offset 4-byte aligned
+};
+
+// Four consecutive edges e .. e + 3 of one lane (e a multiple of 4); ok[y]: edge y exists.
+__device__ __forceinline__ void mgs_store4(const OutArrays &O, long long e, const bool ok[4], const int gi[4], const int gj[4],
+                                           const unsigned tb[4], const float v[4][3], const float d[4]) {
+    if (O.al16 && ok[0] && ok[3]) {
+        *reinterpret_cast<int4 *>(O.src + e) = make_int4(gi[0], gi[1], gi[2], gi[3]);
+        *reinterpret_cast<int4 *>(O.dst + e) = make_int4(gj[0], gj[1], gj[2], gj[3]);
+        float4 *pv = reinterpret_cast<float4 *>(O.vec + 3 * e);
+        pv[0] = make_float4(v[0][0], v[0][1], v[0][2], v[1][0]);
+        pv[1] = make_float4(v[1][1], v[1][2], v[2][0], v[2][1]);
+        pv[2] = make_float4(v[2][2], v[3][0], v[3][1], v[3][2]);
+        // 12 offset bytes: tau of four edges (a code's .y = b0 b1 b2 0 from the top byte down), signed
+        const unsigned t0 = tb[0] ^ 0x80808000u, t1 = tb[1] ^ 0x80808000u, t2 = tb[2] ^ 0x80808000u, t3 = tb[3] ^ 0x80808000u;
+        unsigned *po = reinterpret_cast<unsigned *>(O.offset + 3 * e);
+        po[0] = __byte_perm(t0, t1, 0x7123);       // bytes in memory: t0.b3 t0.b2 t0.b1 t1.b3
+        po[1] = __byte_perm(t1, t2, 0x6712);       //                  t1.b2 t1.b1 t2.b3 t2.b2
+        po[2] = __byte_perm(t2, t3, 0x5671);       //                  t2.b1 t3.b3 t3.b2 t3.b1
+        if (O.dist) *reinterpret_cast<float4 *>(O.dist + e) = make_float4(d[0], d[1], d[2], d[3]);
+    } else {
+#pragma unroll
+        for (int y = 0; y < 4; ++y)
+            if (ok[y]) {
+                O.src[e + y] = gi[y];
+                O.dst[e + y] = gj[y];
+                O.vec[3 * (e + y)] = v[y][0]; O.vec[3 * (e + y) + 1] = v[y][1]; O.vec[3 * (e + y) + 2] = v[y][2];
+                const unsigned t = tb[y] ^ 0x80808000u;
+                O.offset[3 * (e + y)] = (int8_t)(t >> 24); O.offset[3 * (e + y) + 1] = (int8_t)(t >> 16);
+                O.offset[3 * (e + y) + 2] = (int8_t)(t >> 8);
+                if (O.dist) O.dist[e + y] = d[y];
+            }
+    }
+}
+
 // Second phase of a warp whose codes are in the pool: codes -> their final place, row_ptr from local to
 // final offsets, and for every MGS_SLICE-th edge of the output the record the write kernel starts from.
-__device__ __forceinline__ void mgs_place(const ScanArgs &A, const SSmem &ws, unsigned total, int row_lo, int row_hi,
+__device__ __forceinline__ void mgs_place(const ScanArgs &A, const int *list, unsigned total, int row_lo, int row_hi,
                                           unsigned long long base, int lane) {
     {
         const long long room = A.capacity - (long long)base;
@@ -518,11 +607,11 @@ __device__ __forceinline__ void mgs_place(const ScanArgs &A, const SSmem &ws, un
         uint2 *dst = A.codes + base;
         unsigned x = lane;
         for (; x + 96 < lim; x += 128) {               // four loads in flight
-            const uint2 c0 = *mgs_pool_addr(A, ws, x), c1 = *mgs_pool_addr(A, ws, x + 32),
-                        c2 = *mgs_pool_addr(A, ws, x + 64), c3 = *mgs_pool_addr(A, ws, x + 96);
+            const uint2 c0 = *mgs_pool_addr(A, list, x), c1 = *mgs_pool_addr(A, list, x + 32),
+                        c2 = *mgs_pool_addr(A, list, x + 64), c3 = *mgs_pool_addr(A, list, x + 96);
             dst[x] = c0; dst[x + 32] = c1; dst[x + 64] = c2; dst[x + 96] = c3;
         }
-        for (; x < lim; x += 32) dst[x] = *mgs_pool_addr(A, ws, x);
+        for (; x < lim; x += 32) dst[x] = *mgs_pool_addr(A, list, x);
     }
     for (int r0 = row_lo; r0 < row_hi; r0 += 32) {
         const int r = r0 + lane;
@@ -547,6 +636,120 @@ __device__ __forceinline__ void mgs_place(const ScanArgs &A, const SSmem &ws, un
     }
 }
 
+// Second phase of a warp whose codes are in the pool, writing the caller's arrays itself (no code stream,
+// no write kernel): row_ptr from local to final offsets, then batches of 128 edges, lane <-> four
+// consecutive edges whose global index starts at a multiple of 4, so that every array leaves in aligned
+// 16-byte stores (scalar stores for the ragged first / last lanes of the warp's edges).  Uses the stash
+// area of the warp's shared memory for the row counters and the staged FP64 positions.
+__device__ __forceinline__ void mgs_place_write(const ScanArgs &A, const OutArrays &O, SSmem &ws, const int *list,
+                                                unsigned total, int row_lo, int row_hi, unsigned long long base, int lane) {
+    for (int r0 = row_lo; r0 < row_hi; r0 += 32) {          // my rows: local -> final offsets
+        const int r = r0 + lane;
+        if (r < row_hi) A.row_ptr[r] = (int)(base + (unsigned)A.row_ptr[r]);
+    }
+    __syncwarp();
+    if (total == 0u) return;
+    int *cnt = reinterpret_cast<int *>(ws.stash);
+    double *xs = reinterpret_cast<double *>(ws.stash + 64);            // 3 * MGS_NMAX doubles
+    const long long lim = (long long)total < A.capacity - (long long)base ? (long long)total : A.capacity - (long long)base;
+    int r0 = row_lo, cur_s = -1, a_lo = 0, win = 0, nat = 0;
+    double L[9];
+#pragma unroll
+    for (int c = 0; c < 9; ++c) L[c] = 0.0;
+    for (long long qb = -(long long)(base & 3ull); qb < lim; qb += 128) {
+        const long long gb = (long long)base + qb;                     // global index of the batch's first slot
+        // ---- the lane's codes
+        int gj[4];
+        unsigned tb[4];
+        bool ok[4];
+#pragma unroll
+        for (int y = 0; y < 4; ++y) {
+            const long long q = qb + 4 * lane + y;
+            ok[y] = q >= 0 && q < lim;
+            gj[y] = 0; tb[y] = 0x80808000u;
+            if (ok[y]) { const uint2 c = *mgs_pool_addr(A, list, (unsigned)q); gj[y] = (int)c.x; tb[y] = c.y; }
+        }
+        // ---- rows: row of slot p = r0 + number of my rows r > r0 that start at or before it
+        __syncwarp();
+#pragma unroll
+        for (int x = 0; x < 4; ++x) cnt[32 * x + lane] = 0;
+        __syncwarp();
+        for (int rb = r0 + 1;; rb += 32) {
+            const int r = rb + lane;
+            bool in = false;
+            if (r < row_hi) {
+                const long long start = (long long)A.row_ptr[r];
+                in = start < gb + 128;
+                if (in) atomicAdd(&cnt[start > gb ? (int)(start - gb) : 0], 1);
+            }
+            if (!__all_sync(0xFFFFFFFFu, in)) break;
+        }
+        __syncwarp();
+        int c4[4];
+#pragma unroll
+        for (int y = 0; y < 4; ++y) c4[y] = cnt[4 * lane + y];
+        int incl = c4[0] + c4[1] + c4[2] + c4[3];
+        const int own = incl;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+            if (lane >= o) incl += v;
+        }
+        int row = r0 + incl - own;
+        int gi[4];
+#pragma unroll
+        for (int y = 0; y < 4; ++y) { row += c4[y]; gi[y] = row; }
+        // ---- lattice and positions of the structure of the batch's first row
+        const int rf = __shfl_sync(0xFFFFFFFFu, gi[0], 0);
+        const int s0 = A.atom_struct[rf];
+        if (s0 != cur_s) {
+            cur_s = s0;
+            a_lo = A.rec[s0].first;
+            nat = A.rec[s0].natoms;
+            win = min(MGS_NMAX, nat);
+            const double *pl = A.lat64 + 9 * (size_t)s0;
+#pragma unroll
+            for (int c = 0; c < 9; ++c) L[c] = pl[c];
+            __syncwarp();
+            const double *px = A.pos64 + 3 * (size_t)a_lo;
+            for (int x = lane; x < 3 * win; x += 32) xs[x] = px[x];
+            __syncwarp();
+        }
+        float v[4][3], d[4];
+#pragma unroll
+        for (int y = 0; y < 4; ++y) {
+            v[y][0] = v[y][1] = v[y][2] = 0.f; d[y] = 0.f;
+            if (!ok[y]) continue;
+            double w3[3];
+            const unsigned wi = (unsigned)(gi[y] - a_lo), wj = (unsigned)(gj[y] - a_lo);
+            if (wi < (unsigned)win && wj < (unsigned)win) {
+                mgs_vec(xs + 3 * wi, xs + 3 * wj, tb[y], L, w3);
+            } else {                                   // a structure above the window, or another structure
+                double xi[3], xj[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    xi[c] = A.pos64[3 * (size_t)gi[y] + c];
+                    xj[c] = A.pos64[3 * (size_t)gj[y] + c];
+                }
+                if (wi < (unsigned)nat) mgs_vec(xi, xj, tb[y], L, w3);
+                else {
+                    const int s = A.atom_struct[gi[y]];
+                    double L2[9];
+#pragma unroll
+                    for (int c = 0; c < 9; ++c) L2[c] = A.lat64[9 * (size_t)s + c];
+                    mgs_vec(xi, xj, tb[y], L2, w3);
+                }
+            }
+            v[y][0] = (float)w3[0]; v[y][1] = (float)w3[1]; v[y][2] = (float)w3[2];
+            if (O.dist)
+                d[y] = __fsqrt_rn((float)__dadd_rn(__dadd_rn(__dmul_rn(w3[0], w3[0]), __dmul_rn(w3[1], w3[1])), __dmul_rn(w3[2], w3[2])));
+        }
+        mgs_store4(O, gb + 4 * lane, ok, gi, gj, tb, v, d);
+        r0 = __shfl_sync(0xFFFFFFFFu, gi[3], 31);
+    }
+    __syncwarp();
+}
+
 // ---- launch 1 ---------------------------------------------------------------------------------------
 #ifndef MGS_MIN_CTAS
 #define MGS_MIN_CTAS 5
@@ -560,50 +763,99 @@ mg_cutoff_scan_kernel(const __grid_constant__ ScanArgs A) {
     SSmem &ws = sm.w[warp];
     const unsigned epoch = *reinterpret_cast<volatile unsigned *>(A.ctl + 10) + 1u;   // tag of this call's slots
     RangeCtx RC;
-    mg_range_init(RC, A.rec, A.bpre, A.n_blocks, A.n_struct, (int)gridDim.x * MGS_WARPS, lane);
-    const int rid = (int)blockIdx.x * MGS_WARPS + warp;
+    const int n_warps = (int)gridDim.x * MGS_WARPS;
+    mg_range_init(RC, A.rec, A.bpre, A.n_blocks, A.n_struct, MGS_WAVES * n_warps, lane);
     MGS_STAMP(0)
-    PoolState P;
-    P.wcount = 0u; P.nch = 0; P.ok = true;
-    int row_lo = -1, row_hi = -1;
-    const unsigned long long wtotal = mgs_walk<0>(ws, A, RC, rid, P, row_lo, row_hi, 0ull, lane);
-    if (lane == 0) sm.wsum[warp] = (unsigned)wtotal;
-    __syncthreads();
-    MGS_STAMP(1)
-    unsigned long long total = 0ull, mine = 0ull;
-#pragma unroll
-    for (int w = 0; w < MGS_WARPS; ++w) {
-        if (w < warp) mine += sm.wsum[w];
-        total += sm.wsum[w];
-    }
-    if (tid == 0) mg_st_release(A.slots + blockIdx.x, ((unsigned long long)epoch << 32) | (total & 0xFFFFFFFFull));
-    if (!A.count_only) {
-        // device-wide exclusive scan of K4: sum of the slots before this CTA's (all CTAs are resident)
-        if (warp == 0) {
-            unsigned long long before = 0ull;
-            for (int c0 = 0; c0 < (int)blockIdx.x; c0 += 32) {
-                const int c = c0 + lane;
-                if (c < (int)blockIdx.x) {
-                    unsigned long long v;
-                    while ((unsigned)((v = mg_ld_acquire(A.slots + c)) >> 32) != epoch) __nanosleep(400);
-                    before += v & 0xFFFFFFFFull;
-                }
-            }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) before += __shfl_xor_sync(0xFFFFFFFFu, before, o);
-            if (lane == 0) sm.prefix = before;
-        }
+    // ---- find: the warp's range of every wave, one after the other; the CTA's total of a wave is published
+    // as soon as its four warps are through, so that by the time a CTA wants the prefix of wave w the
+    // other CTAs have long published theirs (they are busy with the waves after it)
+#pragma unroll 1
+    for (int wv = 0; wv < MGS_WAVES; ++wv) {
+        PoolState P;
+        P.wcount = 0u; P.nch = 0; P.ok = true; P.list = ws.chunks[wv];
+        int row_lo = -1, row_hi = -1;
+        const int rid = wv * n_warps + (int)blockIdx.x * MGS_WARPS + warp;
+        const unsigned wtotal = (unsigned)mgs_walk<0>(ws, A, RC, rid, P, row_lo, row_hi, 0ull, lane);
+        __syncthreads();                               // (the previous wave's sums have been read)
+        if (lane == 0) sm.wsum[warp] = wtotal;
         __syncthreads();
-        const unsigned long long before = sm.prefix;
-        MGS_STAMP(2)
-        if (blockIdx.x == gridDim.x - 1 && tid == 0) {           // the last range knows the grand total
-            const unsigned long long tot = before + total;
-            *A.n_edges = (long long)tot;
-            A.row_ptr[A.n_atoms] = (int)tot;
-            if (tot > 0x7FFFFFFFull || (long long)tot > A.capacity) atomicOr(A.status, MGS_CAPACITY);
+        unsigned long long total = 0ull, mine = 0ull;
+#pragma unroll
+        for (int w = 0; w < MGS_WARPS; ++w) {
+            if (w < warp) mine += sm.wsum[w];
+            total += sm.wsum[w];
         }
-        if (P.ok) mgs_place(A, ws, (unsigned)wtotal, row_lo, row_hi, before + mine, lane);
-        else mgs_walk<1>(ws, A, RC, rid, P, row_lo, row_hi, before + mine, lane);
+        if (lane == 0) {
+            int *st = ws.wave[wv];
+            st[0] = (int)wtotal; st[1] = P.nch; st[2] = P.ok ? 1 : 0; st[3] = row_lo; st[4] = row_hi;
+            st[5] = (int)(unsigned)mine; st[6] = (int)(unsigned)total;
+        }
+        if (tid == 0)
+            mg_st_release(A.slots + (size_t)wv * gridDim.x + blockIdx.x, ((unsigned long long)epoch << 32) | (total & 0xFFFFFFFFull));
+    }
+    __syncwarp();
+    MGS_STAMP(1)
+    if (!A.count_only) {
+        OutArrays O;
+        O.src = A.src; O.dst = A.dst; O.offset = A.offset; O.vec = A.vec; O.dist = A.dist;
+        O.al16 = ((reinterpret_cast<unsigned long long>(A.src) | reinterpret_cast<unsigned long long>(A.dst) |
+                   reinterpret_cast<unsigned long long>(A.vec) | reinterpret_cast<unsigned long long>(A.dist)) & 15ull) == 0ull &&
+                 (reinterpret_cast<unsigned long long>(A.offset) & 3ull) == 0ull;
+        unsigned long long waves_before = 0ull;        // edges of the waves before wv
+#pragma unroll 1
+        for (int wv = 0; wv < MGS_WAVES; ++wv) {
+            // device-wide exclusive scan of K4: the slots of this wave before this CTA's, and the whole wave
+            // (all CTAs are resident: cooperative launch)
+            __syncthreads();
+            if (warp == 0) {
+                unsigned long long before = 0ull, all = 0ull;
+                const unsigned long long *sl = A.slots + (size_t)wv * gridDim.x;
+                // (a slot carries its own tag: relaxed loads, four in flight per lane, a lane spins only on a
+                // slot that is not there yet)
+                const int n_need = wv + 1 < MGS_WAVES ? (int)gridDim.x : (int)blockIdx.x;
+                for (int c0 = 0; c0 < n_need; c0 += 128) {
+                    unsigned long long v[4];
+#pragma unroll
+                    for (int x = 0; x < 4; ++x) {
+                        const int c = c0 + 32 * x + lane;
+                        v[x] = c < n_need ? mg_ld_relaxed(sl + c) : ((unsigned long long)epoch << 32);
+                    }
+#pragma unroll
+                    for (int x = 0; x < 4; ++x) {
+                        const int c = c0 + 32 * x + lane;
+                        while ((unsigned)(v[x] >> 32) != epoch) { __nanosleep(100); v[x] = mg_ld_relaxed(sl + c); }
+                        if (c < (int)blockIdx.x) before += v[x] & 0xFFFFFFFFull;
+                        all += v[x] & 0xFFFFFFFFull;
+                    }
+                }
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    before += __shfl_xor_sync(0xFFFFFFFFu, before, o);
+                    all += __shfl_xor_sync(0xFFFFFFFFu, all, o);
+                }
+                if (lane == 0) { sm.prefix = before; sm.wave_all = all; }
+            }
+            __syncthreads();
+            const int *st = ws.wave[wv];
+            const unsigned wtotal = (unsigned)st[0];
+            PoolState P;
+            P.wcount = wtotal; P.nch = st[1]; P.ok = st[2] != 0; P.list = ws.chunks[wv];
+            int row_lo = st[3], row_hi = st[4];
+            const unsigned long long base = waves_before + sm.prefix + (unsigned)st[5];
+            if (wv == MGS_WAVES - 1 && blockIdx.x == gridDim.x - 1 && tid == 0) {    // the last range knows the grand total
+                const unsigned long long tot = waves_before + sm.prefix + (unsigned)st[6];
+                *A.n_edges = (long long)tot;
+                A.row_ptr[A.n_atoms] = (int)tot;
+                if (tot > 0x7FFFFFFFull || (long long)tot > A.capacity) atomicOr(A.status, MGS_CAPACITY);
+            }
+            waves_before += sm.wave_all;
+            const int rid = wv * n_warps + (int)blockIdx.x * MGS_WARPS + warp;
+            if (A.write_here) {
+                if (P.ok) mgs_place_write(A, O, ws, P.list, wtotal, row_lo, row_hi, base, lane);
+                else mgs_walk<2>(ws, A, RC, rid, P, row_lo, row_hi, base, lane);
+            } else if (P.ok) mgs_place(A, P.list, wtotal, row_lo, row_hi, base, lane);
+            else mgs_walk<1>(ws, A, RC, rid, P, row_lo, row_hi, base, lane);
+        }
         MGS_STAMP(3)
     }
     // last CTA out: the call is over (count_only: it also adds the totals up)
@@ -616,7 +868,7 @@ mg_cutoff_scan_kernel(const __grid_constant__ ScanArgs A) {
     if (!sm.last) return;
     if (A.count_only && warp == 0) {
         unsigned long long sum = 0ull;
-        for (int c = lane; c < (int)gridDim.x; c += 32) {
+        for (int c = lane; c < MGS_WAVES * (int)gridDim.x; c += 32) {
             unsigned long long v;
             while ((unsigned)((v = mg_ld_acquire(A.slots + c)) >> 32) != epoch) __nanosleep(100);
             sum += v & 0xFFFFFFFFull;

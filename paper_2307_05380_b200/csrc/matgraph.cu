@@ -34,7 +34,8 @@ struct mg_ctx {
     unsigned *d_wmask = nullptr;          // [n_warps, MG_MASK_WORDS] hit masks kept from count to emit
     int cut_warps = 0, last_cut_warps = 0;
     int fused_occ = 0, fused_coop = 0;    // fused cutoff kernel: CTAs per SM, cooperative launch accepted
-    int legacy = 0;                       // MATGRAPH_LEGACY=1: the two-launch cutoff path of round 1
+    int force_scan = 0, force_legacy = 0; // MATGRAPH_FUSED=1 / MATGRAPH_LEGACY=1: one cutoff path for every batch
+    int write_kernel = 0;                 // MATGRAPH_WRITE_KERNEL=1: edges written by a launch of their own
     unsigned long long *d_slots = nullptr;// [sm_count * fused_occ] per-CTA edge totals tagged with the call's epoch
     uint2 *d_pool = nullptr;              // [pool_chunks, MGS_CHUNK] codes before their final place is known
     size_t pool_chunks = 0;
@@ -42,6 +43,7 @@ struct mg_ctx {
     uint2 *d_codes = nullptr;             // [code_cap] (dst, tau) of every edge, in output order
     int4 *d_slice_row = nullptr;          // [code_cap / MGS_SLICE + 2]
     size_t code_cap = 0;
+    float4 *d_xw4 = nullptr;              // [atom64_cap] wrapped coordinates (cut_prep.cuh)
     double *d_pos64 = nullptr;            // [atom64_cap, 3]
     size_t atom64_cap = 0;
     double *d_lat64 = nullptr;            // [lat64_cap, 9]
@@ -147,14 +149,16 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
                          cudaMalloc(&c->d_wmask, (size_t)MG_OVER * c->cut_warps * MG_MASK_WORDS * sizeof(unsigned)) != cudaSuccess ||
                          cudaMalloc(&c->d_wclock, 64 * (size_t)(c->cut_warps + 2048) * sizeof(unsigned)) != cudaSuccess)) { mg_destroy(c); return MG_ERR_CUDA; }
     }
-    c->legacy = getenv("MATGRAPH_FUSED") ? 0 : 1;   // fused kernel: correct, not yet faster
+    c->write_kernel = getenv("MATGRAPH_WRITE_KERNEL") ? 1 : 0;
+    c->force_scan = getenv("MATGRAPH_FUSED") ? 1 : 0;
+    c->force_legacy = getenv("MATGRAPH_LEGACY") ? 1 : 0;
     if (cudaFuncSetAttribute(mg_cutoff_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)sizeof(ScanSmem)) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->fused_occ, mg_cutoff_scan_kernel, MGS_BLOCK, sizeof(ScanSmem));
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->write_occ, mg_cutoff_write_kernel, MGWR_BLOCK, 0);
     if (c->fused_occ < 1 || c->write_occ < 1) { mg_destroy(c); return MG_ERR_CUDA; }
     {
-        const size_t nc = (size_t)c->sm_count * c->fused_occ;
+        const size_t nc = (size_t)c->sm_count * c->fused_occ * MGS_WAVES;
         if (cudaMalloc(&c->d_slots, nc * sizeof(unsigned long long)) != cudaSuccess ||
             cudaMemset(c->d_slots, 0, nc * sizeof(unsigned long long)) != cudaSuccess ||
             false) { mg_destroy(c); return MG_ERR_CUDA; }
@@ -180,6 +184,7 @@ extern "C" void mg_destroy(mg_ctx *c) {
     cudaFree(c->d_codes);
     cudaFree(c->d_slice_row);
     cudaFree(c->d_pos64);
+    cudaFree(c->d_xw4);
     cudaFree(c->d_lat64);
     cudaFree(c->d_crec);
     cudaFree(c->d_bpre);
@@ -221,9 +226,10 @@ extern "C" mg_status mg_reserve(mg_ctx *c, int32_t n_struct, int32_t n_atoms) {
     }
     if ((size_t)n_atoms + 1 > c->atom64_cap) {
         const size_t cap = (size_t)n_atoms + 1025;
-        cudaFree(c->d_pos64);
-        c->d_pos64 = nullptr; c->atom64_cap = 0;
+        cudaFree(c->d_pos64); cudaFree(c->d_xw4);
+        c->d_pos64 = nullptr; c->d_xw4 = nullptr; c->atom64_cap = 0;
         MG_CUDA(cudaMalloc(&c->d_pos64, cap * 3 * sizeof(double)));
+        MG_CUDA(cudaMalloc(&c->d_xw4, cap * sizeof(float4)));
         c->atom64_cap = cap;
     }
     if ((size_t)n_struct + 1 > c->lat64_cap) {
@@ -380,19 +386,26 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
     }
     const int n_blocks = (n_struct + MG_CP_BLOCK - 1) / MG_CP_BLOCK;
     const bool prof = c->profile && !count_only;
+    // Two cutoff paths: the scan kernel (cut_scan.cuh) and the count + emit pair (cutoff_pairs.cuh).  The pair is
+    // ahead on batches of small cells (BASELINE configs[2]: 73 against 81 us per call), the scan kernel on large
+    // structures; MATGRAPH_FUSED=1 / MATGRAPH_LEGACY=1 force one of them.
+    const bool use_scan = c->force_scan || (!c->force_legacy && n_struct > 0 && n_atoms / n_struct > MG_SMALL_MAX_ATOMS);
     if (prof) { prof_collect(c); cudaEventRecord(c->ev[0], st); }
     {
         CutPrepArgs P;
         P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms; P.r_c = r_c;
-        P.k = 0; P.hint = nullptr; P.use_hint = 0; P.rows_cost = c->legacy ? 0 : 1;
+        P.k = 0; P.hint = nullptr; P.use_hint = 0; P.rows_cost = use_scan ? 1 : 0;
+        P.pos = pos; P.xw4 = use_scan ? c->d_xw4 : nullptr; P.n_sblocks = n_blocks;
         P.rec = c->d_crec; P.bpre = c->d_bpre; P.ctl = c->d_ctl; P.status = c->d_ctl + 4;
-        MG_CUDA(launch_after(c, mg_cut_prep_kernel, n_blocks, MG_CP_BLOCK, 0, st, P));
+        // (scan path: extra blocks wrap the coordinates of the batch's atoms)
+        const int xblocks = use_scan ? (n_atoms + 8 * MG_CP_BLOCK - 1) / (8 * MG_CP_BLOCK) : 0;
+        MG_CUDA(launch_after(c, mg_cut_prep_kernel, n_blocks + (xblocks < 1024 ? xblocks : 1024), MG_CP_BLOCK, 0, st, P));
         c->launches += 1;
     }
-    if (!c->legacy) {
+    if (use_scan) {
         // the code stream holds one 8-byte code per edge the caller's arrays can take
         const size_t need = count_only ? 0 : (size_t)o->capacity;
-        if (need > c->code_cap) {
+        if (c->write_kernel && need > c->code_cap) {
             cudaFree(c->d_codes); cudaFree(c->d_slice_row);
             c->d_codes = nullptr; c->d_slice_row = nullptr; c->code_cap = 0;
             const size_t cap = need + need / 8 + 4096;
@@ -401,10 +414,10 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
             c->code_cap = cap;
         }
         int grid = c->sm_count * c->fused_occ;
-        const int cap_grid = (n_atoms + MGS_WARPS) / MGS_WARPS;   // >= 1 row per warp
+        const int cap_grid = (n_atoms + MGS_WARPS * MGS_WAVES) / (MGS_WARPS * MGS_WAVES);   // >= 1 row per range
         if (grid > cap_grid) grid = cap_grid;
         // pool: the edges the caller can take, in chunks, plus one partly filled chunk per warp
-        const size_t want_chunks = count_only ? 0 : need / MGS_CHUNK + (size_t)grid * MGS_WARPS + 8;
+        const size_t want_chunks = count_only ? 0 : need / MGS_CHUNK + (size_t)grid * MGS_WARPS * MGS_WAVES + 8;
         if (want_chunks > c->pool_chunks) {
             cudaFree(c->d_pool);
             c->d_pool = nullptr; c->pool_chunks = 0;
@@ -413,7 +426,7 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
             c->pool_chunks = cap;
         }
         ScanArgs F;
-        F.pos = pos; F.lattice = lat; F.n_struct = n_struct; F.n_atoms = n_atoms; F.r_c = r_c;
+        F.pos = pos; F.lattice = lat; F.xw4 = c->d_xw4; F.n_struct = n_struct; F.n_atoms = n_atoms; F.r_c = r_c;
         F.row_ptr = o->row_ptr; F.capacity = o->capacity; F.n_edges = (long long *)o->n_edges;
         F.rec = c->d_crec; F.bpre = c->d_bpre; F.n_blocks = n_blocks;
         F.pool = c->d_pool;
@@ -421,6 +434,8 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
         F.n_pool = count_only ? 0 : (c->mask_words < MG_MASK_WORDS ? c->mask_words : (int)(c->pool_chunks < 0x7FFFFFFF ? c->pool_chunks : 0x7FFFFFFF));
         F.slots = c->d_slots; F.ctl = c->d_ctl; F.status = c->d_ctl + 4;
         F.count_only = count_only;
+        F.src = o->src; F.dst = o->dst; F.offset = o->offset; F.vec = o->vec; F.dist = o->dist;
+        F.write_here = c->write_kernel ? 0 : 1;
         F.codes = c->d_codes; F.slice_row = c->d_slice_row; F.atom_struct = c->d_atom_struct;
         F.pos64 = c->d_pos64; F.lat64 = c->d_lat64;
         F.dbg = c->d_wclock;
@@ -434,7 +449,7 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
         MG_CUDA(e);
         c->launches += 1;
         if (prof) cudaEventRecord(c->ev[2], st);
-        if (!count_only && o->capacity > 0) {
+        if (!count_only && o->capacity > 0 && c->write_kernel) {
             WriteArgs W;
             W.codes = c->d_codes; W.slice_row = c->d_slice_row; W.atom_struct = c->d_atom_struct;
             W.pos64 = c->d_pos64; W.lat64 = c->d_lat64; W.row_ptr = o->row_ptr;
@@ -518,6 +533,7 @@ static mg_status launch_knn(mg_ctx *c, const float *pos, const float *lat, const
         CutPrepArgs P;
         P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms; P.r_c = 0.f;
         P.k = k; P.hint = hint; P.use_hint = use_hint; P.rows_cost = 0;
+        P.pos = pos; P.xw4 = nullptr; P.n_sblocks = n_blocks;
         P.rec = c->d_crec; P.bpre = c->d_bpre; P.ctl = c->d_ctl; P.status = c->d_ctl + 4;
         MG_CUDA(launch_after(c, mg_cut_prep_kernel, n_blocks, MG_CP_BLOCK, 0, st, P));
         c->launches += 1;
