@@ -128,6 +128,30 @@ mg_status mg_knn_graph_host(mg_ctx *ctx, const float *pos, const float *lattice,
                             const int32_t *struct_ptr, int32_t n_struct, int32_t n_atoms,
                             int32_t k, const mg_edges *out_host);
 
+/* Symmetric graph (section 3 "Symmetric graph"): the KNN graph is directed; `out` receives the
+ * edges of `in` plus, for every edge (i, j, tau) whose reverse (j, i, -tau) is not in `in`, that reverse
+ * edge (vec negated, same dist), CSR by source, every edge once.  The rows of `in` keep their order; the
+ * added edges follow them in no particular order.  `in` is any graph this library produced (device
+ * arrays, in->n_edges a device scalar; in->capacity bounds the edges read).  out->capacity must hold the
+ * result (at most twice the edges of `in`), else MG_ERR_CAPACITY surfaces from mg_check with the required
+ * count in *out->n_edges.  out->dist needs in->dist.  May grow the workspace on the first call. */
+mg_status mg_symmetrize(mg_ctx *ctx, const mg_edges *in, int32_t n_atoms, const mg_edges *out, void *cuda_stream);
+
+/* Triplets Gamma_2 (Def. 3; "Triplets generation"): the ordered pairs (a, b), a != b, of
+ * edges that share their source.  For source i with edges row_ptr[i] .. row_ptr[i+1]-1 (degree d) the
+ * d (d - 1) pairs are edge_a[t], edge_b[t] (edge indices) for tri_ptr[i] <= t < tri_ptr[i+1], ordered by
+ * (a, b).  All pointers are device pointers; *n_triplets receives tri_ptr[n_atoms] (also when it exceeds
+ * `capacity`: MG_ERR_CAPACITY from mg_check, only triplets below the capacity are written). */
+typedef struct {
+    int64_t *tri_ptr;      /* [n_atoms+1]                                        */
+    int32_t *edge_a;       /* [capacity] first edge of the pair                  */
+    int32_t *edge_b;       /* [capacity] second edge                             */
+    int64_t  capacity;
+    int64_t *n_triplets;   /* one int64, written by the call                     */
+} mg_triplets;
+mg_status mg_triplets_graph(mg_ctx *ctx, const int32_t *row_ptr, int32_t n_atoms, const mg_triplets *out,
+                            void *cuda_stream);
+
 /* SYNCHRONISES the stream, returns the first data-dependent error recorded since the last
  * mg_check (MG_OK if none) and clears the device status word. */
 mg_status mg_check(mg_ctx *ctx, void *cuda_stream);

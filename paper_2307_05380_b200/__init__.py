@@ -23,7 +23,7 @@ MG_MAX_K = 64
 EXPORTS = ["mg_create", "mg_destroy", "mg_reserve", "mg_cutoff_graph", "mg_cutoff_count",
            "mg_knn_graph", "mg_graph_create", "mg_graph_destroy", "mg_update_graph",
            "mg_cutoff_graph_host", "mg_knn_graph_host", "mg_check", "mg_launch_count",
-           "mg_status_string", "mg_set_profile", "mg_profile_read"]
+           "mg_status_string", "mg_set_profile", "mg_profile_read", "mg_symmetrize", "mg_triplets_graph"]
 
 
 class MatGraphError(RuntimeError):
@@ -39,6 +39,11 @@ class _Edges(ctypes.Structure):
 
 
 _LIBH = None
+
+
+class _Triplets(ctypes.Structure):
+    _fields_ = [("tri_ptr", ctypes.c_void_p), ("edge_a", ctypes.c_void_p), ("edge_b", ctypes.c_void_p),
+                ("capacity", ctypes.c_int64), ("n_triplets", ctypes.c_void_p)]
 
 
 def _lib():
@@ -68,6 +73,8 @@ def _lib():
         lib.mg_launch_count.restype = i64
         lib.mg_set_profile.argtypes = [vp, ctypes.c_int]
         lib.mg_profile_read.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(i64)]
+        lib.mg_symmetrize.argtypes = [vp, ep, i32, ep, vp]
+        lib.mg_triplets_graph.argtypes = [vp, vp, i32, ctypes.POINTER(_Triplets), vp]
         lib.mg_status_string.argtypes = [ctypes.c_int]
         lib.mg_status_string.restype = ctypes.c_char_p
         _LIBH = lib
@@ -230,6 +237,27 @@ class Context:
                                     ctypes.byref(out._c()), _stream())
         if rc != 0:
             raise MatGraphError(rc, "mg_update_graph")
+        return out
+
+    def mg_symmetrize(self, inp: Edges, n_atoms: int, out: Edges) -> Edges:
+        rc = _lib().mg_symmetrize(self._h, ctypes.byref(inp._c()), n_atoms, ctypes.byref(out._c()), _stream())
+        if rc != 0:
+            raise MatGraphError(rc, "mg_symmetrize")
+        return out
+
+    def mg_triplets_graph(self, row_ptr, n_atoms: int, capacity: int) -> dict:
+        """Allocates tri_ptr / edge_a / edge_b (device tensors) and runs mg_triplets_graph."""
+        torch = _torch()
+        cap = max(int(capacity), 1)
+        out = dict(tri_ptr=torch.empty(n_atoms + 1, dtype=torch.int64, device=row_ptr.device),
+                   edge_a=torch.empty(cap, dtype=torch.int32, device=row_ptr.device),
+                   edge_b=torch.empty(cap, dtype=torch.int32, device=row_ptr.device),
+                   n_triplets=torch.zeros(1, dtype=torch.int64, device=row_ptr.device), capacity=int(capacity))
+        c = _Triplets(out["tri_ptr"].data_ptr(), out["edge_a"].data_ptr(), out["edge_b"].data_ptr(), int(capacity),
+                      out["n_triplets"].data_ptr())
+        rc = _lib().mg_triplets_graph(self._h, row_ptr.data_ptr(), n_atoms, ctypes.byref(c), _stream())
+        if rc != 0:
+            raise MatGraphError(rc, "mg_triplets_graph")
         return out
 
     def mg_check(self) -> int:

@@ -1,0 +1,189 @@
+// graph_ops.cuh — operations on a finished CSR edge list.
+//
+//   symmetric graph (section 3 "Symmetric graph"): the KNN graph is directed; the
+//     symmetric graph adds, for every edge (i, j, tau), the reverse edge (j, i, -tau) unless it is there
+//     already, and keeps edges unique.  Three launches: flag the edges whose reverse is missing and count
+//     them per target row; exclusive scan -> the new row_ptr; copy the old rows and append the new edges.
+//   triplets (Def. 3: Gamma_2, the pairs of edges that share their source; PAPER.md:131
+//     "Triplets generation"): for a source of degree d the d (d - 1) ordered pairs (a, b), a != b, of its
+//     edges, as two arrays of edge indices, CSR by source.  Two launches: scan of d (d - 1), emit.
+#pragma once
+#include "common.cuh"
+
+#define MGO_BLOCK 256
+#define MGO_SCAN_BLOCK 1024
+
+// Exclusive scan of v(r), r in [0, n), by ONE block of MGO_SCAN_BLOCK threads (chunks of the array in
+// turn; n is the number of atoms of a batch: tens of thousands).  out[r] = base(r) + sum_{q < r} v(q),
+// out[n] = base(n) + total; *total_out = out[n].
+template <class V, class B>
+__device__ __forceinline__ void mgo_block_scan(int n, V value, B base, long long *out64, int32_t *out32,
+                                               long long *total_out) {
+    __shared__ long long s_warp[MGO_SCAN_BLOCK / 32];
+    __shared__ long long s_carry;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) s_carry = 0ll;
+    __syncthreads();
+    for (int r0 = 0; r0 < n; r0 += MGO_SCAN_BLOCK) {
+        const int r = r0 + tid;
+        const long long v = r < n ? value(r) : 0ll;
+        long long incl = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const long long t = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+            if (lane >= o) incl += t;
+        }
+        if (lane == 31) s_warp[warp] = incl;
+        __syncthreads();
+        long long woff = 0ll, btotal = 0ll;
+        for (int w = 0; w < MGO_SCAN_BLOCK / 32; ++w) {
+            const long long t = s_warp[w];
+            if (w < warp) woff += t;
+            btotal += t;
+        }
+        const long long excl = s_carry + woff + incl - v;
+        if (r < n) {
+            if (out64) out64[r] = base(r) + excl;
+            if (out32) out32[r] = (int32_t)(base(r) + excl);
+        }
+        __syncthreads();
+        if (tid == 0) s_carry += btotal;
+        __syncthreads();
+    }
+    if (tid == 0) {
+        const long long tot = base(n) + s_carry;
+        if (out64) out64[n] = tot;
+        if (out32) out32[n] = (int32_t)tot;
+        *total_out = tot;
+    }
+}
+
+// ---- symmetric graph ------------------------------------------------------------------------------
+struct SymArgs {
+    // input graph (CSR by source)
+    const int32_t *row_ptr, *src, *dst;
+    const int8_t *offset;
+    const float *vec, *dist;
+    const long long *n_edges_in;
+    int n_atoms;
+    // output graph
+    int32_t *o_row_ptr, *o_src, *o_dst;
+    int8_t *o_offset;
+    float *o_vec, *o_dist;
+    long long capacity;
+    long long *n_edges_out;
+    // scratch
+    unsigned char *flag;       // [E_in] 1: the reverse edge is missing
+    int *extra;                // [n_atoms] missing reverse edges per target row (zero before the call)
+    int *fill;                 // [n_atoms] cursor of the appended edges (zero before the call)
+    unsigned *status;
+};
+
+// Edge e = (i, j, tau): is (j, i, -tau) in row j?
+__global__ void __launch_bounds__(MGO_BLOCK)
+mg_sym_flag_kernel(const SymArgs A) {
+    mg_grid_dependency_wait();
+    const long long E = *A.n_edges_in;
+    for (long long e = (long long)blockIdx.x * MGO_BLOCK + threadIdx.x; e < E; e += (long long)gridDim.x * MGO_BLOCK) {
+        const int i = A.src[e], j = A.dst[e];
+        const int t0 = -A.offset[3 * e], t1 = -A.offset[3 * e + 1], t2 = -A.offset[3 * e + 2];
+        bool found = false;
+        for (int q = A.row_ptr[j], qe = A.row_ptr[j + 1]; q < qe && !found; ++q)
+            found = A.dst[q] == i && A.offset[3 * (long long)q] == t0 && A.offset[3 * (long long)q + 1] == t1 &&
+                    A.offset[3 * (long long)q + 2] == t2;
+        A.flag[e] = found ? 0 : 1;
+        if (!found) atomicAdd(A.extra + j, 1);
+    }
+}
+
+__global__ void __launch_bounds__(MGO_SCAN_BLOCK)
+mg_sym_scan_kernel(const SymArgs A) {
+    mg_grid_dependency_wait();
+    long long total = 0ll;
+    __shared__ long long s_total;
+    mgo_block_scan(A.n_atoms, [&](int r) { return (long long)A.extra[r]; },
+                   [&](int r) { return (long long)A.row_ptr[r]; }, nullptr, A.o_row_ptr, &s_total);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        total = s_total;
+        *A.n_edges_out = total;
+        if (total > A.capacity || total > 0x7FFFFFFFll) atomicOr(A.status, MGS_CAPACITY);
+    }
+}
+
+__global__ void __launch_bounds__(MGO_BLOCK)
+mg_sym_emit_kernel(const SymArgs A) {
+    mg_grid_dependency_wait();
+    const long long E = *A.n_edges_in;
+    for (long long e = (long long)blockIdx.x * MGO_BLOCK + threadIdx.x; e < E; e += (long long)gridDim.x * MGO_BLOCK) {
+        const int i = A.src[e], j = A.dst[e];
+        const int8_t t0 = A.offset[3 * e], t1 = A.offset[3 * e + 1], t2 = A.offset[3 * e + 2];
+        const float v0 = A.vec[3 * e], v1 = A.vec[3 * e + 1], v2 = A.vec[3 * e + 2];
+        const float d = A.dist ? A.dist[e] : 0.f;
+        const long long po = (long long)A.o_row_ptr[i] + (e - A.row_ptr[i]);     // the old rows keep their order
+        if (po < A.capacity) {
+            A.o_src[po] = i; A.o_dst[po] = j;
+            A.o_offset[3 * po] = t0; A.o_offset[3 * po + 1] = t1; A.o_offset[3 * po + 2] = t2;
+            A.o_vec[3 * po] = v0; A.o_vec[3 * po + 1] = v1; A.o_vec[3 * po + 2] = v2;
+            if (A.o_dist) A.o_dist[po] = d;
+        }
+        if (A.flag[e]) {                               // append (j, i, -tau) to row j
+            const int slot = atomicAdd(A.fill + j, 1);
+            const long long pr = (long long)A.o_row_ptr[j] + (A.row_ptr[j + 1] - A.row_ptr[j]) + slot;
+            if (pr < A.capacity) {
+                A.o_src[pr] = j; A.o_dst[pr] = i;
+                A.o_offset[3 * pr] = (int8_t)-t0; A.o_offset[3 * pr + 1] = (int8_t)-t1; A.o_offset[3 * pr + 2] = (int8_t)-t2;
+                A.o_vec[3 * pr] = -v0; A.o_vec[3 * pr + 1] = -v1; A.o_vec[3 * pr + 2] = -v2;
+                if (A.o_dist) A.o_dist[pr] = d;
+            }
+        }
+    }
+}
+
+// ---- triplets -------------------------------------------------------------------------------------
+struct TripArgs {
+    const int32_t *row_ptr;
+    int n_atoms;
+    long long *tri_ptr;        // [n_atoms + 1]
+    int32_t *edge_a, *edge_b;  // [capacity]
+    long long capacity;
+    long long *n_triplets;
+    unsigned *status;
+};
+
+__global__ void __launch_bounds__(MGO_SCAN_BLOCK)
+mg_trip_scan_kernel(const TripArgs A) {
+    mg_grid_dependency_wait();
+    __shared__ long long s_total;
+    mgo_block_scan(A.n_atoms,
+                   [&](int r) { const long long d = A.row_ptr[r + 1] - A.row_ptr[r]; return d * (d - 1); },
+                   [&](int) { return 0ll; }, A.tri_ptr, nullptr, &s_total);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        *A.n_triplets = s_total;
+        if (s_total > A.capacity) atomicOr(A.status, MGS_CAPACITY);
+    }
+}
+
+// One warp per source row (rows handed round): triplet t of the row = (a, b) with a = t / (d - 1) and b
+// the (t % (d - 1))-th edge other than a; lanes over t, coalesced 4-byte stores.
+__global__ void __launch_bounds__(MGO_BLOCK)
+mg_trip_emit_kernel(const TripArgs A) {
+    mg_grid_dependency_wait();
+    const int lane = threadIdx.x & 31;
+    const int wid = (int)((blockIdx.x * MGO_BLOCK + threadIdx.x) >> 5), nw = (int)((gridDim.x * MGO_BLOCK) >> 5);
+    for (int r = wid; r < A.n_atoms; r += nw) {
+        const int e0 = A.row_ptr[r];
+        const long long d = A.row_ptr[r + 1] - e0;
+        if (d < 2) continue;
+        const long long nt = d * (d - 1), base = A.tri_ptr[r];
+        const int dm = (int)(d - 1);
+        for (long long t = lane; t < nt; t += 32) {
+            const int a = (int)(t / dm), bq = (int)(t - (long long)a * dm), b = bq + (bq >= a ? 1 : 0);
+            if (base + t < A.capacity) {
+                A.edge_a[base + t] = e0 + a;
+                A.edge_b[base + t] = e0 + b;
+            }
+        }
+    }
+}

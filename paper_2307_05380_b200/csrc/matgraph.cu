@@ -16,6 +16,7 @@
 #include "cut_scan.cuh"
 #include "knn_small.cuh"
 #include "knn_pairs.cuh"
+#include "graph_ops.cuh"
 
 struct mg_ctx {
     int device = 0;
@@ -49,6 +50,11 @@ struct mg_ctx {
     double *d_lat64 = nullptr;            // [lat64_cap, 9]
     size_t lat64_cap = 0;
     int write_occ = 0;
+    // scratch of mg_symmetrize (graph_ops.cuh)
+    unsigned char *d_symflag = nullptr;   // [symflag_cap]
+    size_t symflag_cap = 0;
+    int *d_symcnt = nullptr;              // [2, symcnt_cap] missing reverse edges per row, append cursors
+    size_t symcnt_cap = 0;
     CutRec *d_crec = nullptr;             // per-structure records of the cutoff path (cut_prep.cuh)
     unsigned long long *d_bpre = nullptr; // cost prefix over the prep blocks
     size_t crec_cap = 0;
@@ -181,6 +187,8 @@ extern "C" void mg_destroy(mg_ctx *c) {
     cudaFree(c->d_wclock);
     cudaFree(c->d_slots);
     cudaFree(c->d_pool);
+    cudaFree(c->d_symflag);
+    cudaFree(c->d_symcnt);
     cudaFree(c->d_codes);
     cudaFree(c->d_slice_row);
     cudaFree(c->d_pos64);
@@ -420,6 +428,8 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
         const size_t want_chunks = count_only ? 0 : need / MGS_CHUNK + (size_t)grid * MGS_WARPS * MGS_WAVES + 8;
         if (want_chunks > c->pool_chunks) {
             cudaFree(c->d_pool);
+    cudaFree(c->d_symflag);
+    cudaFree(c->d_symcnt);
             c->d_pool = nullptr; c->pool_chunks = 0;
             const size_t cap = want_chunks + want_chunks / 8;
             MG_CUDA(cudaMalloc(&c->d_pool, cap * MGS_CHUNK * sizeof(uint2)));
@@ -636,6 +646,60 @@ extern "C" mg_status mg_update_graph(mg_ctx *c, mg_graph *g, const float *pos, c
                               g->have_hint, (cudaStream_t)stream);
     if (rs == MG_OK) g->have_hint = 1;
     return rs;
+}
+
+// ---- operations on a finished graph (graph_ops.cuh) -------------------------------------------------
+extern "C" mg_status mg_symmetrize(mg_ctx *c, const mg_edges *in, int32_t n_atoms, const mg_edges *out, void *stream) {
+    if (!c || n_atoms < 0 || !in || !in->row_ptr || !in->n_edges || in->capacity < 0 || bad_edges(out, 0)) return MG_ERR_INVALID_ARG;
+    if (in->capacity > 0 && (!in->src || !in->dst || !in->offset || !in->vec)) return MG_ERR_INVALID_ARG;
+    if (out->dist && !in->dist) return MG_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    MG_CUDA(cudaSetDevice(c->device));
+    if ((size_t)in->capacity + 1 > c->symflag_cap) {
+        cudaFree(c->d_symflag);
+        c->d_symflag = nullptr; c->symflag_cap = 0;
+        const size_t cap = (size_t)in->capacity + (size_t)in->capacity / 8 + 1024;
+        MG_CUDA(cudaMalloc(&c->d_symflag, cap));
+        c->symflag_cap = cap;
+    }
+    if ((size_t)n_atoms + 1 > c->symcnt_cap) {
+        cudaFree(c->d_symcnt);
+        c->d_symcnt = nullptr; c->symcnt_cap = 0;
+        const size_t cap = (size_t)n_atoms + 1025;
+        MG_CUDA(cudaMalloc(&c->d_symcnt, 2 * cap * sizeof(int)));
+        c->symcnt_cap = cap;
+    }
+    MG_CUDA(cudaMemsetAsync(c->d_symcnt, 0, 2 * c->symcnt_cap * sizeof(int), st));
+    SymArgs A;
+    A.row_ptr = in->row_ptr; A.src = in->src; A.dst = in->dst; A.offset = in->offset; A.vec = in->vec; A.dist = in->dist;
+    A.n_edges_in = (const long long *)in->n_edges; A.n_atoms = n_atoms;
+    A.o_row_ptr = out->row_ptr; A.o_src = out->src; A.o_dst = out->dst; A.o_offset = out->offset; A.o_vec = out->vec;
+    A.o_dist = out->dist; A.capacity = out->capacity; A.n_edges_out = (long long *)out->n_edges;
+    A.flag = c->d_symflag; A.extra = c->d_symcnt; A.fill = c->d_symcnt + c->symcnt_cap; A.status = c->d_ctl + 4;
+    long long want = (in->capacity + MGO_BLOCK - 1) / MGO_BLOCK;
+    const int grid = (int)(want < 1 ? 1 : (want > (long long)c->sm_count * 16 ? (long long)c->sm_count * 16 : want));
+    MG_CUDA(launch_after(c, mg_sym_flag_kernel, grid, MGO_BLOCK, 0, st, A));
+    MG_CUDA(launch_after(c, mg_sym_scan_kernel, 1, MGO_SCAN_BLOCK, 0, st, A));
+    MG_CUDA(launch_after(c, mg_sym_emit_kernel, grid, MGO_BLOCK, 0, st, A));
+    c->launches += 3;
+    return MG_OK;
+}
+
+extern "C" mg_status mg_triplets_graph(mg_ctx *c, const int32_t *row_ptr, int32_t n_atoms, const mg_triplets *out, void *stream) {
+    if (!c || !row_ptr || n_atoms < 0 || !out || !out->tri_ptr || !out->n_triplets || out->capacity < 0) return MG_ERR_INVALID_ARG;
+    if (out->capacity > 0 && (!out->edge_a || !out->edge_b)) return MG_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    MG_CUDA(cudaSetDevice(c->device));
+    TripArgs A;
+    A.row_ptr = row_ptr; A.n_atoms = n_atoms; A.tri_ptr = (long long *)out->tri_ptr;
+    A.edge_a = out->edge_a; A.edge_b = out->edge_b; A.capacity = out->capacity;
+    A.n_triplets = (long long *)out->n_triplets; A.status = c->d_ctl + 4;
+    MG_CUDA(launch_after(c, mg_trip_scan_kernel, 1, MGO_SCAN_BLOCK, 0, st, A));
+    const long long want = ((long long)n_atoms * 32 + MGO_BLOCK - 1) / MGO_BLOCK;
+    const int grid = (int)(want < 1 ? 1 : (want > (long long)c->sm_count * 8 ? (long long)c->sm_count * 8 : want));
+    MG_CUDA(launch_after(c, mg_trip_emit_kernel, grid, MGO_BLOCK, 0, st, A));
+    c->launches += 2;
+    return MG_OK;
 }
 
 extern "C" mg_status mg_check(mg_ctx *c, void *stream) {

@@ -1,0 +1,99 @@
+"""GPU parity of mg_symmetrize and mg_triplets_graph against
+oracle/graph_ops.py, through the C ABI binding, on the library's own KNN / cutoff graphs."""
+import numpy as np
+import pytest
+
+from oracle import graph_ops as G
+from workloads import crystals as C
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def mg():
+    import paper_2307_05380_b200 as m
+    return m
+
+
+@pytest.fixture(scope="module")
+def ctx(mg):
+    c = mg.Context(0)
+    yield c
+    c.close()
+
+
+def _rows_as_sets(g, n_atoms):
+    tau = np.asarray(g["offset"] if "offset" in g else g["tau"]).reshape(-1, 3).astype(np.int64)
+    keys = [(int(d), int(t[0]), int(t[1]), int(t[2])) for d, t in zip(g["dst"], tau)]
+    rp = np.asarray(g["row_ptr"])
+    return [sorted(keys[rp[i]:rp[i + 1]]) for i in range(n_atoms)]
+
+
+@pytest.mark.parametrize("cfg,k", [(1, 12), (2, 12), (4, 24)])
+def test_symmetrize_knn(mg, ctx, cfg, k):
+    b = C.config_batch(cfg, n_struct=512 if cfg == 2 else None)
+    pos, lat, ptr = mg.to_device(b)
+    knn = ctx.knn_graph(pos, lat, ptr, k, dist=True)
+    out = mg.Edges.allocate(b.n_atoms, 2 * k * b.n_atoms, "cuda", dist=True)
+    ctx.mg_symmetrize(knn, b.n_atoms, out)
+    got = out.to_numpy()
+    assert ctx.mg_check() == 0
+    kn = knn.to_numpy()
+    ref = G.symmetrize(b.n_atoms, kn["src"], kn["dst"], kn["offset"], vec=kn["vec"], dist=kn["dist"])
+    assert got["n_edges"] == ref["n_edges"] and np.array_equal(got["row_ptr"], ref["row_ptr"])
+    assert np.array_equal(got["src"], np.repeat(np.arange(b.n_atoms), np.diff(got["row_ptr"])))
+    assert _rows_as_sets(got, b.n_atoms) == _rows_as_sets(ref, b.n_atoms)            # bit-exact edge sets
+    # the old rows keep their place and order; vec / dist of every edge equal the oracle's (exact: copies and negations)
+    look = {(int(s), int(d), *map(int, t)): (v, dd) for s, d, t, v, dd in zip(ref["src"], ref["dst"], ref["tau"], ref["vec"], ref["dist"])}
+    for s, d, t, v, dd in zip(got["src"], got["dst"], got["offset"], got["vec"], got["dist"]):
+        rv, rd = look[(int(s), int(d), *map(int, t))]
+        assert np.array_equal(np.asarray(rv, np.float32), v) and np.float32(rd) == dd
+    rp_in, rp = kn["row_ptr"], got["row_ptr"]
+    for i in range(0, b.n_atoms, max(1, b.n_atoms // 200)):
+        assert np.array_equal(got["dst"][rp[i]:rp[i] + k], kn["dst"][rp_in[i]:rp_in[i + 1]])
+
+
+def test_symmetrize_cutoff_is_identity_and_capacity_is_reported(mg, ctx):
+    b = C.config_batch(0)
+    pos, lat, ptr = mg.to_device(b)
+    cut = ctx.cutoff_graph(pos, lat, ptr, 5.0, dist=True)
+    e = int(cut.n_edges.item())
+    out = mg.Edges.allocate(b.n_atoms, e, "cuda", dist=True)
+    ctx.mg_symmetrize(cut, b.n_atoms, out)
+    got, cin = out.to_numpy(), cut.to_numpy()
+    assert ctx.mg_check() == 0 and got["n_edges"] == e
+    for key in ("row_ptr", "src", "dst", "offset", "vec", "dist"):
+        assert np.array_equal(got[key], cin[key]), key
+    # a KNN graph needs more room than it has edges: the required count comes back with MG_ERR_CAPACITY
+    knn = ctx.knn_graph(pos, lat, ptr, 4, dist=True)
+    small = mg.Edges.allocate(b.n_atoms, 4 * b.n_atoms, "cuda", dist=True)
+    ctx.mg_symmetrize(knn, b.n_atoms, small)
+    need = int(small.n_edges.item())
+    assert ctx.mg_check() == 6 and need > 4 * b.n_atoms
+    kn = knn.to_numpy()
+    assert need == G.symmetrize(b.n_atoms, kn["src"], kn["dst"], kn["offset"])["n_edges"]
+
+
+@pytest.mark.parametrize("kind", ["knn", "cutoff", "empty"])
+def test_triplets(mg, ctx, kind):
+    import torch
+    b = C.config_batch(1) if kind != "empty" else C.Batch(pos=np.zeros((0, 3), np.float32), lattice=np.zeros((0, 3, 3), np.float32),
+                                                           struct_ptr=np.zeros(1, np.int32))
+    if kind == "empty":
+        row_ptr = torch.zeros(1, dtype=torch.int32, device="cuda")
+    else:
+        pos, lat, ptr = mg.to_device(b)
+        g = ctx.knn_graph(pos, lat, ptr, 12) if kind == "knn" else ctx.cutoff_graph(pos, lat, ptr, 4.0)
+        row_ptr = g.row_ptr
+    ref = G.triplets(row_ptr.cpu().numpy())
+    out = ctx.mg_triplets_graph(row_ptr, b.n_atoms, ref["n_triplets"])
+    assert ctx.mg_check() == 0
+    assert int(out["n_triplets"].item()) == ref["n_triplets"]
+    assert np.array_equal(out["tri_ptr"].cpu().numpy(), ref["tri_ptr"])
+    n = ref["n_triplets"]
+    assert np.array_equal(out["edge_a"][:n].cpu().numpy(), ref["edge_a"]) and np.array_equal(out["edge_b"][:n].cpu().numpy(), ref["edge_b"])
+    if kind == "knn":
+        assert n == 12 * 11 * b.n_atoms
+        short = ctx.mg_triplets_graph(row_ptr, b.n_atoms, n // 2)            # too small: count still reported
+        assert ctx.mg_check() == 6 and int(short["n_triplets"].item()) == n
+        assert np.array_equal(short["edge_a"][:n // 2].cpu().numpy(), ref["edge_a"][:n // 2])
