@@ -94,6 +94,14 @@ mg_status mg_cutoff_graph(mg_ctx *ctx, const float *pos, const float *lattice,
                           const int32_t *struct_ptr, int32_t n_struct, int32_t n_atoms,
                           float r_c, const mg_edges *out, void *cuda_stream);
 
+/* Def. 3 with one cutoff per SOURCE atom ("c_i > 0 for 1 <= i <= n"; e.g. covalent radii):
+ * edge (i, j, tau) iff ||rho (x_j - x_i + tau)|| < radii[i], strict.  radii: device float32 [n_atoms].  Such a
+ * graph is not symmetric in general.  A structure with a radius that is not a positive finite number emits
+ * no edges and MG_ERR_UNSUPPORTED surfaces from mg_check.  Otherwise like mg_cutoff_graph. */
+mg_status mg_cutoff_graph_radii(mg_ctx *ctx, const float *pos, const float *lattice,
+                                const int32_t *struct_ptr, int32_t n_struct, int32_t n_atoms,
+                                const float *radii, const mg_edges *out, void *cuda_stream);
+
 /* Two-phase helper: number of edges mg_cutoff_graph would emit.  SYNCHRONISES the stream and
  * writes the count to HOST memory. */
 mg_status mg_cutoff_count(mg_ctx *ctx, const float *pos, const float *lattice,

@@ -50,8 +50,8 @@ def _load():
         lib.mgo_knn_graph.restype = ctypes.c_int
         lib.mgo_free.argtypes = [ctypes.POINTER(_Graph)]
         lib.mgo_free.restype = None
-        lib.mgo_edge_distance.argtypes = [fp, fp] + [ctypes.c_int32] * 5 + [ctypes.POINTER(ctypes.c_double)]
-        lib.mgo_edge_distance.restype = ctypes.c_double
+        lib.mgo_cutoff_graph_radii.argtypes = [fp, fp, ip, ctypes.c_int32, fp, ctypes.POINTER(_Graph)]
+        lib.mgo_cutoff_graph_radii.restype = ctypes.c_int
         lib.mgo_num_threads.restype = ctypes.c_int
         _lib = lib
     return _lib
@@ -106,6 +106,26 @@ def cutoff_graph(pos, lattice, struct_ptr, r_c: float) -> dict:
     rc = float(np.float32(r_c))
     rcode = lib.mgo_cutoff_graph(_ptr(pos, ctypes.c_float), _ptr(lattice, ctypes.c_float),
                                  _ptr(struct_ptr, ctypes.c_int32), lattice.shape[0], rc, ctypes.byref(g))
+    if rcode != 0:
+        raise ValueError(f"singular or non-finite lattice in structure {g.bad_struct}")
+    try:
+        return _take(g, knn=False)
+    finally:
+        lib.mgo_free(ctypes.byref(g))
+
+
+def cutoff_graph_radii(pos, lattice, struct_ptr, radii) -> dict:
+    """Def. 3 with one cutoff per SOURCE atom ("c_i > 0"): edge (i, j, tau) iff d < c_i."""
+    lib = _load()
+    pos, lattice, struct_ptr = _prep(pos, lattice, struct_ptr)
+    radii = np.ascontiguousarray(radii, dtype=np.float32)
+    assert radii.shape == (pos.shape[0],)
+    g = _Graph()
+    rcode = lib.mgo_cutoff_graph_radii(_ptr(pos, ctypes.c_float), _ptr(lattice, ctypes.c_float),
+                                       _ptr(struct_ptr, ctypes.c_int32), lattice.shape[0],
+                                       _ptr(radii, ctypes.c_float), ctypes.byref(g))
+    if rcode == 2:
+        raise ValueError("a radius is not a positive finite number")
     if rcode != 0:
         raise ValueError(f"singular or non-finite lattice in structure {g.bad_struct}")
     try:

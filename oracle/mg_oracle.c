@@ -231,6 +231,48 @@ int mgo_cutoff_graph(const float *pos, const float *lattice, const int32_t *stru
     return 0;
 }
 
+/* Def. 3 with a cutoff per SOURCE atom ("c_i > 0 for 1 <= i <= n": e.g. covalent
+ * radii): edge (i, j, tau) iff ||rho (x_j - x_i + tau)|| < c_i, strict, (i, i, 0) excluded; the box of source
+ * i is that of its own radius.  radii[n_atoms] are FP32 like the other inputs, promoted to double.
+ * Returns 0, 1 for an invalid lattice, 2 if some radius is not a positive finite number. */
+int mgo_cutoff_graph_radii(const float *pos, const float *lattice, const int32_t *struct_ptr,
+                           int32_t n_struct, const float *radii, mgo_graph *g)
+{
+    memset(g, 0, sizeof(*g));
+    g->bad_struct = -1;
+    const int64_t n_atoms = n_struct > 0 ? struct_ptr[n_struct] : 0;
+    for (int64_t i = 0; i < n_atoms; ++i)
+        if (!(radii[i] > 0.0f) || !isfinite((double)radii[i])) return 2;
+    row_t *rows = (row_t *)calloc((size_t)(n_atoms > 0 ? n_atoms : 1), sizeof(row_t));
+    int bad = -1;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int32_t s = 0; s < n_struct; ++s) {
+        const int32_t base = struct_ptr[s], n = struct_ptr[s + 1] - struct_ptr[s];
+        double A[3][3], h[3], V;
+        if (cell_geometry(lattice + 9 * (size_t)s, A, h, &V)) {
+#pragma omp critical
+            if (bad < 0 || s < bad) bad = s;
+            continue;
+        }
+        for (int32_t i = 0; i < n; ++i) {
+            const double r = (double)radii[base + i];
+            int32_t nb[3];
+            box_halfwidth(pos + 3 * (size_t)base, n, h, r, nb);
+            scan_source(pos + 3 * (size_t)base, n, A, nb, i, base, r, &rows[base + i]);
+        }
+    }
+    if (bad >= 0) {
+        for (int64_t i = 0; i < n_atoms; ++i) free(rows[i].e);
+        free(rows);
+        g->bad_struct = bad;
+        return 1;
+    }
+    graph_alloc(g, n_atoms, rows, 0);
+    for (int64_t i = 0; i < n_atoms; ++i) free(rows[i].e);
+    free(rows);
+    return 0;
+}
+
 /* KNN: pick a radius R, collect every image with d < R, enlarge R by 1.5 and start again from
  * scratch while any source of the structure has fewer than k; then sort each row by the total
  * order of R8 and keep the first k.  Every image with d < R was enumerated, so the k smallest
@@ -298,22 +340,6 @@ int mgo_knn_graph(const float *pos, const float *lattice, const int32_t *struct_
     return 0;
 }
 
-/* FP64 distance of one (src, dst, tau) triple, in the oracle's operation order — used by the
- * parity checker to decide whether a mismatching edge lies inside the 1e-5 A band. */
-double mgo_edge_distance(const float *pos, const float *lat9, int32_t i, int32_t j,
-                         int32_t t0, int32_t t1, int32_t t2, double *v_out)
-{
-    double A[3][3];
-    for (int a = 0; a < 3; ++a)
-        for (int c = 0; c < 3; ++c) A[a][c] = (double)lat9[3 * a + c];
-    const double f0 = ((double)pos[3 * j] - (double)pos[3 * i]) + (double)t0;
-    const double f1 = ((double)pos[3 * j + 1] - (double)pos[3 * i + 1]) + (double)t1;
-    const double f2 = ((double)pos[3 * j + 2] - (double)pos[3 * i + 2]) + (double)t2;
-    double v[3];
-    for (int k = 0; k < 3; ++k) v[k] = f0 * A[0][k] + f1 * A[1][k] + f2 * A[2][k];
-    if (v_out) { v_out[0] = v[0]; v_out[1] = v[1]; v_out[2] = v[2]; }
-    return sqrt(v[0] * v[0] + v[1] * v[1] + v[2] * v[2]);
-}
 
 int mgo_num_threads(void)
 {

@@ -23,7 +23,7 @@ MG_MAX_K = 64
 EXPORTS = ["mg_create", "mg_destroy", "mg_reserve", "mg_cutoff_graph", "mg_cutoff_count",
            "mg_knn_graph", "mg_graph_create", "mg_graph_destroy", "mg_update_graph",
            "mg_cutoff_graph_host", "mg_knn_graph_host", "mg_check", "mg_launch_count",
-           "mg_status_string", "mg_set_profile", "mg_profile_read", "mg_symmetrize", "mg_triplets_graph"]
+           "mg_status_string", "mg_set_profile", "mg_profile_read", "mg_symmetrize", "mg_triplets_graph", "mg_cutoff_graph_radii"]
 
 
 class MatGraphError(RuntimeError):
@@ -73,6 +73,7 @@ def _lib():
         lib.mg_launch_count.restype = i64
         lib.mg_set_profile.argtypes = [vp, ctypes.c_int]
         lib.mg_profile_read.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(i64)]
+        lib.mg_cutoff_graph_radii.argtypes = [vp, vp, vp, vp, i32, i32, vp, ep, vp]
         lib.mg_symmetrize.argtypes = [vp, ep, i32, ep, vp]
         lib.mg_triplets_graph.argtypes = [vp, vp, i32, ctypes.POINTER(_Triplets), vp]
         lib.mg_status_string.argtypes = [ctypes.c_int]
@@ -237,6 +238,15 @@ class Context:
                                     ctypes.byref(out._c()), _stream())
         if rc != 0:
             raise MatGraphError(rc, "mg_update_graph")
+        return out
+
+    def mg_cutoff_graph_radii(self, pos, lattice, struct_ptr, radii, out: Edges) -> Edges:
+        n_struct, n_atoms = _check_inputs(pos, lattice, struct_ptr)
+        assert radii.is_cuda and radii.dtype == _torch().float32 and radii.numel() == n_atoms and radii.is_contiguous()
+        rc = _lib().mg_cutoff_graph_radii(self._h, pos.data_ptr(), lattice.data_ptr(), struct_ptr.data_ptr(),
+                                          n_struct, n_atoms, radii.data_ptr(), ctypes.byref(out._c()), _stream())
+        if rc != 0:
+            raise MatGraphError(rc, "mg_cutoff_graph_radii")
         return out
 
     def mg_symmetrize(self, inp: Edges, n_atoms: int, out: Edges) -> Edges:

@@ -86,6 +86,9 @@ struct CutPrepArgs {
                                    // (read when use_hint, then reset to 0: the graph kernel maxes into it)
     int use_hint;
     int rows_cost;                 // cutoff: cost model of the scan kernel (cut_scan.cuh)
+    const float *radii;            // [n_atoms] or NULL: per-atom cutoffs (cutoff graph); the structure's radius is
+                                   // their maximum; a radius that is not a positive finite number makes the
+                                   // structure invalid (MGS_UNSUPPORTED)
     const float *pos;              // with xw4: positions of the batch
     float4 *xw4;                   // [n_atoms] or NULL: wrapped fractional coordinates x - floor(x), .w = the integer
                                    // parts packed (mg_wrap_x): written by the blocks after the first n_sblocks ones
@@ -128,6 +131,17 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
         double vol = 0.0, h[3] = {1.0, 1.0, 1.0};
         unsigned err = mg_cell_spacings_fast(lat, &vol, h);
         float rc = A.r_c;
+        if (A.radii) {
+            rc = 0.f;
+            bool okr = true;
+            for (int i = 0; i < N; ++i) {
+                const float ci = A.radii[r.first + i];
+                okr = okr && ci > 0.f && isfinite(ci);
+                rc = fmaxf(rc, ci);
+            }
+            if (!okr) err |= MGS_UNSUPPORTED;
+            if (!(rc > 0.f) || !isfinite(rc)) rc = 1.f;
+        }
         if (A.k > 0) {                                 // KNN: radius from the density, or from the last call
             const float hv = A.hint && A.use_hint ? A.hint[s] : 0.f;
             rc = MG_KNN_RSCALE * cbrtf(0.2387324f * (MG_KNN_ALPHA * (float)A.k + 1.f) * (float)vol / (float)max(N, 1));

@@ -46,7 +46,8 @@ struct ScanArgs {
     const float *lattice;
     const float4 *xw4;             // [n_atoms] wrapped coordinates + packed integer parts (cut_prep.cuh)
     int n_struct, n_atoms;
-    float r_c;
+    const float *radii;            // [n_atoms] or NULL: cutoff of every SOURCE atom (Def. 3's c_i); NULL: the
+                                   // same cutoff for all (the structure's radius in its CutRec)
     int32_t *row_ptr;
     long long capacity;
     long long *n_edges;
@@ -111,6 +112,7 @@ struct WCtx {
     float nr2, win, rc;
     const float *gx;       // positions of the structure's first atom
     const float4 *xw;      // ... and their wrapped copies
+    const float *cr;       // ... and their cutoffs (NULL: rc for all)
     const float *lat;
     int first, N;
 };
@@ -123,14 +125,18 @@ __device__ __forceinline__ void mgs_ctx(WCtx &C, const ScanArgs &A, const CutRec
     for (int a = 0; a < 3; ++a) C.rho[a] = R->rho[a];
     C.m0 = R->m & 0xFF; C.m1 = (R->m >> 8) & 0xFF; C.m2 = (R->m >> 16) & 0xFF;
     C.mloc = R->mloc;
-    C.rc = A.r_c;
-    C.nr2 = -__fmul_rn(A.r_c, A.r_c);
+    // (with per-atom cutoffs the structure's radius is the largest of them: bounds and the rounding window hold
+    // for every source, the threshold itself is the source's)
+    const float rc = R->radius;
+    C.rc = rc;
+    C.nr2 = -__fmul_rn(rc, rc);
     // FP32 error bound of d2 - rc^2 near the threshold (R23)
-    C.win = 1.1920929e-7f * (2.f * A.r_c * (13.f * R->qmax + 2.f * R->amax_sum) + 4.f * A.r_c * A.r_c);
+    C.win = 1.1920929e-7f * (2.f * rc * (13.f * R->qmax + 2.f * R->amax_sum) + 4.f * rc * rc);
     C.first = R->first;
     C.N = R->natoms;
     C.gx = A.pos + 3 * (size_t)R->first;
     C.xw = A.xw4 + R->first;
+    C.cr = A.radii ? A.radii + R->first : nullptr;
 }
 
 
@@ -174,6 +180,7 @@ struct SPair {
     float qx, qy, qz;
     int l0, l1, l2;
     int self;              // index of the cell tau = 0 in the table if i == j, else -1
+    float rc;              // cutoff of the source
     bool ok;               // valid lane, offsets inside int8
 };
 
@@ -195,6 +202,7 @@ __device__ __forceinline__ SPair mgs_pair(const SSmem &ws, const WCtx &C, bool v
            p.l2 + C.m2 <= 128;
     if (!p.ok) { p.qx = 1e18f; p.qy = 1e18f; p.qz = 1e18f; }
     p.self = i == j ? (-(int)e0 * C.m1 - (int)e1) * C.m2 - (int)e2 : -1;   // (i,i,0) is not an edge (R3)
+    p.rc = C.cr ? C.cr[i] : C.rc;
     return p;
 }
 
@@ -208,7 +216,8 @@ __device__ __forceinline__ unsigned mgs_word_mask(const SSmem &ws, const WCtx &C
     const float4 *Yp = reinterpret_cast<const float4 *>(&ws.T[1][32 * w]);
     const float4 *Zp = reinterpret_cast<const float4 *>(&ws.T[2][32 * w]);
     const float2 qx = make_float2(p.qx, p.qx), qy = make_float2(p.qy, p.qy), qz = make_float2(p.qz, p.qz);
-    const float2 nr2 = make_float2(C.nr2, C.nr2);
+    const float nr2s = C.cr ? -__fmul_rn(p.rc, p.rc) : C.nr2;
+    const float2 nr2 = make_float2(nr2s, nr2s);
     const float win = C.win;
     unsigned mask = 0u;
     bool near = false;
@@ -231,14 +240,14 @@ __device__ __forceinline__ unsigned mgs_word_mask(const SSmem &ws, const WCtx &C
         for (int c = 0; c < nw; ++c) {
             const float Tx = ws.T[0][32 * w + c], Ty = ws.T[1][32 * w + c], Tz = ws.T[2][32 * w + c];
             const float vx = __fadd_rn(p.qx, Tx), vy = __fadd_rn(p.qy, Ty), vz = __fadd_rn(p.qz, Tz);
-            const float y = __fmaf_rn(vz, vz, __fmaf_rn(vy, vy, __fmaf_rn(vx, vx, C.nr2)));
+            const float y = __fmaf_rn(vz, vz, __fmaf_rn(vy, vy, __fmaf_rn(vx, vx, nr2s)));
             if (fabsf(y) < win) {
                 const unsigned tc = ws.tcode[32 * w + c];
                 double v[3];
                 const double d = mg_exact_vec(xi, xj, p.l0 + (int)(tc >> 24), p.l1 + (int)((tc >> 16) & 0xFFu),
                                               p.l2 + (int)((tc >> 8) & 0xFFu), C.lat, v);
                 const unsigned bit = 0x80000000u >> c;
-                mask = d < (double)C.rc ? (mask | bit) : (mask & ~bit);
+                mask = d < (double)p.rc ? (mask | bit) : (mask & ~bit);
             }
         }
     }
@@ -253,7 +262,7 @@ __device__ __forceinline__ unsigned mgs_word_mask(const SSmem &ws, const WCtx &C
 // (wrapped coordinates), the sub-box starts at lo_a = floor(-rho_a - u_a) + 1 (cut_prep.cuh);
 // d2 = |(u + lo + t) . L|^2 in FP32, FP64 decision inside the rounding window (R23).
 // Candidate (j, t) of row i: hit?  tau (relative to the coordinates as given) in tau[3].
-__device__ __forceinline__ bool mgs_cand(const WCtx &C, const float4 xi, int i, int j, int t0, int t1, int t2,
+__device__ __forceinline__ bool mgs_cand(const WCtx &C, const float4 xi, float rci, int i, int j, int t0, int t1, int t2,
                                          int tau[3], bool &bad) {
     const float4 xj = C.xw[j];
     const int ki = __float_as_int(xi.w), kj = __float_as_int(xj.w);
@@ -264,7 +273,7 @@ __device__ __forceinline__ bool mgs_cand(const WCtx &C, const float4 xi, int i, 
     const float vx = __fmaf_rn(f2, C.a[6], __fmaf_rn(f1, C.a[3], __fmul_rn(f0, C.a[0])));
     const float vy = __fmaf_rn(f2, C.a[7], __fmaf_rn(f1, C.a[4], __fmul_rn(f0, C.a[1])));
     const float vz = __fmaf_rn(f2, C.a[8], __fmaf_rn(f1, C.a[5], __fmul_rn(f0, C.a[2])));
-    const float y = __fmaf_rn(vz, vz, __fmaf_rn(vy, vy, __fmaf_rn(vx, vx, C.nr2)));
+    const float y = __fmaf_rn(vz, vz, __fmaf_rn(vy, vy, __fmaf_rn(vx, vx, -__fmul_rn(rci, rci))));
     tau[0] = (int)e0 + t0 + (ki & 1023) - (kj & 1023);
     tau[1] = (int)e1 + t1 + ((ki >> 10) & 1023) - ((kj >> 10) & 1023);
     tau[2] = (int)e2 + t2 + ((ki >> 20) & 1023) - ((kj >> 20) & 1023);
@@ -274,7 +283,7 @@ __device__ __forceinline__ bool mgs_cand(const WCtx &C, const float4 xi, int i, 
     bool hit = y < 0.f;
     if (fabsf(y) < C.win) {                                          // FP32 cannot decide: Def. 3 in FP64
         double v[3];
-        hit = mg_exact_vec(C.gx + 3 * i, C.gx + 3 * j, tau[0], tau[1], tau[2], C.lat, v) < (double)C.rc;
+        hit = mg_exact_vec(C.gx + 3 * i, C.gx + 3 * j, tau[0], tau[1], tau[2], C.lat, v) < (double)rci;
     }
     return hit;
 }
@@ -353,6 +362,7 @@ template <int PHASE>
 __device__ __forceinline__ unsigned mgs_row(const ScanArgs &A, SSmem &ws, PoolState &P, const WCtx &C, int i,
                                             unsigned long long goff, int lane, bool &anybad) {
     const float4 xi = C.xw[i];
+    const float rci = C.cr ? C.cr[i] : C.rc;
     const int M12 = C.m1 * C.m2;
     unsigned cnt = 0u;
     const bool wide = C.mloc >= 32;
@@ -367,7 +377,7 @@ __device__ __forceinline__ unsigned mgs_row(const ScanArgs &A, SSmem &ws, PoolSt
             const int j = j0 + jl;
             int tau[3] = {0, 0, 0};
             bool bad = false;
-            const bool hit = cv && j < C.N && mgs_cand(C, xi, i, j, t0, t1, t2, tau, bad);
+            const bool hit = cv && j < C.N && mgs_cand(C, xi, rci, i, j, t0, t1, t2, tau, bad);
             anybad = anybad || bad;
             const unsigned bal = __ballot_sync(0xFFFFFFFFu, hit);
             if (PHASE == 0 && bal) mgs_pool_reserve(A, ws, P, P.wcount + cnt + 32u, lane);

@@ -186,9 +186,9 @@ extern "C" void mg_destroy(mg_ctx *c) {
     cudaFree(c->d_wmask);
     cudaFree(c->d_wclock);
     cudaFree(c->d_slots);
-    cudaFree(c->d_pool);
     cudaFree(c->d_symflag);
     cudaFree(c->d_symcnt);
+    cudaFree(c->d_pool);
     cudaFree(c->d_codes);
     cudaFree(c->d_slice_row);
     cudaFree(c->d_pos64);
@@ -383,7 +383,7 @@ static mg_status launch_prep(mg_ctx *c, const float *pos, const float *lat, cons
 
 static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, const int32_t *sp,
                                int32_t n_struct, int32_t n_atoms, float r_c, const mg_edges *o,
-                               int count_only, cudaStream_t st) {
+                               int count_only, cudaStream_t st, const float *radii = nullptr) {
     MG_CUDA(cudaSetDevice(c->device));
     mg_status rs = mg_reserve(c, n_struct, n_atoms);
     if (rs != MG_OK) return rs;
@@ -397,13 +397,13 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
     // Two cutoff paths: the scan kernel (cut_scan.cuh) and the count + emit pair (cutoff_pairs.cuh).  The pair is
     // ahead on batches of small cells (BASELINE configs[2]: 73 against 81 us per call), the scan kernel on large
     // structures; MATGRAPH_FUSED=1 / MATGRAPH_LEGACY=1 force one of them.
-    const bool use_scan = c->force_scan || (!c->force_legacy && n_struct > 0 && n_atoms / n_struct > MG_SMALL_MAX_ATOMS);
+    const bool use_scan = radii || c->force_scan || (!c->force_legacy && n_struct > 0 && n_atoms / n_struct > MG_SMALL_MAX_ATOMS);
     if (prof) { prof_collect(c); cudaEventRecord(c->ev[0], st); }
     {
         CutPrepArgs P;
         P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms; P.r_c = r_c;
         P.k = 0; P.hint = nullptr; P.use_hint = 0; P.rows_cost = use_scan ? 1 : 0;
-        P.pos = pos; P.xw4 = use_scan ? c->d_xw4 : nullptr; P.n_sblocks = n_blocks;
+        P.pos = pos; P.xw4 = use_scan ? c->d_xw4 : nullptr; P.n_sblocks = n_blocks; P.radii = radii;
         P.rec = c->d_crec; P.bpre = c->d_bpre; P.ctl = c->d_ctl; P.status = c->d_ctl + 4;
         // (scan path: extra blocks wrap the coordinates of the batch's atoms)
         const int xblocks = use_scan ? (n_atoms + 8 * MG_CP_BLOCK - 1) / (8 * MG_CP_BLOCK) : 0;
@@ -428,15 +428,13 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
         const size_t want_chunks = count_only ? 0 : need / MGS_CHUNK + (size_t)grid * MGS_WARPS * MGS_WAVES + 8;
         if (want_chunks > c->pool_chunks) {
             cudaFree(c->d_pool);
-    cudaFree(c->d_symflag);
-    cudaFree(c->d_symcnt);
             c->d_pool = nullptr; c->pool_chunks = 0;
             const size_t cap = want_chunks + want_chunks / 8;
             MG_CUDA(cudaMalloc(&c->d_pool, cap * MGS_CHUNK * sizeof(uint2)));
             c->pool_chunks = cap;
         }
         ScanArgs F;
-        F.pos = pos; F.lattice = lat; F.xw4 = c->d_xw4; F.n_struct = n_struct; F.n_atoms = n_atoms; F.r_c = r_c;
+        F.pos = pos; F.lattice = lat; F.xw4 = c->d_xw4; F.n_struct = n_struct; F.n_atoms = n_atoms; F.radii = radii;
         F.row_ptr = o->row_ptr; F.capacity = o->capacity; F.n_edges = (long long *)o->n_edges;
         F.rec = c->d_crec; F.bpre = c->d_bpre; F.n_blocks = n_blocks;
         F.pool = c->d_pool;
@@ -511,6 +509,13 @@ extern "C" mg_status mg_cutoff_graph(mg_ctx *c, const float *pos, const float *l
     return launch_cutoff(c, pos, lat, sp, n_struct, n_atoms, r_c, o, 0, (cudaStream_t)stream);
 }
 
+extern "C" mg_status mg_cutoff_graph_radii(mg_ctx *c, const float *pos, const float *lat, const int32_t *sp,
+                                           int32_t n_struct, int32_t n_atoms, const float *radii, const mg_edges *o,
+                                           void *stream) {
+    if (bad_inputs(c, pos, lat, sp, n_struct, n_atoms) || bad_edges(o, 0) || (n_atoms > 0 && !radii)) return MG_ERR_INVALID_ARG;
+    return launch_cutoff(c, pos, lat, sp, n_struct, n_atoms, 1.f, o, 0, (cudaStream_t)stream, radii);
+}
+
 extern "C" mg_status mg_cutoff_count(mg_ctx *c, const float *pos, const float *lat, const int32_t *sp,
                                      int32_t n_struct, int32_t n_atoms, float r_c,
                                      int64_t *n_edges_host, void *stream) {
@@ -543,7 +548,7 @@ static mg_status launch_knn(mg_ctx *c, const float *pos, const float *lat, const
         CutPrepArgs P;
         P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms; P.r_c = 0.f;
         P.k = k; P.hint = hint; P.use_hint = use_hint; P.rows_cost = 0;
-        P.pos = pos; P.xw4 = nullptr; P.n_sblocks = n_blocks;
+        P.pos = pos; P.xw4 = nullptr; P.n_sblocks = n_blocks; P.radii = nullptr;
         P.rec = c->d_crec; P.bpre = c->d_bpre; P.ctl = c->d_ctl; P.status = c->d_ctl + 4;
         MG_CUDA(launch_after(c, mg_cut_prep_kernel, n_blocks, MG_CP_BLOCK, 0, st, P));
         c->launches += 1;

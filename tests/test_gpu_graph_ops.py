@@ -97,3 +97,44 @@ def test_triplets(mg, ctx, kind):
         short = ctx.mg_triplets_graph(row_ptr, b.n_atoms, n // 2)            # too small: count still reported
         assert ctx.mg_check() == 6 and int(short["n_triplets"].item()) == n
         assert np.array_equal(short["edge_a"][:n // 2].cpu().numpy(), ref["edge_a"][:n // 2])
+
+
+# ------------------------------------------------------------------ per-atom cutoffs
+@pytest.mark.parametrize("cfg", [0, 2, 3])
+def test_cutoff_graph_radii(mg, ctx, cfg):
+    import torch
+    import oracle
+    from oracle import check
+    b = C.config_batch(cfg, n_struct={0: None, 2: 512, 3: 2}[cfg])
+    rng = np.random.default_rng(17 + cfg)
+    radii = rng.uniform(2.0, 6.5, b.n_atoms).astype(np.float32)      # "covalent-like": one cutoff per atom
+    ref = oracle.cutoff_graph_radii(b.pos, b.lattice, b.struct_ptr, radii)
+    pos, lat, ptr = mg.to_device(b)
+    out = mg.Edges.allocate(b.n_atoms, ref["n_edges"], "cuda", dist=True)
+    ctx.mg_cutoff_graph_radii(pos, lat, ptr, torch.from_numpy(radii).cuda(), out)
+    got = out.to_numpy()
+    assert ctx.mg_check() == 0
+    assert got["n_edges"] == ref["n_edges"] and np.array_equal(got["row_ptr"], ref["row_ptr"])
+    kg = np.sort(check._keys(got["src"], got["dst"], got["offset"]))
+    ko = np.sort(check._keys(ref["src"], ref["dst"], ref["tau"]))
+    assert np.array_equal(kg, ko)                                     # bit-exact edge sets (FP64 window decision)
+    d64, v64 = oracle.edge_distance(b.pos, b.lattice, b.struct_ptr, got["src"], got["dst"], got["offset"])
+    assert np.abs(got["vec"] - v64).max() <= 1e-5 and np.abs(got["dist"] - d64).max() <= 1e-5
+    assert np.all(d64 < radii[got["src"]].astype(np.float64))
+
+
+def test_cutoff_graph_radii_constant_equals_cutoff_graph(mg, ctx):
+    import torch
+    b = C.config_batch(0)
+    pos, lat, ptr = mg.to_device(b)
+    a = ctx.cutoff_graph(pos, lat, ptr, 5.0, dist=True).to_numpy()
+    out = mg.Edges.allocate(b.n_atoms, a["n_edges"], "cuda", dist=True)
+    ctx.mg_cutoff_graph_radii(pos, lat, ptr, torch.full((b.n_atoms,), 5.0, device="cuda"), out)
+    g = out.to_numpy()
+    assert ctx.mg_check() == 0 and g["n_edges"] == a["n_edges"] and np.array_equal(g["row_ptr"], a["row_ptr"])
+    from oracle import check
+    assert np.array_equal(np.sort(check._keys(g["src"], g["dst"], g["offset"])), np.sort(check._keys(a["src"], a["dst"], a["offset"])))
+    bad = torch.full((b.n_atoms,), 5.0, device="cuda")
+    bad[3] = -1.0
+    ctx.mg_cutoff_graph_radii(pos, lat, ptr, bad, out)
+    assert ctx.mg_check() == 7                                         # MG_ERR_UNSUPPORTED

@@ -448,3 +448,55 @@ def test_checker_accepts_oracle_and_rejects_damage():
         bad[name][j + 1] = a_
     with pytest.raises(AssertionError):
         check.check_knn(b, 12, bad, kref)
+
+
+# ------------------------------------------------------------------ statistics the oracle reports
+def _spacings_np(lat):
+    A = lat.astype(np.float64)
+    V = np.abs(np.linalg.det(A))
+    return np.stack([V / np.linalg.norm(np.cross(A[:, (a + 1) % 3], A[:, (a + 2) % 3]), axis=1) for a in range(3)], axis=1)
+
+
+def test_n_box_and_n_evaluated_are_what_they_say():
+    # n_box = sum_s N_s^2 prod_a (2 ceil(r/h_a) + 1) (the search box of BASELINE.json's north_star);
+    # n_evaluated = the oracle's own box, one cell wider per side, minus the skipped (i, i, 0)
+    b = C.small_batch(20, seed=6)
+    r = 4.25
+    g = oracle.cutoff_graph(b.pos, b.lattice, b.struct_ptr, r)
+    h = _spacings_np(b.lattice)
+    n = np.diff(b.struct_ptr).astype(np.float64)
+    assert g["n_box"] == float(np.sum(n * n * np.prod(2 * np.ceil(r / h) + 1, axis=1)))
+    assert g["n_evaluated"] == int(np.sum(n * n * np.prod(2 * (np.ceil(r / h) + 1) + 1, axis=1) - n))
+
+
+# ------------------------------------------------------------------ per-atom cutoffs
+def test_radii_equal_to_a_constant_is_the_cutoff_graph():
+    b = C.small_batch(10, seed=12)
+    ref = oracle.cutoff_graph(b.pos, b.lattice, b.struct_ptr, 4.0)
+    got = oracle.cutoff_graph_radii(b.pos, b.lattice, b.struct_ptr, np.full(b.n_atoms, 4.0, np.float32))
+    for key in ("row_ptr", "src", "dst", "tau"):
+        assert np.array_equal(ref[key], got[key]), key
+
+
+def test_radii_rows_are_the_rows_of_the_constant_cutoff_graphs():
+    # row i of the per-atom graph = row i of the constant-cutoff graph with r_c = c_i (Def. 3 is per source)
+    b = C.small_batch(6, seed=13)
+    rng = np.random.default_rng(5)
+    radii = rng.choice(np.array([2.5, 3.5, 5.0], np.float32), size=b.n_atoms)
+    got = oracle.cutoff_graph_radii(b.pos, b.lattice, b.struct_ptr, radii)
+    for r in (2.5, 3.5, 5.0):
+        ref = oracle.cutoff_graph(b.pos, b.lattice, b.struct_ptr, r)
+        for i in np.nonzero(radii == np.float32(r))[0]:
+            a = slice(ref["row_ptr"][i], ref["row_ptr"][i + 1])
+            g = slice(got["row_ptr"][i], got["row_ptr"][i + 1])
+            assert np.array_equal(ref["dst"][a], got["dst"][g]) and np.array_equal(ref["tau"][a], got["tau"][g])
+    assert np.all(got["dist"] < radii[got["src"]].astype(np.float64))
+
+
+def test_radii_break_edge_symmetry_sc_two_atoms():
+    # two atoms 0.5 apart along x in a unit cube; c_0 = 0.6 reaches atom 1 (at 0.5, both ways), c_1 = 0.4 reaches nothing
+    b = C.Batch(pos=np.array([[0, 0, 0], [0.5, 0, 0]], np.float32), lattice=np.eye(3, dtype=np.float32)[None],
+                struct_ptr=np.array([0, 2], np.int32))
+    g = oracle.cutoff_graph_radii(b.pos, b.lattice, b.struct_ptr, np.array([0.6, 0.4], np.float32))
+    assert list(np.diff(g["row_ptr"])) == [2, 0]
+    assert sorted(map(tuple, g["tau"].tolist())) == [(-1, 0, 0), (0, 0, 0)] and list(g["dst"]) == [1, 1]
