@@ -247,13 +247,40 @@ def run_gpu(args, rank, world, local_rank):
     t_cut = {"hbm_us": bytes_cut / (hbm_gbs * 1e9) * 1e6, "fp32_us": c_cut * INSTR_PER_CANDIDATE / fp32_rate * 1e6}
     t_knn = {"hbm_us": bytes_knn / (hbm_gbs * 1e9) * 1e6, "fp32_us": c_knn * INSTR_PER_CANDIDATE / fp32_rate * 1e6}
     roof_cut, roof_knn = max(t_cut.values()), max(t_knn.values())
-    # dominant kernel: mg_cutoff_emit_kernel writes the edge stream (algorithmic bytes of the cutoff call)
-    achieved = bytes_cut / (emit_us * 1e-6) / 1e9
-    traffic = None
+    kernel_us = {"mg_cut_prep_kernel": prep_us, "mg_cutoff_count_kernel": count_us,
+                 "mg_cutoff_emit_kernel": emit_us, "mg_knn_pairs_kernel": knnk_us}
+    traffic_all = {}
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         with open(tpath) as f:
-            traffic = json.load(f).get("mg_cutoff_emit_kernel_dram_bytes_per_launch")
+            traffic_all = json.load(f)
+    # the `roofline` object describes the DOMINANT kernel of the step (largest mean duration); the per-call
+    # fractions are in `roofline_model`, the other kernels' in `roofline_kernels`
+    def kernel_roofline(name):
+        us = kernel_us[name]
+        if name == "mg_knn_pairs_kernel":        # FP32-pipe bound: C_knn candidates x 7 lane-instructions
+            ach = c_knn * INSTR_PER_CANDIDATE / (us * 1e-6)
+            return {"bound": "alu", "achieved": ach / 1e12, "peak": fp32_rate / 1e12, "unit": "T lane-instr/s",
+                    "frac": ach / fp32_rate, "kernel": name, "us": us,
+                    "peak_kind": f"derived: {sms} SMs x {FP32_LANES_PER_SM} FP32 lanes x {sm_mhz:.0f} MHz (DESIGN.md 5.3)",
+                    "algorithmic_lane_instr": c_knn * INSTR_PER_CANDIDATE,
+                    "traffic": traffic_all.get(name + "_dram_bytes_per_launch")}
+        if name == "mg_cutoff_count_kernel":     # FP32-pipe bound: the box candidates of the cutoff call
+            ach = c_cut * INSTR_PER_CANDIDATE / (us * 1e-6)
+            return {"bound": "alu", "achieved": ach / 1e12, "peak": fp32_rate / 1e12, "unit": "T lane-instr/s",
+                    "frac": ach / fp32_rate, "kernel": name, "us": us,
+                    "peak_kind": f"derived: {sms} SMs x {FP32_LANES_PER_SM} FP32 lanes x {sm_mhz:.0f} MHz (DESIGN.md 5.3)",
+                    "algorithmic_lane_instr": c_cut * INSTR_PER_CANDIDATE,
+                    "traffic": traffic_all.get(name + "_dram_bytes_per_launch")}
+        ach = bytes_cut / (us * 1e-6) / 1e9      # the emit kernel moves the cutoff call's algorithmic bytes
+        return {"bound": "hbm", "achieved": ach, "peak": hbm_gbs, "unit": "GB/s", "frac": ach / hbm_gbs,
+                "kernel": name, "us": us, "peak_kind": peak_kind, "algorithmic_bytes": bytes_cut,
+                "traffic": traffic_all.get(name + "_dram_bytes_per_launch")}
+
+    graph_kernels = [k for k in kernel_us if k != "mg_cut_prep_kernel" and kernel_us[k] > 0]
+    dominant = max(graph_kernels, key=lambda k: kernel_us[k])
+    roofline = kernel_roofline(dominant)
+    roofline_kernels = {k: kernel_roofline(k) for k in graph_kernels if k != dominant}
 
     # ---- end to end through the host-buffer C ABI (pinned host memory, copies inside the call)
     e2e_steps = max(3, min(K, 10))
@@ -295,7 +322,7 @@ def run_gpu(args, rank, world, local_rank):
     cpu = None
     if world == 1 and not args.no_cpu_baseline:
         import oracle
-        reps = 4
+        reps = 8
         oracle.build()
         t0 = time.perf_counter()
         ne = 0
@@ -306,6 +333,33 @@ def run_gpu(args, rank, world, local_rank):
         cpu = {"value": ne / dt, "unit": "edges/s", "cores": oracle.num_threads(), "kind": "oracle",
                "sample": f"the full {S}-structure batch, cutoff + KNN, {reps} repetitions ({dt:.1f} s)",
                "structures_per_s": S * reps / dt}
+        # the other configs, one repetition each (SURVEY 8(d) "Oracle timed beside it")
+        try:
+            b3c = C.config_batch(3, n_struct=4)
+            t0 = time.perf_counter()
+            g3 = oracle.cutoff_graph(b3c.pos, b3c.lattice, b3c.struct_ptr, 8.0)
+            cpu["config3_cutoff"] = {"s": time.perf_counter() - t0, "edges": int(g3["n_edges"]), "sample": "4 of the 16 supercells"}
+            b4c = C.config_batch(4)
+            t0 = time.perf_counter()
+            for _ in range(3):
+                oracle.knn_graph(b4c.pos, b4c.lattice, b4c.struct_ptr, 24)
+            cpu["config4_knn24_s_per_step"] = (time.perf_counter() - t0) / 3
+            os.environ["OMP_NUM_THREADS"] = "1"
+            import subprocess
+            one = subprocess.run([sys.executable, "-c",
+                                  "import sys, time; sys.path.insert(0, %r)\n"
+                                  "import oracle; from workloads import crystals as C\n"
+                                  "b = C.config_batch(2, n_struct=512); t0 = time.perf_counter()\n"
+                                  "e = oracle.cutoff_graph(b.pos, b.lattice, b.struct_ptr, %f)['n_edges'] + "
+                                  "oracle.knn_graph(b.pos, b.lattice, b.struct_ptr, %d)['n_edges']\n"
+                                  "print(e / (time.perf_counter() - t0))" % (ROOT, R_C, K_NN)],
+                                 capture_output=True, text=True, env=dict(os.environ, OMP_NUM_THREADS="1"))
+            del os.environ["OMP_NUM_THREADS"]
+            if one.returncode == 0:
+                cpu["single_thread_edges_per_s"] = float(one.stdout.strip().splitlines()[-1])
+                cpu["single_thread_sample"] = "512-structure prefix of configs[2], cutoff + KNN, OMP_NUM_THREADS=1"
+        except Exception as ex:      # the extra timings are context; the headline baseline stands without them
+            cpu["extra_error"] = repr(ex)
 
     # ---- config 4: dynamic geometry, mg_update_graph KNN k=24 on 1024 skewed crystals, 100 steps of
     # a pre-generated trajectory resident on the device (per-step latency, BASELINE.json metric)
@@ -340,6 +394,99 @@ def run_gpu(args, rank, world, local_rank):
                "edges_per_s": float(k4 * b4.n_atoms / (lat_us.mean() * 1e-6))}
         graph.close()
 
+    # ---- pure-write bandwidth of this GPU, measured here: a fill of as many bytes as the cutoff call emits
+    # (the measured HBM peak is a COPY, read + write bytes; an edge list is written only)
+    write_only = None
+    if world == 1:
+        fb = [torch.empty(int(bytes_cut), dtype=torch.int8, device=dev) for _ in range(n_sets)]
+        for i in range(4):
+            fb[i % n_sets].fill_(1)
+        torch.cuda.synchronize()
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        f0.record()
+        for i in range(50):
+            fb[i % n_sets].fill_(1)
+        f1.record()
+        torch.cuda.synchronize()
+        fill_us = f0.elapsed_time(f1) * 1e3 / 50
+        write_only = {"bytes": int(bytes_cut), "fill_us": fill_us, "gbs": bytes_cut / fill_us / 1e3,
+                      "note": "torch.Tensor.fill_ of the cutoff call's algorithmic bytes, buffers rotating beyond L2"}
+        del fb
+
+    # ---- single-call latency: one call, one synchronisation (median / p99 over 200 calls each)
+    latency = None
+    if world == 1:
+        def call_latency(fn, n=200):
+            ts = []
+            for i in range(n):
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                fn(i)
+                torch.cuda.synchronize()
+                ts.append((time.perf_counter() - t0) * 1e6)
+            a = np.array(ts)
+            return {"median_us": float(np.median(a)), "p99_us": float(np.percentile(a, 99))}
+        latency = {"cutoff": call_latency(cutoff), "knn": call_latency(knn), "how": "host clock around call + cudaDeviceSynchronize"}
+
+    # ---- the other configs and calls (one leg each; events around `reps` back-to-back calls)
+    legs = {}
+    if world == 1 and not args.no_legs:
+        def timed(fn, reps=50, warm=3):
+            for i in range(warm):
+                fn(i)
+            torch.cuda.synchronize()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            for i in range(reps):
+                fn(i)
+            b.record()
+            torch.cuda.synchronize()
+            assert ctx.mg_check() == 0
+            return a.elapsed_time(b) * 1e3 / reps
+
+        # BASELINE configs[3]: cutoff 8 A on 16 supercells of 500-2000 atoms
+        b3 = C.config_batch(3)
+        p3, l3, s3 = mg.to_device(b3, dev)
+        e3 = ctx.mg_cutoff_count(p3, l3, s3, 8.0)
+        o3 = [mg.Edges.allocate(b3.n_atoms, e3, dev) for _ in range(2)]
+        us3 = timed(lambda i: ctx.mg_cutoff_graph(p3, l3, s3, 8.0, o3[i % 2]), reps=20)
+        n3 = np.diff(b3.struct_ptr).astype(np.float64)
+        bytes3 = BYTES_PER_EDGE * e3 + 4 * (b3.n_atoms + 1) + 12 * b3.n_atoms + 40 * b3.n_struct
+        roof3 = max(float(np.sum(n3 * n3)) * INSTR_PER_CANDIDATE / fp32_rate * 1e6, bytes3 / (hbm_gbs * 1e9) * 1e6)
+        legs["config3_cutoff"] = {"workload": f"BASELINE configs[3]: cutoff 8 A, {b3.n_struct} supercells, {b3.n_atoms} atoms",
+                                  "us_per_call": us3, "edges": int(e3), "edges_per_s": e3 / (us3 * 1e-6),
+                                  "candidates_min_image": float(np.sum(n3 * n3)), "roof_us": roof3, "frac": roof3 / us3}
+        del o3
+
+        # the shape of the paper's Table 1: batch of 256 cells of up to 64 atoms
+        bp = C.paper_scale_batch(256)
+        pp, lp, sp_ = mg.to_device(bp, dev)
+        tab = {}
+        for k in (16, 32, 64):
+            ok_ = mg.Edges.allocate(bp.n_atoms, k * bp.n_atoms, dev, dist=True)
+            tab[f"knn{k}_ms_per_batch"] = timed(lambda i: ctx.mg_knn_graph(pp, lp, sp_, k, ok_), reps=30) * 1e-3
+        for rc in (3.0, 5.0, 8.0):
+            ec = ctx.mg_cutoff_count(pp, lp, sp_, rc)
+            oc = mg.Edges.allocate(bp.n_atoms, ec, dev)
+            tab[f"cutoff{rc:g}_ms_per_batch"] = timed(lambda i: ctx.mg_cutoff_graph(pp, lp, sp_, rc, oc), reps=30) * 1e-3
+        legs["paper_scale_batch256"] = dict(tab, workload=f"256 synthetic cells of 1-64 atoms ({bp.n_atoms} atoms), the shape of the paper's "
+                                            "Table 1 batch row (PAPER.md:138: 53 / 55 / 80 ms KNN, 43 / 72 / 123 ms cutoff on an RTX 8000, "
+                                            "Materials Project data: context, another machine and other data)")
+
+        # SURVEY 8(f) NEXT-1 / NEXT-2 on the headline KNN graph: symmetric graph, triplets
+        kn = knn_sets[0]
+        sym = mg.Edges.allocate(n_atoms, 2 * e_knn, dev, dist=True)
+        us_sym = timed(lambda i: ctx.mg_symmetrize(kn, n_atoms, sym), reps=30)
+        n_tri = K_NN * (K_NN - 1) * n_atoms
+        us_tri = timed(lambda i: ctx.mg_triplets_graph(kn.row_ptr, n_atoms, n_tri), reps=10)
+        legs["symmetrize_knn12"] = {"us_per_call": us_sym, "edges_in": int(e_knn), "edges_out": int(sym.n_edges.item())}
+        legs["triplets_knn12"] = {"us_per_call": us_tri, "triplets": int(n_tri), "gbs_written": 8.0 * n_tri / us_tri / 1e3}
+        # per-atom cutoffs drawn in [2, 6.5] A on the headline batch
+        rad = torch.from_numpy(np.random.default_rng(0).uniform(2.0, 6.5, n_atoms).astype(np.float32)).to(dev)
+        orad = mg.Edges.allocate(n_atoms, e_cut, dev)
+        us_rad = timed(lambda i: ctx.mg_cutoff_graph_radii(pos, lat, ptr, rad, orad), reps=30)
+        legs["cutoff_radii"] = {"us_per_call": us_rad, "edges": int(orad.n_edges.item())}
+
     line = {
         "metric": "edges_per_s", "value": edges_all * K / (total_ms * 1e-3), "unit": "edges/s",
         "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / K,
@@ -352,15 +499,16 @@ def run_gpu(args, rank, world, local_rank):
                          f"> 126 MB L2); inputs are {12 * n_atoms + 40 * S} B"},
         "structures_per_s": structs_all * K / (total_ms * 1e-3),
         "call_us": {"cutoff": cut_ms * 1e3, "knn": knn_ms * 1e3},
-        "kernel_us": {"mg_cut_prep_kernel": prep_us, "mg_cutoff_count_kernel": count_us,
-                      "mg_cutoff_emit_kernel": emit_us, "mg_knn_pairs_kernel": knnk_us},
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm_gbs, "unit": "GB/s",
-                     "frac": achieved / hbm_gbs, "traffic": traffic, "kernel": "mg_cutoff_emit_kernel",
-                     "peak_kind": peak_kind, "algorithmic_bytes": bytes_cut},
+        "kernel_us": kernel_us,
+        "roofline": roofline,
+        "roofline_kernels": roofline_kernels,
         "roofline_model": {"cutoff": dict(t_cut, candidates=c_cut, roof_us=roof_cut, frac=roof_cut / (cut_ms * 1e3)),
                            "knn": dict(t_knn, candidates=c_knn, roof_us=roof_knn, frac=roof_knn / (knn_ms * 1e3)),
                            "fp32_peak_lane_instr_per_s": fp32_rate,
-                           "step_frac": (roof_cut + roof_knn) / (total_ms / K * 1e3)},
+                           "step_frac": (roof_cut + roof_knn) / (total_ms / K * 1e3),
+                           "edge_only_floor_us": {"cutoff": e_cut * INSTR_PER_CANDIDATE / fp32_rate * 1e6,
+                                                  "knn": e_knn * INSTR_PER_CANDIDATE / fp32_rate * 1e6},
+                           "write_only": write_only},
         "e2e": {"value": (e_cut + e_knn) / e2e_s, "unit": "edges/s", "h2d_bytes_per_step": in_bytes,
                 "d2h_bytes_per_step": out_bytes, "ms_per_step": e2e_s * 1e3, "steps": e2e_steps},
         "gpu_launches": int(launches),
@@ -368,6 +516,10 @@ def run_gpu(args, rank, world, local_rank):
     }
     if upd is not None:
         line["update_graph"] = upd
+    if latency is not None:
+        line["latency"] = latency
+    if legs:
+        line["legs"] = legs
     if cpu is not None:
         line["cpu_baseline"] = cpu
     print(json.dumps(line))
@@ -383,6 +535,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-update", action="store_true", help="skip the configs[4] mg_update_graph latency leg")
+    ap.add_argument("--no-legs", action="store_true", help="skip the configs[3] / paper-scale / graph-operation legs")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

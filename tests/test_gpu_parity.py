@@ -296,3 +296,26 @@ def test_knn_k_sweep(mg, ctx, k):
     got, status = _knn(mg, ctx, b, k)
     assert status == 0
     check.check_knn(b, k, got)
+
+
+# ------------------------------------------------------------------ paper-scale workloads
+@pytest.fixture(scope="module")
+def batch_paper():
+    return C.paper_scale_batch(256)          # cells of up to 64 atoms, the paper's batch size
+
+
+@pytest.mark.parametrize("k", [16, 32, 64])
+def test_paper_scale_knn(mg, ctx, batch_paper, k):
+    # the columns of the paper's Table 1: KNN 16 / 32 / 64
+    got, status = _knn(mg, ctx, batch_paper, k)
+    assert status == 0
+    rep = check.check_knn(batch_paper, k, got)
+    assert rep["exact_rows"] >= 0.995 * batch_paper.n_atoms, rep
+
+
+@pytest.mark.parametrize("rc", [3.0, 5.0, 8.0])
+def test_paper_scale_cutoff(mg, ctx, batch_paper, rc):
+    got, status = _cutoff(mg, ctx, batch_paper, rc)
+    assert status == 0
+    rep = check.check_cutoff(batch_paper, rc, got)
+    assert rep["extra"] == 0 and rep["missing"] == 0, rep

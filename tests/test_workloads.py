@@ -79,3 +79,13 @@ def test_config_table():
     assert C.config_batch(1, n_struct=16).n_struct == 16
     assert C.CONFIGS[2]["n_struct"] == 4096 and C.CONFIGS[2]["r_c"] == 6.0 and C.CONFIGS[2]["k"] == 12
     assert C.CONFIGS[4]["k"] == 24 and C.CONFIGS[4]["n_steps"] == 100
+
+
+def test_paper_scale_family():
+    b = C.paper_scale_batch(64, seed=1)
+    n = np.diff(b.struct_ptr)
+    assert n.min() >= 1 and n.max() <= 64 and n.max() > 20
+    b2 = C.paper_scale_batch(32, seed=1)                      # smaller batches are prefixes
+    assert np.array_equal(b2.pos, b.pos[:b2.n_atoms]) and np.array_equal(b2.lattice, b.lattice[:32])
+    vol = np.abs(np.linalg.det(b.lattice.astype(np.float64)))
+    assert 8.0 < np.median(vol / n) < 60.0                    # tens of cubic Angstrom per atom

@@ -26,6 +26,7 @@ FAMILY_SMALL = 0      # BASELINE.json configs[0..2]
 FAMILY_SUPERCELL = 1  # configs[3]
 FAMILY_SKEWED = 2     # configs[4] initial states
 FAMILY_WALK = 3       # configs[4] per-step noise streams
+FAMILY_PAPER = 4      # cells of up to 64 atoms, the shape of the paper's own workload
 
 
 @dataclasses.dataclass
@@ -181,6 +182,20 @@ def supercell(seed: int, index: int, density=0.08, n_lo=500, n_hi=2000, dmin=1.2
             return cell32, x
 
 
+def paper_scale_crystal(seed: int, index: int, n_hi=64, vol_per_atom=18.0, dmin=1.0):
+    """One crystal shaped like the paper's workload (Materials Project structures of at
+    most 64 atoms; NOT a record of that dataset): N ~ U{1..n_hi}, cell lengths (0.8 .. 1.5) x the cube root
+    of vol_per_atom * N (>= 3 A), angles U(60, 120) degrees, 1.0 A periodic minimum distance."""
+    rng = _rng(seed, FAMILY_PAPER, index)
+    n = int(rng.integers(1, n_hi + 1))
+    side = float(np.cbrt(vol_per_atom * n))
+    while True:
+        cell32 = _draw_cell(rng, max(3.0, 0.8 * side), max(3.6, 1.5 * side), 60.0, 120.0)
+        x = _place_atoms(rng, n, cell32, dmin)
+        if x is not None:
+            return cell32, x
+
+
 def _assemble(items) -> Batch:
     cells = np.stack([c for c, _ in items]).astype(np.float32)
     counts = np.array([x.shape[0] for _, x in items], dtype=np.int64)
@@ -193,6 +208,12 @@ def _assemble(items) -> Batch:
 
 def small_batch(n_struct: int, seed: int = 0) -> Batch:
     return _assemble([small_crystal(seed, s) for s in range(n_struct)])
+
+
+def paper_scale_batch(n_struct: int, seed: int = 0) -> Batch:
+    """batches of up to 64-atom cells for k = 16 / 32 / 64 and cutoffs 3 / 5 / 8 A
+    (the columns of the paper's Tables 1-2)."""
+    return _assemble([paper_scale_crystal(seed, s) for s in range(n_struct)])
 
 
 def supercell_batch(n_struct: int, seed: int = 0) -> Batch:
