@@ -80,16 +80,21 @@ typedef struct {
  * Environment read by mg_create (diagnostics only; results do not depend on them):
  *   MATGRAPH_NO_PDL      launch the kernels without programmatic dependent launch;
  *   MATGRAPH_MASK_WORDS  words (0..4096) of the per-warp hit-mask scratch the cutoff count launch
- *                        may use; beyond it the emit launch evaluates the masks again (tests);
+ *                        may use (chunks of the code pool of the one-launch path); beyond it the masks are
+ *                        evaluated / the rows listed a second time (tests);
+ *   MATGRAPH_FUSED, MATGRAPH_LEGACY  force the one-launch / the two-launch cutoff kernels for every batch;
  *   MG_DEBUG             print the CUDA error behind an MG_ERR_CUDA to stderr. */
 mg_status mg_create(mg_ctx **ctx, int device);
 void      mg_destroy(mg_ctx *ctx);
 mg_status mg_reserve(mg_ctx *ctx, int32_t n_struct, int32_t n_atoms);
 
-/* Cutoff graph, Def. 3 with constant c_i = r_c, strict '<'.  One stream-ordered pass:
- * per-structure search bounds n_a = ceil(r_c / h_a) with h_a = V / |a_b x a_c|, image enumeration,
- * FP32 distance filter (FP64 re-evaluation inside the rounding window so that the edge SET equals
- * the FP64 definition), count -> device-wide scan -> emit fused in one kernel. */
+/* Cutoff graph, Def. 3 with constant c_i = r_c, strict '<'.  Stream-ordered, no host
+ * synchronisation: a search-bounds launch (per structure n_a = ceil(r_c / h_a), h_a = V / |a_b x a_c|, the
+ * per-pair sub-box inside that box, a cost prefix that cuts the batch into equal ranges), then image
+ * enumeration with an FP32 distance filter (FP64 decision inside the rounding window, so that the edge SET
+ * is Def. 3's in FP64) and K4's count -> device-wide scan -> emit, as one of two kernel sets chosen per
+ * call: a count launch + an emit launch (batches of small cells), or one cooperative launch that finds,
+ * scans across its resident CTAs and writes (batches of large structures; also mg_cutoff_graph_radii). */
 mg_status mg_cutoff_graph(mg_ctx *ctx, const float *pos, const float *lattice,
                           const int32_t *struct_ptr, int32_t n_struct, int32_t n_atoms,
                           float r_c, const mg_edges *out, void *cuda_stream);

@@ -50,8 +50,7 @@ def _lib():
     """Load (building first if needed) libmatgraph.so; fails loudly when it cannot be had."""
     global _LIBH
     if _LIBH is None:
-        # MATGRAPH_LIB: load a prebuilt libmatgraph.so instead of building the in-tree one
-        path = os.environ.get("MATGRAPH_LIB") or build()
+        path = build()
         lib = ctypes.CDLL(path)
         vp, i32, i64, f32 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_float
         ep = ctypes.POINTER(_Edges)

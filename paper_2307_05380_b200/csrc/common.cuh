@@ -10,10 +10,6 @@
 #define MG_PAIR_TL 320             // cells of the per-warp translation table of the fused cutoff kernel
 #define MG_BLOCK 128               // threads per CTA of the graph kernels
 #define MG_WARPS (MG_BLOCK / 32)
-#define MG_TASK_BUDGET 6144u        // candidates per cutoff task (one warp, one row group)
-#define MG_TASK_ROWS 32             // rows per task: one lane per row in the scan / look-back
-#define MG_WT 256                   // per-warp translation-table tile (cells)
-#define MG_WS 768                   // per-warp stash entries (x2: double buffered)
 
 // device status word bits (first error wins when decoded by mg_check)
 #define MGS_SINGULAR   1u
@@ -22,25 +18,17 @@
 #define MGS_CAPACITY   8u
 #define MGS_UNSUPPORTED 16u
 
-// decoupled look-back descriptor: [63:62] flag, [61:32] epoch (30 bit), [31:0] value
-#define MG_FLAG_AGG  1ull
-#define MG_FLAG_PFX  2ull
-
-// Per-structure record written by mg_prep_kernel (K1: search bounds) and read by the graph kernels.
+// Per-structure record written by mg_prep_kernel (plane spacings, coordinate extents) and read by the
+// warp-per-atom KNN kernel (knn_small.cuh).
 struct StructRec {
-    int n[3];           // cutoff box half widths: every edge has |tau_a| <= n[a]
-    int ncell;          // (2n0+1)(2n1+1)(2n2+1); 0 if the structure is invalid / emits nothing
-    float lo2, hi2;     // FP32 filter window: d2 < lo2 surely inside, d2 >= hi2 surely outside
     float volume;
     unsigned err;       // MGS_* bits
-    int rpt;            // cutoff: source rows per task
-    int cap;            // cutoff: stash entries reserved per row
     float h_dn[3];      // plane spacings rounded down  (KNN bounds)
     float invh_up[3];   // 1 / h rounded up
     float xmin[3], xmax[3];
     float amax[3];      // max |component| of each lattice row (rounding-window bound)
     int first, natoms;
-    int pad[5];
+    int pad[13];
 };
 static_assert(sizeof(StructRec) == 128, "StructRec is two 64-byte lines");
 
@@ -146,7 +134,3 @@ __device__ __forceinline__ void mg_st_release(unsigned long long *p, unsigned lo
     asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
-__device__ __forceinline__ unsigned long long mg_desc(unsigned long long flag, unsigned epoch,
-                                                      unsigned value) {
-    return (flag << 62) | ((unsigned long long)(epoch & 0x3FFFFFFFu) << 32) | value;
-}

@@ -490,11 +490,15 @@ mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
     WarpSmem &sw = s_w[warp];
     // consecutive ranges (often parts of one expensive structure) go to different SMs
     const int wid = warp * gridDim.x + blockIdx.x;
+#ifdef MG_PHASE_CLOCKS
     const long long t_begin = clock64();
+#endif
     RangeCtx RC;
     mg_range_init(RC, A.rec, A.bpre, A.n_blocks, A.n_struct, A.n_ranges, lane);
     mg_count_ranges(sw, A, RC, wid, lane);
+#ifdef MG_PHASE_CLOCKS
     if (lane == 0) A.wclock[wid] = (unsigned)(clock64() - t_begin);
+#endif
     // The emit launch sums the totals of the ranges before its own itself (one coalesced pass per
     // warp, overlapped with the other warps' work): no tail in this launch.  mg_cutoff_count has no
     // emit launch: ---- last CTA out: exclusive scan of the warp totals, grand total
@@ -888,11 +892,15 @@ mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
     EmitSmem &se = reinterpret_cast<EmitSmem *>(smem_raw)[warp];
     // consecutive ranges (often parts of one expensive structure) go to different SMs
     const int wid = warp * gridDim.x + blockIdx.x;
+#ifdef MG_PHASE_CLOCKS
     const long long t_begin = clock64();
+#endif
     RangeCtx RC;
     mg_range_init(RC, A.rec, A.bpre, A.n_blocks, A.n_struct, A.n_ranges, lane);
     mg_emit_ranges(se, A, RC, wid, lane);
+#ifdef MG_PHASE_CLOCKS
     if (lane == 0) A.wclock[A.n_warps + wid] = (unsigned)(clock64() - t_begin);
+#endif
     // last CTA out zeroes the group totals for the next call
     __syncthreads();
     if (threadIdx.x == 0) {

@@ -24,7 +24,6 @@ struct mg_ctx {
     unsigned *d_ctl = nullptr;            // [0..1] cutoff ticket/done, [2..3] knn ticket/done, [4] status,
                                           // [5] knn prep blocks done, [6] number of cutoff tasks, [7] cut-prep block ticket, [8..9] cutoff emit ticket/done
     StructRec *d_rec = nullptr;           // per-structure records (prep.cuh)
-    unsigned *d_cost = nullptr;           // [n_struct+1] task prefix
     size_t rec_cap = 0;
     int32_t *d_atom_struct = nullptr;     // [n_atoms]
     size_t atom_cap = 0;
@@ -61,7 +60,6 @@ struct mg_ctx {
     int32_t *d_rowptr_tmp = nullptr;      // for mg_cutoff_count
     size_t rowptr_cap = 0;
     long long *d_count = nullptr;
-    unsigned epoch = 0;
     int cutoff_occ = 0, count_occ = 0, knn_occ[2] = {0, 0}, knnp_occ = 0;
     int64_t launches = 0;
     int pdl = 1;                          // programmatic dependent launch (MATGRAPH_NO_PDL=1 turns it off)
@@ -197,7 +195,6 @@ extern "C" void mg_destroy(mg_ctx *c) {
     cudaFree(c->d_crec);
     cudaFree(c->d_bpre);
     cudaFree(c->d_rec);
-    cudaFree(c->d_cost);
     cudaFree(c->d_atom_struct);
     cudaFree(c->d_rowptr_tmp);
     cudaFree(c->d_count);
@@ -219,10 +216,9 @@ extern "C" mg_status mg_reserve(mg_ctx *c, int32_t n_struct, int32_t n_atoms) {
     }
     if ((size_t)n_struct + 1 > c->rec_cap) {
         const size_t cap = (size_t)n_struct + 1025;
-        cudaFree(c->d_rec); cudaFree(c->d_cost);
-        c->d_rec = nullptr; c->d_cost = nullptr; c->rec_cap = 0;
+        cudaFree(c->d_rec);
+        c->d_rec = nullptr; c->rec_cap = 0;
         MG_CUDA(cudaMalloc(&c->d_rec, cap * sizeof(StructRec)));
-        MG_CUDA(cudaMalloc(&c->d_cost, cap * sizeof(unsigned)));
         c->rec_cap = cap;
     }
     if ((size_t)n_atoms + 1 > c->atom_cap) {
@@ -257,6 +253,7 @@ extern "C" mg_status mg_reserve(mg_ctx *c, int32_t n_struct, int32_t n_atoms) {
     return MG_OK;
 }
 
+#ifdef MG_PHASE_CLOCKS
 // Tuning aid (not part of the public header): per-warp cycles and range starts of the last cutoff call.
 extern "C" int mg_debug_cut_warps(mg_ctx *c, unsigned *clocks_host, int *starts_host, int max_warps) {
     if (!c) return -1;
@@ -283,6 +280,8 @@ extern "C" int mg_debug_cut_masks(mg_ctx *c, unsigned *host, int n_words) {
     cudaMemcpy(host, c->d_wmask, (size_t)n_words * 4, cudaMemcpyDeviceToHost);
     return 0;
 }
+
+#endif
 
 extern "C" int64_t mg_launch_count(const mg_ctx *c) { return c ? c->launches : 0; }
 
@@ -373,8 +372,7 @@ static mg_status launch_prep(mg_ctx *c, const float *pos, const float *lat, cons
                              int32_t n_struct, int32_t n_atoms, float r_c, cudaStream_t st) {
     PrepArgs P;
     P.pos = pos; P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms;
-    P.r_c = r_c; P.rec = c->d_rec; P.task_prefix = c->d_cost; P.atom_struct = c->d_atom_struct;
-    P.ctl = c->d_ctl; P.status = c->d_ctl + 4;
+    P.rec = c->d_rec; P.atom_struct = c->d_atom_struct; P.status = c->d_ctl + 4;
     mg_prep_kernel<<<(n_struct + MG_PREP_BLOCK / 32 - 1) / (MG_PREP_BLOCK / 32), MG_PREP_BLOCK, 0, st>>>(P);
     MG_CUDA(cudaGetLastError());
     c->launches += 1;

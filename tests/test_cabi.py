@@ -32,6 +32,12 @@ def test_library_builds_loads_and_exports_every_declared_symbol():
     for name in _declared():
         assert hasattr(lib, name), f"{name} declared in matgraph.h but not exported"
     assert sorted(m.EXPORTS) == _declared()
+    # ... and nothing else: the dynamic symbol table holds exactly the header's mg_* functions
+    nm = subprocess.run(["nm", "-D", "--defined-only", path], capture_output=True, text=True)
+    if nm.returncode == 0:
+        exported = sorted({line.split()[-1] for line in nm.stdout.splitlines()
+                           if len(line.split()) >= 3 and line.split()[-2] in "TW" and line.split()[-1].startswith("mg_")})
+        assert exported == _declared(), set(exported) ^ set(_declared())
     lib.mg_status_string.restype = ctypes.c_char_p
     assert lib.mg_status_string(0) == b"ok"
     assert b"capacity" in lib.mg_status_string(6)
