@@ -397,7 +397,7 @@ def run_gpu(args, rank, world, local_rank):
     # ---- pure-write bandwidth of this GPU, measured here: a fill of as many bytes as the cutoff call emits
     # (the measured HBM peak is a COPY, read + write bytes; an edge list is written only)
     write_only = None
-    if world == 1:
+    if world == 1 and not args.no_latency:
         fb = [torch.empty(int(bytes_cut), dtype=torch.int8, device=dev) for _ in range(n_sets)]
         for i in range(4):
             fb[i % n_sets].fill_(1)
@@ -415,7 +415,7 @@ def run_gpu(args, rank, world, local_rank):
 
     # ---- single-call latency: one call, one synchronisation (median / p99 over 200 calls each)
     latency = None
-    if world == 1:
+    if world == 1 and not args.no_latency:
         def call_latency(fn, n=200):
             ts = []
             for i in range(n):
@@ -535,6 +535,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-update", action="store_true", help="skip the configs[4] mg_update_graph latency leg")
+    ap.add_argument("--no-latency", action="store_true", help="skip the single-call latency and write-only bandwidth measurements")
     ap.add_argument("--no-legs", action="store_true", help="skip the configs[3] / paper-scale / graph-operation legs")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
