@@ -47,9 +47,23 @@ struct KnnSmem {
     WarpSmem w;                    // table, staged positions
     unsigned long long stash[MG_KSTASH];
     int rowoff[MG_SMALL_MAX_ATOMS + 1];
-    float xo[MG_SMALL_MAX_ATOMS][3];   // positions as given + lattice: operands of the exact FP64 distance
-    float lat[12];
+    double xd[MG_SMALL_MAX_ATOMS][3];  // positions as given + lattice, promoted once per structure: operands of the
+    double latd[9];                    // exact FP64 distance
 };
+
+// Exact squared distance of one image from the staged FP64 operands: f = (x_j - x_i) + tau, v = f . L, no FMA
+// contraction, sums left to right (R15: the oracle's operation order, so d2 is the oracle's d^2).
+__device__ __forceinline__ double mg_knn_exact_d2(const double *xi, const double *xj, int t0, int t1, int t2,
+                                                   const double *L, double v[3]) {
+    // (double)t without a conversion instruction: 2^52 + 2^31 + t has t + 2^31 in its low mantissa word
+    const double f0 = __dadd_rn(__dsub_rn(xj[0], xi[0]), __hiloint2double(0x43300000, t0 ^ 0x80000000) - 4503601774854144.0);
+    const double f1 = __dadd_rn(__dsub_rn(xj[1], xi[1]), __hiloint2double(0x43300000, t1 ^ 0x80000000) - 4503601774854144.0);
+    const double f2 = __dadd_rn(__dsub_rn(xj[2], xi[2]), __hiloint2double(0x43300000, t2 ^ 0x80000000) - 4503601774854144.0);
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+        v[c] = __dadd_rn(__dadd_rn(__dmul_rn(f0, L[c]), __dmul_rn(f1, L[3 + c])), __dmul_rn(f2, L[6 + c]));
+    return __dadd_rn(__dadd_rn(__dmul_rn(v[0], v[0]), __dmul_rn(v[1], v[1])), __dmul_rn(v[2], v[2]));
+}
 
 // Growing-radius search of one source row with the routine of knn_small.cuh (rare path).  Uses the
 // table area of the warp's shared memory as scratch: the caller rebuilds the table afterwards.
@@ -224,8 +238,8 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                 for (int i = ia; i < ib; ++i) mg_knn_row_fallback(ks, A, s, k.first, N, i, lane);
             } else {
                 __syncwarp();
-                for (int j = lane; j < 3 * N; j += 32) (&ks.xo[0][0])[j] = A.pos[3 * (size_t)k.first + j];
-                if (lane < 9) ks.lat[lane] = F.lat[lane];
+                for (int j = lane; j < 3 * N; j += 32) (&ks.xd[0][0])[j] = (double)A.pos[3 * (size_t)k.first + j];
+                if (lane < 9) ks.latd[lane] = (double)F.lat[lane];
                 __syncwarp();
                 F.win = 0.f;                                   // no exact threshold decision here
                 // every image with true d2 < R^2 - win is a hit; a k-th key below R^2 - 2 win is safe
@@ -294,7 +308,7 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                                 const unsigned ord = ((unsigned)j << 24) | (tie >> 8);
                                 double dd = 1e300, vv[3] = {0.0, 0.0, 0.0};
                                 if (sel)
-                                    dd = mg_exact_vec(ks.xo[i], ks.xo[j], t0, t1, t2, ks.lat, vv);
+                                    dd = mg_knn_exact_d2(ks.xd[i], ks.xd[j], t0, t1, t2, ks.latd, vv);
                                 int rank = lane;
                                 {
                                     const double nd = __shfl_down_sync(0xFFFFFFFFu, dd, 1);
@@ -311,7 +325,7 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                                 }
                                 if (!sel) rank = 64;
                                 // Alg. 1 line 4: the k-th image must be safely inside the explored radius
-                                const bool settled = rank != K - 1 || dd * dd < lim2d;
+                                const bool settled = rank != K - 1 || dd < lim2d;
                                 if (__all_sync(0xFFFFFFFFu, settled)) {
                                     if (rank < K) {
                                         const long long e = (long long)K * gi + rank;
@@ -321,8 +335,8 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                                         A.offset[3 * e + 2] = (int8_t)t2;
                                         A.vec[3 * e] = (float)vv[0]; A.vec[3 * e + 1] = (float)vv[1];
                                         A.vec[3 * e + 2] = (float)vv[2];
-                                        if (A.dist) A.dist[e] = (float)dd;
-                                        if (rank == K - 1) dkmax = fmaxf(dkmax, __double2float_ru(dd));
+                                        if (A.dist) A.dist[e] = __fsqrt_rn((float)dd);
+                                        if (rank == K - 1) dkmax = fmaxf(dkmax, __fsqrt_ru(__double2float_ru(dd)));
                                     }
                                     continue;
                                 }
@@ -360,7 +374,7 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                         const int nsel = K + __popc(__ballot_sync(0xFFFFFFFFu, amb));
                         double dd = 1e300, vv[3] = {0.0, 0.0, 0.0};
                         if (lane < nsel)
-                            dd = mg_exact_vec(ks.xo[i], ks.xo[j], t0, t1, t2, ks.lat, vv);
+                            dd = mg_knn_exact_d2(ks.xd[i], ks.xd[j], t0, t1, t2, ks.latd, vv);
                         int rank = 0;
                         for (int l = 0; l < nsel; ++l) {
                             const double od = __shfl_sync(0xFFFFFFFFu, dd, l);
@@ -373,8 +387,8 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                             A.dst[e] = k.first + j;
                             A.offset[3 * e] = (int8_t)t0; A.offset[3 * e + 1] = (int8_t)t1; A.offset[3 * e + 2] = (int8_t)t2;
                             A.vec[3 * e] = (float)vv[0]; A.vec[3 * e + 1] = (float)vv[1]; A.vec[3 * e + 2] = (float)vv[2];
-                            if (A.dist) A.dist[e] = (float)dd;
-                            if (rank == K - 1) dkmax = fmaxf(dkmax, __double2float_ru(dd));
+                            if (A.dist) A.dist[e] = __fsqrt_rn((float)dd);
+                            if (rank == K - 1) dkmax = fmaxf(dkmax, __fsqrt_ru(__double2float_ru(dd)));
                         }
                     }
 #ifdef MG_PHASE_CLOCKS

@@ -238,7 +238,9 @@ __device__ inline void mg_knn_source(const KnnArgs &A, const StructRec &R, const
             const unsigned u0 = c / (D1f * D2f), rem = c - u0 * (D1f * D2f), u1 = rem / D2f;
             jj[s] = (int)j;
             tt[s][0] = (int)u0 - n[0]; tt[s][1] = (int)u1 - n[1]; tt[s][2] = (int)(rem - u1 * D2f) - n[2];
-            dd[s] = mg_exact_vec(xs + 3 * i, xs + 3 * jj[s], tt[s][0], tt[s][1], tt[s][2], lat9, vv[s]);
+            mg_exact_vec(xs + 3 * i, xs + 3 * jj[s], tt[s][0], tt[s][1], tt[s][2], lat9, vv[s]);
+            // ranked by the FP64 SQUARED distance (the pair-lane kernel does the same: no FP64 square root)
+            dd[s] = __dadd_rn(__dadd_rn(__dmul_rn(vv[s][0], vv[s][0]), __dmul_rn(vv[s][1], vv[s][1])), __dmul_rn(vv[s][2], vv[s][2]));
         }
     }
 #pragma unroll
@@ -268,14 +270,16 @@ __device__ inline void mg_knn_source(const KnnArgs &A, const StructRec &R, const
             A.vec[3 * e] = valid ? (float)vv[s][0] : 0.f;
             A.vec[3 * e + 1] = valid ? (float)vv[s][1] : 0.f;
             A.vec[3 * e + 2] = valid ? (float)vv[s][2] : 0.f;
-            if (A.dist) A.dist[e] = valid ? (float)dd[s] : 0.f;
+            // (dist = sqrt in FP32 of the FP64 squared distance, like the pair-lane kernel: a row gives the same bits
+            // whichever routine produced it)
+            if (A.dist) A.dist[e] = valid ? __fsqrt_rn((float)dd[s]) : 0.f;
             if (valid) dmax = fmax(dmax, dd[s]);
         }
     }
     if (A.radius_hint) {
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) dmax = fmax(dmax, __shfl_xor_sync(0xFFFFFFFFu, dmax, o));
-        if (lane == 0) A.radius_hint[gi] = __double2float_ru(dmax);
+        if (lane == 0) A.radius_hint[gi] = __fsqrt_ru(__double2float_ru(dmax));
     }
 }
 
