@@ -199,29 +199,32 @@ __device__ __forceinline__ void mg_pair_masks(const WarpSmem &sw, const FindCtx 
     const float nr2 = F.nr2, win = F.win;
     if (W == 1 && ncl == 1) {                     // one image per pair (cells wider than 2 r_c): T_0 = 0
         const float y = __fmaf_rn(qz, qz, __fmaf_rn(qy, qy, __fmaf_rn(qx, qx, nr2)));
-        mask[0] = y < win ? 1u : 0u;
+        mask[0] = y < 0.f ? 0x80000000u : 0u;
         near = fabsf(y) < win;
     } else
 #pragma unroll
     for (int w = 0; w < W; ++w) {
-        mask[w] = 0u;
-        const int n4 = min(8, max(0, (ncl - 32 * w + 3) >> 2));      // warp-uniform
+        // bit 31 - c <-> cell 32 w + c: the sign bits of y = |q' + T|^2 - r^2 are shifted in one by one, two
+        // groups of four cells per trip (a group past the word's cells holds sentinels)
+        unsigned m = 0u;
+        const int n4 = min(8, max(0, (ncl - 32 * w + 3) >> 2)), n4r = (n4 + 1) & ~1;      // warp-uniform
         const float4 *Xp = reinterpret_cast<const float4 *>(mg_tplane(sw, 0) + 32 * w);
         const float4 *Yp = reinterpret_cast<const float4 *>(mg_tplane(sw, 1) + 32 * w);
         const float4 *Zp = reinterpret_cast<const float4 *>(mg_tplane(sw, 2) + 32 * w);
 #pragma unroll 1                  // a loop, not 8 copies: the kernels are bound by instruction fetch
-        for (int g = 0; g < n4; ++g) {
-            unsigned sub = 0u;
-            float y[4];
+        for (int g = 0; g < n4r; g += 2) {
+            float y[8];
             mg_filter4(Xp[g], Yp[g], Zp[g], make_float2(qx, qx), make_float2(qy, qy), make_float2(qz, qz),
-                       make_float2(nr2, nr2), y);
+                       make_float2(nr2, nr2), *reinterpret_cast<float (*)[4]>(&y[0]));
+            mg_filter4(Xp[g + 1], Yp[g + 1], Zp[g + 1], make_float2(qx, qx), make_float2(qy, qy), make_float2(qz, qz),
+                       make_float2(nr2, nr2), *reinterpret_cast<float (*)[4]>(&y[4]));
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                if (y[c] < win) sub |= 1u << c;
+            for (int c = 0; c < 8; ++c) {
+                m = __funnelshift_l(__float_as_uint(y[c]), m, 1);
                 near = near || fabsf(y[c]) < win;
             }
-            mask[w] |= sub << (4 * g);
         }
+        mask[w] = n4r == 0 ? 0u : (n4r < 8 ? m << (32 - 4 * n4r) : m);
     }
     if (near) {                                   // rare: decide the window cells in FP64
         const float *xi = F.pos + 3 * (size_t)gi, *xj = F.pos + 3 * (size_t)gj;
@@ -234,7 +237,7 @@ __device__ __forceinline__ void mg_pair_masks(const WarpSmem &sw, const FindCtx 
                 double v[3];
                 const double d = mg_exact_vec(xi, xj, l0 + (int)(tc >> 24), l1 + (int)((tc >> 16) & 0xFFu),
                                               l2 + (int)((tc >> 8) & 0xFFu), F.lat, v);
-                const unsigned bit = 1u << (c & 31);
+                const unsigned bit = 0x80000000u >> (c & 31);
 #pragma unroll
                 for (int w = 0; w < W; ++w)
                     if (w == (c >> 5)) mask[w] = d < (double)F.rc ? (mask[w] | bit) : (mask[w] & ~bit);
@@ -284,7 +287,7 @@ __device__ __forceinline__ void mg_block_masks(const WarpSmem &sw, const FindCtx
     const int cs = p.self - tile0;
 #pragma unroll
     for (int w = 0; w < W; ++w)
-        if (p.self >= 0 && cs >= 32 * w && cs < 32 * w + 32) mask[w] &= ~(1u << (cs & 31));
+        if (p.self >= 0 && cs >= 32 * w && cs < 32 * w + 32) mask[w] &= ~(0x80000000u >> (cs & 31));
 }
 
 // The same for ONE word of the mask — cells [32 w, 32 w + 32) of the table tile that starts at cell
@@ -301,23 +304,25 @@ __device__ __forceinline__ unsigned mg_word_mask(const WarpSmem &sw, const FindC
     bool near = false;
     if (ncl == 1 && tile0 == 0) {                                // one image per pair: T_0 = 0
         const float y = __fmaf_rn(p.qz, p.qz, __fmaf_rn(p.qy, p.qy, __fmaf_rn(p.qx, p.qx, nr2)));
-        mask = y < win ? 1u : 0u;
+        mask = y < 0.f ? 0x80000000u : 0u;
         near = fabsf(y) < win;
     } else {
-        const int n4 = (nw + 3) >> 2;
+        // bit 31 - c <-> cell c of the word: sign bits shifted in, two groups of four cells per trip
+        const int n4r = (((nw + 3) >> 2) + 1) & ~1;
 #pragma unroll 1
-        for (int g = 0; g < n4; ++g) {
-            unsigned sub = 0u;
-            float y[4];
+        for (int g = 0; g < n4r; g += 2) {
+            float y[8];
             mg_filter4(Xp[g], Yp[g], Zp[g], make_float2(p.qx, p.qx), make_float2(p.qy, p.qy),
-                       make_float2(p.qz, p.qz), make_float2(nr2, nr2), y);
+                       make_float2(p.qz, p.qz), make_float2(nr2, nr2), *reinterpret_cast<float (*)[4]>(&y[0]));
+            mg_filter4(Xp[g + 1], Yp[g + 1], Zp[g + 1], make_float2(p.qx, p.qx), make_float2(p.qy, p.qy),
+                       make_float2(p.qz, p.qz), make_float2(nr2, nr2), *reinterpret_cast<float (*)[4]>(&y[4]));
 #pragma unroll
-            for (int c = 0; c < 4; ++c) {
-                if (y[c] < win) sub |= 1u << c;
+            for (int c = 0; c < 8; ++c) {
+                mask = __funnelshift_l(__float_as_uint(y[c]), mask, 1);
                 near = near || fabsf(y[c]) < win;
             }
-            mask |= sub << (4 * g);
         }
+        mask = n4r < 8 ? mask << (32 - 4 * n4r) : mask;
     }
     if (near) {                                   // rare: decide the window cells in FP64
         const float *xi = F.pos + 3 * (size_t)gi, *xj = F.pos + 3 * (size_t)gj;
@@ -330,12 +335,12 @@ __device__ __forceinline__ unsigned mg_word_mask(const WarpSmem &sw, const FindC
                 double v[3];
                 const double d = mg_exact_vec(xi, xj, p.l0 + (int)(tc >> 24), p.l1 + (int)((tc >> 16) & 0xFFu),
                                               p.l2 + (int)((tc >> 8) & 0xFFu), F.lat, v);
-                mask = d < (double)F.rc ? (mask | (1u << c)) : (mask & ~(1u << c));
+                mask = d < (double)F.rc ? (mask | (0x80000000u >> c)) : (mask & ~(0x80000000u >> c));
             }
         }
     }
     const int cs = p.self - tile0 - 32 * w;       // (i, i, 0) is not an edge
-    if (p.self >= 0 && cs >= 0 && cs < 32) mask &= ~(1u << cs);
+    if (p.self >= 0 && cs >= 0 && cs < 32) mask &= ~(0x80000000u >> cs);
     return mask;
 }
 
@@ -422,7 +427,7 @@ __device__ __forceinline__ unsigned mg_single_word(const WarpSmem &sw, const Cut
     const PairLane p = mg_pair_setup(sw, F, valid, i, j);
     if (report && valid && !p.ok) atomicOr(A.status, MGS_OFFSET);
     const unsigned m = mg_word_mask(sw, F, p, k.first + i, k.first + j, 0, 0, 1);
-    return __ballot_sync(0xFFFFFFFFu, (m & 1u) != 0u);
+    return __ballot_sync(0xFFFFFFFFu, (m >> 31) != 0u);
 }
 
 // (its own structure setup: no table, no FP64 positions in the count launch)
@@ -711,8 +716,8 @@ __device__ __forceinline__ void mg_emit_struct(EmitSmem &se, const CutoffArgs &A
                         if (w >= nW) break;
                         unsigned mk = mine ? mask[w] : 0u;
                         while (mk) {
-                            const int b = __ffs(mk) - 1;
-                            mk &= mk - 1;
+                            const int b = __clz(mk);
+                            mk &= ~(0x80000000u >> b);
                             se.stash[pos++] = paircode + sw.tcode[32 * w + b];
                         }
                     }

@@ -161,8 +161,8 @@ __device__ __forceinline__ int mg_knn_find(KnnSmem &ks, const Task &k, const Fin
         for (int w = 0; w < W; ++w) {
             unsigned mk = mask[w];
             while (mk) {
-                const int b = __ffs(mk) - 1;
-                mk &= mk - 1;
+                const int b = __clz(mk);
+                mk &= ~(0x80000000u >> b);
                 const float4 T = mg_tcell(sw, 32 * w + b);
                 const float vx = __fadd_rn(p.qx, T.x), vy = __fadd_rn(p.qy, T.y), vz = __fadd_rn(p.qz, T.z);
                 const float d2 = __fmaf_rn(vz, vz, __fmaf_rn(vy, vy, __fmul_rn(vx, vx)));
