@@ -16,6 +16,7 @@
 // Exclusive scan of v(r), r in [0, n), by ONE block of MGO_SCAN_BLOCK threads (chunks of the array in
 // turn; n is the number of atoms of a batch: tens of thousands).  out[r] = base(r) + sum_{q < r} v(q),
 // out[n] = base(n) + total; *total_out = out[n].
+#define MGO_SCAN_ITEMS 8
 template <class V, class B>
 __device__ __forceinline__ void mgo_block_scan(int n, V value, B base, long long *out64, int32_t *out32,
                                                long long *total_out) {
@@ -24,10 +25,16 @@ __device__ __forceinline__ void mgo_block_scan(int n, V value, B base, long long
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) s_carry = 0ll;
     __syncthreads();
-    for (int r0 = 0; r0 < n; r0 += MGO_SCAN_BLOCK) {
-        const int r = r0 + tid;
-        const long long v = r < n ? value(r) : 0ll;
-        long long incl = v;
+    // chunks of MGO_SCAN_BLOCK * MGO_SCAN_ITEMS values: a thread owns MGO_SCAN_ITEMS consecutive ones
+    for (int r0 = 0; r0 < n; r0 += MGO_SCAN_BLOCK * MGO_SCAN_ITEMS) {
+        const int rb = r0 + tid * MGO_SCAN_ITEMS;
+        long long v[MGO_SCAN_ITEMS], own = 0ll;
+#pragma unroll
+        for (int x = 0; x < MGO_SCAN_ITEMS; ++x) {
+            v[x] = rb + x < n ? value(rb + x) : 0ll;
+            own += v[x];
+        }
+        long long incl = own;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             const long long t = __shfl_up_sync(0xFFFFFFFFu, incl, o);
@@ -41,10 +48,15 @@ __device__ __forceinline__ void mgo_block_scan(int n, V value, B base, long long
             if (w < warp) woff += t;
             btotal += t;
         }
-        const long long excl = s_carry + woff + incl - v;
-        if (r < n) {
-            if (out64) out64[r] = base(r) + excl;
-            if (out32) out32[r] = (int32_t)(base(r) + excl);
+        long long excl = s_carry + woff + incl - own;
+#pragma unroll
+        for (int x = 0; x < MGO_SCAN_ITEMS; ++x) {
+            const int r = rb + x;
+            if (r < n) {
+                if (out64) out64[r] = base(r) + excl;
+                if (out32) out32[r] = (int32_t)(base(r) + excl);
+            }
+            excl += v[x];
         }
         __syncthreads();
         if (tid == 0) s_carry += btotal;
@@ -178,12 +190,23 @@ mg_trip_emit_kernel(const TripArgs A) {
         if (d < 2) continue;
         const long long nt = d * (d - 1), base = A.tri_ptr[r];
         const int dm = (int)(d - 1);
-        for (long long t = lane; t < nt; t += 32) {
-            const int a = (int)(t / dm), bq = (int)(t - (long long)a * dm), b = bq + (bq >= a ? 1 : 0);
-            if (base + t < A.capacity) {
-                A.edge_a[base + t] = e0 + a;
-                A.edge_b[base + t] = e0 + b;
+        if (nt < (1ll << 20)) {                        // t / dm through the float reciprocal (exact below 2^20)
+            const float inv = 1.f / (float)dm;
+            int32_t *pa = A.edge_a + base, *pb = A.edge_b + base;
+            const long long room = A.capacity - base;
+            const int lim = room >= nt ? (int)nt : (room > 0 ? (int)room : 0);
+            for (int t = lane; t < lim; t += 32) {
+                const int a = __float2int_rz(__fmul_rn((float)t + 0.5f, inv)), bq = t - a * dm;
+                pa[t] = e0 + a;
+                pb[t] = e0 + bq + (bq >= a ? 1 : 0);
             }
-        }
+        } else
+            for (long long t = lane; t < nt; t += 32) {
+                const int a = (int)(t / dm), bq = (int)(t - (long long)a * dm), b = bq + (bq >= a ? 1 : 0);
+                if (base + t < A.capacity) {
+                    A.edge_a[base + t] = e0 + a;
+                    A.edge_b[base + t] = e0 + b;
+                }
+            }
     }
 }
