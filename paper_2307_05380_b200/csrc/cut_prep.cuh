@@ -20,7 +20,9 @@
 #include "common.cuh"
 
 #define MG_CP_BLOCK 128
+#ifndef MG_STASH
 #define MG_STASH 1024              // stash entries per warp of the emit kernel (cutoff_pairs.cuh)
+#endif
 #ifndef MG_KNN_ALPHA
 #define MG_KNN_ALPHA 1.45f         // KNN: expected images inside the first search radius, in units of k
 #define MG_KNN_RSCALE 1.05f        // ... and the safety factor on that radius

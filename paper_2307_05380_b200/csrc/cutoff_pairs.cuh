@@ -485,7 +485,10 @@ __device__ __forceinline__ void mg_count_ranges(WarpSmem &sw, const CutoffArgs &
     }
 }
 
-__global__ void __launch_bounds__(MG_BLOCK, 4)
+#ifndef MG_CUT_CTAS
+#define MG_CUT_CTAS 4
+#endif
+__global__ void __launch_bounds__(MG_BLOCK, MG_CUT_CTAS)
 mg_cutoff_count_kernel(const __grid_constant__ CutoffArgs A) {
     mg_grid_dependency_wait();
     __shared__ WarpSmem s_w[MG_WARPS];
@@ -889,7 +892,7 @@ __device__ __forceinline__ void mg_emit_ranges(EmitSmem &se, const CutoffArgs &A
     }
 }
 
-__global__ void __launch_bounds__(MG_BLOCK, 4)
+__global__ void __launch_bounds__(MG_BLOCK, MG_CUT_CTAS)
 mg_cutoff_emit_kernel(const __grid_constant__ CutoffArgs A) {
     mg_grid_dependency_wait();
     extern __shared__ __align__(16) unsigned char smem_raw[];

@@ -250,3 +250,73 @@ def test_repeated_calls_are_deterministic_sets(mg, ctx):
     ka = check._keys(a["src"], a["dst"], a["offset"])
     kc = check._keys(c["src"], c["dst"], c["offset"])
     assert np.array_equal(np.sort(ka), np.sort(kc))
+
+
+# ------------------------------------------------------------------ the one-launch scan kernel on every kind of batch
+# mg_cutoff_graph picks its kernels per call (cut_scan.cuh for batches of large structures, the count +
+# emit pair otherwise); MATGRAPH_FUSED=1 sends every batch through the scan kernel.
+@pytest.fixture()
+def scan_ctx(mg, monkeypatch):
+    monkeypatch.setenv("MATGRAPH_FUSED", "1")
+    c = mg.Context(0)
+    yield c
+    c.close()
+
+
+def test_scan_kernel_small_cells_and_mixed_batches(mg, scan_ctx):
+    small = C.small_batch(40, seed=8)
+    rng = np.random.default_rng(3)
+    cell = (np.diag([9.0, 10.0, 11.0]) + rng.uniform(-1, 1, (3, 3))).astype(np.float32)
+    big = C.Batch(pos=rng.random((150, 3), dtype=np.float32), lattice=cell[None], struct_ptr=np.array([0, 150], np.int32))
+    empty = C.Batch(pos=np.zeros((0, 3), np.float32), lattice=np.eye(3, dtype=np.float32)[None], struct_ptr=np.array([0, 0], np.int32))
+    for b, rc in ((C.config_batch(0), 5.0), (C.concat([small, empty, big, small]), 6.5), (C.config_batch(2, n_struct=300), 6.0)):
+        pos, lat, ptr = mg.to_device(b)
+        got = scan_ctx.cutoff_graph(pos, lat, ptr, rc, dist=True).to_numpy()
+        assert scan_ctx.mg_check() == 0
+        rep = check.check_cutoff(b, rc, got)
+        assert rep["extra"] == 0 and rep["missing"] == 0, rep
+
+
+def test_scan_kernel_pool_exhausted_and_dense_rows(mg, monkeypatch):
+    # a pool of a few chunks (test knob): warps whose codes do not fit list their rows a second time and write edge
+    # by edge; dense cells: blocks with more hits than the stash holds go in passes of consecutive lanes
+    monkeypatch.setenv("MATGRAPH_FUSED", "1")
+    items = []
+    for s in range(4):
+        rng = np.random.default_rng(200 + s)
+        n = int(rng.integers(3, 21))
+        cell = np.diag(rng.uniform(3.0, 4.0, 3)).astype(np.float32)
+        cell[1, 0] = np.float32(rng.uniform(-1, 1))
+        items.append((cell, rng.random((n, 3), dtype=np.float32)))
+    dense = C._assemble(items)
+    b = C.concat([C.small_batch(30, seed=6), dense])
+    ref = None
+    for words in ("0", "3", "40", "4096"):
+        monkeypatch.setenv("MATGRAPH_MASK_WORDS", words)
+        c = mg.Context(0)
+        try:
+            pos, lat, ptr = mg.to_device(b)
+            got = c.cutoff_graph(pos, lat, ptr, 7.0, dist=True).to_numpy()
+            assert c.mg_check() == 0
+            rep = check.check_cutoff(b, 7.0, got)
+            assert rep["extra"] == 0 and rep["missing"] == 0, (words, rep)
+            key = (got["n_edges"], got["row_ptr"].tobytes())
+            ref = ref or key
+            assert key == ref
+        finally:
+            c.close()
+
+
+def test_scan_kernel_capacity_and_count(mg, scan_ctx):
+    b = C.small_batch(16, seed=2)
+    pos, lat, ptr = mg.to_device(b)
+    need = scan_ctx.mg_cutoff_count(pos, lat, ptr, 5.0)
+    full = scan_ctx.cutoff_graph(pos, lat, ptr, 5.0, capacity=need).to_numpy()
+    assert scan_ctx.mg_check() == 0 and full["n_edges"] == need
+    got = scan_ctx.cutoff_graph(pos, lat, ptr, 5.0, capacity=need // 2 + 1).to_numpy()
+    assert scan_ctx.mg_check() == 6 and got["n_edges"] == need
+    assert np.array_equal(got["row_ptr"], full["row_ptr"])
+    m = need // 2 + 1
+    assert np.array_equal(got["src"], full["src"][:m])
+    kg = check._keys(got["src"], got["dst"], got["offset"])
+    assert set(kg.tolist()) <= set(check._keys(full["src"], full["dst"], full["offset"]).tolist())
