@@ -319,3 +319,15 @@ def test_paper_scale_cutoff(mg, ctx, batch_paper, rc):
     assert status == 0
     rep = check.check_cutoff(batch_paper, rc, got)
     assert rep["extra"] == 0 and rep["missing"] == 0, rep
+
+
+@pytest.mark.parametrize("name,k", [("fcc_conv", 24), ("fcc_prim", 24), ("bcc_conv", 20), ("diamond", 10), ("hcp", 15), ("rocksalt", 30)])
+def test_knn_inside_a_degenerate_shell(mg, ctx, name, k):
+    # k ends in the middle of a symmetric shell (e.g. FCC: 12 + 6 + 24 neighbours, k = 24 cuts the third shell):
+    # many images share the k-th distance exactly, the oracle breaks the tie by (dst, tau); whatever subset the
+    # library returns must be k distinct images, all inside the 1e-5 A tie band of the oracle's (check_knn)
+    b = C.textbook(name, a=3.61)
+    got, status = _knn(mg, ctx, b, k)
+    assert status == 0
+    rep = check.check_knn(b, k, got)
+    assert rep["n_edges"] == k * b.n_atoms
