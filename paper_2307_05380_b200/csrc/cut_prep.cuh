@@ -20,6 +20,8 @@
 #include "common.cuh"
 
 #define MG_CP_BLOCK 128
+#define MGB_MAXSLAB 16             // cell list (cut_bins.cuh): slabs per axis, at most
+#define MGB_MINSLAB 6              // ... fewer than this: the five-slab stencil would cover the axis, one slab instead
 #ifndef MG_STASH
 #define MG_STASH 1024              // stash entries per warp of the emit kernel (cutoff_pairs.cuh)
 #endif
@@ -46,6 +48,8 @@
 #define MG_CS_EDGE 17.f
 #define MG_CS_STRUCT 4000.f
 #define MG_CS_ROWCELL 25.f
+#define MG_CS_BINCAND 16.f         // binned rows (cut_bins.cuh): per candidate left by the stencil
+#define MG_CS_BINROW 1500.f        // ... per source row (the stencil's table)
 #endif
 // ... and of the KNN launch: per candidate cell, per block of 32 pairs, per source row (selection),
 // per structure
@@ -73,7 +77,7 @@ struct CutRec {              // 64 bytes
     float amax_sum;          // sum_a max_c |L_ac|
     float qmax;              // Q = sum_a (rho_a + 1) max_c |L_ac|
     float radius;            // KNN: search radius of the structure (cutoff graph: r_c)
-    int pad;
+    int bins;                // cell list (cut_bins.cuh): nb_0 | nb_1 << 8 | nb_2 << 16 | 1 << 24; 0: not binned
 };
 static_assert(sizeof(CutRec) == 64, "CutRec is one 64-byte line");
 
@@ -177,6 +181,7 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
         r.err = err;
         if (err) atomicOr(A.status, err);
         r.paircost = 1u;
+        r.bins = 0;
         if (r.mloc > 0) {
             const float lam = (float)N * 4.18879f * rc * rc * rc / (float)vol;   // edges per row
             // warp instructions per pair (count + emit launches): 11 per candidate, ~250 per block
@@ -202,10 +207,30 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
                                 MG_CS_STRUCT / ((float)N * (float)N);
             const float crow = MG_CS_ROWCELL * (float)mloc + MG_CS_EDGE * lam / (float)N + MG_CS_STRUCT / ((float)N * (float)N);
             const bool rows = N > MG_SMALL_MAX_ATOMS || mloc > MG_PAIR_TL;
-            const float cnew = 0.25f * (rows ? crow : cscan);      // (quarter cycles: keeps the prefix far from overflow)
+            // K2 cell list (cut_bins.cuh): a large structure in the minimum-image regime; nb_a <= 2 / rho_a slabs
+            // (with a margin far above the FP32 rounding of the slab index), one slab where the five-slab
+            // stencil would cover the axis anyway, and no more bins than atoms
+            float frac = 1.f;
+            if (A.k == 0 && A.rows_cost && N > MG_SMALL_MAX_ATOMS && mloc == 1) {
+                int nb[3];
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    const float f = floorf(2.f / (r.rho[a] * 1.0001f));
+                    nb[a] = f >= (float)MGB_MINSLAB ? (int)fminf(f, (float)MGB_MAXSLAB) : 1;
+                }
+                while (nb[0] * nb[1] * nb[2] > N) {
+                    const int a = nb[0] >= nb[1] && nb[0] >= nb[2] ? 0 : (nb[1] >= nb[2] ? 1 : 2);
+                    nb[a] = nb[a] > MGB_MINSLAB ? nb[a] - 1 : 1;
+                }
+                r.bins = nb[0] | (nb[1] << 8) | (nb[2] << 16) | (1 << 24);
+#pragma unroll
+                for (int a = 0; a < 3; ++a) frac *= nb[a] > 1 ? 5.f / (float)nb[a] : 1.f;
+            }
+            const float cbin = MG_CS_BINCAND * frac + MG_CS_BINROW / (float)N + MG_CS_EDGE * lam / (float)N +
+                               MG_CS_STRUCT / ((float)N * (float)N);
+            const float cnew = 0.25f * (r.bins ? cbin : (rows ? crow : cscan));   // (quarter cycles: keeps the prefix far from overflow)
             r.paircost = (unsigned)fminf(16.f * (A.k > 0 ? (N > MG_SMALL_MAX_ATOMS ? ckb : ck) : (A.rows_cost ? cnew : c)) + 1.f, 16777216.f);
         }
-        r.pad = 0;
         cost = (unsigned long long)((long long)N * N) * r.paircost;
     }
     // ---- block-wide exclusive scan of the cost

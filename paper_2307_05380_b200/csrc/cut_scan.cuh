@@ -26,6 +26,7 @@
 #pragma once
 #include "common.cuh"
 #include "cut_prep.cuh"
+#include "cut_bins.cuh"
 #include "ranges.cuh"
 
 #define MGS_BLOCK 128
@@ -45,6 +46,9 @@ struct ScanArgs {
     const float *pos;
     const float *lattice;
     const float4 *xw4;             // [n_atoms] wrapped coordinates + packed integer parts (cut_prep.cuh)
+    const float4 *xs4;             // [n_atoms] ... in bin order, the structures with a cell list (cut_bins.cuh)
+    const int *sj, *si;            // [n_atoms] ... the local atom index of each entry; the entry of each atom
+    const int *bin_start;          // [n_atoms + 2 n_struct + 2] ... first entry of each bin
     int n_struct, n_atoms;
     const float *radii;            // [n_atoms] or NULL: cutoff of every SOURCE atom (Def. 3's c_i); NULL: the
                                    // same cutoff for all (the structure's radius in its CutRec)
@@ -115,6 +119,9 @@ struct WCtx {
     const float *cr;       // ... and their cutoffs (NULL: rc for all)
     const float *lat;
     int first, N;
+    int nb0, nb1, nb2;     // cell list (cut_bins.cuh): slabs per axis; nb0 == 0: none
+    const float4 *xs;      // ... entries in bin order
+    const int *sj, *si, *bs; // ... their atoms; the entry of each atom; first entry of each bin
 };
 
 __device__ __forceinline__ void mgs_ctx(WCtx &C, const ScanArgs &A, const CutRec *R, int s) {
@@ -137,6 +144,14 @@ __device__ __forceinline__ void mgs_ctx(WCtx &C, const ScanArgs &A, const CutRec
     C.gx = A.pos + 3 * (size_t)R->first;
     C.xw = A.xw4 + R->first;
     C.cr = A.radii ? A.radii + R->first : nullptr;
+    const int bins = R->bins;
+    C.nb0 = bins >> 24 ? bins & 0xFF : 0; C.nb1 = (bins >> 8) & 0xFF; C.nb2 = (bins >> 16) & 0xFF;
+    C.xs = A.xs4 + R->first;
+    C.sj = A.sj + R->first;
+    C.si = A.si + R->first;
+    C.bs = A.bin_start + R->first + 2 * s;
+    // (an atom far from the origin or not finite: the generic rows, which check every offset)
+    if (C.nb0 && C.bs[C.nb0 * C.nb1 * C.nb2 + 1] == 0) C.nb0 = 0;
 }
 
 
@@ -397,6 +412,144 @@ __device__ __forceinline__ unsigned mgs_row(const ScanArgs &A, SSmem &ws, PoolSt
     return cnt;
 }
 
+// One source row of a structure with a cell list (cut_bins.cuh; one-cell sub-box): the candidates are
+// the atoms of the 5 x 5 columns of bins around the row's bin (5 consecutive slabs of the last axis each:
+// one or, across the periodic wrap, two runs of entries), walked as ONE sequence, lane <-> candidate, so
+// that every trip but the last is full.
+template <int PHASE>
+__device__ __forceinline__ unsigned mgs_row_binned(const ScanArgs &A, SSmem &ws, PoolState &P, const WCtx &C, int i,
+                                                   unsigned long long goff, int lane) {
+    const float4 xi = C.xw[i];
+    const float rci = C.cr ? C.cr[i] : C.rc;
+    // ---- the row's columns: exclusive prefix of their lengths, first run (start, length), start of the second
+    int *tp = reinterpret_cast<int *>(&ws.mk[0][0]), *ta1 = tp + 32, *tn1 = tp + 64, *ta2 = tp + 96;
+    const int s0 = C.nb0 > 1 ? 5 : 1, s1 = C.nb1 > 1 ? 5 : 1, ncol = s0 * s1;
+    int a1 = 0, n1 = 0, a2 = 0, n2 = 0;
+    if (lane < ncol) {
+        const int q = s1 == 5 ? lane / 5 : lane;
+        int c0 = mgb_axis(xi.x, C.nb0) + (s0 == 5 ? q - 2 : 0), c1 = mgb_axis(xi.y, C.nb1) + (s1 == 5 ? lane - 5 * q - 2 : 0);
+        c0 += c0 < 0 ? C.nb0 : 0; c0 -= c0 >= C.nb0 ? C.nb0 : 0;
+        c1 += c1 < 0 ? C.nb1 : 0; c1 -= c1 >= C.nb1 ? C.nb1 : 0;
+        const int *col = C.bs + (c0 * C.nb1 + c1) * C.nb2;
+        if (C.nb2 == 1) { a1 = col[0]; n1 = col[1] - a1; }
+        else {
+            const int lo = mgb_axis(xi.z, C.nb2) - 2, hi = lo + 4;          // nb2 >= 6: the five slabs are distinct
+            if (lo < 0) { a1 = col[0]; n1 = col[hi + 1] - a1; a2 = col[C.nb2 + lo]; n2 = col[C.nb2] - a2; }
+            else if (hi >= C.nb2) { a1 = col[lo]; n1 = col[C.nb2] - a1; a2 = col[0]; n2 = col[hi - C.nb2 + 1] - a2; }
+            else { a1 = col[lo]; n1 = col[hi + 1] - a1; }
+        }
+    }
+    int incl = n1 + n2;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    const int total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+    __syncwarp();
+    tp[lane] = incl - (n1 + n2); ta1[lane] = a1; tn1[lane] = n1; ta2[lane] = a2;   // (lanes >= ncol: prefix = total)
+    __syncwarp();
+    // ---- the candidates.  A hit is the image of j nearest to i in fractional coordinates (rho_a < 1/2:
+    // no other image can be inside r_c): f = u - rint(u), u = x_j - x_i (wrapped), d2 in FP32, FP64 decision
+    // inside the rounding window.  A trip only TESTS its candidates (two per lane, v and v + 32, in packed
+    // FP32; rint(u) = (u + 1.5 * 2^23) - 1.5 * 2^23, whose low mantissa bits are rint(u) mod 4); the hits go
+    // to the stash as (entry, rint(u) mod 4) words and become codes, lane <-> hit, when the stash leaves.
+    unsigned *st = reinterpret_cast<unsigned *>(&ws.stash[0]);     // 2 MGS_STASH words
+    const int ki = __float_as_int(xi.w);
+    const float nr2 = -__fmul_rn(rci, rci), win = C.win;
+    const int self = C.si[i];
+    unsigned cnt = 0u, ns = 0u, done = 0u;
+    const unsigned lt = (1u << lane) - 1u;
+    const float2 nx0 = make_float2(-xi.x, -xi.x), nx1 = make_float2(-xi.y, -xi.y), nx2 = make_float2(-xi.z, -xi.z);
+    const float2 MAG = make_float2(12582912.f, 12582912.f), NMAG = make_float2(-12582912.f, -12582912.f);
+    const float2 M1 = make_float2(-1.f, -1.f), Z2 = make_float2(0.f, 0.f), nr22 = make_float2(nr2, nr2);
+    const float2 a0 = make_float2(C.a[0], C.a[0]), a1v = make_float2(C.a[1], C.a[1]), a2v = make_float2(C.a[2], C.a[2]),
+                 a3 = make_float2(C.a[3], C.a[3]), a4 = make_float2(C.a[4], C.a[4]), a5 = make_float2(C.a[5], C.a[5]),
+                 a6 = make_float2(C.a[6], C.a[6]), a7 = make_float2(C.a[7], C.a[7]), a8 = make_float2(C.a[8], C.a[8]);
+    int cA = 0, cB = 0;
+    for (int v0 = 0; v0 < total || ns; v0 += 64) {
+        if (v0 < total) {
+            const int vA = v0 + lane, vB = vA + 32;
+            const bool okA = vA < total, okB = vB < total;
+            int idxA = 0, idxB = 0;
+            if (okA) {                                                        // (ncol <= 25: tp[26..31] = total > v)
+                while (tp[cA + 1] <= vA) ++cA;
+                const int r = vA - tp[cA], n1c = tn1[cA];
+                idxA = r < n1c ? ta1[cA] + r : ta2[cA] + (r - n1c);
+            }
+            if (okB) {
+                cB = max(cB, cA);
+                while (tp[cB + 1] <= vB) ++cB;
+                const int r = vB - tp[cB], n1c = tn1[cB];
+                idxB = r < n1c ? ta1[cB] + r : ta2[cB] + (r - n1c);
+            }
+            const float4 xA = C.xs[idxA], xB = C.xs[idxB];
+            const float2 u0 = mg_add2(make_float2(xA.x, xB.x), nx0), u1 = mg_add2(make_float2(xA.y, xB.y), nx1),
+                         u2 = mg_add2(make_float2(xA.z, xB.z), nx2);
+            const float2 m0 = mg_add2(u0, MAG), m1 = mg_add2(u1, MAG), m2 = mg_add2(u2, MAG);
+            const float2 f0 = mg_fma2(mg_add2(m0, NMAG), M1, u0), f1 = mg_fma2(mg_add2(m1, NMAG), M1, u1),
+                         f2 = mg_fma2(mg_add2(m2, NMAG), M1, u2);
+            const float2 vx = mg_fma2(f2, a6, mg_fma2(f1, a3, mg_fma2(f0, a0, Z2)));
+            const float2 vy = mg_fma2(f2, a7, mg_fma2(f1, a4, mg_fma2(f0, a1v, Z2)));
+            const float2 vz = mg_fma2(f2, a8, mg_fma2(f1, a5, mg_fma2(f0, a2v, Z2)));
+            const float2 y = mg_fma2(vz, vz, mg_fma2(vy, vy, mg_fma2(vx, vx, nr22)));
+            bool hitA = okA && y.x < 0.f, hitB = okB && y.y < 0.f;
+            const unsigned wordA = (unsigned)idxA | ((__float_as_uint(m0.x) & 3u) << 16) | ((__float_as_uint(m1.x) & 3u) << 18) |
+                                   ((__float_as_uint(m2.x) & 3u) << 20);
+            const unsigned wordB = (unsigned)idxB | ((__float_as_uint(m0.y) & 3u) << 16) | ((__float_as_uint(m1.y) & 3u) << 18) |
+                                   ((__float_as_uint(m2.y) & 3u) << 20);
+            if (fminf(fabsf(y.x), fabsf(y.y)) < win) {                        // FP32 cannot decide: Def. 3 in FP64
+#pragma unroll 1
+                for (int h = 0; h < 2; ++h) {
+                    const float yh = h ? y.y : y.x;
+                    if (!(h ? okB : okA) || !(fabsf(yh) < win)) continue;
+                    const unsigned w = h ? wordB : wordA;
+                    const int idx = (int)(w & 0xFFFFu), kj = __float_as_int((h ? xB : xA).w), j = C.sj[idx];
+                    const int t0 = 1 - (int)(((w >> 16) + 1u) & 3u) + (ki & 1023) - (kj & 1023),
+                              t1 = 1 - (int)(((w >> 18) + 1u) & 3u) + ((ki >> 10) & 1023) - ((kj >> 10) & 1023),
+                              t2 = 1 - (int)(((w >> 20) + 1u) & 3u) + ((ki >> 20) & 1023) - ((kj >> 20) & 1023);
+                    double w3[3];
+                    const bool e = mg_exact_vec(C.gx + 3 * i, C.gx + 3 * j, t0, t1, t2, C.lat, w3) < (double)rci;
+                    if (h) hitB = e; else hitA = e;
+                }
+            }
+            hitA = hitA && idxA != self;                                      // (i, i, 0) is not an edge (R3)
+            hitB = hitB && idxB != self;
+            const unsigned balA = __ballot_sync(0xFFFFFFFFu, hitA), balB = __ballot_sync(0xFFFFFFFFu, hitB);
+            const unsigned nA = __popc(balA);
+            if (hitA) st[ns + __popc(balA & lt)] = wordA;
+            if (hitB) st[ns + nA + __popc(balB & lt)] = wordB;
+            ns += nA + __popc(balB);
+            cnt += nA + __popc(balB);
+            if (ns <= 2 * MGS_STASH - 64 && v0 + 64 < total) continue;
+        }
+        // ---- the stash leaves: entry -> (dst, tau) code, lane <-> hit
+        __syncwarp();
+        if (PHASE == 0) mgs_pool_reserve(A, ws, P, P.wcount + done + ns, lane);
+        for (unsigned x = lane; x < ns; x += 32) {
+            const unsigned w = st[x];
+            const int idx = (int)(w & 0xFFFFu);
+            const int kj = __float_as_int(C.xs[idx].w), j = C.sj[idx];
+            int tau[3];                            // the word holds rint(u_a) mod 4; tau = -rint(u) + k_i - k_j
+            tau[0] = 1 - (int)(((w >> 16) + 1u) & 3u) + (ki & 1023) - (kj & 1023);
+            tau[1] = 1 - (int)(((w >> 18) + 1u) & 3u) + ((ki >> 10) & 1023) - ((kj >> 10) & 1023);
+            tau[2] = 1 - (int)(((w >> 20) + 1u) & 3u) + ((ki >> 20) & 1023) - ((kj >> 20) & 1023);
+            // (cut_bins.cuh: the atoms are finite and within 63 cells of the origin, so |tau| <= 127)
+            const uint2 code = make_uint2((unsigned)(C.first + j), ((unsigned)(tau[0] + 128) << 24) |
+                                          ((unsigned)(tau[1] + 128) << 16) | ((unsigned)(tau[2] + 128) << 8));
+            if (PHASE == 0) {
+                if (P.ok) *mgs_pool_addr(A, P.list, P.wcount + done + x) = code;
+            } else if (PHASE == 2) {
+                mgs_emit_one(A, (long long)(goff + done + x), C.first + i, C.first + j, C.gx, i, j, tau, C.lat);
+            } else if ((long long)(goff + done + x) < A.capacity) A.codes[goff + done + x] = code;
+        }
+        done += ns;
+        ns = 0u;
+        __syncwarp();
+    }
+    return cnt;
+}
+
 // ---- the walk of a warp over its rows -------------------------------------------------------------
 // PHASE 0 (find): hits of every block -> codes in the pool, row_ptr = offsets LOCAL to the warp, the
 //   products of the rows (atom_struct, pos64, lat64); returns the warp's edge count (on every lane).
@@ -441,7 +594,8 @@ __device__ __forceinline__ unsigned long long mgs_walk(SSmem &ws, const ScanArgs
                 for (int i = ia; i < ib; ++i) {
                     bool anybad = false;
                     if (lane == 0) A.row_ptr[C.first + i] = (int)MGS_HERE;
-                    const unsigned cnt = mgs_row<PHASE>(A, ws, P, C, i, goff, lane, anybad);
+                    const unsigned cnt = C.nb0 ? mgs_row_binned<PHASE>(A, ws, P, C, i, goff, lane)
+                                               : mgs_row<PHASE>(A, ws, P, C, i, goff, lane, anybad);
                     if (PHASE == 0) {
                         if (anybad) atomicOr(A.status, __float_as_int(C.xw[i].w) == 0 ? MGS_NONFINITE : MGS_OFFSET);
                         P.wcount += cnt;

@@ -320,3 +320,83 @@ def test_scan_kernel_capacity_and_count(mg, scan_ctx):
     assert np.array_equal(got["src"], full["src"][:m])
     kg = check._keys(got["src"], got["dst"], got["offset"])
     assert set(kg.tolist()) <= set(check._keys(full["src"], full["dst"], full["offset"]).tolist())
+
+
+# ---- K2: the cell list of large structures (csrc/cut_bins.cuh) --------------------------------------
+def _big_cell(rng, lengths, n, skew=0.0, shift=0.0):
+    cell = np.diag(np.asarray(lengths, np.float64))
+    cell[1, 0] = skew * lengths[0]
+    cell[2, 1] = -0.5 * skew * lengths[1]
+    x = rng.random((n, 3), dtype=np.float32) + np.float32(shift)
+    return cell.astype(np.float32), x.astype(np.float32)
+
+
+def test_cell_list_shapes_and_wraps(mg, ctx):
+    # slabs on three, two, one and no axis (cell lengths from 3 to 12 cutoffs), skewed cells, coordinates on the
+    # boundary of the cell (0, 1 - ulp, exactly representable slab edges) and outside it, in one batch with small
+    # structures: every structure above 64 atoms in the minimum-image regime goes through the binned rows
+    rng = np.random.default_rng(77)
+    rc = 4.0
+    items = [_big_cell(rng, (50.0, 40.0, 30.0), 900),               # 12 / 10 / 7 cutoffs: slabs on all axes
+             _big_cell(rng, (45.0, 13.0, 36.0), 500, skew=0.3),     # middle axis short: one slab there
+             _big_cell(rng, (12.0, 11.0, 48.0), 300),               # only the last axis has slabs
+             _big_cell(rng, (11.0, 12.0, 13.0), 200, skew=0.2),     # no slabs: one bin
+             _big_cell(rng, (64.0, 64.0, 64.0), 150),               # more bins than atoms: slabs are merged
+             _big_cell(rng, (40.0, 40.0, 40.0), 700, shift=-2.0)]   # coordinates in [-2, -1): wrapped
+    edge = np.array([[0.0, 0.0, 0.0], [1.0 - 2.0 ** -24, 0.5, 0.25], [0.125, 0.875, 1.0 - 2.0 ** -24],
+                     [0.5, 0.0, 0.75], [2.0 ** -24, 0.999999, 0.0]], np.float32)
+    items[0][1][:5] = edge
+    b = C.concat([C.small_batch(5, seed=4), C._assemble(items), C.small_batch(3, seed=5)])
+    got, status = _run_cutoff(mg, ctx, b, rc)
+    assert status == 0
+    rep = check.check_cutoff(b, rc, got)
+    assert rep["extra"] == 0 and rep["missing"] == 0 and rep["n_edges"] > 10000, rep
+    # the same call again: same arrays, bit for bit (the cell list is built in index order, no atomics race)
+    again, _ = _run_cutoff(mg, ctx, b, rc)
+    for k in ("row_ptr", "src", "dst", "offset", "vec", "dist"):
+        assert np.array_equal(got[k], again[k]), k
+
+
+def test_cell_list_far_atoms_radii_and_small_pool(mg, monkeypatch):
+    rng = np.random.default_rng(78)
+    cell, x = _big_cell(rng, (30.0, 32.0, 34.0), 400, skew=0.1)
+    far = x.copy()
+    far[7, 0] += np.float32(70.0)                                   # 70 cells away: the structure takes the generic rows
+    near = C._assemble([(cell, x)])
+    b_far = C._assemble([(cell, far)])
+    c = mg.Context(0)
+    try:
+        pos, lat, ptr = mg.to_device(b_far)
+        got = c.cutoff_graph(pos, lat, ptr, 4.5, dist=True).to_numpy()
+        assert c.mg_check() == 0                                    # |tau| = 70 still fits int8
+        rep = check.check_cutoff(b_far, 4.5, got)
+        assert rep["extra"] == 0 and rep["missing"] == 0 and np.abs(got["offset"]).max() >= 69
+        bad = far.copy()
+        bad[9, 1] = np.float32(np.nan)
+        pos, lat, ptr = mg.to_device(C._assemble([(cell, bad)]))
+        c.cutoff_graph(pos, lat, ptr, 4.5, dist=True)
+        assert c.mg_check() != 0                                    # a NaN coordinate is reported
+        # per-atom cutoffs on a binned structure
+        radii = rng.uniform(2.0, 4.5, size=near.n_atoms).astype(np.float32)
+        pos, lat, ptr = mg.to_device(near)
+        import torch
+        ref = oracle.cutoff_graph_radii(near.pos, near.lattice, near.struct_ptr, radii)
+        out = mg.Edges.allocate(near.n_atoms, int(ref["n_edges"]) + 8, pos.device, dist=True)
+        got = c.mg_cutoff_graph_radii(pos, lat, ptr, torch.from_numpy(radii).to(pos.device), out).to_numpy()
+        assert c.mg_check() == 0
+        kg = np.sort(check._keys(got["src"], got["dst"], got["offset"]))
+        kr = np.sort(check._keys(ref["src"], ref["dst"], ref["tau"]))
+        assert np.array_equal(kg, kr) and np.array_equal(got["row_ptr"], ref["row_ptr"])
+    finally:
+        c.close()
+    # a pool of three chunks: the warps list their rows again and write edge by edge
+    monkeypatch.setenv("MATGRAPH_MASK_WORDS", "3")
+    c = mg.Context(0)
+    try:
+        pos, lat, ptr = mg.to_device(near)
+        got = c.cutoff_graph(pos, lat, ptr, 6.0, dist=True).to_numpy()
+        assert c.mg_check() == 0
+        rep = check.check_cutoff(near, 6.0, got)
+        assert rep["extra"] == 0 and rep["missing"] == 0 and rep["n_edges"] > 3 * 512, rep
+    finally:
+        c.close()
