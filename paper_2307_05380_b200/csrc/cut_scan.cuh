@@ -1,28 +1,28 @@
 // cut_scan.cuh — cutoff graph (K3 distance filter, K4 count -> device-wide scan -> emit, K6 batching,
-// SURVEY.md 8(a)) in two launches:
+// SURVEY.md 8(a)) in ONE cooperative launch; DESIGN.md 5.7.
 //
-//   mg_cutoff_scan_kernel   finds the edges.  Co-resident CTAs whose warps work on their own:
-//     warp r of the grid (r = 4 * blockIdx.x + warp) owns the source rows whose first pair lies in the r-th of
-//     n_ranges equally expensive, contiguous ranges of the batch's ordered pairs in (structure, i, j)
-//     order — the CSR order of the output (cut_prep.cuh).  It walks its rows twice:
-//       count   per structure: wrapped positions and the table of local translations staged in the
-//               warp's shared memory; blocks of 32 ordered pairs, lane <-> pair: FP32 filter over the
-//               pair's sub-box (FP64 decision inside the rounding window, R23); the 32-bit
-//               hit masks go to the warp's scratch in global memory (L2 resident);
-//       scan    warp totals -> CTA total, published in a slot tagged with the call's epoch; warp 0
-//               sums the slots of the CTAs before its own (all CTAs are resident: cooperative launch):
-//               the device-wide exclusive scan of K4 without a launch of its own;
-//       list    the same walk: masks read back, the hits of a block compacted in (row, j, t) order
-//               into 8-byte codes (dst, tau) at their FINAL position in one code stream; row_ptr,
-//               the atom -> structure map, FP64 copies of positions and lattices, and for every 128th
-//               edge the row it belongs to.
-//   mg_cutoff_write_kernel  turns the code stream into the caller's arrays.  Perfectly balanced (a warp
-//     takes slices of 128 consecutive edges, whatever structure they come from), no staging, lane <-> four
-//     consecutive edges: src from row_ptr, vec = ((x_dst - x_src) + tau) . L in FP64 in the oracle's
-//     operation order, rounded once (R24); every array leaves in aligned 16-byte stores.
+//   mg_cutoff_scan_kernel.  Co-resident CTAs whose warps work on their own: warp r of the grid (r = 4 *
+//     blockIdx.x + warp) owns the source rows whose first pair lies in the r-th of n_ranges equally expensive,
+//     contiguous ranges of the batch's ordered pairs in (structure, i, j) order — the CSR order of the
+//     output (cut_prep.cuh).
+//       find    per structure: wrapped positions and the table of local translations staged in the warp's
+//               shared memory; blocks of 32 ordered pairs, lane <-> pair: FP32 filter over the pair's sub-box
+//               (FP64 decision inside the rounding window, R23), 32-bit hit masks in shared memory,
+//               hits compacted in (row, j, t) order into 8-byte codes (dst, tau) that go to chunks of a pool
+//               (the warp does not know yet where its edges start); row_ptr local to the warp;
+//       scan    warp totals -> CTA total, published in a slot tagged with the call's epoch; warp 0 sums
+//               the slots of the CTAs before its own (all CTAs are resident: cooperative launch): the
+//               device-wide exclusive scan of K4 without a launch of its own;
+//       write   the warp turns its codes into the caller's arrays: lane <-> four consecutive edges, src
+//               from row_ptr, vec = ((x_dst - x_src) + tau) . L in FP64 in the oracle's operation order,
+//               rounded once (R24); every array leaves in aligned 16-byte stores.
+//     A warp whose codes did not fit the pool walks its rows a second time and writes edge by edge.
+//   mg_cutoff_write_kernel (MATGRAPH_WRITE_KERNEL=1, an A/B variant): the write phase as a launch of its
+//     own over one code stream, a warp per slice of 128 consecutive edges.
 //
 // Structures the pair-lane path does not take (more than MGS_NMAX atoms, a sub-box of more than MGS_TL
-// cells) go row by row: lanes over the candidates (j, t) of one source row, ballot compaction.
+// cells) go row by row, lanes over the candidates of one source row: through the cell list of
+// cut_bins.cuh when the sub-box is one cell (mgs_row_binned), else over all (j, t) (mgs_row).
 #pragma once
 #include "common.cuh"
 #include "cut_prep.cuh"
