@@ -98,7 +98,38 @@ struct SSmem {                         // one warp's shared memory
     unsigned mk[MGS_TL / 32][32];      // hit masks of the current block
     int chunks[MGS_WAVES][MGS_MAXCH];  // the chunks of the pool that hold the codes of the warp's ranges
     int wave[MGS_WAVES][8];            // per range: edges, chunks, pool ok, first row, end of rows, edges of the warps before (2 words)
+    unsigned long long bar[2];         // mbarriers of the two candidate buffers (binned rows: TMA bulk copies)
+    unsigned bphase;                   // ... their phase bits
 };
+
+// The candidate buffers of the binned rows: the staging area of the pair-lane path (T | tcode | x is one
+// contiguous, 16-byte aligned piece of the warp's shared memory), two buffers of MGS_CH entries.
+#define MGS_CH 192
+static_assert(2 * MGS_CH * sizeof(float4) <= sizeof(float) * 3 * (MGS_TL + 4) + sizeof(unsigned) * MGS_TL + sizeof(float4) * MGS_NMAX,
+              "two candidate buffers fit the staging area");
+static_assert((sizeof(float) * 3 * (MGS_TL + 4)) % 16 == 0 && (sizeof(unsigned) * MGS_TL) % 16 == 0, "staging area is contiguous");
+
+// ---- TMA bulk copies (global -> the warp's shared memory) that complete on an mbarrier
+__device__ __forceinline__ unsigned mgs_saddr(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mgs_bar_init(unsigned long long *bar) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(mgs_saddr(bar)) : "memory");
+}
+__device__ __forceinline__ void mgs_bar_expect(unsigned long long *bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(mgs_saddr(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mgs_bar_wait(unsigned long long *bar, unsigned phase) {
+    unsigned done = 0u;
+    const unsigned a = mgs_saddr(bar);
+    while (!done)
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.b32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(a), "r"(phase) : "memory");
+}
+__device__ __forceinline__ void mgs_bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 :: "r"(mgs_saddr(dst)), "l"(src), "r"(bytes), "r"(mgs_saddr(bar)) : "memory");
+}
+// (generic-proxy accesses to shared memory before, async-proxy accesses after)
+__device__ __forceinline__ void mgs_fence_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 struct ScanSmem {
     SSmem w[MGS_WARPS];
@@ -415,7 +446,9 @@ __device__ __forceinline__ unsigned mgs_row(const ScanArgs &A, SSmem &ws, PoolSt
 // One source row of a structure with a cell list (cut_bins.cuh; one-cell sub-box): the candidates are
 // the atoms of the 5 x 5 columns of bins around the row's bin (5 consecutive slabs of the last axis each:
 // one or, across the periodic wrap, two runs of entries), walked as ONE sequence, lane <-> candidate, so
-// that every trip but the last is full.
+// that every trip but the last is full.  (BASELINE.json north_star: "stages each structure's positions ...
+// in shared memory (TMA bulk copy where the structure is large)": the runs reach shared memory by
+// cp.async.bulk.)
 template <int PHASE>
 __device__ __forceinline__ unsigned mgs_row_binned(const ScanArgs &A, SSmem &ws, PoolState &P, const WCtx &C, int i,
                                                    unsigned long long goff, int lane) {
@@ -449,16 +482,51 @@ __device__ __forceinline__ unsigned mgs_row_binned(const ScanArgs &A, SSmem &ws,
     __syncwarp();
     tp[lane] = incl - (n1 + n2); ta1[lane] = a1; tn1[lane] = n1; ta2[lane] = a2;   // (lanes >= ncol: prefix = total)
     __syncwarp();
-    // ---- the candidates.  A hit is the image of j nearest to i in fractional coordinates (rho_a < 1/2:
-    // no other image can be inside r_c): f = u - rint(u), u = x_j - x_i (wrapped), d2 in FP32, FP64 decision
-    // inside the rounding window.  A trip only TESTS its candidates (two per lane, v and v + 32, in packed
-    // FP32; rint(u) = (u + 1.5 * 2^23) - 1.5 * 2^23, whose low mantissa bits are rint(u) mod 4); the hits go
-    // to the stash as (entry, rint(u) mod 4) words and become codes, lane <-> hit, when the stash leaves.
+    // ---- the candidates.  The runs of the row's columns are copied, in sequence order, into two buffers of
+    // MGS_CH entries in the warp's shared memory by TMA bulk copies (every lane issues the pieces of its own
+    // column; the copy of chunk k + 1 flies while chunk k is tested), so a trip reads candidate v at buf[v].
+    // A hit is the image of j nearest to i in fractional coordinates (rho_a < 1/2: no other image can be inside
+    // r_c): f = u - rint(u), u = x_j - x_i (wrapped), d2 in FP32, FP64 decision inside the rounding window.
+    // A trip only TESTS its candidates (two per lane, v and v + 32, in packed FP32; rint(u) = (u + 1.5 * 2^23)
+    // - 1.5 * 2^23, whose low mantissa bits are rint(u) mod 4); the hits go to the stash as (v, rint(u) mod 4)
+    // words and become codes, lane <-> hit, when the stash leaves.
     unsigned *st = reinterpret_cast<unsigned *>(&ws.stash[0]);     // 2 MGS_STASH words
+    float4 *buf = reinterpret_cast<float4 *>(&ws.T[0][0]);         // 2 x MGS_CH entries
     const int ki = __float_as_int(xi.w);
     const float nr2 = -__fmul_rn(rci, rci), win = C.win;
-    const int self = C.si[i];
+    // the row's own entry as a candidate number: it sits in the centre column
+    int vself;
+    {
+        const int cs = (s0 == 5 ? 2 : 0) * s1 + (s1 == 5 ? 2 : 0), self = C.si[i];
+        const int pa1 = __shfl_sync(0xFFFFFFFFu, a1, cs), pn1 = __shfl_sync(0xFFFFFFFFu, n1, cs),
+                  pa2 = __shfl_sync(0xFFFFFFFFu, a2, cs), pp = __shfl_sync(0xFFFFFFFFu, incl - (n1 + n2), cs);
+        vself = pp + (self >= pa1 && self < pa1 + pn1 ? self - pa1 : pn1 + self - pa2);
+    }
+    // entry of candidate v (hits only)
+    auto entry = [&](int v) {
+        int c = 0;                                                            // last column with tp[c] <= v
+#pragma unroll
+        for (int st = 16; st; st >>= 1) c += tp[c + st] <= v ? st : 0;        // (ncol <= 25: tp[26..31] = total > v)
+        const int r = v - tp[c], n1c = tn1[c];
+        return r < n1c ? ta1[c] + r : ta2[c] + (r - n1c);
+    };
+    // the pieces of this lane's column inside chunk [base, base + MGS_CH) -> buffer b
+    const int myp = incl - (n1 + n2);
+    auto issue = [&](int base, int b) {
+        const int nchunk = min(MGS_CH, total - base);
+        if (lane == 0) mgs_bar_expect(&ws.bar[b], 16u * (unsigned)nchunk);
+        __syncwarp();
+        const int r_lo = max(base - myp, 0), r_hi = min(base + MGS_CH - myp, n1 + n2);
+        if (r_lo < r_hi) {
+            float4 *dst = buf + b * MGS_CH + (myp - base);
+            const int e1 = min(r_hi, n1);
+            if (r_lo < e1) mgs_bulk_g2s(dst + r_lo, C.xs + a1 + r_lo, 16u * (unsigned)(e1 - r_lo), &ws.bar[b]);
+            const int b2 = max(r_lo, n1);
+            if (b2 < r_hi) mgs_bulk_g2s(dst + b2, C.xs + a2 + (b2 - n1), 16u * (unsigned)(r_hi - b2), &ws.bar[b]);
+        }
+    };
     unsigned cnt = 0u, ns = 0u, done = 0u;
+    unsigned phase = ws.bphase;
     const unsigned lt = (1u << lane) - 1u;
     const float2 nx0 = make_float2(-xi.x, -xi.x), nx1 = make_float2(-xi.y, -xi.y), nx2 = make_float2(-xi.z, -xi.z);
     const float2 MAG = make_float2(12582912.f, 12582912.f), NMAG = make_float2(-12582912.f, -12582912.f);
@@ -466,24 +534,20 @@ __device__ __forceinline__ unsigned mgs_row_binned(const ScanArgs &A, SSmem &ws,
     const float2 a0 = make_float2(C.a[0], C.a[0]), a1v = make_float2(C.a[1], C.a[1]), a2v = make_float2(C.a[2], C.a[2]),
                  a3 = make_float2(C.a[3], C.a[3]), a4 = make_float2(C.a[4], C.a[4]), a5 = make_float2(C.a[5], C.a[5]),
                  a6 = make_float2(C.a[6], C.a[6]), a7 = make_float2(C.a[7], C.a[7]), a8 = make_float2(C.a[8], C.a[8]);
-    int cA = 0, cB = 0;
+    mgs_fence_async();                             // (the staging area may hold the pair-lane path's tables)
+    __syncwarp();
+    if (total > 0) issue(0, 0);
     for (int v0 = 0; v0 < total || ns; v0 += 64) {
         if (v0 < total) {
+            const int k = v0 / MGS_CH, b = k & 1, t = v0 - k * MGS_CH;
+            if (t == 0) {                          // a new chunk: wait for it, send for the next one
+                mgs_bar_wait(&ws.bar[b], (phase >> b) & 1u);
+                phase ^= 1u << b;
+                if ((k + 1) * MGS_CH < total) issue((k + 1) * MGS_CH, b ^ 1);
+            }
             const int vA = v0 + lane, vB = vA + 32;
             const bool okA = vA < total, okB = vB < total;
-            int idxA = 0, idxB = 0;
-            if (okA) {                                                        // (ncol <= 25: tp[26..31] = total > v)
-                while (tp[cA + 1] <= vA) ++cA;
-                const int r = vA - tp[cA], n1c = tn1[cA];
-                idxA = r < n1c ? ta1[cA] + r : ta2[cA] + (r - n1c);
-            }
-            if (okB) {
-                cB = max(cB, cA);
-                while (tp[cB + 1] <= vB) ++cB;
-                const int r = vB - tp[cB], n1c = tn1[cB];
-                idxB = r < n1c ? ta1[cB] + r : ta2[cB] + (r - n1c);
-            }
-            const float4 xA = C.xs[idxA], xB = C.xs[idxB];
+            const float4 xA = buf[b * MGS_CH + t + lane], xB = buf[b * MGS_CH + t + 32 + lane];
             const float2 u0 = mg_add2(make_float2(xA.x, xB.x), nx0), u1 = mg_add2(make_float2(xA.y, xB.y), nx1),
                          u2 = mg_add2(make_float2(xA.z, xB.z), nx2);
             const float2 m0 = mg_add2(u0, MAG), m1 = mg_add2(u1, MAG), m2 = mg_add2(u2, MAG);
@@ -494,9 +558,9 @@ __device__ __forceinline__ unsigned mgs_row_binned(const ScanArgs &A, SSmem &ws,
             const float2 vz = mg_fma2(f2, a8, mg_fma2(f1, a5, mg_fma2(f0, a2v, Z2)));
             const float2 y = mg_fma2(vz, vz, mg_fma2(vy, vy, mg_fma2(vx, vx, nr22)));
             bool hitA = okA && y.x < 0.f, hitB = okB && y.y < 0.f;
-            const unsigned wordA = (unsigned)idxA | ((__float_as_uint(m0.x) & 3u) << 16) | ((__float_as_uint(m1.x) & 3u) << 18) |
+            const unsigned wordA = (unsigned)vA | ((__float_as_uint(m0.x) & 3u) << 16) | ((__float_as_uint(m1.x) & 3u) << 18) |
                                    ((__float_as_uint(m2.x) & 3u) << 20);
-            const unsigned wordB = (unsigned)idxB | ((__float_as_uint(m0.y) & 3u) << 16) | ((__float_as_uint(m1.y) & 3u) << 18) |
+            const unsigned wordB = (unsigned)vB | ((__float_as_uint(m0.y) & 3u) << 16) | ((__float_as_uint(m1.y) & 3u) << 18) |
                                    ((__float_as_uint(m2.y) & 3u) << 20);
             if (fminf(fabsf(y.x), fabsf(y.y)) < win) {                        // FP32 cannot decide: Def. 3 in FP64
 #pragma unroll 1
@@ -504,7 +568,7 @@ __device__ __forceinline__ unsigned mgs_row_binned(const ScanArgs &A, SSmem &ws,
                     const float yh = h ? y.y : y.x;
                     if (!(h ? okB : okA) || !(fabsf(yh) < win)) continue;
                     const unsigned w = h ? wordB : wordA;
-                    const int idx = (int)(w & 0xFFFFu), kj = __float_as_int((h ? xB : xA).w), j = C.sj[idx];
+                    const int idx = entry((int)(w & 0xFFFFu)), kj = __float_as_int((h ? xB : xA).w), j = C.sj[idx];
                     const int t0 = 1 - (int)(((w >> 16) + 1u) & 3u) + (ki & 1023) - (kj & 1023),
                               t1 = 1 - (int)(((w >> 18) + 1u) & 3u) + ((ki >> 10) & 1023) - ((kj >> 10) & 1023),
                               t2 = 1 - (int)(((w >> 20) + 1u) & 3u) + ((ki >> 20) & 1023) - ((kj >> 20) & 1023);
@@ -513,8 +577,8 @@ __device__ __forceinline__ unsigned mgs_row_binned(const ScanArgs &A, SSmem &ws,
                     if (h) hitB = e; else hitA = e;
                 }
             }
-            hitA = hitA && idxA != self;                                      // (i, i, 0) is not an edge (R3)
-            hitB = hitB && idxB != self;
+            hitA = hitA && vA != vself;                                       // (i, i, 0) is not an edge (R3)
+            hitB = hitB && vB != vself;
             const unsigned balA = __ballot_sync(0xFFFFFFFFu, hitA), balB = __ballot_sync(0xFFFFFFFFu, hitB);
             const unsigned nA = __popc(balA);
             if (hitA) st[ns + __popc(balA & lt)] = wordA;
@@ -528,7 +592,7 @@ __device__ __forceinline__ unsigned mgs_row_binned(const ScanArgs &A, SSmem &ws,
         if (PHASE == 0) mgs_pool_reserve(A, ws, P, P.wcount + done + ns, lane);
         for (unsigned x = lane; x < ns; x += 32) {
             const unsigned w = st[x];
-            const int idx = (int)(w & 0xFFFFu);
+            const int idx = entry((int)(w & 0xFFFFu));
             const int kj = __float_as_int(C.xs[idx].w), j = C.sj[idx];
             int tau[3];                            // the word holds rint(u_a) mod 4; tau = -rint(u) + k_i - k_j
             tau[0] = 1 - (int)(((w >> 16) + 1u) & 3u) + (ki & 1023) - (kj & 1023);
@@ -547,6 +611,7 @@ __device__ __forceinline__ unsigned mgs_row_binned(const ScanArgs &A, SSmem &ws,
         ns = 0u;
         __syncwarp();
     }
+    if (lane == 0) ws.bphase = phase;
     return cnt;
 }
 
@@ -926,6 +991,9 @@ mg_cutoff_scan_kernel(const __grid_constant__ ScanArgs A) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     SSmem &ws = sm.w[warp];
     const unsigned epoch = *reinterpret_cast<volatile unsigned *>(A.ctl + 10) + 1u;   // tag of this call's slots
+    if (lane == 0) { mgs_bar_init(&ws.bar[0]); mgs_bar_init(&ws.bar[1]); ws.bphase = 0u; }
+    mgs_fence_async();
+    __syncwarp();
     RangeCtx RC;
     const int n_warps = (int)gridDim.x * MGS_WARPS;
     mg_range_init(RC, A.rec, A.bpre, A.n_blocks, A.n_struct, MGS_WAVES * n_warps, lane);
