@@ -16,9 +16,10 @@
 // memory, exclusive scan, stable scatter (atoms of a bin stay in index order, so the result does not depend on
 // the timing of atomics).  Output, per structure s with first atom f: bin_start[f + 2 s + b], b in
 // [0, nbins], positions LOCAL to the structure, and at b = nbins + 1 a flag: 1 if every atom is finite and
-// within 63 cells of the origin (then no offset of an edge can leave int8 and the rows need not check);
-// xs4[f + p] / sj[f + p] = wrapped coordinates (and packed integer parts) / index of the p-th atom in bin
-// order; si[f + j] = p, the place of atom j.
+// within 15 cells of the origin (then no offset of an edge can leave int8 and the rows need not check);
+// xs4[f + p] = the p-th atom in bin order: wrapped coordinates, and in .w its local index j and the
+// integer parts k_a of its coordinates, j | (k_0 + 16) << 16 | (k_1 + 16) << 21 | (k_2 + 16) << 26
+// (mgb_pack): a row of the scan kernel needs nothing else about a candidate.
 #pragma once
 #include "common.cuh"
 #include "cut_prep.cuh"
@@ -35,12 +36,16 @@ __device__ __forceinline__ int mgb_bin(const float4 x, int nb0, int nb1, int nb2
     return (mgb_axis(x.x, nb0) * nb1 + mgb_axis(x.y, nb1)) * nb2 + mgb_axis(x.z, nb2);
 }
 
+// .w of a sorted entry from the packed integer parts of cut_prep.cuh (10 bits each, biased by 512; the
+// structure's atoms are within 15 cells of the origin, else the entry is not used) and the atom's index
+__device__ __forceinline__ int mgb_pack(int kk, int j) {
+    return j | ((((kk & 1023) - 496) & 31) << 16) | (((((kk >> 10) & 1023) - 496) & 31) << 21) | (((((kk >> 20) & 1023) - 496) & 31) << 26);
+}
+
 struct BinArgs {
     const CutRec *rec;
     const float4 *xw4;         // [n_atoms] wrapped coordinates (cut_prep.cuh)
     float4 *xs4;               // [n_atoms] the same, in bin order inside each binned structure
-    int *sj;                   // [n_atoms] local atom index of the entry
-    int *si;                   // [n_atoms] entry of the local atom
     int *bin_start;            // [n_atoms + 2 n_struct + 2]
     int n_struct;
 };
@@ -137,7 +142,7 @@ mg_cut_bin_kernel(const BinArgs A) {
                 const int p = (int)row[b] + __popc(peers & ((1u << lane) - 1u));
                 __syncwarp();
                 if (lane == 31 - __clz(peers)) row[b] = (unsigned short)(p + 1);   // the last lane of the group leaves the cursor
-                if (v) { A.xs4[first + p] = xj; A.sj[first + p] = j; A.si[first + j] = p; }
+                if (v) { xj.w = __int_as_float(mgb_pack(__float_as_int(xj.w), j)); A.xs4[first + p] = xj; }
                 __syncwarp();
             }
     }

@@ -46,8 +46,7 @@ struct ScanArgs {
     const float *pos;
     const float *lattice;
     const float4 *xw4;             // [n_atoms] wrapped coordinates + packed integer parts (cut_prep.cuh)
-    const float4 *xs4;             // [n_atoms] ... in bin order, the structures with a cell list (cut_bins.cuh)
-    const int *sj, *si;            // [n_atoms] ... the local atom index of each entry; the entry of each atom
+    const float4 *xs4;             // [n_atoms] ... in bin order, .w = atom index and integer parts (cut_bins.cuh)
     const int *bin_start;          // [n_atoms + 2 n_struct + 2] ... first entry of each bin
     int n_struct, n_atoms;
     const float *radii;            // [n_atoms] or NULL: cutoff of every SOURCE atom (Def. 3's c_i); NULL: the
@@ -152,7 +151,7 @@ struct WCtx {
     int first, N;
     int nb0, nb1, nb2;     // cell list (cut_bins.cuh): slabs per axis; nb0 == 0: none
     const float4 *xs;      // ... entries in bin order
-    const int *sj, *si, *bs; // ... their atoms; the entry of each atom; first entry of each bin
+    const int *bs;         // ... first entry of each bin
 };
 
 __device__ __forceinline__ void mgs_ctx(WCtx &C, const ScanArgs &A, const CutRec *R, int s) {
@@ -178,8 +177,6 @@ __device__ __forceinline__ void mgs_ctx(WCtx &C, const ScanArgs &A, const CutRec
     const int bins = R->bins;
     C.nb0 = bins >> 24 ? bins & 0xFF : 0; C.nb1 = (bins >> 8) & 0xFF; C.nb2 = (bins >> 16) & 0xFF;
     C.xs = A.xs4 + R->first;
-    C.sj = A.sj + R->first;
-    C.si = A.si + R->first;
     C.bs = A.bin_start + R->first + 2 * s;
     // (an atom far from the origin or not finite: the generic rows, which check every offset)
     if (C.nb0 && C.bs[C.nb0 * C.nb1 * C.nb2 + 1] == 0) C.nb0 = 0;
@@ -443,6 +440,14 @@ __device__ __forceinline__ unsigned mgs_row(const ScanArgs &A, SSmem &ws, PoolSt
     return cnt;
 }
 
+// tau of a hit of a binned row: codes = rint(u_a) mod 4 (2 bits per axis), ki = the source's packed integer
+// parts (cut_prep.cuh), wj = .w of the target's sorted entry (cut_bins.cuh): tau = -rint(u) + k_i - k_j.
+__device__ __forceinline__ void mgs_bin_tau(unsigned codes, int ki, int wj, int tau[3]) {
+    tau[0] = 1 - (int)((codes + 1u) & 3u) + ((ki & 1023) - 512) - (((wj >> 16) & 31) - 16);
+    tau[1] = 1 - (int)(((codes >> 2) + 1u) & 3u) + (((ki >> 10) & 1023) - 512) - (((wj >> 21) & 31) - 16);
+    tau[2] = 1 - (int)(((codes >> 4) + 1u) & 3u) + (((ki >> 20) & 1023) - 512) - (((wj >> 26) & 31) - 16);
+}
+
 // One source row of a structure with a cell list (cut_bins.cuh; one-cell sub-box): the candidates are
 // the atoms of the 5 x 5 columns of bins around the row's bin (5 consecutive slabs of the last axis each:
 // one or, across the periodic wrap, two runs of entries), walked as ONE sequence, lane <-> candidate, so
@@ -490,26 +495,10 @@ __device__ __forceinline__ unsigned mgs_row_binned(const ScanArgs &A, SSmem &ws,
     // A trip only TESTS its candidates (two per lane, v and v + 32, in packed FP32; rint(u) = (u + 1.5 * 2^23)
     // - 1.5 * 2^23, whose low mantissa bits are rint(u) mod 4); the hits go to the stash as (v, rint(u) mod 4)
     // words and become codes, lane <-> hit, when the stash leaves.
-    unsigned *st = reinterpret_cast<unsigned *>(&ws.stash[0]);     // 2 MGS_STASH words
+    uint2 *st = ws.stash;                                          // MGS_STASH hits: (rint(u) mod 4 codes, .w of the entry)
     float4 *buf = reinterpret_cast<float4 *>(&ws.T[0][0]);         // 2 x MGS_CH entries
     const int ki = __float_as_int(xi.w);
     const float nr2 = -__fmul_rn(rci, rci), win = C.win;
-    // the row's own entry as a candidate number: it sits in the centre column
-    int vself;
-    {
-        const int cs = (s0 == 5 ? 2 : 0) * s1 + (s1 == 5 ? 2 : 0), self = C.si[i];
-        const int pa1 = __shfl_sync(0xFFFFFFFFu, a1, cs), pn1 = __shfl_sync(0xFFFFFFFFu, n1, cs),
-                  pa2 = __shfl_sync(0xFFFFFFFFu, a2, cs), pp = __shfl_sync(0xFFFFFFFFu, incl - (n1 + n2), cs);
-        vself = pp + (self >= pa1 && self < pa1 + pn1 ? self - pa1 : pn1 + self - pa2);
-    }
-    // entry of candidate v (hits only)
-    auto entry = [&](int v) {
-        int c = 0;                                                            // last column with tp[c] <= v
-#pragma unroll
-        for (int st = 16; st; st >>= 1) c += tp[c + st] <= v ? st : 0;        // (ncol <= 25: tp[26..31] = total > v)
-        const int r = v - tp[c], n1c = tn1[c];
-        return r < n1c ? ta1[c] + r : ta2[c] + (r - n1c);
-    };
     // the pieces of this lane's column inside chunk [base, base + MGS_CH) -> buffer b
     const int myp = incl - (n1 + n2);
     auto issue = [&](int base, int b) {
@@ -558,47 +547,41 @@ __device__ __forceinline__ unsigned mgs_row_binned(const ScanArgs &A, SSmem &ws,
             const float2 vz = mg_fma2(f2, a8, mg_fma2(f1, a5, mg_fma2(f0, a2v, Z2)));
             const float2 y = mg_fma2(vz, vz, mg_fma2(vy, vy, mg_fma2(vx, vx, nr22)));
             bool hitA = okA && y.x < 0.f, hitB = okB && y.y < 0.f;
-            const unsigned wordA = (unsigned)vA | ((__float_as_uint(m0.x) & 3u) << 16) | ((__float_as_uint(m1.x) & 3u) << 18) |
-                                   ((__float_as_uint(m2.x) & 3u) << 20);
-            const unsigned wordB = (unsigned)vB | ((__float_as_uint(m0.y) & 3u) << 16) | ((__float_as_uint(m1.y) & 3u) << 18) |
-                                   ((__float_as_uint(m2.y) & 3u) << 20);
+            const unsigned wordA = (__float_as_uint(m0.x) & 3u) | ((__float_as_uint(m1.x) & 3u) << 2) | ((__float_as_uint(m2.x) & 3u) << 4);
+            const unsigned wordB = (__float_as_uint(m0.y) & 3u) | ((__float_as_uint(m1.y) & 3u) << 2) | ((__float_as_uint(m2.y) & 3u) << 4);
             if (fminf(fabsf(y.x), fabsf(y.y)) < win) {                        // FP32 cannot decide: Def. 3 in FP64
 #pragma unroll 1
                 for (int h = 0; h < 2; ++h) {
                     const float yh = h ? y.y : y.x;
                     if (!(h ? okB : okA) || !(fabsf(yh) < win)) continue;
-                    const unsigned w = h ? wordB : wordA;
-                    const int idx = entry((int)(w & 0xFFFFu)), kj = __float_as_int((h ? xB : xA).w), j = C.sj[idx];
-                    const int t0 = 1 - (int)(((w >> 16) + 1u) & 3u) + (ki & 1023) - (kj & 1023),
-                              t1 = 1 - (int)(((w >> 18) + 1u) & 3u) + ((ki >> 10) & 1023) - ((kj >> 10) & 1023),
-                              t2 = 1 - (int)(((w >> 20) + 1u) & 3u) + ((ki >> 20) & 1023) - ((kj >> 20) & 1023);
+                    int tau[3];
+                    const int wj = __float_as_int((h ? xB : xA).w);
+                    mgs_bin_tau(h ? wordB : wordA, ki, wj, tau);
+                    const int j = wj & 0xFFFF, t0 = tau[0], t1 = tau[1], t2 = tau[2];
                     double w3[3];
                     const bool e = mg_exact_vec(C.gx + 3 * i, C.gx + 3 * j, t0, t1, t2, C.lat, w3) < (double)rci;
                     if (h) hitB = e; else hitA = e;
                 }
             }
-            hitA = hitA && vA != vself;                                       // (i, i, 0) is not an edge (R3)
-            hitB = hitB && vB != vself;
+            hitA = hitA && (__float_as_int(xA.w) & 0xFFFF) != i;               // (i, i, 0) is not an edge (R3)
+            hitB = hitB && (__float_as_int(xB.w) & 0xFFFF) != i;
             const unsigned balA = __ballot_sync(0xFFFFFFFFu, hitA), balB = __ballot_sync(0xFFFFFFFFu, hitB);
             const unsigned nA = __popc(balA);
-            if (hitA) st[ns + __popc(balA & lt)] = wordA;
-            if (hitB) st[ns + nA + __popc(balB & lt)] = wordB;
+            if (hitA) st[ns + __popc(balA & lt)] = make_uint2(wordA, __float_as_uint(xA.w));
+            if (hitB) st[ns + nA + __popc(balB & lt)] = make_uint2(wordB, __float_as_uint(xB.w));
             ns += nA + __popc(balB);
             cnt += nA + __popc(balB);
-            if (ns <= 2 * MGS_STASH - 64 && v0 + 64 < total) continue;
+            if (ns <= MGS_STASH - 64 && v0 + 64 < total) continue;
         }
         // ---- the stash leaves: entry -> (dst, tau) code, lane <-> hit
         __syncwarp();
         if (PHASE == 0) mgs_pool_reserve(A, ws, P, P.wcount + done + ns, lane);
         for (unsigned x = lane; x < ns; x += 32) {
-            const unsigned w = st[x];
-            const int idx = entry((int)(w & 0xFFFFu));
-            const int kj = __float_as_int(C.xs[idx].w), j = C.sj[idx];
-            int tau[3];                            // the word holds rint(u_a) mod 4; tau = -rint(u) + k_i - k_j
-            tau[0] = 1 - (int)(((w >> 16) + 1u) & 3u) + (ki & 1023) - (kj & 1023);
-            tau[1] = 1 - (int)(((w >> 18) + 1u) & 3u) + ((ki >> 10) & 1023) - ((kj >> 10) & 1023);
-            tau[2] = 1 - (int)(((w >> 20) + 1u) & 3u) + ((ki >> 20) & 1023) - ((kj >> 20) & 1023);
-            // (cut_bins.cuh: the atoms are finite and within 63 cells of the origin, so |tau| <= 127)
+            const uint2 w = st[x];
+            const int j = (int)(w.y & 0xFFFFu);
+            int tau[3];
+            mgs_bin_tau(w.x, ki, (int)w.y, tau);
+            // (cut_bins.cuh: the atoms are finite and within 15 cells of the origin, so |tau| <= 31)
             const uint2 code = make_uint2((unsigned)(C.first + j), ((unsigned)(tau[0] + 128) << 24) |
                                           ((unsigned)(tau[1] + 128) << 16) | ((unsigned)(tau[2] + 128) << 8));
             if (PHASE == 0) {

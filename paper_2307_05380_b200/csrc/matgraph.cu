@@ -45,7 +45,6 @@ struct mg_ctx {
     size_t code_cap = 0;
     float4 *d_xw4 = nullptr;              // [atom64_cap] wrapped coordinates (cut_prep.cuh)
     float4 *d_xs4 = nullptr;              // [atom64_cap] ... in bin order (cut_bins.cuh)
-    int *d_sj = nullptr, *d_si = nullptr; // [atom64_cap] ... the atoms of the entries, the entries of the atoms
     int *d_binstart = nullptr;            // [bin_cap] first entry of each bin
     size_t bin_cap = 0;
     double *d_pos64 = nullptr;            // [atom64_cap, 3]
@@ -196,8 +195,6 @@ extern "C" void mg_destroy(mg_ctx *c) {
     cudaFree(c->d_pos64);
     cudaFree(c->d_xw4);
     cudaFree(c->d_xs4);
-    cudaFree(c->d_sj);
-    cudaFree(c->d_si);
     cudaFree(c->d_binstart);
     cudaFree(c->d_lat64);
     cudaFree(c->d_crec);
@@ -238,13 +235,11 @@ extern "C" mg_status mg_reserve(mg_ctx *c, int32_t n_struct, int32_t n_atoms) {
     }
     if ((size_t)n_atoms + 1 > c->atom64_cap) {
         const size_t cap = (size_t)n_atoms + 1025;
-        cudaFree(c->d_pos64); cudaFree(c->d_xw4); cudaFree(c->d_xs4); cudaFree(c->d_sj); cudaFree(c->d_si);
-        c->d_pos64 = nullptr; c->d_xw4 = nullptr; c->d_xs4 = nullptr; c->d_sj = nullptr; c->d_si = nullptr; c->atom64_cap = 0;
+        cudaFree(c->d_pos64); cudaFree(c->d_xw4); cudaFree(c->d_xs4);
+        c->d_pos64 = nullptr; c->d_xw4 = nullptr; c->d_xs4 = nullptr; c->atom64_cap = 0;
         MG_CUDA(cudaMalloc(&c->d_pos64, cap * 3 * sizeof(double)));
         MG_CUDA(cudaMalloc(&c->d_xw4, cap * sizeof(float4)));
         MG_CUDA(cudaMalloc(&c->d_xs4, cap * sizeof(float4)));
-        MG_CUDA(cudaMalloc(&c->d_sj, cap * sizeof(int)));
-        MG_CUDA(cudaMalloc(&c->d_si, cap * sizeof(int)));
         c->atom64_cap = cap;
     }
     if ((size_t)n_atoms + 2 * (size_t)n_struct + 2 > c->bin_cap) {
@@ -451,13 +446,13 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
         }
         {                                   // K2: the cell lists of the large structures (cut_bins.cuh)
             BinArgs B;
-            B.rec = c->d_crec; B.xw4 = c->d_xw4; B.xs4 = c->d_xs4; B.sj = c->d_sj; B.si = c->d_si; B.bin_start = c->d_binstart;
+            B.rec = c->d_crec; B.xw4 = c->d_xw4; B.xs4 = c->d_xs4; B.bin_start = c->d_binstart;
             B.n_struct = n_struct;
             MG_CUDA(launch_after(c, mg_cut_bin_kernel, n_struct < 65536 ? n_struct : 65536, MGB_BLOCK, 0, st, B));
             c->launches += 1;
         }
         ScanArgs F;
-        F.xs4 = c->d_xs4; F.sj = c->d_sj; F.si = c->d_si; F.bin_start = c->d_binstart;
+        F.xs4 = c->d_xs4; F.bin_start = c->d_binstart;
         F.pos = pos; F.lattice = lat; F.xw4 = c->d_xw4; F.n_struct = n_struct; F.n_atoms = n_atoms; F.radii = radii;
         F.row_ptr = o->row_ptr; F.capacity = o->capacity; F.n_edges = (long long *)o->n_edges;
         F.rec = c->d_crec; F.bpre = c->d_bpre; F.n_blocks = n_blocks;
