@@ -90,8 +90,8 @@ mg_cut_bin_kernel(const BinArgs A) {
                 if (j < j_hi) {
                     const float4 xj = x[j];
                     const int kk = __float_as_int(xj.w);
-                    bad = bad || kk == 0 || abs((kk & 1023) - 512) > 63 || abs(((kk >> 10) & 1023) - 512) > 63 ||
-                          abs(((kk >> 20) & 1023) - 512) > 63;
+                    bad = bad || kk == 0 || abs((kk & 1023) - 512) > 15 || abs(((kk >> 10) & 1023) - 512) > 15 ||
+                          abs(((kk >> 20) & 1023) - 512) > 15;
                     b = mgb_bin(xj, nb0, nb1, nb2);
                 }
                 const unsigned peers = __match_any_sync(0xFFFFFFFFu, b);

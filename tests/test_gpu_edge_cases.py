@@ -364,6 +364,10 @@ def test_cell_list_far_atoms_radii_and_small_pool(mg, monkeypatch):
     far[7, 0] += np.float32(70.0)                                   # 70 cells away: the structure takes the generic rows
     near = C._assemble([(cell, x)])
     b_far = C._assemble([(cell, far)])
+    mid = x.copy()
+    mid[11, 1] += np.float32(20.0)                                  # 20 cells away: outside the 15 cells a sorted entry can pack
+    mid[12, 2] -= np.float32(15.0)                                  # ... and exactly at its edge
+    b_mid = C._assemble([(cell, mid)])
     c = mg.Context(0)
     try:
         pos, lat, ptr = mg.to_device(b_far)
@@ -371,6 +375,11 @@ def test_cell_list_far_atoms_radii_and_small_pool(mg, monkeypatch):
         assert c.mg_check() == 0                                    # |tau| = 70 still fits int8
         rep = check.check_cutoff(b_far, 4.5, got)
         assert rep["extra"] == 0 and rep["missing"] == 0 and np.abs(got["offset"]).max() >= 69
+        pos, lat, ptr = mg.to_device(b_mid)
+        got = c.cutoff_graph(pos, lat, ptr, 4.5, dist=True).to_numpy()
+        assert c.mg_check() == 0
+        rep = check.check_cutoff(b_mid, 4.5, got)
+        assert rep["extra"] == 0 and rep["missing"] == 0 and np.abs(got["offset"]).max() >= 19
         bad = far.copy()
         bad[9, 1] = np.float32(np.nan)
         pos, lat, ptr = mg.to_device(C._assemble([(cell, bad)]))
