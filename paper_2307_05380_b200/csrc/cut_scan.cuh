@@ -73,7 +73,7 @@ struct ScanArgs {
     int4 *slice_row;               // [ceil(capacity / MGS_SLICE) + 1] for edge MGS_SLICE * k: its row, first atom and
                                    // end of the atoms of the row's structure, the structure
     int32_t *atom_struct;          // [n_atoms]
-    double *pos64;                 // [n_atoms, 3]
+    double *pos64;                 // [n_atoms, 4] FP64 copies of the positions, one 32-byte sector per atom
     double *lat64;                 // [n_struct, 9]
     unsigned *dbg;                 // MG_PHASE_CLOCKS builds: globaltimer at the phase boundaries, per-warp cycles
 };
@@ -337,9 +337,9 @@ __device__ __forceinline__ void mgs_row_products(const ScanArgs &A, const WCtx &
     for (int i = ia + lane; i < ib; i += 32) {
         const int g = C.first + i;
         A.atom_struct[g] = s;
-        A.pos64[3 * (size_t)g] = (double)C.gx[3 * i];
-        A.pos64[3 * (size_t)g + 1] = (double)C.gx[3 * i + 1];
-        A.pos64[3 * (size_t)g + 2] = (double)C.gx[3 * i + 2];
+        double2 *p = reinterpret_cast<double2 *>(A.pos64 + 4 * (size_t)g);
+        p[0] = make_double2((double)C.gx[3 * i], (double)C.gx[3 * i + 1]);
+        p[1] = make_double2((double)C.gx[3 * i + 2], 0.0);
     }
     if (ia == 0 && lane < 9) A.lat64[9 * (size_t)s + lane] = (double)C.lat[lane];
 }
@@ -923,8 +923,11 @@ __device__ __forceinline__ void mgs_place_write(const ScanArgs &A, const OutArra
 #pragma unroll
             for (int c = 0; c < 9; ++c) L[c] = pl[c];
             __syncwarp();
-            const double *px = A.pos64 + 3 * (size_t)a_lo;
-            for (int x = lane; x < 3 * win; x += 32) xs[x] = px[x];
+            const double2 *px = reinterpret_cast<const double2 *>(A.pos64 + 4 * (size_t)a_lo);
+            for (int a = lane; a < win; a += 32) {
+                const double2 p0 = px[2 * a], p1 = px[2 * a + 1];
+                xs[3 * a] = p0.x; xs[3 * a + 1] = p0.y; xs[3 * a + 2] = p1.x;
+            }
             __syncwarp();
         }
         float v[4][3], d[4];
@@ -938,10 +941,12 @@ __device__ __forceinline__ void mgs_place_write(const ScanArgs &A, const OutArra
                 mgs_vec(xs + 3 * wi, xs + 3 * wj, tb[y], L, w3);
             } else {                                   // a structure above the window, or another structure
                 double xi[3], xj[3];
-#pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    xi[c] = A.pos64[3 * (size_t)gi[y] + c];
-                    xj[c] = A.pos64[3 * (size_t)gj[y] + c];
+                {                                      // one sector per atom, two 16-byte loads
+                    const double2 *pi = reinterpret_cast<const double2 *>(A.pos64 + 4 * (size_t)gi[y]);
+                    const double2 *pj = reinterpret_cast<const double2 *>(A.pos64 + 4 * (size_t)gj[y]);
+                    const double2 i0 = pi[0], i1 = pi[1], j0 = pj[0], j1 = pj[1];
+                    xi[0] = i0.x; xi[1] = i0.y; xi[2] = i1.x;
+                    xj[0] = j0.x; xj[1] = j0.y; xj[2] = j1.x;
                 }
                 if (wi < (unsigned)nat) mgs_vec(xi, xj, tb[y], L, w3);
                 else {
@@ -1179,9 +1184,12 @@ mg_cutoff_write_kernel(const __grid_constant__ WriteArgs A) {
         if (r0 + 1 + lane <= A.n_atoms) start0 = (long long)__ldg(A.row_ptr + r0 + 1 + lane);
         __syncwarp();
         {
-            const int nx = 3 * min(MGWR_WIN, a_hi - a_lo);
-            const double *px = A.pos64 + 3 * (size_t)a_lo;
-            for (int x = lane; x < nx; x += 32) xs[x] = __ldg(px + x);
+            const int na = min(MGWR_WIN, a_hi - a_lo);
+            const double2 *px = reinterpret_cast<const double2 *>(A.pos64 + 4 * (size_t)a_lo);
+            for (int a = lane; a < na; a += 32) {
+                const double2 p0 = __ldg(px + 2 * a), p1 = __ldg(px + 2 * a + 1);
+                xs[3 * a] = p0.x; xs[3 * a + 1] = p0.y; xs[3 * a + 2] = p1.x;
+            }
         }
 #pragma unroll
         for (int x = 0; x < MGS_SLICE / 32; ++x) cnt[32 * x + lane] = 0;
@@ -1233,8 +1241,8 @@ mg_cutoff_write_kernel(const __grid_constant__ WriteArgs A) {
                 for (int c = 0; c < 9; ++c) L2[c] = __ldg(A.lat64 + 9 * (size_t)s + c);
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
-                    xi[c] = __ldg(A.pos64 + 3 * (size_t)row + c);
-                    xj[c] = __ldg(A.pos64 + 3 * (size_t)gj[y] + c);
+                    xi[c] = __ldg(A.pos64 + 4 * (size_t)row + c);
+                    xj[c] = __ldg(A.pos64 + 4 * (size_t)gj[y] + c);
                 }
                 mgwr_vec(xi, xj, tb[y], L2, w3);
             }

@@ -47,7 +47,7 @@ struct mg_ctx {
     float4 *d_xs4 = nullptr;              // [atom64_cap] ... in bin order (cut_bins.cuh)
     int *d_binstart = nullptr;            // [bin_cap] first entry of each bin
     size_t bin_cap = 0;
-    double *d_pos64 = nullptr;            // [atom64_cap, 3]
+    double *d_pos64 = nullptr;            // [atom64_cap, 4]
     size_t atom64_cap = 0;
     double *d_lat64 = nullptr;            // [lat64_cap, 9]
     size_t lat64_cap = 0;
@@ -237,7 +237,7 @@ extern "C" mg_status mg_reserve(mg_ctx *c, int32_t n_struct, int32_t n_atoms) {
         const size_t cap = (size_t)n_atoms + 1025;
         cudaFree(c->d_pos64); cudaFree(c->d_xw4); cudaFree(c->d_xs4);
         c->d_pos64 = nullptr; c->d_xw4 = nullptr; c->d_xs4 = nullptr; c->atom64_cap = 0;
-        MG_CUDA(cudaMalloc(&c->d_pos64, cap * 3 * sizeof(double)));
+        MG_CUDA(cudaMalloc(&c->d_pos64, cap * 4 * sizeof(double)));
         MG_CUDA(cudaMalloc(&c->d_xw4, cap * sizeof(float4)));
         MG_CUDA(cudaMalloc(&c->d_xs4, cap * sizeof(float4)));
         c->atom64_cap = cap;
