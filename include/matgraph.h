@@ -58,7 +58,8 @@ typedef enum {
     MG_ERR_NONFINITE = 4,
     MG_ERR_OFFSET_RANGE = 5,   /* a search box needs |tau| > 127 (int8 offsets)            */
     MG_ERR_CAPACITY = 6,       /* more edges than mg_edges.capacity (or than 2^31-1)       */
-    MG_ERR_UNSUPPORTED = 7     /* k or structure size outside what this build handles      */
+    MG_ERR_UNSUPPORTED = 7,    /* k or structure size outside what this build handles      */
+    MG_ERR_TOO_LARGE = 8       /* mg_symmetrize_static: sizes beyond its static scratch    */
 } mg_status;
 
 enum { MG_KIND_CUTOFF = 0, MG_KIND_KNN = 1 };
@@ -149,6 +150,28 @@ mg_status mg_knn_graph_host(mg_ctx *ctx, const float *pos, const float *lattice,
  * result (at most twice the edges of `in`), else MG_ERR_CAPACITY surfaces from mg_check with the required
  * count in *out->n_edges.  out->dist needs in->dist.  May grow the workspace on the first call. */
 mg_status mg_symmetrize(mg_ctx *ctx, const mg_edges *in, int32_t n_atoms, const mg_edges *out, void *cuda_stream);
+
+/* mg_symmetrize for callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): the same operation on the same kernels, same arguments and results as mg_symmetrize, but it
+ * needs no mg_ctx and calls no cudaMalloc / cudaFree / allocating library routine.  Its scratch (one flag
+ * byte per input edge, two counters per atom, a status word) lives in ONE file-scope static device array
+ * of about 4.5 MB that every GPU holds from the moment it loads the library until the process exits.
+ *   limits   n_atoms <= MG_STATIC_MAX_ATOMS and in->capacity <= MG_STATIC_MAX_EDGES, else MG_ERR_TOO_LARGE
+ *            (nothing is launched); out->capacity is the caller's and is not limited.
+ *   device   the CUDA device the arrays live on; the call makes it current.  The first call on a device
+ *            looks the array's address up (cudaGetSymbolAddress) and reads the SM count: make that call
+ *            outside a stream capture.
+ *   errors   no status word is reported: *out->n_edges always receives the required edge count, and a
+ *            value above out->capacity means the result was cut off at the capacity (mg_check does not see
+ *            this call).  `in` must be a complete graph (*in->n_edges <= in->capacity).
+ *   sharing  every call on a device uses the same array, which keeps the last call's contents; the call
+ *            clears what must start at zero on `cuda_stream`.  Two calls that overlap on the GPU (different
+ *            streams without an ordering between them, or a captured graph replayed concurrently with
+ *            another call) race on it and give wrong graphs: order them. */
+#define MG_STATIC_MAX_ATOMS 65536
+#define MG_STATIC_MAX_EDGES 4194304
+mg_status mg_symmetrize_static(int32_t device, const mg_edges *in, int32_t n_atoms, const mg_edges *out,
+                               void *cuda_stream);
 
 /* Triplets Gamma_2 (Def. 3; "Triplets generation"): the ordered pairs (a, b), a != b, of
  * edges that share their source.  For source i with edges row_ptr[i] .. row_ptr[i+1]-1 (degree d) the

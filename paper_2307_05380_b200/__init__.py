@@ -23,7 +23,8 @@ MG_MAX_K = 64
 EXPORTS = ["mg_create", "mg_destroy", "mg_reserve", "mg_cutoff_graph", "mg_cutoff_count",
            "mg_knn_graph", "mg_graph_create", "mg_graph_destroy", "mg_update_graph",
            "mg_cutoff_graph_host", "mg_knn_graph_host", "mg_check", "mg_launch_count",
-           "mg_status_string", "mg_set_profile", "mg_profile_read", "mg_symmetrize", "mg_triplets_graph", "mg_cutoff_graph_radii"]
+           "mg_status_string", "mg_set_profile", "mg_profile_read", "mg_symmetrize", "mg_triplets_graph", "mg_cutoff_graph_radii",
+           "mg_symmetrize_static"]
 
 
 class MatGraphError(RuntimeError):
@@ -74,6 +75,7 @@ def _lib():
         lib.mg_profile_read.argtypes = [vp, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(i64)]
         lib.mg_cutoff_graph_radii.argtypes = [vp, vp, vp, vp, i32, i32, vp, ep, vp]
         lib.mg_symmetrize.argtypes = [vp, ep, i32, ep, vp]
+        lib.mg_symmetrize_static.argtypes = [i32, ep, i32, ep, vp]
         lib.mg_triplets_graph.argtypes = [vp, vp, i32, ctypes.POINTER(_Triplets), vp]
         lib.mg_status_string.argtypes = [ctypes.c_int]
         lib.mg_status_string.restype = ctypes.c_char_p
@@ -335,6 +337,21 @@ class Context:
         _, n_atoms = _check_inputs(pos, lattice, struct_ptr)
         out = Edges.allocate(n_atoms, k * n_atoms, pos.device, dist)
         return self.mg_knn_graph(pos, lattice, struct_ptr, k, out)
+
+
+# limits of mg_symmetrize_static (include/matgraph.h)
+MG_STATIC_MAX_ATOMS = 65536
+MG_STATIC_MAX_EDGES = 4194304
+
+
+def mg_symmetrize_static(inp: Edges, n_atoms: int, out: Edges, device: int = 0) -> Edges:
+    """mg_symmetrize without a context and without any allocation by the library (static device scratch;
+    n_atoms <= MG_STATIC_MAX_ATOMS, inp.capacity <= MG_STATIC_MAX_EDGES).  Calls on one device must not
+    overlap on the GPU."""
+    rc = _lib().mg_symmetrize_static(device, ctypes.byref(inp._c()), n_atoms, ctypes.byref(out._c()), _stream())
+    if rc != 0:
+        raise MatGraphError(rc, "mg_symmetrize_static")
+    return out
 
 
 def to_device(batch, device="cuda"):

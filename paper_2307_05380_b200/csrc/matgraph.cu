@@ -5,6 +5,7 @@
 
 #include <cuda_runtime.h>
 #include <math.h>
+#include <mutex>
 #include <new>
 #include <stdlib.h>
 #include <string.h>
@@ -109,6 +110,7 @@ extern "C" const char *mg_status_string(mg_status s) {
         case MG_ERR_OFFSET_RANGE: return "search box needs |tau| > 127";
         case MG_ERR_CAPACITY: return "edge capacity exceeded";
         case MG_ERR_UNSUPPORTED: return "unsupported k or structure size";
+        case MG_ERR_TOO_LARGE: return "more atoms or edges than the static scratch of mg_symmetrize_static holds";
     }
     return "unknown status";
 }
@@ -723,6 +725,69 @@ extern "C" mg_status mg_triplets_graph(mg_ctx *c, const int32_t *row_ptr, int32_
     const int grid = (int)(want < 1 ? 1 : (want > (long long)c->sm_count * 8 ? (long long)c->sm_count * 8 : want));
     MG_CUDA(launch_after(c, mg_trip_emit_kernel, grid, MGO_BLOCK, 0, st, A));
     c->launches += 2;
+    return MG_OK;
+}
+
+// ---- mg_symmetrize without allocation (include/matgraph.h) -------------------------------------------
+// The scratch of the three symmetrize kernels in a file-scope device array: a status word (one 256-byte
+// line), the two counters per atom (extra | fill, packed behind one another for the call's n_atoms) and
+// one flag byte per input edge.  Every GPU that loads the library holds it until the process exits.
+#define MGST_HEAD 256
+#define MGST_COUNTERS (2 * (size_t)MG_STATIC_MAX_ATOMS * sizeof(int) + 512)
+#define MGST_BYTES (MGST_HEAD + MGST_COUNTERS + (size_t)MG_STATIC_MAX_EDGES + 256)
+static __device__ __align__(256) unsigned char mg_static_scratch[MGST_BYTES];
+
+// In host code `mg_static_scratch` is a stand-in, not a device address: the address the kernels get is
+// looked up once per device, with that device current.
+#define MGST_MAX_DEVICES 64
+static std::mutex g_static_lock;
+static unsigned char *g_static_ptr[MGST_MAX_DEVICES];
+static int g_static_sms[MGST_MAX_DEVICES];
+
+extern "C" mg_status mg_symmetrize_static(int32_t device, const mg_edges *in, int32_t n_atoms, const mg_edges *out,
+                                          void *stream) {
+    if (device < 0 || device >= MGST_MAX_DEVICES || n_atoms < 0 || !in || !in->row_ptr || !in->n_edges || in->capacity < 0 ||
+        bad_edges(out, 0))
+        return MG_ERR_INVALID_ARG;
+    if (in->capacity > 0 && (!in->src || !in->dst || !in->offset || !in->vec)) return MG_ERR_INVALID_ARG;
+    if (out->dist && !in->dist) return MG_ERR_INVALID_ARG;
+    if (n_atoms > MG_STATIC_MAX_ATOMS || in->capacity > (long long)MG_STATIC_MAX_EDGES) return MG_ERR_TOO_LARGE;
+    cudaStream_t st = (cudaStream_t)stream;
+    MG_CUDA(cudaSetDevice(device));
+    unsigned char *base;
+    int sms;
+    {
+        std::lock_guard<std::mutex> guard(g_static_lock);
+        if (!g_static_ptr[device]) {
+            void *p = nullptr;
+            int n = 0;
+            MG_CUDA(cudaGetSymbolAddress(&p, mg_static_scratch));
+            MG_CUDA(cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, device));
+            if (!p || n < 1) return MG_ERR_CUDA;
+            g_static_sms[device] = n;
+            g_static_ptr[device] = (unsigned char *)p;
+        }
+        base = g_static_ptr[device];
+        sms = g_static_sms[device];
+    }
+    // the array keeps the last call's contents: status word and both counter arrays start at zero
+    const size_t na = ((size_t)n_atoms + 63) & ~(size_t)63;               // counters of a call: [na] extra | [na] fill
+    MG_CUDA(cudaMemsetAsync(base, 0, MGST_HEAD + 2 * na * sizeof(int), st));
+    SymArgs A;
+    A.row_ptr = in->row_ptr; A.src = in->src; A.dst = in->dst; A.offset = in->offset; A.vec = in->vec; A.dist = in->dist;
+    A.n_edges_in = (const long long *)in->n_edges; A.n_atoms = n_atoms;
+    A.o_row_ptr = out->row_ptr; A.o_src = out->src; A.o_dst = out->dst; A.o_offset = out->offset; A.o_vec = out->vec;
+    A.o_dist = out->dist; A.capacity = out->capacity; A.n_edges_out = (long long *)out->n_edges;
+    A.status = reinterpret_cast<unsigned *>(base);
+    A.extra = reinterpret_cast<int *>(base + MGST_HEAD);
+    A.fill = A.extra + na;
+    A.flag = base + MGST_HEAD + MGST_COUNTERS;       // (every flag the emit kernel reads is written by the flag kernel)
+    long long want = (in->capacity + MGO_BLOCK - 1) / MGO_BLOCK;
+    const int grid = (int)(want < 1 ? 1 : (want > (long long)sms * 16 ? (long long)sms * 16 : want));
+    mg_sym_flag_kernel<<<grid, MGO_BLOCK, 0, st>>>(A);
+    mg_sym_scan_kernel<<<1, MGO_SCAN_BLOCK, 0, st>>>(A);
+    mg_sym_emit_kernel<<<grid, MGO_BLOCK, 0, st>>>(A);
+    MG_CUDA(cudaGetLastError());
     return MG_OK;
 }
 
