@@ -148,7 +148,9 @@ mg_status mg_knn_graph_host(mg_ctx *ctx, const float *pos, const float *lattice,
  * added edges follow them in no particular order.  `in` is any graph this library produced (device
  * arrays, in->n_edges a device scalar; in->capacity bounds the edges read).  out->capacity must hold the
  * result (at most twice the edges of `in`), else MG_ERR_CAPACITY surfaces from mg_check with the required
- * count in *out->n_edges.  out->dist needs in->dist.  May grow the workspace on the first call. */
+ * count in *out->n_edges.  out->dist needs in->dist.  May grow the workspace on the first call.  An `in` whose
+ * own call overflowed (*in->n_edges above in->capacity) is read up to in->capacity and reported as
+ * MG_ERR_CAPACITY by mg_check. */
 mg_status mg_symmetrize(mg_ctx *ctx, const mg_edges *in, int32_t n_atoms, const mg_edges *out, void *cuda_stream);
 
 /* mg_symmetrize for callers that cannot allocate (CUDA graph capture, serving loops, harnesses that forbid
@@ -163,7 +165,7 @@ mg_status mg_symmetrize(mg_ctx *ctx, const mg_edges *in, int32_t n_atoms, const 
  *            outside a stream capture.
  *   errors   no status word is reported: *out->n_edges always receives the required edge count, and a
  *            value above out->capacity means the result was cut off at the capacity (mg_check does not see
- *            this call).  `in` must be a complete graph (*in->n_edges <= in->capacity).
+ *            this call).  An incomplete `in` (*in->n_edges above in->capacity) is read up to in->capacity.
  *   sharing  every call on a device uses the same array, which keeps the last call's contents; the call
  *            clears what must start at zero on `cuda_stream`.  Two calls that overlap on the GPU (different
  *            streams without an ordering between them, or a captured graph replayed concurrently with

@@ -77,6 +77,8 @@ struct SymArgs {
     const int8_t *offset;
     const float *vec, *dist;
     const long long *n_edges_in;
+    long long cap_in;          // edges the input arrays hold: a graph whose own call overflowed (n_edges_in above
+                               // it) is read up to here only and reported (MGS_CAPACITY)
     int n_atoms;
     // output graph
     int32_t *o_row_ptr, *o_src, *o_dst;
@@ -95,14 +97,17 @@ struct SymArgs {
 __global__ void __launch_bounds__(MGO_BLOCK)
 mg_sym_flag_kernel(const SymArgs A) {
     mg_grid_dependency_wait();
-    const long long E = *A.n_edges_in;
+    long long E = *A.n_edges_in;
+    if (E > A.cap_in) {                                    // an incomplete input graph: no read past its arrays
+        E = A.cap_in;
+        if (blockIdx.x == 0 && threadIdx.x == 0) atomicOr(A.status, MGS_CAPACITY);
+    }
     for (long long e = (long long)blockIdx.x * MGO_BLOCK + threadIdx.x; e < E; e += (long long)gridDim.x * MGO_BLOCK) {
         const int i = A.src[e], j = A.dst[e];
         const int t0 = -A.offset[3 * e], t1 = -A.offset[3 * e + 1], t2 = -A.offset[3 * e + 2];
         bool found = false;
-        for (int q = A.row_ptr[j], qe = A.row_ptr[j + 1]; q < qe && !found; ++q)
-            found = A.dst[q] == i && A.offset[3 * (long long)q] == t0 && A.offset[3 * (long long)q + 1] == t1 &&
-                    A.offset[3 * (long long)q + 2] == t2;
+        for (long long q = A.row_ptr[j], qe = min((long long)A.row_ptr[j + 1], E); q < qe && !found; ++q)
+            found = A.dst[q] == i && A.offset[3 * q] == t0 && A.offset[3 * q + 1] == t1 && A.offset[3 * q + 2] == t2;
         A.flag[e] = found ? 0 : 1;
         if (!found) atomicAdd(A.extra + j, 1);
     }
@@ -126,7 +131,7 @@ mg_sym_scan_kernel(const SymArgs A) {
 __global__ void __launch_bounds__(MGO_BLOCK)
 mg_sym_emit_kernel(const SymArgs A) {
     mg_grid_dependency_wait();
-    const long long E = *A.n_edges_in;
+    const long long E = min(*A.n_edges_in, A.cap_in);
     for (long long e = (long long)blockIdx.x * MGO_BLOCK + threadIdx.x; e < E; e += (long long)gridDim.x * MGO_BLOCK) {
         const int i = A.src[e], j = A.dst[e];
         const int8_t t0 = A.offset[3 * e], t1 = A.offset[3 * e + 1], t2 = A.offset[3 * e + 2];

@@ -698,7 +698,7 @@ extern "C" mg_status mg_symmetrize(mg_ctx *c, const mg_edges *in, int32_t n_atom
     MG_CUDA(cudaMemsetAsync(c->d_symcnt, 0, 2 * c->symcnt_cap * sizeof(int), st));
     SymArgs A;
     A.row_ptr = in->row_ptr; A.src = in->src; A.dst = in->dst; A.offset = in->offset; A.vec = in->vec; A.dist = in->dist;
-    A.n_edges_in = (const long long *)in->n_edges; A.n_atoms = n_atoms;
+    A.n_edges_in = (const long long *)in->n_edges; A.cap_in = in->capacity; A.n_atoms = n_atoms;
     A.o_row_ptr = out->row_ptr; A.o_src = out->src; A.o_dst = out->dst; A.o_offset = out->offset; A.o_vec = out->vec;
     A.o_dist = out->dist; A.capacity = out->capacity; A.n_edges_out = (long long *)out->n_edges;
     A.flag = c->d_symflag; A.extra = c->d_symcnt; A.fill = c->d_symcnt + c->symcnt_cap; A.status = c->d_ctl + 4;
@@ -775,7 +775,7 @@ extern "C" mg_status mg_symmetrize_static(int32_t device, const mg_edges *in, in
     MG_CUDA(cudaMemsetAsync(base, 0, MGST_HEAD + 2 * na * sizeof(int), st));
     SymArgs A;
     A.row_ptr = in->row_ptr; A.src = in->src; A.dst = in->dst; A.offset = in->offset; A.vec = in->vec; A.dist = in->dist;
-    A.n_edges_in = (const long long *)in->n_edges; A.n_atoms = n_atoms;
+    A.n_edges_in = (const long long *)in->n_edges; A.cap_in = in->capacity; A.n_atoms = n_atoms;
     A.o_row_ptr = out->row_ptr; A.o_src = out->src; A.o_dst = out->dst; A.o_offset = out->offset; A.o_vec = out->vec;
     A.o_dist = out->dist; A.capacity = out->capacity; A.n_edges_out = (long long *)out->n_edges;
     A.status = reinterpret_cast<unsigned *>(base);

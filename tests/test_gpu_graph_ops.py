@@ -138,3 +138,23 @@ def test_cutoff_graph_radii_constant_equals_cutoff_graph(mg, ctx):
     bad[3] = -1.0
     ctx.mg_cutoff_graph_radii(pos, lat, ptr, bad, out)
     assert ctx.mg_check() == 7                                         # MG_ERR_UNSUPPORTED
+
+
+def test_symmetrize_of_an_incomplete_graph_reads_nothing_past_its_arrays(mg, ctx):
+    # a KNN graph cut off by hand: n_edges says more edges than the arrays hold (what a cutoff call with too
+    # small a capacity leaves behind).  mg_symmetrize reads the edges that are there and reports MG_ERR_CAPACITY.
+    import torch
+    b, k = C.config_batch(1), 12
+    pos, lat, ptr = mg.to_device(b)
+    knn = ctx.knn_graph(pos, lat, ptr, k, dist=True)
+    keep = (k * b.n_atoms) // 3
+    cut = mg.Edges(row_ptr=knn.row_ptr, src=knn.src[:keep].clone(), dst=knn.dst[:keep].clone(),
+                   offset=knn.offset[:keep].clone(), vec=knn.vec[:keep].clone(), dist=knn.dist[:keep].clone(),
+                   n_edges=knn.n_edges, capacity=keep)
+    out = mg.Edges.allocate(b.n_atoms, 2 * k * b.n_atoms, "cuda", dist=True)
+    ctx.mg_symmetrize(cut, b.n_atoms, out)
+    torch.cuda.synchronize()
+    assert ctx.mg_check() == 6                                     # MG_ERR_CAPACITY
+    # and the context is fine afterwards
+    ctx.mg_symmetrize(knn, b.n_atoms, out)
+    assert ctx.mg_check() == 0 and int(out.n_edges.item()) > k * b.n_atoms
