@@ -29,6 +29,9 @@
 #define MG_KNN_ALPHA 1.45f         // KNN: expected images inside the first search radius, in units of k
 #define MG_KNN_RSCALE 1.05f        // ... and the safety factor on that radius
 #endif
+#ifndef MG_KNN_HINT
+#define MG_KNN_HINT 1.08f           // mg_update_graph: search radius in units of the structure's largest k-th distance of the last call
+#endif
 // cost model of the cutoff path, in warp instructions (tuned on config 2, profiles/)
 #ifndef MG_STRUCT_COST
 #define MG_STRUCT_COST 900.f       // staging one structure (latency, both launches)
@@ -151,7 +154,7 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
         if (A.k > 0) {                                 // KNN: radius from the density, or from the last call
             const float hv = A.hint && A.use_hint ? A.hint[s] : 0.f;
             rc = MG_KNN_RSCALE * cbrtf(0.2387324f * (MG_KNN_ALPHA * (float)A.k + 1.f) * (float)vol / (float)max(N, 1));
-            if (hv > 0.f && isfinite(hv)) rc = 1.02f * hv + 1e-3f;
+            if (hv > 0.f && isfinite(hv)) rc = MG_KNN_HINT * hv + 1e-3f;
             if (!(rc > 1e-6f) || !isfinite(rc)) rc = 1.f;
             if (A.hint) A.hint[s] = 0.f;
         }
@@ -193,8 +196,10 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
             const float c = ((float)((mloc + 3) & ~3) * percell + perblock) * (1.f / 32.f) +
                             MG_C_EDGE * lam / (float)N + MG_STRUCT_COST / ((float)N * (float)N);
             // KNN: one launch, no edge stream (constants from a sweep over four seeds of config 2 and config 4)
-            const float ck = ((float)((mloc + 3) & ~3) * MG_KC_CELL + MG_KC_BLOCK) * (1.f / 32.f) + MG_KC_ROW / (float)N +
-                             MG_KC_STRUCT / ((float)N * (float)N);
+            // (a table above 256 cells: one source row at a time, lanes over the cells of each pair's sub-box, about 35
+            // instructions per 32 cells and 80 per pair)
+            const float ck = (mloc > 256 ? (float)mloc * (35.f / 32.f) + 80.f : ((float)((mloc + 3) & ~3) * MG_KC_CELL + MG_KC_BLOCK) * (1.f / 32.f)) +
+                             MG_KC_ROW / (float)N + MG_KC_STRUCT / ((float)N * (float)N);
             // (KNN above the staging limit: warp-per-row growing-radius search, about 40 per pair-cell)
             const float ckb = 40.f * (float)mloc / 32.f + 600.f / (float)N;
             // cutoff, scan kernel (cut_scan.cuh), in cycles a warp spends (fit on BASELINE configs[2], per-warp

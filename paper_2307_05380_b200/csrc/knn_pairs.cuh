@@ -185,6 +185,57 @@ __device__ __noinline__ int mg_knn_find_wide(KnnSmem &ks, const Task &k, const F
     return mg_knn_find<8>(ks, k, F, i0, qa, qb, lane);
 }
 
+// A structure whose table does not fit the warp's shared memory (mloc > MG_TLOC: strongly skewed cells, which have
+// few atoms): ONE source row i at a time, lanes over the CELLS of the pair's sub-box (lane <-> pair would leave all
+// but N lanes idle through thousands of cells), the translation t . L evaluated on the fly with the table's
+// arithmetic.  The row's hits go to out[0 .. cap) (the stash).  Returns their
+// number (hits beyond cap are dropped: the caller checks).
+#define MG_KNN_TILED_MAX 4096      // cells; beyond: the growing-radius routine
+__device__ __noinline__ int mg_knn_find_cells(KnnSmem &ks, const Task &k, const FindCtx &F, int i, int lane,
+                                              unsigned long long *out, int cap) {
+    const WarpSmem &sw = ks.w;
+    const int N = k.natoms, m1 = (F.m >> 8) & 0xFF, m2 = (F.m >> 16) & 0xFF, M12 = m1 * m2;
+    const float inv12 = 1.f / (float)M12, inv2 = 1.f / (float)m2;     // (mloc <= 4096: the float reciprocal is exact)
+    const float r2 = -F.nr2;
+    const unsigned lt = (1u << lane) - 1u;
+    int run = 0;
+    for (int j = 0; j < N; ++j) {
+        const PairLane p = mg_pair_setup(sw, F, true, i, j);          // the same on every lane
+        if (!p.ok) return cap + 1;                                     // offsets outside int8: the growing-radius routine decides (and reports)
+        const unsigned paircode = ((unsigned)(p.l0 + 128) << 24) | ((unsigned)(p.l1 + 128) << 16) |
+                                  ((unsigned)(p.l2 + 128) << 8) | (unsigned)j;
+        // four cells per lane and trip (c0 + lane + 32 u): four independent chains in flight
+        for (int c0 = 0; c0 < F.mloc; c0 += 128) {
+            bool hit[4];
+            unsigned long long key[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int c = c0 + 32 * u + lane;
+                const int t0 = mg_fdiv(c, inv12), r = c - t0 * M12, t1 = mg_fdiv(r, inv2), t2 = r - t1 * m2;
+                const float f0 = (float)t0, f1 = (float)t1, f2 = (float)t2;
+                const float Tx = __fmaf_rn(f2, F.a[6], __fmaf_rn(f1, F.a[3], __fmul_rn(f0, F.a[0])));
+                const float Ty = __fmaf_rn(f2, F.a[7], __fmaf_rn(f1, F.a[4], __fmul_rn(f0, F.a[1])));
+                const float Tz = __fmaf_rn(f2, F.a[8], __fmaf_rn(f1, F.a[5], __fmul_rn(f0, F.a[2])));
+                const float vx = __fadd_rn(p.qx, Tx), vy = __fadd_rn(p.qy, Ty), vz = __fadd_rn(p.qz, Tz);
+                const float d2 = __fmaf_rn(vz, vz, __fmaf_rn(vy, vy, __fmul_rn(vx, vx)));
+                hit[u] = c < F.mloc && d2 < r2 && c != p.self;         // (i, i, 0) is not an edge (R3)
+                key[u] = ((unsigned long long)__float_as_uint(d2) << 32) |
+                         (paircode + (((unsigned)t0 << 24) | ((unsigned)t1 << 16) | ((unsigned)t2 << 8)));
+            }
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const unsigned bal = __ballot_sync(0xFFFFFFFFu, hit[u]);
+                if (hit[u]) {
+                    const int pos = run + __popc(bal & lt);
+                    if (pos < cap) out[pos] = key[u];
+                }
+                run += __popc(bal);
+            }
+        }
+    }
+    return run;
+}
+
 __global__ void __launch_bounds__(MG_BLOCK, 3)
 mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
     mg_grid_dependency_wait();
@@ -210,6 +261,9 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
     mg_warp_range(RC, wid, c0, c1);
     int s, qa;
     MG_KT(0, mg_range_start(RC, c0, s, qa, lane))
+#ifdef MG_PHASE_CLOCKS
+    const int dbg_s0 = s;
+#endif
     for (; s < A.n_struct; ++s, qa = 0) {
         const CutRec *R = A.rec + s;
         int qb;
@@ -247,7 +301,8 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                 const float lim2 = __fmaf_rn(-2.f, win, __fmul_rn(rad, rad));
                 const double lim2d = (double)rad * (double)rad - (double)win;
                 // rows per group: expected hits fit the stash
-                const int rpt = max(1, min(MG_SMALL_MAX_ATOMS, (int)((float)MG_KSTASH / (2.2f * MG_KNN_ALPHA * (float)K + 8.f))));
+                const bool tiled = F.mloc > MG_TLOC && F.mloc <= MG_KNN_TILED_MAX;
+                const int rpt = tiled ? 1 : max(1, min(MG_SMALL_MAX_ATOMS, (int)((float)MG_KSTASH / (2.2f * MG_KNN_ALPHA * (float)K + 8.f))));
                 float dkmax = 0.f;
                 for (int i0 = ia; i0 < ib; i0 += rpt) {
                     const int nr = min(rpt, ib - i0);
@@ -258,7 +313,8 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                     if (F.mloc <= 32) total = mg_knn_find<1>(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
                     else if (F.mloc <= 64) total = mg_knn_find<2>(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
                     else if (F.mloc <= MG_TLOC) total = mg_knn_find_wide(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
-                    else total = MG_KSTASH + 1;                  // table does not fit: row by row below
+                    else if (tiled) { total = mg_knn_find_cells(ks, k, F, i0, lane, ks.stash, MG_KSTASH); if (lane == 0) ks.rowoff[0] = 0; }
+                    else total = MG_KSTASH + 1;                  // a table of thousands of cells: row by row below
 #ifdef MG_PHASE_CLOCKS
                     tk[2] += clock64() - tf_;
                     const long long ts_ = clock64();
@@ -411,6 +467,7 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
     if (A.dbg && lane == 0) {
         for (int x = 0; x < 6; ++x) A.dbg[(size_t)x * A.n_warps + wid] = (unsigned)tk[x];
         A.dbg[(size_t)6 * A.n_warps + wid] = (unsigned)(clock64() - tk_begin);
+        A.dbg[(size_t)7 * A.n_warps + wid] = (unsigned)dbg_s0;
     }
 #endif
 }

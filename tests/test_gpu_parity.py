@@ -331,3 +331,21 @@ def test_knn_inside_a_degenerate_shell(mg, ctx, name, k):
     assert status == 0
     rep = check.check_knn(b, k, got)
     assert rep["n_edges"] == k * b.n_atoms
+
+
+@pytest.mark.parametrize("k", [24, 32])
+def test_knn_sheared_cells_with_tables_above_256_cells(mg, ctx, k):
+    # strongly sheared cells: the per-pair sub-box has hundreds to thousands of cells, the warp's table holds 256.
+    # The pair-lane kernel walks such a structure one source row at a time, the table tile by tile
+    # (mg_knn_find_tiled); above 4096 cells the growing-radius routine takes the rows.  Mixed with ordinary
+    # skewed cells (BASELINE configs[4] family), which hold a few such structures of their own.
+    rng = np.random.default_rng(31)
+    items = []
+    for s, n in ((1.0, 1), (1.0, 3), (0.7, 2), (0.7, 5), (0.5, 1), (0.5, 4), (0.4, 1), (0.33, 2)):
+        cell = np.array([[14.0, 0.0, 0.0], [13.8, s, 0.0], [13.7, 0.5 * s, s]], np.float32)
+        items.append((cell, rng.random((n, 3), dtype=np.float32)))
+    b = C.concat([C.skewed_batch(120, seed=11), C._assemble(items), C.small_batch(6, seed=3)])
+    got, status = _knn(mg, ctx, b, k)
+    assert status == 0
+    rep = check.check_knn(b, k, got)
+    assert rep["n_edges"] == k * b.n_atoms
