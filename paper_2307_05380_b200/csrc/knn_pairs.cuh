@@ -236,6 +236,18 @@ __device__ __noinline__ int mg_knn_find_cells(KnnSmem &ks, const Task &k, const 
     return run;
 }
 
+// Could a pair of the staged structure have offsets outside int8?  l_a = e_a + k_ia - k_ja with -rho_a - 2 < e_a <= 1
+// and the m_a cells from there on must stay within [-127, 127]: certainly so when every atom is within 40 cells of the
+// origin and no axis of the sub-box has more than 40 cells.
+__device__ __forceinline__ bool mg_knn_far(const WarpSmem &sw, const FindCtx &F, int N, int lane) {
+    bool far = (F.m & 0xFF) > 40 || ((F.m >> 8) & 0xFF) > 40 || ((F.m >> 16) & 0xFF) > 40;
+    for (int j = lane; j < N; j += 32) {
+        const int kk = __float_as_int(sw.x[j].w);
+        far = far || abs((kk & 1023) - 512) > 40 || abs(((kk >> 10) & 1023) - 512) > 40 || abs(((kk >> 20) & 1023) - 512) > 40;
+    }
+    return __any_sync(0xFFFFFFFFu, far);
+}
+
 __global__ void __launch_bounds__(MG_BLOCK, 3)
 mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
     mg_grid_dependency_wait();
@@ -287,8 +299,10 @@ mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
                     A.vec[3 * o] = 0.f; A.vec[3 * o + 1] = 0.f; A.vec[3 * o + 2] = 0.f;
                     if (A.dist) A.dist[o] = 0.f;
                 }
-            } else if (F.big) {
-                // above the staging limit: every row by the growing-radius routine (round 1)
+            } else if (F.big || mg_knn_far(sw, F, N, lane)) {
+                // above the staging limit, or atoms so many cells apart that a pair's offsets may leave int8 (the find
+                // gives such a pair no candidates and says nothing): every row by the growing-radius routine, which
+                // walks whole boxes of cells and reports MGS_OFFSET
                 for (int i = ia; i < ib; ++i) mg_knn_row_fallback(ks, A, s, k.first, N, i, lane);
             } else {
                 __syncwarp();

@@ -409,3 +409,21 @@ def test_cell_list_far_atoms_radii_and_small_pool(mg, monkeypatch):
         assert rep["extra"] == 0 and rep["missing"] == 0 and rep["n_edges"] > 3 * 512, rep
     finally:
         c.close()
+
+
+def test_knn_atoms_more_than_127_cells_apart(mg, ctx):
+    # two atoms in a 3 A cube, the second one given 100 / 130 cells along x: the nearest neighbours of atom 0 are images
+    # of atom 1 at 2.6 A, ahead of its own images at 3 A.  At 100 cells their offsets fit int8 and the rows are the
+    # oracle's; at 130 they do not, and the call must say so — k = 6 is the case where atom 0's own six images would
+    # fill the row and hide the missing pair.
+    cell = np.diag([3.0, 3.0, 3.0]).astype(np.float32)
+    for shift, expect in ((100.0, 0), (130.0, 5)):
+        x = np.array([[0.0, 0.0, 0.0], [0.5 + shift, 0.5, 0.5]], np.float32)
+        b = C._assemble([(cell, x)])
+        pos, lat, ptr = mg.to_device(b)
+        for k in (6, 8, 14):
+            got = ctx.knn_graph(pos, lat, ptr, k, dist=True).to_numpy()
+            assert ctx.mg_check() == expect, (shift, k)              # 5: MG_ERR_OFFSET_RANGE
+            if expect == 0:
+                check.check_knn(b, k, got)
+                assert np.abs(got["offset"]).max() >= 100
