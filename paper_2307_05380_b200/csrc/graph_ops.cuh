@@ -3,7 +3,7 @@
 //   symmetric graph (section 3 "Symmetric graph"): the KNN graph is directed; the
 //     symmetric graph adds, for every edge (i, j, tau), the reverse edge (j, i, -tau) unless it is there
 //     already, and keeps edges unique.  Three launches: flag the edges whose reverse is missing and count
-//     them per target row; exclusive scan -> the new row_ptr; copy the old rows and append the new edges.
+//     them per target row; exclusive scan (two launches) -> the new row_ptr; copy the old rows and append the new edges.
 //   triplets (Def. 3: Gamma_2, the pairs of edges that share their source; PAPER.md:131
 //     "Triplets generation"): for a source of degree d the d (d - 1) ordered pairs (a, b), a != b, of its
 //     edges, as two arrays of edge indices, CSR by source.  Two launches: scan of d (d - 1), emit.
@@ -13,57 +13,90 @@
 #define MGO_BLOCK 256
 #define MGO_SCAN_BLOCK 1024
 
-// Exclusive scan of v(r), r in [0, n), by ONE block of MGO_SCAN_BLOCK threads (chunks of the array in
-// turn; n is the number of atoms of a batch: tens of thousands).  out[r] = base(r) + sum_{q < r} v(q),
-// out[n] = base(n) + total; *total_out = out[n].
+// Exclusive scan of v(r), r in [0, n), in two launches of ceil(n / MGO_CHUNK) blocks (no block waits for another):
+//   mgo_chunk_total   block b sums the values of its chunk [b MGO_CHUNK, (b + 1) MGO_CHUNK) -> partial[b];
+//   mgo_chunk_scan    block b adds up the partials before it, scans its chunk (a thread owns MGO_SCAN_ITEMS consecutive
+//                     values) and writes out[r] = base(r) + sum_{q < r} v(q); the last block also out[n] = base(n) +
+//                     total and *total_out.
+// (One block for all rows took 39 us on the 43 578 rows of BASELINE configs[2]: latency, not work.)
 #define MGO_SCAN_ITEMS 8
-template <class V, class B>
-__device__ __forceinline__ void mgo_block_scan(int n, V value, B base, long long *out64, int32_t *out32,
-                                               long long *total_out) {
-    __shared__ long long s_warp[MGO_SCAN_BLOCK / 32];
-    __shared__ long long s_carry;
+#define MGO_CHUNK (MGO_SCAN_BLOCK * MGO_SCAN_ITEMS)
+
+__host__ __device__ __forceinline__ int mgo_scan_blocks(int n) { return n > 0 ? (n + MGO_CHUNK - 1) / MGO_CHUNK : 1; }
+
+// sum of x over the block (valid on thread 0 ... and, after the barrier, in *s_out for all)
+__device__ __forceinline__ long long mgo_block_sum(long long x, long long *s_warp, long long *s_out) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    if (tid == 0) s_carry = 0ll;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xFFFFFFFFu, x, o);
+    if (lane == 0) s_warp[warp] = x;
     __syncthreads();
-    // chunks of MGO_SCAN_BLOCK * MGO_SCAN_ITEMS values: a thread owns MGO_SCAN_ITEMS consecutive ones
-    for (int r0 = 0; r0 < n; r0 += MGO_SCAN_BLOCK * MGO_SCAN_ITEMS) {
-        const int rb = r0 + tid * MGO_SCAN_ITEMS;
-        long long v[MGO_SCAN_ITEMS], own = 0ll;
-#pragma unroll
-        for (int x = 0; x < MGO_SCAN_ITEMS; ++x) {
-            v[x] = rb + x < n ? value(rb + x) : 0ll;
-            own += v[x];
-        }
-        long long incl = own;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const long long t = __shfl_up_sync(0xFFFFFFFFu, incl, o);
-            if (lane >= o) incl += t;
-        }
-        if (lane == 31) s_warp[warp] = incl;
-        __syncthreads();
-        long long woff = 0ll, btotal = 0ll;
-        for (int w = 0; w < MGO_SCAN_BLOCK / 32; ++w) {
-            const long long t = s_warp[w];
-            if (w < warp) woff += t;
-            btotal += t;
-        }
-        long long excl = s_carry + woff + incl - own;
-#pragma unroll
-        for (int x = 0; x < MGO_SCAN_ITEMS; ++x) {
-            const int r = rb + x;
-            if (r < n) {
-                if (out64) out64[r] = base(r) + excl;
-                if (out32) out32[r] = (int32_t)(base(r) + excl);
-            }
-            excl += v[x];
-        }
-        __syncthreads();
-        if (tid == 0) s_carry += btotal;
-        __syncthreads();
-    }
     if (tid == 0) {
-        const long long tot = base(n) + s_carry;
+        long long t = 0ll;
+        for (int w = 0; w < MGO_SCAN_BLOCK / 32; ++w) t += s_warp[w];
+        *s_out = t;
+    }
+    __syncthreads();
+    return *s_out;
+}
+
+template <class V>
+__device__ __forceinline__ void mgo_chunk_total(int n, V value, long long *partial) {
+    __shared__ long long s_warp[MGO_SCAN_BLOCK / 32];
+    __shared__ long long s_sum;
+    const int rb = (int)blockIdx.x * MGO_CHUNK + (int)threadIdx.x * MGO_SCAN_ITEMS;
+    long long own = 0ll;
+#pragma unroll
+    for (int x = 0; x < MGO_SCAN_ITEMS; ++x) own += rb + x < n ? value(rb + x) : 0ll;
+    const long long t = mgo_block_sum(own, s_warp, &s_sum);
+    if (threadIdx.x == 0) partial[blockIdx.x] = t;
+}
+
+template <class V, class B>
+__device__ __forceinline__ void mgo_chunk_scan(int n, V value, B base, const long long *partial, long long *out64,
+                                               int32_t *out32, long long *total_out) {
+    __shared__ long long s_warp[MGO_SCAN_BLOCK / 32];
+    __shared__ long long s_sum;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // the chunks before this one
+    long long before = 0ll;
+    for (int q = tid; q < (int)blockIdx.x; q += MGO_SCAN_BLOCK) before += partial[q];
+    const long long off = mgo_block_sum(before, s_warp, &s_sum);
+    __syncthreads();
+    // this chunk
+    const int rb = (int)blockIdx.x * MGO_CHUNK + tid * MGO_SCAN_ITEMS;
+    long long v[MGO_SCAN_ITEMS], own = 0ll;
+#pragma unroll
+    for (int x = 0; x < MGO_SCAN_ITEMS; ++x) {
+        v[x] = rb + x < n ? value(rb + x) : 0ll;
+        own += v[x];
+    }
+    long long incl = own;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const long long t = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+        if (lane >= o) incl += t;
+    }
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    long long woff = 0ll, btotal = 0ll;
+    for (int w = 0; w < MGO_SCAN_BLOCK / 32; ++w) {
+        const long long t = s_warp[w];
+        if (w < warp) woff += t;
+        btotal += t;
+    }
+    long long excl = off + woff + incl - own;
+#pragma unroll
+    for (int x = 0; x < MGO_SCAN_ITEMS; ++x) {
+        const int r = rb + x;
+        if (r < n) {
+            if (out64) out64[r] = base(r) + excl;
+            if (out32) out32[r] = (int32_t)(base(r) + excl);
+        }
+        excl += v[x];
+    }
+    if (tid == 0 && blockIdx.x == gridDim.x - 1) {
+        const long long tot = base(n) + off + btotal;
         if (out64) out64[n] = tot;
         if (out32) out32[n] = (int32_t)tot;
         *total_out = tot;
@@ -90,6 +123,7 @@ struct SymArgs {
     unsigned char *flag;       // [E_in] 1: the reverse edge is missing
     int *extra;                // [n_atoms] missing reverse edges per target row (zero before the call)
     int *fill;                 // [n_atoms] cursor of the appended edges (zero before the call)
+    long long *part;           // [ceil(n_atoms / MGO_CHUNK)] chunk totals of the scan
     unsigned *status;
 };
 
@@ -114,15 +148,20 @@ mg_sym_flag_kernel(const SymArgs A) {
 }
 
 __global__ void __launch_bounds__(MGO_SCAN_BLOCK)
+mg_sym_part_kernel(const SymArgs A) {
+    mg_grid_dependency_wait();
+    mgo_chunk_total(A.n_atoms, [&](int r) { return (long long)A.extra[r]; }, A.part);
+}
+
+__global__ void __launch_bounds__(MGO_SCAN_BLOCK)
 mg_sym_scan_kernel(const SymArgs A) {
     mg_grid_dependency_wait();
-    long long total = 0ll;
     __shared__ long long s_total;
-    mgo_block_scan(A.n_atoms, [&](int r) { return (long long)A.extra[r]; },
-                   [&](int r) { return (long long)A.row_ptr[r]; }, nullptr, A.o_row_ptr, &s_total);
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        total = s_total;
+    if (threadIdx.x == 0) s_total = -1ll;
+    mgo_chunk_scan(A.n_atoms, [&](int r) { return (long long)A.extra[r]; },
+                   [&](int r) { return (long long)A.row_ptr[r]; }, A.part, nullptr, A.o_row_ptr, &s_total);
+    if (threadIdx.x == 0 && blockIdx.x == gridDim.x - 1) {       // (thread 0 of the last block wrote s_total itself)
+        const long long total = s_total;
         *A.n_edges_out = total;
         if (total > A.capacity || total > 0x7FFFFFFFll) atomicOr(A.status, MGS_CAPACITY);
     }
@@ -165,18 +204,25 @@ struct TripArgs {
     int32_t *edge_a, *edge_b;  // [capacity]
     long long capacity;
     long long *n_triplets;
+    long long *part;           // [ceil(n_atoms / MGO_CHUNK)] chunk totals of the scan
     unsigned *status;
 };
+
+__global__ void __launch_bounds__(MGO_SCAN_BLOCK)
+mg_trip_part_kernel(const TripArgs A) {
+    mg_grid_dependency_wait();
+    mgo_chunk_total(A.n_atoms, [&](int r) { const long long d = A.row_ptr[r + 1] - A.row_ptr[r]; return d * (d - 1); }, A.part);
+}
 
 __global__ void __launch_bounds__(MGO_SCAN_BLOCK)
 mg_trip_scan_kernel(const TripArgs A) {
     mg_grid_dependency_wait();
     __shared__ long long s_total;
-    mgo_block_scan(A.n_atoms,
+    if (threadIdx.x == 0) s_total = -1ll;
+    mgo_chunk_scan(A.n_atoms,
                    [&](int r) { const long long d = A.row_ptr[r + 1] - A.row_ptr[r]; return d * (d - 1); },
-                   [&](int) { return 0ll; }, A.tri_ptr, nullptr, &s_total);
-    __syncthreads();
-    if (threadIdx.x == 0) {
+                   [&](int) { return 0ll; }, A.part, A.tri_ptr, nullptr, &s_total);
+    if (threadIdx.x == 0 && blockIdx.x == gridDim.x - 1) {
         *A.n_triplets = s_total;
         if (s_total > A.capacity) atomicOr(A.status, MGS_CAPACITY);
     }

@@ -58,6 +58,8 @@ struct mg_ctx {
     size_t symflag_cap = 0;
     int *d_symcnt = nullptr;              // [2, symcnt_cap] missing reverse edges per row, append cursors
     size_t symcnt_cap = 0;
+    long long *d_scanpart = nullptr;      // [scanpart_cap] chunk totals of the scans of graph_ops.cuh
+    size_t scanpart_cap = 0;
     CutRec *d_crec = nullptr;             // per-structure records of the cutoff path (cut_prep.cuh)
     unsigned long long *d_bpre = nullptr; // cost prefix over the prep blocks
     size_t crec_cap = 0;
@@ -191,6 +193,7 @@ extern "C" void mg_destroy(mg_ctx *c) {
     cudaFree(c->d_slots);
     cudaFree(c->d_symflag);
     cudaFree(c->d_symcnt);
+    cudaFree(c->d_scanpart);
     cudaFree(c->d_pool);
     cudaFree(c->d_codes);
     cudaFree(c->d_slice_row);
@@ -257,6 +260,13 @@ extern "C" mg_status mg_reserve(mg_ctx *c, int32_t n_struct, int32_t n_atoms) {
         c->d_lat64 = nullptr; c->lat64_cap = 0;
         MG_CUDA(cudaMalloc(&c->d_lat64, cap * 9 * sizeof(double)));
         c->lat64_cap = cap;
+    }
+    if ((size_t)mgo_scan_blocks(n_atoms) > c->scanpart_cap) {
+        const size_t cap = (size_t)mgo_scan_blocks(n_atoms) + 64;
+        cudaFree(c->d_scanpart);
+        c->d_scanpart = nullptr; c->scanpart_cap = 0;
+        MG_CUDA(cudaMalloc(&c->d_scanpart, cap * sizeof(long long)));
+        c->scanpart_cap = cap;
     }
     if ((size_t)n_atoms + 1 > c->rowptr_cap) {
         const size_t cap = (size_t)n_atoms + 1025;
@@ -695,6 +705,13 @@ extern "C" mg_status mg_symmetrize(mg_ctx *c, const mg_edges *in, int32_t n_atom
         MG_CUDA(cudaMalloc(&c->d_symcnt, 2 * cap * sizeof(int)));
         c->symcnt_cap = cap;
     }
+    if ((size_t)mgo_scan_blocks(n_atoms) > c->scanpart_cap) {
+        const size_t cap = (size_t)mgo_scan_blocks(n_atoms) + 64;
+        cudaFree(c->d_scanpart);
+        c->d_scanpart = nullptr; c->scanpart_cap = 0;
+        MG_CUDA(cudaMalloc(&c->d_scanpart, cap * sizeof(long long)));
+        c->scanpart_cap = cap;
+    }
     MG_CUDA(cudaMemsetAsync(c->d_symcnt, 0, 2 * c->symcnt_cap * sizeof(int), st));
     SymArgs A;
     A.row_ptr = in->row_ptr; A.src = in->src; A.dst = in->dst; A.offset = in->offset; A.vec = in->vec; A.dist = in->dist;
@@ -702,12 +719,14 @@ extern "C" mg_status mg_symmetrize(mg_ctx *c, const mg_edges *in, int32_t n_atom
     A.o_row_ptr = out->row_ptr; A.o_src = out->src; A.o_dst = out->dst; A.o_offset = out->offset; A.o_vec = out->vec;
     A.o_dist = out->dist; A.capacity = out->capacity; A.n_edges_out = (long long *)out->n_edges;
     A.flag = c->d_symflag; A.extra = c->d_symcnt; A.fill = c->d_symcnt + c->symcnt_cap; A.status = c->d_ctl + 4;
+    A.part = c->d_scanpart;
     long long want = (in->capacity + MGO_BLOCK - 1) / MGO_BLOCK;
     const int grid = (int)(want < 1 ? 1 : (want > (long long)c->sm_count * 16 ? (long long)c->sm_count * 16 : want));
     MG_CUDA(launch_after(c, mg_sym_flag_kernel, grid, MGO_BLOCK, 0, st, A));
-    MG_CUDA(launch_after(c, mg_sym_scan_kernel, 1, MGO_SCAN_BLOCK, 0, st, A));
+    MG_CUDA(launch_after(c, mg_sym_part_kernel, mgo_scan_blocks(n_atoms), MGO_SCAN_BLOCK, 0, st, A));
+    MG_CUDA(launch_after(c, mg_sym_scan_kernel, mgo_scan_blocks(n_atoms), MGO_SCAN_BLOCK, 0, st, A));
     MG_CUDA(launch_after(c, mg_sym_emit_kernel, grid, MGO_BLOCK, 0, st, A));
-    c->launches += 3;
+    c->launches += 4;
     return MG_OK;
 }
 
@@ -716,15 +735,24 @@ extern "C" mg_status mg_triplets_graph(mg_ctx *c, const int32_t *row_ptr, int32_
     if (out->capacity > 0 && (!out->edge_a || !out->edge_b)) return MG_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)stream;
     MG_CUDA(cudaSetDevice(c->device));
+    if ((size_t)mgo_scan_blocks(n_atoms) > c->scanpart_cap) {
+        const size_t cap = (size_t)mgo_scan_blocks(n_atoms) + 64;
+        cudaFree(c->d_scanpart);
+        c->d_scanpart = nullptr; c->scanpart_cap = 0;
+        MG_CUDA(cudaMalloc(&c->d_scanpart, cap * sizeof(long long)));
+        c->scanpart_cap = cap;
+    }
     TripArgs A;
+    A.part = c->d_scanpart;
     A.row_ptr = row_ptr; A.n_atoms = n_atoms; A.tri_ptr = (long long *)out->tri_ptr;
     A.edge_a = out->edge_a; A.edge_b = out->edge_b; A.capacity = out->capacity;
     A.n_triplets = (long long *)out->n_triplets; A.status = c->d_ctl + 4;
-    MG_CUDA(launch_after(c, mg_trip_scan_kernel, 1, MGO_SCAN_BLOCK, 0, st, A));
+    MG_CUDA(launch_after(c, mg_trip_part_kernel, mgo_scan_blocks(n_atoms), MGO_SCAN_BLOCK, 0, st, A));
+    MG_CUDA(launch_after(c, mg_trip_scan_kernel, mgo_scan_blocks(n_atoms), MGO_SCAN_BLOCK, 0, st, A));
     const long long want = ((long long)n_atoms * 32 + MGO_BLOCK - 1) / MGO_BLOCK;
     const int grid = (int)(want < 1 ? 1 : (want > (long long)c->sm_count * 8 ? (long long)c->sm_count * 8 : want));
     MG_CUDA(launch_after(c, mg_trip_emit_kernel, grid, MGO_BLOCK, 0, st, A));
-    c->launches += 2;
+    c->launches += 3;
     return MG_OK;
 }
 
@@ -733,6 +761,7 @@ extern "C" mg_status mg_triplets_graph(mg_ctx *c, const int32_t *row_ptr, int32_
 // line), the two counters per atom (extra | fill, packed behind one another for the call's n_atoms) and
 // one flag byte per input edge.  Every GPU that loads the library holds it until the process exits.
 #define MGST_HEAD 256
+static_assert(64 + (MG_STATIC_MAX_ATOMS / MGO_CHUNK + 1) * sizeof(long long) <= MGST_HEAD, "the chunk totals fit the header");
 #define MGST_COUNTERS (2 * (size_t)MG_STATIC_MAX_ATOMS * sizeof(int) + 512)
 #define MGST_BYTES (MGST_HEAD + MGST_COUNTERS + (size_t)MG_STATIC_MAX_EDGES + 256)
 static __device__ __align__(256) unsigned char mg_static_scratch[MGST_BYTES];
@@ -779,13 +808,15 @@ extern "C" mg_status mg_symmetrize_static(int32_t device, const mg_edges *in, in
     A.o_row_ptr = out->row_ptr; A.o_src = out->src; A.o_dst = out->dst; A.o_offset = out->offset; A.o_vec = out->vec;
     A.o_dist = out->dist; A.capacity = out->capacity; A.n_edges_out = (long long *)out->n_edges;
     A.status = reinterpret_cast<unsigned *>(base);
+    A.part = reinterpret_cast<long long *>(base + 64);          // (MG_STATIC_MAX_ATOMS / MGO_CHUNK = 8 chunk totals)
     A.extra = reinterpret_cast<int *>(base + MGST_HEAD);
     A.fill = A.extra + na;
     A.flag = base + MGST_HEAD + MGST_COUNTERS;       // (every flag the emit kernel reads is written by the flag kernel)
     long long want = (in->capacity + MGO_BLOCK - 1) / MGO_BLOCK;
     const int grid = (int)(want < 1 ? 1 : (want > (long long)sms * 16 ? (long long)sms * 16 : want));
     mg_sym_flag_kernel<<<grid, MGO_BLOCK, 0, st>>>(A);
-    mg_sym_scan_kernel<<<1, MGO_SCAN_BLOCK, 0, st>>>(A);
+    mg_sym_part_kernel<<<mgo_scan_blocks(n_atoms), MGO_SCAN_BLOCK, 0, st>>>(A);
+    mg_sym_scan_kernel<<<mgo_scan_blocks(n_atoms), MGO_SCAN_BLOCK, 0, st>>>(A);
     mg_sym_emit_kernel<<<grid, MGO_BLOCK, 0, st>>>(A);
     MG_CUDA(cudaGetLastError());
     return MG_OK;

@@ -158,3 +158,43 @@ def test_symmetrize_of_an_incomplete_graph_reads_nothing_past_its_arrays(mg, ctx
     # and the context is fine afterwards
     ctx.mg_symmetrize(knn, b.n_atoms, out)
     assert ctx.mg_check() == 0 and int(out.n_edges.item()) > k * b.n_atoms
+
+
+def test_graph_ops_row_offsets_at_full_size(mg, ctx):
+    # BASELINE configs[2] (43 578 atoms: the scans of graph_ops.cuh run over six chunks of 8192 rows): the row offsets of
+    # both calls against their definitions written in numpy, sampled rows of the triplets against Def. 3's Gamma_2
+    import torch
+    b, k = C.config_batch(2), 12
+    pos, lat, ptr = mg.to_device(b)
+    knn = ctx.knn_graph(pos, lat, ptr, k, dist=True)
+    out = mg.Edges.allocate(b.n_atoms, 2 * k * b.n_atoms, "cuda", dist=True)
+    ctx.mg_symmetrize(knn, b.n_atoms, out)
+    assert ctx.mg_check() == 0
+    kn, got = knn.to_numpy(), out.to_numpy()
+
+    def key(s, d, t):
+        t = t.astype(np.int64) + 128
+        return ((s.astype(np.int64) * b.n_atoms + d.astype(np.int64)) << 24) | (t[:, 0] << 16) | (t[:, 1] << 8) | t[:, 2]
+    fwd = key(kn["src"], kn["dst"], kn["offset"])
+    rev = key(kn["dst"], kn["src"], -kn["offset"].astype(np.int64))
+    missing = ~np.isin(rev, fwd)
+    extra = np.bincount(kn["dst"][missing], minlength=b.n_atoms)        # a missing reverse edge lands in the row of its dst
+    want = np.concatenate([[0], np.cumsum(k + extra)])
+    assert np.array_equal(got["row_ptr"], want) and got["n_edges"] == want[-1]
+    assert np.array_equal(np.sort(key(got["src"], got["dst"], got["offset"])), np.sort(np.concatenate([fwd, rev[missing]])))
+    # triplets of the symmetric graph (rows of different lengths)
+    tri = ctx.mg_triplets_graph(out.row_ptr, b.n_atoms, 1)
+    n_tri = int(tri["n_triplets"])
+    assert ctx.mg_check() == 6                                     # one slot was not enough: MG_ERR_CAPACITY, count known
+    d = np.diff(got["row_ptr"]).astype(np.int64)
+    want_t = np.concatenate([[0], np.cumsum(d * (d - 1))])
+    assert n_tri == want_t[-1]
+    tri = ctx.mg_triplets_graph(out.row_ptr, b.n_atoms, n_tri)
+    assert ctx.mg_check() == 0
+    tp = tri["tri_ptr"].cpu().numpy()
+    assert np.array_equal(tp, want_t)
+    ea, eb = tri["edge_a"].cpu().numpy(), tri["edge_b"].cpu().numpy()
+    for i in (0, 1, 8191, 8192, 8193, 16384, 24575, 32768, b.n_atoms - 1):
+        e0, di = got["row_ptr"][i], int(d[i])
+        pairs = [(e0 + a, e0 + c) for a in range(di) for c in range(di) if a != c]
+        assert list(zip(ea[tp[i]:tp[i + 1]], eb[tp[i]:tp[i + 1]])) == pairs
