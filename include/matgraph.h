@@ -179,7 +179,8 @@ mg_status mg_symmetrize_static(int32_t device, const mg_edges *in, int32_t n_ato
  * edges that share their source.  For source i with edges row_ptr[i] .. row_ptr[i+1]-1 (degree d) the
  * d (d - 1) pairs are edge_a[t], edge_b[t] (edge indices) for tri_ptr[i] <= t < tri_ptr[i+1], ordered by
  * (a, b).  All pointers are device pointers; *n_triplets receives tri_ptr[n_atoms] (also when it exceeds
- * `capacity`: MG_ERR_CAPACITY from mg_check, only triplets below the capacity are written). */
+ * `capacity`: MG_ERR_CAPACITY from mg_check, only triplets below the capacity are written).  Keeps one
+ * partial sum per 8192 atoms in the context: may grow the workspace on the first call (mg_reserve covers it). */
 typedef struct {
     int64_t *tri_ptr;      /* [n_atoms+1]                                        */
     int32_t *edge_a;       /* [capacity] first edge of the pair                  */
