@@ -494,7 +494,14 @@ def run_gpu(args, rank, world, local_rank):
         sym = mg.Edges.allocate(n_atoms, 2 * e_knn, dev, dist=True)
         us_sym = timed(lambda i: ctx.mg_symmetrize(kn, n_atoms, sym), reps=30)
         n_tri = K_NN * (K_NN - 1) * n_atoms
-        us_tri = timed(lambda i: ctx.mg_triplets_graph(kn.row_ptr, n_atoms, n_tri), reps=10)
+        # (outputs allocated once, as a caller in a loop would; the binding's convenience call allocates per call)
+        tri_ptr = torch.empty(n_atoms + 1, dtype=torch.int64, device=dev)
+        tri_a, tri_b = torch.empty(n_tri, dtype=torch.int32, device=dev), torch.empty(n_tri, dtype=torch.int32, device=dev)
+        tri_n = torch.zeros(1, dtype=torch.int64, device=dev)
+        tri_c = mg._Triplets(tri_ptr.data_ptr(), tri_a.data_ptr(), tri_b.data_ptr(), n_tri, tri_n.data_ptr())
+        rp_knn = ctypes.c_void_p(kn.row_ptr.data_ptr())
+        us_tri = timed(lambda i: lib.mg_triplets_graph(h, rp_knn, n_atoms, ctypes.byref(tri_c), st), reps=30)
+        assert int(tri_n.item()) == n_tri
         legs["symmetrize_knn12"] = {"us_per_call": us_sym, "edges_in": int(e_knn), "edges_out": int(sym.n_edges.item())}
         legs["triplets_knn12"] = {"us_per_call": us_tri, "triplets": int(n_tri), "gbs_written": 8.0 * n_tri / us_tri / 1e3}
         # per-atom cutoffs drawn in [2, 6.5] A on the headline batch
