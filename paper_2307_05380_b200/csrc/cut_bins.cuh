@@ -47,13 +47,15 @@ struct BinArgs {
     const float4 *xw4;         // [n_atoms] wrapped coordinates (cut_prep.cuh)
     float4 *xs4;               // [n_atoms] the same, in bin order inside each binned structure
     int *bin_start;            // [n_atoms + 2 n_struct + 2]
+    const int *binlist;        // the structures to sort (written by the prep kernel), ctl[13] of them
+    const unsigned *ctl;
     int n_struct;
 };
 
 #define MGB_BLOCK 512
 #define MGB_HWORDS 24000           // 16-bit counters of a block: warps x (bins + 32)
 
-// One block per structure.  The atoms are cut into W contiguous segments, one per warp (W <= 16, fewer when
+// One block per listed structure.  The atoms are cut into W contiguous segments, one per warp (W <= 16, fewer when
 // the structure has so many bins that W rows of counters do not fit); a warp counts its segment into its
 // own row of 16-bit counters, the block turns the counters into cursors in (bin, warp) order, and every
 // warp scatters its segment in index order: atoms of a bin stay sorted by index, whatever the timing.
@@ -64,7 +66,10 @@ mg_cut_bin_kernel(const BinArgs A) {
     __shared__ int s_wsum[MGB_BLOCK / 32];
     __shared__ int s_carry, s_bad;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    for (int s = blockIdx.x; s < A.n_struct; s += gridDim.x) {
+    const int n_list = min((int)A.ctl[13], A.n_struct);   // (a batch of small cells: zero, every block leaves at once)
+    for (int q = blockIdx.x; q < n_list; q += gridDim.x) {
+        const int s = A.binlist[q];
+        if ((unsigned)s >= (unsigned)A.n_struct) continue;
         const CutRec *R = A.rec + s;
         const int bins = R->bins;
         if (!(bins >> 24)) continue;            // (the same for every thread of the block)

@@ -102,9 +102,11 @@ struct CutPrepArgs {
     float4 *xw4;                   // [n_atoms] or NULL: wrapped fractional coordinates x - floor(x), .w = the integer
                                    // parts packed (mg_wrap_x): written by the blocks after the first n_sblocks ones
     int n_sblocks;                 // blocks that hold structures (the grid may have more: they only wrap coordinates)
+    int *binlist;                  // [n_struct] or NULL: the structures that get a cell list (cut_bins.cuh), in any order;
+                                   // their number in ctl[13] (zero before the call: the scan kernel leaves it so)
     CutRec *rec;                   // [n_struct]
     unsigned long long *bpre;      // [blocks + 1] block sums -> exclusive prefix; [blocks] = total
-    unsigned *ctl;                 // [7] blocks done
+    unsigned *ctl;                 // [7] blocks done, [13] structures with a cell list
     unsigned *status;
 };
 
@@ -216,7 +218,7 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
             // (with a margin far above the FP32 rounding of the slab index), one slab where the five-slab
             // stencil would cover the axis anyway, and no more bins than atoms
             float frac = 1.f;
-            if (A.k == 0 && A.rows_cost && N > MG_SMALL_MAX_ATOMS && mloc == 1) {
+            if (A.k == 0 && A.rows_cost && A.binlist && N > MG_SMALL_MAX_ATOMS && mloc == 1) {
                 int nb[3];
 #pragma unroll
                 for (int a = 0; a < 3; ++a) {
@@ -228,6 +230,10 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
                     nb[a] = nb[a] > MGB_MINSLAB ? nb[a] - 1 : 1;
                 }
                 r.bins = nb[0] | (nb[1] << 8) | (nb[2] << 16) | (1 << 24);
+                {
+                    const unsigned slot = atomicAdd(A.ctl + 13, 1u);
+                    if (slot < (unsigned)A.n_struct) A.binlist[slot] = s;      // (always, unless a failed call left its count behind)
+                }
 #pragma unroll
                 for (int a = 0; a < 3; ++a) frac *= nb[a] > 1 ? 5.f / (float)nb[a] : 1.f;
             }

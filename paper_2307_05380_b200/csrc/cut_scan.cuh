@@ -154,6 +154,7 @@ struct WCtx {
     const int *bs;         // ... first entry of each bin
 };
 
+template <bool BINNED>
 __device__ __forceinline__ void mgs_ctx(WCtx &C, const ScanArgs &A, const CutRec *R, int s) {
     C.lat = A.lattice + 9 * (size_t)s;
 #pragma unroll
@@ -174,7 +175,7 @@ __device__ __forceinline__ void mgs_ctx(WCtx &C, const ScanArgs &A, const CutRec
     C.gx = A.pos + 3 * (size_t)R->first;
     C.xw = A.xw4 + R->first;
     C.cr = A.radii ? A.radii + R->first : nullptr;
-    const int bins = R->bins;
+    const int bins = BINNED ? R->bins : 0;      // (the instance without cell lists: every large structure by the generic rows)
     C.nb0 = bins >> 24 ? bins & 0xFF : 0; C.nb1 = (bins >> 8) & 0xFF; C.nb2 = (bins >> 16) & 0xFF;
     C.xs = A.xs4 + R->first;
     C.bs = A.bin_start + R->first + 2 * s;
@@ -603,7 +604,7 @@ __device__ __forceinline__ unsigned mgs_row_binned(const ScanArgs &A, SSmem &ws,
 //   products of the rows (atom_struct, pos64, lat64); returns the warp's edge count (on every lane).
 // PHASE 1 (list again): for a warp whose codes did not fit the pool: the same walk with the final
 //   offset goff known: row_ptr, slice records and codes go straight to their place.
-template <int PHASE>
+template <int PHASE, bool BINNED>
 __device__ __forceinline__ unsigned long long mgs_walk(SSmem &ws, const ScanArgs &A, const RangeCtx &RC, int rid,
                                                        PoolState &P, int &row_lo, int &row_hi,
                                                        unsigned long long goff, int lane) {
@@ -628,7 +629,7 @@ __device__ __forceinline__ unsigned long long mgs_walk(SSmem &ws, const ScanArgs
         if (ib > ia) {
             const int mloc = R->mloc;
             WCtx C;
-            mgs_ctx(C, A, R, s);
+            mgs_ctx<BINNED>(C, A, R, s);
             if (PHASE == 0) {
                 mgs_row_products(A, C, s, ia, ib, lane);
                 if (row_lo < 0) row_lo = C.first + ia;
@@ -642,7 +643,7 @@ __device__ __forceinline__ unsigned long long mgs_walk(SSmem &ws, const ScanArgs
                 for (int i = ia; i < ib; ++i) {
                     bool anybad = false;
                     if (lane == 0) A.row_ptr[C.first + i] = (int)MGS_HERE;
-                    const unsigned cnt = C.nb0 ? mgs_row_binned<PHASE>(A, ws, P, C, i, goff, lane)
+                    const unsigned cnt = BINNED && C.nb0 ? mgs_row_binned<PHASE>(A, ws, P, C, i, goff, lane)
                                                : mgs_row<PHASE>(A, ws, P, C, i, goff, lane, anybad);
                     if (PHASE == 0) {
                         if (anybad) atomicOr(A.status, __float_as_int(C.xw[i].w) == 0 ? MGS_NONFINITE : MGS_OFFSET);
@@ -931,6 +932,8 @@ __device__ __forceinline__ void mgs_place_write(const ScanArgs &A, const OutArra
             __syncwarp();
         }
         float v[4][3], d[4];
+        double xi[3] = {0.0, 0.0, 0.0};                // position of the source of the lane's last edge outside the window
+        int xi_of = -1;                                // (a lane's four edges are nearly always one row: loaded once)
 #pragma unroll
         for (int y = 0; y < 4; ++y) {
             v[y][0] = v[y][1] = v[y][2] = 0.f; d[y] = 0.f;
@@ -940,12 +943,16 @@ __device__ __forceinline__ void mgs_place_write(const ScanArgs &A, const OutArra
             if (wi < (unsigned)win && wj < (unsigned)win) {
                 mgs_vec(xs + 3 * wi, xs + 3 * wj, tb[y], L, w3);
             } else {                                   // a structure above the window, or another structure
-                double xi[3], xj[3];
+                double xj[3];
                 {                                      // one sector per atom, two 16-byte loads
-                    const double2 *pi = reinterpret_cast<const double2 *>(A.pos64 + 4 * (size_t)gi[y]);
                     const double2 *pj = reinterpret_cast<const double2 *>(A.pos64 + 4 * (size_t)gj[y]);
-                    const double2 i0 = pi[0], i1 = pi[1], j0 = pj[0], j1 = pj[1];
-                    xi[0] = i0.x; xi[1] = i0.y; xi[2] = i1.x;
+                    const double2 j0 = pj[0], j1 = pj[1];
+                    if (gi[y] != xi_of) {
+                        const double2 *pi = reinterpret_cast<const double2 *>(A.pos64 + 4 * (size_t)gi[y]);
+                        const double2 i0 = pi[0], i1 = pi[1];
+                        xi[0] = i0.x; xi[1] = i0.y; xi[2] = i1.x;
+                        xi_of = gi[y];
+                    }
                     xj[0] = j0.x; xj[1] = j0.y; xj[2] = j1.x;
                 }
                 if (wi < (unsigned)nat) mgs_vec(xi, xj, tb[y], L, w3);
@@ -971,6 +978,10 @@ __device__ __forceinline__ void mgs_place_write(const ScanArgs &A, const OutArra
 #ifndef MGS_MIN_CTAS
 #define MGS_MIN_CTAS 5
 #endif
+// BINNED: with the cell-list rows (batches of large structures).  The instance without them is the kernel for
+// everything else that comes this way (per-atom cutoffs on small cells, MATGRAPH_FUSED): the cell-list code costs the
+// pair-lane loops registers (90 against 82 us per call on BASELINE configs[2]).
+template <bool BINNED>
 __global__ void __launch_bounds__(MGS_BLOCK, MGS_MIN_CTAS)
 mg_cutoff_scan_kernel(const __grid_constant__ ScanArgs A) {
     mg_grid_dependency_wait();
@@ -995,7 +1006,7 @@ mg_cutoff_scan_kernel(const __grid_constant__ ScanArgs A) {
         P.wcount = 0u; P.nch = 0; P.ok = true; P.list = ws.chunks[wv];
         int row_lo = -1, row_hi = -1;
         const int rid = wv * n_warps + (int)blockIdx.x * MGS_WARPS + warp;
-        const unsigned wtotal = (unsigned)mgs_walk<0>(ws, A, RC, rid, P, row_lo, row_hi, 0ull, lane);
+        const unsigned wtotal = (unsigned)mgs_walk<0, BINNED>(ws, A, RC, rid, P, row_lo, row_hi, 0ull, lane);
         __syncthreads();                               // (the previous wave's sums have been read)
         if (lane == 0) sm.wsum[warp] = wtotal;
         __syncthreads();
@@ -1072,9 +1083,9 @@ mg_cutoff_scan_kernel(const __grid_constant__ ScanArgs A) {
             const int rid = wv * n_warps + (int)blockIdx.x * MGS_WARPS + warp;
             if (A.write_here) {
                 if (P.ok) mgs_place_write(A, O, ws, P.list, wtotal, row_lo, row_hi, base, lane);
-                else mgs_walk<2>(ws, A, RC, rid, P, row_lo, row_hi, base, lane);
+                else mgs_walk<2, BINNED>(ws, A, RC, rid, P, row_lo, row_hi, base, lane);
             } else if (P.ok) mgs_place(A, P.list, wtotal, row_lo, row_hi, base, lane);
-            else mgs_walk<1>(ws, A, RC, rid, P, row_lo, row_hi, base, lane);
+            else mgs_walk<1, BINNED>(ws, A, RC, rid, P, row_lo, row_hi, base, lane);
         }
         MGS_STAMP(3)
     }
@@ -1103,6 +1114,7 @@ mg_cutoff_scan_kernel(const __grid_constant__ ScanArgs A) {
     if (tid == 0) {
         A.ctl[11] = 0u;
         A.ctl[12] = 0u;
+        A.ctl[13] = 0u;                                // (the list of structures with a cell list: empty for the next call)
         __threadfence();
         *reinterpret_cast<volatile unsigned *>(A.ctl + 10) = epoch;
     }

@@ -47,6 +47,7 @@ struct mg_ctx {
     float4 *d_xw4 = nullptr;              // [atom64_cap] wrapped coordinates (cut_prep.cuh)
     float4 *d_xs4 = nullptr;              // [atom64_cap] ... in bin order (cut_bins.cuh)
     int *d_binstart = nullptr;            // [bin_cap] first entry of each bin
+    int *d_binlist = nullptr;             // [crec_cap] structures with a cell list (written by the prep kernel)
     size_t bin_cap = 0;
     double *d_pos64 = nullptr;            // [atom64_cap, 4]
     size_t atom64_cap = 0;
@@ -163,9 +164,16 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
     c->write_kernel = getenv("MATGRAPH_WRITE_KERNEL") ? 1 : 0;
     c->force_scan = getenv("MATGRAPH_FUSED") ? 1 : 0;
     c->force_legacy = getenv("MATGRAPH_LEGACY") ? 1 : 0;
-    if (cudaFuncSetAttribute(mg_cutoff_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    if (cudaFuncSetAttribute(mg_cutoff_scan_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)sizeof(ScanSmem)) != cudaSuccess ||
+        cudaFuncSetAttribute(mg_cutoff_scan_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)sizeof(ScanSmem)) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->fused_occ, mg_cutoff_scan_kernel, MGS_BLOCK, sizeof(ScanSmem));
+    {                                       // both instances run with the same grid: the smaller of their occupancies
+        int occ_b = 0, occ_p = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_b, mg_cutoff_scan_kernel<true>, MGS_BLOCK, sizeof(ScanSmem));
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_p, mg_cutoff_scan_kernel<false>, MGS_BLOCK, sizeof(ScanSmem));
+        c->fused_occ = occ_b < occ_p ? occ_b : occ_p;
+    }
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->write_occ, mg_cutoff_write_kernel, MGWR_BLOCK, 0);
     if (c->fused_occ < 1 || c->write_occ < 1) { mg_destroy(c); return MG_ERR_CUDA; }
     {
@@ -201,6 +209,7 @@ extern "C" void mg_destroy(mg_ctx *c) {
     cudaFree(c->d_xw4);
     cudaFree(c->d_xs4);
     cudaFree(c->d_binstart);
+    cudaFree(c->d_binlist);
     cudaFree(c->d_lat64);
     cudaFree(c->d_crec);
     cudaFree(c->d_bpre);
@@ -218,9 +227,10 @@ extern "C" mg_status mg_reserve(mg_ctx *c, int32_t n_struct, int32_t n_atoms) {
     MG_CUDA(cudaSetDevice(c->device));
     if ((size_t)n_struct + 1 > c->crec_cap) {
         const size_t cap = (size_t)n_struct + 1025;
-        cudaFree(c->d_crec); cudaFree(c->d_bpre);
-        c->d_crec = nullptr; c->d_bpre = nullptr; c->crec_cap = 0;
+        cudaFree(c->d_crec); cudaFree(c->d_bpre); cudaFree(c->d_binlist);
+        c->d_crec = nullptr; c->d_bpre = nullptr; c->d_binlist = nullptr; c->crec_cap = 0;
         MG_CUDA(cudaMalloc(&c->d_crec, cap * sizeof(CutRec)));
+        MG_CUDA(cudaMalloc(&c->d_binlist, cap * sizeof(int)));
         MG_CUDA(cudaMalloc(&c->d_bpre, (cap / MG_CP_BLOCK + 3) * sizeof(unsigned long long)));
         c->crec_cap = cap;
     }
@@ -421,12 +431,16 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
     // ahead on batches of small cells (BASELINE configs[2]: 73 against 81 us per call), the scan kernel on large
     // structures; MATGRAPH_FUSED=1 / MATGRAPH_LEGACY=1 force one of them.
     const bool use_scan = radii || c->force_scan || (!c->force_legacy && n_struct > 0 && n_atoms / n_struct > MG_SMALL_MAX_ATOMS);
+    // ... and the scan kernel in its instance with cell lists (cut_bins.cuh) for batches of large structures; the other
+    // instance takes a large structure among small ones by its generic rows
+    const bool use_bins = use_scan && n_atoms / n_struct > MG_SMALL_MAX_ATOMS;
     if (prof) { prof_collect(c); cudaEventRecord(c->ev[0], st); }
     {
         CutPrepArgs P;
         P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms; P.r_c = r_c;
         P.k = 0; P.hint = nullptr; P.use_hint = 0; P.rows_cost = use_scan ? 1 : 0;
         P.pos = pos; P.xw4 = use_scan ? c->d_xw4 : nullptr; P.n_sblocks = n_blocks; P.radii = radii;
+        P.binlist = use_bins ? c->d_binlist : nullptr;     // (NULL: no structure gets a cell list)
         P.rec = c->d_crec; P.bpre = c->d_bpre; P.ctl = c->d_ctl; P.status = c->d_ctl + 4;
         // (scan path: extra blocks wrap the coordinates of the batch's atoms)
         const int xblocks = use_scan ? (n_atoms + 8 * MG_CP_BLOCK - 1) / (8 * MG_CP_BLOCK) : 0;
@@ -456,11 +470,12 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
             MG_CUDA(cudaMalloc(&c->d_pool, cap * MGS_CHUNK * sizeof(uint2)));
             c->pool_chunks = cap;
         }
-        {                                   // K2: the cell lists of the large structures (cut_bins.cuh)
+        if (use_bins) {                     // K2: the cell lists of the large structures (cut_bins.cuh)
             BinArgs B;
             B.rec = c->d_crec; B.xw4 = c->d_xw4; B.xs4 = c->d_xs4; B.bin_start = c->d_binstart;
-            B.n_struct = n_struct;
-            MG_CUDA(launch_after(c, mg_cut_bin_kernel, n_struct < 65536 ? n_struct : 65536, MGB_BLOCK, 0, st, B));
+            B.n_struct = n_struct; B.binlist = c->d_binlist; B.ctl = c->d_ctl;
+            const int bgrid = n_struct < 2 * c->sm_count ? n_struct : 2 * c->sm_count;
+            MG_CUDA(launch_after(c, mg_cut_bin_kernel, bgrid, MGB_BLOCK, 0, st, B));
             c->launches += 1;
         }
         ScanArgs F;
@@ -479,11 +494,12 @@ static mg_status launch_cutoff(mg_ctx *c, const float *pos, const float *lat, co
         F.pos64 = c->d_pos64; F.lat64 = c->d_lat64;
         F.dbg = c->d_wclock;
         if (prof) cudaEventRecord(c->ev[1], st);
-        cudaError_t e = launch_after(c, mg_cutoff_scan_kernel, grid, MGS_BLOCK, sizeof(ScanSmem), st, F, c->fused_coop != 0);
+        void (*scan_kernel)(const ScanArgs) = use_bins ? mg_cutoff_scan_kernel<true> : mg_cutoff_scan_kernel<false>;
+        cudaError_t e = launch_after(c, scan_kernel, grid, MGS_BLOCK, sizeof(ScanSmem), st, F, c->fused_coop != 0);
         if (e != cudaSuccess && c->fused_coop) {        // cooperative + programmatic launch refused together
             cudaGetLastError();
             c->fused_coop = 0;
-            e = launch_after(c, mg_cutoff_scan_kernel, grid, MGS_BLOCK, sizeof(ScanSmem), st, F, false);
+            e = launch_after(c, scan_kernel, grid, MGS_BLOCK, sizeof(ScanSmem), st, F, false);
         }
         MG_CUDA(e);
         c->launches += 1;
@@ -579,7 +595,7 @@ static mg_status launch_knn(mg_ctx *c, const float *pos, const float *lat, const
         CutPrepArgs P;
         P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms; P.r_c = 0.f;
         P.k = k; P.hint = hint; P.use_hint = use_hint; P.rows_cost = 0;
-        P.pos = pos; P.xw4 = nullptr; P.n_sblocks = n_blocks; P.radii = nullptr;
+        P.pos = pos; P.xw4 = nullptr; P.n_sblocks = n_blocks; P.radii = nullptr; P.binlist = nullptr;
         P.rec = c->d_crec; P.bpre = c->d_bpre; P.ctl = c->d_ctl; P.status = c->d_ctl + 4;
         MG_CUDA(launch_after(c, mg_cut_prep_kernel, n_blocks, MG_CP_BLOCK, 0, st, P));
         c->launches += 1;
