@@ -51,7 +51,7 @@
 #define MG_CS_EDGE 17.f
 #define MG_CS_STRUCT 4000.f
 #define MG_CS_ROWCELL 25.f
-#define MG_CS_BINCAND 16.f         // binned rows (cut_bins.cuh): per candidate left by the stencil
+#define MG_CS_BINCAND 2.f          // binned rows (cut_bins.cuh): per candidate left by the stencil (swept on configs[3]: 16 / 8 / 4 / 2 / 1 -> 153.3 / 152.0 / 151.3 / 148.6 / 148.9 us)
 #define MG_CS_BINROW 1500.f        // ... per source row (the stencil's table)
 #endif
 // ... and of the KNN launch: per candidate cell, per block of 32 pairs, per source row (selection),
