@@ -84,6 +84,8 @@ typedef struct {
  *                        may use (chunks of the code pool of the one-launch path); beyond it the masks are
  *                        evaluated / the rows listed a second time (tests);
  *   MATGRAPH_FUSED, MATGRAPH_LEGACY  force the one-launch / the two-launch cutoff kernels for every batch;
+ *   MATGRAPH_WRITE_KERNEL  one-launch path: the edge arrays are written by a launch of their own (A/B variant);
+ *   MATGRAPH_NO_COOP     one-launch path: plain instead of cooperative launch (its grid is sized to be resident);
  *   MG_DEBUG             print the CUDA error behind an MG_ERR_CUDA to stderr. */
 mg_status mg_create(mg_ctx **ctx, int device);
 void      mg_destroy(mg_ctx *ctx);

@@ -427,3 +427,31 @@ def test_knn_atoms_more_than_127_cells_apart(mg, ctx):
             if expect == 0:
                 check.check_knn(b, k, got)
                 assert np.abs(got["offset"]).max() >= 100
+
+
+@pytest.mark.parametrize("env", [{"MATGRAPH_NO_PDL": "1"}, {"MATGRAPH_LEGACY": "1"},
+                                 {"MATGRAPH_FUSED": "1", "MATGRAPH_WRITE_KERNEL": "1"},
+                                 {"MATGRAPH_FUSED": "1", "MATGRAPH_NO_COOP": "1"},
+                                 {"MATGRAPH_FUSED": "1", "MATGRAPH_NO_PDL": "1"}])
+def test_launch_knobs_give_the_same_graphs(mg, monkeypatch, env):
+    # the knobs of include/matgraph.h pick other launches for the same graphs: small cells, a supercell (cell list) and a
+    # dense cell in one batch, cutoff and KNN against the oracle under each of them
+    for key, val in env.items():
+        monkeypatch.setenv(key, val)
+    rng = np.random.default_rng(12)
+    dense = C._assemble([(np.diag([3.2, 3.4, 3.6]).astype(np.float32), rng.random((9, 3), dtype=np.float32))])
+    batches = [C.concat([C.small_batch(20, seed=21), dense, C.small_batch(4, seed=22)]), C.supercell_batch(2, seed=3)]
+    c = mg.Context(0)
+    try:
+        for b, rc, k in ((batches[0], 6.0, 12), (batches[1], 5.0, 0)):
+            pos, lat, ptr = mg.to_device(b)
+            got = c.cutoff_graph(pos, lat, ptr, rc, dist=True).to_numpy()
+            assert c.mg_check() == 0
+            rep = check.check_cutoff(b, rc, got)
+            assert rep["extra"] == 0 and rep["missing"] == 0 and rep["n_edges"] > 0, (env, rep)
+            if k:
+                gk = c.knn_graph(pos, lat, ptr, k, dist=True).to_numpy()
+                assert c.mg_check() == 0
+                check.check_knn(b, k, gk)
+    finally:
+        c.close()
