@@ -2,11 +2,11 @@
 //
 //   symmetric graph (section 3 "Symmetric graph"): the KNN graph is directed; the
 //     symmetric graph adds, for every edge (i, j, tau), the reverse edge (j, i, -tau) unless it is there
-//     already, and keeps edges unique.  Three launches: flag the edges whose reverse is missing and count
+//     already, and keeps edges unique.  Four launches: flag the edges whose reverse is missing and count
 //     them per target row; exclusive scan (two launches) -> the new row_ptr; copy the old rows and append the new edges.
 //   triplets (Def. 3: Gamma_2, the pairs of edges that share their source; PAPER.md:131
 //     "Triplets generation"): for a source of degree d the d (d - 1) ordered pairs (a, b), a != b, of its
-//     edges, as two arrays of edge indices, CSR by source.  Two launches: scan of d (d - 1), emit.
+//     edges, as two arrays of edge indices, CSR by source.  Three launches: scan of d (d - 1) (two), emit.
 #pragma once
 #include "common.cuh"
 

@@ -1,5 +1,6 @@
 // knn_pairs.cuh — k-nearest-neighbour multigraph, k <= 32 (structures above MG_SMALL_MAX_ATOMS atoms
-// go row by row through the growing-radius routine of knn_small.cuh).
+// go row by row through the growing-radius routine of knn_small.cuh, and so do structures whose atoms are
+// given more than 40 cells apart: mg_knn_far).
 //
 // Problem: per source the k smallest keys (d, dst, tau_x, tau_y, tau_z) over all periodic images
 // except (i,i,0) (Alg. 2 lines 2-5, made deterministic: DESIGN.md R2, R8).
@@ -10,7 +11,9 @@
 // of source rows (cutoff_pairs.cuh):
 //   find    lane <-> ordered pair (i, j): hit mask over the pair's sub-box (d2 < R^2 in FP32),
 //           hits -> shared-memory stash as 64-bit keys (d2 bits | tau + 128 bytes, j) in (row, j)
-//           order: "evaluate_area" + "concatenate" of Alg. 1-2;
+//           order: "evaluate_area" + "concatenate" of Alg. 1-2.  A sub-box of more than 256 cells
+//           (strongly sheared cells) does not fit the warp's table: one row at a time, lanes over the
+//           cells of each pair's sub-box (mg_knn_find_cells);
 //   select  per source row: bitonic sort of its keys, 32 at a time, keeping the 32 smallest (Alg. 2's
 //           "sort, keep k").  Alg. 1 line 4: if the k-th key is not safely inside R (or fewer than k
 //           images were found) the row is searched again by the growing-radius routine of
