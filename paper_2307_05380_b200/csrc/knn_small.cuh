@@ -1,4 +1,5 @@
-// knn_small.cuh — k-nearest-neighbour multigraph for structures of <= MG_SMALL_MAX_ATOMS atoms.
+// knn_small.cuh — k-nearest-neighbour multigraph by a growing-radius search, one warp per source atom (k up to 64;
+// structures of <= MG_SMALL_MAX_ATOMS atoms are staged in shared memory, larger ones are read in place).
 //
 // Problem: per source the k smallest keys (d, dst, tau_x, tau_y, tau_z) over all periodic images
 // except (i,i,0) (Alg. 2 lines 2-5, made deterministic: DESIGN.md R2, R8).
@@ -313,8 +314,10 @@ mg_knn_small_kernel(const KnnArgs A) {
             }
             continue;
         }
+        // (a structure above the staging limit: cartesian positions evaluated on the fly)
+        const bool big = R.natoms > MG_SMALL_MAX_ATOMS;
         __syncwarp();
-        for (int j = lane; j < R.natoms; j += 32) {
+        for (int j = lane; j < (big ? 0 : R.natoms); j += 32) {
             const float *x = A.pos + 3 * (size_t)(R.first + j);
             const float x0 = x[0], x1 = x[1], x2 = x[2];
             float4 p;
@@ -325,7 +328,7 @@ mg_knn_small_kernel(const KnnArgs A) {
             sp[j] = p;
         }
         __syncwarp();
-        mg_knn_source<KPL>(A, R, lat9, sp, s_buf[warp], i, lane);
+        mg_knn_source<KPL>(A, R, lat9, big ? nullptr : sp, s_buf[warp], i, lane);
     }
     __syncthreads();
     if (tid == 0) {

@@ -58,7 +58,6 @@ mg_prep_kernel(const PrepArgs A) {
             double vol = 0.0, h[3] = {1.0, 1.0, 1.0};
             unsigned err = mg_cell_spacings(lat, &vol, h);
             if (!finite) err |= MGS_NONFINITE;
-            if (N > MG_SMALL_MAX_ATOMS) err |= MGS_UNSUPPORTED;
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
                 r.xmin[a] = N ? lo[a] : 0.f;

@@ -349,3 +349,29 @@ def test_knn_sheared_cells_with_tables_above_256_cells(mg, ctx, k):
     assert status == 0
     rep = check.check_knn(b, k, got)
     assert rep["n_edges"] == k * b.n_atoms
+
+
+@pytest.mark.parametrize("k", [33, 40, 64])
+def test_knn_above_32_neighbours_on_structures_above_64_atoms(mg, ctx, k):
+    # k > 32 takes the warp-per-atom kernel of knn_small.cuh; structures above its staging limit of 64 atoms are read in
+    # place (they used to be refused with MG_ERR_UNSUPPORTED)
+    rng = np.random.default_rng(41)
+    items = []
+    for n, lens in ((100, (9.0, 10.0, 11.0)), (300, (14.0, 15.0, 13.0)), (65, (7.0, 7.5, 8.0))):
+        cell = (np.diag(lens) + rng.uniform(-0.8, 0.8, (3, 3))).astype(np.float32)
+        items.append((cell, rng.random((n, 3), dtype=np.float32)))
+    b = C.concat([C.small_batch(5, seed=51), C._assemble(items), C.small_batch(3, seed=52)])
+    got, status = _knn(mg, ctx, b, k)
+    assert status == 0
+    rep = check.check_knn(b, k, got)
+    assert rep["n_edges"] == k * b.n_atoms
+    # ... and under mg_update_graph (per-atom radius hints), against a fresh call on the moved atoms
+    import torch
+    pos, lat, ptr = mg.to_device(b)
+    graph = ctx.mg_graph_create(mg.MG_KIND_KNN, ptr, b.n_atoms, k=k)
+    out = mg.Edges.allocate(b.n_atoms, k * b.n_atoms, "cuda", dist=True)
+    for t in C.walk(b, 2, seed=9):
+        ctx.mg_update_graph(graph, torch.from_numpy(t.pos).cuda(), torch.from_numpy(t.lattice).cuda(), out)
+        assert ctx.mg_check() == 0
+        check.check_knn(t, k, out.to_numpy())
+    graph.close()
