@@ -251,240 +251,17 @@ __device__ __forceinline__ bool mg_knn_far(const WarpSmem &sw, const FindCtx &F,
     return __any_sync(0xFFFFFFFFu, far);
 }
 
-__global__ void __launch_bounds__(MG_BLOCK, 3)
-mg_knn_pairs_kernel(const __grid_constant__ KnnPairsArgs A) {
-    mg_grid_dependency_wait();
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    KnnSmem &ks = reinterpret_cast<KnnSmem *>(smem_raw)[warp];
-    WarpSmem &sw = ks.w;
-    for (long long t = (long long)blockIdx.x * MG_BLOCK + threadIdx.x; t <= A.n_atoms; t += (long long)gridDim.x * MG_BLOCK)
-        A.row_ptr[t] = (int)((long long)A.k * t);
-    if (blockIdx.x == 0 && threadIdx.x == 0) *A.n_edges = (long long)A.k * A.n_atoms;
-    const int K = A.k;
-    RangeCtx RC;
-    mg_range_init(RC, A.rec, A.bpre, A.n_blocks, A.n_struct, A.n_warps, lane);
-    const int wid = warp * gridDim.x + blockIdx.x;
-#ifdef MG_PHASE_CLOCKS
-    long long tk[6] = {0, 0, 0, 0, 0, 0};
-    const long long tk_begin = clock64();
-#define MG_KT(i, stmt) { const long long t_ = clock64(); stmt; tk[i] += clock64() - t_; }
+// The kernel (knn_pairs_kernel.inc) is compiled twice, in two translation units: here as mg_knn_pairs_kernel for
+// k <= 16 (the headline), in knn_large.cu (which defines MG_KNN_LARGE_TU) as mg_knn_pairs_large_kernel for k > 16, whose
+// rows mostly have 33 .. 64 hits and get a fast path of their own.  Two modules on purpose: with both kernels in one the
+// headline's kernel — same SASS, same place in the module — measured 1 us of 57 slower on cold outputs.
+#ifdef MG_KNN_LARGE_TU
+#define MG_KNN_KERNEL_NAME mg_knn_pairs_large_kernel
+#define MG_KNN_LARGE 1
 #else
-#define MG_KT(i, stmt) { stmt; }
+#define MG_KNN_KERNEL_NAME mg_knn_pairs_kernel
+#define MG_KNN_LARGE 0
 #endif
-    unsigned long long c0, c1;
-    mg_warp_range(RC, wid, c0, c1);
-    int s, qa;
-    MG_KT(0, mg_range_start(RC, c0, s, qa, lane))
-#ifdef MG_PHASE_CLOCKS
-    const int dbg_s0 = s;
-#endif
-    for (; s < A.n_struct; ++s, qa = 0) {
-        const CutRec *R = A.rec + s;
-        int qb;
-        if (!mg_segment(RC, R, s, qa, c1, qb)) break;
-        const int N = R->natoms;
-        // source rows whose first pair lies in [qa, qb)
-        const int ia = N ? (qa + N - 1) / N : 0, ib = N ? (qb + N - 1) / N : 0;
-        Task k;
-        FindCtx F;
-        if (ib > ia) {
-            const float rad = R->radius;
-            bool live_;
-            MG_KT(1, live_ = mg_struct_setup(sw, nullptr, A.pos, A.lattice, A.status, rad, R, s, k, F, lane))
-            if (!live_) {
-                // invalid lattice / positions: placeholder rows (src = dst, zero vec); mg_check reports
-                for (int e = ia * K + lane; e < ib * K; e += 32) {
-                    const long long o = (long long)K * R->first + e;
-                    const int g = R->first + e / K;
-                    A.src[o] = g; A.dst[o] = g;
-                    A.offset[3 * o] = 0; A.offset[3 * o + 1] = 0; A.offset[3 * o + 2] = 0;
-                    A.vec[3 * o] = 0.f; A.vec[3 * o + 1] = 0.f; A.vec[3 * o + 2] = 0.f;
-                    if (A.dist) A.dist[o] = 0.f;
-                }
-            } else if (F.big || mg_knn_far(sw, F, N, lane)) {
-                // above the staging limit, or atoms so many cells apart that a pair's offsets may leave int8 (the find
-                // gives such a pair no candidates and says nothing): every row by the growing-radius routine, which
-                // walks whole boxes of cells and reports MGS_OFFSET
-                for (int i = ia; i < ib; ++i) mg_knn_row_fallback(ks, A, s, k.first, N, i, lane);
-            } else {
-                __syncwarp();
-                for (int j = lane; j < 3 * N; j += 32) (&ks.xd[0][0])[j] = (double)A.pos[3 * (size_t)k.first + j];
-                if (lane < 9) ks.latd[lane] = (double)F.lat[lane];
-                __syncwarp();
-                F.win = 0.f;                                   // no exact threshold decision here
-                // every image with true d2 < R^2 - win is a hit; a k-th key below R^2 - 2 win is safe
-                const float win = 1.1920929e-7f * (2.f * rad * (13.f * R->qmax + 2.f * R->amax_sum) + 4.f * rad * rad);
-                const float lim2 = __fmaf_rn(-2.f, win, __fmul_rn(rad, rad));
-                const double lim2d = (double)rad * (double)rad - (double)win;
-                // rows per group: expected hits fit the stash
-                const bool tiled = F.mloc > MG_TLOC && F.mloc <= MG_KNN_TILED_MAX;
-                const int rpt = tiled ? 1 : max(1, min(MG_SMALL_MAX_ATOMS, (int)((float)MG_KSTASH / (2.2f * MG_KNN_ALPHA * (float)K + 8.f))));
-                float dkmax = 0.f;
-                for (int i0 = ia; i0 < ib; i0 += rpt) {
-                    const int nr = min(rpt, ib - i0);
-                    int total;
-#ifdef MG_PHASE_CLOCKS
-                    const long long tf_ = clock64();
-#endif
-                    if (F.mloc <= 32) total = mg_knn_find<1>(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
-                    else if (F.mloc <= 64) total = mg_knn_find<2>(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
-                    else if (F.mloc <= MG_TLOC) total = mg_knn_find_wide(ks, k, F, i0, i0 * N, (i0 + nr) * N, lane);
-                    else if (tiled) { total = mg_knn_find_cells(ks, k, F, i0, lane, ks.stash, MG_KSTASH); if (lane == 0) ks.rowoff[0] = 0; }
-                    else total = MG_KSTASH + 1;                  // a table of thousands of cells: row by row below
-#ifdef MG_PHASE_CLOCKS
-                    tk[2] += clock64() - tf_;
-                    const long long ts_ = clock64();
-#endif
-                    __syncwarp();
-                    if (lane == 0) ks.rowoff[nr] = total;
-                    __syncwarp();
-                    bool dirty = false;
-                    for (int r = 0; r < nr; ++r) {
-                        const int i = i0 + r, gi = k.first + i;
-                        bool ok = total <= MG_KSTASH;
-                        mg_key key = MG_KEY_INF;
-                        float kth_d2 = 0.f;
-                        if (ok) {
-                            const int b0 = ks.rowoff[r], cnt = ks.rowoff[r + 1] - b0;
-                            ok = cnt >= K;
-                            if (ok && cnt <= 32) {
-                                // fast path: one hit per lane.  A 32-bit bitonic sort of (FP32 d2 with the lane
-                                // in its low 5 bits) brings the hits in near order; the first k plus every hit
-                                // FP32 cannot tell from the k-th get their exact FP64 distance; if they are
-                                // already in the order (d, dst, tau) the lane is the rank, else rank by counting
-                                const mg_key mine = lane < cnt ? ks.stash[b0 + lane] : MG_KEY_INF;
-                                unsigned sk = lane < cnt ? (((unsigned)(mine >> 32) & ~31u) | (unsigned)lane) : 0xFFFFFFFFu;
-                                // (bitonic network in its "flip" form: every exchange gives the minimum to the
-                                // lower lane, so the 15 directions are 5 lane bits kept in predicates)
-#pragma unroll
-                                for (int k2 = 2; k2 <= 32; k2 <<= 1) {
-                                    {
-                                        const unsigned o = __shfl_xor_sync(0xFFFFFFFFu, sk, k2 - 1);
-                                        sk = (lane & (k2 >> 1)) == 0 ? min(sk, o) : max(sk, o);
-                                    }
-#pragma unroll
-                                    for (int jj = k2 >> 2; jj > 0; jj >>= 1) {
-                                        const unsigned o = __shfl_xor_sync(0xFFFFFFFFu, sk, jj);
-                                        sk = (lane & jj) == 0 ? min(sk, o) : max(sk, o);
-                                    }
-                                }
-                                const unsigned tie = __shfl_sync(0xFFFFFFFFu, (unsigned)mine, (int)(sk & 31u));
-                                const float d2q = __uint_as_float(sk & ~31u);
-                                const float d2k = __shfl_sync(0xFFFFFFFFu, d2q, K - 1);
-                                // 2 win: FP32 error of both; 2^-17 d2: the 5 bits given to the lane
-                                const bool sel = lane < cnt && (lane < K || d2q <= __fmaf_rn(d2k, 1.6e-5f, __fmaf_rn(2.f, win, d2k)));
-                                const int nsel = __popc(__ballot_sync(0xFFFFFFFFu, sel));       // sorted: a prefix
-                                const int j = (int)(tie & 0xFFu);
-                                const int t0 = (int)(tie >> 24) - 128, t1 = (int)((tie >> 16) & 0xFFu) - 128,
-                                          t2 = (int)((tie >> 8) & 0xFFu) - 128;
-                                const unsigned ord = ((unsigned)j << 24) | (tie >> 8);
-                                double dd = 1e300, vv[3] = {0.0, 0.0, 0.0};
-                                if (sel)
-                                    dd = mg_knn_exact_d2(ks.xd[i], ks.xd[j], t0, t1, t2, ks.latd, vv);
-                                int rank = lane;
-                                {
-                                    const double nd = __shfl_down_sync(0xFFFFFFFFu, dd, 1);
-                                    const unsigned no = __shfl_down_sync(0xFFFFFFFFu, ord, 1);
-                                    const bool inv = lane + 1 < nsel && (nd < dd || (nd == dd && no < ord));
-                                    if (__any_sync(0xFFFFFFFFu, inv)) {
-                                        rank = 0;
-                                        for (int l = 0; l < nsel; ++l) {
-                                            const double od = __shfl_sync(0xFFFFFFFFu, dd, l);
-                                            const unsigned oo = __shfl_sync(0xFFFFFFFFu, ord, l);
-                                            rank += (od < dd || (od == dd && oo < ord)) ? 1 : 0;
-                                        }
-                                    }
-                                }
-                                if (!sel) rank = 64;
-                                // Alg. 1 line 4: the k-th image must be safely inside the explored radius
-                                const bool settled = rank != K - 1 || dd < lim2d;
-                                if (__all_sync(0xFFFFFFFFu, settled)) {
-                                    if (rank < K) {
-                                        const long long e = (long long)K * gi + rank;
-                                        A.src[e] = gi;
-                                        A.dst[e] = k.first + j;
-                                        A.offset[3 * e] = (int8_t)t0; A.offset[3 * e + 1] = (int8_t)t1;
-                                        A.offset[3 * e + 2] = (int8_t)t2;
-                                        A.vec[3 * e] = (float)vv[0]; A.vec[3 * e + 1] = (float)vv[1];
-                                        A.vec[3 * e + 2] = (float)vv[2];
-                                        if (A.dist) A.dist[e] = __fsqrt_rn((float)dd);
-                                        if (rank == K - 1) dkmax = fmaxf(dkmax, __fsqrt_ru(__double2float_ru(dd)));
-                                    }
-                                    continue;
-                                }
-                                ok = false;
-                            }
-                            if (ok) {
-                                key = mg_sort32(lane < cnt ? ks.stash[b0 + lane] : MG_KEY_INF, lane);
-                                for (int c = 32; c < cnt; c += 32) {
-                                    mg_key keys1[1] = {key};
-                                    mg_knn_merge<1>(keys1, c + lane < cnt ? ks.stash[b0 + c + lane] : MG_KEY_INF, lane);
-                                    key = keys1[0];
-                                }
-                                const mg_key kth = __shfl_sync(0xFFFFFFFFu, key, K - 1);
-                                kth_d2 = __uint_as_float((unsigned)(kth >> 32));
-                                ok = kth != MG_KEY_INF && kth_d2 < lim2;
-                            }
-                        }
-                        if (!ok) {                             // Alg. 1 line 4: not settled inside R
-                            MG_KT(4, mg_knn_row_fallback(ks, A, s, k.first, N, i, lane))
-#ifdef MG_PHASE_CLOCKS
-                            tk[5] += 1;
-#endif
-                            dirty = true;
-                            continue;
-                        }
-                        // exact FP64 distance of the selected entries, final order (d, dst, tau), emit
-                        const unsigned tie = (unsigned)key;    // tau + 128 bytes | j: orders like (dst, tau)... see below
-                        const int j = (int)(tie & 0xFFu);
-                        const int t0 = (int)(tie >> 24) - 128, t1 = (int)((tie >> 16) & 0xFFu) - 128,
-                                  t2 = (int)((tie >> 8) & 0xFFu) - 128;
-                        const unsigned ord = ((unsigned)j << 24) | (tie >> 8);      // (dst, tau_x, tau_y, tau_z)
-                        // entries after the k-th that FP32 cannot tell from it take part in the exact ranking
-                        const bool amb = lane >= K && key != MG_KEY_INF &&
-                                         __uint_as_float((unsigned)(key >> 32)) <= __fmaf_rn(2.f, win, kth_d2);
-                        const int nsel = K + __popc(__ballot_sync(0xFFFFFFFFu, amb));
-                        double dd = 1e300, vv[3] = {0.0, 0.0, 0.0};
-                        if (lane < nsel)
-                            dd = mg_knn_exact_d2(ks.xd[i], ks.xd[j], t0, t1, t2, ks.latd, vv);
-                        int rank = 0;
-                        for (int l = 0; l < nsel; ++l) {
-                            const double od = __shfl_sync(0xFFFFFFFFu, dd, l);
-                            const unsigned oo = __shfl_sync(0xFFFFFFFFu, ord, l);
-                            rank += (od < dd || (od == dd && oo < ord)) ? 1 : 0;
-                        }
-                        if (lane < nsel && rank < K) {
-                            const long long e = (long long)K * gi + rank;
-                            A.src[e] = gi;
-                            A.dst[e] = k.first + j;
-                            A.offset[3 * e] = (int8_t)t0; A.offset[3 * e + 1] = (int8_t)t1; A.offset[3 * e + 2] = (int8_t)t2;
-                            A.vec[3 * e] = (float)vv[0]; A.vec[3 * e + 1] = (float)vv[1]; A.vec[3 * e + 2] = (float)vv[2];
-                            if (A.dist) A.dist[e] = __fsqrt_rn((float)dd);
-                            if (rank == K - 1) dkmax = fmaxf(dkmax, __fsqrt_ru(__double2float_ru(dd)));
-                        }
-                    }
-#ifdef MG_PHASE_CLOCKS
-                    tk[3] += clock64() - ts_;
-#endif
-                    if (dirty && F.mloc <= MG_TLOC) {          // the fallback used the table area as scratch
-                        mg_warp_table(sw, F.a, (F.m >> 8) & 0xFF, (F.m >> 16) & 0xFF, F.mloc, 0, lane);
-                    }
-                }
-                if (A.hint) {
-#pragma unroll
-                    for (int o = 16; o > 0; o >>= 1) dkmax = fmaxf(dkmax, __shfl_xor_sync(0xFFFFFFFFu, dkmax, o));
-                    if (lane == 0 && dkmax > 0.f) atomicMax(reinterpret_cast<int *>(A.hint + s), __float_as_int(dkmax));
-                }
-            }
-        }
-        if (qb < N * N) break;
-    }
-#ifdef MG_PHASE_CLOCKS
-    if (A.dbg && lane == 0) {
-        for (int x = 0; x < 6; ++x) A.dbg[(size_t)x * A.n_warps + wid] = (unsigned)tk[x];
-        A.dbg[(size_t)6 * A.n_warps + wid] = (unsigned)(clock64() - tk_begin);
-        A.dbg[(size_t)7 * A.n_warps + wid] = (unsigned)dbg_s0;
-    }
-#endif
-}
+#include "knn_pairs_kernel.inc"
+#undef MG_KNN_KERNEL_NAME
+#undef MG_KNN_LARGE

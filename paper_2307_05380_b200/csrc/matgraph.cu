@@ -19,6 +19,10 @@
 #include "knn_pairs.cuh"
 #include "graph_ops.cuh"
 
+// the pair-lane KNN kernel for k > 16 is a module of its own (knn_large.cu)
+cudaError_t mg_knn_large_setup(int *occ);
+cudaError_t mg_knn_large_launch(const void *args, size_t args_bytes, int grid, cudaStream_t st, int pdl);
+
 struct mg_ctx {
     int device = 0;
     int sm_count = 0;
@@ -150,6 +154,11 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
     if (cudaFuncSetAttribute(mg_knn_pairs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              (int)(MG_WARPS * sizeof(KnnSmem))) != cudaSuccess) { mg_destroy(c); return MG_ERR_CUDA; }
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->knnp_occ, mg_knn_pairs_kernel, MG_BLOCK, (MG_WARPS * sizeof(KnnSmem)));
+    {                                       // the kernel for k > 16 (knn_large.cu): the same grid for both
+        int occ_l = 0;
+        if (mg_knn_large_setup(&occ_l) != cudaSuccess || occ_l < 1) { mg_destroy(c); return MG_ERR_CUDA; }
+        if (occ_l < c->knnp_occ) c->knnp_occ = occ_l;
+    }
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->knn_occ[0], mg_knn_small_kernel<1>, MG_BLOCK, 0);
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->knn_occ[1], mg_knn_small_kernel<2>, MG_BLOCK, 0);
     {
@@ -612,7 +621,8 @@ static mg_status launch_knn(mg_ctx *c, const float *pos, const float *lat, const
         if (grid > cap_grid) grid = cap_grid;
         A.n_warps = grid * MG_WARPS;
         if (c->profile) cudaEventRecord(c->ev[1], st);
-        MG_CUDA(launch_after(c, mg_knn_pairs_kernel, grid, MG_BLOCK, MG_WARPS * sizeof(KnnSmem), st, A));
+        if (k > 16) MG_CUDA(mg_knn_large_launch(&A, sizeof(A), grid, st, c->pdl));
+        else MG_CUDA(launch_after(c, mg_knn_pairs_kernel, grid, MG_BLOCK, MG_WARPS * sizeof(KnnSmem), st, A));
         c->launches += 1;
         if (c->profile) { cudaEventRecord(c->ev[3], st); c->pend_kind = 1; }
         return MG_OK;
