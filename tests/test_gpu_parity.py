@@ -375,3 +375,18 @@ def test_knn_above_32_neighbours_on_structures_above_64_atoms(mg, ctx, k):
         assert ctx.mg_check() == 0
         check.check_knn(t, k, out.to_numpy())
     graph.close()
+
+
+def test_cutoff_1500_atoms_with_spacings_below_two_cutoffs(mg, ctx):
+    # one structure of 1500 atoms in a cell of 25-27 A, r_c = 14 A: plane spacings below 2 r_c, so an ordered pair has up
+    # to eight candidate images (no minimum-image regime, no cell list): the generic rows of the scan kernel, lanes over
+    # (target, cell); about 1.5 M edges, compared with the oracle edge by edge
+    rng = np.random.default_rng(15)
+    cell = (np.diag([25.0, 26.0, 27.0]) + rng.uniform(-1.5, 1.5, (3, 3))).astype(np.float32)
+    big = C.Batch(pos=rng.random((1500, 3), dtype=np.float32), lattice=cell[None], struct_ptr=np.array([0, 1500], np.int32))
+    b = C.concat([big, C.small_batch(4, seed=17)])
+    got, status = _cutoff(mg, ctx, b, 14.0)
+    assert status == 0
+    rep = check.check_cutoff(b, 14.0, got)
+    assert rep["extra"] == 0 and rep["missing"] == 0 and rep["n_edges"] > 1_000_000, rep
+    assert np.abs(got["offset"]).max() >= 1                      # images of other cells are among the edges
