@@ -472,7 +472,12 @@ def run_gpu(args, rank, world, local_rank):
         legs["config3_cutoff"] = {"workload": f"BASELINE configs[3]: cutoff 8 A, {b3.n_struct} supercells, {b3.n_atoms} atoms",
                                   "us_per_call": us3, "edges": int(e3), "edges_per_s": e3 / (us3 * 1e-6),
                                   "candidates_min_image": float(np.sum(n3 * n3)), "roof_us": roof3, "frac": roof3 / us3}
-        del o3
+        # ... and KNN on the same supercells (knn_bins.cu: a warp per row through the cell list)
+        ok3 = [mg.Edges.allocate(b3.n_atoms, K_NN * b3.n_atoms, dev, dist=True) for _ in range(2)]
+        us3k = timed(lambda i: ctx.mg_knn_graph(p3, l3, s3, K_NN, ok3[i % 2]), reps=20)
+        legs["config3_knn12"] = {"workload": f"KNN k={K_NN} on the supercells of BASELINE configs[3]", "us_per_call": us3k,
+                                 "edges": int(K_NN * b3.n_atoms), "edges_per_s": K_NN * b3.n_atoms / (us3k * 1e-6)}
+        del o3, ok3
 
         # the shape of the paper's Table 1: batch of 256 cells of up to 64 atoms
         bp = C.paper_scale_batch(256)

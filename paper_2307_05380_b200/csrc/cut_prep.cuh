@@ -155,7 +155,12 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
         }
         if (A.k > 0) {                                 // KNN: radius from the density, or from the last call
             const float hv = A.hint && A.use_hint ? A.hint[s] : 0.f;
-            rc = MG_KNN_RSCALE * cbrtf(0.2387324f * (MG_KNN_ALPHA * (float)A.k + 1.f) * (float)vol / (float)max(N, 1));
+            // expected images inside: 1.45 k + 1; in a large structure (a warp per row through the cell list, knn_bins.cu:
+            // a row that comes up short costs a search over all N atoms) k + 4 sqrt(k) + 2 if that is more — for atoms
+            // placed at random the count inside R is about Poisson, and 18 expected leave 5 % of the rows below 12
+            float expect = MG_KNN_ALPHA * (float)A.k + 1.f;
+            if (N > MG_SMALL_MAX_ATOMS) expect = fmaxf(expect, (float)A.k + 4.f * sqrtf((float)A.k) + 2.f);
+            rc = MG_KNN_RSCALE * cbrtf(0.2387324f * expect * (float)vol / (float)max(N, 1));
             if (hv > 0.f && isfinite(hv)) rc = MG_KNN_HINT * hv + 1e-3f;
             if (!(rc > 1e-6f) || !isfinite(rc)) rc = 1.f;
             if (A.hint) A.hint[s] = 0.f;
@@ -218,7 +223,8 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
             // (with a margin far above the FP32 rounding of the slab index), one slab where the five-slab
             // stencil would cover the axis anyway, and no more bins than atoms
             float frac = 1.f;
-            if (A.k == 0 && A.rows_cost && A.binlist && N > MG_SMALL_MAX_ATOMS && mloc == 1) {
+            // (the cutoff graph's scan kernel, and KNN on batches of large structures: knn_bins.cu)
+            if ((A.k > 0 || A.rows_cost) && A.binlist && N > MG_SMALL_MAX_ATOMS && mloc == 1) {
                 int nb[3];
 #pragma unroll
                 for (int a = 0; a < 3; ++a) {

@@ -22,6 +22,10 @@
 // the pair-lane KNN kernel for k > 16 is a module of its own (knn_large.cu)
 cudaError_t mg_knn_large_setup(int *occ);
 cudaError_t mg_knn_large_launch(const void *args, size_t args_bytes, int grid, cudaStream_t st, int pdl);
+// ... and so is the KNN kernel for batches of large structures (knn_bins.cu)
+#include "knn_bins_args.cuh"
+cudaError_t mg_knn_bins_setup(int *occ);
+cudaError_t mg_knn_bins_launch(const KnnBinsArgs *a, int grid, cudaStream_t st, int pdl);
 
 struct mg_ctx {
     int device = 0;
@@ -71,7 +75,7 @@ struct mg_ctx {
     int32_t *d_rowptr_tmp = nullptr;      // for mg_cutoff_count
     size_t rowptr_cap = 0;
     long long *d_count = nullptr;
-    int cutoff_occ = 0, count_occ = 0, knn_occ[2] = {0, 0}, knnp_occ = 0;
+    int cutoff_occ = 0, count_occ = 0, knn_occ[2] = {0, 0}, knnp_occ = 0, knnb_occ = 0;
     int64_t launches = 0;
     int pdl = 1;                          // programmatic dependent launch (MATGRAPH_NO_PDL=1 turns it off)
     int profile = 0;                      // mg_set_profile: events around the kernels of the next calls
@@ -158,6 +162,7 @@ extern "C" mg_status mg_create(mg_ctx **out, int device) {
         int occ_l = 0;
         if (mg_knn_large_setup(&occ_l) != cudaSuccess || occ_l < 1) { mg_destroy(c); return MG_ERR_CUDA; }
         if (occ_l < c->knnp_occ) c->knnp_occ = occ_l;
+        if (mg_knn_bins_setup(&c->knnb_occ) != cudaSuccess || c->knnb_occ < 1) { mg_destroy(c); return MG_ERR_CUDA; }
     }
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->knn_occ[0], mg_knn_small_kernel<1>, MG_BLOCK, 0);
     cudaOccupancyMaxActiveBlocksPerMultiprocessor(&c->knn_occ[1], mg_knn_small_kernel<2>, MG_BLOCK, 0);
@@ -598,6 +603,35 @@ static mg_status launch_knn(mg_ctx *c, const float *pos, const float *lat, const
     MG_CUDA(cudaSetDevice(c->device));
     mg_status rs = mg_reserve(c, n_struct, n_atoms);
     if (rs != MG_OK) return rs;
+    if (k <= 32 && n_struct > 0 && n_atoms / n_struct > MG_SMALL_MAX_ATOMS) {
+        // a batch of large structures: one warp per row through the cell list (knn_bins.cu); four launches: prep (which
+        // also wraps the coordinates and picks the slab counts), the sort by bin, the rows, the reset of the list
+        const int n_blocks = (n_struct + MG_CP_BLOCK - 1) / MG_CP_BLOCK;
+        CutPrepArgs P;
+        P.lattice = lat; P.struct_ptr = sp; P.n_struct = n_struct; P.n_atoms = n_atoms; P.r_c = 0.f;
+        P.k = k; P.hint = hint; P.use_hint = use_hint; P.rows_cost = 0;
+        P.pos = pos; P.xw4 = c->d_xw4; P.n_sblocks = n_blocks; P.radii = nullptr; P.binlist = c->d_binlist;
+        P.rec = c->d_crec; P.bpre = c->d_bpre; P.ctl = c->d_ctl; P.status = c->d_ctl + 4;
+        const int xblocks = (n_atoms + 8 * MG_CP_BLOCK - 1) / (8 * MG_CP_BLOCK);
+        MG_CUDA(launch_after(c, mg_cut_prep_kernel, n_blocks + (xblocks < 1024 ? xblocks : 1024), MG_CP_BLOCK, 0, st, P));
+        BinArgs B;
+        B.rec = c->d_crec; B.xw4 = c->d_xw4; B.xs4 = c->d_xs4; B.bin_start = c->d_binstart;
+        B.n_struct = n_struct; B.binlist = c->d_binlist; B.ctl = c->d_ctl;
+        const int bgrid = n_struct < 2 * c->sm_count ? n_struct : 2 * c->sm_count;
+        MG_CUDA(launch_after(c, mg_cut_bin_kernel, bgrid, MGB_BLOCK, 0, st, B));
+        KnnBinsArgs A;
+        A.pos = pos; A.lattice = lat; A.struct_ptr = sp; A.n_struct = n_struct; A.n_atoms = n_atoms; A.k = k;
+        A.row_ptr = o->row_ptr; A.src = o->src; A.dst = o->dst; A.offset = o->offset; A.vec = o->vec; A.dist = o->dist;
+        A.n_edges = (long long *)o->n_edges; A.hint = hint; A.rec = c->d_crec; A.xw4 = c->d_xw4; A.xs4 = c->d_xs4;
+        A.bin_start = c->d_binstart; A.status = c->d_ctl + 4;
+        int grid = c->sm_count * c->knnb_occ;
+        const int cap_grid = (n_atoms + MG_WARPS - 1) / MG_WARPS;
+        if (grid > cap_grid) grid = cap_grid;
+        MG_CUDA(mg_knn_bins_launch(&A, grid, st, c->pdl));
+        MG_CUDA(cudaMemsetAsync(c->d_ctl + 13, 0, sizeof(unsigned), st));      // (the list of binned structures: empty again)
+        c->launches += 3;
+        return MG_OK;
+    }
     if (k <= 32 && n_struct > 0) {                      // pair-lane kernel (knn_pairs.cuh)
         const int n_blocks = (n_struct + MG_CP_BLOCK - 1) / MG_CP_BLOCK;
         if (c->profile) { prof_collect(c); cudaEventRecord(c->ev[0], st); }

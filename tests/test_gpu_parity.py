@@ -390,3 +390,54 @@ def test_cutoff_1500_atoms_with_spacings_below_two_cutoffs(mg, ctx):
     rep = check.check_cutoff(b, 14.0, got)
     assert rep["extra"] == 0 and rep["missing"] == 0 and rep["n_edges"] > 1_000_000, rep
     assert np.abs(got["offset"]).max() >= 1                      # images of other cells are among the edges
+
+
+def _random_structure(rng, n, lens, jitter=1.0):
+    cell = (np.diag(np.asarray(lens, np.float64)) + rng.uniform(-jitter, jitter, (3, 3))).astype(np.float32)
+    return cell, rng.random((n, 3), dtype=np.float32)
+
+
+@pytest.mark.parametrize("k", [1, 12, 27, 32])
+def test_knn_batches_of_large_structures_through_the_cell_list(mg, ctx, k):
+    # batches whose structures average more than 64 atoms take knn_bins.cu: one warp per row, candidates from the cell list
+    # where the structure has one (large cell, R / h < 1/2), the growing-radius routine for everything else in the batch
+    rng = np.random.default_rng(61 + k)
+    items = [_random_structure(rng, 700, (24.0, 26.0, 22.0)),       # cell list on all axes
+             _random_structure(rng, 400, (40.0, 9.0, 30.0)),        # one short axis: no slabs there
+             _random_structure(rng, 90, (6.0, 6.5, 7.0), 0.3),      # dense: several images per pair, no cell list
+             _random_structure(rng, 3, (4.0, 5.0, 6.0), 0.2),       # a small one among them
+             (np.eye(3, dtype=np.float32), np.zeros((0, 3), np.float32)),   # an empty one
+             _random_structure(rng, 70, (20.0, 21.0, 19.0))]
+    items[5][1][17] += np.float32(16.0)                             # an atom 16 cells away: that structure's cell list is not used
+    items[0][1][:3] = np.array([[0.0, 0.0, 0.0], [1.0 - 2.0 ** -24, 0.5, 0.5], [0.5, 0.0, 1.0 - 2.0 ** -24]], np.float32)
+    b = C._assemble(items)
+    assert b.n_atoms / b.n_struct > 64
+    got, status = _knn(mg, ctx, b, k)
+    assert status == 0
+    rep = check.check_knn(b, k, got)
+    assert rep["n_edges"] == k * b.n_atoms
+
+
+def test_knn_update_graph_on_large_structures(mg, ctx):
+    import torch
+    b = C.config_batch(3, n_struct=3)
+    k = 12
+    pos, lat, ptr = mg.to_device(b)
+    graph = ctx.mg_graph_create(mg.MG_KIND_KNN, ptr, b.n_atoms, k=k)
+    out = mg.Edges.allocate(b.n_atoms, k * b.n_atoms, "cuda", dist=True)
+    for t in C.walk(b, 3, seed=4, sigma=0.004):
+        ctx.mg_update_graph(graph, torch.from_numpy(t.pos).cuda(), torch.from_numpy(t.lattice).cuda(), out)
+        assert ctx.mg_check() == 0
+        check.check_knn(t, k, out.to_numpy())
+    graph.close()
+    # an invalid lattice among large structures: placeholder rows there, the error from mg_check, the others right
+    bad = C.Batch(pos=b.pos, lattice=b.lattice.copy(), struct_ptr=b.struct_ptr)
+    bad.lattice.reshape(-1, 9)[1, :] = 0.0
+    pos, lat, ptr = mg.to_device(bad)
+    g = ctx.knn_graph(pos, lat, ptr, k, dist=True).to_numpy()
+    assert ctx.mg_check() == 3                                     # MG_ERR_SINGULAR_LATTICE
+    lo, hi = bad.struct_ptr[1], bad.struct_ptr[2]
+    assert np.array_equal(g["dst"][k * lo:k * hi], np.repeat(np.arange(lo, hi), k))
+    first = C.Batch(pos=b.pos[:b.struct_ptr[1]], lattice=b.lattice[:1], struct_ptr=b.struct_ptr[:2])
+    ref = oracle.knn_graph(first.pos, first.lattice, first.struct_ptr, k)
+    assert np.array_equal(g["dst"][:k * lo], ref["dst"])
