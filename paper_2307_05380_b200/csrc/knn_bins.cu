@@ -79,14 +79,16 @@ __device__ __forceinline__ int mgkb_find(KnnSmem &ks, const KnnBinsArgs &A, cons
     // mantissa bits are rint(u) mod 4), d2 in FP32
     uint2 *meta = reinterpret_cast<uint2 *>(ks.w.T);
     const unsigned lt = (1u << lane) - 1u;
-    int run = 0, c = 0;
+    int run = 0;
     for (int v0 = 0; v0 < total; v0 += 32) {
         const int v = v0 + lane;
         bool hit = false;
         unsigned long long key = 0ull;
         uint2 m = make_uint2(0u, 0u);
         if (v < total) {
-            while (tp[c + 1] <= v) ++c;                                       // (ncol <= 25: tp[26 .. 31] = total > v)
+            int c = 0;                                                        // the last column with tp[c] <= v
+#pragma unroll
+            for (int st = 16; st; st >>= 1) c += tp[c + st] <= v ? st : 0;    // (ncol <= 25: tp[26 .. 31] = total > v)
             const int r = v - tp[c], n1c = tn1[c];
             const float4 xj = xs[r < n1c ? ta1[c] + r : ta2[c] + (r - n1c)];
             const float u0 = __fsub_rn(xj.x, xi.x), u1 = __fsub_rn(xj.y, xi.y), u2 = __fsub_rn(xj.z, xi.z);
