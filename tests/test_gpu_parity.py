@@ -209,13 +209,14 @@ def test_config4_update_steps(mg, ctx):
     graph.close()
 
 
-def test_update_graph_in_a_cuda_graph(mg, ctx):
+@pytest.mark.parametrize("cfg,n_struct,k,sigma", [(4, 128, 12, 0.02), (4, 128, 24, 0.02), (3, 2, 12, 0.004)])
+def test_update_graph_in_a_cuda_graph(mg, ctx, cfg, n_struct, k, sigma):
     # mg_update_graph allocates nothing and never synchronises: capture one step in a CUDA graph,
     # replay it on new geometry written into the captured input buffers, compare with fresh calls
+    # (the pair-lane kernel, the one for k > 16 in its own module, the one for batches of large structures in its own)
     import torch
-    k = 12
-    b0 = C.config_batch(4, n_struct=128)
-    steps = list(C.walk(b0, 4, seed=3))
+    b0 = C.config_batch(cfg, n_struct=n_struct)
+    steps = list(C.walk(b0, 4, seed=3, sigma=sigma))
     ptr = torch.from_numpy(b0.struct_ptr).cuda()
     pos_buf = torch.from_numpy(steps[0].pos).cuda()
     lat_buf = torch.from_numpy(steps[0].lattice).cuda()
