@@ -1,5 +1,6 @@
 """Randomised parity against the oracle, fixed seeds: inputs no hand-written case thought of.  Three generators —
-large structures for the cutoff graph (cell list and generic rows), sheared / shifted / tiny cells for KNN, and
+large structures for the cutoff graph (cell list and generic rows), sheared / shifted / tiny cells and batches of large
+structures for KNN, and
 whole batches through every entry point (cutoff, per-atom cutoffs, KNN, symmetrize, triplets, update sequences)."""
 import numpy as np
 import pytest
@@ -76,6 +77,38 @@ def test_soak_knn_sheared_and_shifted_cells(mg, ctx, seed):
             if mode == 2: x = (x + rng.integers(-30, 31, size=(n, 3))).astype(np.float32)
             if mode == 3: x[0] += np.float32(rng.integers(41, 90))      # beyond the 40-cell guard of the pair-lane kernel
             items.append((cell, x.astype(np.float32)))
+        b = C._assemble(items)
+        pos, lat, ptr = mg.to_device(b)
+        got = ctx.knn_graph(pos, lat, ptr, k, dist=True).to_numpy()
+        assert ctx.mg_check() == 0, (seed, case, k)
+        check.check_knn(b, k, got)
+
+
+@pytest.mark.parametrize("seed", [401, 402])
+def test_soak_knn_batches_of_large_structures(mg, ctx, seed):
+    # batches that average more than 64 atoms per structure: a warp per row through the cell list (knn_bins.cu), with the
+    # densities, cell shapes and coordinate ranges that decide whether a structure has one, and a dense cluster whose rows
+    # overflow the warp's hit buffer
+    rng = np.random.default_rng(seed)
+    for case in range(10):
+        items = []
+        k = int(rng.choice([1, 2, 6, 12, 20, 32]))
+        for s in range(int(rng.integers(1, 4))):
+            n = int(rng.integers(65, 500))
+            side = (n / float(rng.uniform(0.02, 0.12))) ** (1 / 3)
+            lens = side * rng.uniform(0.6, 1.6, 3)
+            ang = rng.uniform(70, 110, 3)
+            cell = C.cell_from_parameters(lens[0], lens[1], lens[2], ang[0], ang[1], ang[2])
+            cell = np.asarray(cell if cell is not None else np.diag(lens), np.float32)
+            x = rng.random((n, 3), dtype=np.float32)
+            mode = rng.integers(0, 5)
+            if mode == 1: x = (x * np.float32(3.0) - np.float32(1.0)).astype(np.float32)
+            if mode == 2: x[: n // 4] = np.round(x[: n // 4] * 8) / 8
+            if mode == 3: x = (x + np.float32(rng.integers(-14, 15))).astype(np.float32)
+            if mode == 4: x[: n // 3] = x[0] + rng.normal(0, 0.01, (n // 3, 3)).astype(np.float32)
+            items.append((cell, x.astype(np.float32)))
+        if rng.random() < 0.3:
+            items.append(C.small_crystal(int(rng.integers(1 << 30)), 0))
         b = C._assemble(items)
         pos, lat, ptr = mg.to_device(b)
         got = ctx.knn_graph(pos, lat, ptr, k, dist=True).to_numpy()
