@@ -159,7 +159,7 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
             // a row that comes up short costs a search over all N atoms) k + 4 sqrt(k) + 2 if that is more — for atoms
             // placed at random the count inside R is about Poisson, and 18 expected leave 5 % of the rows below 12
             float expect = MG_KNN_ALPHA * (float)A.k + 1.f;
-            if (N > MG_SMALL_MAX_ATOMS) expect = fmaxf(expect, (float)A.k + 4.f * sqrtf((float)A.k) + 2.f);
+            if (N > MG_SMALL_MAX_ATOMS || A.binlist) expect = fmaxf(expect, (float)A.k + 4.f * sqrtf((float)A.k) + 2.f);   // (binlist: every row of the batch is a warp's, knn_bins.cu)
             rc = MG_KNN_RSCALE * cbrtf(0.2387324f * expect * (float)vol / (float)max(N, 1));
             if (hv > 0.f && isfinite(hv)) rc = MG_KNN_HINT * hv + 1e-3f;
             if (!(rc > 1e-6f) || !isfinite(rc)) rc = 1.f;
@@ -224,7 +224,8 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
             // stencil would cover the axis anyway, and no more bins than atoms
             float frac = 1.f;
             // (the cutoff graph's scan kernel, and KNN on batches of large structures: knn_bins.cu)
-            if ((A.k > 0 || A.rows_cost) && A.binlist && N > MG_SMALL_MAX_ATOMS && mloc == 1) {
+            // (... where a small structure gets a list too: one bin, or a few, instead of the growing-radius routine)
+            if ((A.k > 0 || A.rows_cost) && A.binlist && (N > MG_SMALL_MAX_ATOMS || A.k > 0) && mloc == 1) {
                 int nb[3];
 #pragma unroll
                 for (int a = 0; a < 3; ++a) {

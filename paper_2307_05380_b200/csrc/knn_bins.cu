@@ -29,7 +29,8 @@ namespace mg_knn_bins_tu {
 #include "knn_small.cuh"
 #include "knn_pairs.cuh"
 
-#define MGKB_HITS 640              // hits of a row the table area of the warp's shared memory holds (entry word, codes)
+#define MGKB_HITS 640              // hits of a row the table area of the warp's shared memory holds (atom, offset bytes)
+#define MGKB_BOX_MAX 512           // cells of a per-pair sub-box the rows of a structure without a cell list walk
 
 // tau of a hit: codes = rint(u_a) mod 4 (2 bits per axis), ki = the source's packed integer parts (cut_prep.cuh), wj = .w
 // of the target's sorted entry (cut_bins.cuh): tau = -rint(u) + k_i - k_j.
@@ -39,8 +40,12 @@ __device__ __forceinline__ void mgkb_tau(unsigned codes, int ki, int wj, int tau
     tau[2] = 1 - (int)(((codes >> 4) + 1u) & 3u) + (((ki >> 20) & 1023) - 512) - (((wj >> 26) & 31) - 16);
 }
 
-// Hits of row i of structure s (first atom `first`) -> ks.stash (key = d2 bits | hit number) and the table area (entry
-// word, codes).  Returns their number (more than MGKB_HITS: the caller gives up).
+__device__ __forceinline__ unsigned mgkb_pack_tau(const int tau[3]) {
+    return ((unsigned)(tau[0] + 128) << 16) | ((unsigned)(tau[1] + 128) << 8) | (unsigned)(tau[2] + 128);
+}
+
+// Hits of row i of structure s (first atom `first`) -> ks.stash (key = d2 bits | hit number) and the table area (atom,
+// offset bytes).  Returns their number (more than MGKB_HITS: the caller gives up).
 __device__ __forceinline__ int mgkb_find(KnnSmem &ks, const KnnBinsArgs &A, const CutRec *R, int s, int first, int i,
                                          const float a[9], float r2, int lane) {
     const float4 *xw = reinterpret_cast<const float4 *>(A.xw4) + first, *xs = reinterpret_cast<const float4 *>(A.xs4) + first;
@@ -101,8 +106,12 @@ __device__ __forceinline__ int mgkb_find(KnnSmem &ks, const KnnBinsArgs &A, cons
             const float d2 = __fmaf_rn(vz, vz, __fmaf_rn(vy, vy, __fmul_rn(vx, vx)));
             hit = d2 < r2 && (__float_as_int(xj.w) & 0xFFFF) != i;           // (i, i, 0) is not an edge (R3)
             key = (unsigned long long)__float_as_uint(d2) << 32;
-            m = make_uint2(__float_as_uint(xj.w), (__float_as_uint(m0) & 3u) | ((__float_as_uint(m1) & 3u) << 2) |
-                                                      ((__float_as_uint(m2) & 3u) << 4));
+            if (hit) {                                                        // the hit's atom and offset
+                int tau[3];
+                mgkb_tau((__float_as_uint(m0) & 3u) | ((__float_as_uint(m1) & 3u) << 2) | ((__float_as_uint(m2) & 3u) << 4),
+                         __float_as_int(xi.w), __float_as_int(xj.w), tau);
+                m = make_uint2(__float_as_uint(xj.w) & 0xFFFFu, mgkb_pack_tau(tau));
+            }
         }
         const unsigned bal = __ballot_sync(0xFFFFFFFFu, hit);
         if (hit) {
@@ -114,10 +123,68 @@ __device__ __forceinline__ int mgkb_find(KnnSmem &ks, const KnnBinsArgs &A, cons
     __syncwarp();
     return run;
 }
+// The same for a structure WITHOUT a cell list (several images per pair: R / h_a >= 1/2 on some axis, or atoms far from
+// the origin): lanes over (target, cell) of the per-pair sub-box of cut_prep.cuh — u = x_j - x_i (wrapped), first cell
+// lo_a = floor(-rho_a - u_a) + 1, m_a cells from there — every target, no pruning.  Offsets outside int8 or a non-finite
+// coordinate: gives up (the growing-radius routine decides and reports).
+__device__ __forceinline__ int mgkb_find_box(KnnSmem &ks, const KnnBinsArgs &A, const CutRec *R, int first, int N, int i,
+                                             const float a[9], float r2, int lane) {
+    const float4 *xw = reinterpret_cast<const float4 *>(A.xw4) + first;
+    const float4 xi = xw[i];
+    const int ki = __float_as_int(xi.w);
+    const float rho0 = R->rho[0], rho1 = R->rho[1], rho2 = R->rho[2];
+    const int m1 = (R->m >> 8) & 0xFF, m2 = (R->m >> 16) & 0xFF, mloc = R->mloc, M12 = m1 * m2;
+    const bool wide = mloc >= 32;
+    const int J = wide ? 1 : 32 / mloc, jl = wide ? 0 : lane / mloc, npass = wide ? (mloc + 31) >> 5 : 1;
+    uint2 *meta = reinterpret_cast<uint2 *>(ks.w.T);
+    const unsigned lt = (1u << lane) - 1u;
+    int run = 0;
+    bool bad = ki == 0;
+    for (int ps = 0; ps < npass; ++ps) {
+        const int c = wide ? 32 * ps + lane : lane - jl * mloc;
+        const bool cv = wide ? c < mloc : jl < J;
+        const int t0 = c / M12, rr = c - t0 * M12, t1 = rr / m2, t2 = rr - t1 * m2;
+        for (int j0 = 0; j0 < N; j0 += J) {
+            const int j = j0 + jl;
+            bool hit = false;
+            unsigned long long key = 0ull;
+            uint2 m = make_uint2(0u, 0u);
+            if (cv && j < N) {
+                const float4 xj = xw[j];
+                const int kj = __float_as_int(xj.w);
+                const float u0 = __fsub_rn(xj.x, xi.x), u1 = __fsub_rn(xj.y, xi.y), u2 = __fsub_rn(xj.z, xi.z);
+                const float e0 = floorf(__fsub_rn(-rho0, u0)) + 1.f, e1 = floorf(__fsub_rn(-rho1, u1)) + 1.f,
+                            e2 = floorf(__fsub_rn(-rho2, u2)) + 1.f;
+                const float f0 = __fadd_rn(u0, e0 + (float)t0), f1 = __fadd_rn(u1, e1 + (float)t1), f2 = __fadd_rn(u2, e2 + (float)t2);
+                const float vx = __fmaf_rn(f2, a[6], __fmaf_rn(f1, a[3], __fmul_rn(f0, a[0])));
+                const float vy = __fmaf_rn(f2, a[7], __fmaf_rn(f1, a[4], __fmul_rn(f0, a[1])));
+                const float vz = __fmaf_rn(f2, a[8], __fmaf_rn(f1, a[5], __fmul_rn(f0, a[2])));
+                const float d2 = __fmaf_rn(vz, vz, __fmaf_rn(vy, vy, __fmul_rn(vx, vx)));
+                int tau[3];
+                tau[0] = (int)e0 + t0 + (ki & 1023) - (kj & 1023);
+                tau[1] = (int)e1 + t1 + ((ki >> 10) & 1023) - ((kj >> 10) & 1023);
+                tau[2] = (int)e2 + t2 + ((ki >> 20) & 1023) - ((kj >> 20) & 1023);
+                bad = bad || kj == 0 || tau[0] < -127 || tau[1] < -127 || tau[2] < -127 || tau[0] > 127 || tau[1] > 127 || tau[2] > 127;
+                hit = !bad && d2 < r2 && !(i == j && (tau[0] | tau[1] | tau[2]) == 0);   // (i, i, 0) is not an edge (R3)
+                key = (unsigned long long)__float_as_uint(d2) << 32;
+                m = make_uint2((unsigned)j, mgkb_pack_tau(tau));
+            }
+            const unsigned bal = __ballot_sync(0xFFFFFFFFu, hit);
+            if (hit) {
+                const int pos = run + __popc(bal & lt);
+                if (pos < MGKB_HITS) { ks.stash[pos] = key | (unsigned)pos; meta[pos] = m; }
+            }
+            run += __popc(bal);
+        }
+    }
+    __syncwarp();
+    return __any_sync(0xFFFFFFFFu, bad) ? MGKB_HITS + 1 : run;
+}
+
 // One row through the cell list.  Returns false if the row did not settle inside R (the caller hands it to the growing-
 // radius routine); *dk: its k-th distance.
-__device__ __forceinline__ bool mgkb_row(KnnSmem &ks, const KnnBinsArgs &A, const CutRec *R, int s, int first, int i,
-                                         int lane, float *dk) {
+__device__ __forceinline__ bool mgkb_row(KnnSmem &ks, const KnnBinsArgs &A, const CutRec *R, int s, int first, int N, int i,
+                                         bool binned, int lane, float *dk) {
     const int K = A.k, gi = first + i;
     const float *lat = A.lattice + 9 * (size_t)s;
     float a[9];
@@ -128,7 +195,7 @@ __device__ __forceinline__ bool mgkb_row(KnnSmem &ks, const KnnBinsArgs &A, cons
     // R^2 - 2 win is safe
     const float win = 1.1920929e-7f * (2.f * rad * (13.f * R->qmax + 2.f * R->amax_sum) + 4.f * rad * rad);
     const float lim2 = __fmaf_rn(-2.f, win, r2);
-    const int total = mgkb_find(ks, A, R, s, first, i, a, r2, lane);
+    const int total = binned ? mgkb_find(ks, A, R, s, first, i, a, r2, lane) : mgkb_find_box(ks, A, R, first, N, i, a, r2, lane);
     if (total < K || total > MGKB_HITS) return false;
     // the 32 smallest FP32 keys (Alg. 2's "sort, keep k", 32 at a time)
     mg_key key = mg_sort32(lane < total ? ks.stash[lane] : MG_KEY_INF, lane);
@@ -144,14 +211,13 @@ __device__ __forceinline__ bool mgkb_row(KnnSmem &ks, const KnnBinsArgs &A, cons
     const bool amb = lane >= K && key != MG_KEY_INF && __uint_as_float((unsigned)(key >> 32)) <= __fmaf_rn(2.f, win, kth_d2);
     const int nsel = K + __popc(__ballot_sync(0xFFFFFFFFu, amb));
     const uint2 *meta = reinterpret_cast<const uint2 *>(ks.w.T);
-    const int ki = __float_as_int(reinterpret_cast<const float4 *>(A.xw4)[gi].w);
     int j = 0, tau[3] = {0, 0, 0};
     unsigned long long ord = ~0ull;
     double dd = 1e300, vv[3] = {0.0, 0.0, 0.0};
     if (lane < nsel) {
         const uint2 m = meta[(unsigned)key];                                 // (the key's low word is the hit's number)
-        j = (int)(m.x & 0xFFFFu);
-        mgkb_tau(m.y, ki, (int)m.x, tau);
+        j = (int)m.x;
+        tau[0] = (int)(m.y >> 16) - 128; tau[1] = (int)((m.y >> 8) & 0xFFu) - 128; tau[2] = (int)(m.y & 0xFFu) - 128;
         double xi[3], xj[3], L[9];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
@@ -229,7 +295,8 @@ mg_knn_bins_kernel(const __grid_constant__ KnnBinsArgs A) {
         if (binned) binned = A.bin_start[first + 2 * s + (bins & 0xFF) * ((bins >> 8) & 0xFF) * ((bins >> 16) & 0xFF) + 1] != 0;
         float dk = 0.f;
         __syncwarp();
-        if (binned && mgkb_row(ks, A, R, s, first, i, lane, &dk)) {
+        // (no cell list: every target over the per-pair sub-box, unless that is thousands of cells)
+        if ((binned || R->mloc <= MGKB_BOX_MAX) && mgkb_row(ks, A, R, s, first, N, i, binned, lane, &dk)) {
             if (A.hint && lane == 0 && dk > 0.f) atomicMax(reinterpret_cast<int *>(A.hint + s), __float_as_int(dk));
             continue;
         }
