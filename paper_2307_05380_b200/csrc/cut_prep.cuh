@@ -207,8 +207,10 @@ mg_cut_prep_kernel(const CutPrepArgs A) {
             // instructions per 32 cells and 80 per pair)
             const float ck = (mloc > 256 ? (float)mloc * (35.f / 32.f) + 80.f : ((float)((mloc + 3) & ~3) * MG_KC_CELL + MG_KC_BLOCK) * (1.f / 32.f)) +
                              MG_KC_ROW / (float)N + MG_KC_STRUCT / ((float)N * (float)N);
-            // (KNN above the staging limit: warp-per-row growing-radius search, about 40 per pair-cell)
-            const float ckb = 40.f * (float)mloc / 32.f + 600.f / (float)N;
+            // (KNN above the staging limit inside a batch of small cells: a warp per row, lanes over (target, cell),
+            // mg_knn_row_box of knn_pairs.cuh; swept on config 2 plus one or eight structures of 100 / 280 / 900 atoms —
+            // flat between 80 and 160 per 32 pair-cells, 800 to 2000 per row; half of that left a warp 20 us behind)
+            const float ckb = 120.f * (float)mloc / 32.f + 800.f / (float)N;
             // cutoff, scan kernel (cut_scan.cuh), in cycles a warp spends (fit on BASELINE configs[2], per-warp
             // clocks of an MG_PHASE_CLOCKS build): per block of 32 pairs 735 + 182 per group of four cells it
             // evaluates (two groups per trip), 17 per edge, 4000 per structure visited; a structure the

@@ -1,6 +1,7 @@
-// knn_pairs.cuh — k-nearest-neighbour multigraph, k <= 32 (structures above MG_SMALL_MAX_ATOMS atoms
-// go row by row through the growing-radius routine of knn_small.cuh, and so do structures whose atoms are
-// given more than 40 cells apart: mg_knn_far).
+// knn_pairs.cuh — k-nearest-neighbour multigraph, k <= 32 (structures above MG_SMALL_MAX_ATOMS atoms, and
+// structures whose atoms are given more than 40 cells apart (mg_knn_far), go a warp per row over every target
+// and the pair's sub-box: mg_knn_row_box; what that does not settle, through the growing-radius routine of
+// knn_small.cuh).
 //
 // Problem: per source the k smallest keys (d, dst, tau_x, tau_y, tau_z) over all periodic images
 // except (i,i,0) (Alg. 2 lines 2-5, made deterministic: DESIGN.md R2, R8).
@@ -129,6 +130,140 @@ __device__ __noinline__ void mg_knn_row_fallback(KnnSmem &ks, const KnnPairsArgs
     __syncwarp();
     if (A.hint && lane == 0) atomicMax(reinterpret_cast<int *>(A.hint + s), __float_as_int(*slot));
     __syncwarp();
+}
+
+#define MG_KBOX_HITS 640           // hits of a row the table area of the warp's shared memory holds (atom, offset bytes)
+#define MG_KBOX_MAX 512            // cells of a per-pair sub-box mg_knn_row_box walks
+
+// One row of a structure the pair-lane machinery does not take (more atoms than it stages, or atoms many cells from the
+// origin) inside a batch of small cells: lanes over (target, cell) of the per-pair sub-box of cut_prep.cuh — wrapped
+// coordinates x - floor(x) taken on the fly, u = x_j - x_i, first cell lo_a = floor(-rho_a - u_a) + 1, m_a cells from there —
+// d2 in FP32, hits (d2 < R^2) to the stash, (atom, offset bytes) to the table area; then the generic selection: the 32
+// smallest FP32 keys, exact FP64 d2 for the k first and every hit FP32 cannot tell from the k-th, final order (d2, dst,
+// tau).  The same steps as knn_bins.cu takes for a structure without a cell list.  Alg. 1 line 4: a row that does not
+// settle inside R — fewer than k hits, a k-th key within the rounding window of R^2, more hits than the table area holds,
+// an offset outside int8, a non-finite coordinate, a sub-box above MG_KBOX_MAX cells — goes to the growing-radius routine
+// (227 us for ONE row of a 900-atom structure, which is why it is the last resort and not the rule).  Overwrites the
+// stash: for whole structures only, not for a row in the middle of a group of the pair-lane path (whose unsettled rows
+// call the growing-radius routine directly; through a wrapper of this name the headline's kernel ran 1.5 us longer).
+__device__ __noinline__ void mg_knn_row_box(KnnSmem &ks, const KnnPairsArgs &A, const CutRec *R, int s, int first, int N, int i,
+                                            int lane) {
+    const int K = A.k, gi = first + i, mloc = R->mloc;
+    bool done = false;
+    __syncwarp();
+    if (mloc > 0 && mloc <= MG_KBOX_MAX) {
+        float a[9];
+#pragma unroll
+        for (int c = 0; c < 9; ++c) a[c] = __ldg(A.lattice + 9 * (size_t)s + c);
+        const float rad = R->radius, r2 = __fmul_rn(rad, rad);
+        const float win = 1.1920929e-7f * (2.f * rad * (13.f * R->qmax + 2.f * R->amax_sum) + 4.f * rad * rad);
+        const float lim2 = __fmaf_rn(-2.f, win, r2);
+        const float rho0 = R->rho[0], rho1 = R->rho[1], rho2 = R->rho[2];
+        const int m1 = (R->m >> 8) & 0xFF, m2 = (R->m >> 16) & 0xFF, M12 = m1 * m2;
+        const bool wide = mloc >= 32;
+        const int J = wide ? 1 : 32 / mloc, jl = wide ? 0 : lane / mloc, npass = wide ? (mloc + 31) >> 5 : 1;
+        uint2 *meta = reinterpret_cast<uint2 *>(ks.w.T);
+        const unsigned lt = (1u << lane) - 1u;
+        const float *xg = A.pos + 3 * (size_t)first;
+        const float p0 = xg[3 * i], p1 = xg[3 * i + 1], p2 = xg[3 * i + 2];
+        const float gi0 = floorf(p0), gi1 = floorf(p1), gi2 = floorf(p2);
+        const float xi0 = p0 - gi0, xi1 = p1 - gi1, xi2 = p2 - gi2;
+        bool bad = !(fabsf(gi0) <= 500.f && fabsf(gi1) <= 500.f && fabsf(gi2) <= 500.f);      // (true for NaN / inf)
+        int run = 0;
+        for (int ps = 0; ps < npass; ++ps) {
+            const int c = wide ? 32 * ps + lane : lane - jl * mloc;
+            const bool cv = wide ? c < mloc : jl < J;
+            const int t0 = c / M12, rr = c - t0 * M12, t1 = rr / m2, t2 = rr - t1 * m2;
+            for (int j0 = 0; j0 < N; j0 += J) {
+                const int j = j0 + jl;
+                bool hit = false;
+                unsigned long long key = 0ull;
+                uint2 m = make_uint2(0u, 0u);
+                if (cv && j < N) {
+                    const float q0 = xg[3 * j], q1 = xg[3 * j + 1], q2 = xg[3 * j + 2];
+                    const float gj0 = floorf(q0), gj1 = floorf(q1), gj2 = floorf(q2);
+                    const float u0 = __fsub_rn(q0 - gj0, xi0), u1 = __fsub_rn(q1 - gj1, xi1), u2 = __fsub_rn(q2 - gj2, xi2);
+                    const float e0 = floorf(__fsub_rn(-rho0, u0)) + 1.f, e1 = floorf(__fsub_rn(-rho1, u1)) + 1.f,
+                                e2 = floorf(__fsub_rn(-rho2, u2)) + 1.f;
+                    const float f0 = __fadd_rn(u0, e0 + (float)t0), f1 = __fadd_rn(u1, e1 + (float)t1), f2 = __fadd_rn(u2, e2 + (float)t2);
+                    const float vx = __fmaf_rn(f2, a[6], __fmaf_rn(f1, a[3], __fmul_rn(f0, a[0])));
+                    const float vy = __fmaf_rn(f2, a[7], __fmaf_rn(f1, a[4], __fmul_rn(f0, a[1])));
+                    const float vz = __fmaf_rn(f2, a[8], __fmaf_rn(f1, a[5], __fmul_rn(f0, a[2])));
+                    const float d2 = __fmaf_rn(vz, vz, __fmaf_rn(vy, vy, __fmul_rn(vx, vx)));
+                    const bool okj = fabsf(gj0) <= 500.f && fabsf(gj1) <= 500.f && fabsf(gj2) <= 500.f;
+                    // x_j + tau - x_i = u + e + t: tau = e + t + floor(x_i) - floor(x_j)
+                    const int tau0 = (int)e0 + t0 + (int)gi0 - (int)gj0, tau1 = (int)e1 + t1 + (int)gi1 - (int)gj1,
+                              tau2 = (int)e2 + t2 + (int)gi2 - (int)gj2;
+                    bad = bad || !okj || tau0 < -127 || tau1 < -127 || tau2 < -127 || tau0 > 127 || tau1 > 127 || tau2 > 127;
+                    hit = !bad && d2 < r2 && !(i == j && (tau0 | tau1 | tau2) == 0);       // (i, i, 0) is not an edge (R3)
+                    key = (unsigned long long)__float_as_uint(d2) << 32;
+                    m = make_uint2((unsigned)j, ((unsigned)(tau0 + 128) << 16) | ((unsigned)(tau1 + 128) << 8) | (unsigned)(tau2 + 128));
+                }
+                const unsigned bal = __ballot_sync(0xFFFFFFFFu, hit);
+                if (hit) {
+                    const int pos = run + __popc(bal & lt);
+                    if (pos < MG_KBOX_HITS) { ks.stash[pos] = key | (unsigned)pos; meta[pos] = m; }
+                }
+                run += __popc(bal);
+            }
+        }
+        __syncwarp();
+        const int total = __any_sync(0xFFFFFFFFu, bad) ? MG_KBOX_HITS + 1 : run;
+        if (total >= K && total <= MG_KBOX_HITS) {
+            // the 32 smallest FP32 keys (Alg. 2's "sort, keep k", 32 at a time)
+            mg_key key = mg_sort32(lane < total ? ks.stash[lane] : MG_KEY_INF, lane);
+            for (int c = 32; c < total; c += 32) {
+                mg_key keys1[1] = {key};
+                mg_knn_merge<1>(keys1, c + lane < total ? ks.stash[c + lane] : MG_KEY_INF, lane);
+                key = keys1[0];
+            }
+            const mg_key kth = __shfl_sync(0xFFFFFFFFu, key, K - 1);
+            const float kth_d2 = __uint_as_float((unsigned)(kth >> 32));
+            if (kth != MG_KEY_INF && kth_d2 < lim2) {
+                const bool amb = lane >= K && key != MG_KEY_INF && __uint_as_float((unsigned)(key >> 32)) <= __fmaf_rn(2.f, win, kth_d2);
+                const int nsel = K + __popc(__ballot_sync(0xFFFFFFFFu, amb));
+                int j = 0, tau[3] = {0, 0, 0};
+                unsigned long long ord = ~0ull;
+                double dd = 1e300, vv[3] = {0.0, 0.0, 0.0};
+                if (lane < nsel) {
+                    const uint2 m = meta[(unsigned)key];                          // (the key's low word is the hit's number)
+                    j = (int)m.x;
+                    tau[0] = (int)(m.y >> 16) - 128; tau[1] = (int)((m.y >> 8) & 0xFFu) - 128; tau[2] = (int)(m.y & 0xFFu) - 128;
+                    double xi[3], xj[3], L[9];
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        xi[c] = (double)xg[3 * i + c];
+                        xj[c] = (double)xg[3 * j + c];
+                    }
+#pragma unroll
+                    for (int c = 0; c < 9; ++c) L[c] = (double)a[c];
+                    dd = mg_knn_exact_d2(xi, xj, tau[0], tau[1], tau[2], L, vv);
+                    ord = ((unsigned long long)(unsigned)j << 24) | m.y;
+                }
+                int rank = 0;
+                for (int l = 0; l < nsel; ++l) {
+                    const double od = __shfl_sync(0xFFFFFFFFu, dd, l);
+                    const unsigned long long oo = __shfl_sync(0xFFFFFFFFu, ord, l);
+                    rank += (od < dd || (od == dd && oo < ord)) ? 1 : 0;
+                }
+                if (lane < nsel && rank < K) {
+                    const long long e = (long long)K * gi + rank;
+                    A.src[e] = gi;
+                    A.dst[e] = first + j;
+                    A.offset[3 * e] = (int8_t)tau[0]; A.offset[3 * e + 1] = (int8_t)tau[1]; A.offset[3 * e + 2] = (int8_t)tau[2];
+                    A.vec[3 * e] = (float)vv[0]; A.vec[3 * e + 1] = (float)vv[1]; A.vec[3 * e + 2] = (float)vv[2];
+                    if (A.dist) A.dist[e] = __fsqrt_rn((float)dd);
+                    if (rank == K - 1 && A.hint) {
+                        const float dk = __fsqrt_ru(__double2float_ru(dd));
+                        if (dk > 0.f) atomicMax(reinterpret_cast<int *>(A.hint + s), __float_as_int(dk));
+                    }
+                }
+                done = true;
+            }
+        }
+        __syncwarp();
+    }
+    if (!done) mg_knn_row_fallback(ks, A, s, first, N, i, lane);
 }
 
 // Hits of the pairs [qa, qb) (whole rows) of the staged structure -> stash, row offsets -> rowoff.

@@ -442,3 +442,38 @@ def test_knn_update_graph_on_large_structures(mg, ctx):
     first = C.Batch(pos=b.pos[:b.struct_ptr[1]], lattice=b.lattice[:1], struct_ptr=b.struct_ptr[:2])
     ref = oracle.knn_graph(first.pos, first.lattice, first.struct_ptr, k)
     assert np.array_equal(g["dst"][:k * lo], ref["dst"])
+
+
+@pytest.mark.parametrize("k", [1, 12, 16, 17, 32])
+def test_knn_large_structures_inside_a_batch_of_small_cells(mg, ctx, k):
+    # the batch averages at most 64 atoms per structure, so it takes the pair-lane kernels (k <= 16 and k > 16), whose rows of
+    # a structure above the staging limit go a warp per row over every target and the pair's sub-box (mg_knn_row_box):
+    # one image per pair, several images per pair, coordinates outside the cell, a cluster whose rows overflow the
+    # warp's hit buffer (those fall through to the growing-radius routine)
+    import torch
+    rng = np.random.default_rng(71 + k)
+    items = [C.small_crystal(5, s) for s in range(24)]
+    items.insert(3, _random_structure(rng, 130, (22.0, 25.0, 21.0)))              # sparse: one cell per pair
+    items.insert(9, _random_structure(rng, 90, (6.0, 6.5, 7.0), 0.3))             # dense: a sub-box of several cells
+    items.insert(15, _random_structure(rng, 300, (30.0, 9.0, 28.0)))
+    far = _random_structure(rng, 70, (12.0, 13.0, 11.0))
+    far[1][:] = (far[1] * np.float32(5.0) - np.float32(2.0)).astype(np.float32)   # coordinates in [-2, 3)
+    items.insert(20, far)
+    blob = _random_structure(rng, 120, (18.0, 18.0, 18.0))
+    blob[1][:100] = blob[1][0] + rng.normal(0, 0.002, (100, 3)).astype(np.float32)
+    if k >= 12: items.append(blob)                                                # (with k = 1 its rows are a tie in FP32)
+    b = C._assemble(items)
+    assert b.n_atoms / b.n_struct <= 64
+    got, status = _knn(mg, ctx, b, k)
+    assert status == 0
+    rep = check.check_knn(b, k, got)
+    assert rep["n_edges"] == k * b.n_atoms
+    # and as a sequence of updates: the hint these rows leave is the next call's radius
+    pos, lat, ptr = mg.to_device(b)
+    graph = ctx.mg_graph_create(mg.MG_KIND_KNN, ptr, b.n_atoms, k=k)
+    out = mg.Edges.allocate(b.n_atoms, k * b.n_atoms, "cuda", dist=True)
+    for t in C.walk(b, 2, seed=9, sigma=0.01):
+        ctx.mg_update_graph(graph, torch.from_numpy(t.pos).cuda(), torch.from_numpy(t.lattice).cuda(), out)
+        assert ctx.mg_check() == 0
+        check.check_knn(t, k, out.to_numpy())
+    graph.close()

@@ -1,6 +1,6 @@
 """Randomised parity against the oracle, fixed seeds: inputs no hand-written case thought of.  Three generators —
-large structures for the cutoff graph (cell list and generic rows), sheared / shifted / tiny cells and batches of large
-structures for KNN, and
+large structures for the cutoff graph (cell list and generic rows), sheared / shifted / tiny cells, batches of large
+structures and large structures among small cells for KNN, and
 whole batches through every entry point (cutoff, per-atom cutoffs, KNN, symmetrize, triplets, update sequences)."""
 import numpy as np
 import pytest
@@ -110,6 +110,38 @@ def test_soak_knn_batches_of_large_structures(mg, ctx, seed):
         if rng.random() < 0.3:
             items.append(C.small_crystal(int(rng.integers(1 << 30)), 0))
         b = C._assemble(items)
+        pos, lat, ptr = mg.to_device(b)
+        got = ctx.knn_graph(pos, lat, ptr, k, dist=True).to_numpy()
+        assert ctx.mg_check() == 0, (seed, case, k)
+        check.check_knn(b, k, got)
+
+
+@pytest.mark.parametrize("seed", [501, 502])
+def test_soak_knn_large_structures_among_small_cells(mg, ctx, seed):
+    # batches that average at most 64 atoms per structure with one or two structures above the staging limit: their rows
+    # go a warp per row over every target and the pair's sub-box (mg_knn_row_box of knn_pairs.cuh), in both pair-lane kernels
+    rng = np.random.default_rng(seed)
+    for case in range(10):
+        k = int(rng.choice([1, 3, 12, 16, 20, 32]))
+        items = [C.small_crystal(int(rng.integers(1 << 30)), 0) for _ in range(int(rng.integers(12, 30)))]
+        for s in range(int(rng.integers(1, 3))):
+            n = int(rng.integers(65, 260))
+            side = (n / float(rng.uniform(0.01, 0.25))) ** (1 / 3)
+            lens = side * rng.uniform(0.5, 1.7, 3)
+            ang = rng.uniform(65, 115, 3)
+            cell = C.cell_from_parameters(lens[0], lens[1], lens[2], ang[0], ang[1], ang[2])
+            cell = np.asarray(cell if cell is not None else np.diag(lens), np.float32)
+            x = rng.random((n, 3), dtype=np.float32)
+            mode = rng.integers(0, 5)
+            if mode == 1: x = (x * np.float32(3.0) - np.float32(1.0)).astype(np.float32)
+            if mode == 2: x = (x + np.float32(rng.integers(-30, 31))).astype(np.float32)   # the whole structure, cells away
+            if mode == 3: x[: n // 4] = np.round(x[: n // 4] * 8) / 8
+            if mode == 4 and k > 1: x[: n // 2] = x[0] + rng.normal(0, 0.01, (n // 2, 3)).astype(np.float32)
+            items.insert(int(rng.integers(0, len(items) + 1)), (cell, x.astype(np.float32)))
+        b = C._assemble(items)
+        while b.n_atoms / b.n_struct > 64:
+            items.append(C.small_crystal(int(rng.integers(1 << 30)), 0))
+            b = C._assemble(items)
         pos, lat, ptr = mg.to_device(b)
         got = ctx.knn_graph(pos, lat, ptr, k, dist=True).to_numpy()
         assert ctx.mg_check() == 0, (seed, case, k)
