@@ -494,6 +494,22 @@ def run_gpu(args, rank, world, local_rank):
                                             "Table 1 batch row (PAPER.md:138: 53 / 55 / 80 ms KNN, 43 / 72 / 123 ms cutoff on an RTX 8000, "
                                             "Materials Project data: context, another machine and other data)")
 
+        # a few large structures among the small cells of the headline batch (a Materials-Project-like mix: the batch still
+        # averages below 64 atoms per structure, so it takes the headline's kernels, mg_knn_row_box)
+        mixed = {}
+        for tag, big in (("plus_1x100_atoms", [C.supercell(7, 0, density=100 / 20.0 ** 3 / 0.9, n_lo=100, n_hi=140)]),
+                         ("plus_8x900_atoms", [C.supercell(7, s_, n_lo=900, n_hi=1100) for s_ in range(8)])):
+            bm = C.concat([batch, C._assemble(big)])
+            pm, lm, sm_ = mg.to_device(bm, dev)
+            om = mg.Edges.allocate(bm.n_atoms, K_NN * bm.n_atoms, dev, dist=True)
+            mixed[tag] = {"n_atoms": int(bm.n_atoms), "knn_us_per_call": timed(lambda i: ctx.mg_knn_graph(pm, lm, sm_, K_NN, om), reps=20)}
+            em = ctx.mg_cutoff_count(pm, lm, sm_, R_C)
+            om = mg.Edges.allocate(bm.n_atoms, em, dev)
+            mixed[tag]["cutoff_us_per_call"] = timed(lambda i: ctx.mg_cutoff_graph(pm, lm, sm_, R_C, om), reps=20)
+            del om
+        legs["config2_with_large_structures"] = dict(mixed, workload="BASELINE configs[2] plus one 100-140-atom / eight 900-1100-atom "
+                                                     f"structures, KNN k={K_NN} and cutoff {R_C:g} A")
+
         # SURVEY 8(f) NEXT-1 / NEXT-2 on the headline KNN graph: symmetric graph, triplets
         kn = knn_sets[0]
         sym = mg.Edges.allocate(n_atoms, 2 * e_knn, dev, dist=True)
