@@ -1,4 +1,4 @@
-// knn_bins.cu — k-nearest-neighbour graph (k <= 32) for batches of LARGE structures: one warp per source row, candidates
+// knn_bins.cu — k-nearest-neighbour graph (k <= 64) for batches of LARGE structures: one warp per source row, candidates
 // from the fractional-coordinate cell list of cut_bins.cuh (SURVEY.md 8(a) K2 + K5; "route KNN for
 // N > 64 through the same structure instead of the row-by-row fallback").
 //
@@ -251,6 +251,162 @@ __device__ __forceinline__ bool mgkb_row(KnnSmem &ks, const KnnBinsArgs &A, cons
     *dk = dkk;
     return true;
 }
+// The same with KPL sorted FP32 keys per lane (k <= 32 KPL; slot q of lane l holds rank 32 q + l), for 32 < k <= 64.  Out
+// of line and apart from mgkb_row: as one template, inlined, the rows of k <= 32 ran 13 % slower (config 3, k = 12: 94.8
+// against 82.5 us per call).
+template <int KPL>
+__device__ __noinline__ bool mgkb_row_wide(KnnSmem &ks, const KnnBinsArgs &A, const CutRec *R, int s, int first, int N, int i,
+                                         bool binned, int lane, float *dk) {
+    const int K = A.k, gi = first + i;
+    const float *lat = A.lattice + 9 * (size_t)s;
+    float a[9];
+#pragma unroll
+    for (int c = 0; c < 9; ++c) a[c] = __ldg(lat + c);
+    const float rad = R->radius, r2 = __fmul_rn(rad, rad);
+    // FP32 error bound of d2 near R^2 (R23): every image with true d2 < R^2 - win is a hit; a k-th key below
+    // R^2 - 2 win is safe
+    const float win = 1.1920929e-7f * (2.f * rad * (13.f * R->qmax + 2.f * R->amax_sum) + 4.f * rad * rad);
+    const float lim2 = __fmaf_rn(-2.f, win, r2);
+    const int total = binned ? mgkb_find(ks, A, R, s, first, i, a, r2, lane) : mgkb_find_box(ks, A, R, first, N, i, a, r2, lane);
+    if (total < K || total > MGKB_HITS) return false;
+    // the 32 KPL smallest FP32 keys (Alg. 2's "sort, keep k", 32 at a time)
+    mg_key keys[KPL];
+    if (KPL == 1) {
+        keys[0] = mg_sort32(lane < total ? ks.stash[lane] : MG_KEY_INF, lane);
+        for (int c = 32; c < total; c += 32) mg_knn_merge<KPL>(keys, c + lane < total ? ks.stash[c + lane] : MG_KEY_INF, lane);
+    } else {
+#pragma unroll
+        for (int q = 0; q < KPL; ++q) keys[q] = MG_KEY_INF;
+        for (int c = 0; c < total; c += 32) mg_knn_merge<KPL>(keys, c + lane < total ? ks.stash[c + lane] : MG_KEY_INF, lane);
+    }
+    const mg_key kth = __shfl_sync(0xFFFFFFFFu, keys[(K - 1) >> 5], (K - 1) & 31);
+    const float kth_d2 = __uint_as_float((unsigned)(kth >> 32));
+    if (kth == MG_KEY_INF || !(kth_d2 < lim2)) return false;
+    // exact FP64 d2 of the k first and of every hit FP32 cannot tell from the k-th; final order (d2, dst, tau)
+    int nsel = K;
+#pragma unroll
+    for (int q = 0; q < KPL; ++q) {
+        const bool amb = 32 * q + lane >= K && keys[q] != MG_KEY_INF &&
+                         __uint_as_float((unsigned)(keys[q] >> 32)) <= __fmaf_rn(2.f, win, kth_d2);
+        nsel += __popc(__ballot_sync(0xFFFFFFFFu, amb));
+    }
+    const uint2 *meta = reinterpret_cast<const uint2 *>(ks.w.T);
+    int j[KPL], tau[KPL][3];
+    unsigned long long ord[KPL];
+    double dd[KPL], vv[KPL][3];
+    double xi[3], L[9];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) xi[c] = (double)A.pos[3 * (size_t)gi + c];
+#pragma unroll
+    for (int c = 0; c < 9; ++c) L[c] = (double)a[c];
+#pragma unroll
+    for (int q = 0; q < KPL; ++q) {
+        j[q] = 0; tau[q][0] = tau[q][1] = tau[q][2] = 0; ord[q] = ~0ull; dd[q] = 1e300;
+        vv[q][0] = vv[q][1] = vv[q][2] = 0.0;
+        if (32 * q + lane < nsel) {
+            const uint2 m = meta[(unsigned)keys[q]];                         // (the key's low word is the hit's number)
+            j[q] = (int)m.x;
+            tau[q][0] = (int)(m.y >> 16) - 128; tau[q][1] = (int)((m.y >> 8) & 0xFFu) - 128; tau[q][2] = (int)(m.y & 0xFFu) - 128;
+            double xj[3];
+#pragma unroll
+            for (int c = 0; c < 3; ++c) xj[c] = (double)A.pos[3 * (size_t)(first + j[q]) + c];
+            dd[q] = mg_knn_exact_d2(xi, xj, tau[q][0], tau[q][1], tau[q][2], L, vv[q]);
+            ord[q] = ((unsigned long long)(unsigned)j[q] << 24) | m.y;
+        }
+    }
+    int rank[KPL];
+#pragma unroll
+    for (int q = 0; q < KPL; ++q) rank[q] = 0;
+#pragma unroll
+    for (int q2 = 0; q2 < KPL; ++q2) {
+        const int cnt2 = min(32, nsel - 32 * q2);
+        for (int l = 0; l < cnt2; ++l) {
+            const double od = __shfl_sync(0xFFFFFFFFu, dd[q2], l);
+            const unsigned long long oo = __shfl_sync(0xFFFFFFFFu, ord[q2], l);
+#pragma unroll
+            for (int q = 0; q < KPL; ++q) rank[q] += (od < dd[q] || (od == dd[q] && oo < ord[q])) ? 1 : 0;
+        }
+    }
+    float dkk = 0.f;
+#pragma unroll
+    for (int q = 0; q < KPL; ++q)
+        if (32 * q + lane < nsel && rank[q] < K) {
+            const long long e = (long long)K * gi + rank[q];
+            A.src[e] = gi;
+            A.dst[e] = first + j[q];
+            A.offset[3 * e] = (int8_t)tau[q][0]; A.offset[3 * e + 1] = (int8_t)tau[q][1]; A.offset[3 * e + 2] = (int8_t)tau[q][2];
+            A.vec[3 * e] = (float)vv[q][0]; A.vec[3 * e + 1] = (float)vv[q][1]; A.vec[3 * e + 2] = (float)vv[q][2];
+            if (A.dist) A.dist[e] = __fsqrt_rn((float)dd[q]);
+            if (rank[q] == K - 1) dkk = __fsqrt_ru(__double2float_ru(dd[q]));
+        }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) dkk = fmaxf(dkk, __shfl_xor_sync(0xFFFFFFFFu, dkk, o));
+    *dk = dkk;
+    return true;
+}
+
+// The growing-radius routine of knn_small.cuh for one row with two sorted keys per lane (32 < k <= 64): what
+// mg_knn_row_fallback of knn_pairs.cuh is for k <= 32, the same steps.
+__device__ __noinline__ void mgkb_grow2(KnnSmem &ks, const KnnPairsArgs &A, int s, int first, int N, int i, int lane) {
+    const float *lat9 = A.lattice + 9 * (size_t)s;
+    float4 *sp = reinterpret_cast<float4 *>(ks.w.T);
+    mg_key *buf = reinterpret_cast<mg_key *>(ks.w.T + MG_SMALL_MAX_ATOMS);
+    StructRec R;
+    float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f};
+    __syncwarp();
+    const bool big = N > MG_SMALL_MAX_ATOMS;      // too large to stage: positions on the fly
+    for (int j = lane; j < N; j += 32) {
+        const float *x = A.pos + 3 * (size_t)(first + j);
+        const float x0 = x[0], x1 = x[1], x2 = x[2];
+        lo[0] = fminf(lo[0], x0); lo[1] = fminf(lo[1], x1); lo[2] = fminf(lo[2], x2);
+        hi[0] = fmaxf(hi[0], x0); hi[1] = fmaxf(hi[1], x1); hi[2] = fmaxf(hi[2], x2);
+        if (big) continue;
+        float4 p;
+        p.x = __fmaf_rn(x2, lat9[6], __fmaf_rn(x1, lat9[3], __fmul_rn(x0, lat9[0])));
+        p.y = __fmaf_rn(x2, lat9[7], __fmaf_rn(x1, lat9[4], __fmul_rn(x0, lat9[1])));
+        p.z = __fmaf_rn(x2, lat9[8], __fmaf_rn(x1, lat9[5], __fmul_rn(x0, lat9[2])));
+        p.w = 0.f;
+        sp[j] = p;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1)
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            lo[a] = fminf(lo[a], __shfl_xor_sync(0xFFFFFFFFu, lo[a], o));
+            hi[a] = fmaxf(hi[a], __shfl_xor_sync(0xFFFFFFFFu, hi[a], o));
+        }
+    __syncwarp();
+    float lat[9];
+#pragma unroll
+    for (int c = 0; c < 9; ++c) lat[c] = lat9[c];
+    double vol = 1.0, h[3] = {1.0, 1.0, 1.0};
+    mg_cell_spacings(lat, &vol, h);                   // the lattice is valid: prep checked it
+    R.first = first;
+    R.natoms = N;
+    R.volume = (float)vol;
+    R.err = 0u;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        R.xmin[a] = lo[a];
+        R.xmax[a] = hi[a];
+        R.h_dn[a] = __double2float_rd(h[a] * (1.0 - 1e-6));
+        R.invh_up[a] = __double2float_ru((1.0 + 1e-6) / h[a]);
+        R.amax[a] = fmaxf(fabsf(lat[3 * a]), fmaxf(fabsf(lat[3 * a + 1]), fabsf(lat[3 * a + 2])));
+    }
+    KnnArgs K;
+    K.pos = A.pos; K.lattice = A.lattice; K.struct_ptr = A.struct_ptr;
+    K.n_struct = A.n_struct; K.n_atoms = A.n_atoms; K.k = A.k;
+    K.row_ptr = A.row_ptr; K.src = A.src; K.dst = A.dst; K.offset = A.offset;
+    K.vec = A.vec; K.dist = A.dist; K.n_edges = A.n_edges;
+    float *slot = reinterpret_cast<float *>(ks.w.T + MG_SMALL_MAX_ATOMS + 16);   // k-th distance comes back here
+    K.radius_hint = A.hint ? slot - (first + i) : nullptr; K.use_hint = 0;
+    K.rec = nullptr; K.atom_struct = nullptr; K.ctl = nullptr; K.status = A.status;
+    mg_knn_source<2>(K, R, lat9, big ? nullptr : sp, buf, i, lane);
+    __syncwarp();
+    if (A.hint && lane == 0) atomicMax(reinterpret_cast<int *>(A.hint + s), __float_as_int(*slot));
+    __syncwarp();
+}
+
 __global__ void __launch_bounds__(MG_BLOCK)
 mg_knn_bins_kernel(const __grid_constant__ KnnBinsArgs A) {
     mg_grid_dependency_wait();
@@ -296,12 +452,15 @@ mg_knn_bins_kernel(const __grid_constant__ KnnBinsArgs A) {
         float dk = 0.f;
         __syncwarp();
         // (no cell list: every target over the per-pair sub-box, unless that is thousands of cells)
-        if ((binned || R->mloc <= MGKB_BOX_MAX) && mgkb_row(ks, A, R, s, first, N, i, binned, lane, &dk)) {
+        const bool list = binned || R->mloc <= MGKB_BOX_MAX;
+        if (list && (K <= 32 ? mgkb_row(ks, A, R, s, first, N, i, binned, lane, &dk)
+                             : mgkb_row_wide<2>(ks, A, R, s, first, N, i, binned, lane, &dk))) {
             if (A.hint && lane == 0 && dk > 0.f) atomicMax(reinterpret_cast<int *>(A.hint + s), __float_as_int(dk));
             continue;
         }
         __syncwarp();
-        mg_knn_row_fallback(ks, P, s, first, N, i, lane);                 // (the growing-radius routine; sets the hint itself)
+        if (K <= 32) mg_knn_row_fallback(ks, P, s, first, N, i, lane);    // (the growing-radius routine; sets the hint itself)
+        else mgkb_grow2(ks, P, s, first, N, i, lane);
     }
 }
 }  // namespace mg_knn_bins_tu

@@ -603,8 +603,8 @@ static mg_status launch_knn(mg_ctx *c, const float *pos, const float *lat, const
     MG_CUDA(cudaSetDevice(c->device));
     mg_status rs = mg_reserve(c, n_struct, n_atoms);
     if (rs != MG_OK) return rs;
-    if (k <= 32 && n_struct > 0 && n_atoms / n_struct > MG_SMALL_MAX_ATOMS) {
-        // a batch of large structures: one warp per row through the cell list (knn_bins.cu); four launches: prep (which
+    if (n_struct > 0 && n_atoms / n_struct > MG_SMALL_MAX_ATOMS) {
+        // a batch of large structures (any k): one warp per row through the cell list (knn_bins.cu); four launches: prep (which
         // also wraps the coordinates and picks the slab counts), the sort by bin, the rows, the reset of the list
         const int n_blocks = (n_struct + MG_CP_BLOCK - 1) / MG_CP_BLOCK;
         CutPrepArgs P;

@@ -398,7 +398,7 @@ def _random_structure(rng, n, lens, jitter=1.0):
     return cell, rng.random((n, 3), dtype=np.float32)
 
 
-@pytest.mark.parametrize("k", [1, 12, 27, 32])
+@pytest.mark.parametrize("k", [1, 12, 27, 32, 33, 64])
 def test_knn_batches_of_large_structures_through_the_cell_list(mg, ctx, k):
     # batches whose structures average more than 64 atoms take knn_bins.cu: one warp per row, candidates from the cell list
     # where the structure has one (large cell, R / h < 1/2), the growing-radius routine for everything else in the batch
@@ -419,10 +419,10 @@ def test_knn_batches_of_large_structures_through_the_cell_list(mg, ctx, k):
     assert rep["n_edges"] == k * b.n_atoms
 
 
-def test_knn_update_graph_on_large_structures(mg, ctx):
+@pytest.mark.parametrize("k", [12, 40])
+def test_knn_update_graph_on_large_structures(mg, ctx, k):
     import torch
     b = C.config_batch(3, n_struct=3)
-    k = 12
     pos, lat, ptr = mg.to_device(b)
     graph = ctx.mg_graph_create(mg.MG_KIND_KNN, ptr, b.n_atoms, k=k)
     out = mg.Edges.allocate(b.n_atoms, k * b.n_atoms, "cuda", dist=True)

@@ -92,7 +92,7 @@ def test_soak_knn_batches_of_large_structures(mg, ctx, seed):
     rng = np.random.default_rng(seed)
     for case in range(10):
         items = []
-        k = int(rng.choice([1, 2, 6, 12, 20, 32]))
+        k = int(rng.choice([1, 2, 6, 12, 20, 32, 40, 64]))
         for s in range(int(rng.integers(1, 4))):
             n = int(rng.integers(65, 500))
             side = (n / float(rng.uniform(0.02, 0.12))) ** (1 / 3)
