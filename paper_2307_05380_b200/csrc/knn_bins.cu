@@ -314,17 +314,34 @@ __device__ __noinline__ bool mgkb_row_wide(KnnSmem &ks, const KnnBinsArgs &A, co
             ord[q] = ((unsigned long long)(unsigned)j[q] << 24) | m.y;
         }
     }
+    // (the FP32 keys mostly are the final order already: one look at each entry's predecessor tells, and only a row where
+    // FP64 or the tie-break disagrees counts, as in knn_small.cuh)
     int rank[KPL];
+    bool ok = true;
 #pragma unroll
-    for (int q = 0; q < KPL; ++q) rank[q] = 0;
+    for (int q = 0; q < KPL; ++q) {
+        rank[q] = 32 * q + lane;
+        double pd = __shfl_up_sync(0xFFFFFFFFu, dd[q], 1);
+        unsigned long long po = __shfl_up_sync(0xFFFFFFFFu, ord[q], 1);
+        if (q > 0) {
+            const double ld = __shfl_sync(0xFFFFFFFFu, dd[q > 0 ? q - 1 : 0], 31);
+            const unsigned long long lo = __shfl_sync(0xFFFFFFFFu, ord[q > 0 ? q - 1 : 0], 31);
+            if (lane == 0) { pd = ld; po = lo; }
+        }
+        if (32 * q + lane < nsel) ok = ok && (32 * q + lane == 0 || pd < dd[q] || (pd == dd[q] && po < ord[q]));
+    }
+    if (!__all_sync(0xFFFFFFFFu, ok)) {
 #pragma unroll
-    for (int q2 = 0; q2 < KPL; ++q2) {
-        const int cnt2 = min(32, nsel - 32 * q2);
-        for (int l = 0; l < cnt2; ++l) {
-            const double od = __shfl_sync(0xFFFFFFFFu, dd[q2], l);
-            const unsigned long long oo = __shfl_sync(0xFFFFFFFFu, ord[q2], l);
+        for (int q = 0; q < KPL; ++q) rank[q] = 0;
 #pragma unroll
-            for (int q = 0; q < KPL; ++q) rank[q] += (od < dd[q] || (od == dd[q] && oo < ord[q])) ? 1 : 0;
+        for (int q2 = 0; q2 < KPL; ++q2) {
+            const int cnt2 = min(32, nsel - 32 * q2);
+            for (int l = 0; l < cnt2; ++l) {
+                const double od = __shfl_sync(0xFFFFFFFFu, dd[q2], l);
+                const unsigned long long oo = __shfl_sync(0xFFFFFFFFu, ord[q2], l);
+#pragma unroll
+                for (int q = 0; q < KPL; ++q) rank[q] += (od < dd[q] || (od == dd[q] && oo < ord[q])) ? 1 : 0;
+            }
         }
     }
     float dkk = 0.f;

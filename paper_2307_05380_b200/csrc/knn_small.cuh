@@ -244,20 +244,44 @@ __device__ inline void mg_knn_source(const KnnArgs &A, const StructRec &R, const
             dd[s] = __dadd_rn(__dadd_rn(__dmul_rn(vv[s][0], vv[s][0]), __dmul_rn(vv[s][1], vv[s][1])), __dmul_rn(vv[s][2], vv[s][2]));
         }
     }
+    // (two keys per lane: ranking 64 entries by counting is 1.5 k instructions a row, a fifth of the k = 64 kernel —
+    // but the FP32 keys mostly ARE the final order; one look at each entry's predecessor tells, and only a row where
+    // FP64 or the tie-break disagrees with the FP32 order, or one with placeholders, counts)
+    bool in_order = false;
+    if (KPL > 1) {
+        bool ok = true;
+#pragma unroll
+        for (int s = 0; s < KPL; ++s) {
+            const int r = 32 * s + lane;
+            const unsigned tie = (unsigned)keys[s];
+            double pd = __shfl_up_sync(0xFFFFFFFFu, dd[s], 1);
+            unsigned pt = __shfl_up_sync(0xFFFFFFFFu, tie, 1);
+            if (s > 0) {
+                const double ld = __shfl_sync(0xFFFFFFFFu, dd[s > 0 ? s - 1 : 0], 31);
+                const unsigned lt = __shfl_sync(0xFFFFFFFFu, (unsigned)keys[s > 0 ? s - 1 : 0], 31);
+                if (lane == 0) { pd = ld; pt = lt; }
+            }
+            if (r < k) ok = ok && keys[s] != MG_KEY_INF && (r == 0 || pd < dd[s] || (pd == dd[s] && pt < tie));
+        }
+        in_order = __all_sync(0xFFFFFFFFu, ok);
+    }
 #pragma unroll
     for (int s = 0; s < KPL; ++s) {
         const int r = 32 * s + lane;
         const unsigned tie = (unsigned)keys[s];
         const bool valid = r < k && keys[s] != MG_KEY_INF;
         int rank = 0;
+        if (KPL > 1 && in_order) rank = r;
+        else {
 #pragma unroll
-        for (int s2 = 0; s2 < KPL; ++s2) {
-            const unsigned tie2 = (unsigned)keys[s2];
-            const int cnt2 = min(32, k - 32 * s2);
-            for (int l = 0; l < cnt2; ++l) {
-                const double od = __shfl_sync(0xFFFFFFFFu, dd[s2], l);
-                const unsigned ot = __shfl_sync(0xFFFFFFFFu, tie2, l);
-                rank += (od < dd[s] || (od == dd[s] && ot < tie)) ? 1 : 0;
+            for (int s2 = 0; s2 < KPL; ++s2) {
+                const unsigned tie2 = (unsigned)keys[s2];
+                const int cnt2 = min(32, k - 32 * s2);
+                for (int l = 0; l < cnt2; ++l) {
+                    const double od = __shfl_sync(0xFFFFFFFFu, dd[s2], l);
+                    const unsigned ot = __shfl_sync(0xFFFFFFFFu, tie2, l);
+                    rank += (od < dd[s] || (od == dd[s] && ot < tie)) ? 1 : 0;
+                }
             }
         }
         if (r < k) {
